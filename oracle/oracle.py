@@ -1,0 +1,197 @@
+"""ctypes front end of the plain FP64 CPU oracle (oracle/fstat_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It never imports the CUDA package
+``paper_2407_10797_b200`` and the CUDA package never imports it.
+
+``build()`` compiles the C file with gcc (-O2, no fast-math, OpenMP over particles) into
+oracle/libfstat_oracle.so; every function below is a thin marshalling wrapper, the arithmetic is all
+in the C file, which cites the PAPER.md passage each step follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "fstat_oracle.c")
+_LIB = os.path.join(_HERE, "libfstat_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+
+class Options(C.Structure):
+    _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double),
+                ("orbit_kappa", C.c_double), ("orbit_lambda", C.c_double)]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle if the shared object is missing or older than the source."""
+    with _lock:
+        if (not force and os.path.exists(_LIB)
+                and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            return _LIB
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+               "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+        return _LIB
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        L.oracle_default_options.argtypes = [C.POINTER(Options)]
+        L.oracle_params_valid.argtypes = [C.POINTER(C.c_double)]
+        L.oracle_params_valid.restype = C.c_int
+        L.oracle_pn_alpha.argtypes = [C.c_double, C.c_double, C.POINTER(C.c_double)]
+        L.oracle_phase.argtypes = [C.POINTER(C.c_double), C.c_double, C.POINTER(Options),
+                                   C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.oracle_orbit.argtypes = [C.c_double, C.POINTER(Options), C.POINTER(C.c_double)]
+        L.oracle_sky_basis.argtypes = [C.c_double, C.c_double] + [C.POINTER(C.c_double)] * 3
+        L.oracle_response.argtypes = [C.POINTER(C.c_double), C.c_double, C.c_double, C.POINTER(Options),
+                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.oracle_template.argtypes = [C.POINTER(C.c_double), C.c_int64, C.POINTER(C.c_double),
+                                      C.POINTER(Options), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.oracle_inner_products.argtypes = [C.POINTER(C.c_double)] * 4 + [C.c_double, C.c_int64, C.c_int64,
+                                            C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.oracle_fstat_from_NM.argtypes = [C.POINTER(C.c_double)] * 4
+        L.oracle_fstat_from_NM.restype = C.c_int
+        L.oracle_fstat_batch.argtypes = [C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                         C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_int64), C.c_int64,
+                                         C.POINTER(C.c_double), C.POINTER(Options), C.c_int, C.c_int,
+                                         C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                         C.POINTER(C.c_int32)]
+        L.oracle_fstat_batch.restype = C.c_int
+        L.oracle_max_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def default_options(**kw) -> Options:
+    o = Options()
+    lib().oracle_default_options(C.byref(o))
+    for k, v in kw.items():
+        setattr(o, k, v)
+    return o
+
+
+def _opt(o: Optional[Options]) -> Options:
+    return default_options() if o is None else o
+
+
+def _par(p) -> np.ndarray:
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    assert p.shape[-1] == 6
+    return p
+
+
+def params_valid(par) -> bool:
+    return bool(lib().oracle_params_valid(_dp(_par(par))))
+
+
+def pn_alpha(eta: float, v: float) -> np.ndarray:
+    a = np.zeros(7)
+    lib().oracle_pn_alpha(float(eta), float(v), _dp(a))
+    return a
+
+
+def phase(par, f: float, opt: Optional[Options] = None) -> Tuple[float, float]:
+    """(Psi_0(f), t_f) for one particle at one frequency."""
+    psi, tf = C.c_double(), C.c_double()
+    lib().oracle_phase(_dp(_par(par)), float(f), C.byref(_opt(opt)), C.byref(psi), C.byref(tf))
+    return psi.value, tf.value
+
+
+def orbit(t: float, opt: Optional[Options] = None) -> np.ndarray:
+    """[3][3] spacecraft positions (rows: spacecraft 1, 2, 3) at time t, metres."""
+    p = np.zeros((3, 3))
+    lib().oracle_orbit(float(t), C.byref(_opt(opt)), _dp(p))
+    return p
+
+
+def sky_basis(theta: float, phi: float):
+    k, u, v = np.zeros(3), np.zeros(3), np.zeros(3)
+    lib().oracle_sky_basis(float(theta), float(phi), _dp(k), _dp(u), _dp(v))
+    return k, u, v
+
+
+def response(par, f: float, t: float, opt: Optional[Options] = None) -> Tuple[complex, complex]:
+    """(T_plus, T_cross) of TDI X at frequency f with the constellation at time t."""
+    tp, tc = np.zeros(2), np.zeros(2)
+    lib().oracle_response(_dp(_par(par)), float(f), float(t), C.byref(_opt(opt)), _dp(tp), _dp(tc))
+    return complex(tp[0], tp[1]), complex(tc[0], tc[1])
+
+
+def template(par, freq, opt: Optional[Options] = None) -> Tuple[np.ndarray, np.ndarray]:
+    """(u_plus, u_cross) complex128 arrays over ``freq`` for one particle."""
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    n = freq.shape[0]
+    up, uc = np.zeros(n, dtype=np.complex128), np.zeros(n, dtype=np.complex128)
+    lib().oracle_template(_dp(_par(par)), n, _dp(freq), C.byref(_opt(opt)),
+                          up.ctypes.data_as(C.POINTER(C.c_double)), uc.ctypes.data_as(C.POINTER(C.c_double)))
+    return up, uc
+
+
+def inner_products(dw, inv_sn, u_plus, u_cross, df: float, lo: int, hi: int, use_ld: bool = False):
+    """(N[4], M[4][4]) over bins [lo, hi)."""
+    dw = np.ascontiguousarray(dw, dtype=np.complex128)
+    inv_sn = np.ascontiguousarray(inv_sn, dtype=np.float64)
+    u_plus = np.ascontiguousarray(u_plus, dtype=np.complex128)
+    u_cross = np.ascontiguousarray(u_cross, dtype=np.complex128)
+    N, M = np.zeros(4), np.zeros((4, 4))
+    cd = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    lib().oracle_inner_products(cd(dw), _dp(inv_sn), cd(u_plus), cd(u_cross), float(df), int(lo), int(hi),
+                                int(use_ld), _dp(N), _dp(M))
+    return N, M
+
+
+def fstat_from_NM(N, M):
+    """(F, a[4], singular_flag) = max_a [a.N - a^T M a / 2]."""
+    N = np.ascontiguousarray(N, dtype=np.float64)
+    M = np.ascontiguousarray(M, dtype=np.float64)
+    F = C.c_double()
+    a = np.zeros(4)
+    flag = lib().oracle_fstat_from_NM(_dp(N), _dp(M), C.byref(F), _dp(a))
+    return F.value, a, int(flag)
+
+
+def fstat_batch(freq, dw, inv_sn, edges, params, opt: Optional[Options] = None, use_ld: bool = False,
+                n_threads: int = 0, want_NM: bool = False):
+    """F[P], Fk[P][n_part] (and NM[P][n_part][20], flags[P][n_part] when want_NM) for P particles."""
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    dw = np.ascontiguousarray(dw, dtype=np.complex128)
+    inv_sn = np.ascontiguousarray(inv_sn, dtype=np.float64)
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    params = _par(params).reshape(-1, 6)
+    P, n_part, n = params.shape[0], edges.shape[0] - 1, freq.shape[0]
+    assert edges[0] == 0 and edges[-1] == n and np.all(np.diff(edges) > 0)
+    F = np.zeros(P)
+    Fk = np.zeros((P, n_part))
+    NM = np.zeros((P, n_part, 20)) if want_NM else None
+    flags = np.zeros((P, n_part), dtype=np.int32)
+    rc = lib().oracle_fstat_batch(n, _dp(freq), dw.ctypes.data_as(C.POINTER(C.c_double)), _dp(inv_sn),
+                                  n_part, edges.ctypes.data_as(C.POINTER(C.c_int64)), P, _dp(params),
+                                  C.byref(_opt(opt)), int(use_ld), int(n_threads), _dp(F), _dp(Fk),
+                                  _dp(NM) if want_NM else None, flags.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != 0:
+        raise MemoryError("oracle_fstat_batch: allocation failed")
+    if want_NM:
+        return F, Fk, NM, flags
+    return F, Fk
+
+
+def max_threads() -> int:
+    return int(lib().oracle_max_threads())

@@ -1,0 +1,455 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself or with the CUDA path.  Each pin is chosen so that a
+plausible mistake in one part of oracle/fstat_oracle.c (a dropped term, a wrong sign or index, a
+transposed operand, a wrong Fourier convention) fails it.  CPU only.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import optimize, stats
+
+import synthetic as syn
+import td_sim
+
+YR = syn.YEAR_S
+GMSUN = 4.925490947641267e-6
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+with open(os.path.join(HERE, "golden", "paper_values.json")) as fh:
+    PAPER = json.load(fh)
+
+
+def _ip(a, b, sn, df):
+    """<a, b> = 4 df Re sum a conj(b) / S_n, retyped from PAPER.md:66 Eq. 4 (rectangle rule)."""
+    return 4.0 * df * float(np.sum((a * np.conj(b)).real / sn))
+
+
+# ----------------------------------------------------------------------------- P1: epilogue
+def test_p1_fstat_equals_bruteforce_maximum_of_loglikelihood(orc, tiny):
+    """F_k = max over the four amplitudes of Lambda = <d,h> - <h,h>/2 (PAPER.md:62 Eq. 3, :77 Eq. 5, :85 Eq. 7),
+    found here by numerical maximisation from several starts, never via N, M or a linear solve."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:3]
+    edges = ds.edges(4)
+    F, Fk = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par)
+    rng = np.random.default_rng(7)
+    for p in range(par.shape[0]):
+        up, uc = orc.template(par[p], ds.freq)
+        tot = 0.0
+        for j in range(4):
+            sl = slice(edges[j], edges[j + 1])
+            d, sn = ds.data[sl], ds.sn[sl]
+            basis = [up[sl], uc[sl], 1j * up[sl], 1j * uc[sl]]
+            scale = [1.0 / math.sqrt(_ip(b, b, sn, ds.df)) for b in basis]     # condition the search only
+            basis = [b * s for b, s in zip(basis, scale)]
+
+            def neg_lambda(a):
+                h = a[0] * basis[0] + a[1] * basis[1] + a[2] * basis[2] + a[3] * basis[3]
+                return -(_ip(d, h, sn, ds.df) - 0.5 * _ip(h, h, sn, ds.df))
+
+            best = np.inf
+            for _ in range(3):
+                r = optimize.minimize(neg_lambda, rng.standard_normal(4), method="BFGS", options={"gtol": 1e-10})
+                r = optimize.minimize(neg_lambda, r.x, method="Nelder-Mead",
+                                      options={"xatol": 1e-11, "fatol": 1e-14, "maxiter": 4000})
+                best = min(best, r.fun)
+            assert -best == pytest.approx(Fk[p, j], rel=1e-8, abs=1e-10)
+            tot += -best
+        assert tot == pytest.approx(F[p], rel=1e-8)
+
+
+def test_p1b_singular_partition_is_the_supremum(orc, tiny):
+    """One-bin partitions: the four templates span only two real dimensions, M is singular, and the
+    maximum of Lambda is reached by fitting the bin exactly: F_k = 4 df |d|^2 / (2 S_n)."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:2]
+    n = 6
+    edges = np.arange(n + 1, dtype=np.int64)
+    F, Fk, NM, flags = orc.fstat_batch(ds.freq[:n], ds.dw[:n], ds.inv_sn[:n], edges, par, want_NM=True)
+    expect = 0.5 * 4.0 * ds.df * np.abs(ds.data[:n]) ** 2 / ds.sn[:n]
+    assert np.all(flags == 1)
+    np.testing.assert_allclose(Fk, np.broadcast_to(expect, Fk.shape), rtol=1e-9)
+    # two-bin partitions: four real dimensions, regular M, the data are still fitted exactly
+    edges2 = np.arange(0, n + 1, 2, dtype=np.int64)
+    F2, Fk2, _, flags2 = orc.fstat_batch(ds.freq[:n], ds.dw[:n], ds.inv_sn[:n], edges2, par, want_NM=True)
+    assert np.all(flags2 == 0)
+    np.testing.assert_allclose(Fk2, np.broadcast_to(expect.reshape(-1, 2).sum(1), Fk2.shape), rtol=1e-6)
+
+
+# ----------------------------------------------------------------------------- P2: zero noise
+@pytest.mark.parametrize("n_part", [1, 4, 16])
+def test_p2_zero_noise_two_f_equals_snr_squared(orc, n_part):
+    """Data = injection only, evaluated at the injected Theta_I: 2 F_k = <h,h>_k, sum = rho^2 = 144."""
+    ds = syn.make_dataset(syn.CONFIGS[0], orc.template, noise=False)
+    edges = ds.edges(n_part)
+    F, Fk = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, ds.inj_params[None, :])
+    assert 2.0 * F[0] == pytest.approx(144.0, rel=1e-10)
+    for j in range(n_part):
+        sl = slice(edges[j], edges[j + 1])
+        hh = _ip(ds.injection[sl], ds.injection[sl], ds.sn[sl], ds.df)
+        assert 2.0 * Fk[0, j] == pytest.approx(hh, rel=1e-8)
+
+
+def test_p2b_mismatched_template_recovers_less_than_snr_squared(orc):
+    ds = syn.make_dataset(syn.CONFIGS[0], orc.template, noise=False)
+    par = ds.inj_params.copy()
+    par[1] *= 1.0 + 1e-4                                   # chirp mass off by 1e-4: > 1e5 cycles decohere
+    F, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), par[None, :])
+    assert 0.0 <= 2.0 * F[0] < 0.5 * 144.0
+
+
+# ----------------------------------------------------------------------------- P3: chi-square
+def test_p3_pure_noise_is_chi_square_with_4np_dof(orc):
+    """Over stationary Gaussian noise 2 F_k ~ chi^2(4) and 2 F ~ chi^2(4 N_p) (north_star)."""
+    cfg = syn.CONFIGS[0]
+    _, n, f = syn.frequency_grid(cfg.T, cfg.f_lo, cfg.f_hi)
+    sn = syn.psd_tdi_x(f)
+    n_part = 4
+    edges = syn.equal_bin_edges(n, n_part)
+    par = syn.draw_particles(cfg)                           # 64 templates
+    twoF, twoFk = [], []
+    for seed in range(1000, 1160):                          # 160 noise realisations -> 10240 pairs
+        d = syn.coloured_noise(sn, cfg.T, seed)
+        F, Fk = orc.fstat_batch(f, d / sn, 1.0 / sn, edges, par)
+        twoF.append(2.0 * F)
+        twoFk.append(2.0 * Fk.ravel())
+    twoF, twoFk = np.concatenate(twoF), np.concatenate(twoFk)
+    nF, nk = twoF.size, twoFk.size
+    assert nF >= 10000
+    assert abs(twoF.mean() - 4 * n_part) < 5.0 * math.sqrt(8 * n_part / nF)
+    assert abs(twoF.var() - 8 * n_part) < 0.1 * 8 * n_part
+    assert abs(twoFk.mean() - 4.0) < 5.0 * math.sqrt(8.0 / nk)
+    assert abs(twoFk.var() - 8.0) < 0.05 * 8.0
+    assert stats.kstest(twoF, "chi2", args=(4 * n_part,)).pvalue > 1e-3
+    assert stats.kstest(twoFk[::7], "chi2", args=(4,)).pvalue > 1e-3
+
+
+# ----------------------------------------------------------------------------- P4: combine
+def test_p4_np1_is_the_coherent_statistic_and_sums_add(orc, tiny):
+    """N_seg = 1 is the fully coherent F; N and M of the partitions add up to the coherent ones."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:4]
+    F1, Fk1, NM1, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), par, want_NM=True)
+    np.testing.assert_array_equal(F1, Fk1[:, 0])
+    for p in range(4):
+        up, uc = orc.template(par[p], ds.freq)
+        N, M = orc.inner_products(ds.dw, ds.inv_sn, up, uc, ds.df, 0, ds.n_bins)
+        Fcoh, _, flag = orc.fstat_from_NM(N, M)
+        assert flag == 0 and Fcoh == F1[p]
+        # N^i = <d, A^i>, M^ij = <A^i, A^j> retyped in numpy
+        A = [up, uc, 1j * up, 1j * uc]
+        for i in range(4):
+            assert N[i] == pytest.approx(_ip(ds.data, A[i], ds.sn, ds.df), rel=1e-10, abs=1e-12 * np.abs(N).max())
+            for j in range(4):
+                assert M[i, j] == pytest.approx(_ip(A[i], A[j], ds.sn, ds.df), rel=1e-10, abs=1e-12 * M[0, 0])
+    _, Fk7, NM7, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(7), par, want_NM=True)
+    np.testing.assert_allclose(NM7.sum(axis=1), NM1[:, 0], rtol=1e-9, atol=1e-12 * np.abs(NM1).max())
+    # semi-coherent statistic can only gain from the extra freedom: sum_k F_k >= F_coherent
+    assert np.all(Fk7.sum(1) >= F1 - 1e-9)
+
+
+def test_p5_hermitian_closed_form_equals_4x4_solve(orc, tiny):
+    """The 8-sum 2x2 Hermitian form the GPU epilogue uses equals the oracle's 4x4 Cholesky."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:8]
+    _, Fk, NM, flags = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par, want_NM=True)
+    N, M = NM[..., :4], NM[..., 4:].reshape(NM.shape[0], NM.shape[1], 4, 4)
+    scale = M[..., 0, 0]
+    # structure of M: real embedding of [[m_pp, conj(m_pc)], [m_pc, m_cc]]
+    np.testing.assert_allclose(M[..., 0, 0], M[..., 2, 2], rtol=1e-12)
+    np.testing.assert_allclose(M[..., 1, 1], M[..., 3, 3], rtol=1e-12)
+    np.testing.assert_allclose(M[..., 0, 1], M[..., 2, 3], rtol=1e-12, atol=1e-14 * scale.max())
+    np.testing.assert_allclose(M[..., 0, 3], -M[..., 1, 2], rtol=1e-12, atol=1e-14 * scale.max())
+    assert np.all(np.abs(M[..., 0, 2]) <= 1e-13 * scale) and np.all(np.abs(M[..., 1, 3]) <= 1e-13 * M[..., 1, 1])
+    zp, zc = N[..., 0] + 1j * N[..., 2], N[..., 1] + 1j * N[..., 3]
+    mpp, mcc = M[..., 0, 0], M[..., 1, 1]
+    mpc = M[..., 0, 1] + 1j * M[..., 0, 3]
+    best = None
+    for cand in (mpc, np.conj(mpc)):                       # orientation is fixed by whichever reproduces F
+        twoF = (mcc * abs(zp) ** 2 + mpp * abs(zc) ** 2 - 2.0 * (np.conj(zp) * cand * zc).real) / (mpp * mcc - abs(cand) ** 2)
+        err = np.max(np.abs(0.5 * twoF - Fk) / np.maximum(Fk, 1e-3))
+        best = err if best is None else min(best, err)
+    assert best < 1e-11
+    assert np.all(flags == 0)
+
+
+# ----------------------------------------------------------------------------- P6: phase
+def test_p6_time_frequency_map_is_the_derivative_of_the_phase(orc):
+    """t_f = (1/2pi) dPsi_0/df (Eq. 20): analytic derivative vs central difference."""
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        par = np.array([rng.uniform(1, 8) * YR, rng.uniform(20, 80), rng.uniform(0.05, 0.25),
+                        1.0, 2.0, rng.uniform(0, 0.1)])
+        f = rng.uniform(0.01, 0.1)
+        h = 1e-6 * f
+        _, tf = orc.phase(par, f)
+        # remove the huge linear term before differencing so the difference keeps ~9 digits
+        g = lambda x: orc.phase(par, x)[0] - 2.0 * math.pi * x * par[0]
+        num = par[0] + (g(f + h) - g(f - h)) / (2.0 * h) / (2.0 * math.pi)
+        assert tf == pytest.approx(num, rel=1e-8)
+        assert tf < par[0]                                 # emitted before coalescence
+
+
+def test_p6_newtonian_limit_and_pn_coefficients(orc):
+    """v -> 0: Psi_0 -> 2 pi f tc - pi/4 + (3/128)(pi Mc f)^(-5/3) and t_f -> tc - (5/256) Mc^(-5/3) (pi f)^(-8/3)
+    (textbook Newtonian chirp); the O(v^2) correction has the 1PN coefficient 3715/756 + 55 eta/9."""
+    tc, e0 = 1.0e7, 0.0
+    for eta in (0.25, 0.1):
+        par = np.array([tc, 0.5, eta, 1.0, 2.0, e0])
+        Mc = par[1] * GMSUN
+        M = Mc * eta ** -0.6
+        for f in (1e-6, 3e-6):
+            psi, tf = orc.phase(par, f)
+            lead = 3.0 / 128.0 * (math.pi * Mc * f) ** (-5.0 / 3.0)
+            v = (math.pi * M * f) ** (1.0 / 3.0)
+            ratio = (psi - 2.0 * math.pi * f * tc + math.pi / 4.0) / lead
+            assert ratio == pytest.approx(1.0, abs=10.0 * v * v)
+            assert (ratio - 1.0) / v ** 2 == pytest.approx(3715.0 / 756.0 + 55.0 * eta / 9.0, rel=2e-2)
+            tau = 5.0 / 256.0 * Mc ** (-5.0 / 3.0) * (math.pi * f) ** (-8.0 / 3.0)
+            assert (tc - tf) / tau == pytest.approx(1.0, abs=10.0 * v * v)
+
+
+def test_p6_eccentric_term_scaling(orc):
+    """phi_e = -(3/128)(pi Mc f)^(-5/3) (2355/1462) e0^2 (f_ref/f)^(19/9) (reading A3): quadratic in e0,
+    zero at e0 = 0, and with e0 defined at f_ref = 10 mHz."""
+    par0 = np.array([1.1e8, 30.0, 0.24, 1.0, 2.0, 0.0])
+    Mc = 30.0 * GMSUN
+    for f in (0.01, 0.02, 0.05):
+        lead = 3.0 / 128.0 * (math.pi * Mc * f) ** (-5.0 / 3.0)
+        d = []
+        for e0 in (0.05, 0.1):
+            par = par0.copy(); par[5] = e0
+            d.append(orc.phase(par, f)[0] - orc.phase(par0, f)[0])
+        assert d[1] / d[0] == pytest.approx(4.0, rel=1e-6)
+        assert d[0] / lead == pytest.approx(-(2355.0 / 1462.0) * 0.05 ** 2 * (0.01 / f) ** (19.0 / 9.0), rel=1e-6)
+    # a different reference frequency rescales the term by (f_ref'/f_ref)^(19/9)
+    par = par0.copy(); par[5] = 0.05
+    o2 = orc.default_options(f_ref_e0=0.02)
+    d1 = orc.phase(par, 0.03)[0] - orc.phase(par0, 0.03)[0]
+    d2 = orc.phase(par, 0.03, o2)[0] - orc.phase(par0, 0.03, o2)[0]
+    assert d2 / d1 == pytest.approx(2.0 ** (19.0 / 9.0), rel=1e-6)
+
+
+def test_p6_phase_rounding_error_bounded_by_mpmath(orc):
+    """FP64 evaluation of Psi_0 (|Psi_0| up to 1.5e8 rad) is within 1e-7 rad of a 40-digit evaluation."""
+    import mpmath as mp
+    mp.mp.dps = 40
+
+    def psi_mp(par, f):
+        tc, Mc, eta, e0 = mp.mpf(par[0]), mp.mpf(par[1]) * mp.mpf(GMSUN), mp.mpf(par[2]), mp.mpf(par[5])
+        f = mp.mpf(f)
+        M = Mc * eta ** mp.mpf("-0.6")
+        v = (mp.pi * M * f) ** (mp.mpf(1) / 3)
+        g = mp.mpf("0.5772156649015329")
+        a = [1, 0, mp.mpf(3715) / 756 + 55 * eta / 9, -16 * mp.pi,
+             mp.mpf(15293365) / 508032 + 27145 * eta / 504 + 3085 * eta ** 2 / 72,
+             mp.pi * (mp.mpf(38645) / 756 - 65 * eta / 9) * (1 + 3 * mp.log(v * mp.sqrt(6))),
+             mp.mpf(11583231236531) / 4694215680 - 640 * mp.pi ** 2 / 3 - 6848 * g / 21
+             + eta * (-mp.mpf(15737765635) / 3048192 + 2255 * mp.pi ** 2 / 12)
+             + 76055 * eta ** 2 / 1728 - 127825 * eta ** 3 / 1296 - mp.mpf(6848) / 21 * mp.log(4 * v)]
+        s = sum(a[k] * v ** k for k in range(7)) - mp.mpf(2355) / 1462 * e0 ** 2 * (mp.mpf("0.01") / f) ** (mp.mpf(19) / 9)
+        return 2 * mp.pi * f * tc - mp.pi / 4 + mp.mpf(3) / 128 * (mp.pi * Mc * f) ** (-mp.mpf(5) / 3) * s
+
+    rng = np.random.default_rng(11)
+    for _ in range(25):
+        par = np.array([rng.uniform(2.5, 7.5) * YR, rng.uniform(20, 40), rng.uniform(0.2, 0.25), 1.0, 2.0, rng.uniform(0, 0.1)])
+        f = float(rng.uniform(0.01, 0.1))
+        assert abs(float(mp.mpf(orc.phase(par, f)[0]) - psi_mp(par, f))) < 1e-7
+
+
+def test_p10_paper_sanity_cycles_and_tf(orc):
+    """PAPER.md:30 (> 1e5 cycles in 2.5 yr) and :229 (T_f < 1e6 s) hold for the paper's cases / search range;
+    Table III vs VI fixes delta_mu <-> eta (reading A18)."""
+    T = PAPER["observation"]["T_yr"] * YR
+    c = PAPER["case_C_table_VI_true_value"]
+    assert (1.0 - c["table_VI"] ** 2) / 4.0 == pytest.approx(c["table_III"], abs=5e-5)
+    for name in ("A", "B"):
+        case = PAPER["cases"][name]
+        eta = (1.0 - case["delta_mu"] ** 2) / 4.0
+        par = np.array([case["tc_yr"] * YR, case["Mc"], eta, case["theta"], case["phi"], case["e0"]])
+        f_at = lambda t: optimize.brentq(lambda f: orc.phase(par, f)[1] - t, 1e-3, 0.5)
+        f0, f1 = f_at(0.0), f_at(T)
+        Phi = lambda f: 2.0 * math.pi * f * orc.phase(par, f)[1] - orc.phase(par, f)[0]
+        cycles = (Phi(f1) - Phi(f0)) / (2.0 * math.pi)
+        assert cycles > PAPER["observation"]["min_cycles"]
+        assert 0.005 < f0 < f1 < 0.05                      # in the LISA band below the 10 s Nyquist
+    # T_f^2 = |Psi''| / (4 pi) = (dt_f/df) / 2 over the search range, worst case = lightest system at 10 mHz
+    for Mc in PAPER["observation"]["Mc_range"]:
+        par = np.array([3.5 * YR, Mc, 0.25, 1.0, 2.0, 0.0])
+        for f in (0.01, 0.02, 0.05):
+            h = 1e-5 * f
+            dtf = (orc.phase(par, f + h)[1] - orc.phase(par, f - h)[1]) / (2 * h)
+            assert math.sqrt(0.5 * dtf) < PAPER["observation"]["max_T_f_s"]
+
+
+# ----------------------------------------------------------------------------- P7: orbit
+def test_p7_orbit_matches_exact_kepler_ellipses_to_third_order(orc):
+    """Analytic orbit to O(e^2) vs exact Keplerian ellipses: residual is O(e^3)."""
+    L = 2.5e9
+    e = L / (2.0 * math.sqrt(3.0) * td_sim.AU)
+    t = np.linspace(-0.3 * YR, 7.7 * YR, 400)
+    exact = td_sim.kepler_positions(t, L)
+    for i, ti in enumerate(t):
+        p = orc.orbit(ti)
+        err = np.linalg.norm(p - exact[:, :, i], axis=1) / td_sim.AU
+        assert np.all(err < 6.0 * e ** 3)                  # a wrong e^2 coefficient would give ~e^2 = 2.3e-5
+    # with non-zero kappa, lambda too
+    o = orc.default_options(orbit_kappa=0.7, orbit_lambda=-1.9)
+    ex = td_sim.kepler_positions(np.array([1.23e7]), L, 0.7, -1.9)[:, :, 0]
+    assert np.all(np.linalg.norm(orc.orbit(1.23e7, o) - ex, axis=1) / td_sim.AU < 6.0 * e ** 3)
+
+
+def test_p7_orbit_invariants(orc):
+    L, AU = 2.5e9, td_sim.AU
+    e = L / (2.0 * math.sqrt(3.0) * AU)
+    for t in np.linspace(0.0, YR, 37):
+        p = orc.orbit(t)
+        for a, b in ((0, 1), (1, 2), (2, 0)):
+            assert abs(np.linalg.norm(p[a] - p[b]) / L - 1.0) < 0.0025      # breathing arms, O(e)
+        cen = p.mean(axis=0)
+        assert abs(np.linalg.norm(cen) / AU - 1.0) < 30.0 * e * e              # centre on the 1 AU circle
+        np.testing.assert_allclose(orc.orbit(t + YR), p, rtol=0, atol=1e-3)    # period exactly one year
+    # constellation centre starts on the x axis for kappa = 0 and moves counter-clockwise
+    assert orc.orbit(0.0).mean(axis=0)[0] > 0.99 * AU
+    assert orc.orbit(0.01 * YR).mean(axis=0)[1] > 0.0
+
+
+# ----------------------------------------------------------------------------- P8: response
+def test_p8_long_wavelength_limit(orc):
+    """f -> 0: T_P -> 2 (2 pi f L/c)^2 (n13.e_P.n13 - n12.e_P.n12) exp(-2 pi i f k.p1/c), the
+    second time derivative of the differential arm strain.  Modulus agrees to O(x^2), x = pi f L/c; keeping the
+    O(x) light-travel phases exp(-i x (4 + k.n1j)) of each arm the complex value agrees to O(x^2)."""
+    L = 2.5e9
+    rng = np.random.default_rng(5)
+    for _ in range(10):
+        th, ph, t = math.acos(rng.uniform(-1, 1)), rng.uniform(0, 2 * math.pi), rng.uniform(0, 3 * YR)
+        par = np.array([0.0, 30.0, 0.25, th, ph, 0.0])
+        p = orc.orbit(t)
+        k, u, v = orc.sky_basis(th, ph)
+        n12, n13 = (p[1] - p[0]) / L, (p[2] - p[0]) / L
+        xi = lambda n: ((u @ n) ** 2 - (v @ n) ** 2, 2.0 * (u @ n) * (v @ n))
+        for f in (1e-6, 1e-5, 1e-3):
+            x = math.pi * f * L / syn.C_SI
+            w = 2.0 * x
+            dop = np.exp(-2j * math.pi * f * (k @ p[0]) / syn.C_SI)
+            Tp, Tc = orc.response(par, f, t)
+            for T, a13, a12 in ((Tp, xi(n13)[0], xi(n12)[0]), (Tc, xi(n13)[1], xi(n12)[1])):
+                lim0 = 2.0 * w * w * (a13 - a12) * dop
+                lim1 = 2.0 * w * w * dop * np.exp(-4j * x) * (a13 * np.exp(-1j * x * (k @ n13)) - a12 * np.exp(-1j * x * (k @ n12)))
+                scale = 2.0 * w * w * (abs(a13) + abs(a12))
+                assert abs(abs(T) - abs(lim0)) < (20.0 * x * x + 1e-7) * scale
+                assert abs(T - lim1) < (20.0 * x * x + 1e-7) * scale
+
+
+def test_p8_tdi_null_and_sky_basis(orc):
+    """|T_P| vanishes where 1 - z^2 = 0 (f = c/2L, the null of first-generation X, hazard H4);
+    (k, u, v) is a right-handed orthonormal triad with k pointing from the source to the SSB."""
+    par = np.array([0.0, 30.0, 0.25, 0.9, 4.0, 0.0])
+    f_null = syn.C_SI / (2.0 * 2.5e9)
+    T0 = orc.response(par, 0.9 * f_null, 1e7)
+    Tn = orc.response(par, f_null, 1e7)
+    assert abs(Tn[0]) < 1e-12 * abs(T0[0]) and abs(Tn[1]) < 1e-12 * abs(T0[1])
+    k, u, v = orc.sky_basis(0.9, 4.0)
+    src = np.array([math.sin(0.9) * math.cos(4.0), math.sin(0.9) * math.sin(4.0), math.cos(0.9)])
+    np.testing.assert_allclose(k, -src, atol=1e-15)
+    for a, b in ((k, u), (k, v), (u, v)):
+        assert abs(a @ b) < 1e-15
+    np.testing.assert_allclose(np.cross(u, v), k, atol=1e-15)
+
+
+def test_p8_f_is_invariant_under_polarisation_rotation(orc, tiny):
+    """Rotating the polarisation basis by psi mixes (u_+, u_x) by a real rotation by 2 psi and cannot change
+    F (reading A11).  Checked by rotating the oracle's templates and redoing the inner products."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[5]
+    up, uc = orc.template(par, ds.freq)
+    N, M = orc.inner_products(ds.dw, ds.inv_sn, up, uc, ds.df, 0, ds.n_bins)
+    F0 = orc.fstat_from_NM(N, M)[0]
+    for psi in (0.3, 1.2):
+        c, s = math.cos(2 * psi), math.sin(2 * psi)
+        N2, M2 = orc.inner_products(ds.dw, ds.inv_sn, c * up + s * uc, -s * up + c * uc, ds.df, 0, ds.n_bins)
+        assert orc.fstat_from_NM(N2, M2)[0] == pytest.approx(F0, rel=1e-11)
+
+
+def test_p8_sky_periodicity_and_pole(orc, tiny):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:2].copy()
+    F0, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par)
+    par2 = par.copy(); par2[:, 4] += 2.0 * math.pi
+    F1, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par2)
+    np.testing.assert_allclose(F1, F0, rtol=1e-6)          # 2 pi in phi only moves rounding
+    # at the pole phi is a pure polarisation rotation: F does not depend on it
+    par[:, 3] = 0.0
+    Fa, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par)
+    par[:, 4] += 1.0
+    Fb, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par)
+    np.testing.assert_allclose(Fa, Fb, rtol=1e-8)
+
+
+# ----------------------------------------------------------------------------- P9: time domain
+def test_p9_frequency_domain_response_matches_time_domain_simulation(orc):
+    """with N = 0 the match with the approximation-free signal exceeds 0.999.  The time-domain
+    signal is built from Keplerian orbits, four explicit one-way links and explicit TDI delays (tests/td_sim.py);
+    its FFT is compared, as a COMPLEX overlap, with x~(f) = T(f) h~(f) of Eq. 17 on the bins whose t_f lies in
+    the untapered interior.  A wrong sign of t_f, of the Doppler term, of the Fourier convention, a swapped
+    link direction or a wrong TDI delay all drive the overlap far below 0.999."""
+    from scipy.signal.windows import tukey
+    L = 2.5e9
+    par = np.array([1.6 * YR, 40.0, 0.24, 1.1, 2.3, 0.03])
+    dt, N = 16.0, 2 ** 20
+    T = N * dt                                             # 0.53 yr: the antenna pattern turns by 3.3 rad
+    fg = np.linspace(0.015, 0.03, 12001)
+    pt = np.array([orc.phase(par, f) for f in fg])
+    sel = (pt[:, 1] > -0.03 * YR) & (pt[:, 1] < T + 0.03 * YR)
+    chirp = td_sim.Chirp(fg[sel], pt[sel, 0], pt[sel, 1])
+    cp, cc = 0.8 * np.exp(0.3j), 0.5 * np.exp(-1.1j)
+    t = np.arange(N) * dt
+    x = td_sim.tdi_x_time_domain(t, chirp, cp, cc, par[3], par[4], L)
+    X = np.fft.rfft(x * tukey(N, 0.2)) * dt
+    fk = np.arange(N // 2 + 1) / T
+    tf_k = np.interp(fk, fg, pt[:, 1])
+    band = (tf_k > 0.25 * T) & (tf_k < 0.75 * T)
+    assert band.sum() > 20000
+    up, uc = orc.template(par, fk[band])
+    Xfd, Xtd = cp * up + cc * uc, X[band]
+    overlap = np.sum(Xtd * np.conj(Xfd)) / math.sqrt(np.sum(abs(Xtd) ** 2) * np.sum(abs(Xfd) ** 2))
+    assert overlap.real > 0.999
+    assert abs(overlap.imag) < 0.03
+    assert math.sqrt(np.sum(abs(Xtd) ** 2) / np.sum(abs(Xfd) ** 2)) == pytest.approx(1.0, abs=5e-3)
+
+
+# ----------------------------------------------------------------------------- misc
+def test_invalid_particles_fly(orc, tiny):
+    """Invalid intrinsic parameters get F = -inf (let-them-fly), others are untouched."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:6].copy()
+    par[1, 1] = -3.0; par[2, 2] = 0.26; par[3, 5] = -0.01; par[4, 0] = np.nan
+    F, Fk = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par)
+    assert np.all(np.isneginf(F[1:5])) and np.all(np.isneginf(Fk[1:5]))
+    assert np.isfinite(F[0]) and np.isfinite(F[5])
+
+
+def test_long_double_accumulation_agrees(orc, tiny):
+    """Compensated FP64 sums vs long-double sums (hazard H3 switch)."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:16]
+    Fa, Fka = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par, use_ld=False)
+    Fb, Fkb = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par, use_ld=True)
+    np.testing.assert_allclose(Fka, Fkb, rtol=1e-9)
+
+
+def test_semicoherent_peak_broadens_with_more_partitions(orc):
+    """PAPER.md:124-126 / Fig. 1: away from the true chirp mass the noiseless semi-coherent statistic
+    keeps a larger fraction of its peak value when N_seg is larger."""
+    ds = syn.make_dataset(syn.CONFIGS[0], orc.template, noise=False)
+    par = ds.inj_params.copy()
+    par[1] *= 1.0 + 2e-5
+    frac = []
+    for n_part in (1, 4, 16, 64):
+        F, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(n_part), par[None, :])
+        frac.append(2.0 * F[0] / 144.0)
+    assert frac[0] < frac[1] < frac[2] < frac[3] <= 1.0 + 1e-9
