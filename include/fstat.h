@@ -1,0 +1,186 @@
+/*
+ * fstat.h -- C ABI of the B200-native batched semi-coherent F-statistic (arXiv 2407.10797).
+ *
+ * The library evaluates, for P PSO particles at once, the paper's fitness function
+ *
+ *     F(Theta_I) = sum_{k=1..N_p} F_k ,      F_k = 1/2 N_k^T M_k^-1 N_k            (Eq. 7,
+ *                                                                                   :110 Eq. 11, :117 Eq. 12)
+ *
+ * where N_k^i = <d, A^i>_k and M_k^ij = <A^i, A^j>_k are the noise-weighted inner products
+ * (PAPER.md:66 Eq. 4, :89-91 Eq. 8-9) restricted to frequency partition k, and A^1..A^4 are the four
+ * basis templates of the linear decomposition h = sum a_i A^i (Eq. 5) built from the
+ * restricted-PN stationary-phase waveform h~(f) = A f^(-7/6) exp(-i Psi(f)) (PAPER.md:397-405
+ * Eq. A1-A3) times the leading-order frequency-domain LISA TDI-X response T(f) evaluated at
+ * t_f = (1/2pi) dPsi/df (Eq. 17-20 with N = 0; orbit :198).  N_p = 1 is the fully
+ * coherent statistic.  F is the SUM of the F_k, not the mean of Eq. 11 (DESIGN.md
+ * reading A12).  Every step runs in hand-written sm_100a CUDA kernels; no template is written to
+ * memory; there is no CPU fallback (calls fail with FSTAT_ECUDA when no usable device exists).
+ *
+ * Conventions common to all calls
+ *   - All floating-point data are IEEE double.  "host" / "device" is stated per pointer.
+ *   - Every call returns an fstat_status and never throws or aborts.
+ *   - A plan may be used by one host thread at a time and has one evaluation in flight at a time
+ *     (its workspace lives inside the plan).  Distinct plans are independent.
+ */
+#ifndef FSTAT_H_
+#define FSTAT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define FSTAT_API
+#else
+#define FSTAT_API __attribute__((visibility("default")))
+#endif
+
+typedef struct fstat_plan fstat_plan;    /* opaque; created and destroyed by the library */
+
+typedef enum {
+    FSTAT_OK = 0,
+    FSTAT_EINVAL = 1,        /* an argument violates the contract below (see fstat_last_error)  */
+    FSTAT_ENOMEM = 2,        /* host or device allocation failed                                 */
+    FSTAT_ECUDA = 3,         /* a CUDA runtime call or kernel launch failed / no device          */
+    FSTAT_EUNSUPPORTED = 4   /* valid request outside this build's limits (e.g. n_bins >= 2^31)  */
+} fstat_status;
+
+/* Options of a plan.  Obtain defaults with fstat_default_options; opts == NULL means defaults. */
+typedef struct {
+    double f_ref_e0;          /* frequency [Hz] at which e0 is defined; default 0.01      */
+    double arm_length_m;      /* LISA arm length L [m]; default 2.5e9                                   */
+    double orbit_kappa;       /* initial orbital phase of the constellation centre [rad]; default 0     */
+    double orbit_lambda;      /* initial orientation of the constellation [rad]; default 0              */
+    int32_t device;           /* CUDA device ordinal; -1 (default) = the calling thread's current one   */
+    int32_t inputs_on_device; /* 0 (default): freq/dw/inv_sn are host pointers; 1: device pointers      */
+    int32_t max_segment_bins; /* 0 (default) = automatic.  Upper bound on the number of bins one CTA    *
+                               * sums before handing its partial sums to the epilogue (tuning / tests)  */
+    int32_t reserved;
+} fstat_options;
+
+FSTAT_API void fstat_default_options(fstat_options *opts);
+
+/*
+ * fstat_plan_create -- copy one TDI channel's frequency-domain data into the device and fold every
+ * particle-independent factor of the template and of the inner product (PAPER.md:66 Eq. 4; :397
+ * Eq. A1; :404 Eq. A3) into per-bin tables.
+ *
+ *   out         [out] receives the plan; set to NULL on failure.
+ *   n_bins      number of frequency bins N, 1 <= N < 2^31.
+ *   freq_hz     [N] strictly positive, strictly ascending, uniform grid f_k = k/T (df = 1/T is taken
+ *               as (f[N-1]-f[0])/(N-1), or f[0] when N == 1).  Non-uniformity > 1e-6 df is EINVAL.
+ *   dw_re_im    [N][2] interleaved re, im of  d~(f_k) / S_n(f_k)   (data weighted by the one-sided PSD).
+ *   inv_sn      [N] 1 / S_n(f_k), finite and > 0.
+ *   n_part      number of partitions N_p >= 1 (N_p = 1: fully coherent).
+ *   part_edges  [N_p+1] HOST pointer, bin offsets 0 = e_0 < e_1 < ... < e_{N_p} = N; partition k is the
+ *               half-open bin range [e_k, e_{k+1})  (Eq. 12; fixed data-side edges,
+ *               DESIGN.md reading A13).
+ *   opts        may be NULL.
+ *
+ * freq_hz, dw_re_im, inv_sn are host or device pointers according to opts->inputs_on_device.  The plan
+ * copies everything it needs: the caller may free or overwrite its arrays once the call returns.
+ * Errors: EINVAL for NULL pointers, a non-positive / non-ascending / non-uniform grid, non-finite dw or
+ * inv_sn, inv_sn <= 0, bad edges, an empty partition; ENOMEM; ECUDA; EUNSUPPORTED.
+ */
+FSTAT_API fstat_status fstat_plan_create(fstat_plan **out,
+                                         int64_t n_bins, const double *freq_hz,
+                                         const double *dw_re_im, const double *inv_sn,
+                                         int32_t n_part, const int64_t *part_edges,
+                                         const fstat_options *opts);
+
+/*
+ * fstat_plan_set_partitions -- replace the partition edges of an existing plan (same data, another
+ * N_p: the hierarchy stages of PAPER.md:168-174 differ only in N_seg).  Same rules for part_edges
+ * (HOST pointer) as in fstat_plan_create.  On error the plan keeps its previous partitions.
+ */
+FSTAT_API fstat_status fstat_plan_set_partitions(fstat_plan *plan, int32_t n_part,
+                                                 const int64_t *part_edges);
+
+/*
+ * fstat_eval_batch -- evaluate F and the per-partition F_k for P particles ("the
+ * computation of the semi-coherent F-statistic for each particle can be carried out in parallel").
+ *
+ *   params  [P][6] DEVICE pointer, row-major: t_c [s from the first sample], M_c [solar masses], eta,
+ *           theta [rad, ecliptic colatitude], phi [rad, ecliptic longitude], e0 (eta in
+ *           place of delta_mu, eta = (1 - delta_mu^2)/4, reading A18).
+ *   F       [P] DEVICE pointer, out.
+ *   Fk      [P][N_p] DEVICE pointer, row-major, out; may be NULL.
+ *   cuda_stream  a cudaStream_t (NULL = the legacy default stream).  The call only enqueues work on
+ *           that stream and returns; results are valid once the stream has reached that point.
+ *
+ * A particle with a non-finite parameter, M_c <= 0, eta outside (0, 0.25] or e0 < 0 is not an error:
+ * it gets F = -inf and F_k = -inf (PSO's "let them fly" fitness).  P == 0 is a no-op.
+ * Errors: EINVAL (NULL plan/params/F with P > 0, P < 0), ENOMEM (workspace growth), ECUDA.
+ */
+FSTAT_API fstat_status fstat_eval_batch(fstat_plan *plan, int64_t P,
+                                        const double *params, double *F, double *Fk,
+                                        void *cuda_stream);
+
+/*
+ * fstat_eval_batch_host -- the same evaluation with HOST buffers: copies params to the device,
+ * evaluates, copies F (and Fk when non-NULL) back and waits for completion before returning.
+ * Pinned host memory makes the copies asynchronous DMA; pageable memory works too.
+ */
+FSTAT_API fstat_status fstat_eval_batch_host(fstat_plan *plan, int64_t P,
+                                             const double *params_host, double *F_host,
+                                             double *Fk_host, void *cuda_stream);
+
+/*
+ * fstat_eval_template -- NOT on the hot path: write the two complex basis templates of ONE parameter
+ * vector over the plan's whole grid,
+ *     u_P(f_k) = T_P(f_k; t_f) f_k^(-7/6) exp(-i Psi_0(f_k)),  P in {+, x}
+ * (PAPER.md:397 Eq. A1 with the amplitude constant of Eq. A2 dropped, reading A21; :206
+ * Eq. 17 with N = 0), from which the four real basis templates of PAPER.md:77 Eq. 5 are
+ * A^1 = u_+, A^2 = u_x, A^3 = i u_+, A^4 = i u_x.  It runs the same device code as fstat_eval_batch
+ * and exists to synthesise injections (h = sum a_i A^i) and for element-wise tests.
+ *
+ *   params_host  [6] HOST pointer (t_c, M_c, eta, theta, phi, e0); an invalid vector is EINVAL here.
+ *   u_plus, u_cross  [N][2] DEVICE pointers, interleaved re, im, out.
+ * Synchronous: returns after the stream has finished the work.
+ */
+FSTAT_API fstat_status fstat_eval_template(fstat_plan *plan, const double *params_host,
+                                           double *u_plus, double *u_cross, void *cuda_stream);
+
+/* fstat_plan_destroy -- free a plan and its device memory.  NULL is allowed. */
+FSTAT_API void fstat_plan_destroy(fstat_plan *plan);
+
+/* Plan introspection (all NULL-safe; return 0 / -1 for a NULL plan). */
+FSTAT_API int64_t fstat_plan_n_bins(const fstat_plan *plan);
+FSTAT_API int32_t fstat_plan_n_part(const fstat_plan *plan);
+FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
+/* Number of (particle-group, segment) work items = CTAs the main kernel launches for P particles. */
+FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
+/* Number of kernels one fstat_eval_batch call launches (prologue + main + epilogue). */
+FSTAT_API int32_t fstat_launches_per_eval(void);
+/* Device time of the main (fused template + inner product) kernel in the most recent evaluations on
+ * this plan: CUDA events are recorded on the call's stream around that kernel at every fstat_eval_batch
+ * (ring of 128).  Writes the milliseconds of the last min(n_last, 128, evaluations so far) calls, oldest
+ * first, to the HOST array ms_out and returns how many were written.  Synchronises on those events. */
+FSTAT_API int32_t fstat_plan_main_kernel_ms(fstat_plan *plan, int32_t n_last, double *ms_out);
+
+/*
+ * fstat_edges_equal_bins -- "equal-bin partitions": e_j = floor(j * n_bins / n_part), j = 0..n_part,
+ * written to the HOST array edges_out[n_part+1].  EINVAL if n_part < 1 or n_part > n_bins.
+ */
+FSTAT_API fstat_status fstat_edges_equal_bins(int64_t n_bins, int32_t n_part, int64_t *edges_out);
+
+/*
+ * fstat_probe_pipe_peak -- measure, on the given device, the sustained rate of a dependent-free stream
+ * of FP64 FMA (which = 0), FP32 FMA (which = 1) or MUFU.SIN (which = 2) instructions, in thread-level
+ * instructions per second, over roughly `millis` milliseconds.  It is the measured denominator of the
+ * "alu" roofline bench.py reports.  Also returns the SM count.
+ */
+FSTAT_API fstat_status fstat_probe_pipe_peak(int32_t device, int32_t which, double millis,
+                                             double *inst_per_s, int32_t *n_sm);
+
+FSTAT_API const char *fstat_status_str(fstat_status s);
+/* Human-readable reason of the most recent failing call on this plan; plan == NULL returns the
+ * reason of the most recent failing fstat_plan_create on the calling thread.  Never NULL. */
+FSTAT_API const char *fstat_last_error(const fstat_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FSTAT_H_ */

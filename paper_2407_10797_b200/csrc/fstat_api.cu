@@ -1,0 +1,538 @@
+// fstat_api.cu -- the C ABI declared in include/fstat.h: plan management, argument validation,
+// segmentation of the frequency band into CTA work items, workspace, launches.  Host code only; every
+// arithmetic step of the hot path lives in fstat_kernels.cu.  There is no CPU fallback.
+#include "../../include/fstat.h"
+#include "fstat_internal.h"
+
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace fstat;
+
+struct fstat_plan {
+    int device = 0;
+    int n_sm = 0;
+    int64_t n_bins = 0;
+    double df = 0.0;
+    fstat_options opt{};
+    int32_t n_part = 0;
+    std::vector<int64_t> edges;        // host copy [n_part+1]
+    double *d_table = nullptr;         // [n_bins][kTabW]
+    // segmentation (depends on the partitions and on the number of particle groups)
+    int32_t seg_groups = -1;           // n_groups the current segmentation was made for
+    int32_t n_seg = 0;
+    int32_t *d_seg_edge = nullptr;     // [n_seg+1]
+    int32_t *d_part_seg = nullptr;     // [n_part+1]
+    size_t seg_cap = 0, part_cap = 0;
+    // workspace
+    double *d_coef = nullptr;  size_t coef_cap = 0;      // doubles
+    int32_t *d_valid = nullptr; size_t valid_cap = 0;    // ints
+    double *d_partial = nullptr; size_t partial_cap = 0; // doubles
+    // host-buffer path
+    double *d_params = nullptr, *d_F = nullptr, *d_Fk = nullptr;
+    size_t params_cap = 0, F_cap = 0, Fk_cap = 0;
+    OrbitCoef orb{};
+    // ring of event pairs around the main kernel of the most recent evaluations (bench roofline)
+    static constexpr int kRing = 128;
+    cudaEvent_t ev0[kRing] = {}, ev1[kRing] = {};
+    int64_t n_timed = 0;
+    std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static fstat_status fail(fstat_plan *pl, fstat_status s, const std::string &msg)
+{
+    if (pl) pl->err = msg; else g_create_err = msg;
+    return s;
+}
+
+#define CU_TRY(pl, call)                                                                             \
+    do {                                                                                             \
+        cudaError_t e__ = (call);                                                                    \
+        if (e__ != cudaSuccess) {                                                                    \
+            const bool oom__ = (e__ == cudaErrorMemoryAllocation);                                   \
+            cudaGetLastError();                                                                      \
+            return fail(pl, oom__ ? FSTAT_ENOMEM : FSTAT_ECUDA,                                      \
+                        std::string(#call) + ": " + cudaGetErrorString(e__));                        \
+        }                                                                                            \
+    } while (0)
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int dev) { ok = (cudaGetDevice(&prev) == cudaSuccess) && (cudaSetDevice(dev) == cudaSuccess); }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+template <class T>
+cudaError_t grow(T **ptr, size_t *cap, size_t need)
+{
+    if (need <= *cap) return cudaSuccess;
+    if (*ptr) { cudaFree(*ptr); *ptr = nullptr; *cap = 0; }
+    cudaError_t e = cudaMalloc((void **)ptr, need * sizeof(T));
+    if (e == cudaSuccess) *cap = need;
+    return e;
+}
+
+bool edges_valid(int64_t n_bins, int32_t n_part, const int64_t *e, std::string *why)
+{
+    if (n_part < 1) { *why = "n_part < 1"; return false; }
+    if (!e) { *why = "part_edges is NULL"; return false; }
+    if (e[0] != 0) { *why = "part_edges[0] != 0"; return false; }
+    if (e[n_part] != n_bins) { *why = "part_edges[n_part] != n_bins"; return false; }
+    for (int32_t k = 0; k < n_part; ++k)
+        if (!(e[k + 1] > e[k])) { *why = "part_edges not strictly increasing (empty partition)"; return false; }
+    return true;
+}
+
+// Split every partition into near-equal segments of at most max_len bins.  A segment never crosses a
+// partition edge, so the main kernel needs no per-bin edge test and writes plain partial sums.
+void make_segments(const std::vector<int64_t> &edges, int64_t max_len, std::vector<int32_t> *seg_edge,
+                   std::vector<int32_t> *part_seg)
+{
+    const size_t n_part = edges.size() - 1;
+    seg_edge->clear();
+    part_seg->assign(n_part + 1, 0);
+    seg_edge->push_back(0);
+    for (size_t k = 0; k < n_part; ++k) {
+        const int64_t lo = edges[k], len = edges[k + 1] - edges[k];
+        const int64_t n = (len + max_len - 1) / max_len;
+        (*part_seg)[k] = (int32_t)(seg_edge->size() - 1);
+        for (int64_t s = 1; s <= n; ++s) seg_edge->push_back((int32_t)(lo + (len * s) / n));
+    }
+    (*part_seg)[n_part] = (int32_t)(seg_edge->size() - 1);
+}
+
+int64_t auto_segment_len(const fstat_plan *pl, int32_t n_groups)
+{
+    if (pl->opt.max_segment_bins > 0) return pl->opt.max_segment_bins;
+    // aim at >= 24 CTAs per SM in flight order (8 waves at 3 CTAs/SM) so the tail wave is short
+    const int64_t target_ctas = (int64_t)pl->n_sm * 24;
+    int64_t want_seg = (target_ctas + n_groups - 1) / n_groups;
+    if (want_seg < 1) want_seg = 1;
+    int64_t len = (pl->n_bins + want_seg - 1) / want_seg;
+    len = ((len + kTileBins - 1) / kTileBins) * kTileBins;
+    if (len < 4 * kTileBins) len = 4 * kTileBins;
+    if (len > 64 * kTileBins) len = 64 * kTileBins;
+    return len;
+}
+
+fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
+{
+    if (pl->seg_groups == n_groups) return FSTAT_OK;
+    std::vector<int32_t> seg_edge, part_seg;
+    make_segments(pl->edges, auto_segment_len(pl, n_groups), &seg_edge, &part_seg);
+    CU_TRY(pl, grow(&pl->d_seg_edge, &pl->seg_cap, seg_edge.size()));
+    CU_TRY(pl, grow(&pl->d_part_seg, &pl->part_cap, part_seg.size()));
+    // synchronous copies: they order after any earlier evaluation that still reads the old arrays
+    CU_TRY(pl, cudaDeviceSynchronize());
+    CU_TRY(pl, cudaMemcpy(pl->d_seg_edge, seg_edge.data(), seg_edge.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    CU_TRY(pl, cudaMemcpy(pl->d_part_seg, part_seg.data(), part_seg.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    pl->n_seg = (int32_t)seg_edge.size() - 1;
+    pl->seg_groups = n_groups;
+    return FSTAT_OK;
+}
+
+int64_t n_segments_for(const fstat_plan *pl, int32_t n_groups)
+{
+    const int64_t max_len = auto_segment_len(pl, n_groups);
+    int64_t n = 0;
+    for (size_t k = 0; k + 1 < pl->edges.size(); ++k) n += (pl->edges[k + 1] - pl->edges[k] + max_len - 1) / max_len;
+    return n;
+}
+
+}  // namespace
+
+// The orbit of PAPER.md:198 (analytic, second order in the eccentricity e = L / (2 sqrt(3) AU); formulas
+// of DESIGN.md reading A9) written as trigonometric polynomials in alpha = 2 pi t / yr + kappa.
+void fstat::make_orbit_coef(double L, double lambda, OrbitCoef *out)
+{
+    const long double R = kAU, pi = 3.14159265358979323846264338327950288L;
+    const long double e = (long double)L / (2.0L * sqrtl(3.0L) * R);
+    long double Pn[3][3][7];
+    for (int n = 0; n < 3; ++n) {
+        const long double be = 2.0L * pi * n / 3.0L + (long double)lambda;
+        const long double cb = cosl(be), sb = sinl(be), c2b = cosl(2 * be), s2b = sinl(2 * be);
+        long double(*C)[7] = Pn[n];
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 7; ++j) C[i][j] = 0.0L;
+        // x
+        C[0][0] = -1.5L * e * R * cb;
+        C[0][1] = R - 1.25L * e * e * R - 0.625L * e * e * R * c2b;
+        C[0][2] = -0.625L * e * e * R * s2b;
+        C[0][3] = 0.5L * e * R * cb;
+        C[0][4] = 0.5L * e * R * sb;
+        C[0][5] = 0.375L * e * e * R * c2b;
+        C[0][6] = 0.375L * e * e * R * s2b;
+        // y
+        C[1][0] = -1.5L * e * R * sb;
+        C[1][1] = -0.625L * e * e * R * s2b;
+        C[1][2] = R - 1.25L * e * e * R + 0.625L * e * e * R * c2b;
+        C[1][3] = -0.5L * e * R * sb;
+        C[1][4] = 0.5L * e * R * cb;
+        C[1][5] = -0.375L * e * e * R * s2b;
+        C[1][6] = 0.375L * e * e * R * c2b;
+        // z = -sqrt3 e R cos(a - b) + sqrt3 e^2 R (3/2 - cos(2a - 2b)/2)
+        const long double s3 = sqrtl(3.0L);
+        C[2][0] = 1.5L * s3 * e * e * R;
+        C[2][1] = -s3 * e * R * cb;
+        C[2][2] = -s3 * e * R * sb;
+        C[2][3] = -0.5L * s3 * e * e * R * c2b;
+        C[2][4] = -0.5L * s3 * e * e * R * s2b;
+    }
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 7; ++j) {
+            out->c[0][i][j] = (double)(4.0L * Pn[0][i][j] / (long double)kC);
+            out->c[1][i][j] = (double)((Pn[1][i][j] - Pn[0][i][j]) / (long double)L);
+            out->c[2][i][j] = (double)((Pn[2][i][j] - Pn[0][i][j]) / (long double)L);
+        }
+}
+
+extern "C" {
+
+void fstat_default_options(fstat_options *o)
+{
+    if (!o) return;
+    memset(o, 0, sizeof(*o));
+    o->f_ref_e0 = 0.01;
+    o->arm_length_m = 2.5e9;
+    o->orbit_kappa = 0.0;
+    o->orbit_lambda = 0.0;
+    o->device = -1;
+    o->inputs_on_device = 0;
+    o->max_segment_bins = 0;
+}
+
+const char *fstat_status_str(fstat_status s)
+{
+    switch (s) {
+        case FSTAT_OK: return "FSTAT_OK";
+        case FSTAT_EINVAL: return "FSTAT_EINVAL";
+        case FSTAT_ENOMEM: return "FSTAT_ENOMEM";
+        case FSTAT_ECUDA: return "FSTAT_ECUDA";
+        case FSTAT_EUNSUPPORTED: return "FSTAT_EUNSUPPORTED";
+    }
+    return "FSTAT_?";
+}
+
+const char *fstat_last_error(const fstat_plan *pl) { return pl ? pl->err.c_str() : g_create_err.c_str(); }
+
+fstat_status fstat_edges_equal_bins(int64_t n_bins, int32_t n_part, int64_t *edges_out)
+{
+    if (!edges_out || n_part < 1 || n_bins < 1 || (int64_t)n_part > n_bins) return FSTAT_EINVAL;
+    for (int32_t j = 0; j <= n_part; ++j)
+        edges_out[j] = (int64_t)(((__int128)j * (__int128)n_bins) / (__int128)n_part);
+    return FSTAT_OK;
+}
+
+static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const double *freq, const double *dw,
+                                     const double *isn)
+{
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaDeviceProp prop;
+    CU_TRY(pl, cudaGetDeviceProperties(&prop, pl->device));
+    pl->n_sm = prop.multiProcessorCount;
+    if (prop.major < 10)
+        return fail(pl, FSTAT_ECUDA, "device is not sm_100-class (this library ships sm_100a code only)");
+    CU_TRY(pl, main_kernel_configure());
+
+    const double *d_freq = freq, *d_dw = dw, *d_isn = isn;
+    double *tmp = nullptr;
+    if (!pl->opt.inputs_on_device) {
+        CU_TRY(pl, cudaMalloc((void **)&tmp, (size_t)n_bins * 4 * sizeof(double)));
+        cudaError_t e = cudaMemcpy(tmp, freq, (size_t)n_bins * sizeof(double), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(tmp + n_bins, dw, (size_t)n_bins * 2 * sizeof(double), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(tmp + 3 * n_bins, isn, (size_t)n_bins * sizeof(double), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { cudaFree(tmp); CU_TRY(pl, e); }
+        d_freq = tmp; d_dw = tmp + n_bins; d_isn = tmp + 3 * n_bins;
+    }
+    // df as the oracle-independent statement of the contract: (f[N-1] - f[0]) / (N - 1)
+    double fe[2] = {0, 0};
+    cudaError_t e = cudaMemcpy(&fe[0], d_freq, sizeof(double), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(&fe[1], d_freq + (n_bins - 1), sizeof(double), cudaMemcpyDeviceToHost);
+    uint32_t *d_err = nullptr;
+    if (e == cudaSuccess) e = cudaMalloc((void **)&d_err, sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemset(d_err, 0, sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_table, (size_t)n_bins * kTabW * sizeof(double));
+    uint32_t bits = 0;
+    if (e == cudaSuccess) {
+        pl->df = (n_bins > 1) ? (fe[1] - fe[0]) / (double)(n_bins - 1) : fe[0];
+        if (!(pl->df > 0.0) || !isfinite(pl->df)) bits |= ERR_FREQ_ORDER;
+        else {
+            e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->opt.f_ref_e0,
+                                   pl->d_table, d_err, 0);
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+            if (e == cudaSuccess) e = cudaMemcpy(&bits, d_err, sizeof(uint32_t), cudaMemcpyDeviceToHost);
+        }
+    }
+    if (tmp) cudaFree(tmp);
+    if (d_err) cudaFree(d_err);
+    CU_TRY(pl, e);
+    if (bits) {
+        std::string why;
+        if (bits & ERR_FREQ_NONPOS) why += "freq_hz has a non-positive or non-finite entry; ";
+        if (bits & ERR_FREQ_ORDER) why += "freq_hz is not strictly ascending; ";
+        if (bits & ERR_FREQ_UNIFORM) why += "freq_hz is not a uniform grid; ";
+        if (bits & ERR_DW_NONFINITE) why += "dw_re_im has a non-finite entry; ";
+        if (bits & ERR_ISN_NONFINITE) why += "inv_sn has a non-finite entry; ";
+        if (bits & ERR_ISN_NONPOS) why += "inv_sn has an entry <= 0; ";
+        return fail(pl, FSTAT_EINVAL, why);
+    }
+    make_orbit_coef(pl->opt.arm_length_m, pl->opt.orbit_lambda, &pl->orb);
+    for (int i = 0; i < fstat_plan::kRing; ++i) {
+        CU_TRY(pl, cudaEventCreate(&pl->ev0[i]));
+        CU_TRY(pl, cudaEventCreate(&pl->ev1[i]));
+    }
+    return FSTAT_OK;
+}
+
+static void plan_free(fstat_plan *pl)
+{
+    if (!pl) return;
+    DeviceGuard g(pl->device);
+    cudaFree(pl->d_table); cudaFree(pl->d_seg_edge); cudaFree(pl->d_part_seg); cudaFree(pl->d_coef);
+    cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
+    for (int i = 0; i < fstat_plan::kRing; ++i) {
+        if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
+        if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
+    }
+    delete pl;
+}
+
+fstat_status fstat_plan_create(fstat_plan **out, int64_t n_bins, const double *freq_hz, const double *dw_re_im,
+                               const double *inv_sn, int32_t n_part, const int64_t *part_edges,
+                               const fstat_options *opts)
+{
+    if (!out) return fail(nullptr, FSTAT_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (n_bins < 1) return fail(nullptr, FSTAT_EINVAL, "n_bins < 1");
+    if (n_bins >= (int64_t)1 << 31) return fail(nullptr, FSTAT_EUNSUPPORTED, "n_bins >= 2^31");
+    if (!freq_hz || !dw_re_im || !inv_sn) return fail(nullptr, FSTAT_EINVAL, "freq_hz, dw_re_im or inv_sn is NULL");
+    std::string why;
+    if (!edges_valid(n_bins, n_part, part_edges, &why)) return fail(nullptr, FSTAT_EINVAL, why);
+    fstat_options o;
+    fstat_default_options(&o);
+    if (opts) o = *opts;
+    if (!(o.f_ref_e0 > 0.0) || !(o.arm_length_m > 0.0) || !isfinite(o.orbit_kappa) || !isfinite(o.orbit_lambda) ||
+        o.max_segment_bins < 0)
+        return fail(nullptr, FSTAT_EINVAL, "bad option value");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, FSTAT_ECUDA, "no CUDA device available (there is no CPU fallback)");
+    }
+    int dev = o.device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return fail(nullptr, FSTAT_ECUDA, "cudaGetDevice failed");
+    if (dev >= n_dev) return fail(nullptr, FSTAT_EINVAL, "device ordinal out of range");
+
+    fstat_plan *pl = new (std::nothrow) fstat_plan;
+    if (!pl) return fail(nullptr, FSTAT_ENOMEM, "host allocation failed");
+    pl->device = dev;
+    pl->n_bins = n_bins;
+    pl->opt = o;
+    pl->n_part = n_part;
+    try {
+        pl->edges.assign(part_edges, part_edges + n_part + 1);
+    } catch (...) {
+        delete pl;
+        return fail(nullptr, FSTAT_ENOMEM, "host allocation failed");
+    }
+    fstat_status s = plan_create_impl(pl, n_bins, freq_hz, dw_re_im, inv_sn);
+    if (s != FSTAT_OK) {
+        g_create_err = pl->err;
+        plan_free(pl);
+        return s;
+    }
+    *out = pl;
+    return FSTAT_OK;
+}
+
+fstat_status fstat_plan_set_partitions(fstat_plan *pl, int32_t n_part, const int64_t *part_edges)
+{
+    if (!pl) return FSTAT_EINVAL;
+    std::string why;
+    if (!edges_valid(pl->n_bins, n_part, part_edges, &why)) return fail(pl, FSTAT_EINVAL, why);
+    try {
+        pl->edges.assign(part_edges, part_edges + n_part + 1);
+    } catch (...) {
+        return fail(pl, FSTAT_ENOMEM, "host allocation failed");
+    }
+    pl->n_part = n_part;
+    pl->seg_groups = -1;    // re-segment on the next evaluation
+    return FSTAT_OK;
+}
+
+void fstat_plan_destroy(fstat_plan *pl) { plan_free(pl); }
+
+int64_t fstat_plan_n_bins(const fstat_plan *pl) { return pl ? pl->n_bins : 0; }
+int32_t fstat_plan_n_part(const fstat_plan *pl) { return pl ? pl->n_part : 0; }
+int32_t fstat_plan_device(const fstat_plan *pl) { return pl ? pl->device : -1; }
+int32_t fstat_launches_per_eval(void) { return 3; }
+
+int64_t fstat_plan_n_ctas(const fstat_plan *pl, int64_t P)
+{
+    if (!pl || P < 1) return 0;
+    const int64_t n_groups = (P + kThreads - 1) / kThreads;
+    return n_groups * n_segments_for(pl, (int32_t)n_groups);
+}
+
+int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out)
+{
+    if (!pl || !ms_out || n_last < 1) return 0;
+    DeviceGuard g(pl->device);
+    int64_t n = pl->n_timed < fstat_plan::kRing ? pl->n_timed : fstat_plan::kRing;
+    if (n > n_last) n = n_last;
+    int32_t w = 0;
+    for (int64_t i = pl->n_timed - n; i < pl->n_timed; ++i) {      // oldest first
+        const int s = (int)(i % fstat_plan::kRing);
+        float ms = -1.f;
+        if (cudaEventSynchronize(pl->ev1[s]) != cudaSuccess) { cudaGetLastError(); break; }
+        if (cudaEventElapsedTime(&ms, pl->ev0[s], pl->ev1[s]) != cudaSuccess) { cudaGetLastError(); break; }
+        ms_out[w++] = (double)ms;
+    }
+    return w;
+}
+
+fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, void *stream)
+{
+    if (!pl) return FSTAT_EINVAL;
+    if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
+    if (P == 0) return FSTAT_OK;
+    if (!params || !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)stream;
+
+    const int64_t n_groups = (P + kThreads - 1) / kThreads;
+    const int64_t P_pad = n_groups * kThreads;
+    fstat_status s = ensure_segments(pl, (int32_t)n_groups);
+    if (s != FSTAT_OK) return s;
+    if ((int64_t)pl->n_seg * n_groups >= ((int64_t)1 << 31))
+        return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
+    CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)P_pad * kNCoef));
+    CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_partial, &pl->partial_cap, (size_t)pl->n_seg * kNAcc * (size_t)P_pad));
+
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef, pl->d_valid, st));
+    MainArgs a;
+    a.table = pl->d_table;
+    a.coef = pl->d_coef;
+    a.seg_edge = pl->d_seg_edge;
+    a.partial = pl->d_partial;
+    a.P_pad = P_pad;
+    a.P = (int32_t)P;
+    a.n_groups = (int32_t)n_groups;
+    a.n_seg = pl->n_seg;
+    a.orb = pl->orb;
+    const int slot = (int)(pl->n_timed % fstat_plan::kRing);
+    CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
+    CU_TRY(pl, launch_main(a, st));
+    CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
+    ++pl->n_timed;
+    CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, P, P_pad, pl->n_part, F, Fk, st));
+    return FSTAT_OK;
+}
+
+fstat_status fstat_eval_batch_host(fstat_plan *pl, int64_t P, const double *params_host, double *F_host,
+                                   double *Fk_host, void *stream)
+{
+    if (!pl) return FSTAT_EINVAL;
+    if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
+    if (P == 0) return FSTAT_OK;
+    if (!params_host || !F_host) return fail(pl, FSTAT_EINVAL, "params_host or F_host is NULL");
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(pl, grow(&pl->d_params, &pl->params_cap, (size_t)P * 6));
+    CU_TRY(pl, grow(&pl->d_F, &pl->F_cap, (size_t)P));
+    if (Fk_host) CU_TRY(pl, grow(&pl->d_Fk, &pl->Fk_cap, (size_t)P * (size_t)pl->n_part));
+    CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, (size_t)P * 6 * sizeof(double), cudaMemcpyHostToDevice, st));
+    fstat_status s = fstat_eval_batch(pl, P, pl->d_params, pl->d_F, Fk_host ? pl->d_Fk : nullptr, stream);
+    if (s != FSTAT_OK) return s;
+    CU_TRY(pl, cudaMemcpyAsync(F_host, pl->d_F, (size_t)P * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (Fk_host)
+        CU_TRY(pl, cudaMemcpyAsync(Fk_host, pl->d_Fk, (size_t)P * (size_t)pl->n_part * sizeof(double),
+                                   cudaMemcpyDeviceToHost, st));
+    CU_TRY(pl, cudaStreamSynchronize(st));
+    return FSTAT_OK;
+}
+
+fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, double *u_plus, double *u_cross,
+                                 void *stream)
+{
+    if (!pl) return FSTAT_EINVAL;
+    if (!params_host || !u_plus || !u_cross) return fail(pl, FSTAT_EINVAL, "params_host, u_plus or u_cross is NULL");
+    const double *q = params_host;
+    for (int i = 0; i < 6; ++i)
+        if (!isfinite(q[i])) return fail(pl, FSTAT_EINVAL, "non-finite parameter");
+    if (!(q[1] > 0.0) || !(q[2] > 0.0 && q[2] <= 0.25) || !(q[5] >= 0.0))
+        return fail(pl, FSTAT_EINVAL, "parameter outside the physical domain (M_c > 0, 0 < eta <= 1/4, e0 >= 0)");
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(pl, grow(&pl->d_params, &pl->params_cap, (size_t)6));
+    CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)kThreads * kNCoef));
+    CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)kThreads));
+    CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
+    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef,
+                               pl->d_valid, st));
+    CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, u_plus, u_cross, st));
+    CU_TRY(pl, cudaStreamSynchronize(st));
+    return FSTAT_OK;
+}
+
+fstat_status fstat_probe_pipe_peak(int32_t device, int32_t which, double millis, double *inst_per_s, int32_t *n_sm_out)
+{
+    if (!inst_per_s || which < 0 || which > 2) return FSTAT_EINVAL;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); return FSTAT_ECUDA; }
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return FSTAT_ECUDA;
+    if (dev >= n_dev) return FSTAT_EINVAL;
+    DeviceGuard g(dev);
+    if (!g.ok) return FSTAT_ECUDA;
+    int n_sm = 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return FSTAT_ECUDA;
+    if (n_sm_out) *n_sm_out = n_sm;
+    double *sink = nullptr;
+    if (cudaMalloc((void **)&sink, sizeof(double)) != cudaSuccess) return FSTAT_ENOMEM;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int n_blocks = n_sm * 8;
+    int iters = 2000;
+    fstat_status rc = FSTAT_OK;
+    double best = 0.0;
+    // calibrate, then repeat until about `millis` of kernel time has been spent; keep the best rate
+    double spent = 0.0;
+    for (int rep = 0; rep < 64 && rc == FSTAT_OK; ++rep) {
+        cudaEventRecord(e0, 0);
+        if (launch_probe(which, n_blocks, iters, sink, 0) != cudaSuccess) { rc = FSTAT_ECUDA; break; }
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { rc = FSTAT_ECUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double inst = (double)n_blocks * 256.0 * (double)iters * 64.0;
+        if (ms > 0.f && rep > 0) { const double r = inst / (ms * 1e-3); if (r > best) best = r; }
+        if (rep > 0) spent += ms;
+        if (ms < 2.0f && iters < (1 << 24)) iters *= 4;
+        if (spent >= millis && rep >= 3) break;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    *inst_per_s = best;
+    return rc;
+}
+
+}  // extern "C"

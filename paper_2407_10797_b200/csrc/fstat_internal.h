@@ -1,0 +1,88 @@
+// fstat_internal.h -- shared between the C-ABI host code (fstat_api.cu) and the kernels
+// (fstat_kernels.cu): constants, table layout, launcher prototypes.  Product path only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fstat {
+
+// physical constants
+constexpr double kC = 299792458.0;                 // m/s
+constexpr double kGMsunC3 = 4.925490947641267e-6;  // G Msun / c^3 [s]
+constexpr double kAU = 149597870700.0;             // m
+constexpr double kYear = 31557600.0;               // Julian year [s]
+constexpr double kEulerGamma = 0.5772156649015329;
+constexpr double kPi = 3.14159265358979323846;
+
+// ---- per-bin table ("a0", plan time): kTabW doubles per frequency bin, one contiguous row so that a
+// tile of bins is ONE TMA bulk copy.  Phase basis B_j and its derivative D_j = (dB_j/df)/year:
+//   Psi [quarter turns] = c1 + c0 f + sum_{j=2..9} c_j B_j(f),   alpha [quarter turns] = a0 + sum c_j D_j(f)
+enum TabCol : int {
+    T_F = 0,      // f
+    T_LNF,        // ln f
+    T_FM53,       // f^(-5/3)
+    T_FM1,        // f^(-1)
+    T_FM23,       // f^(-2/3)
+    T_FM13,       // f^(-1/3)
+    T_FP13,       // f^(1/3)
+    T_FP13LN,     // f^(1/3) ln f
+    T_FM349,      // f^(-34/9)
+    T_XQ,         // 2 f L / c  = (pi f L / c) in quarter turns
+    T_D0,         // D_j, j = 2..9 in the order of the B_j above (8 columns: T_D0 .. T_D0+7)
+    T_C2X = 18,   // cos(2 pi f L / c)
+    T_S2X,        // sin(2 pi f L / c)
+    T_DWR,        // Re, Im of  4 df f^(-7/6) conj(K_f) d~/S_n,   K_f = -i (1 - z^2), z = exp(-2 pi i f L/c)
+    T_DWI,
+    T_W,          // 4 df f^(-7/3) |K_f|^2 / S_n
+    T_X,          // pi f L / c [rad]
+    kTabW = 24
+};
+
+constexpr int kNCoef = 20;   // per-particle coefficients: c0..c9, a0, k[3], u[3], v[3]
+constexpr int kNAcc = 8;     // z_+ (re, im), z_x (re, im), m_pp, m_cc, m_pc (re, im)
+constexpr int kThreads = 128;    // particles per CTA of the main kernel (one thread = one particle)
+constexpr int kTileBins = 64;    // bins per TMA tile (64 * 24 * 8 B = 12 KiB)
+constexpr int kStages = 3;       // TMA ring depth
+
+// Orbit model coefficients: coordinate = C[0] + C[1] cos a + C[2] sin a + C[3] cos 2a + C[4] sin 2a
+//                                        + C[5] cos 3a + C[6] sin 3a      (z has C[5] = C[6] = 0)
+// vec 0: 4 p_1 / c  [quarter turns per Hz];  vec 1: (p_2 - p_1)/L;  vec 2: (p_3 - p_1)/L.
+struct OrbitCoef {
+    double c[3][3][7];
+};
+
+struct MainArgs {
+    const double *table;      // [n_bins][kTabW]
+    const double *coef;       // [kNCoef][P_pad]
+    const int32_t *seg_edge;  // [n_seg + 1]
+    double *partial;          // [n_seg][kNAcc][P_pad]
+    int64_t P_pad;
+    int32_t P;
+    int32_t n_groups;
+    int32_t n_seg;
+    OrbitCoef orb;
+};
+
+// error bits raised by the table kernel (input validation on the device)
+enum : uint32_t {
+    ERR_FREQ_NONPOS = 1u, ERR_FREQ_ORDER = 2u, ERR_FREQ_UNIFORM = 4u, ERR_DW_NONFINITE = 8u,
+    ERR_ISN_NONFINITE = 16u, ERR_ISN_NONPOS = 32u
+};
+
+cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
+                               double df, double arm_length_m, double f_ref_e0, double *table,
+                               uint32_t *err_bits, cudaStream_t st);
+cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
+                            double *coef, int32_t *valid, cudaStream_t st);
+cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
+cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
+                            int64_t P_pad, int32_t n_part, double *F, double *Fk, cudaStream_t st);
+cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
+                            const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st);
+cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaStream_t st);
+size_t main_kernel_smem_bytes();
+cudaError_t main_kernel_configure();
+
+void make_orbit_coef(double arm_length_m, double lambda, OrbitCoef *out);
+
+}  // namespace fstat

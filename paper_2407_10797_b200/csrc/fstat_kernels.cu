@@ -1,0 +1,568 @@
+// fstat_kernels.cu -- sm_100a kernels of the batched semi-coherent F-statistic (arXiv 2407.10797).
+//
+//   build_table_kernel   (a0, plan time)  per-bin, particle-independent factors of Eq. A1/A3 and Eq. 4
+//   prologue_kernel      (a1)             per-particle PN / eccentric phase coefficients and sky vectors
+//   fstat_main_kernel    (a2-a5)          fused phase + t_f + orbit + TDI-X response + inner products;
+//                                         one thread = one particle, bins streamed through shared memory
+//                                         by TMA bulk copies; no template ever leaves the registers
+//   epilogue_kernel      (a6)             2 F_k = z^H G^-1 z per partition, F = sum_k F_k
+//
+// Citations are to /root/reference/PAPER.md (line, equation) and to DESIGN.md readings (A1..A24).
+#include "fstat_device.cuh"
+#include "fstat_internal.h"
+
+#include <math.h>
+
+namespace fstat {
+
+// =================================================================================================
+// a0: per-bin table
+// =================================================================================================
+__global__ void build_table_kernel(const double *__restrict__ freq, const double *__restrict__ dw,
+                                   const double *__restrict__ isn, int64_t n_bins, double df, double L,
+                                   double *__restrict__ table, uint32_t *__restrict__ err_bits)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_bins) return;
+    const double f = freq[i];
+    uint32_t err = 0;
+    if (!(f > 0.0) || !isfinite(f)) err |= ERR_FREQ_NONPOS;
+    if (i > 0 && !(f > freq[i - 1])) err |= ERR_FREQ_ORDER;
+    if (n_bins > 1 && !(fabs(f - (freq[0] + (double)i * df)) <= 1e-6 * df)) err |= ERR_FREQ_UNIFORM;
+    const double dr = dw[2 * i], di = dw[2 * i + 1], w = isn[i];
+    if (!isfinite(dr) || !isfinite(di)) err |= ERR_DW_NONFINITE;
+    if (!isfinite(w)) err |= ERR_ISN_NONFINITE;
+    else if (!(w > 0.0)) err |= ERR_ISN_NONPOS;
+    if (err) { atomicOr(err_bits, err); return; }
+
+    double *row = table + i * kTabW;
+    const double lnf = log(f);
+    const double cb = cbrt(f);                 // f^(1/3)
+    const double icb = 1.0 / cb;               // f^(-1/3)
+    const double fm23 = icb * icb;
+    const double fm1 = 1.0 / f;
+    const double fm53 = fm1 * fm23;
+    const double fm349 = pow(f, -34.0 / 9.0);
+    const double iyr = 1.0 / kYear;
+    row[T_F] = f;
+    row[T_LNF] = lnf;
+    row[T_FM53] = fm53;
+    row[T_FM1] = fm1;
+    row[T_FM23] = fm23;
+    row[T_FM13] = icb;
+    row[T_FP13] = cb;
+    row[T_FP13LN] = cb * lnf;
+    row[T_FM349] = fm349;
+    row[T_XQ] = 2.0 * f * L / kC;
+    // D_j = (dB_j/df) / year, same order as B_2..B_9
+    row[T_D0 + 0] = fm1 * iyr;                                   // ln f
+    row[T_D0 + 1] = (-5.0 / 3.0) * fm53 * fm1 * iyr;              // f^(-5/3)
+    row[T_D0 + 2] = -fm1 * fm1 * iyr;                             // f^(-1)
+    row[T_D0 + 3] = (-2.0 / 3.0) * fm53 * iyr;                    // f^(-2/3)
+    row[T_D0 + 4] = (-1.0 / 3.0) * icb * fm1 * iyr;               // f^(-1/3)
+    row[T_D0 + 5] = (1.0 / 3.0) * fm23 * iyr;                     // f^(1/3)
+    row[T_D0 + 6] = fm23 * (1.0 + lnf / 3.0) * iyr;               // f^(1/3) ln f
+    row[T_D0 + 7] = (-34.0 / 9.0) * fm349 * fm1 * iyr;            // f^(-34/9)
+    const double x = kPi * f * L / kC;
+    double s2x, c2x;
+    sincos(2.0 * x, &s2x, &c2x);
+    row[T_C2X] = c2x;
+    row[T_S2X] = s2x;
+    // conj(K_f) = 2 sin 2x (cos 2x + i sin 2x), |K_f|^2 = 4 sin^2 2x   (K_f = -i (1 - z^2))
+    const double amp = 4.0 * df * pow(f, -7.0 / 6.0);
+    const double kr = 2.0 * s2x * c2x, ki = 2.0 * s2x * s2x;
+    row[T_DWR] = amp * (dr * kr - di * ki);
+    row[T_DWI] = amp * (dr * ki + di * kr);
+    row[T_W] = 4.0 * df * pow(f, -7.0 / 3.0) * (4.0 * s2x * s2x) * w;
+    row[T_X] = x;
+}
+
+cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
+                               double df, double arm_length_m, double /*f_ref_e0*/, double *table,
+                               uint32_t *err_bits, cudaStream_t st)
+{
+    const int nt = 256;
+    const int64_t nb = (n_bins + nt - 1) / nt;
+    build_table_kernel<<<(unsigned)nb, nt, 0, st>>>(freq, dw, isn, n_bins, df, arm_length_m, table, err_bits);
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// a1: per-particle coefficients (PAPER.md:404 Eq. A3 with readings A1-A3; :71 parameter meanings)
+// =================================================================================================
+__global__ void prologue_kernel(const double *__restrict__ params, int64_t P, int64_t P_pad, double f_ref,
+                                double kappa, double *__restrict__ coef, int32_t *__restrict__ valid)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P_pad) return;
+    double c[kNCoef];
+#pragma unroll
+    for (int j = 0; j < kNCoef; ++j) c[j] = 0.0;
+    int ok = 0;
+    if (p < P) {
+        const double tc = params[6 * p + 0], Mc = params[6 * p + 1], eta = params[6 * p + 2];
+        const double theta = params[6 * p + 3], phi = params[6 * p + 4], e0 = params[6 * p + 5];
+        ok = isfinite(tc) && isfinite(Mc) && isfinite(eta) && isfinite(theta) && isfinite(phi) && isfinite(e0) &&
+             (Mc > 0.0) && (eta > 0.0) && (eta <= 0.25) && (e0 >= 0.0);
+        if (ok) {
+            const double pi = kPi;
+            const double Mcs = Mc * kGMsunC3;
+            const double M = Mcs * pow(eta, -0.6);
+            const double V = cbrt(pi * M);                                    // v = V f^(1/3)
+            const double Kq = (3.0 / 128.0) * pow(pi * Mcs, -5.0 / 3.0) * (2.0 / pi);   // quarter turns
+            const double V2 = V * V, V3 = V2 * V, V4 = V2 * V2, V5 = V4 * V, V6 = V3 * V3;
+            const double lnV = log(V);
+            const double al2 = 3715.0 / 756.0 + 55.0 * eta / 9.0;
+            const double al3 = -16.0 * pi;
+            const double al4 = 15293365.0 / 508032.0 + 27145.0 * eta / 504.0 + 3085.0 * eta * eta / 72.0;
+            const double a5c = pi * (38645.0 / 756.0 - 65.0 * eta / 9.0);    // alpha_5 = a5c (1 + 3 ln(v/v_lso))
+            const double a6c = 11583231236531.0 / 4694215680.0 - 640.0 * pi * pi / 3.0 - 6848.0 * kEulerGamma / 21.0 +
+                               eta * (-15737765635.0 / 3048192.0 + 2255.0 * pi * pi / 12.0) +
+                               76055.0 * eta * eta / 1728.0 - 127825.0 * eta * eta * eta / 1296.0;
+            const double ln_vlso = -0.5 * log(6.0);
+            c[0] = 4.0 * tc;                                                   // 2 pi f tc
+            c[1] = -0.5 + Kq * V5 * a5c * (1.0 + 3.0 * lnV - 3.0 * ln_vlso);   // -pi/4 + constant part of k = 5
+            c[2] = Kq * V5 * a5c;                                              // ln f
+            c[3] = Kq;                                                         // f^(-5/3), alpha_0 = 1
+            c[4] = Kq * al2 * V2;                                              // f^(-1)
+            c[5] = Kq * al3 * V3;                                              // f^(-2/3)
+            c[6] = Kq * al4 * V4;                                              // f^(-1/3)
+            c[7] = Kq * V6 * (a6c - (6848.0 / 21.0) * (log(4.0) + lnV));       // f^(1/3)
+            c[8] = -Kq * V6 * (6848.0 / 63.0);                                 // f^(1/3) ln f
+            c[9] = -Kq * (2355.0 / 1462.0) * e0 * e0 * pow(f_ref, 19.0 / 9.0); // f^(-34/9)  (reading A3)
+            c[10] = 4.0 * tc / kYear + 2.0 * kappa / pi;                       // a0
+            double st, ct, sp, cp;
+            sincos(theta, &st, &ct);
+            sincos(phi, &sp, &cp);
+            c[11] = -st * cp; c[12] = -st * sp; c[13] = -ct;                   // k (propagation direction)
+            c[14] = ct * cp;  c[15] = ct * sp;  c[16] = -st;                   // u
+            c[17] = sp;       c[18] = -cp;      c[19] = 0.0;                   // v
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < kNCoef; ++j) coef[(int64_t)j * P_pad + p] = c[j];
+    valid[p] = ok;
+}
+
+cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
+                            double *coef, int32_t *valid, cudaStream_t st)
+{
+    const int nt = 128;
+    prologue_kernel<<<(unsigned)((P_pad + nt - 1) / nt), nt, 0, st>>>(params, P, P_pad, f_ref_e0, kappa, coef, valid);
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// a2-a5: the fused main kernel
+// =================================================================================================
+struct __align__(16) MainSmem {
+    double tile[kStages][kTileBins * kTabW];
+    uint64_t full[kStages];
+};
+
+size_t main_kernel_smem_bytes() { return sizeof(MainSmem); }
+
+// one orbit coordinate from the trig basis (1, c1, s1, c2, s2, c3, s3)
+__device__ __forceinline__ double orb7(const double *C, double c1, double s1, double c2, double s2, double c3, double s3)
+{
+    double r = fma(C[1], c1, C[0]);
+    r = fma(C[2], s1, r);
+    r = fma(C[3], c2, r);
+    r = fma(C[4], s2, r);
+    r = fma(C[5], c3, r);
+    return fma(C[6], s3, r);
+}
+__device__ __forceinline__ double orb5(const double *C, double c1, double s1, double c2, double s2)
+{
+    double r = fma(C[1], c1, C[0]);
+    r = fma(C[2], s1, r);
+    r = fma(C[3], c2, r);
+    return fma(C[4], s2, r);
+}
+
+// One arm 1 -> j of TDI-X at one bin.  mu = k.n, un = u.n, vn = v.n with n = (p_j - p_1)/L.
+//   g = exp(-i a) [ sinc(a) + z sinc(b) ] x,   a = x (1 + mu), b = x (1 - mu), z = exp(-2 i x)
+// (sum of the two one-way links of the arm, PAPER.md:196 Eq. 15, :206 Eq. 17 with N = 0; the common
+// factor -i and the Doppler phase of spacecraft 1 are applied outside).  rho = 1 / ((1+mu)(1-mu)).
+__device__ __forceinline__ void arm_response(double xq, double x, double c2x, double s2x, double Pm, double Qm,
+                                             double rho, double &gr, double &gi)
+{
+    double sa, ca;
+    sincos_qt(xq * Pm, sa, ca);
+    double sb = fma(s2x, ca, -c2x * sa);                 // sin(2x - a) = sin b
+    if (Qm < 9.765625e-4) {                              // b -> 0: the difference formula cancels; series
+        const double b = x * Qm, b2 = b * b;
+        sb = b * fma(b2, fma(b2, 1.0 / 120.0, -1.0 / 6.0), 1.0);
+    }
+    const double sca = sa * Qm * rho;                    // x sinc(a)
+    const double scb = sb * Pm * rho;                    // x sinc(b)
+    const double br = fma(c2x, scb, sca);
+    const double bi = -s2x * scb;
+    gr = fma(ca, br, sa * bi);
+    gi = fma(ca, bi, -sa * br);
+}
+
+// One (particle, bin): a2 phase + t_f, a3 orbit + TDI-X response.  `row` is the bin's table row, c[] the
+// particle's coefficients.  Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1
+// included) and T'_+ , T'_x with  T_P = K_f T'_P,  K_f = -i (1 - z^2)  folded into the table.
+__device__ __forceinline__ void bin_template(const double2 *__restrict__ row, const double (&c)[kNCoef],
+                                             const OrbitCoef &orb, double &psi_out, double &sps, double &cps,
+                                             double &tpr, double &tpi, double &tcr, double &tci)
+{
+    const double kx = c[11], ky = c[12], kz = c[13];
+    const double ux = c[14], uy = c[15], uz = c[16];
+    const double vx = c[17], vy = c[18], vz = c[19];
+    const double2 r0 = row[0], r1 = row[1], r2 = row[2], r3 = row[3], r4 = row[4];
+    const double2 d0 = row[5], d1 = row[6], d2 = row[7], d3 = row[8];
+    const double2 zz = row[9], wx = row[11];
+    const double f = r0.x;
+
+    // ---- a2: SPA phase (quarter turns) and orbital phase at t_f  (Eq. A3 :404, Eq. 20 :220)
+    double psi = fma(c[0], f, c[1]);
+    psi = fma(c[2], r0.y, psi);
+    psi = fma(c[3], r1.x, psi);
+    psi = fma(c[4], r1.y, psi);
+    psi = fma(c[5], r2.x, psi);
+    psi = fma(c[6], r2.y, psi);
+    psi = fma(c[7], r3.x, psi);
+    psi = fma(c[8], r3.y, psi);
+    psi = fma(c[9], r4.x, psi);
+    const double xq = r4.y;
+    double alq = fma(c[2], d0.x, c[10]);
+    alq = fma(c[3], d0.y, alq);
+    alq = fma(c[4], d1.x, alq);
+    alq = fma(c[5], d1.y, alq);
+    alq = fma(c[6], d2.x, alq);
+    alq = fma(c[7], d2.y, alq);
+    alq = fma(c[8], d3.x, alq);
+    alq = fma(c[9], d3.y, alq);
+
+    // ---- a3: orbit to O(e^2) at t_f (reading A9), arm geometry
+    double s1, c1;
+    sincos_qt(alq, s1, c1);
+    const double c2 = fma(c1, c1, -s1 * s1), s2 = 2.0 * s1 * c1;
+    const double c3 = fma(c1, c2, -s1 * s2), s3 = fma(s1, c2, c1 * s2);
+    const double p1x = orb7(orb.c[0][0], c1, s1, c2, s2, c3, s3);
+    const double p1y = orb7(orb.c[0][1], c1, s1, c2, s2, c3, s3);
+    const double p1z = orb5(orb.c[0][2], c1, s1, c2, s2);
+    const double n2x = orb7(orb.c[1][0], c1, s1, c2, s2, c3, s3);
+    const double n2y = orb7(orb.c[1][1], c1, s1, c2, s2, c3, s3);
+    const double n2z = orb5(orb.c[1][2], c1, s1, c2, s2);
+    const double n3x = orb7(orb.c[2][0], c1, s1, c2, s2, c3, s3);
+    const double n3y = orb7(orb.c[2][1], c1, s1, c2, s2, c3, s3);
+    const double n3z = orb5(orb.c[2][2], c1, s1, c2, s2);
+    const double kp = fma(kx, p1x, fma(ky, p1y, kz * p1z));        // 4 k.p_1/c
+    const double mu2 = fma(kx, n2x, fma(ky, n2y, kz * n2z));
+    const double mu3 = fma(kx, n3x, fma(ky, n3y, kz * n3z));
+    const double un2 = fma(ux, n2x, fma(uy, n2y, uz * n2z));
+    const double un3 = fma(ux, n3x, fma(uy, n3y, uz * n3z));
+    const double vn2 = fma(vx, n2x, fma(vy, n2y, vz * n2z));
+    const double vn3 = fma(vx, n3x, fma(vy, n3y, vz * n3z));
+
+    // carrier: Psi_0 + Doppler phase of spacecraft 1 (reading A4), exp(+i Psi)
+    psi = fma(f, kp, psi);
+    sincos_qt(psi, sps, cps);
+
+    // two arms
+    const double P2 = fmax(1.0 + mu2, 1e-30), Q2 = fmax(1.0 - mu2, 1e-30);
+    const double P3 = fmax(1.0 + mu3, 1e-30), Q3 = fmax(1.0 - mu3, 1e-30);
+    const double den2 = P2 * Q2, den3 = P3 * Q3;
+    const double R = rcp_fast(den2 * den3);
+    double g2r, g2i, g3r, g3i;
+    arm_response(xq, wx.y, zz.x, zz.y, P2, Q2, den3 * R, g2r, g2i);
+    arm_response(xq, wx.y, zz.x, zz.y, P3, Q3, den2 * R, g3r, g3i);
+    const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;   // n.e_+.n, n.e_x.n
+    const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
+    // T'_P = xi_P3 g_3 - xi_P2 g_2   (TDI-X: arm 3 minus arm 2, reading A7)
+    tpr = fma(xp3, g3r, -xp2 * g2r);
+    tpi = fma(xp3, g3i, -xp2 * g2i);
+    tcr = fma(xc3, g3r, -xc2 * g2r);
+    tci = fma(xc3, g3i, -xc2 * g2i);
+    psi_out = psi;
+}
+
+__global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_constant__ MainArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    MainSmem &sm = *reinterpret_cast<MainSmem *>(smem_raw);
+
+    const int tid = threadIdx.x;
+    const int grp = blockIdx.x % a.n_groups;
+    const int seg = blockIdx.x / a.n_groups;
+    const int64_t p = (int64_t)grp * kThreads + tid;           // < P_pad by construction
+
+    const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
+    const int n_bins = hi - lo;
+    const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
+    const double *src = a.table + (int64_t)lo * kTabW;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(&sm.full[s], 1);
+        mbar_fence_init();
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) {
+            if (s < n_tiles) {
+                const int nb = min(kTileBins, n_bins - s * kTileBins);
+                const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
+                mbar_expect_tx(&sm.full[s], bytes);
+                tma_load_1d(sm.tile[s], src + (int64_t)s * kTileBins * kTabW, bytes, &sm.full[s]);
+            }
+        }
+    }
+
+    // per-particle coefficients (a1), coalesced
+    double c[kNCoef];
+#pragma unroll
+    for (int j = 0; j < kNCoef; ++j) c[j] = a.coef[(int64_t)j * a.P_pad + p];
+    __syncthreads();
+
+    double acc[kNAcc];
+#pragma unroll
+    for (int j = 0; j < kNAcc; ++j) acc[j] = 0.0;
+
+    for (int t = 0; t < n_tiles; ++t) {
+        const int slot = t % kStages;
+        mbar_wait(&sm.full[slot], (uint32_t)((t / kStages) & 1));
+        const int nb = min(kTileBins, n_bins - t * kTileBins);
+        const double *tile = sm.tile[slot];
+        double in[kNAcc];
+#pragma unroll
+        for (int j = 0; j < kNAcc; ++j) in[j] = 0.0;
+
+#pragma unroll 1
+        for (int b = 0; b < nb; ++b) {
+            const double2 *row = reinterpret_cast<const double2 *>(tile + b * kTabW);
+            const double2 dwv = row[10];
+            double psi, sps, cps, tpr, tpi, tcr, tci;
+            bin_template(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
+
+            // ---- a4: inner products (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117)
+            const double qr = fma(dwv.x, cps, -dwv.y * sps);               // dw' exp(+i Psi)
+            const double qi = fma(dwv.x, sps, dwv.y * cps);
+            in[0] = fma(qr, tpr, fma(qi, tpi, in[0]));                      // z_+ += q conj(T'_+)
+            in[1] = fma(qi, tpr, fma(-qr, tpi, in[1]));
+            in[2] = fma(qr, tcr, fma(qi, tci, in[2]));                      // z_x
+            in[3] = fma(qi, tcr, fma(-qr, tci, in[3]));
+            const double w = row[11].x;
+            in[4] = fma(w, fma(tpr, tpr, tpi * tpi), in[4]);                // m_pp
+            in[5] = fma(w, fma(tcr, tcr, tci * tci), in[5]);                // m_cc
+            in[6] = fma(w, fma(tpr, tcr, tpi * tci), in[6]);                // m_pc = sum w T'_+ conj(T'_x)
+            in[7] = fma(w, fma(tpi, tcr, -tpr * tci), in[7]);
+        }
+#pragma unroll
+        for (int j = 0; j < kNAcc; ++j) acc[j] += in[j];
+
+        __syncthreads();                                 // every thread is done with this slot
+        if (tid == 0 && t + kStages < n_tiles) {
+            const int tn = t + kStages;
+            const int nbn = min(kTileBins, n_bins - tn * kTileBins);
+            const uint32_t bytes = (uint32_t)nbn * kTabW * sizeof(double);
+            mbar_expect_tx(&sm.full[slot], bytes);
+            tma_load_1d(sm.tile[slot], src + (int64_t)tn * kTileBins * kTabW, bytes, &sm.full[slot]);
+        }
+    }
+
+    double *out = a.partial + ((int64_t)seg * kNAcc) * a.P_pad + p;
+#pragma unroll
+    for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
+}
+
+cudaError_t main_kernel_configure()
+{
+    return cudaFuncSetAttribute(fstat_main_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)sizeof(MainSmem));
+}
+
+cudaError_t launch_main(const MainArgs &a, cudaStream_t st)
+{
+    const int64_t n_cta = (int64_t)a.n_groups * a.n_seg;
+    fstat_main_kernel<<<(unsigned)n_cta, kThreads, sizeof(MainSmem), st>>>(a);
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// Template dump (not on the hot path): u_P(f_k) = f^(-7/6) K_f T'_P exp(-i psi) for ONE particle over the
+// whole grid, one thread per bin, through the same bin_template() the main kernel uses.  Serves
+// fstat_eval_template (injection synthesis, element-wise parity tests of a2/a3).
+// =================================================================================================
+__global__ void __launch_bounds__(128) template_kernel(const double *__restrict__ table,
+                                                       const double *__restrict__ coef, int64_t P_pad,
+                                                       int64_t n_bins, const __grid_constant__ OrbitCoef orb,
+                                                       double2 *__restrict__ u_plus, double2 *__restrict__ u_cross)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_bins) return;
+    double c[kNCoef];
+#pragma unroll
+    for (int j = 0; j < kNCoef; ++j) c[j] = coef[(int64_t)j * P_pad];
+    const double2 *row = reinterpret_cast<const double2 *>(table + i * kTabW);
+    double psi, sps, cps, tpr, tpi, tcr, tci;
+    bin_template(row, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
+    const double f = row[0].x;
+    const double amp = pow(f, -7.0 / 6.0);
+    const double c2x = row[9].x, s2x = row[9].y;
+    // K_f = 2 sin(2x) exp(-2 i x);  carrier exp(-i psi) = cps - i sps
+    const double kr = 2.0 * s2x * c2x * amp, ki = -2.0 * s2x * s2x * amp;
+    const double er = kr * cps + ki * sps, ei = ki * cps - kr * sps;      // amp K_f exp(-i psi)
+    u_plus[i] = make_double2(er * tpr - ei * tpi, er * tpi + ei * tpr);
+    u_cross[i] = make_double2(er * tcr - ei * tci, er * tci + ei * tcr);
+}
+
+cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
+                            const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st)
+{
+    const int nt = 128;
+    template_kernel<<<(unsigned)((n_bins + nt - 1) / nt), nt, 0, st>>>(
+        table, coef, P_pad, n_bins, orb, reinterpret_cast<double2 *>(u_plus), reinterpret_cast<double2 *>(u_cross));
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// a6: epilogue.  2 F_k = z^H G^-1 z, G = [[m_pp, conj(m_pc)], [m_pc, m_cc]]  (the 4x4 real system of
+// PAPER.md:85 Eq. 7 is the real embedding of this 2x2 Hermitian one).  Evaluated
+// by Gram-Schmidt: 2 F_k = |z_+|^2/m_pp + |z_x - (m_pc/m_pp) z_+|^2 / (m_cc - |m_pc|^2/m_pp).
+// Rank-deficient G (reading A15): only the non-degenerate direction(s) contribute.
+// Block = 32 particles (x) by 8 partition lanes (y); partition index k = y, y + 8, ...
+// =================================================================================================
+constexpr int kEpiX = 32, kEpiY = 8;
+
+__global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__restrict__ partial,
+                                                               const int32_t *__restrict__ part_seg,
+                                                               const int32_t *__restrict__ valid, int64_t P,
+                                                               int64_t P_pad, int32_t n_part,
+                                                               double *__restrict__ F, double *__restrict__ Fk)
+{
+    __shared__ double sF[kEpiY][kEpiX];
+    __shared__ double sT[kEpiY][kEpiX + 1];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int64_t p0 = (int64_t)blockIdx.x * kEpiX;
+    const int64_t p = p0 + tx;
+    const bool live = p < P;
+    const bool ok = live && valid[p] != 0;
+    const double ninf = -INFINITY;
+    double fsum = 0.0;
+    for (int k0 = 0; k0 < n_part; k0 += kEpiY) {
+        const int k = k0 + ty;
+        double fk = 0.0;
+        if (k < n_part && live) {
+            const int s0 = part_seg[k], s1 = part_seg[k + 1];
+            double v[kNAcc];
+#pragma unroll
+            for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
+            for (int s = s0; s < s1; ++s) {
+                const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
+#pragma unroll
+                for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
+            }
+            const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
+            const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
+            double twoF = 0.0;
+            if (mpp > 0.0) {
+                const double inv = 1.0 / mpp;
+                twoF = (zpr * zpr + zpi * zpi) * inv;
+                const double cr = mr * inv, ci = mi * inv;                      // m_pc / m_pp
+                const double schur = mcc - (mr * mr + mi * mi) * inv;
+                if (schur > 1e-13 * mcc) {
+                    const double yr = zcr - (cr * zpr - ci * zpi);
+                    const double yi = zci - (cr * zpi + ci * zpr);
+                    twoF += (yr * yr + yi * yi) / schur;
+                }
+            } else if (mcc > 0.0) {
+                twoF = (zcr * zcr + zci * zci) / mcc;
+            }
+            fk = ok ? 0.5 * twoF : ninf;
+            if (ok) fsum += fk;
+        }
+        if (Fk != nullptr) {                              // transpose through shared memory: coalesced rows
+            sT[ty][tx] = fk;
+            __syncthreads();
+            // 256 threads write a 32 (particles) x 8 (partitions) tile: thread -> (particle = id / 8, k = id % 8)
+            const int id = ty * kEpiX + tx;
+            const int pp = id / kEpiY, kk = id % kEpiY;
+            if (p0 + pp < P && k0 + kk < n_part) Fk[(p0 + pp) * (int64_t)n_part + k0 + kk] = sT[kk][pp];
+            __syncthreads();
+        }
+    }
+    sF[ty][tx] = fsum;
+    __syncthreads();
+    if (ty == 0 && live) {
+        double s = 0.0;
+#pragma unroll
+        for (int y = 0; y < kEpiY; ++y) s += sF[y][tx];
+        F[p] = ok ? s : ninf;
+    }
+}
+
+cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
+                            int64_t P_pad, int32_t n_part, double *F, double *Fk, cudaStream_t st)
+{
+    const dim3 blk(kEpiX, kEpiY);
+    const unsigned nb = (unsigned)((P + kEpiX - 1) / kEpiX);
+    epilogue_kernel<<<nb, blk, 0, st>>>(partial, part_seg, valid, P, P_pad, n_part, F, Fk);
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// pipe-peak probes: dependent-free instruction streams (8 chains per thread), for the roofline
+// denominators.  Thread-level instructions per launch: blocks*256*iters*64.
+// =================================================================================================
+template <int WHICH>
+__global__ void __launch_bounds__(256) probe_kernel(int iters, double *sink)
+{
+    if (WHICH == 0) {
+        double x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = 1.0 + 1e-9 * (threadIdx.x + j);
+        const double m = 0.999999999, b = 1e-12;
+        for (int i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = fma(x[j], m, b);
+        }
+        double s = 0.0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += x[j];
+        if (s == 123.456) sink[0] = s;
+    } else if (WHICH == 1) {
+        float x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = 1.0f + 1e-6f * (threadIdx.x + j);
+        const float m = 0.9999999f, b = 1e-9f;
+        for (int i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = fmaf(x[j], m, b);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += x[j];
+        if (s == 123.456f) sink[0] = s;
+    } else {
+        float x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = 0.1f + 1e-3f * (threadIdx.x + j);
+        for (int i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) asm volatile("sin.approx.ftz.f32 %0, %0;" : "+f"(x[j]));
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += x[j];
+        if (s == 123.456f) sink[0] = s;
+    }
+}
+
+cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaStream_t st)
+{
+    if (which == 0) probe_kernel<0><<<n_blocks, 256, 0, st>>>(iters, sink);
+    else if (which == 1) probe_kernel<1><<<n_blocks, 256, 0, st>>>(iters, sink);
+    else probe_kernel<2><<<n_blocks, 256, 0, st>>>(iters, sink);
+    return cudaGetLastError();
+}
+
+}  // namespace fstat

@@ -1,0 +1,288 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Bar (BASELINE.json north_star): relative error <= 1e-5 on every F and F_k.
+
+All tests here need a B200 (``-m gpu``).  The oracle is called only from this test code."""
+import math
+
+import numpy as np
+import pytest
+
+import synthetic as syn
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-5          # north_star's tolerance, strict relative, on every F and every F_k
+
+
+@pytest.fixture(scope="module")
+def fs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2407_10797_b200 import build
+    build.build()
+    import paper_2407_10797_b200 as fs
+    fs.load_library()
+    return fs
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+@pytest.fixture(scope="module")
+def first_stage(orc):
+    """Config 1 data (1 577 880 bins, seeded noise + SNR-12 injection from the oracle's template)."""
+    return syn.make_dataset(syn.CONFIGS[1], orc.template)
+
+
+def _rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return np.abs(a - b) / np.abs(b)
+
+
+def _gpu_eval(fs, torch, ds, edges, params, opts=None, want_Fk=True):
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, opts) as plan:
+        p = torch.as_tensor(np.ascontiguousarray(params), device="cuda")
+        F, Fk = fs.fstat_eval_batch(plan, p, want_Fk=want_Fk)
+        torch.cuda.synchronize()
+        return F.cpu().numpy(), (Fk.cpu().numpy() if Fk is not None else None)
+
+
+# ------------------------------------------------------------------------------------------ config 0
+def test_tiny_all_particles_every_F_and_Fk(fs, torch_, orc, tiny):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)
+    edges = ds.edges(4)
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par)
+    F_g, Fk_g = _gpu_eval(fs, torch_, ds, edges, par)
+    assert F_g.shape == (64,) and Fk_g.shape == (64, 4)
+    assert _rel(Fk_g, Fk_o).max() <= RTOL
+    assert _rel(F_g, F_o).max() <= RTOL
+    # far inside the bar with the present all-FP64 kernel; guards against silent precision loss
+    assert _rel(Fk_g, Fk_o).max() <= 1e-8
+
+
+def test_tiny_at_the_injection_recovers_the_snr(fs, torch_, orc):
+    """Zero noise, evaluated at the injected parameters: 2F = rho^2 = 144 (Eq. 7)."""
+    ds = syn.make_dataset(syn.CONFIGS[0], orc.template, noise=False)
+    F_g, Fk_g = _gpu_eval(fs, torch_, ds, ds.edges(4), ds.inj_params[None, :])
+    assert 2.0 * F_g[0] == pytest.approx(144.0, rel=1e-9)
+    assert Fk_g.sum() == pytest.approx(F_g[0], rel=1e-13)
+
+
+def test_template_matches_oracle_bin_by_bin(fs, torch_, orc, tiny):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
+        for p in (0, 17, 63):
+            up_o, uc_o = orc.template(par[p], ds.freq)
+            up_g, uc_g = fs.fstat_eval_template(plan, par[p])
+            scale = max(np.abs(up_o).max(), np.abs(uc_o).max())
+            assert np.abs(up_g.cpu().numpy() - up_o).max() <= 1e-7 * scale
+            assert np.abs(uc_g.cpu().numpy() - uc_o).max() <= 1e-7 * scale
+        with pytest.raises(fs.FstatError):
+            fs.fstat_eval_template(plan, [1e8, -3.0, 0.2, 1.0, 1.0, 0.0])
+
+
+# ------------------------------------------------------------------------------- edge cases, config 0
+@pytest.mark.parametrize("P", [1, 2, 127, 128, 129, 300])
+def test_ragged_particle_counts(fs, torch_, orc, tiny, P):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg, P)
+    edges = ds.edges(4)
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par)
+    F_g, Fk_g = _gpu_eval(fs, torch_, ds, edges, par)
+    assert _rel(Fk_g, Fk_o).max() <= RTOL and _rel(F_g, F_o).max() <= RTOL
+
+
+def test_ragged_partition_edges_and_short_segments(fs, torch_, orc, tiny):
+    """Arbitrary (non-equal, non-tile-aligned) edges, partitions shorter than one tile, partitions cut
+    into several CTA segments (max_segment_bins), and the same through fstat_plan_set_partitions."""
+    ds = tiny
+    n = ds.n_bins
+    par = syn.draw_particles(ds.cfg, 40)
+    edge_sets = [
+        np.array([0, 1, 3, 66, 67, 130, 777, 1024, 2095, n]),
+        np.array([0, n]),
+        np.array([0, 63, 64, 65, 128, n - 2, n]),
+        np.arange(0, n + 1, 8)[: (n // 8) + 1].tolist() + ([n] if n % 8 else []),
+    ]
+    for seg in (0, 64, 100):
+        opts = fs.fstat_default_options(max_segment_bins=seg)
+        with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), opts) as plan:
+            p = torch_.as_tensor(par, device="cuda")
+            for edges in edge_sets:
+                edges = np.asarray(edges, dtype=np.int64)
+                fs.fstat_plan_set_partitions(plan, edges)
+                assert fs.fstat_plan_n_part(plan) == len(edges) - 1
+                F_g, Fk_g = fs.fstat_eval_batch(plan, p)
+                F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par)
+                assert _rel(Fk_g.cpu().numpy(), Fk_o).max() <= RTOL, (seg, len(edges))
+                assert _rel(F_g.cpu().numpy(), F_o).max() <= RTOL, (seg, len(edges))
+
+
+def test_one_bin_partitions_take_the_singular_branch(fs, torch_, orc, tiny):
+    """A one-bin partition makes M singular (reading A15): F_k = 4 df |d|^2 / (2 S_n) for any template."""
+    ds = tiny
+    n = 12
+    par = syn.draw_particles(ds.cfg, 5)
+    edges = np.arange(n + 1, dtype=np.int64)
+
+    class Sub:
+        freq, dw, inv_sn = ds.freq[:n], ds.dw[:n], ds.inv_sn[:n]
+    F_g, Fk_g = _gpu_eval(fs, torch_, Sub, edges, par)
+    F_o, Fk_o = orc.fstat_batch(Sub.freq, Sub.dw, Sub.inv_sn, edges, par)
+    expect = 0.5 * 4.0 * ds.df * np.abs(ds.data[:n]) ** 2 / ds.sn[:n]
+    np.testing.assert_allclose(Fk_g, np.broadcast_to(expect, Fk_g.shape), rtol=1e-9)
+    assert _rel(Fk_g, Fk_o).max() <= RTOL and _rel(F_g, F_o).max() <= RTOL
+
+
+def test_invalid_particles_get_minus_infinity(fs, torch_, orc, tiny):
+    """Let-them-fly: non-physical parameter vectors are not errors; F = F_k = -inf."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg, 10)
+    par[1, 1] = -5.0            # Mc <= 0
+    par[3, 2] = 0.26            # eta > 1/4
+    par[4, 2] = 0.0             # eta <= 0
+    par[6, 5] = -1e-3           # e0 < 0
+    par[8, 0] = np.nan
+    par[9, 4] = np.inf
+    bad = [1, 3, 4, 6, 8, 9]
+    good = [0, 2, 5, 7]
+    F_g, Fk_g = _gpu_eval(fs, torch_, ds, ds.edges(4), par)
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, ds.edges(4), par)
+    assert np.all(np.isneginf(F_g[bad])) and np.all(np.isneginf(Fk_g[bad]))
+    assert np.all(np.isneginf(F_o[bad]))
+    assert _rel(Fk_g[good], Fk_o[good]).max() <= RTOL and _rel(F_g[good], F_o[good]).max() <= RTOL
+
+
+def test_empty_batch_and_null_Fk(fs, torch_, orc, tiny):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg, 9)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(4)) as plan:
+        F, Fk = fs.fstat_eval_batch(plan, torch_.empty((0, 6), dtype=torch_.float64, device="cuda"))
+        assert F.numel() == 0
+        F1, none = fs.fstat_eval_batch(plan, torch_.as_tensor(par, device="cuda"), want_Fk=False)
+        assert none is None
+        F2, Fk2 = fs.fstat_eval_batch(plan, torch_.as_tensor(par, device="cuda"))
+        torch_.cuda.synchronize()
+        assert torch_.equal(F1, F2)
+        ms = fs.fstat_plan_main_kernel_ms(plan, 8)
+        assert len(ms) == 2 and np.all(ms > 0.0)
+
+
+def test_host_buffer_call_and_device_resident_inputs_agree(fs, torch_, orc, tiny):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)
+    edges = ds.edges(4)
+    F_d, Fk_d = _gpu_eval(fs, torch_, ds, edges, par)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges) as plan:
+        F_h, Fk_h = fs.fstat_eval_batch_host(plan, par)                      # pageable numpy
+        pin = torch_.as_tensor(par).pin_memory()
+        F_p, Fk_p = fs.fstat_eval_batch_host(plan, pin)                      # pinned tensors
+    np.testing.assert_array_equal(F_h, F_d)
+    np.testing.assert_array_equal(Fk_h, Fk_d)
+    np.testing.assert_array_equal(F_p.numpy(), F_d)
+    np.testing.assert_array_equal(Fk_p.numpy(), Fk_d)
+    # plan built from device-resident inputs
+    f_t = torch_.as_tensor(ds.freq, device="cuda")
+    dw_t = torch_.as_tensor(ds.dw, device="cuda")
+    w_t = torch_.as_tensor(ds.inv_sn, device="cuda")
+    with fs.fstat_plan_create(f_t, dw_t, w_t, edges) as plan:
+        F2, Fk2 = fs.fstat_eval_batch(plan, torch_.as_tensor(par, device="cuda"))
+        np.testing.assert_array_equal(F2.cpu().numpy(), F_d)
+        np.testing.assert_array_equal(Fk2.cpu().numpy(), Fk_d)
+
+
+def test_plan_create_rejects_bad_data_on_the_device(fs, torch_, tiny):
+    ds = tiny
+    e = ds.edges(4)
+    bad_f = ds.freq.copy(); bad_f[100] += 0.3 * ds.df
+    bad_w = ds.inv_sn.copy(); bad_w[5] = 0.0
+    bad_d = ds.dw.copy(); bad_d[7] = np.nan
+    for args in ((bad_f, ds.dw, ds.inv_sn), (ds.freq, ds.dw, bad_w), (ds.freq, bad_d, ds.inv_sn),
+                 (ds.freq[::-1].copy(), ds.dw, ds.inv_sn)):
+        with pytest.raises(fs.FstatError) as ei:
+            fs.fstat_plan_create(*args, e)
+        assert ei.value.status == 1
+
+
+def test_a_non_blocking_stream_is_honoured(fs, torch_, orc, tiny):
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)
+    F_ref, _ = _gpu_eval(fs, torch_, ds, ds.edges(4), par)
+    st = torch_.cuda.Stream()
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(4)) as plan:
+        p = torch_.as_tensor(par, device="cuda")
+        torch_.cuda.synchronize()
+        with torch_.cuda.stream(st):
+            F, Fk = fs.fstat_eval_batch(plan, p)
+        st.synchronize()
+        np.testing.assert_array_equal(F.cpu().numpy(), F_ref)
+
+
+# ----------------------------------------------- full-size configs, in bench.py's launch configuration
+def _check_sampled(fs, torch, orc, ds, n_part, params, sample, rtol=RTOL):
+    """GPU evaluates the whole batch (the launch configuration bench.py times); the oracle re-computes the
+    sampled particles one by one; every F and F_k of those particles must agree."""
+    edges = ds.edges(n_part)
+    F_g, Fk_g = _gpu_eval(fs, torch, ds, edges, params)
+    assert np.all(np.isfinite(F_g)) and np.all(np.isfinite(Fk_g))
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, params[sample])
+    rk, rf = _rel(Fk_g[sample], Fk_o), _rel(F_g[sample], F_o)
+    assert rk.max() <= rtol, "worst F_k rel err %.3g" % rk.max()
+    assert rf.max() <= rtol, "worst F rel err %.3g" % rf.max()
+    np.testing.assert_allclose(Fk_g.sum(axis=1), F_g, rtol=1e-12)
+    return F_g, Fk_g
+
+
+def test_config1_first_stage_np1024_sampled_particles(fs, torch_, orc, first_stage):
+    ds = first_stage
+    par = syn.draw_particles(ds.cfg)                       # P = 2048
+    sample = np.random.default_rng(11).choice(par.shape[0], 6, replace=False)
+    _check_sampled(fs, torch_, orc, ds, 1024, par, sample)
+
+
+def test_config2_middle_stages_sampled_particles(fs, torch_, orc, first_stage):
+    ds = first_stage
+    cfg = syn.CONFIGS[2]
+    par = syn.draw_particles(cfg)                          # P = 8192 = 8 swarms x 1024
+    sample = np.random.default_rng(12).choice(par.shape[0], 4, replace=False)
+    for n_part in cfg.n_part:
+        _check_sampled(fs, torch_, orc, ds, n_part, par, sample)
+
+
+def test_config3_final_coherent_sampled_particles(fs, torch_, orc, first_stage):
+    ds = first_stage
+    cfg = syn.CONFIGS[3]
+    par = syn.draw_particles(cfg)                          # P = 4096, N_p = 1
+    sample = np.random.default_rng(13).choice(par.shape[0], 4, replace=False)
+    F_g, _ = _check_sampled(fs, torch_, orc, ds, 1, par, sample)
+    # the box surrounds the injection: the statistic is large there (2F ~ rho^2 = 144 at the peak)
+    inj = ds.inj_params[None, :]
+    F_i, _ = _gpu_eval(fs, torch_, ds, ds.edges(1), inj)
+    assert 2.0 * F_i[0] > 100.0
+
+
+def test_config4_wide_band_sampled_particles(fs, torch_, orc):
+    cfg = syn.CONFIGS[4]
+    ds = syn.make_dataset(cfg, orc.template)               # 7 100 460 bins, crosses the TDI null (H4)
+    par = syn.draw_particles(cfg, 256)
+    sample = np.random.default_rng(14).choice(256, 3, replace=False)
+    for n_part in cfg.n_part:
+        _check_sampled(fs, torch_, orc, ds, n_part, par, sample)
+
+
+def test_noise_only_statistic_has_chi2_mean(fs, torch_, first_stage):
+    """Property at full size (no oracle needed): over pure noise 2 F_k ~ chi^2(4) for every partition,
+    so the mean of 2F over N_p = 1024 partitions and many templates is 4 (reading A17)."""
+    cfg = syn.CONFIGS[1]
+    ds = syn.make_dataset(cfg, None)
+    par = syn.draw_particles(cfg, 256)
+    F_g, Fk_g = _gpu_eval(fs, torch_, ds, ds.edges(1024), par)
+    m = 2.0 * Fk_g.mean()
+    # 256 templates share one noise realisation: effective sample >= 1024 independent partitions
+    assert abs(m - 4.0) < 5.0 * math.sqrt(8.0 / 1024.0)
