@@ -61,8 +61,9 @@ def test_tiny_all_particles_every_F_and_Fk(fs, torch_, orc, tiny):
     assert F_g.shape == (64,) and Fk_g.shape == (64, 4)
     assert _rel(Fk_g, Fk_o).max() <= RTOL
     assert _rel(F_g, F_o).max() <= RTOL
-    # far inside the bar with the present all-FP64 kernel; guards against silent precision loss
-    assert _rel(Fk_g, Fk_o).max() <= 1e-8
+    # The FP64 carrier phase (up to 1.5e8 rad, ulp 3e-8 rad) is rounded differently by the two sides (hazard
+    # H1): ~1e-7 is the floor on chance-small F_k; anything above 1e-6 would be a real precision loss here.
+    assert _rel(Fk_g, Fk_o).max() <= 1e-6
 
 
 def test_tiny_at_the_injection_recovers_the_snr(fs, torch_, orc):
