@@ -57,7 +57,12 @@ typedef struct {
     int32_t inputs_on_device; /* 0 (default): freq/dw/inv_sn are host pointers; 1: device pointers      */
     int32_t max_segment_bins; /* 0 (default) = automatic.  Upper bound on the number of bins one CTA    *
                                * sums before handing its partial sums to the epilogue (tuning / tests)  */
-    int32_t reserved;
+    int32_t force_level;      /* -2 (default): the stride of the interpolating kernel is chosen per (particle      *
+                               * group, segment) from an a-priori error bound; -1: direct kernel everywhere       *
+                               * (every bin evaluated in full, no interpolation); 0..5: stride 8 << level          *
+                               * wherever the segment allows it, regardless of the bound (tests / tuning)          */
+    double interp_tol;        /* scale of the interpolation error tolerances; 1.0 (default) = carrier phase        *
+                               * 1e-7 rad and TDI response 1e-7 relative            */
 } fstat_options;
 
 FSTAT_API void fstat_default_options(fstat_options *opts);
@@ -152,9 +157,16 @@ FSTAT_API int32_t fstat_plan_n_part(const fstat_plan *plan);
 FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
 /* Number of (particle-group, segment) work items = CTAs the main kernel launches for P particles. */
 FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
-/* Number of kernels one fstat_eval_batch call launches (prologue + main + epilogue). */
+/* Number of kernels one fstat_eval_batch call launches (prologue, stride selection, interpolating main
+ * kernel, direct main kernel, epilogue). */
 FSTAT_API int32_t fstat_launches_per_eval(void);
-/* Device time of the main (fused template + inner product) kernel in the most recent evaluations on
+/* How the most recent fstat_eval_batch on this plan was split between the direct kernel and the six
+ * strides of the interpolating kernel: bins_out[0] / [1..6] = sum over the (particle group, segment) work
+ * items run by the direct kernel / at stride 8, 16, 32, 64, 128, 256 of the segment's bin count (multiply
+ * by 128 particles per group for template-bins); subblocks_out[1..6] = number of node intervals those
+ * items walked (one full-model node evaluation each).  HOST arrays of 7.  Synchronises the device. */
+FSTAT_API fstat_status fstat_plan_level_bins(fstat_plan *plan, int64_t *bins_out, int64_t *subblocks_out);
+/* Device time of the main (fused template + inner product) kernels in the most recent evaluations on
  * this plan: CUDA events are recorded on the call's stream around that kernel at every fstat_eval_batch
  * (ring of 128).  Writes the milliseconds of the last min(n_last, 128, evaluations so far) calls, oldest
  * first, to the HOST array ms_out and returns how many were written.  Synchronises on those events. */

@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
     "fstat_eval_batch_host", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_launches_per_eval",
-    "fstat_plan_main_kernel_ms", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
+    "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
 )
 
@@ -35,7 +35,7 @@ class Options(C.Structure):
     """fstat_options of include/fstat.h."""
     _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double), ("orbit_kappa", C.c_double),
                 ("orbit_lambda", C.c_double), ("device", C.c_int32), ("inputs_on_device", C.c_int32),
-                ("max_segment_bins", C.c_int32), ("reserved", C.c_int32)]
+                ("max_segment_bins", C.c_int32), ("force_level", C.c_int32), ("interp_tol", C.c_double)]
 
 
 def library_path() -> str:
@@ -77,6 +77,8 @@ def load_library():
         L.fstat_plan_n_ctas.restype = i64
         L.fstat_launches_per_eval.argtypes = []
         L.fstat_launches_per_eval.restype = i32
+        L.fstat_plan_level_bins.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+        L.fstat_plan_level_bins.restype = C.c_int
         L.fstat_plan_main_kernel_ms.argtypes = [vp, i32, dp]
         L.fstat_plan_main_kernel_ms.restype = i32
         L.fstat_edges_equal_bins.argtypes = [i64, i32, C.POINTER(i64)]
@@ -290,6 +292,14 @@ def fstat_plan_n_ctas(plan: Plan, P: int) -> int:
 
 def fstat_launches_per_eval() -> int:
     return int(load_library().fstat_launches_per_eval())
+
+
+def fstat_plan_level_bins(plan: Plan) -> Tuple[np.ndarray, np.ndarray]:
+    """(bins[7], subblocks[7]) of the most recent evaluation: index 0 = direct kernel, 1..6 = stride 8..256."""
+    b, s = np.zeros(7, dtype=np.int64), np.zeros(7, dtype=np.int64)
+    _check(load_library().fstat_plan_level_bins(plan.handle, b.ctypes.data_as(C.POINTER(C.c_int64)),
+                                                s.ctypes.data_as(C.POINTER(C.c_int64))), "fstat_plan_level_bins", plan)
+    return b, s
 
 
 def fstat_plan_main_kernel_ms(plan: Plan, n_last: int = 1) -> np.ndarray:

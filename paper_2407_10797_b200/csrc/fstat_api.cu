@@ -23,13 +23,29 @@ struct fstat_plan {
     fstat_options opt{};
     int32_t n_part = 0;
     std::vector<int64_t> edges;        // host copy [n_part+1]
-    double *d_table = nullptr;         // [n_bins][kTabW]
+    double f0 = 0.0;                   // freq[0]
+    double *d_table = nullptr;         // [n_bins][kTabW]   (direct kernel, template dump, Gram build)
+    double *d_dwp = nullptr;           // [n_bins][2]       folded data (interpolating kernel)
+    double *d_node = nullptr;          // [n_node_rows][kTabW]
+    int64_t n_node_rows = 0;
+    bool fast_ok = false;              // the node grid (256 bins beyond both ends) stays at f > 0
+    // partition-dependent tables of the interpolating kernel
+    int32_t *d_edges32 = nullptr; size_t edges32_cap = 0;
+    int32_t *d_cnt = nullptr; size_t cnt_cap = 0;          // scratch [n_part]
+    double *d_gram[kNLevels] = {}; size_t gram_cap[kNLevels] = {};
+    std::vector<int32_t> cnt[kNLevels];                    // host copies (segment -> first sub-block)
     // segmentation (depends on the partitions and on the number of particle groups)
     int32_t seg_groups = -1;           // n_groups the current segmentation was made for
     int32_t n_seg = 0;
     int32_t *d_seg_edge = nullptr;     // [n_seg+1]
     int32_t *d_part_seg = nullptr;     // [n_part+1]
     size_t seg_cap = 0, part_cap = 0;
+    std::vector<int32_t> seg_edge_h;   // host copy of d_seg_edge
+    int32_t *d_seg_gbase = nullptr; size_t gbase_cap = 0;  // [n_seg][kNLevels]
+    SegCrit *d_seg_crit = nullptr; size_t crit_cap = 0;    // [n_seg]
+    int8_t *d_seg_maxlvl = nullptr; size_t maxlvl_cap = 0; // [n_seg]
+    int8_t *d_level = nullptr; size_t level_cap = 0;       // [n_groups][n_seg] of the most recent evaluation
+    int32_t last_groups = 0;
     // workspace
     double *d_coef = nullptr;  size_t coef_cap = 0;      // doubles
     int32_t *d_valid = nullptr; size_t valid_cap = 0;    // ints
@@ -94,60 +110,138 @@ bool edges_valid(int64_t n_bins, int32_t n_part, const int64_t *e, std::string *
     return true;
 }
 
-// Split every partition into near-equal segments of at most max_len bins.  A segment never crosses a
-// partition edge, so the main kernel needs no per-bin edge test and writes plain partial sums.
-void make_segments(const std::vector<int64_t> &edges, int64_t max_len, std::vector<int32_t> *seg_edge,
-                   std::vector<int32_t> *part_seg)
+// Cut every partition into CTA work items ("segments").  A segment never crosses a partition edge, so
+// the main kernels need no per-bin edge test and write plain partial sums.
+//   aligned: the cuts inside a partition are the multiples of max_len (itself a multiple of kMaxStride),
+//            so that node intervals of every stride and the 256-bin data tiles never straddle a segment
+//            boundary other than a partition edge -- the layout the interpolating kernel needs;
+//   else:    near-equal pieces of at most max_len bins (tuning / tests; direct kernel only).
+void make_segments(const std::vector<int64_t> &edges, int64_t max_len, bool aligned,
+                   std::vector<int32_t> *seg_edge, std::vector<int32_t> *part_seg)
 {
     const size_t n_part = edges.size() - 1;
     seg_edge->clear();
     part_seg->assign(n_part + 1, 0);
     seg_edge->push_back(0);
     for (size_t k = 0; k < n_part; ++k) {
-        const int64_t lo = edges[k], len = edges[k + 1] - edges[k];
-        const int64_t n = (len + max_len - 1) / max_len;
+        const int64_t lo = edges[k], hi = edges[k + 1], len = hi - lo;
         (*part_seg)[k] = (int32_t)(seg_edge->size() - 1);
-        for (int64_t s = 1; s <= n; ++s) seg_edge->push_back((int32_t)(lo + (len * s) / n));
+        if (aligned) {
+            for (int64_t c = (lo / max_len + 1) * max_len; c < hi; c += max_len) seg_edge->push_back((int32_t)c);
+            seg_edge->push_back((int32_t)hi);
+        } else {
+            const int64_t n = (len + max_len - 1) / max_len;
+            for (int64_t s = 1; s <= n; ++s) seg_edge->push_back((int32_t)(lo + (len * s) / n));
+        }
     }
     (*part_seg)[n_part] = (int32_t)(seg_edge->size() - 1);
+}
+
+bool segments_aligned(const fstat_plan *pl)
+{
+    return pl->opt.max_segment_bins <= 0 || pl->opt.max_segment_bins % kMaxStride == 0;
 }
 
 int64_t auto_segment_len(const fstat_plan *pl, int32_t n_groups)
 {
     if (pl->opt.max_segment_bins > 0) return pl->opt.max_segment_bins;
-    // aim at >= 24 CTAs per SM in flight order (8 waves at 3 CTAs/SM) so the tail wave is short
-    const int64_t target_ctas = (int64_t)pl->n_sm * 24;
+    // aim at >= 48 work items per SM so that the tail wave is short; multiples of kMaxStride
+    const int64_t target_ctas = (int64_t)pl->n_sm * 48;
     int64_t want_seg = (target_ctas + n_groups - 1) / n_groups;
     if (want_seg < 1) want_seg = 1;
     int64_t len = (pl->n_bins + want_seg - 1) / want_seg;
-    len = ((len + kTileBins - 1) / kTileBins) * kTileBins;
-    if (len < 4 * kTileBins) len = 4 * kTileBins;
-    if (len > 64 * kTileBins) len = 64 * kTileBins;
+    len = ((len + kMaxStride - 1) / kMaxStride) * kMaxStride;
+    if (len < 4 * kMaxStride) len = 4 * kMaxStride;
+    if (len > 64 * kMaxStride) len = 64 * kMaxStride;
     return len;
+}
+
+int64_t n_segments_for(const fstat_plan *pl, int32_t n_groups)
+{
+    std::vector<int32_t> seg_edge, part_seg;
+    make_segments(pl->edges, auto_segment_len(pl, n_groups), segments_aligned(pl), &seg_edge, &part_seg);
+    return (int64_t)seg_edge.size() - 1;
+}
+
+// Per-segment factors of the a-priori interpolation error bound (see schedule_kernel; DESIGN.md
+// "Stride selection").  Psi_q = Psi in quarter turns = ... + c3 f^(-5/3) + c9 f^(-34/9); t_f = Psi_q'/4.
+SegCrit make_seg_crit(double f_lo, double f_hi, double df, double part_len)
+{
+    const double Om = 2.0 * kPi / kYear;
+    SegCrit q;
+    q.p1 = 1.15 * Om * df * 0.25 * (40.0 / 9.0) * pow(f_lo, -11.0 / 3.0);
+    q.p2 = 1.15 * Om * df * 0.25 * (1462.0 / 81.0) * pow(f_lo, -52.0 / 9.0);
+    const double df4 = df * df * df * df;
+    q.q1 = (3.0 / 128.0) * (6160.0 / 81.0) * pow(f_lo, -17.0 / 3.0) * df4;
+    q.q2 = (3.0 / 128.0) * (4637464.0 / 6561.0) * pow(f_lo, -70.0 / 9.0) * df4;
+    q.ad = (3.0 / 128.0) * 4.0 * f_hi * 1.01 * kAU / kC;
+    const double r = f_hi / 0.01;
+    q.ct = 0.15 * (r > 1.0 ? r * r : 1.0);
+    q.kl = 0.05 * part_len;
+    q.pad = 0.0;
+    return q;
 }
 
 fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
 {
     if (pl->seg_groups == n_groups) return FSTAT_OK;
     std::vector<int32_t> seg_edge, part_seg;
-    make_segments(pl->edges, auto_segment_len(pl, n_groups), &seg_edge, &part_seg);
+    const bool aligned = segments_aligned(pl);
+    make_segments(pl->edges, auto_segment_len(pl, n_groups), aligned, &seg_edge, &part_seg);
+    const size_t n_seg = seg_edge.size() - 1;
+    std::vector<int32_t> gbase(n_seg * kNLevels);
+    std::vector<SegCrit> crit(n_seg);
+    std::vector<int8_t> maxlvl(n_seg);
+    for (size_t k = 0; k + 1 < part_seg.size(); ++k)
+        for (int32_t sgi = part_seg[k]; sgi < part_seg[k + 1]; ++sgi) {
+            const int64_t lo = seg_edge[sgi], hi = seg_edge[sgi + 1];
+            for (int l = 0; l < kNLevels; ++l)
+                gbase[(size_t)sgi * kNLevels + l] = (int32_t)((lo >> (kLevel0Shift + l)) + pl->cnt[l][k]);
+            crit[sgi] = make_seg_crit(pl->f0 + (double)lo * pl->df, pl->f0 + (double)hi * pl->df, pl->df,
+                                      (double)(pl->edges[k + 1] - pl->edges[k]));
+            maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && hi - lo >= 8) ? kNLevels - 1 : -1);
+        }
     CU_TRY(pl, grow(&pl->d_seg_edge, &pl->seg_cap, seg_edge.size()));
     CU_TRY(pl, grow(&pl->d_part_seg, &pl->part_cap, part_seg.size()));
+    CU_TRY(pl, grow(&pl->d_seg_gbase, &pl->gbase_cap, gbase.size()));
+    CU_TRY(pl, grow(&pl->d_seg_crit, &pl->crit_cap, crit.size()));
+    CU_TRY(pl, grow(&pl->d_seg_maxlvl, &pl->maxlvl_cap, maxlvl.size()));
     // synchronous copies: they order after any earlier evaluation that still reads the old arrays
     CU_TRY(pl, cudaDeviceSynchronize());
     CU_TRY(pl, cudaMemcpy(pl->d_seg_edge, seg_edge.data(), seg_edge.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
     CU_TRY(pl, cudaMemcpy(pl->d_part_seg, part_seg.data(), part_seg.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-    pl->n_seg = (int32_t)seg_edge.size() - 1;
+    CU_TRY(pl, cudaMemcpy(pl->d_seg_gbase, gbase.data(), gbase.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    CU_TRY(pl, cudaMemcpy(pl->d_seg_crit, crit.data(), crit.size() * sizeof(SegCrit), cudaMemcpyHostToDevice));
+    CU_TRY(pl, cudaMemcpy(pl->d_seg_maxlvl, maxlvl.data(), maxlvl.size() * sizeof(int8_t), cudaMemcpyHostToDevice));
+    pl->seg_edge_h = seg_edge;
+    pl->n_seg = (int32_t)n_seg;
     pl->seg_groups = n_groups;
     return FSTAT_OK;
 }
 
-int64_t n_segments_for(const fstat_plan *pl, int32_t n_groups)
+// Gram matrices of every stride level for the plan's current partitions (plan create / set_partitions).
+fstat_status build_gram_tables(fstat_plan *pl)
 {
-    const int64_t max_len = auto_segment_len(pl, n_groups);
-    int64_t n = 0;
-    for (size_t k = 0; k + 1 < pl->edges.size(); ++k) n += (pl->edges[k + 1] - pl->edges[k] + max_len - 1) / max_len;
-    return n;
+    const int32_t n_part = pl->n_part;
+    std::vector<int32_t> e32(n_part + 1);
+    for (int32_t k = 0; k <= n_part; ++k) e32[k] = (int32_t)pl->edges[k];
+    CU_TRY(pl, cudaDeviceSynchronize());       // earlier evaluations may still read the old tables
+    CU_TRY(pl, grow(&pl->d_edges32, &pl->edges32_cap, e32.size()));
+    CU_TRY(pl, grow(&pl->d_cnt, &pl->cnt_cap, (size_t)n_part));
+    CU_TRY(pl, cudaMemcpy(pl->d_edges32, e32.data(), e32.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    for (int l = 0; l < kNLevels; ++l) {
+        const int64_t S = (int64_t)kMinStride << l;
+        std::vector<int32_t> &cnt = pl->cnt[l];
+        cnt.assign(n_part, 0);
+        for (int32_t k = 1; k < n_part; ++k) cnt[k] = cnt[k - 1] + ((pl->edges[k] % S) != 0 ? 1 : 0);
+        if (!pl->fast_ok) continue;
+        const int64_t n_sub = (pl->n_bins + S - 1) / S + cnt[n_part - 1];
+        CU_TRY(pl, grow(&pl->d_gram[l], &pl->gram_cap[l], (size_t)n_sub * kNGram));
+        CU_TRY(pl, cudaMemcpy(pl->d_cnt, cnt.data(), (size_t)n_part * sizeof(int32_t), cudaMemcpyHostToDevice));
+        CU_TRY(pl, launch_build_gram(pl->d_table, pl->d_edges32, n_part, pl->n_bins, l, pl->d_cnt, pl->d_gram[l], 0));
+        CU_TRY(pl, cudaDeviceSynchronize());   // d_cnt is reused by the next level
+    }
+    return FSTAT_OK;
 }
 
 }  // namespace
@@ -209,6 +303,8 @@ void fstat_default_options(fstat_options *o)
     o->device = -1;
     o->inputs_on_device = 0;
     o->max_segment_bins = 0;
+    o->force_level = -2;
+    o->interp_tol = 1.0;
 }
 
 const char *fstat_status_str(fstat_status s)
@@ -244,6 +340,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     if (prop.major < 10)
         return fail(pl, FSTAT_ECUDA, "device is not sm_100-class (this library ships sm_100a code only)");
     CU_TRY(pl, main_kernel_configure());
+    CU_TRY(pl, fast_kernel_configure());
 
     const double *d_freq = freq, *d_dw = dw, *d_isn = isn;
     double *tmp = nullptr;
@@ -263,13 +360,21 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     if (e == cudaSuccess) e = cudaMalloc((void **)&d_err, sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMemset(d_err, 0, sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_table, (size_t)n_bins * kTabW * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_dwp, (size_t)n_bins * 2 * sizeof(double));
+    // node rows for bins -256 .. (floor((N-1)/256) + 2) * 256 in steps of kNodeStride
+    pl->n_node_rows = kNodePad + (((n_bins - 1) / kMaxStride + 2) * kMaxStride) / kNodeStride + 1;
+    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_node, (size_t)pl->n_node_rows * kTabW * sizeof(double));
     uint32_t bits = 0;
     if (e == cudaSuccess) {
         pl->df = (n_bins > 1) ? (fe[1] - fe[0]) / (double)(n_bins - 1) : fe[0];
         if (!(pl->df > 0.0) || !isfinite(pl->df)) bits |= ERR_FREQ_ORDER;
         else {
-            e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->opt.f_ref_e0,
-                                   pl->d_table, d_err, 0);
+            pl->f0 = fe[0];
+            pl->fast_ok = (fe[0] - (double)(kMaxStride + 1) * pl->df > 0.0) && n_bins > 1;
+            e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->d_table,
+                                   pl->d_dwp, d_err, 0);
+            if (e == cudaSuccess)
+                e = launch_build_nodes(d_freq, n_bins, pl->df, pl->opt.arm_length_m, pl->n_node_rows, pl->d_node, 0);
             if (e == cudaSuccess) e = cudaDeviceSynchronize();
             if (e == cudaSuccess) e = cudaMemcpy(&bits, d_err, sizeof(uint32_t), cudaMemcpyDeviceToHost);
         }
@@ -288,6 +393,10 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
         return fail(pl, FSTAT_EINVAL, why);
     }
     make_orbit_coef(pl->opt.arm_length_m, pl->opt.orbit_lambda, &pl->orb);
+    {
+        fstat_status gs = build_gram_tables(pl);
+        if (gs != FSTAT_OK) return gs;
+    }
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         CU_TRY(pl, cudaEventCreate(&pl->ev0[i]));
         CU_TRY(pl, cudaEventCreate(&pl->ev1[i]));
@@ -301,6 +410,9 @@ static void plan_free(fstat_plan *pl)
     DeviceGuard g(pl->device);
     cudaFree(pl->d_table); cudaFree(pl->d_seg_edge); cudaFree(pl->d_part_seg); cudaFree(pl->d_coef);
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
+    cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
+    for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
+    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
@@ -323,7 +435,8 @@ fstat_status fstat_plan_create(fstat_plan **out, int64_t n_bins, const double *f
     fstat_default_options(&o);
     if (opts) o = *opts;
     if (!(o.f_ref_e0 > 0.0) || !(o.arm_length_m > 0.0) || !isfinite(o.orbit_kappa) || !isfinite(o.orbit_lambda) ||
-        o.max_segment_bins < 0)
+        o.max_segment_bins < 0 || o.force_level < -2 || o.force_level >= kNLevels || !(o.interp_tol > 0.0) ||
+        !isfinite(o.interp_tol))
         return fail(nullptr, FSTAT_EINVAL, "bad option value");
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
@@ -368,7 +481,9 @@ fstat_status fstat_plan_set_partitions(fstat_plan *pl, int32_t n_part, const int
     }
     pl->n_part = n_part;
     pl->seg_groups = -1;    // re-segment on the next evaluation
-    return FSTAT_OK;
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    return build_gram_tables(pl);
 }
 
 void fstat_plan_destroy(fstat_plan *pl) { plan_free(pl); }
@@ -376,13 +491,34 @@ void fstat_plan_destroy(fstat_plan *pl) { plan_free(pl); }
 int64_t fstat_plan_n_bins(const fstat_plan *pl) { return pl ? pl->n_bins : 0; }
 int32_t fstat_plan_n_part(const fstat_plan *pl) { return pl ? pl->n_part : 0; }
 int32_t fstat_plan_device(const fstat_plan *pl) { return pl ? pl->device : -1; }
-int32_t fstat_launches_per_eval(void) { return 3; }
+int32_t fstat_launches_per_eval(void) { return 5; }
 
 int64_t fstat_plan_n_ctas(const fstat_plan *pl, int64_t P)
 {
     if (!pl || P < 1) return 0;
     const int64_t n_groups = (P + kThreads - 1) / kThreads;
     return n_groups * n_segments_for(pl, (int32_t)n_groups);
+}
+
+fstat_status fstat_plan_level_bins(fstat_plan *pl, int64_t *bins_out, int64_t *subblocks_out)
+{
+    if (!pl || !bins_out || !subblocks_out) return FSTAT_EINVAL;
+    for (int l = 0; l <= kNLevels; ++l) bins_out[l] = subblocks_out[l] = 0;
+    if (pl->last_groups < 1 || pl->seg_groups != pl->last_groups) return FSTAT_OK;
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    const size_t n = (size_t)pl->n_seg * (size_t)pl->last_groups;
+    std::vector<int8_t> lv(n);
+    CU_TRY(pl, cudaDeviceSynchronize());
+    CU_TRY(pl, cudaMemcpy(lv.data(), pl->d_level, n, cudaMemcpyDeviceToHost));
+    for (int32_t gidx = 0; gidx < pl->last_groups; ++gidx)
+        for (int32_t sgi = 0; sgi < pl->n_seg; ++sgi) {
+            const int l = lv[(size_t)gidx * pl->n_seg + sgi];
+            const int64_t lo = pl->seg_edge_h[sgi], hi = pl->seg_edge_h[sgi + 1];
+            bins_out[l + 1] += hi - lo;
+            if (l >= 0) subblocks_out[l + 1] += ((hi - 1) >> (kLevel0Shift + l)) - (lo >> (kLevel0Shift + l)) + 1;
+        }
+    return FSTAT_OK;
 }
 
 int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out)
@@ -422,12 +558,32 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)P_pad * kNCoef));
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)P_pad));
     CU_TRY(pl, grow(&pl->d_partial, &pl->partial_cap, (size_t)pl->n_seg * kNAcc * (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_level, &pl->level_cap, (size_t)pl->n_seg * (size_t)n_groups));
+    pl->last_groups = (int32_t)n_groups;
 
     CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef, pl->d_valid, st));
+    CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
+                               pl->d_seg_maxlvl, pl->opt.interp_tol * 1e-7 * (2.0 / kPi), pl->opt.interp_tol * 1e-7,
+                               pl->opt.force_level, pl->d_level, st));
+    FastArgs fa;
+    fa.dwp = pl->d_dwp;
+    fa.node = pl->d_node;
+    for (int l = 0; l < kNLevels; ++l) fa.gram[l] = pl->d_gram[l];
+    fa.coef = pl->d_coef;
+    fa.seg_edge = pl->d_seg_edge;
+    fa.seg_gbase = pl->d_seg_gbase;
+    fa.level = pl->d_level;
+    fa.partial = pl->d_partial;
+    fa.P_pad = P_pad;
+    fa.n_groups = (int32_t)n_groups;
+    fa.n_seg = pl->n_seg;
+    fa.df = pl->df;
+    fa.orb = pl->orb;
     MainArgs a;
     a.table = pl->d_table;
     a.coef = pl->d_coef;
     a.seg_edge = pl->d_seg_edge;
+    a.level = pl->d_level;
     a.partial = pl->d_partial;
     a.P_pad = P_pad;
     a.P = (int32_t)P;
@@ -436,6 +592,7 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     a.orb = pl->orb;
     const int slot = (int)(pl->n_timed % fstat_plan::kRing);
     CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
+    if (pl->fast_ok) CU_TRY(pl, launch_fast(fa, st));
     CU_TRY(pl, launch_main(a, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;

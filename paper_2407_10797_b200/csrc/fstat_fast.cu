@@ -1,0 +1,464 @@
+// fstat_fast.cu -- the interpolating main kernel of the batched semi-coherent F-statistic and its
+// plan-time tables.
+//
+// Idea: per (particle, bin) the template is u_P = K_f f^(-7/6) T'_P e^{-i Phi} with
+// a FAST carrier phase Phi (many radians per bin) and SLOW factors: T'_+, T'_x and the non-linear part
+// of Phi vary on the scale of the orbital phase at t_f, i.e. over hundreds to thousands of bins.  The
+// kernel therefore evaluates the full FP64 model (model_eval, the same device code the direct kernel runs
+// at every bin) only at NODES every S bins and carries the slow factors between nodes with the cubic
+// through the four surrounding nodes.  With T'(i) a cubic in the bin index inside a sub-block,
+//     z_P  = sum_i dw'_i e^{+i Phi_i} conj(T'_P(i)) = sum_n conj(c^P_n) A_n ,
+//     A_n  = sum_i q_i C(j1 - i + n - 1, n)        (n-fold running sums of q_i = dw'_i e^{+i Phi_i}),
+//     m_PQ = sum_i w'_i T'_P(i) conj(T'_Q(i))      = sum_ab y^P_a G_ab conj(y^Q_b)
+// with c^P_n the Newton (binomial-basis) coefficients of the cubic, y^P_a its four node values and
+// G_ab = sum_i w'_i l_a(i) l_b(i) a plan-time Gram matrix of the Lagrange basis.  Per bin that leaves:
+// the phase by forward differences (exact range reduction in quarter turns), one sincos, one complex
+// product with the folded data and four complex running sums -- about 30 FP64 instructions instead of
+// 265.  S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
+// work items for which no stride is accurate enough are left to the direct kernel.
+//
+// Inner products: PAPER.md:66 Eq. 4, :89-91 Eq. 8-9, :117 Eq. 12.  Template: :397-405 Eq. A1-A3,
+// :206-229 Eq. 17-20 (N = 0).
+#include "fstat_device.cuh"
+#include "fstat_internal.h"
+#include "fstat_model.cuh"
+
+#include <math.h>
+
+namespace fstat {
+
+// =================================================================================================
+// plan time: node table.  Row r holds the particle-independent basis at bin b = (r - kNodePad) * 8;
+// inside the band the frequency is the caller's freq[b] (so that nodes and bins see the same number),
+// outside it is the uniform continuation of the grid.
+// =================================================================================================
+__global__ void build_nodes_kernel(const double *__restrict__ freq, int64_t n_bins, double df, double L,
+                                   int64_t n_rows, double *__restrict__ node)
+{
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_rows) return;
+    const int64_t b = (r - kNodePad) * kNodeStride;
+    double f;
+    if (b < 0) f = freq[0] + (double)b * df;
+    else if (b >= n_bins) f = freq[n_bins - 1] + (double)(b - (n_bins - 1)) * df;
+    else f = freq[b];
+    double *row = node + r * kTabW;
+    if (f > 0.0) fill_basis_row(f, L, row);
+    else {
+#pragma unroll
+        for (int j = 0; j < kTabW; ++j) row[j] = 0.0;
+        row[T_F] = f;
+    }
+    row[T_DWR] = 0.0;
+    row[T_DWI] = 0.0;
+    row[T_W] = 0.0;
+}
+
+cudaError_t launch_build_nodes(const double *freq, int64_t n_bins, double df, double arm_length_m,
+                               int64_t n_rows, double *node, cudaStream_t st)
+{
+    const int nt = 128;
+    build_nodes_kernel<<<(unsigned)((n_rows + nt - 1) / nt), nt, 0, st>>>(freq, n_bins, df, arm_length_m, n_rows, node);
+    return cudaGetLastError();
+}
+
+// Lagrange basis of the nodes t = -1, 0, 1, 2 at t
+__device__ __forceinline__ void lagrange4(double t, double (&l)[4])
+{
+    const double tp = t + 1.0, tm = t - 1.0, tm2 = t - 2.0;
+    l[0] = -t * tm * tm2 * (1.0 / 6.0);
+    l[1] = tp * tm * tm2 * 0.5;
+    l[2] = -tp * t * tm2 * 0.5;
+    l[3] = tp * t * tm * (1.0 / 6.0);
+}
+
+// =================================================================================================
+// plan time (per partition set): Gram matrices.  Level `level` cuts every partition at the multiples of
+// S = 8 << level; sub-block [j0, j1) of node interval m = j0 / S in partition k has the table index
+// m + cnt[k], cnt[k] = number of interior partition edges e_1..e_k that are not multiples of S.
+// One thread per node interval; it walks its bins and flushes at every partition edge.
+// =================================================================================================
+__global__ void build_gram_kernel(const double *__restrict__ table, const int32_t *__restrict__ edges,
+                                  int32_t n_part, int64_t n_bins, int level, const int32_t *__restrict__ cnt,
+                                  double *__restrict__ gram)
+{
+    const int S = kMinStride << level;
+    const int64_t m = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t b0 = m * S;
+    if (b0 >= n_bins) return;
+    const int64_t b1 = (b0 + S < n_bins) ? b0 + S : n_bins;
+    // partition of bin b0: largest k with edges[k] <= b0
+    int lo = 0, hi = n_part;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if ((int64_t)edges[mid] <= b0) lo = mid; else hi = mid;
+    }
+    int k = lo;
+    const double rS = 1.0 / (double)S;
+    double g[kNGram];
+#pragma unroll
+    for (int j = 0; j < kNGram; ++j) g[j] = 0.0;
+    for (int64_t i = b0; i < b1; ++i) {
+        if (i == (int64_t)edges[k + 1]) {                  // partition edge inside the interval: flush
+            double *out = gram + (m + cnt[k]) * kNGram;
+#pragma unroll
+            for (int j = 0; j < kNGram; ++j) { out[j] = g[j]; g[j] = 0.0; }
+            ++k;
+        }
+        const double w = table[i * kTabW + T_W];
+        double l[4];
+        lagrange4((double)(i - b0) * rS, l);
+        int j = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = a; b < 4; ++b) g[j++] += w * l[a] * l[b];
+    }
+    double *out = gram + (m + cnt[k]) * kNGram;
+#pragma unroll
+    for (int j = 0; j < kNGram; ++j) out[j] = g[j];
+}
+
+cudaError_t launch_build_gram(const double *table, const int32_t *edges, int32_t n_part, int64_t n_bins,
+                              int level, const int32_t *cnt, double *gram, cudaStream_t st)
+{
+    const int S = kMinStride << level;
+    const int64_t n_int = (n_bins + S - 1) / S;
+    const int nt = 128;
+    build_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(table, edges, n_part, n_bins, level, cnt, gram);
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// a1b: stride selection.  One CTA per particle group: the group's largest chirp coefficient c3 (the
+// f^(-5/3) term) and eccentric coefficient |c9| bound, through SegCrit, the orbital phase advance per
+// bin omega and with it the interpolation errors of the carrier phase and of the response at stride S:
+//     E_phi(S) = S^4 (c3 q1 + |c9| q2 + ad omega^4)   [quarter turns],
+//     E_T(S)   = ct (omega S)^4 / min(1, kl omega)     (relative, as seen through M_k^-1).
+// The level written is the largest one that meets both tolerances, or -1 (direct kernel).
+// =================================================================================================
+__global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__restrict__ coef,
+                                                            const int32_t *__restrict__ valid, int64_t P_pad,
+                                                            int32_t n_seg, const SegCrit *__restrict__ crit,
+                                                            const int8_t *__restrict__ seg_maxlvl, double tol_phi_qt,
+                                                            double tol_resp, int32_t force_level,
+                                                            int8_t *__restrict__ level)
+{
+    __shared__ double s3[kThreads / 32], s9[kThreads / 32];
+    const int tid = threadIdx.x;
+    const int grp = blockIdx.x;
+    const int64_t p = (int64_t)grp * kThreads + tid;
+    double c3 = 0.0, c9 = 0.0;
+    if (valid[p]) {
+        c3 = fabs(coef[3 * P_pad + p]);
+        c9 = fabs(coef[9 * P_pad + p]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        c3 = fmax(c3, __shfl_xor_sync(0xffffffffu, c3, o));
+        c9 = fmax(c9, __shfl_xor_sync(0xffffffffu, c9, o));
+    }
+    if ((tid & 31) == 0) { s3[tid >> 5] = c3; s9[tid >> 5] = c9; }
+    __syncthreads();
+    c3 = s3[0]; c9 = s9[0];
+#pragma unroll
+    for (int w = 1; w < kThreads / 32; ++w) { c3 = fmax(c3, s3[w]); c9 = fmax(c9, s9[w]); }
+
+    for (int seg = tid; seg < n_seg; seg += kThreads) {
+        const int mx = seg_maxlvl[seg];
+        int lvl;
+        if (force_level >= -1) {
+            lvl = force_level < mx ? force_level : mx;
+        } else {
+            const SegCrit q = crit[seg];
+            const double om = fma(c3, q.p1, c9 * q.p2);
+            const double om2 = om * om, om4 = om2 * om2;
+            const double ephi1 = fma(c3, q.q1, fma(c9, q.q2, q.ad * om4));   // per S^4
+            // the response error is seen through M_k^-1: a partition over which the response barely changes
+            // (kl omega < 1) has a near-singular M_k and amplifies it by 1 / sqrt(det) (hazard H3)
+            const double kom = q.kl * om;
+            const double eT1 = (kom < 1.0) ? q.ct * om2 * om / q.kl : q.ct * om4;
+            lvl = -1;
+            for (int l = 0; l <= mx; ++l) {
+                const double S = (double)(kMinStride << l), S2 = S * S, S4 = S2 * S2;
+                if (ephi1 * S4 <= tol_phi_qt && eT1 * S4 <= tol_resp) lvl = l;
+            }
+        }
+        level[(int64_t)grp * n_seg + seg] = (int8_t)lvl;
+    }
+}
+
+cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
+                            int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
+                            double tol_resp, int32_t force_level, int8_t *level, cudaStream_t st)
+{
+    schedule_kernel<<<(unsigned)n_groups, kThreads, 0, st>>>(coef, valid, P_pad, n_seg, crit, seg_maxlvl,
+                                                            tol_phi_qt, tol_resp, force_level, level);
+    return cudaGetLastError();
+}
+
+// =================================================================================================
+// a2-a5, interpolating kernel.  Grid = particle groups x segments (same work items as the direct kernel),
+// CTA = 128 threads = 128 particles.  The folded data dw' of the segment streams through a 4-stage
+// shared-memory ring of 256-bin tiles (TMA bulk copies, mbarrier completion); every thread reads the
+// same element (broadcast).  Node rows and Gram matrices are warp-uniform global loads (L1/L2 hits).
+// =================================================================================================
+struct __align__(16) FastSmem {
+    double2 tile[kFastStages][kFastTile];
+    uint64_t full[kFastStages];
+};
+
+// x - 4 rint(x / 4): exact for |x| < 2^51
+__device__ __forceinline__ double red4(double x) { return fma(-4.0, rint(0.25 * x), x); }
+
+// (c * f) mod 4 to full precision: the product is split exactly into hi + lo by one FMA
+__device__ __forceinline__ double mulmod4(double c, double f)
+{
+    const double hi = c * f;
+    const double lo = fma(c, f, -hi);
+    return red4(hi) + lo;
+}
+
+// sin and cos of (pi/2) w for |w| <= 1/2 (near-minimax in w^2; errors 3.4e-12 and 4.8e-11)
+__device__ __forceinline__ void sincos_small(double w, double &ps, double &pc)
+{
+    const double w2 = w * w;
+    double s = 1.582063035564773e-4;
+    s = fma(s, w2, -4.6812662567262455e-3);
+    s = fma(s, w2, 7.9692582725630620e-2);
+    s = fma(s, w2, -0.64596409614679535);
+    s = fma(s, w2, 1.5707963267880999);
+    ps = s * w;
+    double c = 9.036280663802505e-4;
+    c = fma(c, w2, -2.086006950026408e-2);
+    c = fma(c, w2, 0.25366920365511348);
+    c = fma(c, w2, -1.2337005406331622);
+    pc = fma(c, w2, 0.99999999995248942);
+}
+
+// Newton-basis coefficients c_n (basis C(u + n - 1, n), u = j1 - i) of the cubic through the node values
+// y0..y3 at t = -1, 0, 1, 2 (t = s / S), for a sub-block that ends U bins after node 0.
+__device__ __forceinline__ void newton_coefs(double y0, double y1, double y2, double y3, double rS, double U,
+                                             double (&c)[4])
+{
+    const double d0 = y0 - y1, d2 = y2 - y1, d3 = y3 - y1;
+    const double a1 = fma(d0, -1.0 / 3.0, fma(d3, -1.0 / 6.0, d2));
+    const double a2 = 0.5 * (d0 + d2);
+    const double a3 = fma(d2, -0.5, (d3 - d0) * (1.0 / 6.0));
+    const double g1 = a1 * rS, g2 = a2 * rS * rS, g3 = a3 * rS * rS * rS;
+    const double e0 = fma(U, fma(U, fma(U, g3, g2), g1), y1);
+    const double e1 = -fma(U, fma(3.0 * U, g3, 2.0 * g2), g1);
+    const double e2 = fma(3.0 * U, g3, g2);
+    const double e3 = -g3;
+    c[0] = e0;
+    c[1] = e1 - e2 + e3;
+    c[2] = fma(-6.0, e3, 2.0 * e2);
+    c[3] = 6.0 * e3;
+}
+
+__device__ __forceinline__ void load_coef(const double *__restrict__ cf, int64_t P_pad, double (&c)[kNCoef])
+{
+#pragma unroll
+    for (int j = 0; j < kNCoef; ++j) c[j] = cf[(int64_t)j * P_pad];
+}
+
+__global__ void __launch_bounds__(kThreads, 3) fstat_fast_kernel(const __grid_constant__ FastArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    FastSmem &sm = *reinterpret_cast<FastSmem *>(smem_raw);
+
+    const int tid = threadIdx.x;
+    const int grp = blockIdx.x % a.n_groups;
+    const int seg = blockIdx.x / a.n_groups;
+    const int lvl = a.level[(int64_t)grp * a.n_seg + seg];
+    if (lvl < 0) return;                                     // CTA-uniform: left to the direct kernel
+    const int sh = kLevel0Shift + lvl;
+    const double rS = 1.0 / (double)(1 << sh);
+    const int64_t p = (int64_t)grp * kThreads + tid;         // < P_pad by construction
+    const double *cf = a.coef + p;
+
+    const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
+    const int t_first = lo >> 8;
+    const int n_tiles = ((hi - 1) >> 8) - t_first + 1;
+    const double2 *dwp = reinterpret_cast<const double2 *>(a.dwp);
+
+    auto issue_tile = [&](int t) {                           // t = tile number relative to t_first
+        const int slot = t % kFastStages;
+        const int b0 = max(lo, (t_first + t) << 8), b1 = min(hi, (t_first + t + 1) << 8);
+        const uint32_t bytes = (uint32_t)(b1 - b0) * (uint32_t)sizeof(double2);
+        mbar_expect_tx(&sm.full[slot], bytes);
+        tma_load_1d(&sm.tile[slot][b0 & (kFastTile - 1)], dwp + b0, bytes, &sm.full[slot]);
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kFastStages; ++s) mbar_init(&sm.full[s], 1);
+        mbar_fence_init();
+        for (int s = 0; s < kFastStages && s < n_tiles; ++s) issue_tile(s);
+    }
+
+    // linear phase term 2 pi f t_c in quarter turns: per-bin advance, reduced mod 4
+    const double c0 = cf[0];
+    const double slope = mulmod4(c0, a.df);
+
+    // node window: values at nodes m-1, m, m+1, m+2 of (psi_nl, T'_+ re, im, T'_x re, im)
+    double yph[4], ypr[4], ypi[4], ycr[4], yci[4];
+    int m = lo >> sh;
+    {
+        double c[kNCoef];
+        load_coef(cf, a.P_pad, c);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double2 *row = reinterpret_cast<const double2 *>(
+                a.node + ((int64_t)kNodePad + ((int64_t)(m + k - 1) << lvl)) * kTabW);
+            model_eval(row, c, a.orb, yph[k], ypr[k], ypi[k], ycr[k], yci[k]);
+        }
+    }
+    __syncthreads();                                         // barriers initialised before anyone waits
+
+    double acc[kNAcc];
+#pragma unroll
+    for (int j = 0; j < kNAcc; ++j) acc[j] = 0.0;
+
+    const double *gram = a.gram[lvl] + (int64_t)a.seg_gbase[seg * kNLevels + lvl] * kNGram;
+    int cur_tile = -1;
+    int j0 = lo;
+    while (j0 < hi) {
+        const int node0 = m << sh;                           // bin of node "0" of this interval
+        const int j1 = min(hi, node0 + (1 << sh));
+        // ---- new node m+2
+        double fnode;
+        {
+            double c[kNCoef];
+            load_coef(cf, a.P_pad, c);
+            const double2 *row = reinterpret_cast<const double2 *>(
+                a.node + ((int64_t)kNodePad + ((int64_t)(m + 2) << lvl)) * kTabW);
+            model_eval(row, c, a.orb, yph[3], ypr[3], ypi[3], ycr[3], yci[3]);
+            fnode = a.node[((int64_t)kNodePad + ((int64_t)m << lvl)) * kTabW + T_F];
+        }
+        // ---- carrier phase: cubic through the 4 nodes + exact linear term, as forward differences
+        double t, D1, D2, D3;
+        {
+            const double d0 = yph[0] - yph[1], d2 = yph[2] - yph[1], d3 = yph[3] - yph[1];
+            const double a1 = fma(d0, -1.0 / 3.0, fma(d3, -1.0 / 6.0, d2));
+            const double a2 = 0.5 * (d0 + d2);
+            const double a3 = fma(d2, -0.5, (d3 - d0) * (1.0 / 6.0));
+            const double G0 = red4(yph[1]) + mulmod4(c0, fnode);
+            const double G1 = red4(fma(a1, rS, slope));
+            const double G2 = a2 * rS * rS, G3 = a3 * rS * rS * rS;
+            const double s0 = (double)(j0 - node0);
+            t = fma(s0, fma(s0, fma(s0, G3, G2), G1), G0);
+            D1 = fma(G3, fma(3.0 * s0, s0 + 1.0, 1.0), fma(G2, fma(2.0, s0, 1.0), G1));
+            D2 = fma(G3, fma(6.0, s0, 6.0), 2.0 * G2);
+            D3 = 6.0 * G3;
+        }
+        // ---- the tile that holds [j0, j1)
+        const int tl = (j0 >> 8) - t_first;
+        if (tl != cur_tile) {
+            if (cur_tile >= 0) {
+                __syncthreads();                             // every thread is done with the previous tile
+                if (tid == 0 && cur_tile + kFastStages < n_tiles) issue_tile(cur_tile + kFastStages);
+            }
+            cur_tile = tl;
+            mbar_wait(&sm.full[tl % kFastStages], (uint32_t)((tl / kFastStages) & 1));
+        }
+        const double2 *tp = &sm.tile[tl % kFastStages][j0 & (kFastTile - 1)];
+        const int nb = j1 - j0;
+
+        // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3
+        double A0r = 0.0, A0i = 0.0, A1r = 0.0, A1i = 0.0, A2r = 0.0, A2i = 0.0, A3r = 0.0, A3i = 0.0;
+        int qacc = 0;
+        const double MAGIC = 6755399441055744.0;             // 1.5 * 2^52
+#pragma unroll 2
+        for (int b = 0; b < nb; ++b) {
+            const double2 d = tp[b];
+            const double tm = t + MAGIC;
+            qacc += __double2loint(tm);
+            const double w = t - (tm - MAGIC);
+            double ps, pc;
+            sincos_small(w, ps, pc);
+            const bool swap = (qacc & 1) != 0;
+            const double ss = swap ? pc : ps;
+            const double cc = swap ? ps : pc;
+            const int sflip = (qacc & 2) << 30;
+            const int cflip = ((qacc + 1) & 2) << 30;
+            const double sn = __hiloint2double(__double2hiint(ss) ^ sflip, __double2loint(ss));
+            const double cs = __hiloint2double(__double2hiint(cc) ^ cflip, __double2loint(cc));
+            const double qr = fma(d.x, cs, -d.y * sn);
+            const double qi = fma(d.x, sn, d.y * cs);
+            A0r += qr; A0i += qi;
+            A1r += A0r; A1i += A0i;
+            A2r += A1r; A2i += A1i;
+            A3r += A2r; A3i += A2i;
+            t = w + D1;
+            D1 += D2;
+            D2 += D3;
+        }
+
+        // ---- z_P += sum_n conj(c^P_n) A_n
+        const double U = (double)(j1 - node0);
+        {
+            double cr[4], ci[4];
+            newton_coefs(ypr[0], ypr[1], ypr[2], ypr[3], rS, U, cr);
+            newton_coefs(ypi[0], ypi[1], ypi[2], ypi[3], rS, U, ci);
+            acc[0] += fma(cr[0], A0r, fma(ci[0], A0i, fma(cr[1], A1r, fma(ci[1], A1i,
+                      fma(cr[2], A2r, fma(ci[2], A2i, fma(cr[3], A3r, ci[3] * A3i)))))));
+            acc[1] += fma(cr[0], A0i, fma(-ci[0], A0r, fma(cr[1], A1i, fma(-ci[1], A1r,
+                      fma(cr[2], A2i, fma(-ci[2], A2r, fma(cr[3], A3i, -ci[3] * A3r)))))));
+            newton_coefs(ycr[0], ycr[1], ycr[2], ycr[3], rS, U, cr);
+            newton_coefs(yci[0], yci[1], yci[2], yci[3], rS, U, ci);
+            acc[2] += fma(cr[0], A0r, fma(ci[0], A0i, fma(cr[1], A1r, fma(ci[1], A1i,
+                      fma(cr[2], A2r, fma(ci[2], A2i, fma(cr[3], A3r, ci[3] * A3i)))))));
+            acc[3] += fma(cr[0], A0i, fma(-ci[0], A0r, fma(cr[1], A1i, fma(-ci[1], A1r,
+                      fma(cr[2], A2i, fma(-ci[2], A2r, fma(cr[3], A3i, -ci[3] * A3r)))))));
+        }
+        // ---- m_PQ += y^P G conj(y^Q)   (Gram matrix of the Lagrange basis over this sub-block)
+        {
+            const double2 *gp = reinterpret_cast<const double2 *>(gram);
+            const double2 g01 = gp[0], g23 = gp[1], g45 = gp[2], g67 = gp[3], g89 = gp[4];
+            const double G[4][4] = {{g01.x, g01.y, g23.x, g23.y},
+                                    {g01.y, g45.x, g45.y, g67.x},
+                                    {g23.x, g45.y, g67.y, g89.x},
+                                    {g23.y, g67.x, g89.x, g89.y}};
+            double mpp = 0.0, mcc = 0.0, mre = 0.0, mim = 0.0;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const double vpr = fma(G[r][0], ypr[0], fma(G[r][1], ypr[1], fma(G[r][2], ypr[2], G[r][3] * ypr[3])));
+                const double vpi = fma(G[r][0], ypi[0], fma(G[r][1], ypi[1], fma(G[r][2], ypi[2], G[r][3] * ypi[3])));
+                const double vcr = fma(G[r][0], ycr[0], fma(G[r][1], ycr[1], fma(G[r][2], ycr[2], G[r][3] * ycr[3])));
+                const double vci = fma(G[r][0], yci[0], fma(G[r][1], yci[1], fma(G[r][2], yci[2], G[r][3] * yci[3])));
+                mpp = fma(ypr[r], vpr, fma(ypi[r], vpi, mpp));
+                mcc = fma(ycr[r], vcr, fma(yci[r], vci, mcc));
+                mre = fma(ypr[r], vcr, fma(ypi[r], vci, mre));      // Re sum y^+ conj(v^x)
+                mim = fma(ypi[r], vcr, fma(-ypr[r], vci, mim));     // Im
+            }
+            acc[4] += mpp; acc[5] += mcc; acc[6] += mre; acc[7] += mim;
+            gram += kNGram;
+        }
+        // ---- slide the node window
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            yph[k] = yph[k + 1]; ypr[k] = ypr[k + 1]; ypi[k] = ypi[k + 1]; ycr[k] = ycr[k + 1]; yci[k] = yci[k + 1];
+        }
+        j0 = j1;
+        ++m;
+    }
+
+    double *out = a.partial + ((int64_t)seg * kNAcc) * a.P_pad + p;
+#pragma unroll
+    for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
+}
+
+cudaError_t fast_kernel_configure()
+{
+    return cudaFuncSetAttribute(fstat_fast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)sizeof(FastSmem));
+}
+
+cudaError_t launch_fast(const FastArgs &a, cudaStream_t st)
+{
+    const int64_t n_cta = (int64_t)a.n_groups * a.n_seg;
+    fstat_fast_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace fstat

@@ -51,10 +51,34 @@ struct OrbitCoef {
     double c[3][3][7];
 };
 
+// ---- interpolating ("fast") path: the slow factors of the template (carrier phase without its linear
+// term, T'_+, T'_x) are evaluated in full FP64 only at nodes every S = 8 << level bins and carried
+// between nodes by the cubic through the four surrounding nodes.
+constexpr int kNLevels = 6;                          // S = 8, 16, 32, 64, 128, 256
+constexpr int kLevel0Shift = 3;
+constexpr int kMinStride = 1 << kLevel0Shift;
+constexpr int kMaxStride = kMinStride << (kNLevels - 1);   // 256; segment cuts inside a partition are multiples of it
+constexpr int kNodeStride = kMinStride;              // the node table has one row every 8 bins
+constexpr int kNodePad = kMaxStride / kNodeStride;   // rows before bin 0 (nodes down to bin -256)
+constexpr int kFastTile = 256;                       // bins per TMA tile of the folded data (4 KiB), 256-aligned
+constexpr int kFastStages = 4;
+constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
+
+// per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)
+struct SegCrit {
+    double p1, p2;   // omega [orbital rad / bin] = c3 p1 + |c9| p2
+    double q1, q2;   // (3/128) |d^4 Psi / dk^4| = c3 q1 + |c9| q2       [quarter turns per bin^4]
+    double ad;       // (3/128) x Doppler phase amplitude                 [quarter turns]
+    double ct;       // response: relative error = ct (omega S)^4
+    double kl;       // 0.05 x partition length [bins]: sqrt(normalised det M_k) >~ min(1, kl omega)  (hazard H3)
+    double pad;
+};
+
 struct MainArgs {
     const double *table;      // [n_bins][kTabW]
     const double *coef;       // [kNCoef][P_pad]
     const int32_t *seg_edge;  // [n_seg + 1]
+    const int8_t *level;      // [n_groups][n_seg] or nullptr; the direct kernel runs the items with level < 0
     double *partial;          // [n_seg][kNAcc][P_pad]
     int64_t P_pad;
     int32_t P;
@@ -69,9 +93,34 @@ enum : uint32_t {
     ERR_ISN_NONFINITE = 16u, ERR_ISN_NONPOS = 32u
 };
 
+struct FastArgs {
+    const double *dwp;            // [n_bins][2] folded data 4 df f^(-7/6) conj(K_f) d/S_n
+    const double *node;           // [n_node_rows][kTabW]; row r <-> bin (r - kNodePad) * kNodeStride
+    const double *gram[kNLevels]; // [n_sub(level)][kNGram]
+    const double *coef;           // [kNCoef][P_pad]
+    const int32_t *seg_edge;      // [n_seg + 1]
+    const int32_t *seg_gbase;     // [n_seg][kNLevels] index of the segment's first sub-block in gram[level]
+    const int8_t *level;          // [n_groups][n_seg]
+    double *partial;              // [n_seg][kNAcc][P_pad]
+    int64_t P_pad;
+    int32_t n_groups;
+    int32_t n_seg;
+    double df;
+    OrbitCoef orb;
+};
+
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
-                               double df, double arm_length_m, double f_ref_e0, double *table,
+                               double df, double arm_length_m, double *table, double *dwp,
                                uint32_t *err_bits, cudaStream_t st);
+cudaError_t launch_build_nodes(const double *freq, int64_t n_bins, double df, double arm_length_m,
+                               int64_t n_rows, double *node, cudaStream_t st);
+cudaError_t launch_build_gram(const double *table, const int32_t *edges, int32_t n_part, int64_t n_bins,
+                              int level, const int32_t *cnt, double *gram, cudaStream_t st);
+cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
+                            int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
+                            double tol_resp, int32_t force_level, int8_t *level, cudaStream_t st);
+cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
+cudaError_t fast_kernel_configure();
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
                             double *coef, int32_t *valid, cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);

@@ -10,6 +10,7 @@
 // Citations are to /root/reference/PAPER.md (line, equation) and to DESIGN.md readings (A1..A24).
 #include "fstat_device.cuh"
 #include "fstat_internal.h"
+#include "fstat_model.cuh"
 
 #include <math.h>
 
@@ -20,7 +21,8 @@ namespace fstat {
 // =================================================================================================
 __global__ void build_table_kernel(const double *__restrict__ freq, const double *__restrict__ dw,
                                    const double *__restrict__ isn, int64_t n_bins, double df, double L,
-                                   double *__restrict__ table, uint32_t *__restrict__ err_bits)
+                                   double *__restrict__ table, double2 *__restrict__ dwp,
+                                   uint32_t *__restrict__ err_bits)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_bins) return;
@@ -36,54 +38,26 @@ __global__ void build_table_kernel(const double *__restrict__ freq, const double
     if (err) { atomicOr(err_bits, err); return; }
 
     double *row = table + i * kTabW;
-    const double lnf = log(f);
-    const double cb = cbrt(f);                 // f^(1/3)
-    const double icb = 1.0 / cb;               // f^(-1/3)
-    const double fm23 = icb * icb;
-    const double fm1 = 1.0 / f;
-    const double fm53 = fm1 * fm23;
-    const double fm349 = pow(f, -34.0 / 9.0);
-    const double iyr = 1.0 / kYear;
-    row[T_F] = f;
-    row[T_LNF] = lnf;
-    row[T_FM53] = fm53;
-    row[T_FM1] = fm1;
-    row[T_FM23] = fm23;
-    row[T_FM13] = icb;
-    row[T_FP13] = cb;
-    row[T_FP13LN] = cb * lnf;
-    row[T_FM349] = fm349;
-    row[T_XQ] = 2.0 * f * L / kC;
-    // D_j = (dB_j/df) / year, same order as B_2..B_9
-    row[T_D0 + 0] = fm1 * iyr;                                   // ln f
-    row[T_D0 + 1] = (-5.0 / 3.0) * fm53 * fm1 * iyr;              // f^(-5/3)
-    row[T_D0 + 2] = -fm1 * fm1 * iyr;                             // f^(-1)
-    row[T_D0 + 3] = (-2.0 / 3.0) * fm53 * iyr;                    // f^(-2/3)
-    row[T_D0 + 4] = (-1.0 / 3.0) * icb * fm1 * iyr;               // f^(-1/3)
-    row[T_D0 + 5] = (1.0 / 3.0) * fm23 * iyr;                     // f^(1/3)
-    row[T_D0 + 6] = fm23 * (1.0 + lnf / 3.0) * iyr;               // f^(1/3) ln f
-    row[T_D0 + 7] = (-34.0 / 9.0) * fm349 * fm1 * iyr;            // f^(-34/9)
-    const double x = kPi * f * L / kC;
-    double s2x, c2x;
-    sincos(2.0 * x, &s2x, &c2x);
-    row[T_C2X] = c2x;
-    row[T_S2X] = s2x;
+    fill_basis_row(f, L, row);
+    const double s2x = row[T_S2X], c2x = row[T_C2X];
     // conj(K_f) = 2 sin 2x (cos 2x + i sin 2x), |K_f|^2 = 4 sin^2 2x   (K_f = -i (1 - z^2))
     const double amp = 4.0 * df * pow(f, -7.0 / 6.0);
     const double kr = 2.0 * s2x * c2x, ki = 2.0 * s2x * s2x;
-    row[T_DWR] = amp * (dr * kr - di * ki);
-    row[T_DWI] = amp * (dr * ki + di * kr);
+    const double qr = amp * (dr * kr - di * ki), qi = amp * (dr * ki + di * kr);
+    row[T_DWR] = qr;
+    row[T_DWI] = qi;
     row[T_W] = 4.0 * df * pow(f, -7.0 / 3.0) * (4.0 * s2x * s2x) * w;
-    row[T_X] = x;
+    dwp[i] = make_double2(qr, qi);
 }
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
-                               double df, double arm_length_m, double /*f_ref_e0*/, double *table,
+                               double df, double arm_length_m, double *table, double *dwp,
                                uint32_t *err_bits, cudaStream_t st)
 {
     const int nt = 256;
     const int64_t nb = (n_bins + nt - 1) / nt;
-    build_table_kernel<<<(unsigned)nb, nt, 0, st>>>(freq, dw, isn, n_bins, df, arm_length_m, table, err_bits);
+    build_table_kernel<<<(unsigned)nb, nt, 0, st>>>(freq, dw, isn, n_bins, df, arm_length_m, table,
+                                                    reinterpret_cast<double2 *>(dwp), err_bits);
     return cudaGetLastError();
 }
 
@@ -162,122 +136,17 @@ struct __align__(16) MainSmem {
 
 size_t main_kernel_smem_bytes() { return sizeof(MainSmem); }
 
-// one orbit coordinate from the trig basis (1, c1, s1, c2, s2, c3, s3)
-__device__ __forceinline__ double orb7(const double *C, double c1, double s1, double c2, double s2, double c3, double s3)
-{
-    double r = fma(C[1], c1, C[0]);
-    r = fma(C[2], s1, r);
-    r = fma(C[3], c2, r);
-    r = fma(C[4], s2, r);
-    r = fma(C[5], c3, r);
-    return fma(C[6], s3, r);
-}
-__device__ __forceinline__ double orb5(const double *C, double c1, double s1, double c2, double s2)
-{
-    double r = fma(C[1], c1, C[0]);
-    r = fma(C[2], s1, r);
-    r = fma(C[3], c2, r);
-    return fma(C[4], s2, r);
-}
-
-// One arm 1 -> j of TDI-X at one bin.  mu = k.n, un = u.n, vn = v.n with n = (p_j - p_1)/L.
-//   g = exp(-i a) [ sinc(a) + z sinc(b) ] x,   a = x (1 + mu), b = x (1 - mu), z = exp(-2 i x)
-// (sum of the two one-way links of the arm, PAPER.md:196 Eq. 15, :206 Eq. 17 with N = 0; the common
-// factor -i and the Doppler phase of spacecraft 1 are applied outside).  rho = 1 / ((1+mu)(1-mu)).
-__device__ __forceinline__ void arm_response(double xq, double x, double c2x, double s2x, double Pm, double Qm,
-                                             double rho, double &gr, double &gi)
-{
-    double sa, ca;
-    sincos_qt(xq * Pm, sa, ca);
-    double sb = fma(s2x, ca, -c2x * sa);                 // sin(2x - a) = sin b
-    if (Qm < 9.765625e-4) {                              // b -> 0: the difference formula cancels; series
-        const double b = x * Qm, b2 = b * b;
-        sb = b * fma(b2, fma(b2, 1.0 / 120.0, -1.0 / 6.0), 1.0);
-    }
-    const double sca = sa * Qm * rho;                    // x sinc(a)
-    const double scb = sb * Pm * rho;                    // x sinc(b)
-    const double br = fma(c2x, scb, sca);
-    const double bi = -s2x * scb;
-    gr = fma(ca, br, sa * bi);
-    gi = fma(ca, bi, -sa * br);
-}
-
-// One (particle, bin): a2 phase + t_f, a3 orbit + TDI-X response.  `row` is the bin's table row, c[] the
-// particle's coefficients.  Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1
-// included) and T'_+ , T'_x with  T_P = K_f T'_P,  K_f = -i (1 - z^2)  folded into the table.
+// One (particle, bin) of the direct kernel: model_eval() plus the linear phase term and the carrier.
+// Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1 included), its sine and
+// cosine, and T'_+ , T'_x.
 __device__ __forceinline__ void bin_template(const double2 *__restrict__ row, const double (&c)[kNCoef],
                                              const OrbitCoef &orb, double &psi_out, double &sps, double &cps,
                                              double &tpr, double &tpi, double &tcr, double &tci)
 {
-    const double kx = c[11], ky = c[12], kz = c[13];
-    const double ux = c[14], uy = c[15], uz = c[16];
-    const double vx = c[17], vy = c[18], vz = c[19];
-    const double2 r0 = row[0], r1 = row[1], r2 = row[2], r3 = row[3], r4 = row[4];
-    const double2 d0 = row[5], d1 = row[6], d2 = row[7], d3 = row[8];
-    const double2 zz = row[9], wx = row[11];
-    const double f = r0.x;
-
-    // ---- a2: SPA phase (quarter turns) and orbital phase at t_f  (Eq. A3 :404, Eq. 20 :220)
-    double psi = fma(c[0], f, c[1]);
-    psi = fma(c[2], r0.y, psi);
-    psi = fma(c[3], r1.x, psi);
-    psi = fma(c[4], r1.y, psi);
-    psi = fma(c[5], r2.x, psi);
-    psi = fma(c[6], r2.y, psi);
-    psi = fma(c[7], r3.x, psi);
-    psi = fma(c[8], r3.y, psi);
-    psi = fma(c[9], r4.x, psi);
-    const double xq = r4.y;
-    double alq = fma(c[2], d0.x, c[10]);
-    alq = fma(c[3], d0.y, alq);
-    alq = fma(c[4], d1.x, alq);
-    alq = fma(c[5], d1.y, alq);
-    alq = fma(c[6], d2.x, alq);
-    alq = fma(c[7], d2.y, alq);
-    alq = fma(c[8], d3.x, alq);
-    alq = fma(c[9], d3.y, alq);
-
-    // ---- a3: orbit to O(e^2) at t_f (reading A9), arm geometry
-    double s1, c1;
-    sincos_qt(alq, s1, c1);
-    const double c2 = fma(c1, c1, -s1 * s1), s2 = 2.0 * s1 * c1;
-    const double c3 = fma(c1, c2, -s1 * s2), s3 = fma(s1, c2, c1 * s2);
-    const double p1x = orb7(orb.c[0][0], c1, s1, c2, s2, c3, s3);
-    const double p1y = orb7(orb.c[0][1], c1, s1, c2, s2, c3, s3);
-    const double p1z = orb5(orb.c[0][2], c1, s1, c2, s2);
-    const double n2x = orb7(orb.c[1][0], c1, s1, c2, s2, c3, s3);
-    const double n2y = orb7(orb.c[1][1], c1, s1, c2, s2, c3, s3);
-    const double n2z = orb5(orb.c[1][2], c1, s1, c2, s2);
-    const double n3x = orb7(orb.c[2][0], c1, s1, c2, s2, c3, s3);
-    const double n3y = orb7(orb.c[2][1], c1, s1, c2, s2, c3, s3);
-    const double n3z = orb5(orb.c[2][2], c1, s1, c2, s2);
-    const double kp = fma(kx, p1x, fma(ky, p1y, kz * p1z));        // 4 k.p_1/c
-    const double mu2 = fma(kx, n2x, fma(ky, n2y, kz * n2z));
-    const double mu3 = fma(kx, n3x, fma(ky, n3y, kz * n3z));
-    const double un2 = fma(ux, n2x, fma(uy, n2y, uz * n2z));
-    const double un3 = fma(ux, n3x, fma(uy, n3y, uz * n3z));
-    const double vn2 = fma(vx, n2x, fma(vy, n2y, vz * n2z));
-    const double vn3 = fma(vx, n3x, fma(vy, n3y, vz * n3z));
-
-    // carrier: Psi_0 + Doppler phase of spacecraft 1 (reading A4), exp(+i Psi)
-    psi = fma(f, kp, psi);
+    double psi_nl;
+    model_eval(row, c, orb, psi_nl, tpr, tpi, tcr, tci);
+    const double psi = fma(c[0], row[0].x, psi_nl);                  // + 2 pi f t_c
     sincos_qt(psi, sps, cps);
-
-    // two arms
-    const double P2 = fmax(1.0 + mu2, 1e-30), Q2 = fmax(1.0 - mu2, 1e-30);
-    const double P3 = fmax(1.0 + mu3, 1e-30), Q3 = fmax(1.0 - mu3, 1e-30);
-    const double den2 = P2 * Q2, den3 = P3 * Q3;
-    const double R = rcp_fast(den2 * den3);
-    double g2r, g2i, g3r, g3i;
-    arm_response(xq, wx.y, zz.x, zz.y, P2, Q2, den3 * R, g2r, g2i);
-    arm_response(xq, wx.y, zz.x, zz.y, P3, Q3, den2 * R, g3r, g3i);
-    const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;   // n.e_+.n, n.e_x.n
-    const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
-    // T'_P = xi_P3 g_3 - xi_P2 g_2   (TDI-X: arm 3 minus arm 2, reading A7)
-    tpr = fma(xp3, g3r, -xp2 * g2r);
-    tpi = fma(xp3, g3i, -xp2 * g2i);
-    tcr = fma(xc3, g3r, -xc2 * g2r);
-    tci = fma(xc3, g3i, -xc2 * g2i);
     psi_out = psi;
 }
 
@@ -289,6 +158,8 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
     const int tid = threadIdx.x;
     const int grp = blockIdx.x % a.n_groups;
     const int seg = blockIdx.x / a.n_groups;
+    // CTA-uniform: work items with a level >= 0 belong to the interpolating kernel (fstat_fast.cu)
+    if (a.level != nullptr && a.level[(int64_t)grp * a.n_seg + seg] >= 0) return;
     const int64_t p = (int64_t)grp * kThreads + tid;           // < P_pad by construction
 
     const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];

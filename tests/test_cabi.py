@@ -50,6 +50,9 @@ def test_library_is_sm100a_and_uses_tma_bulk_copy(fs):
     main = sass[sass.index("fstat_main_kernel"):]
     assert "UBLKCP" in main          # cp.async.bulk (TMA 1-D bulk copy) staging of the per-bin table
     assert "DFMA" in main
+    fast = sass[sass.index("fstat_fast_kernel"):]
+    fast = fast[:fast.index("Function :", 10)] if "Function :" in fast[10:] else fast
+    assert "UBLKCP" in fast and "DFMA" in fast and "DADD" in fast
 
 
 def test_default_options(fs):
@@ -57,6 +60,7 @@ def test_default_options(fs):
     assert o.f_ref_e0 == 0.01 and o.arm_length_m == 2.5e9
     assert o.orbit_kappa == 0.0 and o.orbit_lambda == 0.0
     assert o.device == -1 and o.inputs_on_device == 0 and o.max_segment_bins == 0
+    assert o.force_level == -2 and o.interp_tol == 1.0
 
 
 def test_status_strings(fs):
