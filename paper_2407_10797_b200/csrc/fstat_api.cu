@@ -563,7 +563,7 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
 
     CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef, pl->d_valid, st));
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
-                               pl->d_seg_maxlvl, pl->opt.interp_tol * 1e-7 * (2.0 / kPi), pl->opt.interp_tol * 1e-7,
+                               pl->d_seg_maxlvl, pl->opt.interp_tol * 4e-7 * (2.0 / kPi), pl->opt.interp_tol * 4e-7,
                                pl->opt.force_level, pl->d_level, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;

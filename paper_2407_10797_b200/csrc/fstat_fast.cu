@@ -12,9 +12,8 @@
 //     m_PQ = sum_i w'_i T'_P(i) conj(T'_Q(i))      = sum_ab y^P_a G_ab conj(y^Q_b)
 // with c^P_n the Newton (binomial-basis) coefficients of the cubic, y^P_a its four node values and
 // G_ab = sum_i w'_i l_a(i) l_b(i) a plan-time Gram matrix of the Lagrange basis.  Per bin that leaves:
-// the phase by forward differences (exact range reduction in quarter turns), one sincos, one complex
-// product with the folded data and four complex running sums -- about 30 FP64 instructions instead of
-// 265.  S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
+// the carrier by a rotation recurrence on the forward differences of the phase cubic, one complex
+// product with the folded data and four complex running sums -- 24 FP64 instructions instead of 265.  S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
 // work items for which no stride is accurate enough are left to the direct kernel.
 //
 // Inner products: PAPER.md:66 Eq. 4, :89-91 Eq. 8-9, :117 Eq. 12.  Template: :397-405 Eq. A1-A3,
@@ -219,23 +218,6 @@ __device__ __forceinline__ double mulmod4(double c, double f)
     return red4(hi) + lo;
 }
 
-// sin and cos of (pi/2) w for |w| <= 1/2 (near-minimax in w^2; errors 3.4e-12 and 4.8e-11)
-__device__ __forceinline__ void sincos_small(double w, double &ps, double &pc)
-{
-    const double w2 = w * w;
-    double s = 1.582063035564773e-4;
-    s = fma(s, w2, -4.6812662567262455e-3);
-    s = fma(s, w2, 7.9692582725630620e-2);
-    s = fma(s, w2, -0.64596409614679535);
-    s = fma(s, w2, 1.5707963267880999);
-    ps = s * w;
-    double c = 9.036280663802505e-4;
-    c = fma(c, w2, -2.086006950026408e-2);
-    c = fma(c, w2, 0.25366920365511348);
-    c = fma(c, w2, -1.2337005406331622);
-    pc = fma(c, w2, 0.99999999995248942);
-}
-
 // Newton-basis coefficients c_n (basis C(u + n - 1, n), u = j1 - i) of the cubic through the node values
 // y0..y3 at t = -1, 0, 1, 2 (t = s / S), for a sub-block that ends U bins after node 0.
 __device__ __forceinline__ void newton_coefs(double y0, double y1, double y2, double y3, double rS, double U,
@@ -364,34 +346,35 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fast_kernel(const __grid_co
         const double2 *tp = &sm.tile[tl % kFastStages][j0 & (kFastTile - 1)];
         const int nb = j1 - j0;
 
-        // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3
+        // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3.  The carrier e^{+i Phi_i} is carried by
+        // a three-level rotation recurrence (Phi is a cubic in the bin index inside the sub-block):
+        //   E <- E R,  R <- R Q,  Q <- Q C,   R = e^{i D1}, Q = e^{i D2}, C = e^{i D3}  (forward differences)
+        // 12 FP64 instructions per bin and no range reduction; rounding grows like n^2.5 ulp (1e-10 at n = 256)
+        // and is common to u_+ and u_x, so M_k^-1 does not amplify it.
+        double Er, Ei, Rr, Ri, Qr, Qi, Cr, Ci;
+        sincos_qt(t, Ei, Er);
+        sincos_qt(D1, Ri, Rr);
+        sincos_qt(D2, Qi, Qr);
+        sincos_qt(D3, Ci, Cr);
         double A0r = 0.0, A0i = 0.0, A1r = 0.0, A1i = 0.0, A2r = 0.0, A2i = 0.0, A3r = 0.0, A3i = 0.0;
-        int qacc = 0;
-        const double MAGIC = 6755399441055744.0;             // 1.5 * 2^52
 #pragma unroll 2
         for (int b = 0; b < nb; ++b) {
             const double2 d = tp[b];
-            const double tm = t + MAGIC;
-            qacc += __double2loint(tm);
-            const double w = t - (tm - MAGIC);
-            double ps, pc;
-            sincos_small(w, ps, pc);
-            const bool swap = (qacc & 1) != 0;
-            const double ss = swap ? pc : ps;
-            const double cc = swap ? ps : pc;
-            const int sflip = (qacc & 2) << 30;
-            const int cflip = ((qacc + 1) & 2) << 30;
-            const double sn = __hiloint2double(__double2hiint(ss) ^ sflip, __double2loint(ss));
-            const double cs = __hiloint2double(__double2hiint(cc) ^ cflip, __double2loint(cc));
-            const double qr = fma(d.x, cs, -d.y * sn);
-            const double qi = fma(d.x, sn, d.y * cs);
+            const double qr = fma(d.x, Er, -d.y * Ei);
+            const double qi = fma(d.x, Ei, d.y * Er);
             A0r += qr; A0i += qi;
             A1r += A0r; A1i += A0i;
             A2r += A1r; A2i += A1i;
             A3r += A2r; A3i += A2i;
-            t = w + D1;
-            D1 += D2;
-            D2 += D3;
+            const double er = fma(Er, Rr, -Ei * Ri);
+            Ei = fma(Er, Ri, Ei * Rr);
+            Er = er;
+            const double rr = fma(Rr, Qr, -Ri * Qi);
+            Ri = fma(Rr, Qi, Ri * Qr);
+            Rr = rr;
+            const double qq = fma(Qr, Cr, -Qi * Ci);
+            Qi = fma(Qr, Ci, Qi * Cr);
+            Qr = qq;
         }
 
         // ---- z_P += sum_n conj(c^P_n) A_n
