@@ -32,11 +32,20 @@ import synthetic as syn  # noqa: E402
 METRIC = "template_frequency_bins_per_s"
 UNIT = "template-bins/s"
 
-# FP64-pipe instructions the main kernel issues per template-bin (DFMA + DMUL + DADD + DSETP in the
-# SASS of its per-bin loop, counted with cuobjdump -sass; 2 flop each by the
-# usual FMA convention).  Nominal B200 FP64 peak: 148 SM x 64 FMA/clk x 1.965 GHz x 2 = 37.2 TFLOP/s.
-FP64_INST_PER_TEMPLATE_BIN = 265.0
+# FP64-pipe instructions (DFMA + DMUL + DADD + DSETP in the SASS) of the two main kernels, per unit of work
+# (tests/test_cabi.py re-counts them from the built library):
+#   interpolating kernel: per template-bin (inner loop), per node interval of a particle (full-model node
+#   evaluation, interpolation coefficients, Gram products), per work item of a particle (three extra nodes);
+#   direct kernel: per template-bin.  2 flop each by the usual FMA convention.
+FAST_FP64_PER_BIN = 24.0
+FAST_FP64_PER_INTERVAL = 613.0
+FAST_FP64_PER_ITEM = 721.0
+DIRECT_FP64_PER_BIN = 281.0
 NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
+STRIDES = (0, 8, 16, 32, 64, 128, 256)          # index 0 = direct kernel
+# dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from
+# the ncu --set full capture summarised in profiles/ (None until that capture exists for the current kernel)
+NCU_DRAM_BYTES_PER_LAUNCH = None
 
 
 # ------------------------------------------------------------------------------------------ utilities
@@ -243,13 +252,19 @@ def run_ours(args):
     clocks = ClockSampler(local)
     if rank == 0:
         clocks.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
+    # exactly K timed steps; L2 (126 MB) is flushed before each one by a 256 MiB write that is NOT timed:
+    # every step has its own event pair on the launch stream and the step times are summed
+    scratch = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches_before = fs.fstat_plan_launch_count(plan)
+    for e0, e1 in ev:
+        scratch.fill_(1)
+        e0.record(stream)
         fs.fstat_eval_batch(plan, par, F, Fk, stream)
-    e1.record(stream)
+        e1.record(stream)
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    launches_timed = fs.fstat_plan_launch_count(plan) - launches_before      # our kernels inside the timed steps
+    ms_total = float(sum(e0.elapsed_time(e1) for e0, e1 in ev))
     main_ms = fs.fstat_plan_main_kernel_ms(plan, min(args.steps, 128))
     clk = clocks.stop() if rank == 0 else None
     if dist is not None:
@@ -268,13 +283,14 @@ def run_ours(args):
     for _ in range(min(args.warmup, 3)):
         fs.fstat_eval_batch_host(plan, par_pin, F_pin, Fk_pin, stream)
     barrier()
-    h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    h0.record(stream)
-    for _ in range(args.steps):
+    hv = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for h0, h1 in hv:
+        scratch.fill_(2)
+        h0.record(stream)
         fs.fstat_eval_batch_host(plan, par_pin, F_pin, Fk_pin, stream)
-    h1.record(stream)
+        h1.record(stream)
     barrier()
-    ms_e2e = h0.elapsed_time(h1)
+    ms_e2e = float(sum(h0.elapsed_time(h1) for h0, h1 in hv))
     if dist is not None:
         t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -288,24 +304,37 @@ def run_ours(args):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant (main) kernel: FP64 pipe
+    # ---- roofline of the dominant (main) kernels: FP64 pipe
     main_mean = float(np.mean(main_ms)) if len(main_ms) else float("nan")
+    lvl_bins, lvl_sub = fs.fstat_plan_level_bins(plan)           # per particle group: bins / node intervals per stride
+    n_items = fs.fstat_plan_n_ctas(plan, P)
+    fast_share = float(lvl_bins[1:].sum()) / max(float(lvl_bins.sum()), 1.0)
+    fp64_inst = 128.0 * (FAST_FP64_PER_BIN * float(lvl_bins[1:].sum()) + FAST_FP64_PER_INTERVAL * float(lvl_sub.sum())
+                         + FAST_FP64_PER_ITEM * n_items * fast_share + DIRECT_FP64_PER_BIN * float(lvl_bins[0]))
     fp64_rate, n_sm = fs.fstat_probe_pipe_peak(0, 60.0, local)
     fp32_rate, _ = fs.fstat_probe_pipe_peak(1, 30.0, local)
     mufu_rate, _ = fs.fstat_probe_pipe_peak(2, 30.0, local)
-    achieved = FP64_INST_PER_TEMPLATE_BIN * 2.0 * float(P) * ds.n_bins / (main_mean * 1e-3) / 1e12
+    achieved = fp64_inst * 2.0 / (main_mean * 1e-3) / 1e12
     peak = fp64_rate * 2.0 / 1e12
     hbm_peak, hbm_src = peaks()
-    table_bytes = ds.n_bins * 24 * 8
-    roofline = {"bound": "alu", "kernel": "fstat_main_kernel", "pipe": "fp64", "achieved": achieved, "peak": peak,
-                "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None, "traffic": None,
+    n_groups = (P + 127) // 128
+    # algorithmic HBM bytes of one launch: every particle group streams the folded data (16 B/bin) once, reads
+    # one 192-B node row and one 80-B Gram matrix per node interval, and writes 8 partial sums per work item
+    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * float(lvl_sub.sum()) + 64.0 * 128.0 * n_items
+    roofline = {"bound": "alu", "kernel": "fstat_fast_kernel (+ fstat_main_kernel for the work items it leaves)",
+                "pipe": "fp64", "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
                 "peak_source": "dependent-free DFMA stream measured in this run (fstat_probe_pipe_peak), x2 flop",
                 "nominal_peak": NOMINAL_FP64_TFLOPS, "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                "fp64_inst_per_template_bin": FP64_INST_PER_TEMPLATE_BIN, "main_kernel_ms": main_mean,
-                "main_kernel_share_of_step": main_mean / ms_step,
+                "fp64_inst_per_launch": fp64_inst, "fp64_inst_per_template_bin": fp64_inst / (float(P) * ds.n_bins),
+                "fp64_inst_model": {"fast_per_bin": FAST_FP64_PER_BIN, "fast_per_node_interval": FAST_FP64_PER_INTERVAL,
+                                    "fast_per_work_item": FAST_FP64_PER_ITEM, "direct_per_bin": DIRECT_FP64_PER_BIN},
+                "stride_share_of_bins": {str(S): float(b) / max(float(lvl_bins.sum()), 1.0)
+                                         for S, b in zip(STRIDES, lvl_bins)},
+                "main_kernel_ms": main_mean, "main_kernel_share_of_step": main_mean / ms_step,
                 "measured_pipe_peaks_inst_per_s": {"fp64_fma": fp64_rate, "fp32_fma": fp32_rate, "mufu": mufu_rate},
-                "hbm": {"algorithmic_bytes_per_launch": float(table_bytes) * ((P + 127) // 128),
-                        "achieved_gbs": float(table_bytes) * ((P + 127) // 128) / (main_mean * 1e-3) / 1e9,
+                "hbm": {"algorithmic_bytes_per_launch": hbm_bytes,
+                        "achieved_gbs": hbm_bytes / (main_mean * 1e-3) / 1e9,
                         "peak_gbs": hbm_peak, "peak_source": hbm_src}}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -314,8 +343,7 @@ def run_ours(args):
            "config": {"workload": cfg.name, "T_s": cfg.T, "n_bins": ds.n_bins, "n_part": n_part,
                       "particles_per_gpu": P, "parallelism": "particles sharded over %d GPU(s), plan replicated, "
                       "no collective on the data path" % world,
-                      "l2": "inputs larger than L2: per-bin table %.0f MB streamed once per 128-particle group "
-                            "every step (L2 is 126 MB)" % (table_bytes / 1e6),
+                      "l2": "L2 flushed before every timed step (256 MiB scratch write, outside the timed events)",
                       "n_ctas": fs.fstat_plan_n_ctas(plan, P), "n_sm": n_sm,
                       "plan_create_s": t_plan, "dataset_s": t_data},
            "particles_per_s": float(P) * world / (ms_step * 1e-3),
@@ -323,7 +351,7 @@ def run_ours(args):
                    "d2h_bytes_per_step": int(F_pin.numel() * 8 + Fk_pin.numel() * 8),
                    "ms_per_step": ms_e2e / max(args.steps, 1),
                    "call": "fstat_eval_batch_host (pinned host params in; F and F_k out)"},
-           "gpu_launches": int(fs.fstat_launches_per_eval()) * args.steps,
+           "gpu_launches": int(launches_timed),
            "clocks": clk, "roofline": roofline}
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, ds, n_part, args.cpu_sample)

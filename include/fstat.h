@@ -157,9 +157,10 @@ FSTAT_API int32_t fstat_plan_n_part(const fstat_plan *plan);
 FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
 /* Number of (particle-group, segment) work items = CTAs the main kernel launches for P particles. */
 FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
-/* Number of kernels one fstat_eval_batch call launches (prologue, stride selection, interpolating main
- * kernel, direct main kernel, epilogue). */
-FSTAT_API int32_t fstat_launches_per_eval(void);
+/* Number of CUDA kernels the fstat_eval_batch / fstat_eval_batch_host calls on this plan have launched so
+ * far (per call: prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and
+ * the chunk sums of F when the partitions are split over several epilogue blocks). */
+FSTAT_API int64_t fstat_plan_launch_count(const fstat_plan *plan);
 /* How the most recent fstat_eval_batch on this plan was split between the direct kernel and the six
  * strides of the interpolating kernel: bins_out[0] / [1..6] = sum over the (particle group, segment) work
  * items run by the direct kernel / at stride 8, 16, 32, 64, 128, 256 of the segment's bin count (multiply

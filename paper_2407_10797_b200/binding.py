@@ -19,7 +19,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
     "fstat_eval_batch_host", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
-    "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_launches_per_eval",
+    "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
 )
@@ -75,8 +75,8 @@ def load_library():
         L.fstat_plan_device.restype = i32
         L.fstat_plan_n_ctas.argtypes = [vp, i64]
         L.fstat_plan_n_ctas.restype = i64
-        L.fstat_launches_per_eval.argtypes = []
-        L.fstat_launches_per_eval.restype = i32
+        L.fstat_plan_launch_count.argtypes = [vp]
+        L.fstat_plan_launch_count.restype = i64
         L.fstat_plan_level_bins.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.fstat_plan_level_bins.restype = C.c_int
         L.fstat_plan_main_kernel_ms.argtypes = [vp, i32, dp]
@@ -290,8 +290,8 @@ def fstat_plan_n_ctas(plan: Plan, P: int) -> int:
     return int(load_library().fstat_plan_n_ctas(plan.handle, int(P)))
 
 
-def fstat_launches_per_eval() -> int:
-    return int(load_library().fstat_launches_per_eval())
+def fstat_plan_launch_count(plan: Plan) -> int:
+    return int(load_library().fstat_plan_launch_count(plan.handle))
 
 
 def fstat_plan_level_bins(plan: Plan) -> Tuple[np.ndarray, np.ndarray]:

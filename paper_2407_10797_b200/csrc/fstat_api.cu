@@ -45,6 +45,9 @@ struct fstat_plan {
     SegCrit *d_seg_crit = nullptr; size_t crit_cap = 0;    // [n_seg]
     int8_t *d_seg_maxlvl = nullptr; size_t maxlvl_cap = 0; // [n_seg]
     int8_t *d_level = nullptr; size_t level_cap = 0;       // [n_groups][n_seg] of the most recent evaluation
+    int32_t *d_direct = nullptr; size_t direct_cap = 0;    // [1 + n_groups * n_seg]: count, then the work list
+    int64_t n_launches = 0;                                 // kernels launched by evaluations so far
+    double *d_fpart = nullptr; size_t fpart_cap = 0;       // [n_chunk][P_pad] per-chunk sums of F_k (epilogue)
     int32_t last_groups = 0;
     // workspace
     double *d_coef = nullptr;  size_t coef_cap = 0;      // doubles
@@ -412,7 +415,7 @@ static void plan_free(fstat_plan *pl)
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
-    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level);
+    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
@@ -491,7 +494,7 @@ void fstat_plan_destroy(fstat_plan *pl) { plan_free(pl); }
 int64_t fstat_plan_n_bins(const fstat_plan *pl) { return pl ? pl->n_bins : 0; }
 int32_t fstat_plan_n_part(const fstat_plan *pl) { return pl ? pl->n_part : 0; }
 int32_t fstat_plan_device(const fstat_plan *pl) { return pl ? pl->device : -1; }
-int32_t fstat_launches_per_eval(void) { return 5; }
+int64_t fstat_plan_launch_count(const fstat_plan *pl) { return pl ? pl->n_launches : 0; }
 
 int64_t fstat_plan_n_ctas(const fstat_plan *pl, int64_t P)
 {
@@ -559,12 +562,18 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)P_pad));
     CU_TRY(pl, grow(&pl->d_partial, &pl->partial_cap, (size_t)pl->n_seg * kNAcc * (size_t)P_pad));
     CU_TRY(pl, grow(&pl->d_level, &pl->level_cap, (size_t)pl->n_seg * (size_t)n_groups));
+    CU_TRY(pl, grow(&pl->d_direct, &pl->direct_cap, (size_t)pl->n_seg * (size_t)n_groups + 1));
+    {
+        int32_t chunk = 0;
+        const int32_t n_chunk = epilogue_chunks(P, pl->n_part, &chunk);
+        CU_TRY(pl, grow(&pl->d_fpart, &pl->fpart_cap, (size_t)n_chunk * (size_t)P_pad));
+    }
     pl->last_groups = (int32_t)n_groups;
 
     CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef, pl->d_valid, st));
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
                                pl->d_seg_maxlvl, pl->opt.interp_tol * 4e-7 * (2.0 / kPi), pl->opt.interp_tol * 4e-7,
-                               pl->opt.force_level, pl->d_level, st));
+                               pl->opt.force_level, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;
     fa.node = pl->d_node;
@@ -583,7 +592,9 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     a.table = pl->d_table;
     a.coef = pl->d_coef;
     a.seg_edge = pl->d_seg_edge;
-    a.level = pl->d_level;
+    a.direct_list = pl->d_direct + 1;
+    a.direct_count = pl->d_direct;
+    a.max_ctas = pl->n_sm * 12;
     a.partial = pl->d_partial;
     a.P_pad = P_pad;
     a.P = (int32_t)P;
@@ -596,7 +607,12 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, launch_main(a, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;
-    CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, P, P_pad, pl->n_part, F, Fk, st));
+    CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, P, P_pad, pl->n_part, pl->n_seg, pl->d_fpart,
+                               F, Fk, st));
+    {
+        int32_t chunk = 0;      // prologue, stride selection, [interpolating], direct, epilogue, [chunk sums of F]
+        pl->n_launches += 4 + (pl->fast_ok ? 1 : 0) + (epilogue_chunks(P, pl->n_part, &chunk) > 1 ? 1 : 0);
+    }
     return FSTAT_OK;
 }
 

@@ -13,7 +13,8 @@
 // with c^P_n the Newton (binomial-basis) coefficients of the cubic, y^P_a its four node values and
 // G_ab = sum_i w'_i l_a(i) l_b(i) a plan-time Gram matrix of the Lagrange basis.  Per bin that leaves:
 // the carrier by a rotation recurrence on the forward differences of the phase cubic, one complex
-// product with the folded data and four complex running sums -- 24 FP64 instructions instead of 265.  S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
+// product with the folded data and four complex running sums -- 24 FP64 instructions instead of 281.
+// S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
 // work items for which no stride is accurate enough are left to the direct kernel.
 //
 // Inner products: PAPER.md:66 Eq. 4, :89-91 Eq. 8-9, :117 Eq. 12.  Template: :397-405 Eq. A1-A3,
@@ -141,7 +142,9 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
                                                             int32_t n_seg, const SegCrit *__restrict__ crit,
                                                             const int8_t *__restrict__ seg_maxlvl, double tol_phi_qt,
                                                             double tol_resp, int32_t force_level,
-                                                            int8_t *__restrict__ level)
+                                                            int8_t *__restrict__ level,
+                                                            int32_t *__restrict__ direct_list,
+                                                            int32_t *__restrict__ direct_count)
 {
     __shared__ double s3[kThreads / 32], s9[kThreads / 32];
     const int tid = threadIdx.x;
@@ -184,15 +187,20 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
             }
         }
         level[(int64_t)grp * n_seg + seg] = (int8_t)lvl;
+        if (lvl < 0) direct_list[atomicAdd(direct_count, 1)] = grp * n_seg + seg;   // order is irrelevant
     }
 }
 
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
-                            double tol_resp, int32_t force_level, int8_t *level, cudaStream_t st)
+                            double tol_resp, int32_t force_level, int8_t *level, int32_t *direct_list,
+                            int32_t *direct_count, cudaStream_t st)
 {
+    cudaError_t e = cudaMemsetAsync(direct_count, 0, sizeof(int32_t), st);
+    if (e != cudaSuccess) return e;
     schedule_kernel<<<(unsigned)n_groups, kThreads, 0, st>>>(coef, valid, P_pad, n_seg, crit, seg_maxlvl,
-                                                            tol_phi_qt, tol_resp, force_level, level);
+                                                            tol_phi_qt, tol_resp, force_level, level,
+                                                            direct_list, direct_count);
     return cudaGetLastError();
 }
 

@@ -78,7 +78,9 @@ struct MainArgs {
     const double *table;      // [n_bins][kTabW]
     const double *coef;       // [kNCoef][P_pad]
     const int32_t *seg_edge;  // [n_seg + 1]
-    const int8_t *level;      // [n_groups][n_seg] or nullptr; the direct kernel runs the items with level < 0
+    const int32_t *direct_list;   // work items (group * n_seg + segment) left to the direct kernel ...
+    const int32_t *direct_count;  // ... and how many (both written by schedule_kernel)
+    int32_t max_ctas;             // persistent grid size
     double *partial;          // [n_seg][kNAcc][P_pad]
     int64_t P_pad;
     int32_t P;
@@ -118,14 +120,17 @@ cudaError_t launch_build_gram(const double *table, const int32_t *edges, int32_t
                               int level, const int32_t *cnt, double *gram, cudaStream_t st);
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
-                            double tol_resp, int32_t force_level, int8_t *level, cudaStream_t st);
+                            double tol_resp, int32_t force_level, int8_t *level, int32_t *direct_list,
+                            int32_t *direct_count, cudaStream_t st);
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
                             double *coef, int32_t *valid, cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
 cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
-                            int64_t P_pad, int32_t n_part, double *F, double *Fk, cudaStream_t st);
+                            int64_t P_pad, int32_t n_part, int32_t n_seg, double *Fpart, double *F, double *Fk,
+                            cudaStream_t st);
+int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out);
 cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
                             const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st);
 cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaStream_t st);

@@ -150,93 +150,106 @@ __device__ __forceinline__ void bin_template(const double2 *__restrict__ row, co
     psi_out = psi;
 }
 
+// The direct kernel: every bin of a work item evaluated in full.  Persistent CTAs walk the list of work
+// items the stride selection left to it (schedule_kernel: items for which no interpolation stride meets
+// the error bound -- all of config 0, partitions shorter than 8 bins); an empty list costs one read.
 __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_constant__ MainArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     MainSmem &sm = *reinterpret_cast<MainSmem *>(smem_raw);
 
     const int tid = threadIdx.x;
-    const int grp = blockIdx.x % a.n_groups;
-    const int seg = blockIdx.x / a.n_groups;
-    // CTA-uniform: work items with a level >= 0 belong to the interpolating kernel (fstat_fast.cu)
-    if (a.level != nullptr && a.level[(int64_t)grp * a.n_seg + seg] >= 0) return;
-    const int64_t p = (int64_t)grp * kThreads + tid;           // < P_pad by construction
-
-    const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
-    const int n_bins = hi - lo;
-    const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
-    const double *src = a.table + (int64_t)lo * kTabW;
-
+    const int n_items = *a.direct_count;
+    if ((int)blockIdx.x >= n_items) return;
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < kStages; ++s) mbar_init(&sm.full[s], 1);
         mbar_fence_init();
+    }
+    __syncthreads();
+    int g0 = 0;                                          // tiles consumed so far by this CTA (ring position)
+
+    for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+        const int item = a.direct_list[it];
+        const int grp = item / a.n_seg;
+        const int seg = item - grp * a.n_seg;
+        const int64_t p = (int64_t)grp * kThreads + tid;       // < P_pad by construction
+
+        const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
+        const int n_bins = hi - lo;
+        const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
+        const double *src = a.table + (int64_t)lo * kTabW;
+
+        if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) {
-            if (s < n_tiles) {
-                const int nb = min(kTileBins, n_bins - s * kTileBins);
-                const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
-                mbar_expect_tx(&sm.full[s], bytes);
-                tma_load_1d(sm.tile[s], src + (int64_t)s * kTileBins * kTabW, bytes, &sm.full[s]);
+            for (int s = 0; s < kStages; ++s) {
+                if (s < n_tiles) {
+                    const int slot = (g0 + s) % kStages;
+                    const int nb = min(kTileBins, n_bins - s * kTileBins);
+                    const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
+                    mbar_expect_tx(&sm.full[slot], bytes);
+                    tma_load_1d(sm.tile[slot], src + (int64_t)s * kTileBins * kTabW, bytes, &sm.full[slot]);
+                }
             }
         }
-    }
 
-    // per-particle coefficients (a1), coalesced
-    double c[kNCoef];
+        // per-particle coefficients (a1), coalesced
+        double c[kNCoef];
 #pragma unroll
-    for (int j = 0; j < kNCoef; ++j) c[j] = a.coef[(int64_t)j * a.P_pad + p];
-    __syncthreads();
+        for (int j = 0; j < kNCoef; ++j) c[j] = a.coef[(int64_t)j * a.P_pad + p];
 
-    double acc[kNAcc];
+        double acc[kNAcc];
 #pragma unroll
-    for (int j = 0; j < kNAcc; ++j) acc[j] = 0.0;
+        for (int j = 0; j < kNAcc; ++j) acc[j] = 0.0;
 
-    for (int t = 0; t < n_tiles; ++t) {
-        const int slot = t % kStages;
-        mbar_wait(&sm.full[slot], (uint32_t)((t / kStages) & 1));
-        const int nb = min(kTileBins, n_bins - t * kTileBins);
-        const double *tile = sm.tile[slot];
-        double in[kNAcc];
+        for (int t = 0; t < n_tiles; ++t) {
+            const int g = g0 + t;
+            const int slot = g % kStages;
+            mbar_wait(&sm.full[slot], (uint32_t)((g / kStages) & 1));
+            const int nb = min(kTileBins, n_bins - t * kTileBins);
+            const double *tile = sm.tile[slot];
+            double in[kNAcc];
 #pragma unroll
-        for (int j = 0; j < kNAcc; ++j) in[j] = 0.0;
+            for (int j = 0; j < kNAcc; ++j) in[j] = 0.0;
 
 #pragma unroll 1
-        for (int b = 0; b < nb; ++b) {
-            const double2 *row = reinterpret_cast<const double2 *>(tile + b * kTabW);
-            const double2 dwv = row[10];
-            double psi, sps, cps, tpr, tpi, tcr, tci;
-            bin_template(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
+            for (int b = 0; b < nb; ++b) {
+                const double2 *row = reinterpret_cast<const double2 *>(tile + b * kTabW);
+                const double2 dwv = row[10];
+                double psi, sps, cps, tpr, tpi, tcr, tci;
+                bin_template(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
 
-            // ---- a4: inner products (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117)
-            const double qr = fma(dwv.x, cps, -dwv.y * sps);               // dw' exp(+i Psi)
-            const double qi = fma(dwv.x, sps, dwv.y * cps);
-            in[0] = fma(qr, tpr, fma(qi, tpi, in[0]));                      // z_+ += q conj(T'_+)
-            in[1] = fma(qi, tpr, fma(-qr, tpi, in[1]));
-            in[2] = fma(qr, tcr, fma(qi, tci, in[2]));                      // z_x
-            in[3] = fma(qi, tcr, fma(-qr, tci, in[3]));
-            const double w = row[11].x;
-            in[4] = fma(w, fma(tpr, tpr, tpi * tpi), in[4]);                // m_pp
-            in[5] = fma(w, fma(tcr, tcr, tci * tci), in[5]);                // m_cc
-            in[6] = fma(w, fma(tpr, tcr, tpi * tci), in[6]);                // m_pc = sum w T'_+ conj(T'_x)
-            in[7] = fma(w, fma(tpi, tcr, -tpr * tci), in[7]);
-        }
+                // ---- a4: inner products (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117)
+                const double qr = fma(dwv.x, cps, -dwv.y * sps);               // dw' exp(+i Psi)
+                const double qi = fma(dwv.x, sps, dwv.y * cps);
+                in[0] = fma(qr, tpr, fma(qi, tpi, in[0]));                      // z_+ += q conj(T'_+)
+                in[1] = fma(qi, tpr, fma(-qr, tpi, in[1]));
+                in[2] = fma(qr, tcr, fma(qi, tci, in[2]));                      // z_x
+                in[3] = fma(qi, tcr, fma(-qr, tci, in[3]));
+                const double w = row[11].x;
+                in[4] = fma(w, fma(tpr, tpr, tpi * tpi), in[4]);                // m_pp
+                in[5] = fma(w, fma(tcr, tcr, tci * tci), in[5]);                // m_cc
+                in[6] = fma(w, fma(tpr, tcr, tpi * tci), in[6]);                // m_pc = sum w T'_+ conj(T'_x)
+                in[7] = fma(w, fma(tpi, tcr, -tpr * tci), in[7]);
+            }
 #pragma unroll
-        for (int j = 0; j < kNAcc; ++j) acc[j] += in[j];
+            for (int j = 0; j < kNAcc; ++j) acc[j] += in[j];
 
-        __syncthreads();                                 // every thread is done with this slot
-        if (tid == 0 && t + kStages < n_tiles) {
-            const int tn = t + kStages;
-            const int nbn = min(kTileBins, n_bins - tn * kTileBins);
-            const uint32_t bytes = (uint32_t)nbn * kTabW * sizeof(double);
-            mbar_expect_tx(&sm.full[slot], bytes);
-            tma_load_1d(sm.tile[slot], src + (int64_t)tn * kTileBins * kTabW, bytes, &sm.full[slot]);
+            __syncthreads();                             // every thread is done with this slot
+            if (tid == 0 && t + kStages < n_tiles) {
+                const int tn = t + kStages;
+                const int nbn = min(kTileBins, n_bins - tn * kTileBins);
+                const uint32_t bytes = (uint32_t)nbn * kTabW * sizeof(double);
+                mbar_expect_tx(&sm.full[slot], bytes);
+                tma_load_1d(sm.tile[slot], src + (int64_t)tn * kTileBins * kTabW, bytes, &sm.full[slot]);
+            }
         }
+        g0 += n_tiles;
+
+        double *out = a.partial + ((int64_t)seg * kNAcc) * a.P_pad + p;
+#pragma unroll
+        for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
     }
-
-    double *out = a.partial + ((int64_t)seg * kNAcc) * a.P_pad + p;
-#pragma unroll
-    for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
 }
 
 cudaError_t main_kernel_configure()
@@ -247,7 +260,8 @@ cudaError_t main_kernel_configure()
 
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st)
 {
-    const int64_t n_cta = (int64_t)a.n_groups * a.n_seg;
+    int64_t n_cta = (int64_t)a.n_groups * a.n_seg;
+    if (n_cta > a.max_ctas) n_cta = a.max_ctas;
     fstat_main_kernel<<<(unsigned)n_cta, kThreads, sizeof(MainSmem), st>>>(a);
     return cudaGetLastError();
 }
@@ -294,56 +308,102 @@ cudaError_t launch_template(const double *table, const double *coef, int64_t P_p
 // PAPER.md:85 Eq. 7 is the real embedding of this 2x2 Hermitian one).  Evaluated
 // by Gram-Schmidt: 2 F_k = |z_+|^2/m_pp + |z_x - (m_pc/m_pp) z_+|^2 / (m_cc - |m_pc|^2/m_pp).
 // Rank-deficient G (reading A15): only the non-degenerate direction(s) contribute.
-// Block = 32 particles (x) by 8 partition lanes (y); partition index k = y, y + 8, ...
+// Grid = particle tiles (x) by partition chunks (y); block = 32 particles (x) by 8 lanes (y).
+//   SEG_PAR = false (many partitions, ~1 segment each): lane y owns partitions y, y + 8, ... of the chunk;
+//   SEG_PAR = true  (few partitions, many segments each): the 8 lanes split the segments of one partition
+//                   and are combined through shared memory in a fixed order.
+// Every sum has a fixed order, so F and F_k are bit-reproducible.  F = sum_k F_k (Eq. 11 :110, reading
+// A12) is written directly when there is one chunk, else as per-chunk sums that fsum_kernel adds up.
 // =================================================================================================
 constexpr int kEpiX = 32, kEpiY = 8;
 
+__device__ __forceinline__ double two_F(const double (&v)[kNAcc])
+{
+    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
+    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
+    double twoF = 0.0;
+    if (mpp > 0.0) {
+        const double inv = 1.0 / mpp;
+        twoF = (zpr * zpr + zpi * zpi) * inv;
+        const double cr = mr * inv, ci = mi * inv;                      // m_pc / m_pp
+        const double schur = mcc - (mr * mr + mi * mi) * inv;
+        if (schur > 1e-13 * mcc) {
+            const double yr = zcr - (cr * zpr - ci * zpi);
+            const double yi = zci - (cr * zpi + ci * zpr);
+            twoF += (yr * yr + yi * yi) / schur;
+        }
+    } else if (mcc > 0.0) {
+        twoF = (zcr * zcr + zci * zci) / mcc;
+    }
+    return twoF;
+}
+
+template <bool SEG_PAR>
 __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__restrict__ partial,
                                                                const int32_t *__restrict__ part_seg,
                                                                const int32_t *__restrict__ valid, int64_t P,
-                                                               int64_t P_pad, int32_t n_part,
-                                                               double *__restrict__ F, double *__restrict__ Fk)
+                                                               int64_t P_pad, int32_t n_part, int32_t chunk,
+                                                               double *__restrict__ Fout, double *__restrict__ Fk)
 {
     __shared__ double sF[kEpiY][kEpiX];
     __shared__ double sT[kEpiY][kEpiX + 1];
+    __shared__ double sV[SEG_PAR ? kEpiY : 1][kNAcc][kEpiX];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int64_t p0 = (int64_t)blockIdx.x * kEpiX;
     const int64_t p = p0 + tx;
     const bool live = p < P;
     const bool ok = live && valid[p] != 0;
     const double ninf = -INFINITY;
+    const int k_lo = blockIdx.y * chunk, k_hi = min(n_part, k_lo + chunk);
     double fsum = 0.0;
-    for (int k0 = 0; k0 < n_part; k0 += kEpiY) {
-        const int k = k0 + ty;
+    for (int k0 = k_lo; k0 < k_hi; k0 += kEpiY) {
         double fk = 0.0;
-        if (k < n_part && live) {
-            const int s0 = part_seg[k], s1 = part_seg[k + 1];
-            double v[kNAcc];
+        if (!SEG_PAR) {
+            const int k = k0 + ty;
+            if (k < k_hi && live) {
+                const int s0 = part_seg[k], s1 = part_seg[k + 1];
+                double v[kNAcc];
 #pragma unroll
-            for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
-            for (int s = s0; s < s1; ++s) {
-                const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
+                for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
+                for (int s = s0; s < s1; ++s) {
+                    const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
 #pragma unroll
-                for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
-            }
-            const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
-            const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
-            double twoF = 0.0;
-            if (mpp > 0.0) {
-                const double inv = 1.0 / mpp;
-                twoF = (zpr * zpr + zpi * zpi) * inv;
-                const double cr = mr * inv, ci = mi * inv;                      // m_pc / m_pp
-                const double schur = mcc - (mr * mr + mi * mi) * inv;
-                if (schur > 1e-13 * mcc) {
-                    const double yr = zcr - (cr * zpr - ci * zpi);
-                    const double yi = zci - (cr * zpi + ci * zpr);
-                    twoF += (yr * yr + yi * yi) / schur;
+                    for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
                 }
-            } else if (mcc > 0.0) {
-                twoF = (zcr * zcr + zci * zci) / mcc;
+                fk = ok ? 0.5 * two_F(v) : ninf;
+                if (ok) fsum += fk;
             }
-            fk = ok ? 0.5 * twoF : ninf;
-            if (ok) fsum += fk;
+        } else {
+            // partitions k0 .. k0+7 one after the other; lane ty sums segments s0 + ty, s0 + ty + 8, ...
+            for (int kk = 0; kk < kEpiY && k0 + kk < k_hi; ++kk) {
+                const int s0 = part_seg[k0 + kk], s1 = part_seg[k0 + kk + 1];
+                double v[kNAcc];
+#pragma unroll
+                for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
+                if (live)
+                    for (int s = s0 + ty; s < s1; s += kEpiY) {
+                        const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
+#pragma unroll
+                        for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
+                    }
+#pragma unroll
+                for (int j = 0; j < kNAcc; ++j) sV[SEG_PAR ? ty : 0][j][tx] = v[j];
+                __syncthreads();
+                if (ty == kk) {                           // lane kk finishes partition k0 + kk
+#pragma unroll
+                    for (int j = 0; j < kNAcc; ++j) {
+                        double a = 0.0;
+#pragma unroll
+                        for (int y = 0; y < kEpiY; ++y) a += sV[SEG_PAR ? y : 0][j][tx];
+                        v[j] = a;
+                    }
+                    if (live) {
+                        fk = ok ? 0.5 * two_F(v) : ninf;
+                        if (ok) fsum += fk;
+                    }
+                }
+                __syncthreads();
+            }
         }
         if (Fk != nullptr) {                              // transpose through shared memory: coalesced rows
             sT[ty][tx] = fk;
@@ -351,7 +411,7 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
             // 256 threads write a 32 (particles) x 8 (partitions) tile: thread -> (particle = id / 8, k = id % 8)
             const int id = ty * kEpiX + tx;
             const int pp = id / kEpiY, kk = id % kEpiY;
-            if (p0 + pp < P && k0 + kk < n_part) Fk[(p0 + pp) * (int64_t)n_part + k0 + kk] = sT[kk][pp];
+            if (p0 + pp < P && k0 + kk < k_hi) Fk[(p0 + pp) * (int64_t)n_part + k0 + kk] = sT[kk][pp];
             __syncthreads();
         }
     }
@@ -361,16 +421,51 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
         double s = 0.0;
 #pragma unroll
         for (int y = 0; y < kEpiY; ++y) s += sF[y][tx];
-        F[p] = ok ? s : ninf;
+        if (gridDim.y == 1) Fout[p] = ok ? s : ninf;                        // F itself
+        else Fout[(int64_t)blockIdx.y * P_pad + p] = s;                      // chunk sum, see fsum_kernel
     }
 }
 
-cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
-                            int64_t P_pad, int32_t n_part, double *F, double *Fk, cudaStream_t st)
+__global__ void fsum_kernel(const double *__restrict__ Fpart, const int32_t *__restrict__ valid, int64_t P,
+                            int64_t P_pad, int32_t n_chunk, double *__restrict__ F)
 {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    double s = 0.0;
+    for (int c = 0; c < n_chunk; ++c) s += Fpart[(int64_t)c * P_pad + p];
+    F[p] = valid[p] != 0 ? s : -INFINITY;
+}
+
+int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out)
+{
+    // enough blocks to fill the machine: particle tiles x partition chunks >= ~4 per SM; chunks of >= 8
+    const int64_t tiles = (P + kEpiX - 1) / kEpiX;
+    int64_t want = (4 * 148 + tiles - 1) / tiles;
+    int64_t max_chunks = (n_part + kEpiY - 1) / kEpiY;
+    if (want > max_chunks) want = max_chunks;
+    if (want < 1) want = 1;
+    int32_t chunk = (int32_t)((n_part + want - 1) / want);
+    chunk = ((chunk + kEpiY - 1) / kEpiY) * kEpiY;
+    *chunk_out = chunk;
+    return (n_part + chunk - 1) / chunk;
+}
+
+cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
+                            int64_t P_pad, int32_t n_part, int32_t n_seg, double *Fpart, double *F, double *Fk,
+                            cudaStream_t st)
+{
+    int32_t chunk = 0;
+    const int32_t n_chunk = epilogue_chunks(P, n_part, &chunk);
     const dim3 blk(kEpiX, kEpiY);
-    const unsigned nb = (unsigned)((P + kEpiX - 1) / kEpiX);
-    epilogue_kernel<<<nb, blk, 0, st>>>(partial, part_seg, valid, P, P_pad, n_part, F, Fk);
+    const dim3 grd((unsigned)((P + kEpiX - 1) / kEpiX), (unsigned)n_chunk);
+    double *out = (n_chunk == 1) ? F : Fpart;
+    if (n_seg >= 4 * n_part)
+        epilogue_kernel<true><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, P_pad, n_part, chunk, out, Fk);
+    else
+        epilogue_kernel<false><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, P_pad, n_part, chunk, out, Fk);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess || n_chunk == 1) return e;
+    fsum_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(Fpart, valid, P, P_pad, n_chunk, F);
     return cudaGetLastError();
 }
 
