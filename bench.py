@@ -37,10 +37,10 @@ UNIT = "template-bins/s"
 #   interpolating kernel: per template-bin (inner loop), per node interval of a particle (full-model node
 #   evaluation, interpolation coefficients, Gram products), per work item of a particle (three extra nodes);
 #   direct kernel: per template-bin.  2 flop each by the usual FMA convention.
-FAST_FP64_PER_BIN = 24.0
-FAST_FP64_PER_INTERVAL = 613.0
-FAST_FP64_PER_ITEM = 721.0
-DIRECT_FP64_PER_BIN = 281.0
+FAST_FP64_PER_BIN = 22.0
+FAST_FP64_PER_INTERVAL = 577.0
+FAST_FP64_PER_ITEM = 668.0
+DIRECT_FP64_PER_BIN = 263.0
 NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
 STRIDES = (0, 8, 16, 32, 64, 128, 256)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from

@@ -181,7 +181,7 @@ SegCrit make_seg_crit(double f_lo, double f_hi, double df, double part_len)
     const double r = f_hi / 0.01;
     q.ct = 0.15 * (r > 1.0 ? r * r : 1.0);
     q.kl = 0.05 * part_len;
-    q.pad = 0.0;
+    q.d2 = 1.3 * 4.0 * df / Om;                        // d^2 Psi_q / dk^2 = 4 df dt_f/dk, dt_f/dk = omega / Omega
     return q;
 }
 

@@ -48,7 +48,17 @@ __device__ __forceinline__ void sincos_qt(double t, double &s, double &c)
     c = __hiloint2double(__double2hiint(cc) ^ cflip, __double2loint(cc));
 }
 
-// 1/x for a positive, normal x: hardware seed (MUFU.RCP64H, about 2^-20) and one cubic Newton step
+// sincos of (pi/2) t for |t| < 1/64 (the second and third phase differences of the interpolating kernel;
+// the stride selection sends work items with larger differences to the direct kernel): Taylor series
+// through x^9 / x^8, error < 1e-18.
+__device__ __forceinline__ void sincos_qt_small(double t, double &s, double &c)
+{
+    const double x = 1.570796326794896619231322 * t, x2 = x * x;
+    s = x * fma(x2, fma(x2, fma(x2, fma(x2, 1.0 / 362880.0, -1.0 / 5040.0), 1.0 / 120.0), -1.0 / 6.0), 1.0);
+    c = fma(x2, fma(x2, fma(x2, fma(x2, 1.0 / 40320.0, -1.0 / 720.0), 1.0 / 24.0), -0.5), 1.0);
+}
+
+// 1/x for a normal x of either sign: hardware seed (MUFU.RCP64H, about 2^-20) and one cubic Newton step
 // r <- r + r (e + e^2), e = 1 - x r, which leaves a relative error near 2^-60.
 __device__ __forceinline__ double rcp_fast(double x)
 {

@@ -13,7 +13,7 @@
 // with c^P_n the Newton (binomial-basis) coefficients of the cubic, y^P_a its four node values and
 // G_ab = sum_i w'_i l_a(i) l_b(i) a plan-time Gram matrix of the Lagrange basis.  Per bin that leaves:
 // the carrier by a rotation recurrence on the forward differences of the phase cubic, one complex
-// product with the folded data and four complex running sums -- 24 FP64 instructions instead of 281.
+// product with the folded data and four complex running sums -- 22 FP64 instructions instead of 281.
 // S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
 // work items for which no stride is accurate enough are left to the direct kernel.
 //
@@ -169,11 +169,13 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
     for (int seg = tid; seg < n_seg; seg += kThreads) {
         const int mx = seg_maxlvl[seg];
         int lvl;
-        if (force_level >= -1) {
+        const SegCrit q = crit[seg];
+        const double om = fma(c3, q.p1, c9 * q.p2);
+        if (!(q.d2 * om < 0.015625)) {
+            lvl = -1;                                    // phase differences too large for the small-angle series
+        } else if (force_level >= -1) {
             lvl = force_level < mx ? force_level : mx;
         } else {
-            const SegCrit q = crit[seg];
-            const double om = fma(c3, q.p1, c9 * q.p2);
             const double om2 = om * om, om4 = om2 * om2;
             const double ephi1 = fma(c3, q.q1, fma(c9, q.q2, q.ad * om4));   // per S^4
             // the response error is seen through M_k^-1: a partition over which the response barely changes
@@ -357,20 +359,19 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fast_kernel(const __grid_co
         // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3.  The carrier e^{+i Phi_i} is carried by
         // a three-level rotation recurrence (Phi is a cubic in the bin index inside the sub-block):
         //   E <- E R,  R <- R Q,  Q <- Q C,   R = e^{i D1}, Q = e^{i D2}, C = e^{i D3}  (forward differences)
-        // 12 FP64 instructions per bin and no range reduction; rounding grows like n^2.5 ulp (1e-10 at n = 256)
+        // 12 FP64 instructions per bin (22 with the running sums) and no range reduction; rounding grows like n^2.5 ulp (1e-10 at n = 256)
         // and is common to u_+ and u_x, so M_k^-1 does not amplify it.
         double Er, Ei, Rr, Ri, Qr, Qi, Cr, Ci;
         sincos_qt(t, Ei, Er);
         sincos_qt(D1, Ri, Rr);
-        sincos_qt(D2, Qi, Qr);
-        sincos_qt(D3, Ci, Cr);
+        sincos_qt_small(D2, Qi, Qr);
+        sincos_qt_small(D3, Ci, Cr);
         double A0r = 0.0, A0i = 0.0, A1r = 0.0, A1i = 0.0, A2r = 0.0, A2i = 0.0, A3r = 0.0, A3i = 0.0;
 #pragma unroll 2
         for (int b = 0; b < nb; ++b) {
             const double2 d = tp[b];
-            const double qr = fma(d.x, Er, -d.y * Ei);
-            const double qi = fma(d.x, Ei, d.y * Er);
-            A0r += qr; A0i += qi;
+            A0r = fma(d.x, Er, fma(-d.y, Ei, A0r));       // A_0 += q,  q = dw' E (never formed)
+            A0i = fma(d.x, Ei, fma(d.y, Er, A0i));
             A1r += A0r; A1i += A0i;
             A2r += A1r; A2i += A1i;
             A3r += A2r; A3i += A2i;

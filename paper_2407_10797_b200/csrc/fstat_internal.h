@@ -71,7 +71,7 @@ struct SegCrit {
     double ad;       // (3/128) x Doppler phase amplitude                 [quarter turns]
     double ct;       // response: relative error = ct (omega S)^4
     double kl;       // 0.05 x partition length [bins]: sqrt(normalised det M_k) >~ min(1, kl omega)  (hazard H3)
-    double pad;
+    double d2;       // second phase difference [quarter turns / bin^2] = d2 * omega; must stay below 1/64
 };
 
 struct MainArgs {

@@ -25,31 +25,30 @@ __device__ __forceinline__ double orb5(const double *C, double c1, double s1, do
     return fma(C[4], s2, r);
 }
 
-// x sinc(x P) = sin(x P) / P for |P| below kArmSeries, by its series (P may be slightly NEGATIVE: the arm
-// vector n = (p_j - p_1)/L uses the nominal L, reading A10, so |k.n| reaches 1.0024 for a source along
-// a breathing arm, i.e. P >= -0.0024: below the threshold, so every P that is divided by is positive).
-// (x P)^8 / 9! < 1e-21 for x <= 2.6 (100 mHz).
-constexpr double kArmSeries = 3.90625e-3;    // 2^-8
-__device__ __forceinline__ double xsinc_series(double x, double P)
-{
-    const double a = x * P, a2 = a * a;
-    return x * fma(a2, fma(a2, fma(a2, -1.0 / 5040.0, 1.0 / 120.0), -1.0 / 6.0), 1.0);
-}
-__device__ __forceinline__ double arm_safe(double P) { return fabs(P) < kArmSeries ? 1.0 : P; }
+// 1 + k.n and 1 - k.n are divided by; an exact zero (the only value too small: they are sums with 1) is
+// replaced by 2^-60, for which sin(x P) / P = x to rounding.  They may be slightly NEGATIVE: the arm vector
+// n = (p_j - p_1)/L uses the nominal L (reading A10), so |k.n| reaches 1.0024 for a source along a breathing
+// arm; sin(x P) / P is even in P, nothing special happens there.
+__device__ __forceinline__ double arm_nonzero(double P) { return P == 0.0 ? 0x1p-60 : P; }
 
-// One arm 1 -> j of TDI-X at one frequency.  mu = k.n, with n = (p_j - p_1)/L; Pm = 1 + mu, Qm = 1 - mu;
-// Ps, Qs = arm_safe(Pm), arm_safe(Qm); rho = 1 / (Ps Qs).
+// One arm 1 -> j of TDI-X at one frequency.  mu = k.n, with n = (p_j - p_1)/L; Pm = 1 + mu, Qm = 1 - mu
+// (both non-zero), rho = 1 / (Pm Qm).
 //   g = exp(-i a) [ sinc(a) + z sinc(b) ] x,   a = x (1 + mu), b = x (1 - mu), z = exp(-2 i x)
 // (sum of the two one-way links of the arm, PAPER.md:196 Eq. 15, :206 Eq. 17 with N = 0; the common
-// factor -i and the Doppler phase of spacecraft 1 are applied outside).
-__device__ __forceinline__ void arm_response(double xq, double x, double c2x, double s2x, double Pm, double Qm,
-                                             double Ps, double Qs, double rho, double &gr, double &gi)
+// factor -i and the Doppler phase of spacecraft 1 are applied outside).  Of the two angles a + b = 2x the
+// SMALLER one gets the direct sincos (its sine is divided by the small 1 +- mu and must be relatively
+// accurate); the other follows from the angle-difference formulas.  Branch-free.
+__device__ __forceinline__ void arm_response(double xq, double c2x, double s2x, double Pm, double Qm,
+                                             double rho, double &gr, double &gi)
 {
-    double sa, ca;
-    sincos_qt(xq * Pm, sa, ca);
-    const double sb = fma(s2x, ca, -c2x * sa);           // sin(2x - a) = sin b
-    const double sca = (Ps != Pm) ? xsinc_series(x, Pm) : sa * Qs * rho;     // x sinc(a) = sin(a) / (1 + mu)
-    const double scb = (Qs != Qm) ? xsinc_series(x, Qm) : sb * Ps * rho;     // x sinc(b) = sin(b) / (1 - mu)
+    const bool a_direct = fabs(Pm) <= fabs(Qm);
+    double sd, cd;
+    sincos_qt(xq * (a_direct ? Pm : Qm), sd, cd);
+    const double so = fma(s2x, cd, -c2x * sd);           // sin(2x - d)
+    const double co = fma(c2x, cd, s2x * sd);            // cos(2x - d)
+    const double sa = a_direct ? sd : so, ca = a_direct ? cd : co, sb = a_direct ? so : sd;
+    const double sca = sa * Qm * rho;                    // x sinc(a) = sin(a) / (1 + mu)
+    const double scb = sb * Pm * rho;                    // x sinc(b) = sin(b) / (1 - mu)
     const double br = fma(c2x, scb, sca);
     const double bi = -s2x * scb;
     gr = fma(ca, br, sa * bi);
@@ -69,7 +68,7 @@ __device__ __forceinline__ void model_eval(const double2 *__restrict__ row, cons
     const double vx = c[17], vy = c[18], vz = c[19];
     const double2 r0 = row[0], r1 = row[1], r2 = row[2], r3 = row[3], r4 = row[4];
     const double2 d0 = row[5], d1 = row[6], d2 = row[7], d3 = row[8];
-    const double2 zz = row[9], wx = row[11];
+    const double2 zz = row[9];
     const double f = r0.x;
 
     // ---- a2: SPA phase (quarter turns) and orbital phase at t_f  (Eq. A3 :404, Eq. 20 :220)
@@ -116,13 +115,13 @@ __device__ __forceinline__ void model_eval(const double2 *__restrict__ row, cons
     psi_nl = fma(f, kp, psi);                                       // + Doppler phase of spacecraft 1
 
     // two arms
-    const double P2 = 1.0 + mu2, Q2 = 1.0 - mu2, P3 = 1.0 + mu3, Q3 = 1.0 - mu3;
-    const double P2s = arm_safe(P2), Q2s = arm_safe(Q2), P3s = arm_safe(P3), Q3s = arm_safe(Q3);
-    const double den2 = P2s * Q2s, den3 = P3s * Q3s;     // > 0: |mu| < 1.003, so at most one factor per arm is small
+    const double P2 = arm_nonzero(1.0 + mu2), Q2 = arm_nonzero(1.0 - mu2);
+    const double P3 = arm_nonzero(1.0 + mu3), Q3 = arm_nonzero(1.0 - mu3);
+    const double den2 = P2 * Q2, den3 = P3 * Q3;         // either sign (|mu| may exceed 1 by 0.0024), never 0
     const double R = rcp_fast(den2 * den3);
     double g2r, g2i, g3r, g3i;
-    arm_response(xq, wx.y, zz.x, zz.y, P2, Q2, P2s, Q2s, den3 * R, g2r, g2i);
-    arm_response(xq, wx.y, zz.x, zz.y, P3, Q3, P3s, Q3s, den2 * R, g3r, g3i);
+    arm_response(xq, zz.x, zz.y, P2, Q2, den3 * R, g2r, g2i);
+    arm_response(xq, zz.x, zz.y, P3, Q3, den2 * R, g3r, g3i);
     const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;   // n.e_+.n, n.e_x.n
     const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
     // T'_P = xi_P3 g_3 - xi_P2 g_2   (TDI-X: arm 3 minus arm 2, reading A7)
