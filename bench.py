@@ -32,14 +32,16 @@ import synthetic as syn  # noqa: E402
 METRIC = "template_frequency_bins_per_s"
 UNIT = "template-bins/s"
 
-# FP64-pipe instructions (DFMA + DMUL + DADD + DSETP in the SASS) of the two main kernels, per unit of work
-# (tests/test_cabi.py re-counts them from the built library):
+# FP64-pipe instructions (DFMA + DMUL + DADD + DSETP) of the two main kernels, per unit of work (DESIGN.md
+# "Roofline").  Per template-bin: SASS count of the per-bin loops, re-counted by tests/test_cabi.py.  Per node
+# interval and per work item: EXECUTED counts measured with ncu (sm__inst_executed_pipe_fp64.sum at forced
+# strides 8 / 256 and two segment lengths, profiles/r1_v2.md: 19 / 570 / 667 reproduce all three totals exactly).
 #   interpolating kernel: per template-bin (inner loop), per node interval of a particle (full-model node
 #   evaluation, interpolation coefficients, Gram products), per work item of a particle (three extra nodes);
 #   direct kernel: per template-bin.  2 flop each by the usual FMA convention.
-FAST_FP64_PER_BIN = 22.0
-FAST_FP64_PER_INTERVAL = 577.0
-FAST_FP64_PER_ITEM = 668.0
+FAST_FP64_PER_BIN = 19.0
+FAST_FP64_PER_INTERVAL = 570.0
+FAST_FP64_PER_ITEM = 667.0
 DIRECT_FP64_PER_BIN = 263.0
 NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
 STRIDES = (0, 8, 16, 32, 64, 128, 256)          # index 0 = direct kernel
@@ -50,7 +52,7 @@ NCU_DRAM_BYTES_PER_LAUNCH = None
 
 # ------------------------------------------------------------------------------------------ utilities
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -61,7 +63,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._read, daemon=True)
             self.thr.start()

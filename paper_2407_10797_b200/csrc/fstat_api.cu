@@ -178,6 +178,8 @@ SegCrit make_seg_crit(double f_lo, double f_hi, double df, double part_len)
     q.q1 = (3.0 / 128.0) * (6160.0 / 81.0) * pow(f_lo, -17.0 / 3.0) * df4;
     q.q2 = (3.0 / 128.0) * (4637464.0 / 6561.0) * pow(f_lo, -70.0 / 9.0) * df4;
     q.ad = (3.0 / 128.0) * 4.0 * f_hi * 1.01 * kAU / kC;
+    q.r1 = (440.0 / 27.0) * pow(f_lo, -14.0 / 3.0) * df * df * df;
+    q.r2 = (76024.0 / 729.0) * pow(f_lo, -61.0 / 9.0) * df * df * df;
     const double r = f_hi / 0.01;
     q.ct = 0.15 * (r > 1.0 ? r * r : 1.0);
     q.kl = 0.05 * part_len;

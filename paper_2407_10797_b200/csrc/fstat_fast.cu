@@ -13,7 +13,7 @@
 // with c^P_n the Newton (binomial-basis) coefficients of the cubic, y^P_a its four node values and
 // G_ab = sum_i w'_i l_a(i) l_b(i) a plan-time Gram matrix of the Lagrange basis.  Per bin that leaves:
 // the carrier by a rotation recurrence on the forward differences of the phase cubic, one complex
-// product with the folded data and four complex running sums -- 22 FP64 instructions instead of 281.
+// product with the folded data and four complex running sums -- 19 FP64 instructions instead of 263.
 // S is chosen per (particle group, segment) from an a-priori error bound (schedule_kernel);
 // work items for which no stride is accurate enough are left to the direct kernel.
 //
@@ -171,8 +171,9 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
         int lvl;
         const SegCrit q = crit[seg];
         const double om = fma(c3, q.p1, c9 * q.p2);
-        if (!(q.d2 * om < 0.015625)) {
-            lvl = -1;                                    // phase differences too large for the small-angle series
+        const double d3 = fma(c3, q.r1, fma(c9, q.r2, q.ad * (128.0 / 3.0) * om * om * om));   // |D3|, quarter turns
+        if (!(q.d2 * om < 0.015625) || !(1.25 * d3 <= 0.25 * tol_phi_qt)) {
+            lvl = -1;       // phase differences too large for the small-angle series / the 4-bin hold of D2
         } else if (force_level >= -1) {
             lvl = force_level < mx ? force_level : mx;
         } else {
@@ -356,35 +357,50 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fast_kernel(const __grid_co
         const double2 *tp = &sm.tile[tl % kFastStages][j0 & (kFastTile - 1)];
         const int nb = j1 - j0;
 
-        // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3.  The carrier e^{+i Phi_i} is carried by
-        // a three-level rotation recurrence (Phi is a cubic in the bin index inside the sub-block):
-        //   E <- E R,  R <- R Q,  Q <- Q C,   R = e^{i D1}, Q = e^{i D2}, C = e^{i D3}  (forward differences)
-        // 12 FP64 instructions per bin (22 with the running sums) and no range reduction; rounding grows like n^2.5 ulp (1e-10 at n = 256)
-        // and is common to u_+ and u_x, so M_k^-1 does not amplify it.
+        // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3.  The carrier e^{+i Phi_i} is carried by a
+        // rotation recurrence on the forward differences D1, D2, D3 of the phase cubic:
+        //   E <- E R,  R <- R Q  every bin;   Q <- Q C^4  every 4 bins   (R = e^{i D1}, Q = e^{i D2}, C = e^{i D3}).
+        // Holding D2 at its mid-run value for 4 bins keeps D1 and the phase exact at the run ends; the D1
+        // offset -5/4 D3 centres what is left inside a run: |phase error| <= 1.25 D3, and the stride selection
+        // admits only work items with 1.25 D3 below a quarter of the phase tolerance.  19 FP64 instructions
+        // per bin, no range reduction; rounding grows like n^2.5 ulp (1e-10 at n = 256) and, like every carrier
+        // error, is common to u_+ and u_x, so M_k^-1 does not amplify it.
         double Er, Ei, Rr, Ri, Qr, Qi, Cr, Ci;
         sincos_qt(t, Ei, Er);
-        sincos_qt(D1, Ri, Rr);
-        sincos_qt_small(D2, Qi, Qr);
-        sincos_qt_small(D3, Ci, Cr);
+        sincos_qt(fma(-1.25, D3, D1), Ri, Rr);
+        sincos_qt_small(fma(1.5, D3, D2), Qi, Qr);
+        sincos_qt_small(4.0 * D3, Ci, Cr);
         double A0r = 0.0, A0i = 0.0, A1r = 0.0, A1i = 0.0, A2r = 0.0, A2i = 0.0, A3r = 0.0, A3i = 0.0;
-#pragma unroll 2
-        for (int b = 0; b < nb; ++b) {
-            const double2 d = tp[b];
-            A0r = fma(d.x, Er, fma(-d.y, Ei, A0r));       // A_0 += q,  q = dw' E (never formed)
-            A0i = fma(d.x, Ei, fma(d.y, Er, A0i));
-            A1r += A0r; A1i += A0i;
-            A2r += A1r; A2i += A1i;
-            A3r += A2r; A3i += A2i;
-            const double er = fma(Er, Rr, -Ei * Ri);
-            Ei = fma(Er, Ri, Ei * Rr);
-            Er = er;
-            const double rr = fma(Rr, Qr, -Ri * Qi);
-            Ri = fma(Rr, Qi, Ri * Qr);
-            Rr = rr;
+#define FSTAT_BIN_STEP(d)                                                                            \
+        {                                                                                            \
+            A0r = fma((d).x, Er, fma(-(d).y, Ei, A0r));   /* A_0 += q,  q = dw' E (never formed) */ \
+            A0i = fma((d).x, Ei, fma((d).y, Er, A0i));                                               \
+            A1r += A0r; A1i += A0i;                                                                  \
+            A2r += A1r; A2i += A1i;                                                                  \
+            A3r += A2r; A3i += A2i;                                                                  \
+            const double er = fma(Er, Rr, -Ei * Ri);                                                 \
+            Ei = fma(Er, Ri, Ei * Rr);                                                               \
+            Er = er;                                                                                 \
+            const double rr = fma(Rr, Qr, -Ri * Qi);                                                 \
+            Ri = fma(Rr, Qi, Ri * Qr);                                                               \
+            Rr = rr;                                                                                 \
+        }
+        int b = 0;
+        for (; b + 4 <= nb; b += 4) {
+            const double2 d0 = tp[b], d1 = tp[b + 1], d2 = tp[b + 2], d3 = tp[b + 3];
+            FSTAT_BIN_STEP(d0)
+            FSTAT_BIN_STEP(d1)
+            FSTAT_BIN_STEP(d2)
+            FSTAT_BIN_STEP(d3)
             const double qq = fma(Qr, Cr, -Qi * Ci);
             Qi = fma(Qr, Ci, Qi * Cr);
             Qr = qq;
         }
+        for (; b < nb; ++b) {
+            const double2 d0 = tp[b];
+            FSTAT_BIN_STEP(d0)
+        }
+#undef FSTAT_BIN_STEP
 
         // ---- z_P += sum_n conj(c^P_n) A_n
         const double U = (double)(j1 - node0);

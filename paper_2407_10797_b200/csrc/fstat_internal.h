@@ -71,6 +71,7 @@ struct SegCrit {
     double ad;       // (3/128) x Doppler phase amplitude                 [quarter turns]
     double ct;       // response: relative error = ct (omega S)^4
     double kl;       // 0.05 x partition length [bins]: sqrt(normalised det M_k) >~ min(1, kl omega)  (hazard H3)
+    double r1, r2;   // third phase difference D3 = c3 r1 + |c9| r2 + Doppler part   [quarter turns per bin^3]
     double d2;       // second phase difference [quarter turns / bin^2] = d2 * omega; must stay below 1/64
 };
 
