@@ -118,6 +118,9 @@ def parse_args():
     ap.add_argument("--config", default="first_stage", help="tiny | first_stage | middle_stages | final_coherent | wide_band")
     ap.add_argument("--n-part", type=int, default=None, help="override N_p (default: the config's first)")
     ap.add_argument("--particles", type=int, default=None, help="override P (default: the config's first)")
+    ap.add_argument("--force-level", type=int, default=-2, help="plan option force_level (-2 automatic stride)")
+    ap.add_argument("--max-segment-bins", type=int, default=0, help="plan option max_segment_bins (0 automatic)")
+    ap.add_argument("--interp-tol", type=float, default=1.0, help="plan option interp_tol")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
     return ap.parse_args()
@@ -232,7 +235,9 @@ def run_ours(args):
     ds, t_data = dataset_for(cfg, gpu_template_fn(fs, cfg))
     edges = ds.edges(n_part)
     t0 = time.time()
-    plan = fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges)
+    opts = fs.fstat_default_options(force_level=args.force_level, max_segment_bins=args.max_segment_bins,
+                                    interp_tol=args.interp_tol)
+    plan = fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, opts)
     torch.cuda.synchronize()
     t_plan = time.time() - t0
 
@@ -347,6 +352,8 @@ def run_ours(args):
                       "no collective on the data path" % world,
                       "l2": "L2 flushed before every timed step (256 MiB scratch write, outside the timed events)",
                       "n_ctas": fs.fstat_plan_n_ctas(plan, P), "n_sm": n_sm,
+                      "plan_options": {"force_level": args.force_level, "max_segment_bins": args.max_segment_bins,
+                                       "interp_tol": args.interp_tol},
                       "plan_create_s": t_plan, "dataset_s": t_data},
            "particles_per_s": float(P) * world / (ms_step * 1e-3),
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(par_pin.numel() * 8),
