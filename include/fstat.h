@@ -62,7 +62,7 @@ typedef struct {
                                * (every bin evaluated in full, no interpolation); 0..5: stride 8 << level          *
                                * wherever the segment allows it, regardless of the bound (tests / tuning)          */
     double interp_tol;        /* scale of the interpolation error tolerances; 1.0 (default) = carrier phase        *
-                               * 4e-7 rad and TDI response 4e-7 relative            */
+                               * 4e-7 rad and TDI response 2e-7 relative            */
 } fstat_options;
 
 FSTAT_API void fstat_default_options(fstat_options *opts);
@@ -158,7 +158,7 @@ FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
 /* Number of (particle-group, segment) work items = CTAs the main kernel launches for P particles. */
 FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
 /* Number of CUDA kernels the fstat_eval_batch / fstat_eval_batch_host calls on this plan have launched so
- * far (per call: prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and
+ * far (per call: particle ranking, prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and
  * the chunk sums of F when the partitions are split over several epilogue blocks). */
 FSTAT_API int64_t fstat_plan_launch_count(const fstat_plan *plan);
 /* How the most recent fstat_eval_batch on this plan was split between the direct kernel and the six

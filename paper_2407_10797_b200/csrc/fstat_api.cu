@@ -52,6 +52,8 @@ struct fstat_plan {
     // workspace
     double *d_coef = nullptr;  size_t coef_cap = 0;      // doubles
     int32_t *d_valid = nullptr; size_t valid_cap = 0;    // ints
+    int32_t *d_slot = nullptr; size_t slot_cap = 0;      // [P] particle -> slot (sorted by chirp mass)
+    int32_t *d_perm = nullptr; size_t perm_cap = 0;      // [P_pad] slot -> particle (-1: padding)
     double *d_partial = nullptr; size_t partial_cap = 0; // doubles
     // host-buffer path
     double *d_params = nullptr, *d_F = nullptr, *d_Fk = nullptr;
@@ -417,7 +419,7 @@ static void plan_free(fstat_plan *pl)
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
-    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct);
+    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
@@ -572,9 +574,12 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     }
     pl->last_groups = (int32_t)n_groups;
 
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef, pl->d_valid, st));
+    CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
+    CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, pl->d_coef, pl->d_valid,
+                               pl->d_perm, st));
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
-                               pl->d_seg_maxlvl, pl->opt.interp_tol * 4e-7 * (2.0 / kPi), pl->opt.interp_tol * 4e-7,
+                               pl->d_seg_maxlvl, pl->opt.interp_tol * 4e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
                                pl->opt.force_level, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;
@@ -609,11 +614,11 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, launch_main(a, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;
-    CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, P, P_pad, pl->n_part, pl->n_seg, pl->d_fpart,
+    CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg, pl->d_fpart,
                                F, Fk, st));
     {
-        int32_t chunk = 0;      // prologue, stride selection, [interpolating], direct, epilogue, [chunk sums of F]
-        pl->n_launches += 4 + (pl->fast_ok ? 1 : 0) + (epilogue_chunks(P, pl->n_part, &chunk) > 1 ? 1 : 0);
+        int32_t chunk = 0;      // rank, prologue, stride selection, [interpolating], direct, epilogue, [chunk sums of F]
+        pl->n_launches += 5 + (pl->fast_ok ? 1 : 0) + (epilogue_chunks(P, pl->n_part, &chunk) > 1 ? 1 : 0);
     }
     return FSTAT_OK;
 }
@@ -659,8 +664,8 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
     CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)kThreads * kNCoef));
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)kThreads));
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
-    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_coef,
-                               pl->d_valid, st));
+    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, pl->d_coef,
+                               pl->d_valid, nullptr, st));
     CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, u_plus, u_cross, st));
     CU_TRY(pl, cudaStreamSynchronize(st));
     return FSTAT_OK;

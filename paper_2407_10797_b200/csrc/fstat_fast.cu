@@ -255,7 +255,7 @@ __device__ __forceinline__ void load_coef(const double *__restrict__ cf, int64_t
     for (int j = 0; j < kNCoef; ++j) c[j] = cf[(int64_t)j * P_pad];
 }
 
-__global__ void __launch_bounds__(kThreads, 3) fstat_fast_kernel(const __grid_constant__ FastArgs a)
+__global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_constant__ FastArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     FastSmem &sm = *reinterpret_cast<FastSmem *>(smem_raw);

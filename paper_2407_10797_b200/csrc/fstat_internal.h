@@ -126,11 +126,11 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            double *coef, int32_t *valid, cudaStream_t st);
+                            int32_t *slot_of, double *coef, int32_t *valid, int32_t *perm, cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
-cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
-                            int64_t P_pad, int32_t n_part, int32_t n_seg, double *Fpart, double *F, double *Fk,
-                            cudaStream_t st);
+cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
+                            const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
+                            double *Fpart, double *F, double *Fk, cudaStream_t st);
 int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out);
 cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
                             const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st);

@@ -64,11 +64,16 @@ cudaError_t launch_build_table(const double *freq, const double *dw, const doubl
 // =================================================================================================
 // a1: per-particle coefficients (PAPER.md:404 Eq. A3 with readings A1-A3; :71 parameter meanings)
 // =================================================================================================
+// Particles are evaluated in SLOTS sorted by chirp mass (rank_kernel below): the 128 particles of a CTA then
+// sweep t_f at nearly the same rate, so the stride selection is not held back by one low-mass particle
+// per group.  slot_of == nullptr means the identity (template dump).  perm[slot] = particle, -1 for padding.
 __global__ void prologue_kernel(const double *__restrict__ params, int64_t P, int64_t P_pad, double f_ref,
-                                double kappa, double *__restrict__ coef, int32_t *__restrict__ valid)
+                                double kappa, const int32_t *__restrict__ slot_of, double *__restrict__ coef,
+                                int32_t *__restrict__ valid, int32_t *__restrict__ perm)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P_pad) return;
+    const int64_t slot = (p < P && slot_of != nullptr) ? (int64_t)slot_of[p] : p;
     double c[kNCoef];
 #pragma unroll
     for (int j = 0; j < kNCoef; ++j) c[j] = 0.0;
@@ -77,7 +82,7 @@ __global__ void prologue_kernel(const double *__restrict__ params, int64_t P, in
         const double tc = params[6 * p + 0], Mc = params[6 * p + 1], eta = params[6 * p + 2];
         const double theta = params[6 * p + 3], phi = params[6 * p + 4], e0 = params[6 * p + 5];
         ok = isfinite(tc) && isfinite(Mc) && isfinite(eta) && isfinite(theta) && isfinite(phi) && isfinite(e0) &&
-             (Mc > 0.0) && (eta > 0.0) && (eta <= 0.25) && (e0 >= 0.0);
+             (Mc > 0.0) && (eta > 0.0) && (eta <= 0.25) && (e0 >= 0.0);          // same rule as particle_ok()
         if (ok) {
             const double pi = kPi;
             const double Mcs = Mc * kGMsunC3;
@@ -114,15 +119,55 @@ __global__ void prologue_kernel(const double *__restrict__ params, int64_t P, in
         }
     }
 #pragma unroll
-    for (int j = 0; j < kNCoef; ++j) coef[(int64_t)j * P_pad + p] = c[j];
-    valid[p] = ok;
+    for (int j = 0; j < kNCoef; ++j) coef[(int64_t)j * P_pad + slot] = c[j];
+    valid[slot] = ok;
+    if (perm != nullptr) perm[slot] = (p < P) ? (int32_t)p : -1;
+}
+
+__device__ __forceinline__ bool particle_ok(const double *__restrict__ q)
+{
+    return isfinite(q[0]) && isfinite(q[1]) && isfinite(q[2]) && isfinite(q[3]) && isfinite(q[4]) && isfinite(q[5]) &&
+           (q[1] > 0.0) && (q[2] > 0.0) && (q[2] <= 0.25) && (q[5] >= 0.0);
+}
+
+// slot_of[i] = rank of particle i by (chirp mass rounded to float, index): a stable, deterministic sort by
+// brute force (P^2 integer comparisons through shared-memory tiles; ~1 ms at P = 65536, where one
+// evaluation takes ~200 ms).  Invalid particles sort last.
+__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P,
+                                                   int32_t *__restrict__ slot_of)
+{
+    __shared__ uint32_t skey[256];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    uint32_t my = 0xFFFFFFFFu;
+    if (i < P && particle_ok(params + 6 * (int64_t)i)) my = __float_as_uint((float)params[6 * (int64_t)i + 1]);
+    int rank = 0;
+    for (int j0 = 0; j0 < P; j0 += 256) {
+        const int j = j0 + threadIdx.x;
+        uint32_t k = 0xFFFFFFFFu;
+        if (j < P && particle_ok(params + 6 * (int64_t)j)) k = __float_as_uint((float)params[6 * (int64_t)j + 1]);
+        __syncthreads();
+        skey[threadIdx.x] = k;
+        __syncthreads();
+        const int n = min(256, P - j0);
+        for (int t = 0; t < n; ++t) {
+            const uint32_t kt = skey[t];
+            rank += (kt < my) || (kt == my && j0 + t < i);
+        }
+    }
+    if (i < P) slot_of[i] = rank;
 }
 
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            double *coef, int32_t *valid, cudaStream_t st)
+                            int32_t *slot_of, double *coef, int32_t *valid, int32_t *perm, cudaStream_t st)
 {
+    if (slot_of != nullptr) {
+        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, slot_of);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     const int nt = 128;
-    prologue_kernel<<<(unsigned)((P_pad + nt - 1) / nt), nt, 0, st>>>(params, P, P_pad, f_ref_e0, kappa, coef, valid);
+    prologue_kernel<<<(unsigned)((P_pad + nt - 1) / nt), nt, 0, st>>>(params, P, P_pad, f_ref_e0, kappa, slot_of, coef,
+                                                                      valid, perm);
     return cudaGetLastError();
 }
 
@@ -342,17 +387,21 @@ template <bool SEG_PAR>
 __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__restrict__ partial,
                                                                const int32_t *__restrict__ part_seg,
                                                                const int32_t *__restrict__ valid, int64_t P,
-                                                               int64_t P_pad, int32_t n_part, int32_t chunk,
+                                                               const int32_t *__restrict__ perm, int64_t P_pad,
+                                                               int32_t n_part, int32_t chunk,
                                                                double *__restrict__ Fout, double *__restrict__ Fk)
 {
+    __shared__ int32_t sPerm[kEpiX];
     __shared__ double sF[kEpiY][kEpiX];
     __shared__ double sT[kEpiY][kEpiX + 1];
     __shared__ double sV[SEG_PAR ? kEpiY : 1][kNAcc][kEpiX];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int64_t p0 = (int64_t)blockIdx.x * kEpiX;
-    const int64_t p = p0 + tx;
+    const int64_t p = p0 + tx;                            // slot; the particle it holds is perm[p]
     const bool live = p < P;
     const bool ok = live && valid[p] != 0;
+    if (threadIdx.y == 0) sPerm[tx] = live ? perm[p] : -1;
+    __syncthreads();
     const double ninf = -INFINITY;
     const int k_lo = blockIdx.y * chunk, k_hi = min(n_part, k_lo + chunk);
     double fsum = 0.0;
@@ -411,7 +460,7 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
             // 256 threads write a 32 (particles) x 8 (partitions) tile: thread -> (particle = id / 8, k = id % 8)
             const int id = ty * kEpiX + tx;
             const int pp = id / kEpiY, kk = id % kEpiY;
-            if (p0 + pp < P && k0 + kk < k_hi) Fk[(p0 + pp) * (int64_t)n_part + k0 + kk] = sT[kk][pp];
+            if (p0 + pp < P && k0 + kk < k_hi) Fk[(int64_t)sPerm[pp] * n_part + k0 + kk] = sT[kk][pp];
             __syncthreads();
         }
     }
@@ -421,19 +470,20 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
         double s = 0.0;
 #pragma unroll
         for (int y = 0; y < kEpiY; ++y) s += sF[y][tx];
-        if (gridDim.y == 1) Fout[p] = ok ? s : ninf;                        // F itself
+        if (gridDim.y == 1) Fout[sPerm[tx]] = ok ? s : ninf;                // F itself
         else Fout[(int64_t)blockIdx.y * P_pad + p] = s;                      // chunk sum, see fsum_kernel
     }
 }
 
-__global__ void fsum_kernel(const double *__restrict__ Fpart, const int32_t *__restrict__ valid, int64_t P,
-                            int64_t P_pad, int32_t n_chunk, double *__restrict__ F)
+__global__ void fsum_kernel(const double *__restrict__ Fpart, const int32_t *__restrict__ valid,
+                            const int32_t *__restrict__ perm, int64_t P, int64_t P_pad, int32_t n_chunk,
+                            double *__restrict__ F)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
     double s = 0.0;
     for (int c = 0; c < n_chunk; ++c) s += Fpart[(int64_t)c * P_pad + p];
-    F[p] = valid[p] != 0 ? s : -INFINITY;
+    F[perm[p]] = valid[p] != 0 ? s : -INFINITY;
 }
 
 int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out)
@@ -450,9 +500,9 @@ int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out)
     return (n_part + chunk - 1) / chunk;
 }
 
-cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid, int64_t P,
-                            int64_t P_pad, int32_t n_part, int32_t n_seg, double *Fpart, double *F, double *Fk,
-                            cudaStream_t st)
+cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
+                            const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
+                            double *Fpart, double *F, double *Fk, cudaStream_t st)
 {
     int32_t chunk = 0;
     const int32_t n_chunk = epilogue_chunks(P, n_part, &chunk);
@@ -460,12 +510,12 @@ cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, cons
     const dim3 grd((unsigned)((P + kEpiX - 1) / kEpiX), (unsigned)n_chunk);
     double *out = (n_chunk == 1) ? F : Fpart;
     if (n_seg >= 4 * n_part)
-        epilogue_kernel<true><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, P_pad, n_part, chunk, out, Fk);
+        epilogue_kernel<true><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
     else
-        epilogue_kernel<false><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, P_pad, n_part, chunk, out, Fk);
+        epilogue_kernel<false><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || n_chunk == 1) return e;
-    fsum_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(Fpart, valid, P, P_pad, n_chunk, F);
+    fsum_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(Fpart, valid, perm, P, P_pad, n_chunk, F);
     return cudaGetLastError();
 }
 
