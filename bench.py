@@ -47,7 +47,7 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
 STRIDES = (0, 8, 16, 32, 64, 128, 256)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from
 # the ncu --set full capture summarised in profiles/ (None until that capture exists for the current kernel)
-NCU_DRAM_BYTES_PER_LAUNCH = None
+NCU_DRAM_BYTES_PER_LAUNCH = 169.0e6     # profiles/r1_v2.md: 34.9 MB read + 134.1 MB written (config 1)
 
 
 # ------------------------------------------------------------------------------------------ utilities
@@ -330,7 +330,8 @@ def run_ours(args):
     hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * float(lvl_sub.sum()) + 64.0 * 128.0 * n_items
     roofline = {"bound": "alu", "kernel": "fstat_fast_kernel (+ fstat_main_kernel for the work items it leaves)",
                 "pipe": "fp64", "achieved": achieved, "peak": peak,
-                "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+                "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (cfg.name == "first_stage" and n_part == 1024 and P == 2048) else None,
                 "peak_source": "dependent-free DFMA stream measured in this run (fstat_probe_pipe_peak), x2 flop",
                 "nominal_peak": NOMINAL_FP64_TFLOPS, "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
                 "fp64_inst_per_launch": fp64_inst, "fp64_inst_per_template_bin": fp64_inst / (float(P) * ds.n_bins),
