@@ -290,3 +290,24 @@ def test_noise_only_statistic_has_chi2_mean(fs, torch_, first_stage):
     m = 2.0 * Fk_g.mean()
     # 256 templates share one noise realisation: effective sample >= 1024 independent partitions
     assert abs(m - 4.0) < 5.0 * math.sqrt(8.0 / 1024.0)
+
+
+def test_config1_every_value_interpolating_kernel_against_direct_kernel(fs, torch_, first_stage):
+    """All 2 097 152 F_k of config 1 (P = 2048, N_p = 1024) in bench.py's launch configuration: the
+    interpolating kernel (automatic strides) against the direct kernel, which evaluates the full model at
+    every bin and is itself checked against the oracle above.  No sampling: this is the test that exposed
+    the |k.n| > 1 response bug (4e-4 on a handful of near-singular partitions).  Also the N_p = 16 and
+    N_p = 1 stages on a quarter of the particles."""
+    ds = first_stage
+    par = syn.draw_particles(ds.cfg)
+    for n_part, P in ((1024, 2048), (16, 512), (1, 512)):
+        edges = ds.edges(n_part)
+        F_d, Fk_d = _gpu_eval(fs, torch_, ds, edges, par[:P], fs.fstat_default_options(force_level=-1))
+        with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges) as plan:
+            F_a, Fk_a = fs.fstat_eval_batch(plan, torch_.as_tensor(par[:P], device="cuda"))
+            torch_.cuda.synchronize()
+            bins, _ = fs.fstat_plan_level_bins(plan)
+            F_a, Fk_a = F_a.cpu().numpy(), Fk_a.cpu().numpy()
+        assert bins[0] <= 1e-3 * bins.sum()                    # the interpolating kernel carries the band
+        assert _rel(Fk_a, Fk_d).max() <= 5e-6, (n_part, _rel(Fk_a, Fk_d).max())
+        assert _rel(F_a, F_d).max() <= 1e-6, (n_part, _rel(F_a, F_d).max())
