@@ -44,7 +44,7 @@ FAST_FP64_PER_INTERVAL = 570.0
 FAST_FP64_PER_ITEM = 667.0
 DIRECT_FP64_PER_BIN = 263.0
 NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
-STRIDES = (0, 8, 16, 32, 64, 128, 256)          # index 0 = direct kernel
+STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from
 # the ncu --set full capture summarised in profiles/ (None until that capture exists for the current kernel)
 NCU_DRAM_BYTES_PER_LAUNCH = 169.0e6     # profiles/r1_v2.md: 34.9 MB read + 134.1 MB written (config 1)

@@ -59,7 +59,7 @@ typedef struct {
                                * sums before handing its partial sums to the epilogue (tuning / tests)  */
     int32_t force_level;      /* -2 (default): the stride of the interpolating kernel is chosen per (particle      *
                                * group, segment) from an a-priori error bound; -1: direct kernel everywhere       *
-                               * (every bin evaluated in full, no interpolation); 0..5: stride 8 << level          *
+                               * (every bin evaluated in full, no interpolation); 0..6: stride 8 << level          *
                                * wherever the segment allows it, regardless of the bound (tests / tuning)          */
     double interp_tol;        /* scale of the interpolation error tolerances; 1.0 (default) = carrier phase        *
                                * 4e-7 rad and TDI response 2e-7 relative            */
@@ -161,11 +161,11 @@ FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
  * far (per call: particle ranking, prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and
  * the chunk sums of F when the partitions are split over several epilogue blocks). */
 FSTAT_API int64_t fstat_plan_launch_count(const fstat_plan *plan);
-/* How the most recent fstat_eval_batch on this plan was split between the direct kernel and the six
- * strides of the interpolating kernel: bins_out[0] / [1..6] = sum over the (particle group, segment) work
- * items run by the direct kernel / at stride 8, 16, 32, 64, 128, 256 of the segment's bin count (multiply
- * by 128 particles per group for template-bins); subblocks_out[1..6] = number of node intervals those
- * items walked (one full-model node evaluation each).  HOST arrays of 7.  Synchronises the device. */
+/* How the most recent fstat_eval_batch on this plan was split between the direct kernel and the seven
+ * strides of the interpolating kernel: bins_out[0] / [1..7] = sum over the (particle group, segment) work
+ * items run by the direct kernel / at stride 8, 16, 32, 64, 128, 256, 512 of the segment's bin count
+ * (multiply by 128 particles per group for template-bins); subblocks_out[1..7] = number of node intervals
+ * those items walked (one full-model node evaluation each).  HOST arrays of 8.  Synchronises the device. */
 FSTAT_API fstat_status fstat_plan_level_bins(fstat_plan *plan, int64_t *bins_out, int64_t *subblocks_out);
 /* Device time of the main (fused template + inner product) kernels in the most recent evaluations on
  * this plan: CUDA events are recorded on the call's stream around that kernel at every fstat_eval_batch

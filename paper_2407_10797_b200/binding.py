@@ -295,8 +295,8 @@ def fstat_plan_launch_count(plan: Plan) -> int:
 
 
 def fstat_plan_level_bins(plan: Plan) -> Tuple[np.ndarray, np.ndarray]:
-    """(bins[7], subblocks[7]) of the most recent evaluation: index 0 = direct kernel, 1..6 = stride 8..256."""
-    b, s = np.zeros(7, dtype=np.int64), np.zeros(7, dtype=np.int64)
+    """(bins[8], subblocks[8]) of the most recent evaluation: index 0 = direct kernel, 1..7 = stride 8..512."""
+    b, s = np.zeros(8, dtype=np.int64), np.zeros(8, dtype=np.int64)
     _check(load_library().fstat_plan_level_bins(plan.handle, b.ctypes.data_as(C.POINTER(C.c_int64)),
                                                 s.ctypes.data_as(C.POINTER(C.c_int64))), "fstat_plan_level_bins", plan)
     return b, s

@@ -28,7 +28,7 @@ struct fstat_plan {
     double *d_dwp = nullptr;           // [n_bins][2]       folded data (interpolating kernel)
     double *d_node = nullptr;          // [n_node_rows][kTabW]
     int64_t n_node_rows = 0;
-    bool fast_ok = false;              // the node grid (256 bins beyond both ends) stays at f > 0
+    bool fast_ok = false;              // the node grid (kMaxStride bins beyond both ends) stays at f > 0
     // partition-dependent tables of the interpolating kernel
     int32_t *d_edges32 = nullptr; size_t edges32_cap = 0;
     int32_t *d_cnt = nullptr; size_t cnt_cap = 0;          // scratch [n_part]
@@ -118,7 +118,7 @@ bool edges_valid(int64_t n_bins, int32_t n_part, const int64_t *e, std::string *
 // Cut every partition into CTA work items ("segments").  A segment never crosses a partition edge, so
 // the main kernels need no per-bin edge test and write plain partial sums.
 //   aligned: the cuts inside a partition are the multiples of max_len (itself a multiple of kMaxStride),
-//            so that node intervals of every stride and the 256-bin data tiles never straddle a segment
+//            so that node intervals of every stride and the 512-bin data tiles never straddle a segment
 //            boundary other than a partition edge -- the layout the interpolating kernel needs;
 //   else:    near-equal pieces of at most max_len bins (tuning / tests; direct kernel only).
 void make_segments(const std::vector<int64_t> &edges, int64_t max_len, bool aligned,
@@ -368,7 +368,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     if (e == cudaSuccess) e = cudaMemset(d_err, 0, sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_table, (size_t)n_bins * kTabW * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_dwp, (size_t)n_bins * 2 * sizeof(double));
-    // node rows for bins -256 .. (floor((N-1)/256) + 2) * 256 in steps of kNodeStride
+    // node rows for bins -kMaxStride .. (floor((N-1)/kMaxStride) + 2) * kMaxStride in steps of kNodeStride
     pl->n_node_rows = kNodePad + (((n_bins - 1) / kMaxStride + 2) * kMaxStride) / kNodeStride + 1;
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_node, (size_t)pl->n_node_rows * kTabW * sizeof(double));
     uint32_t bits = 0;

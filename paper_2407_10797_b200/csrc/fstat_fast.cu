@@ -210,7 +210,7 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
 // =================================================================================================
 // a2-a5, interpolating kernel.  Grid = particle groups x segments (same work items as the direct kernel),
 // CTA = 128 threads = 128 particles.  The folded data dw' of the segment streams through a 4-stage
-// shared-memory ring of 256-bin tiles (TMA bulk copies, mbarrier completion); every thread reads the
+// shared-memory ring of 512-bin tiles (TMA bulk copies, mbarrier completion); every thread reads the
 // same element (broadcast).  Node rows and Gram matrices are warp-uniform global loads (L1/L2 hits).
 // =================================================================================================
 struct __align__(16) FastSmem {
@@ -271,13 +271,13 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
     const double *cf = a.coef + p;
 
     const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
-    const int t_first = lo >> 8;
-    const int n_tiles = ((hi - 1) >> 8) - t_first + 1;
+    const int t_first = lo >> kFastTileShift;
+    const int n_tiles = ((hi - 1) >> kFastTileShift) - t_first + 1;
     const double2 *dwp = reinterpret_cast<const double2 *>(a.dwp);
 
     auto issue_tile = [&](int t) {                           // t = tile number relative to t_first
         const int slot = t % kFastStages;
-        const int b0 = max(lo, (t_first + t) << 8), b1 = min(hi, (t_first + t + 1) << 8);
+        const int b0 = max(lo, (t_first + t) << kFastTileShift), b1 = min(hi, (t_first + t + 1) << kFastTileShift);
         const uint32_t bytes = (uint32_t)(b1 - b0) * (uint32_t)sizeof(double2);
         mbar_expect_tx(&sm.full[slot], bytes);
         tma_load_1d(&sm.tile[slot][b0 & (kFastTile - 1)], dwp + b0, bytes, &sm.full[slot]);
@@ -345,7 +345,7 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             D3 = 6.0 * G3;
         }
         // ---- the tile that holds [j0, j1)
-        const int tl = (j0 >> 8) - t_first;
+        const int tl = (j0 >> kFastTileShift) - t_first;
         if (tl != cur_tile) {
             if (cur_tile >= 0) {
                 __syncthreads();                             // every thread is done with the previous tile
@@ -386,6 +386,7 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             Rr = rr;                                                                                 \
         }
         int b = 0;
+#pragma unroll 2
         for (; b + 4 <= nb; b += 4) {
             const double2 d0 = tp[b], d1 = tp[b + 1], d2 = tp[b + 2], d3 = tp[b + 3];
             FSTAT_BIN_STEP(d0)

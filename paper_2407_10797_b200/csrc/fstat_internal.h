@@ -54,13 +54,15 @@ struct OrbitCoef {
 // ---- interpolating ("fast") path: the slow factors of the template (carrier phase without its linear
 // term, T'_+, T'_x) are evaluated in full FP64 only at nodes every S = 8 << level bins and carried
 // between nodes by the cubic through the four surrounding nodes.
-constexpr int kNLevels = 6;                          // S = 8, 16, 32, 64, 128, 256
+constexpr int kNLevels = 7;                          // S = 8, 16, 32, 64, 128, 256, 512
 constexpr int kLevel0Shift = 3;
 constexpr int kMinStride = 1 << kLevel0Shift;
-constexpr int kMaxStride = kMinStride << (kNLevels - 1);   // 256; segment cuts inside a partition are multiples of it
+constexpr int kMaxStride = kMinStride << (kNLevels - 1);   // 512; segment cuts inside a partition are multiples of it
 constexpr int kNodeStride = kMinStride;              // the node table has one row every 8 bins
-constexpr int kNodePad = kMaxStride / kNodeStride;   // rows before bin 0 (nodes down to bin -256)
-constexpr int kFastTile = 256;                       // bins per TMA tile of the folded data (4 KiB), 256-aligned
+constexpr int kNodePad = kMaxStride / kNodeStride;   // rows before bin 0 (nodes down to bin -512)
+constexpr int kFastTileShift = 9;
+constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the folded data (8 KiB), aligned to its size;
+                                                     // >= kMaxStride so that no sub-block straddles two tiles
 constexpr int kFastStages = 4;
 constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
 

@@ -80,10 +80,28 @@ def test_every_forced_stride_matches_oracle(fs, torch_, orc, fine, level):
     assert _rel(F_g, F_o).max() <= RTOL, level
 
 
+def test_largest_stride_at_28_mhz(fs, torch_, orc):
+    """Stride 512 (the largest) needs an orbital phase advance below ~2e-5 rad per bin: forced on a 28 mHz
+    slice, where the automatic selection also picks it for most of the band."""
+    ds = syn.make_dataset(_fine_cfg(0.0280, 0.0281, index=13), orc.template)
+    par = syn.draw_particles(ds.cfg, 40)
+    edges = ds.edges(2)
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par)
+    F_g, Fk_g, bins, _ = _eval(fs, torch_, ds, edges, par, force_level=6)
+    assert bins[7] == ds.n_bins
+    assert _rel(Fk_g, Fk_o).max() <= RTOL and _rel(F_g, F_o).max() <= RTOL
+    par[:, 1] = np.linspace(32.0, 40.0, 40)
+    edges = ds.edges(1)                                   # a wide partition: little near-singular amplification
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par)
+    F_g, Fk_g, bins, _ = _eval(fs, torch_, ds, edges, par)
+    assert bins[7] > 0 and bins[0] == 0
+    assert _rel(Fk_g, Fk_o).max() <= 2e-6 and _rel(F_g, F_o).max() <= 2e-6
+
+
 def test_ragged_edges_cut_node_intervals_and_tiles(fs, torch_, orc, fine):
     """Partition edges that are not multiples of any stride, one-bin partitions (direct kernel: shorter
     than 8 bins; exactly singular M_k), partitions inside one node interval, and a partition spanning
-    many 256-bin tiles; also through fstat_plan_set_partitions and with segment cuts every 256 / 512
+    many 512-bin tiles; also through fstat_plan_set_partitions and with segment cuts every 512 / 1024
     bins.  (Partitions of 2-20 bins are left out on this fine grid: the template barely changes over
     them, M_k is singular to ~1e-12 and no FP64 evaluation, the oracle's included, is good to 1e-5.)"""
     ds = fine
@@ -95,7 +113,7 @@ def test_ragged_edges_cut_node_intervals_and_tiles(fs, torch_, orc, fine):
         np.array([0, n]),
         np.array([0, 100, 200, 250, 1000, 4096, n]),
     ]
-    for seg in (0, 256, 512):
+    for seg in (0, 512, 1024):
         for level in (-2, 0, 5):
             opts = fs.fstat_default_options(max_segment_bins=seg, force_level=level)
             with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), opts) as plan:
@@ -126,7 +144,7 @@ def test_low_frequency_slice_needs_small_strides(fs, torch_, orc):
     F_g, Fk_g, bins, _ = _eval(fs, torch_, ds, edges, par)
     assert bins[4:].sum() == 0 and bins[:4].sum() == ds.n_bins     # nothing at stride >= 64
     assert _rel(Fk_g, Fk_o).max() <= RTOL and _rel(F_g, F_o).max() <= RTOL
-    F_b, Fk_b, _, _ = _eval(fs, torch_, ds, edges, par, force_level=5)
+    F_b, Fk_b, _, _ = _eval(fs, torch_, ds, edges, par, force_level=6)
     assert _rel(Fk_b, Fk_o).max() > 10 * _rel(Fk_g, Fk_o).max()
 
 
@@ -145,16 +163,16 @@ def test_tolerance_option_moves_the_strides(fs, torch_, orc):
     _, _, b1, _ = _eval(fs, torch_, ds, edges, par)
     _, _, b2, _ = _eval(fs, torch_, ds, edges, par, interp_tol=1e-3)
     _, _, b3, _ = _eval(fs, torch_, ds, edges, par, interp_tol=1e3)
-    mean = lambda b: float((b[1:] * (8 << np.arange(6))).sum()) / max(int(b[1:].sum()), 1)
+    mean = lambda b: float((b[1:] * (8 << np.arange(7))).sum()) / max(int(b[1:].sum()), 1)
     assert mean(b2) < mean(b1) < mean(b3)
     with pytest.raises(fs.FstatError):
         fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, fs.fstat_default_options(interp_tol=0.0))
     with pytest.raises(fs.FstatError):
-        fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, fs.fstat_default_options(force_level=6))
+        fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, fs.fstat_default_options(force_level=7))
 
 
 def test_grid_starting_near_zero_frequency_falls_back_to_direct(fs, torch_, orc):
-    """The node grid reaches 256 bins below the band; a band that starts closer to f = 0 than that cannot
+    """The node grid reaches 512 bins below the band; a band that starts closer to f = 0 than that cannot
     be interpolated and must run (correctly) in the direct kernel."""
     T = T25
     k = np.arange(100, 400)
