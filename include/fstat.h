@@ -62,7 +62,7 @@ typedef struct {
                                * (every bin evaluated in full, no interpolation); 0..6: stride 8 << level          *
                                * wherever the segment allows it, regardless of the bound (tests / tuning)          */
     double interp_tol;        /* scale of the interpolation error tolerances; 1.0 (default) = carrier phase        *
-                               * 4e-7 rad and TDI response 2e-7 relative            */
+                               * 1.5e-7 rad and TDI response 2e-7 relative            */
 } fstat_options;
 
 FSTAT_API void fstat_default_options(fstat_options *opts);

@@ -28,7 +28,7 @@ struct fstat_plan {
     double *d_dwp = nullptr;           // [n_bins][2]       folded data (interpolating kernel)
     double *d_node = nullptr;          // [n_node_rows][kTabW]
     int64_t n_node_rows = 0;
-    bool fast_ok = false;              // the node grid (kMaxStride bins beyond both ends) stays at f > 0
+    bool fast_ok = false;              // the node grid (2 kMaxStride bins below, 3 above the band) stays at f > 0
     // partition-dependent tables of the interpolating kernel
     int32_t *d_edges32 = nullptr; size_t edges32_cap = 0;
     int32_t *d_cnt = nullptr; size_t cnt_cap = 0;          // scratch [n_part]
@@ -368,8 +368,8 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     if (e == cudaSuccess) e = cudaMemset(d_err, 0, sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_table, (size_t)n_bins * kTabW * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_dwp, (size_t)n_bins * 2 * sizeof(double));
-    // node rows for bins -kMaxStride .. (floor((N-1)/kMaxStride) + 2) * kMaxStride in steps of kNodeStride
-    pl->n_node_rows = kNodePad + (((n_bins - 1) / kMaxStride + 2) * kMaxStride) / kNodeStride + 1;
+    // node rows for bins -2 kMaxStride .. (floor((N-1)/kMaxStride) + 3) * kMaxStride in steps of kNodeStride
+    pl->n_node_rows = kNodePad + (((n_bins - 1) / kMaxStride + 3) * kMaxStride) / kNodeStride + 1;
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_node, (size_t)pl->n_node_rows * kTabW * sizeof(double));
     uint32_t bits = 0;
     if (e == cudaSuccess) {
@@ -377,7 +377,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
         if (!(pl->df > 0.0) || !isfinite(pl->df)) bits |= ERR_FREQ_ORDER;
         else {
             pl->f0 = fe[0];
-            pl->fast_ok = (fe[0] - (double)(kMaxStride + 1) * pl->df > 0.0) && n_bins > 1;
+            pl->fast_ok = (fe[0] - (double)(2 * kMaxStride + 1) * pl->df > 0.0) && n_bins > 1;
             e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->d_table,
                                    pl->d_dwp, d_err, 0);
             if (e == cudaSuccess)
@@ -579,7 +579,7 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, pl->d_coef, pl->d_valid,
                                pl->d_perm, st));
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
-                               pl->d_seg_maxlvl, pl->opt.interp_tol * 4e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
+                               pl->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
                                pl->opt.force_level, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;

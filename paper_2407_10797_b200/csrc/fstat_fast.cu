@@ -178,11 +178,12 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
             lvl = force_level < mx ? force_level : mx;
         } else {
             const double om2 = om * om, om4 = om2 * om2;
-            const double ephi1 = fma(c3, q.q1, fma(c9, q.q2, q.ad * om4));   // per S^4
+            // per S^4; kEconGain: the economised six-node cubic against the four-node cubic of the bound
+            const double ephi1 = fma(c3, q.q1, fma(c9, q.q2, q.ad * om4)) * (1.0 / kEconGain);
             // the response error is seen through M_k^-1: a partition over which the response barely changes
             // (kl omega < 1) has a near-singular M_k and amplifies it by 1 / sqrt(det) (hazard H3)
             const double kom = q.kl * om;
-            const double eT1 = (kom < 1.0) ? q.ct * om2 * om / q.kl : q.ct * om4;
+            const double eT1 = ((kom < 1.0) ? q.ct * om2 * om / q.kl : q.ct * om4) * (1.0 / kEconGain);
             lvl = -1;
             for (int l = 0; l <= mx; ++l) {
                 const double S = (double)(kMinStride << l), S2 = S * S, S4 = S2 * S2;
@@ -209,14 +210,39 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
 
 // =================================================================================================
 // a2-a5, interpolating kernel.  Grid = particle groups x segments (same work items as the direct kernel),
-// CTA = 128 threads = 128 particles.  The folded data dw' of the segment streams through a 4-stage
+// CTA = 128 threads = 128 particles.  The folded data dw' of the segment streams through a 3-stage
 // shared-memory ring of 512-bin tiles (TMA bulk copies, mbarrier completion); every thread reads the
 // same element (broadcast).  Node rows and Gram matrices are warp-uniform global loads (L1/L2 hits).
 // =================================================================================================
 struct __align__(16) FastSmem {
     double2 tile[kFastStages][kFastTile];
+    double win[kWinNodes][kNSlow][kThreads];   // per-thread ring of the last six node values (column = thread)
     uint64_t full[kFastStages];
 };
+
+// The cubic carried over a node interval [node m, node m+1] is NOT the Lagrange cubic through four nodes but
+// the Chebyshev-economised quintic through the six nodes m-2 .. m+3: the quintic's T_4 and T_5 terms on the
+// interval are dropped, which leaves the 4th-order error term 72 times smaller than the centre-interval error
+// of the four-node cubic (h^4 f/3072 against 3 h^4 f/128) for the same node evaluations.  Row a of
+// kEcon gives the value of that cubic at t = -1, 0, 1, 2 (so that everything downstream -- Newton
+// coefficients, Gram matrices in the four-node Lagrange basis -- is unchanged) from the node values at
+// t = -2 .. 3; rows sum to 1 exactly (rationals with denominator 61440).
+__constant__ double kEcon[4][6] = {
+    {-9133.0 / 61440.0, 6371.0 / 4096.0, -4517.0 / 6144.0, 2209.0 / 6144.0, 33.0 / 4096.0, -2407.0 / 61440.0},
+    {-11.0 / 61440.0, 7.0 / 12288.0, 2047.0 / 2048.0, -1.0 / 6144.0, 5.0 / 12288.0, -3.0 / 20480.0},
+    {-3.0 / 20480.0, 5.0 / 12288.0, -1.0 / 6144.0, 2047.0 / 2048.0, 7.0 / 12288.0, -11.0 / 61440.0},
+    {-2407.0 / 61440.0, 33.0 / 4096.0, 2209.0 / 6144.0, -4517.0 / 6144.0, 6371.0 / 4096.0, -9133.0 / 61440.0}};
+
+// v[k] = node values at t = -2 .. 3.  Returns yref = v[2] (node "0") and e[a] = cubic(t_a) - yref, t_a = -1, 0,
+// 1, 2, from the DIFFERENCES v[k] - yref (the phase values are ~1e7 quarter turns, their differences ~1e3).
+__device__ __forceinline__ void economise(const double (&v)[6], double &yref, double (&e)[4])
+{
+    yref = v[2];
+    const double d0 = v[0] - yref, d1 = v[1] - yref, d3 = v[3] - yref, d4 = v[4] - yref, d5 = v[5] - yref;
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+        e[a] = fma(kEcon[a][0], d0, fma(kEcon[a][1], d1, fma(kEcon[a][3], d3, fma(kEcon[a][4], d4, kEcon[a][5] * d5))));
+}
 
 // x - 4 rint(x / 4): exact for |x| < 2^51
 __device__ __forceinline__ double red4(double x) { return fma(-4.0, rint(0.25 * x), x); }
@@ -293,17 +319,19 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
     const double c0 = cf[0];
     const double slope = mulmod4(c0, a.df);
 
-    // node window: values at nodes m-1, m, m+1, m+2 of (psi_nl, T'_+ re, im, T'_x re, im)
-    double yph[4], ypr[4], ypi[4], ycr[4], yci[4];
+    // node ring: (psi_nl, T'_+ re, im, T'_x re, im) at the last six nodes, slot = (node + 6) % 6
     int m = lo >> sh;
     {
         double c[kNCoef];
         load_coef(cf, a.P_pad, c);
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
+        for (int k = -2; k <= 2; ++k) {
             const double2 *row = reinterpret_cast<const double2 *>(
-                a.node + ((int64_t)kNodePad + ((int64_t)(m + k - 1) << lvl)) * kTabW);
-            model_eval(row, c, a.orb, yph[k], ypr[k], ypi[k], ycr[k], yci[k]);
+                a.node + ((int64_t)kNodePad + ((int64_t)(m + k) * (1 << lvl))) * kTabW);
+            double v0, v1, v2, v3, v4;
+            model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
+            const int slot = (m + k + kWinNodes) % kWinNodes;
+            sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
+            sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
         }
     }
     __syncthreads();                                         // barriers initialised before anyone waits
@@ -318,24 +346,33 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
     while (j0 < hi) {
         const int node0 = m << sh;                           // bin of node "0" of this interval
         const int j1 = min(hi, node0 + (1 << sh));
-        // ---- new node m+2
+        const int s_base = (m - 2 + kWinNodes) % kWinNodes;  // ring slot of node m-2
+        // ---- new node m+3
         double fnode;
         {
             double c[kNCoef];
             load_coef(cf, a.P_pad, c);
             const double2 *row = reinterpret_cast<const double2 *>(
-                a.node + ((int64_t)kNodePad + ((int64_t)(m + 2) << lvl)) * kTabW);
-            model_eval(row, c, a.orb, yph[3], ypr[3], ypi[3], ycr[3], yci[3]);
+                a.node + ((int64_t)kNodePad + ((int64_t)(m + 3) * (1 << lvl))) * kTabW);
+            double v0, v1, v2, v3, v4;
+            model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
+            const int slot = (m + 3 + kWinNodes) % kWinNodes;
+            sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
+            sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
             fnode = a.node[((int64_t)kNodePad + ((int64_t)m << lvl)) * kTabW + T_F];
         }
-        // ---- carrier phase: cubic through the 4 nodes + exact linear term, as forward differences
+        // ---- carrier phase: economised cubic + exact linear term, as forward differences
         double t, D1, D2, D3;
         {
-            const double d0 = yph[0] - yph[1], d2 = yph[2] - yph[1], d3 = yph[3] - yph[1];
+            double v[6], yref, e[4];
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][0][tid];
+            economise(v, yref, e);
+            const double d0 = e[0] - e[1], d2 = e[2] - e[1], d3 = e[3] - e[1];
             const double a1 = fma(d0, -1.0 / 3.0, fma(d3, -1.0 / 6.0, d2));
             const double a2 = 0.5 * (d0 + d2);
             const double a3 = fma(d2, -0.5, (d3 - d0) * (1.0 / 6.0));
-            const double G0 = red4(yph[1]) + mulmod4(c0, fnode);
+            const double G0 = red4(yref) + e[1] + mulmod4(c0, fnode);
             const double G1 = red4(fma(a1, rS, slope));
             const double G2 = a2 * rS * rS, G3 = a3 * rS * rS * rS;
             const double s0 = (double)(j0 - node0);
@@ -403,6 +440,31 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
         }
 #undef FSTAT_BIN_STEP
 
+        // ---- the slow factors of this interval: economised cubic of T'_+, T'_x as values at t = -1, 0, 1, 2
+        double ypr[4], ypi[4], ycr[4], yci[4];
+        {
+            double v[6], yref;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][1][tid];
+            economise(v, yref, ypr);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) ypr[q] += yref;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][2][tid];
+            economise(v, yref, ypi);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) ypi[q] += yref;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][3][tid];
+            economise(v, yref, ycr);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) ycr[q] += yref;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][4][tid];
+            economise(v, yref, yci);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) yci[q] += yref;
+        }
         // ---- z_P += sum_n conj(c^P_n) A_n
         const double U = (double)(j1 - node0);
         {
@@ -442,11 +504,6 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             }
             acc[4] += mpp; acc[5] += mcc; acc[6] += mre; acc[7] += mim;
             gram += kNGram;
-        }
-        // ---- slide the node window
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            yph[k] = yph[k + 1]; ypr[k] = ypr[k + 1]; ypi[k] = ypi[k + 1]; ycr[k] = ycr[k + 1]; yci[k] = yci[k + 1];
         }
         j0 = j1;
         ++m;

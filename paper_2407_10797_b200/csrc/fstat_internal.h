@@ -59,11 +59,14 @@ constexpr int kLevel0Shift = 3;
 constexpr int kMinStride = 1 << kLevel0Shift;
 constexpr int kMaxStride = kMinStride << (kNLevels - 1);   // 512; segment cuts inside a partition are multiples of it
 constexpr int kNodeStride = kMinStride;              // the node table has one row every 8 bins
-constexpr int kNodePad = kMaxStride / kNodeStride;   // rows before bin 0 (nodes down to bin -512)
+constexpr int kNodePad = 2 * kMaxStride / kNodeStride;   // rows before bin 0 (nodes down to bin -1024)
+constexpr int kWinNodes = 6;                         // nodes m-2 .. m+3 feed the cubic of interval [m, m+1]
+constexpr int kNSlow = 5;                            // psi_nl, T'_+ (re, im), T'_x (re, im)
+constexpr double kEconGain = 20.0;                   // 4th-order error of the economised cubic vs the 4-node cubic (72 asymptotically)
 constexpr int kFastTileShift = 9;
 constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the folded data (8 KiB), aligned to its size;
                                                      // >= kMaxStride so that no sub-block straddles two tiles
-constexpr int kFastStages = 4;
+constexpr int kFastStages = 3;
 constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
 
 // per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)
