@@ -202,8 +202,15 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
     for (size_t k = 0; k + 1 < part_seg.size(); ++k)
         for (int32_t sgi = part_seg[k]; sgi < part_seg[k + 1]; ++sgi) {
             const int64_t lo = seg_edge[sgi], hi = seg_edge[sgi + 1];
-            for (int l = 0; l < kNLevels; ++l)
-                gbase[(size_t)sgi * kNLevels + l] = (int32_t)((lo >> (kLevel0Shift + l)) + pl->cnt[l][k]);
+            for (int l = 0; l < kNLevels; ++l) {
+                const int sh = kLevel0Shift + l;
+                const int64_t first = (lo >> sh) + pl->cnt[l][k];
+                const int64_t last = first + (((hi - 1) >> sh) - (lo >> sh));           // sub-blocks the item walks
+                const int64_t n_sub = ((pl->n_bins + ((int64_t)1 << sh) - 1) >> sh) + pl->cnt[l][pl->n_part - 1];
+                if (first < 0 || last >= n_sub)
+                    return fail(pl, FSTAT_ECUDA, "internal: Gram table index out of range");
+                gbase[(size_t)sgi * kNLevels + l] = (int32_t)first;
+            }
             crit[sgi] = make_seg_crit(pl->f0 + (double)lo * pl->df, pl->f0 + (double)hi * pl->df, pl->df,
                                       (double)(pl->edges[k + 1] - pl->edges[k]));
             maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && hi - lo >= 8) ? kNLevels - 1 : -1);
