@@ -124,6 +124,21 @@ FSTAT_API fstat_status fstat_eval_batch(fstat_plan *plan, int64_t P,
                                         void *cuda_stream);
 
 /*
+ * fstat_eval_amplitudes -- the maximum-likelihood extrinsic amplitudes a = M^-1 N of every partition
+ * (Eq. 10; a_1..a_4 multiply the basis templates A^1 = u_+, A^2 = u_x, A^3 = i u_+, A^4 = i u_x of
+ * Eq. 5 :77, and are the reparameterisation of (D_L, psi, iota, phi_c) of Eq. B1 :413 up to the amplitude
+ * constant of Eq. A2 :402, which the templates drop -- DESIGN.md reading A21).  Same kernels as
+ * fstat_eval_batch up to the last one; N_p = 1 gives the coherent estimate App. B asks for.
+ *
+ *   params  [P][6] DEVICE pointer as in fstat_eval_batch.
+ *   amp     [P][N_p][4] DEVICE pointer, row-major, out: a_1, a_2, a_3, a_4.  Invalid particles get NaN; a
+ *           partition whose M is rank-deficient gets the solution with the degenerate component set to 0.
+ * Asynchronous on cuda_stream.  Errors as fstat_eval_batch.
+ */
+FSTAT_API fstat_status fstat_eval_amplitudes(fstat_plan *plan, int64_t P, const double *params, double *amp,
+                                             void *cuda_stream);
+
+/*
  * fstat_eval_batch_host -- the same evaluation with HOST buffers: copies params to the device,
  * evaluates, copies F (and Fk when non-NULL) back and waits for completion before returning.
  * Pinned host memory makes the copies asynchronous DMA; pageable memory works too.

@@ -18,7 +18,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 # every symbol include/fstat.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
-    "fstat_eval_batch_host", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
+    "fstat_eval_batch_host", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
@@ -61,6 +61,8 @@ def load_library():
         L.fstat_plan_set_partitions.restype = C.c_int
         L.fstat_eval_batch.argtypes = [vp, i64, vp, vp, vp, vp]
         L.fstat_eval_batch.restype = C.c_int
+        L.fstat_eval_amplitudes.argtypes = [vp, i64, vp, vp, vp]
+        L.fstat_eval_amplitudes.restype = C.c_int
         L.fstat_eval_batch_host.argtypes = [vp, i64, vp, vp, vp, vp]
         L.fstat_eval_batch_host.restype = C.c_int
         L.fstat_eval_template.argtypes = [vp, dp, vp, vp, vp]
@@ -228,6 +230,19 @@ def fstat_eval_batch(plan: Plan, params, F=None, Fk=None, stream=None, want_Fk: 
     pFk = _dev_ptr(Fk, "Fk", P * plan.n_part) if Fk is not None else None
     _check(load_library().fstat_eval_batch(plan.handle, P, pp, pF, pFk, _stream_ptr(stream)), "fstat_eval_batch", plan)
     return F, Fk
+
+
+def fstat_eval_amplitudes(plan: Plan, params, amp=None, stream=None):
+    """params [P][6] float64 CUDA tensor -> amp [P][N_p][4] CUDA tensor (a_1..a_4 of PAPER.md Eq. 5 / 10)."""
+    import torch
+    P = int(params.shape[0])
+    pp = _dev_ptr(params, "params", 6 * P)
+    if amp is None:
+        amp = torch.empty((P, plan.n_part, 4), dtype=torch.float64, device=params.device)
+    pa = _dev_ptr(amp, "amp", 4 * P * plan.n_part)
+    _check(load_library().fstat_eval_amplitudes(plan.handle, P, pp, pa, _stream_ptr(stream)),
+           "fstat_eval_amplitudes", plan)
+    return amp
 
 
 def fstat_eval_batch_host(plan: Plan, params, F=None, Fk=None, stream=None, want_Fk: bool = True):

@@ -552,12 +552,14 @@ int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out
     return w;
 }
 
-fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, void *stream)
+// a1-a5 for P particles, then a6 (F, F_k) when F != NULL and / or the extrinsic amplitudes when amp != NULL
+static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, double *amp,
+                              void *stream)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
     if (P == 0) return FSTAT_OK;
-    if (!params || !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    if (!params || (!F && !amp)) return fail(pl, FSTAT_EINVAL, "params or the output pointer is NULL");
     if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
     DeviceGuard g(pl->device);
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
@@ -621,13 +623,30 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, launch_main(a, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;
-    CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg, pl->d_fpart,
-                               F, Fk, st));
-    {
-        int32_t chunk = 0;      // rank, prologue, stride selection, [interpolating], direct, epilogue, [chunk sums of F]
-        pl->n_launches += 5 + (pl->fast_ok ? 1 : 0) + (epilogue_chunks(P, pl->n_part, &chunk) > 1 ? 1 : 0);
+    pl->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
+    if (F) {
+        CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg,
+                                   pl->d_fpart, F, Fk, st));
+        int32_t chunk = 0;                             // epilogue, [chunk sums of F]
+        pl->n_launches += 1 + (epilogue_chunks(P, pl->n_part, &chunk) > 1 ? 1 : 0);
+    }
+    if (amp) {
+        CU_TRY(pl, launch_amplitudes(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, amp, st));
+        pl->n_launches += 1;
     }
     return FSTAT_OK;
+}
+
+fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, void *stream)
+{
+    if (pl && P > 0 && !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    return eval_impl(pl, P, params, F, Fk, nullptr, stream);
+}
+
+fstat_status fstat_eval_amplitudes(fstat_plan *pl, int64_t P, const double *params, double *amp, void *stream)
+{
+    if (pl && P > 0 && !amp) return fail(pl, FSTAT_EINVAL, "params or amp is NULL");
+    return eval_impl(pl, P, params, nullptr, nullptr, amp, stream);
 }
 
 fstat_status fstat_eval_batch_host(fstat_plan *pl, int64_t P, const double *params_host, double *F_host,

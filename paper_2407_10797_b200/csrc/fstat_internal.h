@@ -137,6 +137,9 @@ cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, cons
                             const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
                             double *Fpart, double *F, double *Fk, cudaStream_t st);
 int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out);
+cudaError_t launch_amplitudes(const double *partial, const int32_t *part_seg, const int32_t *valid,
+                              const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, double *amp,
+                              cudaStream_t st);
 cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
                             const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st);
 cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaStream_t st);

@@ -486,6 +486,65 @@ __global__ void fsum_kernel(const double *__restrict__ Fpart, const int32_t *__r
     F[perm[p]] = valid[p] != 0 ? s : -INFINITY;
 }
 
+// =================================================================================================
+// Extrinsic amplitudes (SURVEY row f3; PAPER.md:96 Eq. 10, :413 Eq. B1): a = M^-1 N per partition, from the
+// same eight sums.  With alpha_+ = a_1 + i a_3, alpha_x = a_2 + i a_4 (h = alpha_+ u_+ + alpha_x u_x) the
+// stationarity condition of Eq. 6 is the 2x2 Hermitian system  G alpha = z,  G = [[m_pp, conj(m_pc)],
+// [m_pc, m_cc]], solved by the same Gram-Schmidt steps as the epilogue.  Rank-deficient G: the component
+// along the degenerate direction is set to 0.  One thread per (slot, partition).
+// =================================================================================================
+__global__ void __launch_bounds__(128) amplitude_kernel(const double *__restrict__ partial,
+                                                        const int32_t *__restrict__ part_seg,
+                                                        const int32_t *__restrict__ valid,
+                                                        const int32_t *__restrict__ perm, int64_t P, int64_t P_pad,
+                                                        int32_t n_part, double *__restrict__ amp)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.y;
+    if (p >= P) return;
+    double v[kNAcc];
+#pragma unroll
+    for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
+    for (int s = part_seg[k]; s < part_seg[k + 1]; ++s) {
+        const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
+#pragma unroll
+        for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
+    }
+    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
+    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
+    double apr = 0.0, api = 0.0, acr = 0.0, aci = 0.0;
+    if (mpp > 0.0) {
+        const double inv = 1.0 / mpp;
+        const double cr = mr * inv, ci = mi * inv;                          // m_pc / m_pp
+        const double schur = mcc - (mr * mr + mi * mi) * inv;
+        if (schur > 1e-13 * mcc) {
+            acr = (zcr - (cr * zpr - ci * zpi)) / schur;                    // alpha_x = (z_x - (m_pc/m_pp) z_+) / schur
+            aci = (zci - (cr * zpi + ci * zpr)) / schur;
+        }
+        apr = (zpr - (mr * acr + mi * aci)) * inv;                          // alpha_+ = (z_+ - conj(m_pc) alpha_x) / m_pp
+        api = (zpi - (mr * aci - mi * acr)) * inv;
+    } else if (mcc > 0.0) {
+        acr = zcr / mcc;
+        aci = zci / mcc;
+    }
+    const bool ok = valid[p] != 0;
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    double *out = amp + ((int64_t)perm[p] * n_part + k) * 4;
+    out[0] = ok ? apr : nan;     // a_1
+    out[1] = ok ? acr : nan;     // a_2
+    out[2] = ok ? api : nan;     // a_3
+    out[3] = ok ? aci : nan;     // a_4
+}
+
+cudaError_t launch_amplitudes(const double *partial, const int32_t *part_seg, const int32_t *valid,
+                              const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, double *amp,
+                              cudaStream_t st)
+{
+    const dim3 grd((unsigned)((P + 127) / 128), (unsigned)n_part);
+    amplitude_kernel<<<grd, 128, 0, st>>>(partial, part_seg, valid, perm, P, P_pad, n_part, amp);
+    return cudaGetLastError();
+}
+
 int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out)
 {
     // enough blocks to fill the machine: particle tiles x partition chunks >= ~4 per SM; chunks of >= 8

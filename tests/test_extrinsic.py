@@ -1,0 +1,101 @@
+"""extrinsic amplitudes a = M^-1 N (Eq. 10) from the library against the oracle's
+4x4 solve, and the recovery of (D_L, iota, psi, phi_c) by Eq. B2-B3 (:426-440) pinned by the round trip through
+Eq. B1 (:413-420, retyped here)."""
+import math
+
+import numpy as np
+import pytest
+
+import synthetic as syn
+from paper_2407_10797_b200.extrinsic import (amplitude_constant, amplitudes_from_extrinsic,
+                                             extrinsic_from_amplitudes)
+
+
+def _b1(d_l, psi, iota, phi_c):
+    """Eq. B1 as printed (:413-420)."""
+    p = (1.0 + math.cos(iota) ** 2) / 2.0
+    a1 = (math.cos(2 * psi) * p * math.cos(phi_c) - math.sin(2 * psi) * math.cos(iota) * math.sin(phi_c)) / d_l
+    a2 = -(math.sin(2 * psi) * p * math.cos(phi_c) + math.cos(2 * psi) * math.cos(iota) * math.sin(phi_c)) / d_l
+    a3 = -(math.cos(2 * psi) * p * math.sin(phi_c) + math.sin(2 * psi) * math.cos(iota) * math.cos(phi_c)) / d_l
+    a4 = (math.sin(2 * psi) * p * math.sin(phi_c) - math.cos(2 * psi) * math.cos(iota) * math.cos(phi_c)) / d_l
+    return np.array([a1, a2, a3, a4])
+
+
+def test_b2_b3_invert_b1_inside_the_principal_branches():
+    rng = np.random.default_rng(7)
+    for _ in range(200):
+        d_l, psi = rng.uniform(0.3, 5.0), rng.uniform(-math.pi / 4, math.pi / 4)
+        iota, phi_c = rng.uniform(0.0, math.pi), rng.uniform(-math.pi / 2, math.pi / 2)
+        r = extrinsic_from_amplitudes(_b1(d_l, psi, iota, phi_c))
+        assert r["D_L"] == pytest.approx(d_l, rel=1e-10)
+        assert r["iota"] == pytest.approx(iota, abs=2e-6 / max(math.sin(iota), 1e-3))
+        # psi and phi_c become degenerate (only psi +- phi_c is fixed) as the orbit turns face-on
+        tol = 1e-7 / max(1.0 - abs(math.cos(iota)), 1e-3)
+        assert r["psi"] == pytest.approx(psi, abs=tol)
+        assert r["phi_c"] == pytest.approx(phi_c, abs=tol)
+        np.testing.assert_allclose(_b1(r["D_L"], r["psi"], r["iota"], r["phi_c"]), _b1(d_l, psi, iota, phi_c),
+                                   rtol=0, atol=1e-7 / d_l)      # iota loses half the digits near face-on
+        np.testing.assert_allclose(amplitudes_from_extrinsic(d_l, psi, iota, phi_c), _b1(d_l, psi, iota, phi_c),
+                                   rtol=0, atol=1e-15)
+
+
+def test_outside_the_principal_branches_the_recovered_set_reproduces_the_amplitudes():
+    """psi and phi_c are only defined up to the discrete symmetries of Eq. B1; whatever branch Eq. B2 picks,
+    feeding it back through Eq. B1 must give the same four amplitudes (Table I's psi = 1.2501 is outside)."""
+    rng = np.random.default_rng(8)
+    for _ in range(200):
+        d_l, psi = rng.uniform(0.3, 5.0), rng.uniform(-math.pi, math.pi)
+        iota, phi_c = rng.uniform(0.0, math.pi), rng.uniform(-math.pi, math.pi)
+        a = _b1(d_l, psi, iota, phi_c)
+        r = extrinsic_from_amplitudes(a)
+        # psi and phi_c come from two separate arctans and lose digits as the orbit turns face-on
+        tol = 1e-8 / (d_l * max(1.0 - abs(math.cos(iota)), 1e-4))
+        np.testing.assert_allclose(_b1(r["D_L"], r["psi"], r["iota"], r["phi_c"]), a, rtol=0, atol=tol)
+        assert r["D_L"] == pytest.approx(d_l, rel=1e-10) and r["iota"] == pytest.approx(iota, abs=2e-6 / max(math.sin(iota), 1e-3))
+
+
+def test_amplitude_constant_restores_metres():
+    mc, d_l_m = 30.0, 3.0e24                                   # ~100 Mpc
+    k = amplitude_constant(mc)
+    assert k < 0.0 and k == pytest.approx(-math.sqrt(5 / 24) * (30 * 4.925490947641267e-6) ** (5 / 6) / math.pi ** (2 / 3))
+    a_lib = k * _b1(d_l_m / 299792458.0, 0.3, 1.0, -0.4)
+    r = extrinsic_from_amplitudes(a_lib, chirp_mass_msun=mc)
+    assert r["D_L"] == pytest.approx(d_l_m, rel=1e-10) and r["iota"] == pytest.approx(1.0, abs=1e-8)
+
+
+@pytest.mark.gpu
+def test_amplitudes_match_the_oracle_and_recover_the_injection(orc):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2407_10797_b200 as fs
+    year = 31557600.0
+    cfg = syn.Config(14, "amp_slice", 2.5 * year, 0.0200, 0.0201, (4,), (40,), 3.5 * year, "wide")
+    # (i) noisy data, N_p = 4: a = M^-1 N of every partition against the oracle's 4x4 Cholesky solve
+    ds = syn.make_dataset(cfg, orc.template)
+    par = syn.draw_particles(cfg)
+    edges = ds.edges(4)
+    _, _, NM, flags = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par, want_NM=True)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges) as plan:
+        amp = fs.fstat_eval_amplitudes(plan, torch.as_tensor(par, device="cuda")).cpu().numpy()
+        F, Fk = fs.fstat_eval_batch(plan, torch.as_tensor(par, device="cuda"))
+        Fk = Fk.cpu().numpy()
+    assert amp.shape == (par.shape[0], 4, 4)
+    for p in range(par.shape[0]):
+        for k in range(4):
+            N, M = NM[p, k, :4], NM[p, k, 4:].reshape(4, 4)
+            F_o, a_o, _ = orc.fstat_from_NM(N, M)
+            assert np.linalg.norm(amp[p, k] - a_o) <= 1e-5 * np.linalg.norm(a_o)
+            assert 0.5 * amp[p, k] @ N == pytest.approx(Fk[p, k], rel=1e-6)       # F = a.N / 2 at the maximum
+    # (ii) zero noise, N_p = 1, at the injected parameters: the amplitudes are the injected ones (times the
+    # SNR normalisation), and Eq. B2-B3 give back an extrinsic set that reproduces them
+    ds0 = syn.make_dataset(cfg, orc.template, noise=False)
+    a_inj = syn.injection_amplitudes()
+    with fs.fstat_plan_create(ds0.freq, ds0.dw, ds0.inv_sn, ds0.edges(1)) as plan:
+        a0 = fs.fstat_eval_amplitudes(plan, torch.as_tensor(ds0.inj_params[None, :], device="cuda")).cpu().numpy()[0, 0]
+    scale = float(a0 @ a_inj / (a_inj @ a_inj))
+    assert scale > 0.0
+    np.testing.assert_allclose(a0, scale * a_inj, rtol=0, atol=1e-8 * np.linalg.norm(a0))
+    r = extrinsic_from_amplitudes(a0)
+    np.testing.assert_allclose(_b1(r["D_L"], r["psi"], r["iota"], r["phi_c"]), a0, rtol=0, atol=1e-8 * np.linalg.norm(a0))
+    assert r["iota"] == pytest.approx(0.5329, abs=1e-6)        # Table I (:257): the injected inclination
