@@ -203,6 +203,45 @@ FSTAT_API fstat_status fstat_edges_equal_bins(int64_t n_bins, int32_t n_part, in
 FSTAT_API fstat_status fstat_probe_pipe_peak(int32_t device, int32_t which, double millis,
                                              double *inst_per_s, int32_t *n_sm);
 
+/* ------------------------------------------------------------------------------------------------
+ * Particle swarm optimisation on the device (Sec. III.A; Eq. 13-14 :146-150).
+ *
+ * n_swarms independent swarms (PSO runs, :160) of n_particles each are advanced together: every iteration
+ * is "update velocities and positions -> ONE fstat_eval_batch over all particles -> update personal bests",
+ * enqueued on the caller's stream with no host synchronisation.  Settings as in the paper (:158-162): lbest
+ * ring topology (neighbours i-1, i, i+1), x ~ U[lo, hi], v ~ U[lo - x, hi - x] at the start, |v| <= v_max
+ * (in box units), inertia falling linearly from w_start to w_end over n_iter_total iterations, "let them
+ * fly": a particle outside [lo, hi] keeps moving but gets fitness -inf (its parameters are sent as NaN).
+ * Random numbers: Philox4x32-10, counter (particle, iteration, draw, 0), key = seed.
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct fstat_pso fstat_pso;      /* opaque */
+typedef struct {
+    double c1, c2;            /* acceleration constants, default 2, 2 (:162)          */
+    double v_max;             /* velocity clamp in box units, default 0.5 (:162)      */
+    double w_start, w_end;    /* inertia weight at the first / last iteration: 0.9, 0.4 */
+} fstat_pso_options;
+
+FSTAT_API void fstat_pso_default_options(fstat_pso_options *opts);
+
+/* Draw the initial swarms and evaluate them (asynchronous on cuda_stream).  lo, hi: HOST [6] box of
+ * (t_c, M_c, eta, theta, phi, e0).  The plan must outlive the fstat_pso and is used by it for every
+ * evaluation (one evaluation in flight per plan).  EINVAL for bad sizes / box / options. */
+FSTAT_API fstat_status fstat_pso_create(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
+                                        int32_t n_iter_total, const double *lo, const double *hi, uint64_t seed,
+                                        const fstat_pso_options *opts, void *cuda_stream);
+/* Advance all swarms by n_iter iterations; only enqueues work. */
+FSTAT_API fstat_status fstat_pso_iterate(fstat_pso *pso, int32_t n_iter, void *cuda_stream);
+/* Best position (physical parameters) and fitness of every swarm so far: HOST [n_swarms][6], [n_swarms].
+ * Waits for the stream. */
+FSTAT_API fstat_status fstat_pso_best(fstat_pso *pso, double *best_params_host, double *best_f_host,
+                                      void *cuda_stream);
+/* Copy of the swarm state for tests and check-pointing: HOST x, v, pbest [N][6] (unit-box coordinates),
+ * pbest_f, f_last [N], N = n_swarms * n_particles; any pointer may be NULL.  Waits for the stream. */
+FSTAT_API fstat_status fstat_pso_state(fstat_pso *pso, double *x, double *v, double *pbest, double *pbest_f,
+                                       double *f_last, void *cuda_stream);
+FSTAT_API int32_t fstat_pso_iterations_done(const fstat_pso *pso);
+FSTAT_API void fstat_pso_destroy(fstat_pso *pso);       /* NULL is allowed */
+
 FSTAT_API const char *fstat_status_str(fstat_status s);
 /* Human-readable reason of the most recent failing call on this plan; plan == NULL returns the
  * reason of the most recent failing fstat_plan_create on the calling thread.  Never NULL. */

@@ -18,4 +18,6 @@ from .binding import (  # noqa: F401
     fstat_plan_n_part, fstat_plan_device, fstat_plan_n_ctas, fstat_plan_launch_count,
     fstat_plan_main_kernel_ms, fstat_plan_level_bins, fstat_edges_equal_bins, fstat_probe_pipe_peak,
     fstat_status_str, fstat_last_error, library_path, load_library, EXPORTED_SYMBOLS,
+    Pso, PsoOptions, fstat_pso_default_options, fstat_pso_create, fstat_pso_iterate, fstat_pso_best,
+    fstat_pso_state, fstat_pso_iterations_done, fstat_pso_destroy,
 )

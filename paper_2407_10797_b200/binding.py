@@ -22,6 +22,8 @@ EXPORTED_SYMBOLS = (
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
+    "fstat_pso_default_options", "fstat_pso_create", "fstat_pso_iterate", "fstat_pso_best", "fstat_pso_state",
+    "fstat_pso_iterations_done", "fstat_pso_destroy",
 )
 
 
@@ -36,6 +38,12 @@ class Options(C.Structure):
     _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double), ("orbit_kappa", C.c_double),
                 ("orbit_lambda", C.c_double), ("device", C.c_int32), ("inputs_on_device", C.c_int32),
                 ("max_segment_bins", C.c_int32), ("force_level", C.c_int32), ("interp_tol", C.c_double)]
+
+
+class PsoOptions(C.Structure):
+    """fstat_pso_options of include/fstat.h."""
+    _fields_ = [("c1", C.c_double), ("c2", C.c_double), ("v_max", C.c_double), ("w_start", C.c_double),
+                ("w_end", C.c_double)]
 
 
 def library_path() -> str:
@@ -87,6 +95,20 @@ def load_library():
         L.fstat_edges_equal_bins.restype = C.c_int
         L.fstat_probe_pipe_peak.argtypes = [i32, i32, C.c_double, dp, C.POINTER(i32)]
         L.fstat_probe_pipe_peak.restype = C.c_int
+        L.fstat_pso_default_options.argtypes = [C.POINTER(PsoOptions)]
+        L.fstat_pso_default_options.restype = None
+        L.fstat_pso_create.argtypes = [C.POINTER(vp), vp, i32, i32, i32, dp, dp, C.c_uint64, C.POINTER(PsoOptions), vp]
+        L.fstat_pso_create.restype = C.c_int
+        L.fstat_pso_iterate.argtypes = [vp, i32, vp]
+        L.fstat_pso_iterate.restype = C.c_int
+        L.fstat_pso_best.argtypes = [vp, dp, dp, vp]
+        L.fstat_pso_best.restype = C.c_int
+        L.fstat_pso_state.argtypes = [vp, dp, dp, dp, dp, dp, vp]
+        L.fstat_pso_state.restype = C.c_int
+        L.fstat_pso_iterations_done.argtypes = [vp]
+        L.fstat_pso_iterations_done.restype = i32
+        L.fstat_pso_destroy.argtypes = [vp]
+        L.fstat_pso_destroy.restype = None
         L.fstat_status_str.argtypes = [C.c_int]
         L.fstat_status_str.restype = C.c_char_p
         L.fstat_last_error.argtypes = [vp]
@@ -340,3 +362,88 @@ def fstat_status_str(status: int) -> str:
 def fstat_last_error(plan: Optional[Plan] = None) -> str:
     h = plan._h if (plan is not None and plan._h) else None
     return load_library().fstat_last_error(h).decode()
+
+
+# ------------------------------------------------------------------------------------------ device PSO
+class Pso:
+    """Owner of one ``fstat_pso*`` (device-resident swarms bound to a Plan)."""
+
+    def __init__(self, handle: int, plan: Plan, n_swarms: int, n_particles: int):
+        self._h = C.c_void_p(handle)
+        self.plan, self.n_swarms, self.n_particles = plan, int(n_swarms), int(n_particles)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            load_library().fstat_pso_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def fstat_pso_default_options(**kw) -> PsoOptions:
+    o = PsoOptions()
+    load_library().fstat_pso_default_options(C.byref(o))
+    for k, v in kw.items():
+        setattr(o, k, v)
+    return o
+
+
+def fstat_pso_create(plan: Plan, n_swarms: int, n_particles: int, n_iter_total: int, lo, hi, seed: int = 0,
+                     opts: Optional[PsoOptions] = None, stream=None) -> Pso:
+    lo = np.ascontiguousarray(lo, dtype=np.float64).reshape(6)
+    hi = np.ascontiguousarray(hi, dtype=np.float64).reshape(6)
+    out = C.c_void_p()
+    dp = C.POINTER(C.c_double)
+    st = load_library().fstat_pso_create(C.byref(out), plan.handle, int(n_swarms), int(n_particles), int(n_iter_total),
+                                         lo.ctypes.data_as(dp), hi.ctypes.data_as(dp), C.c_uint64(int(seed)),
+                                         C.byref(opts) if opts is not None else None, _stream_ptr(stream))
+    if st != 0:
+        raise FstatError(st, "fstat_pso_create", fstat_last_error(plan))
+    return Pso(out.value, plan, n_swarms, n_particles)
+
+
+def fstat_pso_iterate(pso: Pso, n_iter: int, stream=None) -> None:
+    st = load_library().fstat_pso_iterate(pso._h, int(n_iter), _stream_ptr(stream))
+    if st != 0:
+        raise FstatError(st, "fstat_pso_iterate", fstat_last_error(pso.plan))
+
+
+def fstat_pso_best(pso: Pso, stream=None) -> Tuple[np.ndarray, np.ndarray]:
+    bp, bf = np.empty((pso.n_swarms, 6)), np.empty(pso.n_swarms)
+    dp = C.POINTER(C.c_double)
+    st = load_library().fstat_pso_best(pso._h, bp.ctypes.data_as(dp), bf.ctypes.data_as(dp), _stream_ptr(stream))
+    if st != 0:
+        raise FstatError(st, "fstat_pso_best")
+    return bp, bf
+
+
+def fstat_pso_state(pso: Pso, stream=None):
+    """(x, v, pbest [N][6], pbest_f, f_last [N]) host copies."""
+    n = pso.n_swarms * pso.n_particles
+    x, v, pb = np.empty((n, 6)), np.empty((n, 6)), np.empty((n, 6))
+    pf, fl = np.empty(n), np.empty(n)
+    dp = C.POINTER(C.c_double)
+    st = load_library().fstat_pso_state(pso._h, x.ctypes.data_as(dp), v.ctypes.data_as(dp), pb.ctypes.data_as(dp),
+                                        pf.ctypes.data_as(dp), fl.ctypes.data_as(dp), _stream_ptr(stream))
+    if st != 0:
+        raise FstatError(st, "fstat_pso_state")
+    return x, v, pb, pf, fl
+
+
+def fstat_pso_iterations_done(pso: Pso) -> int:
+    return int(load_library().fstat_pso_iterations_done(pso._h))
+
+
+def fstat_pso_destroy(pso: Optional[Pso]) -> None:
+    if pso is not None:
+        pso.close()
