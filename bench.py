@@ -121,6 +121,8 @@ def parse_args():
     ap.add_argument("--force-level", type=int, default=-2, help="plan option force_level (-2 automatic stride)")
     ap.add_argument("--max-segment-bins", type=int, default=0, help="plan option max_segment_bins (0 automatic)")
     ap.add_argument("--interp-tol", type=float, default=1.0, help="plan option interp_tol")
+    ap.add_argument("--pso", type=int, default=0, metavar="ITERS",
+                    help="also time ITERS iterations of the device PSO (row f1) on this plan: swarms of 128 particles")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
     return ap.parse_args()
@@ -363,6 +365,25 @@ def run_ours(args):
                    "call": "fstat_eval_batch_host (pinned host params in; F and F_k out)"},
            "gpu_launches": int(launches_timed),
            "clocks": clk, "roofline": roofline}
+    if args.pso > 0:
+        # row f1: ITERS iterations of the device PSO (update -> fstat_eval_batch -> personal bests) enqueued back to
+        # back on the stream, no host synchronisation in between; box = the particle ranges of the workload
+        lo, hi = par_np.min(axis=0), par_np.max(axis=0)
+        n_sw = max(P // 128, 1)
+        pso = fs.fstat_pso_create(plan, n_sw, 128, args.pso, lo, hi, seed=1, stream=stream)
+        fs.fstat_pso_iterate(pso, 3, stream)
+        torch.cuda.synchronize()
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        fs.fstat_pso_iterate(pso, args.pso, stream)
+        p1.record(stream)
+        torch.cuda.synchronize()
+        ms_it = p0.elapsed_time(p1) / args.pso
+        _, bf = fs.fstat_pso_best(pso, stream)
+        out["pso"] = {"swarms": n_sw, "particles_per_swarm": 128, "iterations": args.pso, "ms_per_iteration": ms_it,
+                      "template_bins_per_s": float(n_sw * 128) * ds.n_bins / (ms_it * 1e-3),
+                      "overhead_vs_eval_step": ms_it / ms_step - 1.0, "best_F_max": float(bf.max())}
+        fs.fstat_pso_destroy(pso)
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, ds, n_part, args.cpu_sample)
     fs.fstat_plan_destroy(plan)
