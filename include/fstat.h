@@ -170,7 +170,8 @@ FSTAT_API void fstat_plan_destroy(fstat_plan *plan);
 FSTAT_API int64_t fstat_plan_n_bins(const fstat_plan *plan);
 FSTAT_API int32_t fstat_plan_n_part(const fstat_plan *plan);
 FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
-/* Number of (particle-group, segment) work items = CTAs the main kernel launches for P particles. */
+/* Number of CTAs the interpolating main kernel launches for P particles: particle groups of 128 x chunks of
+ * consecutive segments (a chunk is one segment unless the partitions are short). */
 FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
 /* Number of CUDA kernels the fstat_eval_batch / fstat_eval_batch_host calls on this plan have launched so
  * far (per call: particle ranking, prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and

@@ -161,6 +161,15 @@ int64_t auto_segment_len(const fstat_plan *pl, int32_t n_groups)
     return len;
 }
 
+// short segments (narrow partitions): one CTA of the interpolating kernel walks ~4096 bins' worth of consecutive
+// segments, so that the five start-up node evaluations are shared
+int32_t segs_per_cta(int64_t n_bins, int64_t n_seg)
+{
+    const int64_t avg = n_bins / (n_seg > 0 ? n_seg : 1);
+    const int64_t g = avg > 0 ? (4096 + avg / 2) / avg : 1;
+    return (int32_t)(g < 1 ? 1 : (g > 8 ? 8 : g));
+}
+
 int64_t n_segments_for(const fstat_plan *pl, int32_t n_groups)
 {
     std::vector<int32_t> seg_edge, part_seg;
@@ -511,7 +520,9 @@ int64_t fstat_plan_n_ctas(const fstat_plan *pl, int64_t P)
 {
     if (!pl || P < 1) return 0;
     const int64_t n_groups = (P + kThreads - 1) / kThreads;
-    return n_groups * n_segments_for(pl, (int32_t)n_groups);
+    const int64_t n_seg = n_segments_for(pl, (int32_t)n_groups);
+    const int64_t g = segs_per_cta(pl->n_bins, n_seg);
+    return n_groups * ((n_seg + g - 1) / g);
 }
 
 fstat_status fstat_plan_level_bins(fstat_plan *pl, int64_t *bins_out, int64_t *subblocks_out)
@@ -602,6 +613,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.P_pad = P_pad;
     fa.n_groups = (int32_t)n_groups;
     fa.n_seg = pl->n_seg;
+    fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
     fa.df = pl->df;
     fa.orb = pl->orb;
     MainArgs a;

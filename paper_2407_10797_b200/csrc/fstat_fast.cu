@@ -288,32 +288,47 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
 
     const int tid = threadIdx.x;
     const int grp = blockIdx.x % a.n_groups;
-    const int seg = blockIdx.x / a.n_groups;
-    const int lvl = a.level[(int64_t)grp * a.n_seg + seg];
-    if (lvl < 0) return;                                     // CTA-uniform: left to the direct kernel
-    const int sh = kLevel0Shift + lvl;
-    const double rS = 1.0 / (double)(1 << sh);
+    const int chunk = blockIdx.x / a.n_groups;
+    const int seg_begin = chunk * a.segs_per_cta, seg_end = min(a.n_seg, seg_begin + a.segs_per_cta);
+    const int8_t *level = a.level + (int64_t)grp * a.n_seg;
     const int64_t p = (int64_t)grp * kThreads + tid;         // < P_pad by construction
     const double *cf = a.coef + p;
-
-    const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
-    const int t_first = lo >> kFastTileShift;
-    const int n_tiles = ((hi - 1) >> kFastTileShift) - t_first + 1;
     const double2 *dwp = reinterpret_cast<const double2 *>(a.dwp);
 
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kFastStages; ++s) mbar_init(&sm.full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();                                         // barriers initialised before anyone waits
+    int g0 = 0;                                              // tiles consumed so far by this CTA (ring position)
+
+  // A CTA walks a chunk of consecutive segments.  Consecutive segments with the same stride form a RUN: the
+  // data tiles, the node ring and the Gram-table pointer carry on across the partition edges inside a run
+  // (sub-blocks are cut there and the eight sums are flushed per segment); segments left to the direct
+  // kernel (level < 0) are skipped.
+  for (int seg = seg_begin; seg < seg_end;) {
+    const int lvl = level[seg];
+    if (lvl < 0) { ++seg; continue; }                        // CTA-uniform
+    int run_end = seg + 1;
+    while (run_end < seg_end && level[run_end] == lvl) ++run_end;
+    const int sh = kLevel0Shift + lvl;
+    const double rS = 1.0 / (double)(1 << sh);
+
+    const int lo = a.seg_edge[seg], hi = a.seg_edge[run_end];
+    const int t_first = lo >> kFastTileShift;
+    const int n_tiles = ((hi - 1) >> kFastTileShift) - t_first + 1;
+
     auto issue_tile = [&](int t) {                           // t = tile number relative to t_first
-        const int slot = t % kFastStages;
+        const int slot = (g0 + t) % kFastStages;
         const int b0 = max(lo, (t_first + t) << kFastTileShift), b1 = min(hi, (t_first + t + 1) << kFastTileShift);
         const uint32_t bytes = (uint32_t)(b1 - b0) * (uint32_t)sizeof(double2);
         mbar_expect_tx(&sm.full[slot], bytes);
         tma_load_1d(&sm.tile[slot][b0 & (kFastTile - 1)], dwp + b0, bytes, &sm.full[slot]);
     };
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < kFastStages; ++s) mbar_init(&sm.full[s], 1);
-        mbar_fence_init();
+    __syncthreads();                                         // every thread has left the previous run's tiles
+    if (tid == 0)
         for (int s = 0; s < kFastStages && s < n_tiles; ++s) issue_tile(s);
-    }
 
     // linear phase term 2 pi f t_c in quarter turns: per-bin advance, reduced mod 4
     const double c0 = cf[0];
@@ -334,7 +349,7 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
         }
     }
-    __syncthreads();                                         // barriers initialised before anyone waits
+    int m_have = m + 2;                                      // highest node in the ring
 
     double acc[kNAcc];
 #pragma unroll
@@ -342,14 +357,17 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
 
     const double *gram = a.gram[lvl] + (int64_t)a.seg_gbase[seg * kNLevels + lvl] * kNGram;
     int cur_tile = -1;
+    int cur_seg = seg;
+    int seg_hi = a.seg_edge[cur_seg + 1];
     int j0 = lo;
     while (j0 < hi) {
         const int node0 = m << sh;                           // bin of node "0" of this interval
-        const int j1 = min(hi, node0 + (1 << sh));
+        const int j1 = min(seg_hi, node0 + (1 << sh));       // sub-block = node interval cut at the segment edge
         const int s_base = (m - 2 + kWinNodes) % kWinNodes;  // ring slot of node m-2
-        // ---- new node m+3
-        double fnode;
-        {
+        // ---- new node m+3 (unless this sub-block continues an interval already entered)
+        const double fnode = a.node[((int64_t)kNodePad + ((int64_t)m << lvl)) * kTabW + T_F];
+        if (m + 3 > m_have) {
+            m_have = m + 3;
             double c[kNCoef];
             load_coef(cf, a.P_pad, c);
             const double2 *row = reinterpret_cast<const double2 *>(
@@ -359,7 +377,6 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             const int slot = (m + 3 + kWinNodes) % kWinNodes;
             sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
             sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
-            fnode = a.node[((int64_t)kNodePad + ((int64_t)m << lvl)) * kTabW + T_F];
         }
         // ---- carrier phase: economised cubic + exact linear term, as forward differences
         double t, D1, D2, D3;
@@ -389,9 +406,9 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
                 if (tid == 0 && cur_tile + kFastStages < n_tiles) issue_tile(cur_tile + kFastStages);
             }
             cur_tile = tl;
-            mbar_wait(&sm.full[tl % kFastStages], (uint32_t)((tl / kFastStages) & 1));
+            mbar_wait(&sm.full[(g0 + tl) % kFastStages], (uint32_t)(((g0 + tl) / kFastStages) & 1));
         }
-        const double2 *tp = &sm.tile[tl % kFastStages][j0 & (kFastTile - 1)];
+        const double2 *tp = &sm.tile[(g0 + tl) % kFastStages][j0 & (kFastTile - 1)];
         const int nb = j1 - j0;
 
         // ---- per bin: q = dw' e^{+i Phi}; running sums A_0..A_3.  The carrier e^{+i Phi_i} is carried by a
@@ -505,13 +522,19 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             acc[4] += mpp; acc[5] += mcc; acc[6] += mre; acc[7] += mim;
             gram += kNGram;
         }
-        j0 = j1;
-        ++m;
-    }
-
-    double *out = a.partial + ((int64_t)seg * kNAcc) * a.P_pad + p;
+        if (j1 == seg_hi) {                                  // segment finished: flush its eight sums
+            double *out = a.partial + ((int64_t)cur_seg * kNAcc) * a.P_pad + p;
 #pragma unroll
-    for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
+            for (int j = 0; j < kNAcc; ++j) { out[(int64_t)j * a.P_pad] = acc[j]; acc[j] = 0.0; }
+            ++cur_seg;
+            if (cur_seg < run_end) seg_hi = a.seg_edge[cur_seg + 1];
+        }
+        if (j1 == node0 + (1 << sh)) ++m;                    // node interval finished
+        j0 = j1;
+    }
+    g0 += n_tiles;
+    seg = run_end;
+  }
 }
 
 cudaError_t fast_kernel_configure()
@@ -522,7 +545,8 @@ cudaError_t fast_kernel_configure()
 
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st)
 {
-    const int64_t n_cta = (int64_t)a.n_groups * a.n_seg;
+    const int64_t n_chunks = (a.n_seg + a.segs_per_cta - 1) / a.segs_per_cta;
+    const int64_t n_cta = (int64_t)a.n_groups * n_chunks;
     fstat_fast_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);
     return cudaGetLastError();
 }

@@ -113,6 +113,7 @@ struct FastArgs {
     int64_t P_pad;
     int32_t n_groups;
     int32_t n_seg;
+    int32_t segs_per_cta;         // consecutive segments one CTA walks (tiles, node ring carried across their edges)
     double df;
     OrbitCoef orb;
 };

@@ -65,7 +65,7 @@ struct Box { double lo[kDim], hi[kDim]; };
 __global__ void pso_init_kernel(int32_t n, uint64_t seed, double vmax, Box box, double *__restrict__ x,
                                 double *__restrict__ v, double *__restrict__ params)
 {
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= n) return;
     double u[12], xx[kDim];
     draw12((uint32_t)g, 0u, seed, u);
@@ -82,7 +82,7 @@ __global__ void pso_init_kernel(int32_t n, uint64_t seed, double vmax, Box box, 
 __global__ void pso_first_best_kernel(int32_t n, const double *__restrict__ x, const double *__restrict__ F,
                                       double *__restrict__ pbest, double *__restrict__ pbest_f)
 {
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= n) return;
 #pragma unroll
     for (int d = 0; d < kDim; ++d) pbest[g * kDim + d] = x[g * kDim + d];
@@ -94,13 +94,14 @@ __global__ void pso_step_kernel(int32_t n, int32_t n_particles, uint32_t it, uin
                                 const double *__restrict__ pbest, const double *__restrict__ pbest_f,
                                 double *__restrict__ params)
 {
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= n) return;
-    const int sw = g / n_particles, i = g - sw * n_particles;
+    const int64_t sw = g / n_particles;
+    const int i = (int)(g - sw * n_particles);
     // lbest: best personal best among the ring neighbours i-1, i, i+1 (first maximum in that order)
-    const int left = sw * n_particles + (i + n_particles - 1) % n_particles;
-    const int right = sw * n_particles + (i + 1) % n_particles;
-    int lb = left;
+    const int64_t left = sw * n_particles + (i + n_particles - 1) % n_particles;
+    const int64_t right = sw * n_particles + (i + 1) % n_particles;
+    int64_t lb = left;
     double fb = pbest_f[left];
     if (pbest_f[g] > fb) { fb = pbest_f[g]; lb = g; }
     if (pbest_f[right] > fb) { fb = pbest_f[right]; lb = right; }
@@ -125,7 +126,7 @@ __global__ void pso_step_kernel(int32_t n, int32_t n_particles, uint32_t it, uin
 __global__ void pso_update_best_kernel(int32_t n, const double *__restrict__ x, const double *__restrict__ F,
                                        double *__restrict__ pbest, double *__restrict__ pbest_f)
 {
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= n) return;
     if (F[g] > pbest_f[g]) {
         pbest_f[g] = F[g];
@@ -147,7 +148,7 @@ __global__ void __launch_bounds__(128) pso_swarm_best_kernel(int32_t n_particles
     double f = -INFINITY;
     int idx = 0x7fffffff;
     for (int i = tid; i < n_particles; i += 128) {
-        const double fi = pbest_f[sw * n_particles + i];
+        const double fi = pbest_f[(int64_t)sw * n_particles + i];
         if (fi > f || (fi == f && i < idx)) { f = fi; idx = i; }
     }
     sf[tid] = f; si[tid] = idx;
@@ -165,7 +166,7 @@ __global__ void __launch_bounds__(128) pso_swarm_best_kernel(int32_t n_particles
         const double *pb = pbest + ((int64_t)sw * n_particles + i) * kDim;
         best_f[sw] = sf[0];
         for (int d = 0; d < kDim; ++d)
-            best_params[sw * kDim + d] = __dadd_rn(box.lo[d], __dmul_rn(pb[d], __dsub_rn(box.hi[d], box.lo[d])));
+            best_params[(int64_t)sw * kDim + d] = __dadd_rn(box.lo[d], __dmul_rn(pb[d], __dsub_rn(box.hi[d], box.lo[d])));
     }
 }
 
