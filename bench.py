@@ -35,7 +35,8 @@ UNIT = "template-bins/s"
 # FP64-pipe instructions (DFMA + DMUL + DADD + DSETP) of the two main kernels, per unit of work (DESIGN.md
 # "Roofline").  Per template-bin: SASS count of the per-bin loops, re-counted by tests/test_cabi.py.  Per node
 # interval and per work item: EXECUTED counts measured with ncu (sm__inst_executed_pipe_fp64.sum at forced
-# strides 8 / 512 and two segment lengths, profiles/r1_v4.md: 19 / 712 / 1105 reproduce all three totals exactly).
+# strides 8 / 512 and two segment lengths, profiles/r1_v5.md: 19 / 712 / 1105 reproduce all three totals exactly;
+# "work item" = one run of consecutive segments walked by one CTA).
 #   interpolating kernel: per template-bin (inner loop), per node interval of a particle (full-model node
 #   evaluation, interpolation coefficients, Gram products), per work item of a particle (three extra nodes);
 #   direct kernel: per template-bin.  2 flop each by the usual FMA convention.
@@ -47,7 +48,7 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
 STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from
 # the ncu --set full capture summarised in profiles/ (None until that capture exists for the current kernel)
-NCU_DRAM_BYTES_PER_LAUNCH = 188.0e6     # profiles/r1_v4.md: 32.9 MB read + 155.2 MB written (config 1)
+NCU_DRAM_BYTES_PER_LAUNCH = 174.3e6     # profiles/r1_v5.md: 31.6 MB read + 142.7 MB written (config 1)
 
 
 # ------------------------------------------------------------------------------------------ utilities
