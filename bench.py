@@ -35,20 +35,20 @@ UNIT = "template-bins/s"
 # FP64-pipe instructions (DFMA + DMUL + DADD + DSETP) of the two main kernels, per unit of work (DESIGN.md
 # "Roofline").  Per template-bin: SASS count of the per-bin loops, re-counted by tests/test_cabi.py.  Per node
 # interval and per work item: EXECUTED counts measured with ncu (sm__inst_executed_pipe_fp64.sum at forced
-# strides 8 / 512 and two segment lengths, profiles/r1_v5.md: 19 / 712 / 1105 reproduce all three totals exactly;
+# strides 8 / 512 and two segment lengths, profiles/r1_v6.md: 19 / 736 / 1105 (+ 17 per segment, neglected) reproduce all three totals exactly;
 # "work item" = one run of consecutive segments walked by one CTA).
 #   interpolating kernel: per template-bin (inner loop), per node interval of a particle (full-model node
 #   evaluation, interpolation coefficients, Gram products), per work item of a particle (three extra nodes);
 #   direct kernel: per template-bin.  2 flop each by the usual FMA convention.
 FAST_FP64_PER_BIN = 19.0
-FAST_FP64_PER_INTERVAL = 712.0
+FAST_FP64_PER_INTERVAL = 736.0
 FAST_FP64_PER_ITEM = 1105.0
 DIRECT_FP64_PER_BIN = 263.0
 NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
 STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from
 # the ncu --set full capture summarised in profiles/ (None until that capture exists for the current kernel)
-NCU_DRAM_BYTES_PER_LAUNCH = 174.3e6     # profiles/r1_v5.md: 31.6 MB read + 142.7 MB written (config 1)
+NCU_DRAM_BYTES_PER_LAUNCH = 223.5e6     # profiles/r1_v6.md: 31.8 MB read + 191.7 MB written (config 1)
 
 
 # ------------------------------------------------------------------------------------------ utilities
@@ -330,7 +330,7 @@ def run_ours(args):
     n_groups = (P + 127) // 128
     # algorithmic HBM bytes of one launch: every particle group streams the folded data (16 B/bin) once, reads
     # one 192-B node row and one 80-B Gram matrix per node interval, and writes 8 partial sums per work item
-    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * float(lvl_sub.sum()) + 64.0 * 128.0 * n_items
+    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * float(lvl_sub.sum()) + 80.0 * 128.0 * n_items
     roofline = {"bound": "alu", "kernel": "fstat_fast_kernel (+ fstat_main_kernel for the work items it leaves)",
                 "pipe": "fp64", "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,

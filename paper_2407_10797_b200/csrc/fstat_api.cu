@@ -584,7 +584,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
     CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)P_pad * kNCoef));
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)P_pad));
-    CU_TRY(pl, grow(&pl->d_partial, &pl->partial_cap, (size_t)pl->n_seg * kNAcc * (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_partial, &pl->partial_cap, (size_t)pl->n_seg * kNPartial * (size_t)P_pad));
     CU_TRY(pl, grow(&pl->d_level, &pl->level_cap, (size_t)pl->n_seg * (size_t)n_groups));
     CU_TRY(pl, grow(&pl->d_direct, &pl->direct_cap, (size_t)pl->n_seg * (size_t)n_groups + 1));
     {

@@ -359,6 +359,11 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
     int cur_tile = -1;
     int cur_seg = seg;
     int seg_hi = a.seg_edge[cur_seg + 1];
+    // Basis of the segment's sums (hazard H3): (u_+, u_x - c u_+) with c = T'_x / T'_+ at the segment's first
+    // node.  F is invariant under it; over a narrow partition u_x is nearly c u_+, and accumulating the small
+    // remainder directly keeps m_cc - |m_pc|^2 / m_pp from cancelling (rounding / sqrt(det) instead of / det).
+    bool seg_start = true;
+    double c_re = 0.0, c_im = 0.0;
     int j0 = lo;
     while (j0 < hi) {
         const int node0 = m << sh;                           // bin of node "0" of this interval
@@ -482,6 +487,19 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
 #pragma unroll
             for (int q = 0; q < 4; ++q) yci[q] += yref;
         }
+        if (seg_start) {
+            seg_start = false;
+            const double n2 = fma(ypr[1], ypr[1], ypi[1] * ypi[1]), x2 = fma(ycr[1], ycr[1], yci[1] * yci[1]);
+            const bool use = n2 > 1e-6 * x2;                                  // else T'_+ ~ 0 there: keep u_x
+            const double inv = use ? 1.0 / n2 : 0.0;
+            c_re = fma(ycr[1], ypr[1], yci[1] * ypi[1]) * inv;               // T'_x conj(T'_+) / |T'_+|^2
+            c_im = fma(yci[1], ypr[1], -ycr[1] * ypi[1]) * inv;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {                                        // node values of T'_x - c T'_+
+            ycr[q] -= fma(c_re, ypr[q], -c_im * ypi[q]);
+            yci[q] -= fma(c_re, ypi[q], c_im * ypr[q]);
+        }
         // ---- z_P += sum_n conj(c^P_n) A_n
         const double U = (double)(j1 - node0);
         {
@@ -523,9 +541,12 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             gram += kNGram;
         }
         if (j1 == seg_hi) {                                  // segment finished: flush its eight sums
-            double *out = a.partial + ((int64_t)cur_seg * kNAcc) * a.P_pad + p;
+            double *out = a.partial + ((int64_t)cur_seg * kNPartial) * a.P_pad + p;
 #pragma unroll
             for (int j = 0; j < kNAcc; ++j) { out[(int64_t)j * a.P_pad] = acc[j]; acc[j] = 0.0; }
+            out[(int64_t)8 * a.P_pad] = c_re;
+            out[(int64_t)9 * a.P_pad] = c_im;
+            seg_start = true;
             ++cur_seg;
             if (cur_seg < run_end) seg_hi = a.seg_edge[cur_seg + 1];
         }

@@ -40,6 +40,7 @@ enum TabCol : int {
 
 constexpr int kNCoef = 20;   // per-particle coefficients: c0..c9, a0, k[3], u[3], v[3]
 constexpr int kNAcc = 8;     // z_+ (re, im), z_x (re, im), m_pp, m_cc, m_pc (re, im)
+constexpr int kNPartial = 10;   // per (segment, particle): the eight sums in the basis (u_+, u_x - c u_+), then c (re, im)
 constexpr int kThreads = 128;    // particles per CTA of the main kernel (one thread = one particle)
 constexpr int kTileBins = 64;    // bins per TMA tile (64 * 24 * 8 B = 12 KiB)
 constexpr int kStages = 3;       // TMA ring depth
@@ -87,7 +88,7 @@ struct MainArgs {
     const int32_t *direct_list;   // work items (group * n_seg + segment) left to the direct kernel ...
     const int32_t *direct_count;  // ... and how many (both written by schedule_kernel)
     int32_t max_ctas;             // persistent grid size
-    double *partial;          // [n_seg][kNAcc][P_pad]
+    double *partial;          // [n_seg][kNPartial][P_pad]
     int64_t P_pad;
     int32_t P;
     int32_t n_groups;
@@ -109,7 +110,7 @@ struct FastArgs {
     const int32_t *seg_edge;      // [n_seg + 1]
     const int32_t *seg_gbase;     // [n_seg][kNLevels] index of the segment's first sub-block in gram[level]
     const int8_t *level;          // [n_groups][n_seg]
-    double *partial;              // [n_seg][kNAcc][P_pad]
+    double *partial;              // [n_seg][kNPartial][P_pad]
     int64_t P_pad;
     int32_t n_groups;
     int32_t n_seg;

@@ -291,9 +291,11 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
         }
         g0 += n_tiles;
 
-        double *out = a.partial + ((int64_t)seg * kNAcc) * a.P_pad + p;
+        double *out = a.partial + ((int64_t)seg * kNPartial) * a.P_pad + p;
 #pragma unroll
         for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
+        out[(int64_t)8 * a.P_pad] = 0.0;                   // plain basis (u_+, u_x): c = 0
+        out[(int64_t)9 * a.P_pad] = 0.0;
     }
 }
 
@@ -362,6 +364,28 @@ cudaError_t launch_template(const double *table, const double *coef, int64_t P_p
 // =================================================================================================
 constexpr int kEpiX = 32, kEpiY = 8;
 
+// Add the sums of segment s (stored in its own basis (u_+, u_x - c_s u_+)) to v in the basis with constant
+// c*:  u_x - c* u_+ = (u_x - c_s u_+) + D u_+,  D = c_s - c*, so
+//   z~* = z~ + conj(D) z_+,   m~*_pc = m~_pc + conj(D) m_pp,   m~*_cc = m~_cc + 2 Re(D m~_pc) + |D|^2 m_pp.
+// D is a small difference of nearby ratios: nothing cancels here.
+__device__ __forceinline__ void add_segment(const double *__restrict__ partial, int s, int64_t P_pad, int64_t p,
+                                            double cs_r, double cs_i, double (&v)[kNAcc])
+{
+    const double *src = partial + ((int64_t)s * kNPartial) * P_pad + p;
+    double t[kNPartial];
+#pragma unroll
+    for (int j = 0; j < kNPartial; ++j) t[j] = src[(int64_t)j * P_pad];
+    const double dr = t[8] - cs_r, di = t[9] - cs_i;
+    v[0] += t[0];
+    v[1] += t[1];
+    v[2] += fma(dr, t[0], fma(di, t[1], t[2]));
+    v[3] += fma(dr, t[1], fma(-di, t[0], t[3]));
+    v[4] += t[4];
+    v[5] += fma(fma(dr, dr, di * di), t[4], fma(2.0, fma(dr, t[6], -di * t[7]), t[5]));
+    v[6] += fma(dr, t[4], t[6]);
+    v[7] += fma(-di, t[4], t[7]);
+}
+
 __device__ __forceinline__ double two_F(const double (&v)[kNAcc])
 {
     const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
@@ -414,11 +438,9 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
                 double v[kNAcc];
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
-                for (int s = s0; s < s1; ++s) {
-                    const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
-#pragma unroll
-                    for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
-                }
+                const double cs_r = partial[((int64_t)s0 * kNPartial + 8) * P_pad + p];   // common basis: the
+                const double cs_i = partial[((int64_t)s0 * kNPartial + 9) * P_pad + p];   // first segment's
+                for (int s = s0; s < s1; ++s) add_segment(partial, s, P_pad, p, cs_r, cs_i, v);
                 fk = ok ? 0.5 * two_F(v) : ninf;
                 if (ok) fsum += fk;
             }
@@ -429,12 +451,11 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
                 double v[kNAcc];
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
-                if (live)
-                    for (int s = s0 + ty; s < s1; s += kEpiY) {
-                        const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
-#pragma unroll
-                        for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
-                    }
+                if (live) {
+                    const double cs_r = partial[((int64_t)s0 * kNPartial + 8) * P_pad + p];
+                    const double cs_i = partial[((int64_t)s0 * kNPartial + 9) * P_pad + p];
+                    for (int s = s0 + ty; s < s1; s += kEpiY) add_segment(partial, s, P_pad, p, cs_r, cs_i, v);
+                }
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) sV[SEG_PAR ? ty : 0][j][tx] = v[j];
                 __syncthreads();
@@ -505,11 +526,10 @@ __global__ void __launch_bounds__(128) amplitude_kernel(const double *__restrict
     double v[kNAcc];
 #pragma unroll
     for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
-    for (int s = part_seg[k]; s < part_seg[k + 1]; ++s) {
-        const double *src = partial + ((int64_t)s * kNAcc) * P_pad + p;
-#pragma unroll
-        for (int j = 0; j < kNAcc; ++j) v[j] += src[(int64_t)j * P_pad];
-    }
+    const int s_first = part_seg[k];
+    const double cs_r = partial[((int64_t)s_first * kNPartial + 8) * P_pad + p];
+    const double cs_i = partial[((int64_t)s_first * kNPartial + 9) * P_pad + p];
+    for (int s = s_first; s < part_seg[k + 1]; ++s) add_segment(partial, s, P_pad, p, cs_r, cs_i, v);
     const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
     const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
     double apr = 0.0, api = 0.0, acr = 0.0, aci = 0.0;
@@ -523,6 +543,9 @@ __global__ void __launch_bounds__(128) amplitude_kernel(const double *__restrict
         }
         apr = (zpr - (mr * acr + mi * aci)) * inv;                          // alpha_+ = (z_+ - conj(m_pc) alpha_x) / m_pp
         api = (zpi - (mr * aci - mi * acr)) * inv;
+        // the sums are in the basis (u_+, u_x - c* u_+): h = alpha~_+ u_+ + alpha_x (u_x - c* u_+)
+        apr -= cs_r * acr - cs_i * aci;
+        api -= cs_r * aci + cs_i * acr;
     } else if (mcc > 0.0) {
         acr = zcr / mcc;
         aci = zci / mcc;

@@ -48,7 +48,7 @@ def fast_kernel_counts(lib_path: str):
     """FP64 instructions per template-bin of fstat_fast_kernel: its per-bin loops are the innermost loops
     that read the folded data from shared memory (one LDS.128 per bin); every variant the compiler emits
     must have the same FP64 count per bin.  (Per node interval and per work item the executed counts are
-    measured with ncu, profiles/r1_v5.md: rare paths and loop peeling make the static count ambiguous.)"""
+    measured with ncu, profiles/r1_v6.md: rare paths and loop peeling make the static count ambiguous.)"""
     ins = kernel_instructions(lib_path, "fstat_fast_kernel")
     per_bin, per_bin_all = set(), []
     all_loops = loops(ins)

@@ -137,7 +137,7 @@ def test_product_and_oracle_share_no_code():
 def test_bench_fp64_instruction_model_matches_the_sass(fs):
     """bench.py's roofline counts FP64-pipe instructions per template-bin; the same numbers re-derived here
     from the SASS of the built library (tests/sass_util.py).  Per node interval / work item the constants are
-    ncu-measured executed counts (profiles/r1_v5.md)."""
+    ncu-measured executed counts (profiles/r1_v6.md)."""
     import importlib.util
     import sass_util
     spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
