@@ -25,6 +25,10 @@
  * closed forms, central differences and 40-digit mpmath spot checks of the phase; P7 orbit against
  * exact Kepler ellipses and arm-length formula; P8 long-wavelength limit and polarisation-rotation
  * invariance of the response; P9 a time-domain simulation of the four links + TDI delays.
+ * Row f2 (the paper's own segment limits): oracle_template_band below + band_edges /
+ * fstat_bands in oracle.py; pins in tests/test_oracle_bands.py: P11 the band limits against the textbook
+ * 2PN time-to-coalescence series and against the power of a time-domain simulated signal, P12 edges on
+ * hand-computed integers, P13 zero-noise in-band 2F = <h,h>.
  * PARITY UNPINNED (stated in DESIGN.md): the numerical values of alpha_k / phi_e against the
  * authors' code (textbook TaylorF2 values are used, A1/A3) and the paper's absolute SNR values
  * (their PSD file and orbit phase are not available, P10/T8).
@@ -212,6 +216,30 @@ void oracle_template(const double *par, int64_t n, const double *freq, const ora
         u_cross[2 * i]     = Tc[0] * cr - Tc[1] * ci;
         u_cross[2 * i + 1] = Tc[0] * ci + Tc[1] * cr;
     }
+}
+
+/* the paper's own outer segment limits ("the lowest and highest
+ * instantaneous frequencies occurring during the observation period in the template"): the template is
+ * in band at the bins whose stationary time t_f (Eq. 20 :220) falls inside the observation [0, T_obs].
+ * Written out as the definition, bin by bin, with no assumption that t_f is monotone:
+ *   k_lo = number of bins with t_f < 0,   k_hi = number of bins with t_f <= T_obs,
+ * so that, t_f increasing along the grid (checked by *monotone), the in-band bins are [k_lo, k_hi). */
+void oracle_template_band(const double *par, int64_t n, const double *freq, double T_obs,
+                          const oracle_options *opt, int64_t *k_lo, int64_t *k_hi, int *monotone)
+{
+    int64_t lo = 0, hi = 0;
+    int mono = 1;
+    double prev = -INFINITY;
+    for (int64_t i = 0; i < n; ++i) {
+        double psi, tf;
+        oracle_phase(par, freq[i], opt, &psi, &tf);
+        if (tf < 0.0) ++lo;
+        if (tf <= T_obs) ++hi;
+        if (!(tf > prev)) mono = 0;
+        prev = tf;
+    }
+    *k_lo = lo; *k_hi = hi;
+    if (monotone) *monotone = mono;
 }
 
 /* N^i = <d, A^i>, M^ij = <A^i, A^j> over bins [lo, hi) by direct summation (Eq. 4, 8, 9, 12):

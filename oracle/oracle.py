@@ -76,6 +76,9 @@ def lib():
                                          C.POINTER(C.c_int32)]
         L.oracle_fstat_batch.restype = C.c_int
         L.oracle_max_threads.restype = C.c_int
+        L.oracle_template_band.argtypes = [C.POINTER(C.c_double), C.c_int64, C.POINTER(C.c_double), C.c_double,
+                                           C.POINTER(Options), C.POINTER(C.c_int64), C.POINTER(C.c_int64),
+                                           C.POINTER(C.c_int)]
         _lib = L
     return _lib
 
@@ -191,6 +194,64 @@ def fstat_batch(freq, dw, inv_sn, edges, params, opt: Optional[Options] = None, 
     if want_NM:
         return F, Fk, NM, flags
     return F, Fk
+
+
+def template_band(par, freq, T_obs: float, opt: Optional[Options] = None) -> Tuple[int, int]:
+    """Row f2: the bins [k_lo, k_hi) of ``freq`` whose stationary time t_f (Eq. 20 :220) lies in
+    the observation [0, T_obs]: k_lo = #{t_f < 0}, k_hi = #{t_f <= T_obs}, counted bin by bin."""
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    lo, hi, mono = C.c_int64(), C.c_int64(), C.c_int()
+    lib().oracle_template_band(_dp(_par(par)), freq.shape[0], _dp(freq), float(T_obs), C.byref(_opt(opt)),
+                               C.byref(lo), C.byref(hi), C.byref(mono))
+    assert mono.value == 1, "t_f is not increasing along the grid: the band is not an interval"
+    return int(lo.value), int(hi.value)
+
+
+def band_edges(k_lo: int, k_hi: int, n_bins: int, n_seg: int, lattice: int = 1) -> np.ndarray:
+    """Reading A26: the paper fixes only the number of segments and the outer limits (:122).  Here the outer
+    limits are rounded to the nearest multiple of ``lattice`` bins (half up), the band is split into n_seg
+    parts of equal length in lattice cells up to the floor, e_j = C (q_lo + floor(j (q_hi - q_lo) / n_seg)),
+    and every edge is clipped to the grid.  Plain Python integers."""
+    Cc = int(lattice)
+    q_lo, q_hi = (int(k_lo) + Cc // 2) // Cc, (int(k_hi) + Cc // 2) // Cc
+    return np.array([min(Cc * (q_lo + (j * (q_hi - q_lo)) // int(n_seg)), int(n_bins)) for j in range(int(n_seg) + 1)],
+                    dtype=np.int64)
+
+
+def fstat_bands(freq, dw, inv_sn, params, n_seg: int, lattice: int = 1, opt: Optional[Options] = None,
+                use_ld: bool = False):
+    """Row f2: the semi-coherent F-statistic with the paper's own segment limits: for every
+    particle the template is windowed to its band [k_lo, k_hi) (t_f in [0, T_obs], T_obs = 1/df) and that
+    band is cut into n_seg partitions (``band_edges``); F_k from the same inner products and 4x4 solve as
+    ``fstat_batch``; an empty partition contributes F_k = 0.  Returns F[P], Fk[P][n_seg], edges[P][n_seg+1]."""
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    dw = np.ascontiguousarray(dw, dtype=np.complex128)
+    inv_sn = np.ascontiguousarray(inv_sn, dtype=np.float64)
+    params = _par(params).reshape(-1, 6)
+    n = freq.shape[0]
+    df = (freq[-1] - freq[0]) / (n - 1)
+    P = params.shape[0]
+    F, Fk = np.zeros(P), np.zeros((P, n_seg))
+    edges = np.zeros((P, n_seg + 1), dtype=np.int64)
+    for p in range(P):
+        if not params_valid(params[p]):
+            F[p], Fk[p] = -np.inf, -np.inf
+            continue
+        k_lo, k_hi = template_band(params[p], freq, 1.0 / df, opt)
+        e = band_edges(k_lo, k_hi, n, n_seg, lattice)
+        edges[p] = e
+        if e[-1] <= e[0]:
+            continue
+        a, b = int(e[0]), int(e[-1])
+        up = np.zeros(n, dtype=np.complex128)
+        uc = np.zeros(n, dtype=np.complex128)
+        up[a:b], uc[a:b] = template(params[p], freq[a:b], opt)
+        for j in range(n_seg):
+            if e[j + 1] > e[j]:
+                N, M = inner_products(dw, inv_sn, up, uc, df, int(e[j]), int(e[j + 1]), use_ld)
+                Fk[p, j] = fstat_from_NM(N, M)[0]
+        F[p] = float(np.sum(Fk[p].astype(np.longdouble)))
+    return F, Fk, edges
 
 
 def max_threads() -> int:

@@ -69,8 +69,16 @@ CONFIGS: Tuple[Config, ...] = (
 )
 
 
+# Row f2 (the paper's own segment limits) needs templates whose band [f(t=0), f(t=T)] falls
+# inside the grid; the tiny config has none (its particles reach 12.66 mHz at the lowest).  A half-year
+# grid small enough for the oracle, with particles whose bands start below, inside and above the grid
+# and some that merge during the observation.  Not one of BASELINE.json's five configs.
+_T_BANDS = float(2 ** 24)
+BANDS_SMALL = Config(5, "bands_small", _T_BANDS, 0.020, 0.026, (1, 4, 16), (64,), 2.0 * YEAR_S, "bands")
+
+
 def config_by_name(name) -> Config:
-    for c in CONFIGS:
+    for c in CONFIGS + (BANDS_SMALL,):
         if c.name == name or str(c.index) == str(name):
             return c
     raise KeyError(name)
@@ -159,6 +167,10 @@ def draw_particles(cfg: Config, P: Optional[int] = None) -> np.ndarray:
             u[:, 5] = np.clip(u[:, 5], 0.0, None)
             u[:, 3] = np.arccos(u[:, 3])
             out[s * per:(s + 1) * per] = u
+        return out
+    if cfg.particle_rule == "bands":
+        out = _wide_particles(rng, P, cfg.T)
+        out[:, 0] = rng.uniform(1.0 * YEAR_S, 3.0 * YEAR_S, P)
         return out
     if cfg.particle_rule == "final":
         deg = math.pi / 180.0
