@@ -124,6 +124,30 @@ FSTAT_API fstat_status fstat_eval_batch(fstat_plan *plan, int64_t P,
                                         void *cuda_stream);
 
 /*
+ * fstat_eval_batch_bands -- SURVEY row f2: the semi-coherent F-statistic with the paper's OWN segment
+ * limits (the number of segments is the same for all templates; the lowest and highest
+ * limits are "the lowest and highest instantaneous frequencies occurring during the observation period
+ * in the template").  For every particle the template is windowed to the bins [k_lo, k_hi) of the plan's
+ * grid whose stationary time t_f = (1/2pi) dPsi_0/df (Eq. 20 :220) lies in [0, T_obs], T_obs = 1/df
+ * (k_lo = number of bins with t_f < 0, k_hi = number with t_f <= T_obs), and that band is cut into n_seg
+ * partitions with edges (reading A26)
+ *     e_j = min(C (q_lo + floor(j (q_hi - q_lo) / n_seg)), n_bins),  q = floor((k + C/2) / C),  C = edge_lattice,
+ * j = 0..n_seg; F_k over [e_j, e_{j+1}) as in fstat_eval_batch, an empty partition gives F_k = 0, F = sum_k F_k.
+ * The plan's own partition edges play no role.
+ *
+ *   params  [P][6] DEVICE pointer as in fstat_eval_batch.
+ *   n_seg   >= 1; edge_lattice >= 1 bins (1 = edges at any bin).
+ *   F       [P] DEVICE pointer, out.   Fk  [P][n_seg] DEVICE pointer, out; may be NULL.
+ *   band    [P][2] int64 DEVICE pointer, out: k_lo, k_hi of every particle; may be NULL.
+ * Invalid particles get F = F_k = -inf and band (0, 0).  Asynchronous on cuda_stream.  Every in-band bin is
+ * evaluated with the full model (the direct kernel's arithmetic).
+ * Errors: EINVAL (NULL plan/params/F, n_seg < 1, edge_lattice < 1), ENOMEM, ECUDA.
+ */
+FSTAT_API fstat_status fstat_eval_batch_bands(fstat_plan *plan, int64_t P, const double *params, int32_t n_seg,
+                                              int32_t edge_lattice, double *F, double *Fk, int64_t *band,
+                                              void *cuda_stream);
+
+/*
  * fstat_eval_amplitudes -- the maximum-likelihood extrinsic amplitudes a = M^-1 N of every partition
  * (Eq. 10; a_1..a_4 multiply the basis templates A^1 = u_+, A^2 = u_x, A^3 = i u_+, A^4 = i u_x of
  * Eq. 5 :77, and are the reparameterisation of (D_L, psi, iota, phi_c) of Eq. B1 :413 up to the amplitude

@@ -18,7 +18,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 # every symbol include/fstat.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
-    "fstat_eval_batch_host", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
+    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
@@ -71,6 +71,8 @@ def load_library():
         L.fstat_eval_batch.restype = C.c_int
         L.fstat_eval_amplitudes.argtypes = [vp, i64, vp, vp, vp]
         L.fstat_eval_amplitudes.restype = C.c_int
+        L.fstat_eval_batch_bands.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
+        L.fstat_eval_batch_bands.restype = C.c_int
         L.fstat_eval_batch_host.argtypes = [vp, i64, vp, vp, vp, vp]
         L.fstat_eval_batch_host.restype = C.c_int
         L.fstat_eval_template.argtypes = [vp, dp, vp, vp, vp]
@@ -252,6 +254,24 @@ def fstat_eval_batch(plan: Plan, params, F=None, Fk=None, stream=None, want_Fk: 
     pFk = _dev_ptr(Fk, "Fk", P * plan.n_part) if Fk is not None else None
     _check(load_library().fstat_eval_batch(plan.handle, P, pp, pF, pFk, _stream_ptr(stream)), "fstat_eval_batch", plan)
     return F, Fk
+
+
+def fstat_eval_batch_bands(plan: Plan, params, n_seg: int, edge_lattice: int = 1, stream=None, want_Fk: bool = True,
+                           want_band: bool = True):
+    """Row f2: params [P][6] float64 CUDA tensor -> (F [P], Fk [P][n_seg] or None,
+    band [P][2] int64 or None) CUDA tensors, with every template windowed to its own band and that band
+    cut into n_seg partitions.  Asynchronous on ``stream``."""
+    import torch
+    P = int(params.shape[0])
+    pp = _dev_ptr(params, "params", 6 * P)
+    F = torch.empty(P, dtype=torch.float64, device=params.device)
+    Fk = torch.empty((P, int(n_seg)), dtype=torch.float64, device=params.device) if want_Fk else None
+    band = torch.empty((P, 2), dtype=torch.int64, device=params.device) if want_band else None
+    _check(load_library().fstat_eval_batch_bands(plan.handle, P, pp, int(n_seg), int(edge_lattice), _dev_ptr(F, "F", P),
+                                                 _dev_ptr(Fk, "Fk", P * int(n_seg)) if want_Fk else None,
+                                                 band.data_ptr() if want_band else None, _stream_ptr(stream)),
+           "fstat_eval_batch_bands", plan)
+    return F, Fk, band
 
 
 def fstat_eval_amplitudes(plan: Plan, params, amp=None, stream=None):

@@ -55,6 +55,11 @@ struct fstat_plan {
     int32_t *d_slot = nullptr; size_t slot_cap = 0;      // [P] particle -> slot (sorted by chirp mass)
     int32_t *d_perm = nullptr; size_t perm_cap = 0;      // [P_pad] slot -> particle (-1: padding)
     double *d_partial = nullptr; size_t partial_cap = 0; // doubles
+    // row f2 (fstat_eval_batch_bands)
+    int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
+    double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
+    int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
+    double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
     // host-buffer path
     double *d_params = nullptr, *d_F = nullptr, *d_Fk = nullptr;
     size_t params_cap = 0, F_cap = 0, Fk_cap = 0;
@@ -364,6 +369,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
         return fail(pl, FSTAT_ECUDA, "device is not sm_100-class (this library ships sm_100a code only)");
     CU_TRY(pl, main_kernel_configure());
     CU_TRY(pl, fast_kernel_configure());
+    CU_TRY(pl, band_kernel_configure());
 
     const double *d_freq = freq, *d_dw = dw, *d_isn = isn;
     double *tmp = nullptr;
@@ -435,6 +441,7 @@ static void plan_free(fstat_plan *pl)
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
+    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk);
     cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
@@ -659,6 +666,74 @@ fstat_status fstat_eval_amplitudes(fstat_plan *pl, int64_t P, const double *para
 {
     if (pl && P > 0 && !amp) return fail(pl, FSTAT_EINVAL, "params or amp is NULL");
     return eval_impl(pl, P, params, nullptr, nullptr, amp, stream);
+}
+
+fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *params, int32_t n_seg, int32_t edge_lattice,
+                                    double *F, double *Fk, int64_t *band, void *stream)
+{
+    if (!pl) return FSTAT_EINVAL;
+    if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
+    if (n_seg < 1 || edge_lattice < 1) return fail(pl, FSTAT_EINVAL, "n_seg < 1 or edge_lattice < 1");
+    if (P == 0) return FSTAT_OK;
+    if (!params || !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
+    if (pl->n_bins >= ((int64_t)1 << 31) - edge_lattice) return fail(pl, FSTAT_EUNSUPPORTED, "grid too long for 32-bit bins");
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)stream;
+
+    const int64_t n_groups = (P + kThreads - 1) / kThreads;
+    const int64_t P_pad = n_groups * kThreads;
+    // work segments: about 8 items per SM over the whole grid, whole tiles, 256 .. 8192 bins
+    int64_t seg_len = pl->opt.max_segment_bins > 0 ? pl->opt.max_segment_bins
+                                                   : (pl->n_bins * n_groups) / ((int64_t)pl->n_sm * 8);
+    if (pl->opt.max_segment_bins <= 0) seg_len = seg_len < 256 ? 256 : (seg_len > 8192 ? 8192 : seg_len);
+    seg_len = (seg_len + kTileBins - 1) / kTileBins * kTileBins;
+    const int64_t n_wseg = (pl->n_bins + seg_len - 1) / seg_len;
+    if (n_wseg * n_groups >= ((int64_t)1 << 31)) return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
+
+    CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)P_pad * kNCoef));
+    CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
+    CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_band, &pl->band_cap, (size_t)2 * (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_rec, &pl->rec_cap, (size_t)n_wseg * 2 * kNAcc * (size_t)P_pad));
+    CU_TRY(pl, grow(&pl->d_rec_idx, &pl->rec_idx_cap, (size_t)n_wseg * 2 * (size_t)P_pad));
+    if (!Fk) {
+        CU_TRY(pl, grow(&pl->d_band_fk, &pl->band_fk_cap, (size_t)P * (size_t)n_seg));
+        Fk = pl->d_band_fk;
+    }
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, pl->d_coef, pl->d_valid,
+                               pl->d_perm, st));
+    CU_TRY(pl, launch_band_limits(pl->d_table, pl->d_coef, pl->d_valid, pl->d_perm, P_pad, (int32_t)pl->n_bins, 1.0 / pl->df,
+                                  pl->opt.orbit_kappa, pl->d_band, pl->d_band + P_pad, band, st));
+    CU_TRY(pl, cudaMemsetAsync(pl->d_rec_idx, 0xFF, (size_t)n_wseg * 2 * (size_t)P_pad * sizeof(int32_t), st));
+    CU_TRY(pl, cudaMemsetAsync(Fk, 0, (size_t)P * (size_t)n_seg * sizeof(double), st));
+    BandArgs a;
+    a.table = pl->d_table;
+    a.coef = pl->d_coef;
+    a.band_lo = pl->d_band;
+    a.band_hi = pl->d_band + P_pad;
+    a.perm = pl->d_perm;
+    a.rec = pl->d_rec;
+    a.rec_idx = pl->d_rec_idx;
+    a.Fk = Fk;
+    a.P_pad = P_pad;
+    a.n_bins = (int32_t)pl->n_bins;
+    a.n_seg = n_seg;
+    a.lattice = edge_lattice;
+    a.seg_len = (int32_t)seg_len;
+    a.n_wseg = (int32_t)n_wseg;
+    a.n_groups = (int32_t)n_groups;
+    a.orb = pl->orb;
+    const int slot = (int)(pl->n_timed % fstat_plan::kRing);
+    CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
+    CU_TRY(pl, launch_band_main(a, pl->n_sm * 12, st));
+    CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
+    ++pl->n_timed;
+    CU_TRY(pl, launch_band_epilogue(pl->d_rec, pl->d_rec_idx, pl->d_valid, pl->d_perm, P_pad, (int32_t)n_wseg, n_seg, F, Fk, st));
+    pl->n_launches += 5;                               // rank, prologue, band limits, band main, band epilogue
+    return FSTAT_OK;
 }
 
 fstat_status fstat_eval_batch_host(fstat_plan *pl, int64_t P, const double *params_host, double *F_host,

@@ -1,0 +1,302 @@
+// fstat_band.cu -- SURVEY row f2: the semi-coherent F-statistic with the paper's OWN segment limits
+// (PAPER.md:122): the number of segments is fixed for all templates, the outer limits are "the lowest and
+// highest instantaneous frequencies occurring during the observation period in the template", i.e. the
+// bins whose stationary time t_f (Eq. 20 :220) lies in [0, T_obs].  Partition edges therefore differ from
+// particle to particle (reading A26 for where they fall on the grid):
+//
+//   band_kernel          k_lo = #{bins with t_f < 0}, k_hi = #{bins with t_f <= T_obs} per particle, by
+//                        bisection over the per-bin table (t_f increases along the grid)
+//   fstat_band_kernel    the direct kernel (full model at every bin) with per-THREAD partition edges:
+//                        a partition that opens and closes inside one work segment is finished in the
+//                        thread (2 F_k written at once); the fragment before the first edge and the
+//                        one after the last edge of a work segment go to head / tail records
+//   band_epilogue_kernel stitches head / tail records of consecutive work segments into the partitions
+//                        that straddle them, writes their F_k, then F = sum_k F_k in a fixed order
+//
+// First version of the row: every in-band bin costs the full model (263 FP64 instructions); carrying the
+// interpolating kernel over to per-particle edges is described in DESIGN.md section 12.
+#include "fstat_device.cuh"
+#include "fstat_direct.cuh"
+#include "fstat_internal.h"
+#include "fstat_model.cuh"
+
+#include <math.h>
+
+namespace fstat {
+
+// e_j = min(C (q_lo + floor(j D / N)), n_bins)   (reading A26)
+__device__ __forceinline__ int32_t band_edge(int32_t j, int32_t q_lo, int32_t D, int32_t N, int32_t C, int32_t n_bins)
+{
+    const int64_t e = (int64_t)C * ((int64_t)q_lo + ((int64_t)j * D) / N);
+    return (int32_t)(e < (int64_t)n_bins ? e : (int64_t)n_bins);
+}
+
+// Orbital phase at t_f in quarter turns of a year, alpha_q = c10 + sum_j c_j D_j(f) (same FMA chain as
+// model_eval); t_f = (alpha_q - 2 kappa / pi) year / 4.
+__device__ __forceinline__ double tf_seconds(const double *__restrict__ row, const double (&c)[kNCoef], double kappa_qt)
+{
+    double alq = fma(c[2], row[T_D0 + 0], c[10]);
+#pragma unroll
+    for (int j = 1; j < 8; ++j) alq = fma(c[2 + j], row[T_D0 + j], alq);
+    return (alq - kappa_qt) * (0.25 * kYear);
+}
+
+__global__ void __launch_bounds__(128) band_kernel(const double *__restrict__ table, const double *__restrict__ coef,
+                                                   const int32_t *__restrict__ valid,
+                                                   const int32_t *__restrict__ perm, int64_t P_pad, int32_t n_bins,
+                                                   double T_obs, double kappa_qt, int32_t *__restrict__ band_lo,
+                                                   int32_t *__restrict__ band_hi, int64_t *__restrict__ band_out)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;       // slot
+    if (p >= P_pad) return;
+    int32_t k_lo = 0, k_hi = 0;
+    if (valid[p] != 0) {
+        double c[kNCoef];
+#pragma unroll
+        for (int j = 0; j < kNCoef; ++j) c[j] = coef[(int64_t)j * P_pad + p];
+        // first bin with t_f >= 0
+        int32_t a = 0, b = n_bins;
+        while (a < b) {
+            const int32_t m = a + ((b - a) >> 1);
+            if (tf_seconds(table + (int64_t)m * kTabW, c, kappa_qt) < 0.0) a = m + 1; else b = m;
+        }
+        k_lo = a;
+        // first bin with t_f > T_obs
+        b = n_bins;
+        while (a < b) {
+            const int32_t m = a + ((b - a) >> 1);
+            if (tf_seconds(table + (int64_t)m * kTabW, c, kappa_qt) <= T_obs) a = m + 1; else b = m;
+        }
+        k_hi = a;
+    }
+    band_lo[p] = k_lo;
+    band_hi[p] = k_hi;
+    const int32_t q = perm[p];
+    if (band_out != nullptr && q >= 0) {
+        band_out[2 * (int64_t)q] = k_lo;
+        band_out[2 * (int64_t)q + 1] = k_hi;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Main kernel.  Work item = (group of 128 slots) x (work segment of seg_len bins of the grid); persistent
+// CTAs stride over the items and skip those no thread of the group is in band for.
+// Thread state: j = the partition the current bin belongs to (-1 below the band, N above it), e_next = the
+// bin at which partition j closes.  rec[(w * 2 + h) * 8 + i][slot], rec_idx[(w * 2 + h)][slot]: head (h = 0)
+// and tail (h = 1) fragments of work segment w with the partition they belong to (-1: none).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_constant__ BandArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    MainSmem &sm = *reinterpret_cast<MainSmem *>(smem_raw);
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(&sm.full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    int g0 = 0;                                          // tiles consumed so far by this CTA (ring position)
+    const int32_t N = a.n_seg, C = a.lattice;
+    const int n_items = a.n_groups * a.n_wseg;
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int grp = item / a.n_wseg;
+        const int w = item - grp * a.n_wseg;
+        const int64_t p = (int64_t)grp * kThreads + tid;
+        const int lo = w * a.seg_len, hi = min(a.n_bins, lo + a.seg_len);
+
+        const int32_t k_lo = a.band_lo[p], k_hi = a.band_hi[p];
+        const int32_t q_lo = (k_lo + C / 2) / C, D = (k_hi + C / 2) / C - q_lo;
+        const int32_t e0 = band_edge(0, q_lo, D, N, C, a.n_bins), eN = band_edge(N, q_lo, D, N, C, a.n_bins);
+        const bool active = (eN > e0) && (lo < eN) && (hi > e0);
+        if (!__syncthreads_or(active ? 1 : 0)) continue;
+
+        const int n_bins = hi - lo;
+        const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
+        const double *src = a.table + (int64_t)lo * kTabW;
+        if (tid == 0) {
+#pragma unroll
+            for (int s = 0; s < kStages; ++s) {
+                if (s < n_tiles) {
+                    const int slot = (g0 + s) % kStages;
+                    const int nb = min(kTileBins, n_bins - s * kTileBins);
+                    const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
+                    mbar_expect_tx(&sm.full[slot], bytes);
+                    tma_load_1d(sm.tile[slot], src + (int64_t)s * kTileBins * kTabW, bytes, &sm.full[slot]);
+                }
+            }
+        }
+
+        double c[kNCoef];
+#pragma unroll
+        for (int j = 0; j < kNCoef; ++j) c[j] = a.coef[(int64_t)j * a.P_pad + p];
+
+        // the partition bin `lo` belongs to
+        int32_t j, e_next;
+        if (!active) { j = N; e_next = INT32_MAX; }
+        else if (lo < e0) { j = -1; e_next = e0; }
+        else {
+            // largest j with e_j <= lo:  floor(j D / N) <= cells  <=>  j <= ceil((cells + 1) N / D) - 1
+            const int64_t cells = (int64_t)(lo / C) - q_lo;
+            int64_t jj = ((cells + 1) * N + D - 1) / D - 1;
+            if (jj > N - 1) jj = N - 1;
+            j = (int32_t)jj;
+            while (j + 1 < N && band_edge(j + 1, q_lo, D, N, C, a.n_bins) <= lo) ++j;     // (never taken)
+            while (j > 0 && band_edge(j, q_lo, D, N, C, a.n_bins) > lo) --j;
+            e_next = band_edge(j + 1, q_lo, D, N, C, a.n_bins);
+        }
+        bool flushed = false;
+        const int32_t particle = a.perm[p];
+        double *rec_head = a.rec + ((int64_t)(w * 2 + 0) * kNAcc) * a.P_pad + p;
+        double *rec_tail = a.rec + ((int64_t)(w * 2 + 1) * kNAcc) * a.P_pad + p;
+
+        double acc[kNAcc];
+#pragma unroll
+        for (int i = 0; i < kNAcc; ++i) acc[i] = 0.0;
+
+        for (int t = 0; t < n_tiles; ++t) {
+            const int g = g0 + t;
+            const int slot = g % kStages;
+            mbar_wait(&sm.full[slot], (uint32_t)((g / kStages) & 1));
+            const int nb = min(kTileBins, n_bins - t * kTileBins);
+            const double *tile = sm.tile[slot];
+            double in[kNAcc];
+#pragma unroll
+            for (int i = 0; i < kNAcc; ++i) in[i] = 0.0;
+
+#pragma unroll 1
+            for (int b = 0; b < nb; ++b) {
+                const int k = lo + t * kTileBins + b;
+                while (k == e_next) {                                  // partition j closes in front of bin k
+                    if (j >= 0) {
+                        double v[kNAcc];
+#pragma unroll
+                        for (int i = 0; i < kNAcc; ++i) v[i] = acc[i] + in[i];
+                        if (!flushed) {
+#pragma unroll
+                            for (int i = 0; i < kNAcc; ++i) rec_head[(int64_t)i * a.P_pad] = v[i];
+                            a.rec_idx[(int64_t)(w * 2 + 0) * a.P_pad + p] = j;
+                            flushed = true;
+                        } else {
+                            a.Fk[(int64_t)particle * N + j] = 0.5 * two_F(v);
+                        }
+#pragma unroll
+                        for (int i = 0; i < kNAcc; ++i) { acc[i] = 0.0; in[i] = 0.0; }
+                    }
+                    ++j;
+                    e_next = (j < N) ? band_edge(j + 1, q_lo, D, N, C, a.n_bins) : INT32_MAX;
+                }
+                const double mask = (j >= 0 && j < N) ? 1.0 : 0.0;     // the template window (reading A14 lifted)
+                const double2 *row = reinterpret_cast<const double2 *>(tile + b * kTabW);
+                const double2 dwv = row[10];
+                double psi, sps, cps, tpr, tpi, tcr, tci;
+                bin_template(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
+                const double qr = mask * fma(dwv.x, cps, -dwv.y * sps);         // dw' exp(+i Psi)
+                const double qi = mask * fma(dwv.x, sps, dwv.y * cps);
+                in[0] = fma(qr, tpr, fma(qi, tpi, in[0]));                      // z_+ += q conj(T'_+)
+                in[1] = fma(qi, tpr, fma(-qr, tpi, in[1]));
+                in[2] = fma(qr, tcr, fma(qi, tci, in[2]));                      // z_x
+                in[3] = fma(qi, tcr, fma(-qr, tci, in[3]));
+                const double wgt = mask * row[11].x;
+                in[4] = fma(wgt, fma(tpr, tpr, tpi * tpi), in[4]);              // m_pp
+                in[5] = fma(wgt, fma(tcr, tcr, tci * tci), in[5]);              // m_cc
+                in[6] = fma(wgt, fma(tpr, tcr, tpi * tci), in[6]);              // m_pc
+                in[7] = fma(wgt, fma(tpi, tcr, -tpr * tci), in[7]);
+            }
+#pragma unroll
+            for (int i = 0; i < kNAcc; ++i) acc[i] += in[i];
+
+            __syncthreads();                             // every thread is done with this slot
+            if (tid == 0 && t + kStages < n_tiles) {
+                const int tn = t + kStages;
+                const int nbn = min(kTileBins, n_bins - tn * kTileBins);
+                const uint32_t bytes = (uint32_t)nbn * kTabW * sizeof(double);
+                mbar_expect_tx(&sm.full[slot], bytes);
+                tma_load_1d(sm.tile[slot], src + (int64_t)tn * kTileBins * kTabW, bytes, &sm.full[slot]);
+            }
+        }
+        g0 += n_tiles;
+
+        if (j >= 0 && j < N) {                           // the fragment after the last edge: partition j goes on
+#pragma unroll
+            for (int i = 0; i < kNAcc; ++i) rec_tail[(int64_t)i * a.P_pad] = acc[i];
+            a.rec_idx[(int64_t)(w * 2 + 1) * a.P_pad + p] = j;
+        }
+    }
+}
+
+// One thread per slot walks the head / tail records in grid order; consecutive records of the same
+// partition are fragments of it.  Fixed order of every sum: results are bit-reproducible.
+__global__ void __launch_bounds__(128) band_epilogue_kernel(const double *__restrict__ rec,
+                                                            const int32_t *__restrict__ rec_idx,
+                                                            const int32_t *__restrict__ valid,
+                                                            const int32_t *__restrict__ perm, int64_t P_pad,
+                                                            int32_t n_wseg, int32_t N, double *__restrict__ F,
+                                                            double *__restrict__ Fk)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P_pad) return;
+    const int32_t particle = perm[p];
+    if (particle < 0) return;
+    double *row = Fk + (int64_t)particle * N;
+    if (valid[p] == 0) {
+        for (int j = 0; j < N; ++j) row[j] = -INFINITY;
+        F[particle] = -INFINITY;
+        return;
+    }
+    int32_t cur = -1;
+    double v[kNAcc];
+#pragma unroll
+    for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
+    for (int r = 0; r < 2 * n_wseg; ++r) {
+        const int32_t idx = rec_idx[(int64_t)r * P_pad + p];
+        if (idx < 0) continue;
+        if (idx != cur) {
+            if (cur >= 0) row[cur] = 0.5 * two_F(v);
+            cur = idx;
+#pragma unroll
+            for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
+        }
+        const double *src = rec + ((int64_t)r * kNAcc) * P_pad + p;
+#pragma unroll
+        for (int i = 0; i < kNAcc; ++i) v[i] += src[(int64_t)i * P_pad];
+    }
+    if (cur >= 0) row[cur] = 0.5 * two_F(v);
+    double f = 0.0;
+    for (int j = 0; j < N; ++j) f += row[j];             // F = sum_k F_k (Eq. 11 :110, reading A12)
+    F[particle] = f;
+}
+
+cudaError_t band_kernel_configure()
+{
+    return cudaFuncSetAttribute(fstat_band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MainSmem));
+}
+
+cudaError_t launch_band_limits(const double *table, const double *coef, const int32_t *valid, const int32_t *perm,
+                               int64_t P_pad, int32_t n_bins, double T_obs, double kappa, int32_t *band_lo,
+                               int32_t *band_hi, int64_t *band_out, cudaStream_t st)
+{
+    band_kernel<<<(unsigned)((P_pad + 127) / 128), 128, 0, st>>>(table, coef, valid, perm, P_pad, n_bins, T_obs,
+                                                                  2.0 * kappa / kPi, band_lo, band_hi, band_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t st)
+{
+    int64_t n_cta = (int64_t)a.n_groups * a.n_wseg;
+    if (n_cta > max_ctas) n_cta = max_ctas;
+    fstat_band_kernel<<<(unsigned)n_cta, kThreads, sizeof(MainSmem), st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_band_epilogue(const double *rec, const int32_t *rec_idx, const int32_t *valid, const int32_t *perm,
+                                 int64_t P_pad, int32_t n_wseg, int32_t n_seg, double *F, double *Fk, cudaStream_t st)
+{
+    band_epilogue_kernel<<<(unsigned)((P_pad + 127) / 128), 128, 0, st>>>(rec, rec_idx, valid, perm, P_pad, n_wseg,
+                                                                           n_seg, F, Fk);
+    return cudaGetLastError();
+}
+
+}  // namespace fstat

@@ -1,0 +1,55 @@
+// fstat_direct.cuh -- device pieces shared by the two kernels that evaluate the model at every bin
+// (fstat_main_kernel in fstat_kernels.cu, fstat_band_kernel in fstat_band.cu) and by the epilogues:
+// the TMA ring of table rows, one (particle, bin) of the template, and 2 F_k from the eight sums.
+#pragma once
+#include "fstat_device.cuh"
+#include "fstat_internal.h"
+#include "fstat_model.cuh"
+
+namespace fstat {
+
+struct __align__(16) MainSmem {
+    double tile[kStages][kTileBins * kTabW];
+    uint64_t full[kStages];
+};
+
+
+// One (particle, bin) of the direct kernel: model_eval() plus the linear phase term and the carrier.
+// Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1 included), its sine and
+// cosine, and T'_+ , T'_x.
+__device__ __forceinline__ void bin_template(const double2 *__restrict__ row, const double (&c)[kNCoef],
+                                             const OrbitCoef &orb, double &psi_out, double &sps, double &cps,
+                                             double &tpr, double &tpi, double &tcr, double &tci)
+{
+    double psi_nl;
+    model_eval(row, c, orb, psi_nl, tpr, tpi, tcr, tci);
+    const double psi = fma(c[0], row[0].x, psi_nl);                  // + 2 pi f t_c
+    sincos_qt(psi, sps, cps);
+    psi_out = psi;
+}
+
+// 2 F_k = z^H G^-1 z by Gram-Schmidt (Eq. 7 in its 2x2 Hermitian form):
+// |z_+|^2/m_pp + |z_x - (m_pc/m_pp) z_+|^2 / (m_cc - |m_pc|^2/m_pp); rank-deficient G (reading A15): only
+// the non-degenerate direction(s) contribute.
+__device__ __forceinline__ double two_F(const double (&v)[kNAcc])
+{
+    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
+    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
+    double twoF = 0.0;
+    if (mpp > 0.0) {
+        const double inv = 1.0 / mpp;
+        twoF = (zpr * zpr + zpi * zpi) * inv;
+        const double cr = mr * inv, ci = mi * inv;                      // m_pc / m_pp
+        const double schur = mcc - (mr * mr + mi * mi) * inv;
+        if (schur > 1e-13 * mcc) {
+            const double yr = zcr - (cr * zpr - ci * zpi);
+            const double yi = zci - (cr * zpi + ci * zpr);
+            twoF += (yr * yr + yi * yi) / schur;
+        }
+    } else if (mcc > 0.0) {
+        twoF = (zcr * zcr + zci * zci) / mcc;
+    }
+    return twoF;
+}
+
+}  // namespace fstat

@@ -119,6 +119,34 @@ struct FastArgs {
     OrbitCoef orb;
 };
 
+// row f2 (fstat_band.cu): per-particle bands and partition edges
+struct BandArgs {
+    const double *table;      // [n_bins][kTabW]
+    const double *coef;       // [kNCoef][P_pad]
+    const int32_t *band_lo;   // [P_pad] k_lo, k_hi of every slot (bins of the plan's grid)
+    const int32_t *band_hi;
+    const int32_t *perm;      // [P_pad] slot -> particle
+    double *rec;              // [n_wseg][2][kNAcc][P_pad] head / tail fragments
+    int32_t *rec_idx;         // [n_wseg][2][P_pad] the partition a fragment belongs to, -1: none
+    double *Fk;               // [P][n_seg]
+    int64_t P_pad;
+    int32_t n_bins;
+    int32_t n_seg;            // partitions per template (the paper's N_seg)
+    int32_t lattice;          // edges are multiples of this many bins (reading A26)
+    int32_t seg_len;          // bins per work segment
+    int32_t n_wseg;
+    int32_t n_groups;
+    OrbitCoef orb;
+};
+
+cudaError_t launch_band_limits(const double *table, const double *coef, const int32_t *valid, const int32_t *perm,
+                               int64_t P_pad, int32_t n_bins, double T_obs, double kappa, int32_t *band_lo,
+                               int32_t *band_hi, int64_t *band_out, cudaStream_t st);
+cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t st);
+cudaError_t launch_band_epilogue(const double *rec, const int32_t *rec_idx, const int32_t *valid, const int32_t *perm,
+                                 int64_t P_pad, int32_t n_wseg, int32_t n_seg, double *F, double *Fk, cudaStream_t st);
+cudaError_t band_kernel_configure();
+
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
                                double df, double arm_length_m, double *table, double *dwp,
                                uint32_t *err_bits, cudaStream_t st);

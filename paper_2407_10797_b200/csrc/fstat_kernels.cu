@@ -9,6 +9,7 @@
 //
 // Citations are to /root/reference/PAPER.md (line, equation) and to DESIGN.md readings (A1..A24).
 #include "fstat_device.cuh"
+#include "fstat_direct.cuh"
 #include "fstat_internal.h"
 #include "fstat_model.cuh"
 
@@ -174,26 +175,7 @@ cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, doub
 // =================================================================================================
 // a2-a5: the fused main kernel
 // =================================================================================================
-struct __align__(16) MainSmem {
-    double tile[kStages][kTileBins * kTabW];
-    uint64_t full[kStages];
-};
-
 size_t main_kernel_smem_bytes() { return sizeof(MainSmem); }
-
-// One (particle, bin) of the direct kernel: model_eval() plus the linear phase term and the carrier.
-// Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1 included), its sine and
-// cosine, and T'_+ , T'_x.
-__device__ __forceinline__ void bin_template(const double2 *__restrict__ row, const double (&c)[kNCoef],
-                                             const OrbitCoef &orb, double &psi_out, double &sps, double &cps,
-                                             double &tpr, double &tpi, double &tcr, double &tci)
-{
-    double psi_nl;
-    model_eval(row, c, orb, psi_nl, tpr, tpi, tcr, tci);
-    const double psi = fma(c[0], row[0].x, psi_nl);                  // + 2 pi f t_c
-    sincos_qt(psi, sps, cps);
-    psi_out = psi;
-}
 
 // The direct kernel: every bin of a work item evaluated in full.  Persistent CTAs walk the list of work
 // items the stride selection left to it (schedule_kernel: items for which no interpolation stride meets
@@ -384,27 +366,6 @@ __device__ __forceinline__ void add_segment(const double *__restrict__ partial, 
     v[5] += fma(fma(dr, dr, di * di), t[4], fma(2.0, fma(dr, t[6], -di * t[7]), t[5]));
     v[6] += fma(dr, t[4], t[6]);
     v[7] += fma(-di, t[4], t[7]);
-}
-
-__device__ __forceinline__ double two_F(const double (&v)[kNAcc])
-{
-    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
-    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
-    double twoF = 0.0;
-    if (mpp > 0.0) {
-        const double inv = 1.0 / mpp;
-        twoF = (zpr * zpr + zpi * zpi) * inv;
-        const double cr = mr * inv, ci = mi * inv;                      // m_pc / m_pp
-        const double schur = mcc - (mr * mr + mi * mi) * inv;
-        if (schur > 1e-13 * mcc) {
-            const double yr = zcr - (cr * zpr - ci * zpi);
-            const double yi = zci - (cr * zpi + ci * zpr);
-            twoF += (yr * yr + yi * yi) / schur;
-        }
-    } else if (mcc > 0.0) {
-        twoF = (zcr * zcr + zci * zci) / mcc;
-    }
-    return twoF;
 }
 
 template <bool SEG_PAR>

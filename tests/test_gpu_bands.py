@@ -1,0 +1,117 @@
+"""Row f2 on the GPU (fstat_eval_batch_bands: per-template bands and segment limits) against
+the oracle's `fstat_bands`, element by element through the C ABI.  Integer results (band limits) bit-exact;
+F and F_k to north_star's 1e-5 relative."""
+import numpy as np
+import pytest
+
+import synthetic as syn
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def fs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2407_10797_b200 import build
+    build.build()
+    import paper_2407_10797_b200 as fs
+    fs.load_library()
+    return fs
+
+
+@pytest.fixture(scope="module")
+def bands(orc):
+    return syn.make_dataset(syn.BANDS_SMALL, orc.template)
+
+
+def _gpu(fs, ds, par, n_seg, lattice, opts=None):
+    import torch
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), opts) as plan:
+        p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+        F, Fk, band = fs.fstat_eval_batch_bands(plan, p, n_seg, lattice)
+        torch.cuda.synchronize()
+        return F.cpu().numpy(), Fk.cpu().numpy(), band.cpu().numpy()
+
+
+def _check(orc, ds, par, n_seg, lattice, F, Fk, band):
+    F_o, Fk_o, edges = orc.fstat_bands(ds.freq, ds.dw, ds.inv_sn, par, n_seg, lattice)
+    T = ds.cfg.T
+    for p in range(par.shape[0]):
+        if orc.params_valid(par[p]):
+            assert tuple(band[p]) == orc.template_band(par[p], ds.freq, T)
+    live = np.isfinite(Fk_o) & (Fk_o != 0.0)
+    assert np.array_equal(np.isneginf(Fk), np.isneginf(Fk_o))
+    assert np.all(Fk[Fk_o == 0.0] == 0.0)                  # empty partitions and empty bands: exactly zero
+    assert np.max(np.abs(Fk[live] - Fk_o[live]) / np.abs(Fk_o[live])) <= RTOL
+    ok = np.isfinite(F_o) & (F_o != 0.0)
+    assert np.array_equal(np.isneginf(F), np.isneginf(F_o)) and np.all(F[F_o == 0.0] == 0.0)
+    assert np.max(np.abs(F[ok] - F_o[ok]) / np.abs(F_o[ok])) <= RTOL
+    return int(live.sum())
+
+
+@pytest.mark.parametrize("n_seg,lattice", [(1, 1), (4, 1), (16, 1), (16, 64), (64, 128), (7, 3)])
+def test_bands_small_every_F_and_Fk(fs, orc, bands, n_seg, lattice):
+    """64 particles whose bands start below, inside and above the grid (39 non-empty), every F and F_k."""
+    ds = bands
+    par = syn.draw_particles(ds.cfg)
+    F, Fk, band = _gpu(fs, ds, par, n_seg, lattice)
+    n = _check(orc, ds, par, n_seg, lattice, F, Fk, band)
+    assert n >= 30 * n_seg
+
+
+@pytest.mark.parametrize("seg", [64, 320, 4096, 1 << 20])
+def test_bands_work_segment_length_does_not_matter(fs, orc, bands, seg):
+    """Work segments of one tile, a few tiles, many tiles, and one segment for the whole grid: partitions
+    that lie inside one work segment, straddle two, or span many are all stitched the same."""
+    ds = bands
+    par = syn.draw_particles(ds.cfg)[:40]
+    opts = fs.fstat_default_options()
+    opts.max_segment_bins = seg
+    F, Fk, band = _gpu(fs, ds, par, 16, 1, opts)
+    _check(orc, ds, par, 16, 1, F, Fk, band)
+
+
+def test_bands_invalid_particles_and_more_partitions_than_cells(fs, orc, bands):
+    ds = bands
+    par = syn.draw_particles(ds.cfg)[:12].copy()
+    par[1, 1] = -3.0
+    par[4, 2] = 0.3
+    par[7, 0] = np.nan
+    # 200 partitions on a 1024-bin lattice: bands of fewer than 200 cells leave empty partitions
+    F, Fk, band = _gpu(fs, ds, par, 200, 1024)
+    _check(orc, ds, par, 200, 1024, F, Fk, band)
+    assert np.all(band[[1, 4, 7]] == 0)
+
+
+def test_bands_repeatable_and_independent_of_batch_order(fs, bands):
+    import torch
+    ds = bands
+    par = syn.draw_particles(ds.cfg)
+    F1, Fk1, b1 = _gpu(fs, ds, par, 16, 1)
+    F2, Fk2, b2 = _gpu(fs, ds, par, 16, 1)
+    assert np.array_equal(F1, F2) and np.array_equal(Fk1, Fk2) and np.array_equal(b1, b2)
+    perm = np.random.default_rng(0).permutation(par.shape[0])
+    F3, Fk3, b3 = _gpu(fs, ds, par[perm], 16, 1)
+    assert np.array_equal(F3, F1[perm]) and np.array_equal(Fk3, Fk1[perm]) and np.array_equal(b3, b1[perm])
+
+
+def test_bands_first_stage_sample(fs, orc):
+    """Config 1's data and particles (2.5 yr, 1 577 880 bins, N_seg = 1024) in the launch configuration
+    bench.py --bands times; a sample of particles against the oracle, every F_k of the sample."""
+    import torch
+    ds = syn.make_dataset(syn.CONFIGS[1], orc.template)
+    par = syn.draw_particles(ds.cfg)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
+        p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+        F, Fk, band = fs.fstat_eval_batch_bands(plan, p, 1024, 1)
+        torch.cuda.synchronize()
+        F, Fk, band = F.cpu().numpy(), Fk.cpu().numpy(), band.cpu().numpy()
+    width = band[:, 1] - band[:, 0]
+    assert (width > 0).sum() > 1500
+    order = np.argsort(width)
+    sample = np.concatenate([order[-2:], order[(width[order] > 0).argmax():][:2], np.arange(0, 2048, 341)])
+    _check(orc, ds, par[sample], 1024, 1, F[sample], Fk[sample], band[sample])
