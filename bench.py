@@ -124,6 +124,9 @@ def parse_args():
     ap.add_argument("--interp-tol", type=float, default=1.0, help="plan option interp_tol")
     ap.add_argument("--pso", type=int, default=0, metavar="ITERS",
                     help="also time ITERS iterations of the device PSO (row f1) on this plan: swarms of 128 particles")
+    ap.add_argument("--bands", type=int, default=0, metavar="N_SEG",
+                    help="also time fstat_eval_batch_bands (row f2: per-template bands, N_SEG partitions) on this plan")
+    ap.add_argument("--bands-lattice", type=int, default=64, help="edge lattice of --bands in bins (>= 32: interpolating kernel)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
     return ap.parse_args()
@@ -386,6 +389,28 @@ def run_ours(args):
                       "template_bins_per_s": float(n_sw * 128) * ds.n_bins / (ms_it * 1e-3),
                       "overhead_vs_eval_step": ms_it / ms_step - 1.0, "best_F_max": float(bf.max())}
         fs.fstat_pso_destroy(pso)
+    if args.bands > 0:
+        # row f2: the paper's own segment limits; unit = IN-BAND template-bins (bins with t_f in [0, T] per particle)
+        for _ in range(2):
+            _, _, band = fs.fstat_eval_batch_bands(plan, par, args.bands, args.bands_lattice, stream)
+        torch.cuda.synchronize()
+        n_b = max(min(args.steps, 10), 1)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_b)]
+        for e0, e1 in evs:
+            scratch.fill_(3)
+            e0.record(stream)
+            fs.fstat_eval_batch_bands(plan, par, args.bands, args.bands_lattice, stream)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        ms_b = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs]))
+        kms = fs.fstat_plan_main_kernel_ms(plan, n_b)
+        in_band = float((band[:, 1] - band[:, 0]).sum().item())
+        out["bands"] = {"n_seg": args.bands, "edge_lattice": args.bands_lattice, "ms_per_step": ms_b,
+                        "main_kernel_ms": float(np.mean(kms)) if len(kms) else None,
+                        "in_band_template_bins": in_band, "in_band_share_of_grid": in_band / (float(P) * ds.n_bins),
+                        "in_band_template_bins_per_s": in_band * world / (ms_b * 1e-3),
+                        "kernel": "fstat_fast_kernel over the lattice cells" if args.bands_lattice >= 32
+                                  else "fstat_band_kernel (full model at every in-band bin)"}
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, ds, n_part, args.cpu_sample)
     fs.fstat_plan_destroy(plan)

@@ -56,6 +56,9 @@ struct fstat_plan {
     int32_t *d_perm = nullptr; size_t perm_cap = 0;      // [P_pad] slot -> particle (-1: padding)
     double *d_partial = nullptr; size_t partial_cap = 0; // doubles
     // row f2 (fstat_eval_batch_bands)
+    fstat_plan *cells = nullptr;        // internal plan whose partitions are the lattice cells (shares the tables)
+    int32_t cells_lattice = 0;
+    bool shares_tables = false;         // d_table, d_dwp, d_node belong to the parent plan
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
     double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
     int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
@@ -437,6 +440,8 @@ static void plan_free(fstat_plan *pl)
 {
     if (!pl) return;
     DeviceGuard g(pl->device);
+    if (pl->cells) { plan_free(pl->cells); pl->cells = nullptr; }
+    if (pl->shares_tables) { pl->d_table = nullptr; pl->d_dwp = nullptr; pl->d_node = nullptr; }
     cudaFree(pl->d_table); cudaFree(pl->d_seg_edge); cudaFree(pl->d_part_seg); cudaFree(pl->d_coef);
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
@@ -571,8 +576,49 @@ int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out
 }
 
 // a1-a5 for P particles, then a6 (F, F_k) when F != NULL and / or the extrinsic amplitudes when amp != NULL
+static void plan_free(fstat_plan *pl);
+
+// Internal plan for row f2 on a lattice: same tables (shared, not copied), partitions = the lattice cells
+// [0, C), [C, 2C), ... ; its Gram tables are built once per lattice and kept.
+static fstat_status ensure_cell_plan(fstat_plan *pl, int32_t C)
+{
+    if (pl->cells && pl->cells_lattice == C) return FSTAT_OK;
+    if (pl->cells) {
+        cudaDeviceSynchronize();
+        plan_free(pl->cells);
+        pl->cells = nullptr;
+    }
+    fstat_plan *cp = new (std::nothrow) fstat_plan;
+    if (!cp) return fail(pl, FSTAT_ENOMEM, "host allocation failed");
+    cp->device = pl->device; cp->n_sm = pl->n_sm; cp->n_bins = pl->n_bins; cp->df = pl->df; cp->opt = pl->opt;
+    cp->opt.max_segment_bins = 0;
+    cp->f0 = pl->f0; cp->orb = pl->orb; cp->fast_ok = pl->fast_ok;
+    cp->d_table = pl->d_table; cp->d_dwp = pl->d_dwp; cp->d_node = pl->d_node; cp->n_node_rows = pl->n_node_rows;
+    cp->shares_tables = true;
+    try {
+        for (int64_t e = 0; e < pl->n_bins; e += C) cp->edges.push_back(e);
+        cp->edges.push_back(pl->n_bins);
+    } catch (...) {
+        plan_free(cp);
+        return fail(pl, FSTAT_ENOMEM, "host allocation failed");
+    }
+    cp->n_part = (int32_t)(cp->edges.size() - 1);
+    fstat_status s = build_gram_tables(cp);
+    if (s != FSTAT_OK) { pl->err = cp->err; plan_free(cp); return s; }
+    pl->cells = cp;
+    pl->cells_lattice = C;
+    return FSTAT_OK;
+}
+
+// row f2 through the interpolating kernel: the plan evaluated is the internal cells plan
+struct BandReq {
+    int32_t n_seg, lattice;
+    int64_t *band_out;
+    fstat_plan *owner;        // the user's plan: timing ring and launch counter
+};
+
 static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, double *amp,
-                              void *stream)
+                              void *stream, const BandReq *br = nullptr)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
@@ -603,11 +649,23 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
 
     CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
     CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, pl->d_coef, pl->d_valid,
-                               pl->d_perm, st));
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, br ? 1 : 0, pl->d_coef,
+                               pl->d_valid, pl->d_perm, st));
+    BandSched bs{};
+    if (br) {
+        CU_TRY(pl, grow(&pl->d_band, &pl->band_cap, (size_t)2 * (size_t)P_pad));
+        CU_TRY(pl, launch_band_limits(pl->d_table, pl->d_coef, pl->d_valid, pl->d_perm, P_pad, (int32_t)pl->n_bins,
+                                      1.0 / pl->df, pl->opt.orbit_kappa, pl->d_band, pl->d_band + P_pad, br->band_out, st));
+        bs.band_lo = pl->d_band;
+        bs.band_hi = pl->d_band + P_pad;
+        bs.seg_edge = pl->d_seg_edge;
+        bs.n_seg_band = br->n_seg;
+        bs.lattice = br->lattice;
+        bs.n_bins = (int32_t)pl->n_bins;
+    }
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
                                pl->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
-                               pl->opt.force_level, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
+                               pl->opt.force_level, bs, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;
     fa.node = pl->d_node;
@@ -617,10 +675,16 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.seg_gbase = pl->d_seg_gbase;
     fa.level = pl->d_level;
     fa.partial = pl->d_partial;
+    fa.part_sk = br ? 1 : P_pad;                       // row f2: slot-major records (the cells epilogue reads whole records)
+    fa.part_sp = br ? kNPartial : 1;
     fa.P_pad = P_pad;
     fa.n_groups = (int32_t)n_groups;
     fa.n_seg = pl->n_seg;
     fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
+    if (br) {                                          // cells: ~4096 bins per CTA run whatever the lattice
+        const int64_t g = 4096 / br->lattice;
+        fa.segs_per_cta = (int32_t)(g < 1 ? 1 : (g > 128 ? 128 : g));
+    }
     fa.df = pl->df;
     fa.orb = pl->orb;
     MainArgs a;
@@ -631,18 +695,28 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     a.direct_count = pl->d_direct;
     a.max_ctas = pl->n_sm * 12;
     a.partial = pl->d_partial;
+    a.part_sk = fa.part_sk;
+    a.part_sp = fa.part_sp;
     a.P_pad = P_pad;
     a.P = (int32_t)P;
     a.n_groups = (int32_t)n_groups;
     a.n_seg = pl->n_seg;
     a.orb = pl->orb;
-    const int slot = (int)(pl->n_timed % fstat_plan::kRing);
-    CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
+    fstat_plan *tp = br ? br->owner : pl;              // whose timing ring and launch counter
+    const int slot = (int)(tp->n_timed % fstat_plan::kRing);
+    CU_TRY(pl, cudaEventRecord(tp->ev0[slot], st));
     if (pl->fast_ok) CU_TRY(pl, launch_fast(fa, st));
     CU_TRY(pl, launch_main(a, st));
-    CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
-    ++pl->n_timed;
-    pl->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
+    CU_TRY(pl, cudaEventRecord(tp->ev1[slot], st));
+    ++tp->n_timed;
+    tp->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
+    if (br) {
+        CU_TRY(pl, launch_band_cells_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, pl->d_band,
+                                              pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins, pl->n_part, br->n_seg,
+                                              br->lattice, fa.part_sk, fa.part_sp, F, Fk, st));
+        tp->n_launches += 3;                           // band limits, cells epilogue, F sums
+        return FSTAT_OK;
+    }
     if (F) {
         CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg,
                                    pl->d_fpart, F, Fk, st));
@@ -682,6 +756,30 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
     cudaStream_t st = (cudaStream_t)stream;
 
+    if (edge_lattice >= kBandFastLattice && pl->fast_ok && pl->opt.force_level != -1) {
+        // edges on a lattice: the interpolating kernel over the lattice cells (an internal plan that shares the tables)
+        fstat_status s = ensure_cell_plan(pl, edge_lattice);
+        if (s != FSTAT_OK) return s;
+        fstat_plan *cp = pl->cells;
+        cp->opt.force_level = pl->opt.force_level;
+        cp->opt.interp_tol = pl->opt.interp_tol;
+        if (!Fk) {
+            CU_TRY(pl, grow(&pl->d_band_fk, &pl->band_fk_cap, (size_t)P * (size_t)n_seg));
+            Fk = pl->d_band_fk;
+        }
+        // one record of 10 sums per (cell, particle): keep the workspace below ~24 GB by batching the particles
+        const int64_t per_particle = (int64_t)cp->n_part * kNPartial * (int64_t)sizeof(double);
+        int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
+        if (batch < kThreads) batch = kThreads;
+        BandReq br{n_seg, edge_lattice, nullptr, pl};
+        for (int64_t off = 0; off < P; off += batch) {
+            const int64_t n = (P - off < batch) ? P - off : batch;
+            br.band_out = band ? band + 2 * off : nullptr;
+            s = eval_impl(cp, n, params + 6 * off, F + off, Fk + off * n_seg, nullptr, stream, &br);
+            if (s != FSTAT_OK) { pl->err = cp->err; return s; }
+        }
+        return FSTAT_OK;
+    }
     const int64_t n_groups = (P + kThreads - 1) / kThreads;
     const int64_t P_pad = n_groups * kThreads;
     // work segments: about 8 items per SM over the whole grid, whole tiles, 256 .. 8192 bins
@@ -703,7 +801,7 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
         CU_TRY(pl, grow(&pl->d_band_fk, &pl->band_fk_cap, (size_t)P * (size_t)n_seg));
         Fk = pl->d_band_fk;
     }
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, pl->d_coef, pl->d_valid,
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, 1, pl->d_coef, pl->d_valid,
                                pl->d_perm, st));
     CU_TRY(pl, launch_band_limits(pl->d_table, pl->d_coef, pl->d_valid, pl->d_perm, P_pad, (int32_t)pl->n_bins, 1.0 / pl->df,
                                   pl->opt.orbit_kappa, pl->d_band, pl->d_band + P_pad, band, st));
@@ -777,7 +875,7 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
     CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)kThreads * kNCoef));
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)kThreads));
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
-    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, pl->d_coef,
+    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, 0, pl->d_coef,
                                pl->d_valid, nullptr, st));
     CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, u_plus, u_cross, st));
     CU_TRY(pl, cudaStreamSynchronize(st));

@@ -13,8 +13,15 @@
 //   band_epilogue_kernel stitches head / tail records of consecutive work segments into the partitions
 //                        that straddle them, writes their F_k, then F = sum_k F_k in a fixed order
 //
-// First version of the row: every in-band bin costs the full model (263 FP64 instructions); carrying the
-// interpolating kernel over to per-particle edges is described in DESIGN.md section 12.
+// That path takes edges at ANY bin (edge_lattice < 32) and pays the full model at every in-band bin.  With
+// edges on a lattice of C >= 32 bins the interpolating kernel does the work instead: the lattice cells are
+// the (data-side) partitions of an internal plan, fstat_fast_kernel / fstat_main_kernel run unchanged and
+// leave one record of sums per (cell, particle), the stride selection skips the cells no template of a group
+// is in band for, and
+//
+//   band_cells_epilogue_kernel   adds, per particle and partition, the records of the cells between its
+//                                edges (recentred basis, add_segment) and writes F_k
+//   band_fsum_kernel             F = sum_k F_k in a fixed order
 #include "fstat_device.cuh"
 #include "fstat_direct.cuh"
 #include "fstat_internal.h"
@@ -23,13 +30,6 @@
 #include <math.h>
 
 namespace fstat {
-
-// e_j = min(C (q_lo + floor(j D / N)), n_bins)   (reading A26)
-__device__ __forceinline__ int32_t band_edge(int32_t j, int32_t q_lo, int32_t D, int32_t N, int32_t C, int32_t n_bins)
-{
-    const int64_t e = (int64_t)C * ((int64_t)q_lo + ((int64_t)j * D) / N);
-    return (int32_t)(e < (int64_t)n_bins ? e : (int64_t)n_bins);
-}
 
 // Orbital phase at t_f in quarter turns of a year, alpha_q = c10 + sum_j c_j D_j(f) (same FMA chain as
 // model_eval); t_f = (alpha_q - 2 kappa / pi) year / 4.
@@ -267,6 +267,86 @@ __global__ void __launch_bounds__(128) band_epilogue_kernel(const double *__rest
     double f = 0.0;
     for (int j = 0; j < N; ++j) f += row[j];             // F = sum_k F_k (Eq. 11 :110, reading A12)
     F[particle] = f;
+}
+
+// Block = 32 slots (x) by 8 lanes (y); blockIdx.y walks the partitions.  The 8 lanes split the cells of one
+// (slot, partition) -- cell c of the lattice is partition c of the internal plan, its records are segments
+// part_seg[c] .. part_seg[c + 1] -- and are combined through shared memory in a fixed order.
+__global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *__restrict__ partial,
+                                                                  const int32_t *__restrict__ part_seg,
+                                                                  const int32_t *__restrict__ valid,
+                                                                  const int32_t *__restrict__ perm,
+                                                                  const int32_t *__restrict__ band_lo,
+                                                                  const int32_t *__restrict__ band_hi, int64_t P_pad,
+                                                                  int32_t n_bins, int32_t n_cells, int32_t N, int32_t C,
+                                                                  int64_t sk, int64_t sp, double *__restrict__ Fk)
+{
+    __shared__ double sV[8][kNAcc][32];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int64_t p = (int64_t)blockIdx.x * 32 + tx;         // < P_pad: the grid covers P_pad / 32 blocks exactly
+    const int32_t particle = perm[p];
+    const bool ok = particle >= 0 && valid[p] != 0;
+    const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
+    for (int j = blockIdx.y; j < N; j += gridDim.y) {
+        double v[kNAcc];
+#pragma unroll
+        for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
+        int s0 = 0, s1 = 0;
+        if (ok) {
+            const int32_t ea = band_edge(j, q_lo, D, N, C, n_bins), eb = band_edge(j + 1, q_lo, D, N, C, n_bins);
+            const int32_t ca = ea >= n_bins ? n_cells : ea / C, cb = eb >= n_bins ? n_cells : eb / C;
+            s0 = part_seg[ca];
+            s1 = part_seg[cb];
+            if (s1 > s0) {
+                const double *first = partial + ((int64_t)s0 * kNPartial) * P_pad + p * sp;
+                const double cs_r = first[8 * sk], cs_i = first[9 * sk];                  // the first cell's basis
+                for (int s = s0 + ty; s < s1; s += 8) add_segment(partial, s, P_pad, sk, sp, p, cs_r, cs_i, v);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < kNAcc; ++i) sV[ty][i][tx] = v[i];
+        __syncthreads();
+        if (ty == (j & 7) && particle >= 0) {
+#pragma unroll
+            for (int i = 0; i < kNAcc; ++i) {
+                double acc = 0.0;
+#pragma unroll
+                for (int y = 0; y < 8; ++y) acc += sV[y][i][tx];
+                v[i] = acc;
+            }
+            Fk[(int64_t)particle * N + j] = ok ? (s1 > s0 ? 0.5 * two_F(v) : 0.0) : -INFINITY;
+        }
+        __syncthreads();
+    }
+}
+
+// F = sum_k F_k: one warp per particle, lane l adds k = l, l + 32, ..., then a fixed shuffle tree.
+__global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict__ Fk, int64_t P, int32_t N,
+                                                        double *__restrict__ F)
+{
+    const int64_t q = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (q >= P) return;
+    const int lane = threadIdx.x & 31;
+    double f = 0.0;
+    for (int j = lane; j < N; j += 32) f += Fk[q * N + j];   // -inf rows (invalid particles) stay -inf
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) f += __shfl_xor_sync(0xffffffffu, f, o);
+    if (lane == 0) F[q] = f;
+}
+
+cudaError_t launch_band_cells_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
+                                       const int32_t *perm, const int32_t *band_lo, const int32_t *band_hi, int64_t P,
+                                       int64_t P_pad, int32_t n_bins, int32_t n_cells, int32_t n_seg_band,
+                                       int32_t lattice, int64_t part_sk, int64_t part_sp, double *F, double *Fk,
+                                       cudaStream_t st)
+{
+    const int gy = n_seg_band < 4096 ? n_seg_band : 4096;
+    band_cells_epilogue_kernel<<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
+        partial, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, part_sk, part_sp, Fk);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    band_fsum_kernel<<<(unsigned)((P + 3) / 4), 128, 0, st>>>(Fk, P, n_seg_band, F);
+    return cudaGetLastError();
 }
 
 cudaError_t band_kernel_configure()

@@ -142,11 +142,12 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
                                                             int32_t n_seg, const SegCrit *__restrict__ crit,
                                                             const int8_t *__restrict__ seg_maxlvl, double tol_phi_qt,
                                                             double tol_resp, int32_t force_level,
-                                                            int8_t *__restrict__ level,
+                                                            const BandSched bands, int8_t *__restrict__ level,
                                                             int32_t *__restrict__ direct_list,
                                                             int32_t *__restrict__ direct_count)
 {
     __shared__ double s3[kThreads / 32], s9[kThreads / 32];
+    __shared__ int32_t sLo[kThreads / 32], sHi[kThreads / 32], sLen[kThreads / 32];
     const int tid = threadIdx.x;
     const int grp = blockIdx.x;
     const int64_t p = (int64_t)grp * kThreads + tid;
@@ -166,10 +167,37 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
 #pragma unroll
     for (int w = 1; w < kThreads / 32; ++w) { c3 = fmax(c3, s3[w]); c9 = fmax(c9, s9[w]); }
 
+    // row f2: the group's bins [g_lo, g_hi) that at least one template is in band for, and its shortest
+    // partition (the H3 amplification is set by the partitions of the templates, not by the lattice cells)
+    const bool banded = bands.band_lo != nullptr;
+    int32_t g_lo = INT32_MAX, g_hi = 0, g_len = INT32_MAX;
+    if (banded) {
+        if (valid[p]) {
+            const int32_t C = bands.lattice, N = bands.n_seg_band;
+            const int32_t q_lo = (bands.band_lo[p] + C / 2) / C, D = (bands.band_hi[p] + C / 2) / C - q_lo;
+            const int32_t e0 = band_edge(0, q_lo, D, N, C, bands.n_bins), eN = band_edge(N, q_lo, D, N, C, bands.n_bins);
+            if (eN > e0) { g_lo = e0; g_hi = eN; g_len = max((eN - e0) / N, 1); }
+        }
+        g_lo = __reduce_min_sync(0xffffffffu, g_lo);
+        g_hi = __reduce_max_sync(0xffffffffu, g_hi);
+        g_len = __reduce_min_sync(0xffffffffu, g_len);
+        if ((tid & 31) == 0) { sLo[tid >> 5] = g_lo; sHi[tid >> 5] = g_hi; sLen[tid >> 5] = g_len; }
+        __syncthreads();
+#pragma unroll
+        for (int w = 0; w < kThreads / 32; ++w) { g_lo = min(g_lo, sLo[w]); g_hi = max(g_hi, sHi[w]); g_len = min(g_len, sLen[w]); }
+    }
+
     for (int seg = tid; seg < n_seg; seg += kThreads) {
         const int mx = seg_maxlvl[seg];
         int lvl;
-        const SegCrit q = crit[seg];
+        SegCrit q = crit[seg];
+        if (banded) {
+            if (bands.seg_edge[seg + 1] <= g_lo || bands.seg_edge[seg] >= g_hi) {     // nobody is in band here
+                level[(int64_t)grp * n_seg + seg] = (int8_t)-2;
+                continue;
+            }
+            q.kl = 0.05 * (double)g_len;
+        }
         const double om = fma(c3, q.p1, c9 * q.p2);
         const double d3 = fma(c3, q.r1, fma(c9, q.r2, q.ad * (128.0 / 3.0) * om * om * om));   // |D3|, quarter turns
         if (!(q.d2 * om < 0.015625) || !(1.25 * d3 <= 0.25 * tol_phi_qt)) {
@@ -197,13 +225,13 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
 
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
-                            double tol_resp, int32_t force_level, int8_t *level, int32_t *direct_list,
-                            int32_t *direct_count, cudaStream_t st)
+                            double tol_resp, int32_t force_level, const BandSched &bands, int8_t *level,
+                            int32_t *direct_list, int32_t *direct_count, cudaStream_t st)
 {
     cudaError_t e = cudaMemsetAsync(direct_count, 0, sizeof(int32_t), st);
     if (e != cudaSuccess) return e;
     schedule_kernel<<<(unsigned)n_groups, kThreads, 0, st>>>(coef, valid, P_pad, n_seg, crit, seg_maxlvl,
-                                                            tol_phi_qt, tol_resp, force_level, level,
+                                                            tol_phi_qt, tol_resp, force_level, bands, level,
                                                             direct_list, direct_count);
     return cudaGetLastError();
 }
@@ -541,11 +569,11 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             gram += kNGram;
         }
         if (j1 == seg_hi) {                                  // segment finished: flush its eight sums
-            double *out = a.partial + ((int64_t)cur_seg * kNPartial) * a.P_pad + p;
+            double *out = a.partial + ((int64_t)cur_seg * kNPartial) * a.P_pad + p * a.part_sp;
 #pragma unroll
-            for (int j = 0; j < kNAcc; ++j) { out[(int64_t)j * a.P_pad] = acc[j]; acc[j] = 0.0; }
-            out[(int64_t)8 * a.P_pad] = c_re;
-            out[(int64_t)9 * a.P_pad] = c_im;
+            for (int j = 0; j < kNAcc; ++j) { out[(int64_t)j * a.part_sk] = acc[j]; acc[j] = 0.0; }
+            out[(int64_t)8 * a.part_sk] = c_re;
+            out[(int64_t)9 * a.part_sk] = c_im;
             seg_start = true;
             ++cur_seg;
             if (cur_seg < run_end) seg_hi = a.seg_edge[cur_seg + 1];

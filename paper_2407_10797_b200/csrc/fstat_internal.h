@@ -68,6 +68,7 @@ constexpr int kFastTileShift = 9;
 constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the folded data (8 KiB), aligned to its size;
                                                      // >= kMaxStride so that no sub-block straddles two tiles
 constexpr int kFastStages = 3;
+constexpr int kBandFastLattice = 32;                 // row f2: from this edge lattice on the interpolating kernel is used
 constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
 
 // per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)
@@ -88,7 +89,9 @@ struct MainArgs {
     const int32_t *direct_list;   // work items (group * n_seg + segment) left to the direct kernel ...
     const int32_t *direct_count;  // ... and how many (both written by schedule_kernel)
     int32_t max_ctas;             // persistent grid size
-    double *partial;          // [n_seg][kNPartial][P_pad]
+    double *partial;          // [n_seg][kNPartial][P_pad]  (value j of slot p at j * part_sk + p * part_sp)
+    int64_t part_sk, part_sp; // (P_pad, 1): value-major, what the epilogue reads coalesced; (1, kNPartial): row f2's
+                              // cells epilogue reads one slot's record as 80 contiguous bytes
     int64_t P_pad;
     int32_t P;
     int32_t n_groups;
@@ -110,13 +113,32 @@ struct FastArgs {
     const int32_t *seg_edge;      // [n_seg + 1]
     const int32_t *seg_gbase;     // [n_seg][kNLevels] index of the segment's first sub-block in gram[level]
     const int8_t *level;          // [n_groups][n_seg]
-    double *partial;              // [n_seg][kNPartial][P_pad]
+    double *partial;              // [n_seg][kNPartial][P_pad], strides as in MainArgs
+    int64_t part_sk, part_sp;
     int64_t P_pad;
     int32_t n_groups;
     int32_t n_seg;
     int32_t segs_per_cta;         // consecutive segments one CTA walks (tiles, node ring carried across their edges)
     double df;
     OrbitCoef orb;
+};
+
+// row f2: edge j of a template's band, e_j = min(C (q_lo + floor(j D / N)), n_bins)   (reading A26)
+__host__ __device__ __forceinline__ int32_t band_edge(int32_t j, int32_t q_lo, int32_t D, int32_t N, int32_t C,
+                                                      int32_t n_bins)
+{
+    const int64_t e = (int64_t)C * ((int64_t)q_lo + ((int64_t)j * D) / N);
+    return (int32_t)(e < (int64_t)n_bins ? e : (int64_t)n_bins);
+}
+
+// what the stride selection needs to know about the bands (nullptr band_lo: fixed data-side partitions)
+struct BandSched {
+    const int32_t *band_lo;   // [P_pad]
+    const int32_t *band_hi;
+    const int32_t *seg_edge;  // [n_seg + 1]
+    int32_t n_seg_band;       // partitions per template
+    int32_t lattice;
+    int32_t n_bins;
 };
 
 // row f2 (fstat_band.cu): per-particle bands and partition edges
@@ -146,6 +168,11 @@ cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t s
 cudaError_t launch_band_epilogue(const double *rec, const int32_t *rec_idx, const int32_t *valid, const int32_t *perm,
                                  int64_t P_pad, int32_t n_wseg, int32_t n_seg, double *F, double *Fk, cudaStream_t st);
 cudaError_t band_kernel_configure();
+cudaError_t launch_band_cells_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
+                                       const int32_t *perm, const int32_t *band_lo, const int32_t *band_hi, int64_t P,
+                                       int64_t P_pad, int32_t n_bins, int32_t n_cells, int32_t n_seg_band,
+                                       int32_t lattice, int64_t part_sk, int64_t part_sp, double *F, double *Fk,
+                                       cudaStream_t st);
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
                                double df, double arm_length_m, double *table, double *dwp,
@@ -156,12 +183,13 @@ cudaError_t launch_build_gram(const double *table, const int32_t *edges, int32_t
                               int level, const int32_t *cnt, double *gram, cudaStream_t st);
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
-                            double tol_resp, int32_t force_level, int8_t *level, int32_t *direct_list,
-                            int32_t *direct_count, cudaStream_t st);
+                            double tol_resp, int32_t force_level, const BandSched &bands, int8_t *level,
+                            int32_t *direct_list, int32_t *direct_count, cudaStream_t st);
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, double *coef, int32_t *valid, int32_t *perm, cudaStream_t st);
+                            int32_t *slot_of, int32_t rank_by_band, double *coef, int32_t *valid, int32_t *perm,
+                            cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
 cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
                             const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,

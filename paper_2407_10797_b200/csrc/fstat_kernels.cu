@@ -134,18 +134,28 @@ __device__ __forceinline__ bool particle_ok(const double *__restrict__ q)
 // slot_of[i] = rank of particle i by (chirp mass rounded to float, index): a stable, deterministic sort by
 // brute force (P^2 integer comparisons through shared-memory tiles; ~1 ms at P = 65536, where one
 // evaluation takes ~200 ms).  Invalid particles sort last.
-__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P,
+// by_band != 0 (row f2): the key is M_c^(5/3) t_c instead, which orders the templates by the frequency they
+// have at t = 0 (Newtonian: f(0) ~ (M_c^(5/3) t_c)^(-3/8)), so that a group's bands overlap.
+__device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, int by_band)
+{
+    if (!particle_ok(q)) return 0xFFFFFFFFu;
+    if (!by_band) return __float_as_uint((float)q[1]);
+    const double m = q[1] * cbrt(q[1] * q[1]) * q[0];
+    return (m > 0.0) ? __float_as_uint((float)m) : 0u;
+}
+
+__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P, int by_band,
                                                    int32_t *__restrict__ slot_of)
 {
     __shared__ uint32_t skey[256];
     const int i = blockIdx.x * 256 + threadIdx.x;
     uint32_t my = 0xFFFFFFFFu;
-    if (i < P && particle_ok(params + 6 * (int64_t)i)) my = __float_as_uint((float)params[6 * (int64_t)i + 1]);
+    if (i < P) my = rank_key(params + 6 * (int64_t)i, by_band);
     int rank = 0;
     for (int j0 = 0; j0 < P; j0 += 256) {
         const int j = j0 + threadIdx.x;
         uint32_t k = 0xFFFFFFFFu;
-        if (j < P && particle_ok(params + 6 * (int64_t)j)) k = __float_as_uint((float)params[6 * (int64_t)j + 1]);
+        if (j < P) k = rank_key(params + 6 * (int64_t)j, by_band);
         __syncthreads();
         skey[threadIdx.x] = k;
         __syncthreads();
@@ -159,10 +169,11 @@ __global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ pa
 }
 
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, double *coef, int32_t *valid, int32_t *perm, cudaStream_t st)
+                            int32_t *slot_of, int32_t rank_by_band, double *coef, int32_t *valid, int32_t *perm,
+                            cudaStream_t st)
 {
     if (slot_of != nullptr) {
-        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, slot_of);
+        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_by_band, slot_of);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -273,11 +284,11 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
         }
         g0 += n_tiles;
 
-        double *out = a.partial + ((int64_t)seg * kNPartial) * a.P_pad + p;
+        double *out = a.partial + ((int64_t)seg * kNPartial) * a.P_pad + p * a.part_sp;
 #pragma unroll
-        for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.P_pad] = acc[j];
-        out[(int64_t)8 * a.P_pad] = 0.0;                   // plain basis (u_+, u_x): c = 0
-        out[(int64_t)9 * a.P_pad] = 0.0;
+        for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.part_sk] = acc[j];
+        out[(int64_t)8 * a.part_sk] = 0.0;                 // plain basis (u_+, u_x): c = 0
+        out[(int64_t)9 * a.part_sk] = 0.0;
     }
 }
 
@@ -346,28 +357,6 @@ cudaError_t launch_template(const double *table, const double *coef, int64_t P_p
 // =================================================================================================
 constexpr int kEpiX = 32, kEpiY = 8;
 
-// Add the sums of segment s (stored in its own basis (u_+, u_x - c_s u_+)) to v in the basis with constant
-// c*:  u_x - c* u_+ = (u_x - c_s u_+) + D u_+,  D = c_s - c*, so
-//   z~* = z~ + conj(D) z_+,   m~*_pc = m~_pc + conj(D) m_pp,   m~*_cc = m~_cc + 2 Re(D m~_pc) + |D|^2 m_pp.
-// D is a small difference of nearby ratios: nothing cancels here.
-__device__ __forceinline__ void add_segment(const double *__restrict__ partial, int s, int64_t P_pad, int64_t p,
-                                            double cs_r, double cs_i, double (&v)[kNAcc])
-{
-    const double *src = partial + ((int64_t)s * kNPartial) * P_pad + p;
-    double t[kNPartial];
-#pragma unroll
-    for (int j = 0; j < kNPartial; ++j) t[j] = src[(int64_t)j * P_pad];
-    const double dr = t[8] - cs_r, di = t[9] - cs_i;
-    v[0] += t[0];
-    v[1] += t[1];
-    v[2] += fma(dr, t[0], fma(di, t[1], t[2]));
-    v[3] += fma(dr, t[1], fma(-di, t[0], t[3]));
-    v[4] += t[4];
-    v[5] += fma(fma(dr, dr, di * di), t[4], fma(2.0, fma(dr, t[6], -di * t[7]), t[5]));
-    v[6] += fma(dr, t[4], t[6]);
-    v[7] += fma(-di, t[4], t[7]);
-}
-
 template <bool SEG_PAR>
 __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__restrict__ partial,
                                                                const int32_t *__restrict__ part_seg,
@@ -401,7 +390,7 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
                 for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
                 const double cs_r = partial[((int64_t)s0 * kNPartial + 8) * P_pad + p];   // common basis: the
                 const double cs_i = partial[((int64_t)s0 * kNPartial + 9) * P_pad + p];   // first segment's
-                for (int s = s0; s < s1; ++s) add_segment(partial, s, P_pad, p, cs_r, cs_i, v);
+                for (int s = s0; s < s1; ++s) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
                 fk = ok ? 0.5 * two_F(v) : ninf;
                 if (ok) fsum += fk;
             }
@@ -415,7 +404,7 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
                 if (live) {
                     const double cs_r = partial[((int64_t)s0 * kNPartial + 8) * P_pad + p];
                     const double cs_i = partial[((int64_t)s0 * kNPartial + 9) * P_pad + p];
-                    for (int s = s0 + ty; s < s1; s += kEpiY) add_segment(partial, s, P_pad, p, cs_r, cs_i, v);
+                    for (int s = s0 + ty; s < s1; s += kEpiY) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
                 }
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) sV[SEG_PAR ? ty : 0][j][tx] = v[j];
@@ -490,7 +479,7 @@ __global__ void __launch_bounds__(128) amplitude_kernel(const double *__restrict
     const int s_first = part_seg[k];
     const double cs_r = partial[((int64_t)s_first * kNPartial + 8) * P_pad + p];
     const double cs_i = partial[((int64_t)s_first * kNPartial + 9) * P_pad + p];
-    for (int s = s_first; s < part_seg[k + 1]; ++s) add_segment(partial, s, P_pad, p, cs_r, cs_i, v);
+    for (int s = s_first; s < part_seg[k + 1]; ++s) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
     const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
     const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
     double apr = 0.0, api = 0.0, acr = 0.0, aci = 0.0;
