@@ -99,19 +99,53 @@ def test_bands_repeatable_and_independent_of_batch_order(fs, bands):
     assert np.array_equal(F3, F1[perm]) and np.array_equal(Fk3, Fk1[perm]) and np.array_equal(b3, b1[perm])
 
 
-def test_bands_first_stage_sample(fs, orc):
+@pytest.fixture(scope="module")
+def first_stage(orc):
+    return syn.make_dataset(syn.CONFIGS[1], orc.template)
+
+
+@pytest.mark.parametrize("lattice", [1, 64])
+def test_bands_first_stage_sample(fs, orc, first_stage, lattice):
     """Config 1's data and particles (2.5 yr, 1 577 880 bins, N_seg = 1024) in the launch configuration
-    bench.py --bands times; a sample of particles against the oracle, every F_k of the sample."""
+    bench.py --bands times (lattice 1: every in-band bin in full; lattice 64: the interpolating kernel over
+    the lattice cells); a sample of particles against the oracle, every F_k of the sample."""
     import torch
-    ds = syn.make_dataset(syn.CONFIGS[1], orc.template)
+    ds = first_stage
     par = syn.draw_particles(ds.cfg)
     with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
         p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
-        F, Fk, band = fs.fstat_eval_batch_bands(plan, p, 1024, 1)
+        F, Fk, band = fs.fstat_eval_batch_bands(plan, p, 1024, lattice)
         torch.cuda.synchronize()
         F, Fk, band = F.cpu().numpy(), Fk.cpu().numpy(), band.cpu().numpy()
     width = band[:, 1] - band[:, 0]
     assert (width > 0).sum() > 1500
     order = np.argsort(width)
     sample = np.concatenate([order[-2:], order[(width[order] > 0).argmax():][:2], np.arange(0, 2048, 341)])
-    _check(orc, ds, par[sample], 1024, 1, F[sample], Fk[sample], band[sample])
+    _check(orc, ds, par[sample], 1024, lattice, F[sample], Fk[sample], band[sample])
+
+
+@pytest.mark.parametrize("cfg_i,n_seg,lattice", [(1, 1024, 64), (2, 16, 128), (3, 1, 512)])
+def test_bands_interpolating_kernel_against_full_model_every_value(fs, orc, first_stage, cfg_i, n_seg, lattice):
+    """At full size every F and F_k of the interpolating kernel over the lattice cells against the kernel that
+    evaluates the full model at every in-band bin (force_level = -1; itself checked against the oracle above)
+    with the same lattice.  5e-6 leaves the other half of north_star's 1e-5 to the full-model kernel."""
+    import torch
+    ds = first_stage                                      # configs 1-3 share the data; the particles differ
+    par = syn.draw_particles(syn.CONFIGS[cfg_i])
+    direct = fs.fstat_default_options()
+    direct.force_level = -1
+    out = []
+    for opts in (None, direct):
+        with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), opts) as plan:
+            p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+            F, Fk, band = fs.fstat_eval_batch_bands(plan, p, n_seg, lattice)
+            torch.cuda.synchronize()
+            out.append((F.cpu().numpy(), Fk.cpu().numpy(), band.cpu().numpy()))
+    (F_a, Fk_a, b_a), (F_b, Fk_b, b_b) = out
+    assert np.array_equal(b_a, b_b)
+    assert np.array_equal(Fk_a == 0.0, Fk_b == 0.0)
+    live = Fk_b != 0.0
+    assert live.sum() > 0.2 * live.size
+    assert np.max(np.abs(Fk_a[live] - Fk_b[live]) / np.abs(Fk_b[live])) <= 5e-6
+    ok = F_b != 0.0
+    assert np.max(np.abs(F_a[ok] - F_b[ok]) / np.abs(F_b[ok])) <= 5e-6
