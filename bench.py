@@ -389,6 +389,20 @@ def run_ours(args):
                       "template_bins_per_s": float(n_sw * 128) * ds.n_bins / (ms_it * 1e-3),
                       "overhead_vs_eval_step": ms_it / ms_step - 1.0, "best_F_max": float(bf.max())}
         fs.fstat_pso_destroy(pso)
+        if args.bands > 0:
+            # rows f1 x f2: the same swarms with fstat_eval_batch_bands as their fitness
+            po = fs.fstat_pso_default_options(band_n_seg=args.bands, band_lattice=args.bands_lattice)
+            pso = fs.fstat_pso_create(plan, n_sw, 128, args.pso, lo, hi, seed=1, opts=po, stream=stream)
+            fs.fstat_pso_iterate(pso, 3, stream)
+            torch.cuda.synchronize()
+            p0.record(stream)
+            fs.fstat_pso_iterate(pso, args.pso, stream)
+            p1.record(stream)
+            torch.cuda.synchronize()
+            _, bf = fs.fstat_pso_best(pso, stream)
+            out["pso"]["bands_fitness"] = {"n_seg": args.bands, "edge_lattice": args.bands_lattice,
+                                           "ms_per_iteration": p0.elapsed_time(p1) / args.pso, "best_F_max": float(bf.max())}
+            fs.fstat_pso_destroy(pso)
     if args.bands > 0:
         # row f2: the paper's own segment limits; unit = IN-BAND template-bins (bins with t_f in [0, T] per particle)
         for _ in range(2):

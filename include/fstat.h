@@ -244,6 +244,10 @@ typedef struct {
     double c1, c2;            /* acceleration constants, default 2, 2 (:162)          */
     double v_max;             /* velocity clamp in box units, default 0.5 (:162)      */
     double w_start, w_end;    /* inertia weight at the first / last iteration: 0.9, 0.4 */
+    int32_t band_n_seg;       /* 0 (default): fitness = fstat_eval_batch with the plan's partitions;
+                                 >= 1: fitness = fstat_eval_batch_bands with this many segments per template
+                                 (the paper's own segment limits)                             */
+    int32_t band_lattice;     /* edge lattice of that call in bins, default 64                            */
 } fstat_pso_options;
 
 FSTAT_API void fstat_pso_default_options(fstat_pso_options *opts);

@@ -43,7 +43,7 @@ class Options(C.Structure):
 class PsoOptions(C.Structure):
     """fstat_pso_options of include/fstat.h."""
     _fields_ = [("c1", C.c_double), ("c2", C.c_double), ("v_max", C.c_double), ("w_start", C.c_double),
-                ("w_end", C.c_double)]
+                ("w_end", C.c_double), ("band_n_seg", C.c_int32), ("band_lattice", C.c_int32)]
 
 
 def library_path() -> str:

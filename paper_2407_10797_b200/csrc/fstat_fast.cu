@@ -187,7 +187,8 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
         for (int w = 0; w < kThreads / 32; ++w) { g_lo = min(g_lo, sLo[w]); g_hi = max(g_hi, sHi[w]); g_len = min(g_len, sLen[w]); }
     }
 
-    for (int seg = tid; seg < n_seg; seg += kThreads) {
+    // blockIdx.y splits the segments of the group (thousands of lattice cells in row f2)
+    for (int seg = blockIdx.y * kThreads + tid; seg < n_seg; seg += gridDim.y * kThreads) {
         const int mx = seg_maxlvl[seg];
         int lvl;
         SegCrit q = crit[seg];
@@ -230,7 +231,8 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
 {
     cudaError_t e = cudaMemsetAsync(direct_count, 0, sizeof(int32_t), st);
     if (e != cudaSuccess) return e;
-    schedule_kernel<<<(unsigned)n_groups, kThreads, 0, st>>>(coef, valid, P_pad, n_seg, crit, seg_maxlvl,
+    const unsigned gy = (unsigned)((n_seg + 16 * kThreads - 1) / (16 * kThreads));       // <= 16 segments per thread
+    schedule_kernel<<<dim3((unsigned)n_groups, gy < 1 ? 1 : (gy > 64 ? 64 : gy)), kThreads, 0, st>>>(coef, valid, P_pad, n_seg, crit, seg_maxlvl,
                                                             tol_phi_qt, tol_resp, force_level, bands, level,
                                                             direct_list, direct_count);
     return cudaGetLastError();

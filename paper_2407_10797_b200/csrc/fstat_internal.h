@@ -188,7 +188,7 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, int32_t rank_by_band, double *coef, int32_t *valid, int32_t *perm,
+                            int32_t *slot_of, double rank_band_T, double *coef, int32_t *valid, int32_t *perm,
                             cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
 cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,

@@ -134,28 +134,37 @@ __device__ __forceinline__ bool particle_ok(const double *__restrict__ q)
 // slot_of[i] = rank of particle i by (chirp mass rounded to float, index): a stable, deterministic sort by
 // brute force (P^2 integer comparisons through shared-memory tiles; ~1 ms at P = 65536, where one
 // evaluation takes ~200 ms).  Invalid particles sort last.
-// by_band != 0 (row f2): the key is M_c^(5/3) t_c instead, which orders the templates by the frequency they
-// have at t = 0 (Newtonian: f(0) ~ (M_c^(5/3) t_c)^(-3/8)), so that a group's bands overlap.
-__device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, int by_band)
+// band_T > 0 (row f2; band_T = the observation time): the key is M_c^(5/3) t_c instead, which orders the
+// templates by the frequency they have at t = 0 (Newtonian: f(0) ~ (M_c^(5/3) t_c)^(-3/8)), inside classes of
+// similar t_c / T (half octaves: the band's width f(T)/f(0) = (1 - T/t_c)^(-3/8) depends on t_c alone), so that
+// the bands of a group of 128 overlap at both ends.  Batches of fewer than 1024 particles use one class.
+__device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, double band_T, int use_classes)
 {
     if (!particle_ok(q)) return 0xFFFFFFFFu;
-    if (!by_band) return __float_as_uint((float)q[1]);
+    if (!(band_T > 0.0)) return __float_as_uint((float)q[1]);
     const double m = q[1] * cbrt(q[1] * q[1]) * q[0];
-    return (m > 0.0) ? __float_as_uint((float)m) : 0u;
+    if (!(m > 0.0)) return 0u;
+    uint32_t cls = 0;
+    if (use_classes) {
+        const double r = q[0] / band_T;
+        const int c = (r > 1.0) ? (int)(2.0 * log2(r)) : 0;
+        cls = (uint32_t)(c > 14 ? 14 : c);
+    }
+    return (cls << 28) | (__float_as_uint((float)m) >> 4);
 }
 
-__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P, int by_band,
+__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P, double band_T,
                                                    int32_t *__restrict__ slot_of)
 {
     __shared__ uint32_t skey[256];
     const int i = blockIdx.x * 256 + threadIdx.x;
     uint32_t my = 0xFFFFFFFFu;
-    if (i < P) my = rank_key(params + 6 * (int64_t)i, by_band);
+    if (i < P) my = rank_key(params + 6 * (int64_t)i, band_T, P >= 1024);
     int rank = 0;
     for (int j0 = 0; j0 < P; j0 += 256) {
         const int j = j0 + threadIdx.x;
         uint32_t k = 0xFFFFFFFFu;
-        if (j < P) k = rank_key(params + 6 * (int64_t)j, by_band);
+        if (j < P) k = rank_key(params + 6 * (int64_t)j, band_T, P >= 1024);
         __syncthreads();
         skey[threadIdx.x] = k;
         __syncthreads();
@@ -169,11 +178,11 @@ __global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ pa
 }
 
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, int32_t rank_by_band, double *coef, int32_t *valid, int32_t *perm,
+                            int32_t *slot_of, double rank_band_T, double *coef, int32_t *valid, int32_t *perm,
                             cudaStream_t st)
 {
     if (slot_of != nullptr) {
-        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_by_band, slot_of);
+        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_band_T, slot_of);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

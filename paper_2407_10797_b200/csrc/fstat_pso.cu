@@ -172,6 +172,9 @@ __global__ void __launch_bounds__(128) pso_swarm_best_kernel(int32_t n_particles
 
 }  // namespace
 
+struct fstat_pso;
+static fstat_status pso_fitness(fstat_pso *ps, cudaStream_t st);
+
 struct fstat_pso {
     fstat_plan *plan = nullptr;
     int32_t n_swarms = 0, n_particles = 0, n_iter_total = 0, n = 0;
@@ -194,12 +197,22 @@ struct fstat_pso {
         }                                                                                           \
     } while (0)
 
+// the fitness of all particles of all swarms: the plan's fixed partitions, or (rows f1 x f2) per-template bands
+static fstat_status pso_fitness(fstat_pso *ps, cudaStream_t st)
+{
+    if (ps->opt.band_n_seg >= 1)
+        return fstat_eval_batch_bands(ps->plan, ps->n, ps->d_params, ps->opt.band_n_seg, ps->opt.band_lattice, ps->d_F,
+                                      nullptr, nullptr, (void *)st);
+    return fstat_eval_batch(ps->plan, ps->n, ps->d_params, ps->d_F, nullptr, (void *)st);
+}
+
 extern "C" {
 
 void fstat_pso_default_options(fstat_pso_options *o)
 {
     if (!o) return;
     o->c1 = 2.0; o->c2 = 2.0; o->v_max = 0.5; o->w_start = 0.9; o->w_end = 0.4;
+    o->band_n_seg = 0; o->band_lattice = 64;
 }
 
 void fstat_pso_destroy(fstat_pso *ps)
@@ -228,7 +241,7 @@ static fstat_status pso_create_impl(fstat_pso *ps, cudaStream_t st)
     const int nt = 128, nb = (ps->n + nt - 1) / nt;
     pso_init_kernel<<<nb, nt, 0, st>>>(ps->n, ps->seed, ps->opt.v_max, ps->box, ps->d_x, ps->d_v, ps->d_params);
     PSO_TRY(ps, cudaGetLastError());
-    fstat_status s = fstat_eval_batch(ps->plan, ps->n, ps->d_params, ps->d_F, nullptr, (void *)st);
+    fstat_status s = pso_fitness(ps, st);
     if (s != FSTAT_OK) { ps->err = fstat_last_error(ps->plan); return s; }
     pso_first_best_kernel<<<nb, nt, 0, st>>>(ps->n, ps->d_x, ps->d_F, ps->d_pbest, ps->d_pbest_f);
     PSO_TRY(ps, cudaGetLastError());
@@ -247,7 +260,8 @@ fstat_status fstat_pso_create(fstat_pso **out, fstat_plan *plan, int32_t n_swarm
     fstat_pso_options o;
     fstat_pso_default_options(&o);
     if (opts) o = *opts;
-    if (!(o.v_max > 0.0) || !isfinite(o.c1) || !isfinite(o.c2) || !isfinite(o.w_start) || !isfinite(o.w_end))
+    if (!(o.v_max > 0.0) || !isfinite(o.c1) || !isfinite(o.c2) || !isfinite(o.w_start) || !isfinite(o.w_end) ||
+        o.band_n_seg < 0 || (o.band_n_seg >= 1 && o.band_lattice < 1))
         return FSTAT_EINVAL;
     for (int d = 0; d < kDim; ++d)
         if (!isfinite(lo[d]) || !isfinite(hi[d]) || !(hi[d] >= lo[d])) return FSTAT_EINVAL;
@@ -284,7 +298,7 @@ fstat_status fstat_pso_iterate(fstat_pso *ps, int32_t n_iter, void *stream)
                                            ps->opt.v_max, ps->box, ps->d_x, ps->d_v, ps->d_pbest, ps->d_pbest_f,
                                            ps->d_params);
         if (cudaGetLastError() != cudaSuccess) { ps->err = "pso_step_kernel launch failed"; rc = FSTAT_ECUDA; break; }
-        rc = fstat_eval_batch(ps->plan, ps->n, ps->d_params, ps->d_F, nullptr, (void *)st);
+        rc = pso_fitness(ps, st);
         if (rc != FSTAT_OK) { ps->err = fstat_last_error(ps->plan); break; }
         pso_update_best_kernel<<<nb, nt, 0, st>>>(ps->n, ps->d_x, ps->d_F, ps->d_pbest, ps->d_pbest_f);
         if (cudaGetLastError() != cudaSuccess) { ps->err = "pso_update_best_kernel launch failed"; rc = FSTAT_ECUDA; break; }

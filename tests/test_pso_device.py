@@ -138,3 +138,39 @@ def test_many_iterations_without_host_sync_improve_every_swarm(gpu, orc):
             fs.fstat_pso_create(plan, 0, 128, 40, lo, hi)
         with pytest.raises(fs.FstatError):
             fs.fstat_pso_create(plan, 1, 16, 10, hi, lo)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("lattice", [64, 1])
+def test_device_swarms_with_the_papers_segment_limits_as_fitness(gpu, orc, lattice):
+    """Rows f1 x f2: band_n_seg >= 1 makes the swarm's fitness fstat_eval_batch_bands (per-template bands,
+    PAPER.md:122).  Same step-by-step bit-equality of the swarm state with the PSO oracle fed the device's F;
+    the fitness itself against the oracle's fstat_bands at the first and last iteration."""
+    fs = gpu
+    ds = syn.make_dataset(syn.BANDS_SMALL, orc.template)
+    inj = ds.inj_params
+    lo = np.array([inj[0] - 3000.0, inj[1] * 0.998, 0.2, inj[3] - 0.1, inj[4] - 0.1, 0.0])
+    hi = np.array([inj[0] + 3000.0, inj[1] * 1.002, 0.25, inj[3] + 0.1, inj[4] + 0.1, 0.1])
+    n_swarms, n_part, n_iter, seed, n_seg = 2, 16, 6, 99, 4
+    opts = fs.fstat_pso_default_options(band_n_seg=n_seg, band_lattice=lattice)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
+        with fs.fstat_pso_create(plan, n_swarms, n_part, n_iter, lo, hi, seed, opts) as pso:
+            x_o, v_o = po.init(n_swarms, n_part, seed)
+            x, v, pb, pf, fl = fs.fstat_pso_state(pso)
+            np.testing.assert_array_equal(x, x_o)
+            F_o, _, _ = orc.fstat_bands(ds.freq, ds.dw, ds.inv_sn, po.to_params(x_o, lo, hi), n_seg, lattice)
+            assert np.max(np.abs(fl - F_o) / np.abs(F_o)) <= 1e-5
+            pb_o, pf_o = x_o.copy(), fl.copy()
+            for it in range(1, n_iter + 1):
+                fs.fstat_pso_iterate(pso, 1)
+                x, v, pb, pf, fl = fs.fstat_pso_state(pso)
+                x_o, v_o = po.step(x_o, v_o, pb_o, pf_o, n_part, it, n_iter, seed)
+                np.testing.assert_array_equal(x, x_o, err_msg="iteration %d" % it)
+                np.testing.assert_array_equal(v, v_o)
+                par_o = po.to_params(x_o, lo, hi)
+                outside = np.isnan(par_o[:, 0])
+                assert np.all(np.isneginf(fl[outside])) and np.all(np.isfinite(fl[~outside]))
+                pb_o, pf_o = po.update_best(x_o, fl, pb_o, pf_o)
+                np.testing.assert_array_equal(pf, pf_o)
+            F_o, _, _ = orc.fstat_bands(ds.freq, ds.dw, ds.inv_sn, par_o[~outside], n_seg, lattice)
+            assert np.max(np.abs(fl[~outside] - F_o) / np.abs(F_o)) <= 1e-5
