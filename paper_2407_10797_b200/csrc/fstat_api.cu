@@ -649,7 +649,8 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
 
     CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
     CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, br ? 1.0 / pl->df : 0.0, pl->d_coef,
+    const double rank_band[3] = {1.0 / pl->df, pl->f0, pl->f0 + (double)(pl->n_bins - 1) * pl->df};
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, br ? rank_band : nullptr, pl->d_coef,
                                pl->d_valid, pl->d_perm, st));
     BandSched bs{};
     if (br) {
@@ -801,7 +802,8 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
         CU_TRY(pl, grow(&pl->d_band_fk, &pl->band_fk_cap, (size_t)P * (size_t)n_seg));
         Fk = pl->d_band_fk;
     }
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, 1.0 / pl->df, pl->d_coef, pl->d_valid,
+    const double rank_band[3] = {1.0 / pl->df, pl->f0, pl->f0 + (double)(pl->n_bins - 1) * pl->df};
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, rank_band, pl->d_coef, pl->d_valid,
                                pl->d_perm, st));
     CU_TRY(pl, launch_band_limits(pl->d_table, pl->d_coef, pl->d_valid, pl->d_perm, P_pad, (int32_t)pl->n_bins, 1.0 / pl->df,
                                   pl->opt.orbit_kappa, pl->d_band, pl->d_band + P_pad, band, st));
@@ -875,7 +877,7 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
     CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)kThreads * kNCoef));
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)kThreads));
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
-    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, 0.0, pl->d_coef,
+    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, nullptr, pl->d_coef,
                                pl->d_valid, nullptr, st));
     CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, u_plus, u_cross, st));
     CU_TRY(pl, cudaStreamSynchronize(st));

@@ -187,8 +187,9 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
                             int32_t *direct_list, int32_t *direct_count, cudaStream_t st);
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
+// rank_band: nullptr (slots ranked by chirp mass) or HOST {T_obs, f_first, f_last} (row f2: ranked by band)
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, double rank_band_T, double *coef, int32_t *valid, int32_t *perm,
+                            int32_t *slot_of, const double *rank_band, double *coef, int32_t *valid, int32_t *perm,
                             cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
 cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,

@@ -134,37 +134,36 @@ __device__ __forceinline__ bool particle_ok(const double *__restrict__ q)
 // slot_of[i] = rank of particle i by (chirp mass rounded to float, index): a stable, deterministic sort by
 // brute force (P^2 integer comparisons through shared-memory tiles; ~1 ms at P = 65536, where one
 // evaluation takes ~200 ms).  Invalid particles sort last.
-// band_T > 0 (row f2; band_T = the observation time): the key is M_c^(5/3) t_c instead, which orders the
-// templates by the frequency they have at t = 0 (Newtonian: f(0) ~ (M_c^(5/3) t_c)^(-3/8)), inside classes of
-// similar t_c / T (half octaves: the band's width f(T)/f(0) = (1 - T/t_c)^(-3/8) depends on t_c alone), so that
-// the bands of a group of 128 overlap at both ends.  Batches of fewer than 1024 particles use one class.
-__device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, double band_T, int use_classes)
+// band_T > 0 (row f2; band_T = the observation time, [band_f0, band_f1] = the grid): the key is a weighted
+// mean of the Newtonian estimates of the template's frequencies at t = 0 and t = T, clipped to the grid,
+// f(t) = (1/pi) (5 / (256 (t_c - t)))^(3/8) (G M_c / c^3)^(-5/8), so that the bands of a group of 128 overlap
+// at both ends (the upper end weighs more: it moves faster with t_c).  Only the ORDER matters: the bands
+// themselves come from band_kernel.
+__device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, double band_T, double band_f0, double band_f1)
 {
     if (!particle_ok(q)) return 0xFFFFFFFFu;
     if (!(band_T > 0.0)) return __float_as_uint((float)q[1]);
-    const double m = q[1] * cbrt(q[1] * q[1]) * q[0];
-    if (!(m > 0.0)) return 0u;
-    uint32_t cls = 0;
-    if (use_classes) {
-        const double r = q[0] / band_T;
-        const int c = (r > 1.0) ? (int)(2.0 * log2(r)) : 0;
-        cls = (uint32_t)(c > 14 ? 14 : c);
-    }
-    return (cls << 28) | (__float_as_uint((float)m) >> 4);
+    const double tc = q[0];
+    if (!(tc > 0.0)) return 0u;
+    const double m = pow(q[1] * kGMsunC3, -0.625) * (1.0 / kPi) * pow(5.0 / 256.0, 0.375);
+    const double fa = fmin(fmax(m * pow(tc, -0.375), band_f0), band_f1);
+    const double fb = (tc > band_T) ? fmin(fmax(m * pow(tc - band_T, -0.375), band_f0), band_f1) : band_f1;
+    return __float_as_uint((float)(0.4 * fa + 0.6 * fb));
 }
 
-__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P, double band_T,
+__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P, double band_T, double band_f0,
+                                                   double band_f1,
                                                    int32_t *__restrict__ slot_of)
 {
     __shared__ uint32_t skey[256];
     const int i = blockIdx.x * 256 + threadIdx.x;
     uint32_t my = 0xFFFFFFFFu;
-    if (i < P) my = rank_key(params + 6 * (int64_t)i, band_T, P >= 1024);
+    if (i < P) my = rank_key(params + 6 * (int64_t)i, band_T, band_f0, band_f1);
     int rank = 0;
     for (int j0 = 0; j0 < P; j0 += 256) {
         const int j = j0 + threadIdx.x;
         uint32_t k = 0xFFFFFFFFu;
-        if (j < P) k = rank_key(params + 6 * (int64_t)j, band_T, P >= 1024);
+        if (j < P) k = rank_key(params + 6 * (int64_t)j, band_T, band_f0, band_f1);
         __syncthreads();
         skey[threadIdx.x] = k;
         __syncthreads();
@@ -178,11 +177,12 @@ __global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ pa
 }
 
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, double rank_band_T, double *coef, int32_t *valid, int32_t *perm,
+                            int32_t *slot_of, const double *rank_band, double *coef, int32_t *valid, int32_t *perm,
                             cudaStream_t st)
 {
     if (slot_of != nullptr) {
-        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_band_T, slot_of);
+        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_band ? rank_band[0] : 0.0,
+                                                                 rank_band ? rank_band[1] : 0.0, rank_band ? rank_band[2] : 0.0, slot_of);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
