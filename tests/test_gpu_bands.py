@@ -149,3 +149,29 @@ def test_bands_interpolating_kernel_against_full_model_every_value(fs, orc, firs
     assert np.max(np.abs(Fk_a[live] - Fk_b[live]) / np.abs(Fk_b[live])) <= 5e-6
     ok = F_b != 0.0
     assert np.max(np.abs(F_a[ok] - F_b[ok]) / np.abs(F_b[ok])) <= 5e-6
+
+
+def test_bands_wide_band_in_particle_batches(fs, orc):
+    """Config 4's grid (7.1 M bins to 100 mHz, across the TDI null): 111 k lattice cells make the record
+    workspace 8.9 MB per particle, so P = 4096 is evaluated in two particle batches.  A sample against the oracle,
+    and the whole batch against the same particles evaluated 512 at a time (other groups, other strides)."""
+    import torch
+    cfg = syn.CONFIGS[4]
+    ds = syn.make_dataset(cfg, orc.template)
+    par = syn.draw_particles(cfg, 4096)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
+        p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+        F, Fk, band = fs.fstat_eval_batch_bands(plan, p, 16, 64)
+        torch.cuda.synchronize()
+        parts = [fs.fstat_eval_batch_bands(plan, p[i:i + 512].contiguous(), 16, 64) for i in range(0, 4096, 512)]
+        torch.cuda.synchronize()
+    F, Fk, band = F.cpu().numpy(), Fk.cpu().numpy(), band.cpu().numpy()
+    F2 = np.concatenate([q[0].cpu().numpy() for q in parts])
+    Fk2 = np.concatenate([q[1].cpu().numpy() for q in parts])
+    b2 = np.concatenate([q[2].cpu().numpy() for q in parts])
+    assert np.array_equal(band, b2) and np.array_equal(Fk == 0.0, Fk2 == 0.0)
+    live = Fk2 != 0.0
+    assert live.sum() > 0.5 * live.size
+    assert np.max(np.abs(Fk[live] - Fk2[live]) / np.abs(Fk2[live])) <= 5e-6
+    sample = np.array([0, 1500, 2047, 2048, 3000, 4095])      # both batches
+    _check(orc, ds, par[sample], 16, 64, F[sample], Fk[sample], band[sample])
