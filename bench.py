@@ -419,10 +419,17 @@ def run_ours(args):
         ms_b = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs]))
         kms = fs.fstat_plan_main_kernel_ms(plan, n_b)
         in_band = float((band[:, 1] - band[:, 0]).sum().item())
+        # end to end through the host-buffer call: params in, F, F_k and the band limits out
+        fs.fstat_eval_batch_bands_host(plan, par_np, args.bands, args.bands_lattice, stream)
+        t0 = time.perf_counter()
+        for _ in range(n_b):
+            fs.fstat_eval_batch_bands_host(plan, par_np, args.bands, args.bands_lattice, stream)
+        ms_b_e2e = (time.perf_counter() - t0) * 1e3 / n_b
         out["bands"] = {"n_seg": args.bands, "edge_lattice": args.bands_lattice, "ms_per_step": ms_b,
                         "main_kernel_ms": float(np.mean(kms)) if len(kms) else None,
                         "in_band_template_bins": in_band, "in_band_share_of_grid": in_band / (float(P) * ds.n_bins),
                         "in_band_template_bins_per_s": in_band * world / (ms_b * 1e-3),
+                        "e2e_ms_per_step": ms_b_e2e, "e2e_in_band_template_bins_per_s": in_band * world / (ms_b_e2e * 1e-3),
                         "kernel": "fstat_fast_kernel over the lattice cells" if args.bands_lattice >= 32
                                   else "fstat_band_kernel (full model at every in-band bin)"}
     if world == 1 and not args.no_cpu_baseline:

@@ -147,6 +147,13 @@ FSTAT_API fstat_status fstat_eval_batch_bands(fstat_plan *plan, int64_t P, const
                                               int32_t edge_lattice, double *F, double *Fk, int64_t *band,
                                               void *cuda_stream);
 
+/* fstat_eval_batch_bands with HOST buffers (params_host [P][6] in; F_host [P], Fk_host [P][n_seg] or NULL,
+ * band_host [P][2] or NULL out): copies inside, returns after the results have landed.  Pinned buffers make the
+ * copies asynchronous DMA. */
+FSTAT_API fstat_status fstat_eval_batch_bands_host(fstat_plan *plan, int64_t P, const double *params_host,
+                                                   int32_t n_seg, int32_t edge_lattice, double *F_host,
+                                                   double *Fk_host, int64_t *band_host, void *cuda_stream);
+
 /*
  * fstat_eval_amplitudes -- the maximum-likelihood extrinsic amplitudes a = M^-1 N of every partition
  * (Eq. 10; a_1..a_4 multiply the basis templates A^1 = u_+, A^2 = u_x, A^3 = i u_+, A^4 = i u_x of

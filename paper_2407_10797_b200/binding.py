@@ -18,7 +18,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 # every symbol include/fstat.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
-    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
+    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
@@ -73,6 +73,8 @@ def load_library():
         L.fstat_eval_amplitudes.restype = C.c_int
         L.fstat_eval_batch_bands.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
         L.fstat_eval_batch_bands.restype = C.c_int
+        L.fstat_eval_batch_bands_host.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
+        L.fstat_eval_batch_bands_host.restype = C.c_int
         L.fstat_eval_batch_host.argtypes = [vp, i64, vp, vp, vp, vp]
         L.fstat_eval_batch_host.restype = C.c_int
         L.fstat_eval_template.argtypes = [vp, dp, vp, vp, vp]
@@ -271,6 +273,18 @@ def fstat_eval_batch_bands(plan: Plan, params, n_seg: int, edge_lattice: int = 1
                                                  _dev_ptr(Fk, "Fk", P * int(n_seg)) if want_Fk else None,
                                                  band.data_ptr() if want_band else None, _stream_ptr(stream)),
            "fstat_eval_batch_bands", plan)
+    return F, Fk, band
+
+
+def fstat_eval_batch_bands_host(plan: Plan, params, n_seg: int, edge_lattice: int = 1, stream=None):
+    """HOST buffers: params [P][6] float64 numpy array -> (F [P], Fk [P][n_seg], band [P][2] int64) numpy arrays,
+    filled when the call returns."""
+    par = np.ascontiguousarray(params, dtype=np.float64).reshape(-1, 6)
+    P = par.shape[0]
+    F, Fk, band = np.empty(P), np.empty((P, int(n_seg))), np.empty((P, 2), dtype=np.int64)
+    _check(load_library().fstat_eval_batch_bands_host(plan.handle, P, par.ctypes.data, int(n_seg), int(edge_lattice),
+                                                      F.ctypes.data, Fk.ctypes.data, band.ctypes.data, _stream_ptr(stream)),
+           "fstat_eval_batch_bands_host", plan)
     return F, Fk, band
 
 

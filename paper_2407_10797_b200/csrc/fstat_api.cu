@@ -63,6 +63,7 @@ struct fstat_plan {
     double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
     int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
     double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
+    int64_t *d_band_out = nullptr; size_t band_out_cap = 0; // [P][2] (host-buffer call)
     // host-buffer path
     double *d_params = nullptr, *d_F = nullptr, *d_Fk = nullptr;
     size_t params_cap = 0, F_cap = 0, Fk_cap = 0;
@@ -446,7 +447,7 @@ static void plan_free(fstat_plan *pl)
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
-    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk);
+    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out);
     cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
@@ -833,6 +834,35 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
     ++pl->n_timed;
     CU_TRY(pl, launch_band_epilogue(pl->d_rec, pl->d_rec_idx, pl->d_valid, pl->d_perm, P_pad, (int32_t)n_wseg, n_seg, F, Fk, st));
     pl->n_launches += 5;                               // rank, prologue, band limits, band main, band epilogue
+    return FSTAT_OK;
+}
+
+fstat_status fstat_eval_batch_bands_host(fstat_plan *pl, int64_t P, const double *params_host, int32_t n_seg,
+                                         int32_t edge_lattice, double *F_host, double *Fk_host, int64_t *band_host,
+                                         void *stream)
+{
+    if (!pl) return FSTAT_EINVAL;
+    if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
+    if (n_seg < 1 || edge_lattice < 1) return fail(pl, FSTAT_EINVAL, "n_seg < 1 or edge_lattice < 1");
+    if (P == 0) return FSTAT_OK;
+    if (!params_host || !F_host) return fail(pl, FSTAT_EINVAL, "params_host or F_host is NULL");
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(pl, grow(&pl->d_params, &pl->params_cap, (size_t)P * 6));
+    CU_TRY(pl, grow(&pl->d_F, &pl->F_cap, (size_t)P));
+    if (Fk_host) CU_TRY(pl, grow(&pl->d_Fk, &pl->Fk_cap, (size_t)P * (size_t)n_seg));
+    if (band_host) CU_TRY(pl, grow(&pl->d_band_out, &pl->band_out_cap, (size_t)P * 2));
+    CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, (size_t)P * 6 * sizeof(double), cudaMemcpyHostToDevice, st));
+    fstat_status s = fstat_eval_batch_bands(pl, P, pl->d_params, n_seg, edge_lattice, pl->d_F, Fk_host ? pl->d_Fk : nullptr,
+                                            band_host ? pl->d_band_out : nullptr, stream);
+    if (s != FSTAT_OK) return s;
+    CU_TRY(pl, cudaMemcpyAsync(F_host, pl->d_F, (size_t)P * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (Fk_host)
+        CU_TRY(pl, cudaMemcpyAsync(Fk_host, pl->d_Fk, (size_t)P * (size_t)n_seg * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (band_host)
+        CU_TRY(pl, cudaMemcpyAsync(band_host, pl->d_band_out, (size_t)P * 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    CU_TRY(pl, cudaStreamSynchronize(st));
     return FSTAT_OK;
 }
 

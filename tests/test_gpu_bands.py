@@ -105,6 +105,16 @@ def first_stage(orc):
 
 
 @pytest.mark.parametrize("lattice", [1, 64])
+def test_bands_host_buffers_give_the_same_bits(fs, bands, lattice):
+    ds = bands
+    par = syn.draw_particles(ds.cfg)
+    F, Fk, band = _gpu(fs, ds, par, 16, lattice)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
+        F_h, Fk_h, band_h = fs.fstat_eval_batch_bands_host(plan, par, 16, lattice)
+    assert np.array_equal(F, F_h) and np.array_equal(Fk, Fk_h) and np.array_equal(band, band_h)
+
+
+@pytest.mark.parametrize("lattice", [1, 64])
 def test_bands_first_stage_sample(fs, orc, first_stage, lattice):
     """Config 1's data and particles (2.5 yr, 1 577 880 bins, N_seg = 1024) in the launch configuration
     bench.py --bands times (lattice 1: every in-band bin in full; lattice 64: the interpolating kernel over
