@@ -320,6 +320,46 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
     }
 }
 
+// Many partitions of a few cells each (N_seg in the hundreds): one thread per (slot, partition), x = 32 slots,
+// y = 8 partitions per block, no shared memory.  Same sums in the same order per partition as the kernel above
+// would give with one lane (the order of the cells), so both are deterministic; they differ in rounding only.
+__global__ void __launch_bounds__(256) band_cells_epilogue_flat_kernel(const double *__restrict__ partial,
+                                                                       const int32_t *__restrict__ part_seg,
+                                                                       const int32_t *__restrict__ valid,
+                                                                       const int32_t *__restrict__ perm,
+                                                                       const int32_t *__restrict__ band_lo,
+                                                                       const int32_t *__restrict__ band_hi,
+                                                                       int64_t P_pad, int32_t n_bins, int32_t n_cells,
+                                                                       int32_t N, int32_t C, int64_t sk, int64_t sp,
+                                                                       double *__restrict__ Fk)
+{
+    const int64_t p = (int64_t)blockIdx.x * 32 + threadIdx.x;
+    const int32_t particle = perm[p];
+    if (particle < 0) return;
+    const bool ok = valid[p] != 0;
+    const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
+    for (int j = blockIdx.y * 8 + threadIdx.y; j < N; j += gridDim.y * 8) {
+        double fk = -INFINITY;
+        if (ok) {
+            const int32_t ea = band_edge(j, q_lo, D, N, C, n_bins), eb = band_edge(j + 1, q_lo, D, N, C, n_bins);
+            const int32_t ca = ea >= n_bins ? n_cells : ea / C, cb = eb >= n_bins ? n_cells : eb / C;
+            const int s0 = part_seg[ca], s1 = part_seg[cb];
+            fk = 0.0;
+            if (s1 > s0) {
+                double v[kNAcc];
+#pragma unroll
+                for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
+                const double *first = partial + ((int64_t)s0 * kNPartial) * P_pad + p * sp;
+                const double cs_r = first[8 * sk], cs_i = first[9 * sk];
+#pragma unroll 2
+                for (int s = s0; s < s1; ++s) add_segment(partial, s, P_pad, sk, sp, p, cs_r, cs_i, v);
+                fk = 0.5 * two_F(v);
+            }
+        }
+        Fk[(int64_t)particle * N + j] = fk;
+    }
+}
+
 // F = sum_k F_k: one warp per particle, lane l adds k = l, l + 32, ..., then a fixed shuffle tree.
 __global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict__ Fk, int64_t P, int32_t N,
                                                         double *__restrict__ F)
@@ -340,6 +380,17 @@ cudaError_t launch_band_cells_epilogue(const double *partial, const int32_t *par
                                        int32_t lattice, int64_t part_sk, int64_t part_sp, double *F, double *Fk,
                                        cudaStream_t st)
 {
+    if ((int64_t)n_cells < (int64_t)32 * n_seg_band) {      // a few cells per partition: one thread per partition
+        int gy = (n_seg_band + 7) / 8;
+        if (gy > 4096) gy = 4096;
+        band_cells_epilogue_flat_kernel<<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
+            partial, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, part_sk,
+            part_sp, Fk);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        band_fsum_kernel<<<(unsigned)((P + 3) / 4), 128, 0, st>>>(Fk, P, n_seg_band, F);
+        return cudaGetLastError();
+    }
     const int gy = n_seg_band < 4096 ? n_seg_band : 4096;
     band_cells_epilogue_kernel<<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
         partial, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, part_sk, part_sp, Fk);
