@@ -62,6 +62,7 @@ struct fstat_plan {
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
     double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
     int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
+    double *d_rag = nullptr; size_t rag_cap = 0;          // [P_pad][n_seg + 1][2][kNAcc] pieces of the cells the edges split
     double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
     int64_t *d_band_out = nullptr; size_t band_out_cap = 0; // [P][2] (host-buffer call)
     // host-buffer path
@@ -447,7 +448,7 @@ static void plan_free(fstat_plan *pl)
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
-    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out);
+    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out); cudaFree(pl->d_rag);
     cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
@@ -613,7 +614,8 @@ static fstat_status ensure_cell_plan(fstat_plan *pl, int32_t C)
 
 // row f2 through the interpolating kernel: the plan evaluated is the internal cells plan
 struct BandReq {
-    int32_t n_seg, lattice;
+    int32_t n_seg, lattice;   // partitions per template; lattice of the edge rule (reading A26)
+    int32_t cell;             // width of the cells (= lattice, or kBandCell with edges that split the cells)
     int64_t *band_out;
     fstat_plan *owner;        // the user's plan: timing ring and launch counter
 };
@@ -684,7 +686,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.n_seg = pl->n_seg;
     fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
     if (br) {                                          // cells: ~4096 bins per CTA run whatever the lattice
-        const int64_t g = 4096 / br->lattice;
+        const int64_t g = 4096 / br->cell;
         fa.segs_per_cta = (int32_t)(g < 1 ? 1 : (g > 128 ? 128 : g));
     }
     fa.df = pl->df;
@@ -713,10 +715,16 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     ++tp->n_timed;
     tp->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
     if (br) {
-        CU_TRY(pl, launch_band_cells_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, pl->d_band,
-                                              pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins, pl->n_part, br->n_seg,
-                                              br->lattice, fa.part_sk, fa.part_sp, F, Fk, st));
-        tp->n_launches += 3;                           // band limits, cells epilogue, F sums
+        double *rag = nullptr;
+        if (br->cell != br->lattice) {                 // edges at any bin: the cells they fall into are split
+            CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(br->n_seg + 1) * 2 * kNAcc));
+            rag = pl->d_rag;
+        }
+        CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag, pl->d_part_seg, pl->d_valid,
+                                              pl->d_perm, pl->d_band, pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins,
+                                              pl->n_part, br->n_seg, br->lattice, br->cell, fa.part_sk, fa.part_sp, pl->orb,
+                                              F, Fk, st));
+        tp->n_launches += rag ? 4 : 3;                 // band limits, [pieces], cells epilogue, F sums
         return FSTAT_OK;
     }
     if (F) {
@@ -758,9 +766,11 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
     cudaStream_t st = (cudaStream_t)stream;
 
-    if (edge_lattice >= kBandFastLattice && pl->fast_ok && pl->opt.force_level != -1) {
-        // edges on a lattice: the interpolating kernel over the lattice cells (an internal plan that shares the tables)
-        fstat_status s = ensure_cell_plan(pl, edge_lattice);
+    if (pl->fast_ok && pl->opt.force_level != -1) {
+        // the interpolating kernel over cells (an internal plan that shares the tables): the cells are the lattice
+        // itself from 32 bins on; below that they are kBandCell bins wide and the edges split them
+        const int32_t cell = edge_lattice >= kBandFastLattice ? edge_lattice : kBandCell;
+        fstat_status s = ensure_cell_plan(pl, cell);
         if (s != FSTAT_OK) return s;
         fstat_plan *cp = pl->cells;
         cp->opt.force_level = pl->opt.force_level;
@@ -770,10 +780,11 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
             Fk = pl->d_band_fk;
         }
         // one record of 10 sums per (cell, particle): keep the workspace below ~24 GB by batching the particles
-        const int64_t per_particle = (int64_t)cp->n_part * kNPartial * (int64_t)sizeof(double);
+        const int64_t per_particle = ((int64_t)cp->n_part * kNPartial +
+                                      (cell != edge_lattice ? (int64_t)(n_seg + 1) * 2 * kNAcc : 0)) * (int64_t)sizeof(double);
         int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
         if (batch < kThreads) batch = kThreads;
-        BandReq br{n_seg, edge_lattice, nullptr, pl};
+        BandReq br{n_seg, edge_lattice, cell, nullptr, pl};
         for (int64_t off = 0; off < P; off += batch) {
             const int64_t n = (P - off < batch) ? P - off : batch;
             br.band_out = band ? band + 2 * off : nullptr;

@@ -22,6 +22,8 @@
 //   band_cells_epilogue_kernel   adds, per particle and partition, the records of the cells between its
 //                                edges (recentred basis, add_segment) and writes F_k
 //   band_fsum_kernel             F = sum_k F_k in a fixed order
+// and below 32 bins (edges at any bin) the cells are 64 bins wide and
+//   band_ragged_kernel           evaluates, with the full model, the two pieces of every cell an edge splits
 #include "fstat_device.cuh"
 #include "fstat_direct.cuh"
 #include "fstat_internal.h"
@@ -269,94 +271,179 @@ __global__ void __launch_bounds__(128) band_epilogue_kernel(const double *__rest
     F[particle] = f;
 }
 
-// Block = 32 slots (x) by 8 lanes (y); blockIdx.y walks the partitions.  The 8 lanes split the cells of one
-// (slot, partition) -- cell c of the lattice is partition c of the internal plan, its records are segments
-// part_seg[c] .. part_seg[c + 1] -- and are combined through shared memory in a fixed order.
+// The partitions of the templates from the cell records.  Cell c of the internal plan is its partition c: its
+// records are segments part_seg[c] .. part_seg[c + 1], slot-major or value-major (sk, sp).  Cc = width of the
+// cells; C = lattice of the edge rule.  rag == nullptr: C == Cc, every edge is a cell boundary.  Otherwise an
+// edge may split its cell and rag holds the two pieces (band_ragged_kernel): a partition is
+//   right piece of e_j  +  the whole cells between  +  left piece of e_{j+1},
+// or left(e_{j+1}) - left(e_j) when both edges fall into one cell.  Everything is brought to the basis of the
+// first whole cell (recentred basis, add_record) and summed in a fixed order.
+//   LANES == 8: block = 32 slots (x) by 8 lanes (y), blockIdx.y walks the partitions and the lanes split the
+//               cells of one (slot, partition), combined through shared memory  (few, long partitions);
+//   LANES == 1: block = 32 slots by 8 partitions, one thread per (slot, partition)  (many short partitions).
+template <int LANES>
 __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *__restrict__ partial,
+                                                                  const double *__restrict__ rag,
                                                                   const int32_t *__restrict__ part_seg,
                                                                   const int32_t *__restrict__ valid,
                                                                   const int32_t *__restrict__ perm,
                                                                   const int32_t *__restrict__ band_lo,
                                                                   const int32_t *__restrict__ band_hi, int64_t P_pad,
                                                                   int32_t n_bins, int32_t n_cells, int32_t N, int32_t C,
-                                                                  int64_t sk, int64_t sp, double *__restrict__ Fk)
+                                                                  int32_t Cc, int64_t sk, int64_t sp,
+                                                                  double *__restrict__ Fk)
 {
-    __shared__ double sV[8][kNAcc][32];
+    __shared__ double sV[LANES == 8 ? 8 : 1][kNAcc][32];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int64_t p = (int64_t)blockIdx.x * 32 + tx;         // < P_pad: the grid covers P_pad / 32 blocks exactly
     const int32_t particle = perm[p];
     const bool ok = particle >= 0 && valid[p] != 0;
     const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
-    for (int j = blockIdx.y; j < N; j += gridDim.y) {
+    const int j_first = LANES == 8 ? blockIdx.x * 0 + blockIdx.y : blockIdx.y * 8 + ty;
+    const int j_step = LANES == 8 ? gridDim.y : gridDim.y * 8;
+    const int lane = LANES == 8 ? ty : 0;
+    for (int j = j_first; j < N; j += j_step) {
         double v[kNAcc];
 #pragma unroll
         for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
-        int s0 = 0, s1 = 0;
+        bool live = false;                                   // a non-empty partition of a valid particle
         if (ok) {
             const int32_t ea = band_edge(j, q_lo, D, N, C, n_bins), eb = band_edge(j + 1, q_lo, D, N, C, n_bins);
-            const int32_t ca = ea >= n_bins ? n_cells : ea / C, cb = eb >= n_bins ? n_cells : eb / C;
-            s0 = part_seg[ca];
-            s1 = part_seg[cb];
-            if (s1 > s0) {
-                const double *first = partial + ((int64_t)s0 * kNPartial) * P_pad + p * sp;
-                const double cs_r = first[8 * sk], cs_i = first[9 * sk];                  // the first cell's basis
-                for (int s = s0 + ty; s < s1; s += 8) add_segment(partial, s, P_pad, sk, sp, p, cs_r, cs_i, v);
+            if (eb > ea) {
+                live = true;
+                const bool onA = rag == nullptr || (ea % Cc) == 0;
+                const bool onB = rag == nullptr || eb >= n_bins || (eb % Cc) == 0;
+                const int32_t ca = onA ? ea / Cc : ea / Cc + 1, cb = eb >= n_bins ? n_cells : eb / Cc;
+                const double *ra = nullptr, *rb = nullptr;   // pieces of the cells e_j, e_{j+1} split: left, right
+                if (!onA || !onB) {
+                    // the pieces of an edge shared by several (empty) partitions are stored under its first index
+                    int ja = j, jb = j + 1;
+                    while (ja > 0 && band_edge(ja - 1, q_lo, D, N, C, n_bins) == ea) --ja;
+                    while (jb > 0 && band_edge(jb - 1, q_lo, D, N, C, n_bins) == eb) --jb;
+                    ra = rag + (((int64_t)p * (N + 1) + ja) * 2) * kNAcc;
+                    rb = rag + (((int64_t)p * (N + 1) + jb) * 2) * kNAcc;
+                }
+                if (ca > cb) {                               // both edges inside one cell
+                    if (lane == 0) {
+#pragma unroll
+                        for (int i = 0; i < kNAcc; ++i) v[i] = rb[i] - ra[i];
+                    }
+                } else {
+                    const int s0 = part_seg[ca], s1 = part_seg[cb];
+                    double cs_r = 0.0, cs_i = 0.0;           // the first whole cell's basis (plain basis if none)
+                    if (s1 > s0) {
+                        const double *first = partial + ((int64_t)s0 * kNPartial) * P_pad + p * sp;
+                        cs_r = first[8 * sk];
+                        cs_i = first[9 * sk];
+                    }
+                    double t[kNPartial];
+                    t[8] = 0.0; t[9] = 0.0;
+                    if (!onA && lane == 0) {
+#pragma unroll
+                        for (int i = 0; i < kNAcc; ++i) t[i] = ra[kNAcc + i];
+                        add_record(t, cs_r, cs_i, v);
+                    }
+#pragma unroll 2
+                    for (int s = s0 + lane; s < s1; s += LANES) add_segment(partial, s, P_pad, sk, sp, p, cs_r, cs_i, v);
+                    if (!onB && lane == 0) {
+#pragma unroll
+                        for (int i = 0; i < kNAcc; ++i) t[i] = rb[i];
+                        add_record(t, cs_r, cs_i, v);
+                    }
+                }
             }
         }
+        if (LANES == 8) {
 #pragma unroll
-        for (int i = 0; i < kNAcc; ++i) sV[ty][i][tx] = v[i];
-        __syncthreads();
-        if (ty == (j & 7) && particle >= 0) {
+            for (int i = 0; i < kNAcc; ++i) sV[ty][i][tx] = v[i];
+            __syncthreads();
+            if (ty == (j & 7) && particle >= 0) {
 #pragma unroll
-            for (int i = 0; i < kNAcc; ++i) {
-                double acc = 0.0;
+                for (int i = 0; i < kNAcc; ++i) {
+                    double acc = 0.0;
 #pragma unroll
-                for (int y = 0; y < 8; ++y) acc += sV[y][i][tx];
-                v[i] = acc;
+                    for (int y = 0; y < 8; ++y) acc += sV[y][i][tx];
+                    v[i] = acc;
+                }
+                Fk[(int64_t)particle * N + j] = ok ? (live ? 0.5 * two_F(v) : 0.0) : -INFINITY;
             }
-            Fk[(int64_t)particle * N + j] = ok ? (s1 > s0 ? 0.5 * two_F(v) : 0.0) : -INFINITY;
+            __syncthreads();
+        } else if (particle >= 0) {
+            Fk[(int64_t)particle * N + j] = ok ? (live ? 0.5 * two_F(v) : 0.0) : -INFINITY;
         }
-        __syncthreads();
     }
 }
 
-// Many partitions of a few cells each (N_seg in the hundreds): one thread per (slot, partition), x = 32 slots,
-// y = 8 partitions per block, no shared memory.  Same sums in the same order per partition as the kernel above
-// would give with one lane (the order of the cells), so both are deterministic; they differ in rounding only.
-__global__ void __launch_bounds__(256) band_cells_epilogue_flat_kernel(const double *__restrict__ partial,
-                                                                       const int32_t *__restrict__ part_seg,
-                                                                       const int32_t *__restrict__ valid,
-                                                                       const int32_t *__restrict__ perm,
-                                                                       const int32_t *__restrict__ band_lo,
-                                                                       const int32_t *__restrict__ band_hi,
-                                                                       int64_t P_pad, int32_t n_bins, int32_t n_cells,
-                                                                       int32_t N, int32_t C, int64_t sk, int64_t sp,
-                                                                       double *__restrict__ Fk)
+// ---------------------------------------------------------------------------------------------------
+// Edges at ANY bin on top of the cell records (edge_lattice < 32 with the interpolating kernel available): the
+// cells are Cc bins wide; an edge e that is not a cell boundary splits its cell [c Cc, (c + 1) Cc) into a left
+// piece (the end of partition j - 1) and a right piece (the start of partition j).  band_ragged_kernel evaluates
+// those two pieces with the full model, one thread per (slot, edge), straight from the per-bin table:
+// rag[((p (N + 1) + j) 2 + h) 8 + i], h = 0 left / 1 right, plain basis (c = 0).  A partition is then
+//   right piece of e_j  +  the whole cells between  +  left piece of e_{j+1}
+// (both edges in one cell: left(e_{j+1}) - left(e_j)), combined by band_cells_epilogue_kernel.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restrict__ table, const double *__restrict__ coef,
+                                                          const int32_t *__restrict__ valid,
+                                                          const int32_t *__restrict__ band_lo,
+                                                          const int32_t *__restrict__ band_hi, int64_t P_pad,
+                                                          int32_t n_bins, int32_t N, int32_t C, int32_t Cc,
+                                                          const __grid_constant__ OrbitCoef orb, double *__restrict__ rag)
 {
-    const int64_t p = (int64_t)blockIdx.x * 32 + threadIdx.x;
-    const int32_t particle = perm[p];
-    if (particle < 0) return;
-    const bool ok = valid[p] != 0;
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P_pad || valid[p] == 0) return;
     const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
-    for (int j = blockIdx.y * 8 + threadIdx.y; j < N; j += gridDim.y * 8) {
-        double fk = -INFINITY;
-        if (ok) {
-            const int32_t ea = band_edge(j, q_lo, D, N, C, n_bins), eb = band_edge(j + 1, q_lo, D, N, C, n_bins);
-            const int32_t ca = ea >= n_bins ? n_cells : ea / C, cb = eb >= n_bins ? n_cells : eb / C;
-            const int s0 = part_seg[ca], s1 = part_seg[cb];
-            fk = 0.0;
-            if (s1 > s0) {
-                double v[kNAcc];
+    if (D <= 0) return;
+    double c[kNCoef];
 #pragma unroll
-                for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
-                const double *first = partial + ((int64_t)s0 * kNPartial) * P_pad + p * sp;
-                const double cs_r = first[8 * sk], cs_i = first[9 * sk];
-#pragma unroll 2
-                for (int s = s0; s < s1; ++s) add_segment(partial, s, P_pad, sk, sp, p, cs_r, cs_i, v);
-                fk = 0.5 * two_F(v);
-            }
+    for (int i = 0; i < kNCoef; ++i) c[i] = coef[(int64_t)i * P_pad + p];
+    for (int j = blockIdx.y; j <= N; j += gridDim.y) {
+        const int32_t e = band_edge(j, q_lo, D, N, C, n_bins);
+        if (e >= n_bins || e % Cc == 0) continue;                       // a cell boundary: nothing to split
+        if (j > 0 && band_edge(j - 1, q_lo, D, N, C, n_bins) == e) continue;   // same edge as the previous one
+        const int32_t b0 = (e / Cc) * Cc, b1 = min(b0 + Cc, n_bins);
+        double *out = rag + (((int64_t)p * (N + 1) + j) * 2) * kNAcc;
+        double acc[kNAcc];
+#pragma unroll
+        for (int i = 0; i < kNAcc; ++i) acc[i] = 0.0;
+        // the next bin's table row is fetched while this one is evaluated (every thread walks its own rows:
+        // nothing to share through shared memory, and the loads would otherwise sit in front of 263 dependent FP64s)
+        double2 cur[12], nxt[12];
+        {
+            const double2 *r0 = reinterpret_cast<const double2 *>(table + (int64_t)b0 * kTabW);
+#pragma unroll
+            for (int i = 0; i < 12; ++i) cur[i] = r0[i];
         }
-        Fk[(int64_t)particle * N + j] = fk;
+#pragma unroll 1
+        for (int k = b0; k < b1; ++k) {
+            {
+                const double2 *rn = reinterpret_cast<const double2 *>(table + (int64_t)min(k + 1, b1 - 1) * kTabW);
+#pragma unroll
+                for (int i = 0; i < 12; ++i) nxt[i] = rn[i];
+            }
+            if (k == e) {
+#pragma unroll
+                for (int i = 0; i < kNAcc; ++i) { out[i] = acc[i]; acc[i] = 0.0; }
+            }
+            const double2 dwv = cur[10];
+            double psi, sps, cps, tpr, tpi, tcr, tci;
+            bin_template(cur, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
+            const double qr = fma(dwv.x, cps, -dwv.y * sps);
+            const double qi = fma(dwv.x, sps, dwv.y * cps);
+            acc[0] = fma(qr, tpr, fma(qi, tpi, acc[0]));
+            acc[1] = fma(qi, tpr, fma(-qr, tpi, acc[1]));
+            acc[2] = fma(qr, tcr, fma(qi, tci, acc[2]));
+            acc[3] = fma(qi, tcr, fma(-qr, tci, acc[3]));
+            const double wgt = cur[11].x;
+            acc[4] = fma(wgt, fma(tpr, tpr, tpi * tpi), acc[4]);
+            acc[5] = fma(wgt, fma(tcr, tcr, tci * tci), acc[5]);
+            acc[6] = fma(wgt, fma(tpr, tcr, tpi * tci), acc[6]);
+            acc[7] = fma(wgt, fma(tpi, tcr, -tpr * tci), acc[7]);
+#pragma unroll
+            for (int i = 0; i < 12; ++i) cur[i] = nxt[i];
+        }
+#pragma unroll
+        for (int i = 0; i < kNAcc; ++i) out[kNAcc + i] = acc[i];
     }
 }
 
@@ -374,28 +461,35 @@ __global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict
     if (lane == 0) F[q] = f;
 }
 
-cudaError_t launch_band_cells_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
-                                       const int32_t *perm, const int32_t *band_lo, const int32_t *band_hi, int64_t P,
-                                       int64_t P_pad, int32_t n_bins, int32_t n_cells, int32_t n_seg_band,
-                                       int32_t lattice, int64_t part_sk, int64_t part_sp, double *F, double *Fk,
+// rag == nullptr: every edge is a cell boundary (lattice == cell); else the pieces are computed first.
+cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, const double *partial, double *rag,
+                                       const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
+                                       const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
+                                       int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
+                                       int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
                                        cudaStream_t st)
 {
+    cudaError_t e;
+    if (rag != nullptr) {
+        int gy = n_seg_band + 1;
+        if (gy > 2048) gy = 2048;
+        band_ragged_kernel<<<dim3((unsigned)(P_pad / 128), (unsigned)gy), 128, 0, st>>>(
+            table, coef, valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, orb, rag);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
     if ((int64_t)n_cells < (int64_t)32 * n_seg_band) {      // a few cells per partition: one thread per partition
         int gy = (n_seg_band + 7) / 8;
         if (gy > 4096) gy = 4096;
-        band_cells_epilogue_flat_kernel<<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
-            partial, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, part_sk,
-            part_sp, Fk);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        band_fsum_kernel<<<(unsigned)((P + 3) / 4), 128, 0, st>>>(Fk, P, n_seg_band, F);
-        return cudaGetLastError();
+        band_cells_epilogue_kernel<1><<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
+            partial, rag, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
+            part_sk, part_sp, Fk);
+    } else {
+        const int gy = n_seg_band < 4096 ? n_seg_band : 4096;
+        band_cells_epilogue_kernel<8><<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
+            partial, rag, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
+            part_sk, part_sp, Fk);
     }
-    const int gy = n_seg_band < 4096 ? n_seg_band : 4096;
-    band_cells_epilogue_kernel<<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
-        partial, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, part_sk, part_sp, Fk);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
     band_fsum_kernel<<<(unsigned)((P + 3) / 4), 128, 0, st>>>(Fk, P, n_seg_band, F);
     return cudaGetLastError();
 }

@@ -56,14 +56,9 @@ __device__ __forceinline__ double two_F(const double (&v)[kNAcc])
 // c*:  u_x - c* u_+ = (u_x - c_s u_+) + D u_+,  D = c_s - c*, so
 //   z~* = z~ + conj(D) z_+,   m~*_pc = m~_pc + conj(D) m_pp,   m~*_cc = m~_cc + 2 Re(D m~_pc) + |D|^2 m_pp.
 // D is a small difference of nearby ratios: nothing cancels here.
-// (sk, sp): strides of the record's values and of the slots, (P_pad, 1) or (1, kNPartial), see MainArgs.
-__device__ __forceinline__ void add_segment(const double *__restrict__ partial, int s, int64_t P_pad, int64_t sk,
-                                            int64_t sp, int64_t p, double cs_r, double cs_i, double (&v)[kNAcc])
+// t = the ten values of a record (eight sums in the basis with constant (t[8], t[9])).
+__device__ __forceinline__ void add_record(const double (&t)[kNPartial], double cs_r, double cs_i, double (&v)[kNAcc])
 {
-    const double *src = partial + ((int64_t)s * kNPartial) * P_pad + p * sp;
-    double t[kNPartial];
-#pragma unroll
-    for (int j = 0; j < kNPartial; ++j) t[j] = src[(int64_t)j * sk];
     const double dr = t[8] - cs_r, di = t[9] - cs_i;
     v[0] += t[0];
     v[1] += t[1];
@@ -73,6 +68,17 @@ __device__ __forceinline__ void add_segment(const double *__restrict__ partial, 
     v[5] += fma(fma(dr, dr, di * di), t[4], fma(2.0, fma(dr, t[6], -di * t[7]), t[5]));
     v[6] += fma(dr, t[4], t[6]);
     v[7] += fma(-di, t[4], t[7]);
+}
+
+// (sk, sp): strides of the record's values and of the slots, (P_pad, 1) or (1, kNPartial), see MainArgs.
+__device__ __forceinline__ void add_segment(const double *__restrict__ partial, int s, int64_t P_pad, int64_t sk,
+                                            int64_t sp, int64_t p, double cs_r, double cs_i, double (&v)[kNAcc])
+{
+    const double *src = partial + ((int64_t)s * kNPartial) * P_pad + p * sp;
+    double t[kNPartial];
+#pragma unroll
+    for (int j = 0; j < kNPartial; ++j) t[j] = src[(int64_t)j * sk];
+    add_record(t, cs_r, cs_i, v);
 }
 
 }  // namespace fstat

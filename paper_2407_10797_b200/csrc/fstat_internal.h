@@ -68,7 +68,8 @@ constexpr int kFastTileShift = 9;
 constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the folded data (8 KiB), aligned to its size;
                                                      // >= kMaxStride so that no sub-block straddles two tiles
 constexpr int kFastStages = 3;
-constexpr int kBandFastLattice = 32;                 // row f2: from this edge lattice on the interpolating kernel is used
+constexpr int kBandFastLattice = 32;                 // row f2: from this edge lattice on the cells ARE the lattice; below it ...
+constexpr int kBandCell = 64;                        // ... the cells are this wide and the edges split them (band_ragged_kernel)
 constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
 
 // per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)
@@ -168,10 +169,11 @@ cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t s
 cudaError_t launch_band_epilogue(const double *rec, const int32_t *rec_idx, const int32_t *valid, const int32_t *perm,
                                  int64_t P_pad, int32_t n_wseg, int32_t n_seg, double *F, double *Fk, cudaStream_t st);
 cudaError_t band_kernel_configure();
-cudaError_t launch_band_cells_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
-                                       const int32_t *perm, const int32_t *band_lo, const int32_t *band_hi, int64_t P,
-                                       int64_t P_pad, int32_t n_bins, int32_t n_cells, int32_t n_seg_band,
-                                       int32_t lattice, int64_t part_sk, int64_t part_sp, double *F, double *Fk,
+cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, const double *partial, double *rag,
+                                       const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
+                                       const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
+                                       int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
+                                       int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
                                        cudaStream_t st);
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,

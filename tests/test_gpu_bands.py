@@ -53,12 +53,18 @@ def _check(orc, ds, par, n_seg, lattice, F, Fk, band):
     return int(live.sum())
 
 
-@pytest.mark.parametrize("n_seg,lattice", [(1, 1), (4, 1), (16, 1), (16, 64), (64, 128), (7, 3)])
-def test_bands_small_every_F_and_Fk(fs, orc, bands, n_seg, lattice):
-    """64 particles whose bands start below, inside and above the grid (39 non-empty), every F and F_k."""
+@pytest.mark.parametrize("n_seg,lattice,full_model", [(1, 1, 0), (4, 1, 0), (16, 1, 0), (16, 64, 0), (64, 128, 0),
+                                                       (7, 3, 0), (500, 1, 0), (4, 1, 1), (7, 3, 1), (64, 128, 1)])
+def test_bands_small_every_F_and_Fk(fs, orc, bands, n_seg, lattice, full_model):
+    """64 particles whose bands start below, inside and above the grid (39 non-empty), every F and F_k, through
+    the three paths: lattice >= 32 (interpolating kernel over the lattice cells), lattice < 32 (the same over
+    64-bin cells plus the pieces of the cells the edges split; 500 partitions put several edges into one cell),
+    and force_level = -1 (full model at every in-band bin, per-thread edges)."""
     ds = bands
     par = syn.draw_particles(ds.cfg)
-    F, Fk, band = _gpu(fs, ds, par, n_seg, lattice)
+    opts = fs.fstat_default_options()
+    opts.force_level = -1 if full_model else -2
+    F, Fk, band = _gpu(fs, ds, par, n_seg, lattice, opts)
     n = _check(orc, ds, par, n_seg, lattice, F, Fk, band)
     assert n >= 30 * n_seg
 
@@ -71,6 +77,7 @@ def test_bands_work_segment_length_does_not_matter(fs, orc, bands, seg):
     par = syn.draw_particles(ds.cfg)[:40]
     opts = fs.fstat_default_options()
     opts.max_segment_bins = seg
+    opts.force_level = -1                                  # the kernel with per-thread edges (full model at every bin)
     F, Fk, band = _gpu(fs, ds, par, 16, 1, opts)
     _check(orc, ds, par, 16, 1, F, Fk, band)
 
@@ -134,7 +141,7 @@ def test_bands_first_stage_sample(fs, orc, first_stage, lattice):
     _check(orc, ds, par[sample], 1024, lattice, F[sample], Fk[sample], band[sample])
 
 
-@pytest.mark.parametrize("cfg_i,n_seg,lattice", [(1, 1024, 64), (2, 16, 128), (3, 1, 512)])
+@pytest.mark.parametrize("cfg_i,n_seg,lattice", [(1, 1024, 64), (2, 16, 128), (3, 1, 512), (1, 1024, 1), (2, 16, 1)])
 def test_bands_interpolating_kernel_against_full_model_every_value(fs, orc, first_stage, cfg_i, n_seg, lattice):
     """At full size every F and F_k of the interpolating kernel over the lattice cells against the kernel that
     evaluates the full model at every in-band bin (force_level = -1; itself checked against the oracle above)
