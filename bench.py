@@ -126,7 +126,8 @@ def parse_args():
                     help="also time ITERS iterations of the device PSO (row f1) on this plan: swarms of 128 particles")
     ap.add_argument("--bands", type=int, default=0, metavar="N_SEG",
                     help="also time fstat_eval_batch_bands (row f2: per-template bands, N_SEG partitions) on this plan")
-    ap.add_argument("--bands-lattice", type=int, default=64, help="edge lattice of --bands in bins (>= 32: interpolating kernel)")
+    ap.add_argument("--bands-lattice", type=int, default=1,
+                    help="edge lattice of --bands in bins (1: edges at any bin; >= 32: the lattice cells are the work units)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
     return ap.parse_args()
@@ -431,7 +432,8 @@ def run_ours(args):
                         "in_band_template_bins_per_s": in_band * world / (ms_b * 1e-3),
                         "e2e_ms_per_step": ms_b_e2e, "e2e_in_band_template_bins_per_s": in_band * world / (ms_b_e2e * 1e-3),
                         "kernel": "fstat_fast_kernel over the lattice cells" if args.bands_lattice >= 32
-                                  else "fstat_band_kernel (full model at every in-band bin)"}
+                                  else "fstat_fast_kernel over 64..512-bin cells + band_ragged_kernel (pieces of the "
+                                       "cells the edges split, full model)"}
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, ds, n_part, args.cpu_sample)
     fs.fstat_plan_destroy(plan)

@@ -139,8 +139,11 @@ FSTAT_API fstat_status fstat_eval_batch(fstat_plan *plan, int64_t P,
  *   n_seg   >= 1; edge_lattice >= 1 bins (1 = edges at any bin).
  *   F       [P] DEVICE pointer, out.   Fk  [P][n_seg] DEVICE pointer, out; may be NULL.
  *   band    [P][2] int64 DEVICE pointer, out: k_lo, k_hi of every particle; may be NULL.
- * Invalid particles get F = F_k = -inf and band (0, 0).  Asynchronous on cuda_stream.  Every in-band bin is
- * evaluated with the full model (the direct kernel's arithmetic).
+ * Invalid particles get F = F_k = -inf and band (0, 0).  Asynchronous on cuda_stream.
+ * Work: the interpolating kernel over cells of the grid (the lattice cells for edge_lattice >= 32, else cells of
+ * 64..512 bins by n_seg) plus, for edges that split a cell, the full model over the shorter piece of that cell;
+ * with options.force_level == -1 (or a grid that starts within 1025 bins of f = 0) the full model at every in-band
+ * bin.  Workspace: 80 bytes per (cell, particle), evaluated in particle batches of at most 24 GB.
  * Errors: EINVAL (NULL plan/params/F, n_seg < 1, edge_lattice < 1), ENOMEM, ECUDA.
  */
 FSTAT_API fstat_status fstat_eval_batch_bands(fstat_plan *plan, int64_t P, const double *params, int32_t n_seg,
@@ -254,7 +257,7 @@ typedef struct {
     int32_t band_n_seg;       /* 0 (default): fitness = fstat_eval_batch with the plan's partitions;
                                  >= 1: fitness = fstat_eval_batch_bands with this many segments per template
                                  (the paper's own segment limits)                             */
-    int32_t band_lattice;     /* edge lattice of that call in bins, default 64                            */
+    int32_t band_lattice;     /* edge lattice of that call in bins, default 1 (edges at any bin)          */
 } fstat_pso_options;
 
 FSTAT_API void fstat_pso_default_options(fstat_pso_options *opts);

@@ -62,7 +62,7 @@ struct fstat_plan {
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
     double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
     int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
-    double *d_rag = nullptr; size_t rag_cap = 0;          // [P_pad][n_seg + 1][2][kNAcc] pieces of the cells the edges split
+    double *d_rag = nullptr; size_t rag_cap = 0;          // [P_pad][n_seg + 1][kNAcc] the shorter piece of every cell an edge splits
     double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
     int64_t *d_band_out = nullptr; size_t band_out_cap = 0; // [P][2] (host-buffer call)
     // host-buffer path
@@ -717,7 +717,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     if (br) {
         double *rag = nullptr;
         if (br->cell != br->lattice) {                 // edges at any bin: the cells they fall into are split
-            CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(br->n_seg + 1) * 2 * kNAcc));
+            CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(br->n_seg + 1) * kNAcc));
             rag = pl->d_rag;
         }
         CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag, pl->d_part_seg, pl->d_valid,
@@ -769,7 +769,9 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
     if (pl->fast_ok && pl->opt.force_level != -1) {
         // the interpolating kernel over cells (an internal plan that shares the tables): the cells are the lattice
         // itself from 32 bins on; below that they are kBandCell bins wide and the edges split them
-        const int32_t cell = edge_lattice >= kBandFastLattice ? edge_lattice : kBandCell;
+        // (wider cells cost the interpolating kernel less, narrower ones the pieces: ~ (n_seg + 1) cell / 4 bins in full)
+        const int32_t cell = edge_lattice >= kBandFastLattice ? edge_lattice
+                             : (n_seg <= 32 ? 8 * kBandCell : n_seg <= 128 ? 4 * kBandCell : n_seg <= 512 ? 2 * kBandCell : kBandCell);
         fstat_status s = ensure_cell_plan(pl, cell);
         if (s != FSTAT_OK) return s;
         fstat_plan *cp = pl->cells;
@@ -781,7 +783,7 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
         }
         // one record of 10 sums per (cell, particle): keep the workspace below ~24 GB by batching the particles
         const int64_t per_particle = ((int64_t)cp->n_part * kNPartial +
-                                      (cell != edge_lattice ? (int64_t)(n_seg + 1) * 2 * kNAcc : 0)) * (int64_t)sizeof(double);
+                                      (cell != edge_lattice ? (int64_t)(n_seg + 1) * kNAcc : 0)) * (int64_t)sizeof(double);
         int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
         if (batch < kThreads) batch = kThreads;
         BandReq br{n_seg, edge_lattice, cell, nullptr, pl};

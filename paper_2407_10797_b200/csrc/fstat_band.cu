@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
     const int32_t particle = perm[p];
     const bool ok = particle >= 0 && valid[p] != 0;
     const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
-    const int j_first = LANES == 8 ? blockIdx.x * 0 + blockIdx.y : blockIdx.y * 8 + ty;
+    const int j_first = LANES == 8 ? (int)blockIdx.y : (int)blockIdx.y * 8 + ty;
     const int j_step = LANES == 8 ? gridDim.y : gridDim.y * 8;
     const int lane = LANES == 8 ? ty : 0;
     for (int j = j_first; j < N; j += j_step) {
@@ -314,42 +314,47 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
                 const bool onA = rag == nullptr || (ea % Cc) == 0;
                 const bool onB = rag == nullptr || eb >= n_bins || (eb % Cc) == 0;
                 const int32_t ca = onA ? ea / Cc : ea / Cc + 1, cb = eb >= n_bins ? n_cells : eb / Cc;
-                const double *ra = nullptr, *rb = nullptr;   // pieces of the cells e_j, e_{j+1} split: left, right
+                int ja = j, jb = j + 1;
                 if (!onA || !onB) {
-                    // the pieces of an edge shared by several (empty) partitions are stored under its first index
-                    int ja = j, jb = j + 1;
+                    // the piece of an edge shared by several (empty) partitions is stored under its first index
                     while (ja > 0 && band_edge(ja - 1, q_lo, D, N, C, n_bins) == ea) --ja;
                     while (jb > 0 && band_edge(jb - 1, q_lo, D, N, C, n_bins) == eb) --jb;
-                    ra = rag + (((int64_t)p * (N + 1) + ja) * 2) * kNAcc;
-                    rb = rag + (((int64_t)p * (N + 1) + jb) * 2) * kNAcc;
                 }
-                if (ca > cb) {                               // both edges inside one cell
-                    if (lane == 0) {
+                // common basis: the one of the cell that starts at or holds e_j (always evaluated for this group)
+                const double *first = partial + ((int64_t)part_seg[ea / Cc] * kNPartial) * P_pad + p * sp;
+                const double cs_r = first[8 * sk], cs_i = first[9 * sk];
+                // sgn x (left or right piece of the cell edge e splits), e = edge number je of this template
+                auto add_piece = [&](int32_t e, int je, bool want_left, double sgn) {
+                    const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
+                    const bool stored_left = (e - c0) <= (c1 - e);
+                    const double *r = rag + ((int64_t)p * (N + 1) + je) * kNAcc;
+                    double t[kNPartial];
+                    const double sg = (stored_left == want_left) ? sgn : -sgn;
 #pragma unroll
-                        for (int i = 0; i < kNAcc; ++i) v[i] = rb[i] - ra[i];
+                    for (int i = 0; i < kNAcc; ++i) t[i] = sg * r[i];
+                    t[8] = 0.0; t[9] = 0.0;
+                    add_record(t, cs_r, cs_i, v);
+                    if (stored_left != want_left) {          // the wanted piece = the cell's record - the stored piece
+                        for (int sc = part_seg[e / Cc]; sc < part_seg[e / Cc + 1]; ++sc) {
+                            const double *src = partial + ((int64_t)sc * kNPartial) * P_pad + p * sp;
+#pragma unroll
+                            for (int i = 0; i < kNAcc; ++i) t[i] = sgn * src[(int64_t)i * sk];
+                            t[8] = src[8 * sk]; t[9] = src[9 * sk];
+                            add_record(t, cs_r, cs_i, v);
+                        }
+                    }
+                };
+                if (ca > cb) {                               // both edges inside one cell: left(e_{j+1}) - left(e_j)
+                    if (lane == 0) {
+                        add_piece(eb, jb, true, 1.0);
+                        add_piece(ea, ja, true, -1.0);
                     }
                 } else {
+                    if (!onA && lane == 0) add_piece(ea, ja, false, 1.0);
                     const int s0 = part_seg[ca], s1 = part_seg[cb];
-                    double cs_r = 0.0, cs_i = 0.0;           // the first whole cell's basis (plain basis if none)
-                    if (s1 > s0) {
-                        const double *first = partial + ((int64_t)s0 * kNPartial) * P_pad + p * sp;
-                        cs_r = first[8 * sk];
-                        cs_i = first[9 * sk];
-                    }
-                    double t[kNPartial];
-                    t[8] = 0.0; t[9] = 0.0;
-                    if (!onA && lane == 0) {
-#pragma unroll
-                        for (int i = 0; i < kNAcc; ++i) t[i] = ra[kNAcc + i];
-                        add_record(t, cs_r, cs_i, v);
-                    }
 #pragma unroll 2
                     for (int s = s0 + lane; s < s1; s += LANES) add_segment(partial, s, P_pad, sk, sp, p, cs_r, cs_i, v);
-                    if (!onB && lane == 0) {
-#pragma unroll
-                        for (int i = 0; i < kNAcc; ++i) t[i] = rb[i];
-                        add_record(t, cs_r, cs_i, v);
-                    }
+                    if (!onB && lane == 0) add_piece(eb, jb, true, 1.0);
                 }
             }
         }
@@ -378,8 +383,9 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
 // Edges at ANY bin on top of the cell records (edge_lattice < 32 with the interpolating kernel available): the
 // cells are Cc bins wide; an edge e that is not a cell boundary splits its cell [c Cc, (c + 1) Cc) into a left
 // piece (the end of partition j - 1) and a right piece (the start of partition j).  band_ragged_kernel evaluates
-// those two pieces with the full model, one thread per (slot, edge), straight from the per-bin table:
-// rag[((p (N + 1) + j) 2 + h) 8 + i], h = 0 left / 1 right, plain basis (c = 0).  A partition is then
+// the SHORTER of the two pieces with the full model, one thread per (slot, edge), straight from the per-bin
+// table: rag[(p (N + 1) + j) 8 + i], plain basis (c = 0); the other piece is the cell's record minus this one
+// (the cell's record carries the interpolation error of any other cell, the piece none).  A partition is then
 //   right piece of e_j  +  the whole cells between  +  left piece of e_{j+1}
 // (both edges in one cell: left(e_{j+1}) - left(e_j)), combined by band_cells_epilogue_kernel.
 // ---------------------------------------------------------------------------------------------------
@@ -401,8 +407,10 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
         const int32_t e = band_edge(j, q_lo, D, N, C, n_bins);
         if (e >= n_bins || e % Cc == 0) continue;                       // a cell boundary: nothing to split
         if (j > 0 && band_edge(j - 1, q_lo, D, N, C, n_bins) == e) continue;   // same edge as the previous one
-        const int32_t b0 = (e / Cc) * Cc, b1 = min(b0 + Cc, n_bins);
-        double *out = rag + (((int64_t)p * (N + 1) + j) * 2) * kNAcc;
+        const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
+        const bool left = (e - c0) <= (c1 - e);                         // the shorter piece; the other one is cell - piece
+        const int32_t b0 = left ? c0 : e, b1 = left ? e : c1;
+        double *out = rag + ((int64_t)p * (N + 1) + j) * kNAcc;
         double acc[kNAcc];
 #pragma unroll
         for (int i = 0; i < kNAcc; ++i) acc[i] = 0.0;
@@ -420,10 +428,6 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
                 const double2 *rn = reinterpret_cast<const double2 *>(table + (int64_t)min(k + 1, b1 - 1) * kTabW);
 #pragma unroll
                 for (int i = 0; i < 12; ++i) nxt[i] = rn[i];
-            }
-            if (k == e) {
-#pragma unroll
-                for (int i = 0; i < kNAcc; ++i) { out[i] = acc[i]; acc[i] = 0.0; }
             }
             const double2 dwv = cur[10];
             double psi, sps, cps, tpr, tpi, tcr, tci;
@@ -443,7 +447,7 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
             for (int i = 0; i < 12; ++i) cur[i] = nxt[i];
         }
 #pragma unroll
-        for (int i = 0; i < kNAcc; ++i) out[kNAcc + i] = acc[i];
+        for (int i = 0; i < kNAcc; ++i) out[i] = acc[i];
     }
 }
 

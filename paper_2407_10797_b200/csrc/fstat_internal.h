@@ -69,7 +69,7 @@ constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the
                                                      // >= kMaxStride so that no sub-block straddles two tiles
 constexpr int kFastStages = 3;
 constexpr int kBandFastLattice = 32;                 // row f2: from this edge lattice on the cells ARE the lattice; below it ...
-constexpr int kBandCell = 64;                        // ... the cells are this wide and the edges split them (band_ragged_kernel)
+constexpr int kBandCell = 64;                        // ... the cells are 64 .. 512 bins wide (by n_seg) and the edges split them (band_ragged_kernel)
 constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
 
 // per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)

@@ -212,7 +212,7 @@ void fstat_pso_default_options(fstat_pso_options *o)
 {
     if (!o) return;
     o->c1 = 2.0; o->c2 = 2.0; o->v_max = 0.5; o->w_start = 0.9; o->w_end = 0.4;
-    o->band_n_seg = 0; o->band_lattice = 64;
+    o->band_n_seg = 0; o->band_lattice = 1;
 }
 
 void fstat_pso_destroy(fstat_pso *ps)
