@@ -29,6 +29,9 @@
  * fstat_bands in oracle.py; pins in tests/test_oracle_bands.py: P11 the band limits against the textbook
  * 2PN time-to-coalescence series and against the power of a time-domain simulated signal, P12 edges on
  * hand-computed integers, P13 zero-noise in-band 2F = <h,h>.
+ * Row f4 (Eq. 3 :62, the sum over TDI combinations with independent noise): fstat_batch_channels in oracle.py adds
+ * the N and M of this file's oracle_fstat_batch over the channels; pins in tests/test_oracle_channels.py: P14 the
+ * cyclic relabelling behind orbit_lambda + 2 pi/3, brute-force maximisation of Eq. 3, zero-noise network SNR.
  * PARITY UNPINNED (stated in DESIGN.md): the numerical values of alpha_k / phi_e against the
  * authors' code (textbook TaylorF2 values are used, A1/A3) and the paper's absolute SNR values
  * (their PSD file and orbit phase are not available, P10/T8).

@@ -254,5 +254,30 @@ def fstat_bands(freq, dw, inv_sn, params, n_seg: int, lattice: int = 1, opt: Opt
     return F, Fk, edges
 
 
+def fstat_batch_channels(freq, channels, edges, params, use_ld: bool = False):
+    """Row f4 (Eq. 3: Lambda = sum over TDI combinations I with mutually independent noise of
+    <s^I, h^I>_I - |h^I|_I^2 / 2): the four amplitudes are common to all channels, so N^i = sum_I <d_I, A^i_I>_I and
+    M^ij = sum_I <A^i_I, A^j_I>_I (Eq. 8-9 per channel), and F_k = max_a [a.N - a^T M a / 2] as before.
+    ``channels`` = [(dw_I, inv_sn_I, options_I), ...]; the options carry the channel's response (Y and Z are X with
+    the spacecraft relabelled cyclically, i.e. orbit_lambda + 2 pi/3, + 4 pi/3: beta_n = 2 pi n/3 + lambda, reading A9).
+    Returns F[P], Fk[P][n_part]."""
+    params = _par(params).reshape(-1, 6)
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    P, n_part = params.shape[0], edges.shape[0] - 1
+    NM = None
+    for dw, inv_sn, opt in channels:
+        _, _, nm, _ = fstat_batch(freq, dw, inv_sn, edges, params, opt, use_ld=use_ld, want_NM=True)
+        NM = nm if NM is None else NM + nm
+    F, Fk = np.zeros(P), np.zeros((P, n_part))
+    for p in range(P):
+        if not params_valid(params[p]):
+            F[p], Fk[p] = -np.inf, -np.inf
+            continue
+        for k in range(n_part):
+            Fk[p, k] = fstat_from_NM(NM[p, k, :4], NM[p, k, 4:].reshape(4, 4))[0]
+        F[p] = float(np.sum(Fk[p].astype(np.longdouble)))
+    return F, Fk
+
+
 def max_threads() -> int:
     return int(lib().oracle_max_threads())

@@ -553,6 +553,7 @@ fstat_status fstat_plan_level_bins(fstat_plan *pl, int64_t *bins_out, int64_t *s
     for (int32_t gidx = 0; gidx < pl->last_groups; ++gidx)
         for (int32_t sgi = 0; sgi < pl->n_seg; ++sgi) {
             const int l = lv[(size_t)gidx * pl->n_seg + sgi];
+            if (l < -1) continue;                           // (skipped work items exist only in row f2's internal plan)
             const int64_t lo = pl->seg_edge_h[sgi], hi = pl->seg_edge_h[sgi + 1];
             bins_out[l + 1] += hi - lo;
             if (l >= 0) subblocks_out[l + 1] += ((hi - 1) >> (kLevel0Shift + l)) - (lo >> (kLevel0Shift + l)) + 1;
