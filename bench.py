@@ -15,6 +15,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -128,6 +129,8 @@ def parse_args():
                     help="also time fstat_eval_batch_bands (row f2: per-template bands, N_SEG partitions) on this plan")
     ap.add_argument("--bands-lattice", type=int, default=1,
                     help="edge lattice of --bands in bins (1: edges at any bin; >= 32: the lattice cells are the work units)")
+    ap.add_argument("--channels", type=int, default=0, metavar="N",
+                    help="also time fstat_eval_batch_channels (row f4: N TDI channels X, Y, Z with common amplitudes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
     return ap.parse_args()
@@ -434,6 +437,34 @@ def run_ours(args):
                         "kernel": "fstat_fast_kernel over the lattice cells" if args.bands_lattice >= 32
                                   else "fstat_fast_kernel over 64..512-bin cells + band_ragged_kernel (pieces of the "
                                        "cells the edges split, full model)"}
+    if args.channels > 1:
+        # row f4: channel c = the same grid, partitions and particles, noise seed c, response with the spacecraft
+        # relabelled cyclically (orbit_lambda + 2 pi c / 3: X, Y, Z); a1-a5 once per channel, one joint epilogue
+        import dataclasses
+        plans = [plan]
+        for c in range(1, min(args.channels, 3)):
+            o = fs.fstat_default_options()
+            o.force_level, o.max_segment_bins, o.interp_tol = args.force_level, args.max_segment_bins, args.interp_tol
+            o.orbit_lambda = 2.0 * math.pi * c / 3.0
+            ds_c = syn.make_dataset(dataclasses.replace(cfg, noise_seed=cfg.noise_seed + c), None)
+            plans.append(fs.fstat_plan_create(ds_c.freq, ds_c.dw, ds_c.inv_sn, edges, o))
+        for _ in range(2):
+            fs.fstat_eval_batch_channels(plans, par, stream)
+        torch.cuda.synchronize()
+        n_c = max(min(args.steps, 10), 1)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_c)]
+        for e0, e1 in evs:
+            scratch.fill_(4)
+            e0.record(stream)
+            fs.fstat_eval_batch_channels(plans, par, stream)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        ms_c = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs]))
+        out["channels"] = {"n_channels": len(plans), "ms_per_step": ms_c, "ms_per_step_one_channel": ms_step,
+                           "channel_template_bins_per_s": float(P) * ds.n_bins * len(plans) * world / (ms_c * 1e-3),
+                           "data": "noise only in channels 2.. (seeded); timing does not depend on the data"}
+        for pl in plans[1:]:
+            fs.fstat_plan_destroy(pl)
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, ds, n_part, args.cpu_sample)
     fs.fstat_plan_destroy(plan)

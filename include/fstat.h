@@ -158,6 +158,23 @@ FSTAT_API fstat_status fstat_eval_batch_bands_host(fstat_plan *plan, int64_t P, 
                                                    double *Fk_host, int64_t *band_host, void *cuda_stream);
 
 /*
+ * fstat_eval_batch_channels -- SURVEY row f4, the channel sum of PAPER.md:62 Eq. 3: with several TDI combinations I
+ * of mutually independent noise, Lambda = sum_I [<s^I, h^I>_I - |h^I|_I^2 / 2] and the four amplitudes of Eq. 5 are
+ * common to all of them, so N^i = sum_I <d_I, A^i_I>_I, M^ij = sum_I <A^i_I, A^j_I>_I and F_k = N.M^-1.N / 2.
+ * One plan per channel: its own data and 1/S_n^I, and its own response through the options (this library's
+ * response is first-generation Michelson X; Y and Z are X with the spacecraft relabelled cyclically, i.e. with
+ * orbit_lambda + 2 pi/3 and + 4 pi/3).  All plans must share the device, the grid, the partition edges and the other
+ * options.  The a1-a5 kernels run once per channel; one epilogue adds the channels' sums and solves.
+ *
+ *   plans   HOST array of n_channels (1..4) plan handles, all different.
+ *   params, F, Fk, cuda_stream as in fstat_eval_batch (Fk is [P][N_p]).
+ * Errors: EINVAL (NULL, mismatching plans), EUNSUPPORTED (> 4 channels), ENOMEM, ECUDA; the reason is stored in
+ * plans[0].
+ */
+FSTAT_API fstat_status fstat_eval_batch_channels(fstat_plan *const *plans, int32_t n_channels, int64_t P,
+                                                 const double *params, double *F, double *Fk, void *cuda_stream);
+
+/*
  * fstat_eval_amplitudes -- the maximum-likelihood extrinsic amplitudes a = M^-1 N of every partition
  * (Eq. 10; a_1..a_4 multiply the basis templates A^1 = u_+, A^2 = u_x, A^3 = i u_+, A^4 = i u_x of
  * Eq. 5 :77, and are the reparameterisation of (D_L, psi, iota, phi_c) of Eq. B1 :413 up to the amplitude

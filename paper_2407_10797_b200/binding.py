@@ -18,7 +18,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 # every symbol include/fstat.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
-    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
+    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_batch_channels", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
@@ -75,6 +75,8 @@ def load_library():
         L.fstat_eval_batch_bands.restype = C.c_int
         L.fstat_eval_batch_bands_host.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
         L.fstat_eval_batch_bands_host.restype = C.c_int
+        L.fstat_eval_batch_channels.argtypes = [C.POINTER(vp), C.c_int32, i64, vp, vp, vp, vp]
+        L.fstat_eval_batch_channels.restype = C.c_int
         L.fstat_eval_batch_host.argtypes = [vp, i64, vp, vp, vp, vp]
         L.fstat_eval_batch_host.restype = C.c_int
         L.fstat_eval_template.argtypes = [vp, dp, vp, vp, vp]
@@ -286,6 +288,22 @@ def fstat_eval_batch_bands_host(plan: Plan, params, n_seg: int, edge_lattice: in
                                                       F.ctypes.data, Fk.ctypes.data, band.ctypes.data, _stream_ptr(stream)),
            "fstat_eval_batch_bands_host", plan)
     return F, Fk, band
+
+
+def fstat_eval_batch_channels(plans, params, stream=None, want_Fk: bool = True):
+    """Row f4 (Eq. 3): one plan per TDI channel (same grid and partitions) -> (F [P], Fk [P][N_p] or
+    None) CUDA tensors of the statistic with the four amplitudes common to all channels.  Asynchronous."""
+    import torch
+    plans = list(plans)
+    P = int(params.shape[0])
+    pp = _dev_ptr(params, "params", 6 * P)
+    F = torch.empty(P, dtype=torch.float64, device=params.device)
+    Fk = torch.empty((P, plans[0].n_part), dtype=torch.float64, device=params.device) if want_Fk else None
+    arr = (C.c_void_p * len(plans))(*[pl.handle for pl in plans])
+    _check(load_library().fstat_eval_batch_channels(arr, len(plans), P, pp, _dev_ptr(F, "F", P),
+                                                    _dev_ptr(Fk, "Fk", P * plans[0].n_part) if want_Fk else None,
+                                                    _stream_ptr(stream)), "fstat_eval_batch_channels", plans[0])
+    return F, Fk
 
 
 def fstat_eval_amplitudes(plan: Plan, params, amp=None, stream=None):

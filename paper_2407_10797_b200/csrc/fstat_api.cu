@@ -622,12 +622,12 @@ struct BandReq {
 };
 
 static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, double *amp,
-                              void *stream, const BandReq *br = nullptr)
+                              void *stream, const BandReq *br = nullptr, bool sums_only = false)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
     if (P == 0) return FSTAT_OK;
-    if (!params || (!F && !amp)) return fail(pl, FSTAT_EINVAL, "params or the output pointer is NULL");
+    if (!params || (!F && !amp && !sums_only)) return fail(pl, FSTAT_EINVAL, "params or the output pointer is NULL");
     if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
     DeviceGuard g(pl->device);
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
@@ -729,7 +729,10 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         return FSTAT_OK;
     }
     if (F) {
-        CU_TRY(pl, launch_epilogue(pl->d_partial, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg,
+        PartialSet one{};
+        one.p[0] = pl->d_partial;
+        one.n = 1;
+        CU_TRY(pl, launch_epilogue(one, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg,
                                    pl->d_fpart, F, Fk, st));
         int32_t chunk = 0;                             // epilogue, [chunk sums of F]
         pl->n_launches += 1 + (epilogue_chunks(P, pl->n_part, &chunk) > 1 ? 1 : 0);
@@ -745,6 +748,43 @@ fstat_status fstat_eval_batch(fstat_plan *pl, int64_t P, const double *params, d
 {
     if (pl && P > 0 && !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
     return eval_impl(pl, P, params, F, Fk, nullptr, stream);
+}
+
+fstat_status fstat_eval_batch_channels(fstat_plan *const *plans, int32_t n_channels, int64_t P, const double *params,
+                                       double *F, double *Fk, void *stream)
+{
+    if (!plans || n_channels < 1 || !plans[0]) return FSTAT_EINVAL;
+    fstat_plan *p0 = plans[0];
+    if (n_channels > kMaxChannels) return fail(p0, FSTAT_EUNSUPPORTED, "more than 4 channels");
+    if (P < 0) return fail(p0, FSTAT_EINVAL, "P < 0");
+    if (P == 0) return FSTAT_OK;
+    if (!params || !F) return fail(p0, FSTAT_EINVAL, "params or F is NULL");
+    for (int32_t c = 1; c < n_channels; ++c) {
+        const fstat_plan *pc = plans[c];
+        if (!pc) return fail(p0, FSTAT_EINVAL, "a channel's plan is NULL");
+        for (int32_t b = 0; b < c; ++b)
+            if (plans[b] == pc) return fail(p0, FSTAT_EINVAL, "the same plan given for two channels");
+        if (pc->device != p0->device || pc->n_bins != p0->n_bins || pc->df != p0->df || pc->f0 != p0->f0 ||
+            pc->edges != p0->edges || pc->opt.max_segment_bins != p0->opt.max_segment_bins ||
+            pc->opt.f_ref_e0 != p0->opt.f_ref_e0 || pc->opt.orbit_kappa != p0->opt.orbit_kappa)
+            return fail(p0, FSTAT_EINVAL, "the channels' plans differ in device, grid, partitions or options other than the response");
+    }
+    PartialSet ps{};
+    ps.n = n_channels;
+    for (int32_t c = 0; c < n_channels; ++c) {
+        fstat_status s = eval_impl(plans[c], P, params, nullptr, nullptr, nullptr, stream, nullptr, true);
+        if (s != FSTAT_OK) { if (c) p0->err = plans[c]->err; return s; }
+        if (plans[c]->n_seg != p0->n_seg) return fail(p0, FSTAT_ECUDA, "internal: the channels' segmentations differ");
+        ps.p[c] = plans[c]->d_partial;
+    }
+    DeviceGuard g(p0->device);
+    if (!g.ok) return fail(p0, FSTAT_ECUDA, "cudaSetDevice failed");
+    const int64_t P_pad = (P + kThreads - 1) / kThreads * kThreads;
+    CU_TRY(p0, launch_epilogue(ps, p0->d_part_seg, p0->d_valid, p0->d_perm, P, P_pad, p0->n_part, p0->n_seg, p0->d_fpart, F, Fk,
+                               (cudaStream_t)stream));
+    int32_t chunk = 0;
+    p0->n_launches += 1 + (epilogue_chunks(P, p0->n_part, &chunk) > 1 ? 1 : 0);
+    return FSTAT_OK;
 }
 
 fstat_status fstat_eval_amplitudes(fstat_plan *pl, int64_t P, const double *params, double *amp, void *stream)

@@ -194,7 +194,13 @@ cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, doub
                             int32_t *slot_of, const double *rank_band, double *coef, int32_t *valid, int32_t *perm,
                             cudaStream_t st);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
-cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
+// row f4 (Eq. 3 :62): the partial sums of up to kMaxChannels TDI channels, all with the same segment / slot layout
+constexpr int kMaxChannels = 4;
+struct PartialSet {
+    const double *p[kMaxChannels];
+    int32_t n;
+};
+cudaError_t launch_epilogue(const PartialSet &partials, const int32_t *part_seg, const int32_t *valid,
                             const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
                             double *Fpart, double *F, double *Fk, cudaStream_t st);
 int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out);

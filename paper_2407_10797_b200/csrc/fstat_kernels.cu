@@ -367,7 +367,7 @@ cudaError_t launch_template(const double *table, const double *coef, int64_t P_p
 constexpr int kEpiX = 32, kEpiY = 8;
 
 template <bool SEG_PAR>
-__global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__restrict__ partial,
+__global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const PartialSet ps,
                                                                const int32_t *__restrict__ part_seg,
                                                                const int32_t *__restrict__ valid, int64_t P,
                                                                const int32_t *__restrict__ perm, int64_t P_pad,
@@ -397,9 +397,10 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
                 double v[kNAcc];
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
-                const double cs_r = partial[((int64_t)s0 * kNPartial + 8) * P_pad + p];   // common basis: the
-                const double cs_i = partial[((int64_t)s0 * kNPartial + 9) * P_pad + p];   // first segment's
-                for (int s = s0; s < s1; ++s) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
+                const double cs_r = ps.p[0][((int64_t)s0 * kNPartial + 8) * P_pad + p];   // common basis: the first
+                const double cs_i = ps.p[0][((int64_t)s0 * kNPartial + 9) * P_pad + p];   // segment's (of channel 0)
+                for (int c = 0; c < ps.n; ++c)            // Eq. 3 :62: N and M add over the TDI channels
+                    for (int s = s0; s < s1; ++s) add_segment(ps.p[c], s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
                 fk = ok ? 0.5 * two_F(v) : ninf;
                 if (ok) fsum += fk;
             }
@@ -411,9 +412,11 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const double *__
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
                 if (live) {
-                    const double cs_r = partial[((int64_t)s0 * kNPartial + 8) * P_pad + p];
-                    const double cs_i = partial[((int64_t)s0 * kNPartial + 9) * P_pad + p];
-                    for (int s = s0 + ty; s < s1; s += kEpiY) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
+                    const double cs_r = ps.p[0][((int64_t)s0 * kNPartial + 8) * P_pad + p];
+                    const double cs_i = ps.p[0][((int64_t)s0 * kNPartial + 9) * P_pad + p];
+                    for (int c = 0; c < ps.n; ++c)
+                        for (int s = s0 + ty; s < s1; s += kEpiY)
+                            add_segment(ps.p[c], s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
                 }
 #pragma unroll
                 for (int j = 0; j < kNAcc; ++j) sV[SEG_PAR ? ty : 0][j][tx] = v[j];
@@ -541,7 +544,7 @@ int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out)
     return (n_part + chunk - 1) / chunk;
 }
 
-cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, const int32_t *valid,
+cudaError_t launch_epilogue(const PartialSet &partials, const int32_t *part_seg, const int32_t *valid,
                             const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
                             double *Fpart, double *F, double *Fk, cudaStream_t st)
 {
@@ -551,9 +554,9 @@ cudaError_t launch_epilogue(const double *partial, const int32_t *part_seg, cons
     const dim3 grd((unsigned)((P + kEpiX - 1) / kEpiX), (unsigned)n_chunk);
     double *out = (n_chunk == 1) ? F : Fpart;
     if (n_seg >= 4 * n_part)
-        epilogue_kernel<true><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
+        epilogue_kernel<true><<<grd, blk, 0, st>>>(partials, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
     else
-        epilogue_kernel<false><<<grd, blk, 0, st>>>(partial, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
+        epilogue_kernel<false><<<grd, blk, 0, st>>>(partials, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || n_chunk == 1) return e;
     fsum_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(Fpart, valid, perm, P, P_pad, n_chunk, F);

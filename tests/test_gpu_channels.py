@@ -1,0 +1,119 @@
+"""Row f4 on the GPU (fstat_eval_batch_channels: the channel sum of PAPER.md:62 Eq. 3) against the oracle's
+`fstat_batch_channels`, element by element through the C ABI; 1e-5 relative on every F and F_k."""
+import dataclasses
+import math
+
+import numpy as np
+import pytest
+
+import synthetic as syn
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-5
+LAM = 2.0 * math.pi / 3.0
+
+
+@pytest.fixture(scope="module")
+def fs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2407_10797_b200 import build
+    build.build()
+    import paper_2407_10797_b200 as fs
+    fs.load_library()
+    return fs
+
+
+def _channels(orc, cfg, n):
+    """n data sets of one config: channel c sees the response with orbit_lambda = 2 pi c / 3 (X, Y, Z), its own noise
+    seed and the injection through its own response."""
+    out = []
+    for c in range(n):
+        o = orc.default_options(orbit_lambda=c * LAM)
+        ds = syn.make_dataset(dataclasses.replace(cfg, noise_seed=50 + c), lambda p, f, o=o: orc.template(p, f, o))
+        out.append((ds, o))
+    return out
+
+
+def _gpu(fs, chans, edges, par, **opt_kw):
+    import torch
+    plans = []
+    try:
+        for c, (ds, _) in enumerate(chans):
+            o = fs.fstat_default_options()
+            o.orbit_lambda = c * LAM
+            for k, v in opt_kw.items():
+                setattr(o, k, v)
+            plans.append(fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, o))
+        p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+        F, Fk = fs.fstat_eval_batch_channels(plans, p)
+        torch.cuda.synchronize()
+        return F.cpu().numpy(), Fk.cpu().numpy()
+    finally:
+        for pl in plans:
+            fs.fstat_plan_destroy(pl)
+
+
+def _compare(orc, chans, edges, par, F, Fk):
+    ds0 = chans[0][0]
+    F_o, Fk_o = orc.fstat_batch_channels(ds0.freq, [(ds.dw, ds.inv_sn, o) for ds, o in chans], edges, par)
+    fin = np.isfinite(Fk_o)
+    assert np.array_equal(np.isneginf(Fk), ~fin)
+    assert np.max(np.abs(Fk[fin] - Fk_o[fin]) / np.abs(Fk_o[fin])) <= RTOL
+    ok = np.isfinite(F_o)
+    assert np.array_equal(np.isneginf(F), ~ok)
+    assert np.max(np.abs(F[ok] - F_o[ok]) / np.abs(F_o[ok])) <= RTOL
+
+
+@pytest.mark.parametrize("n_ch", [1, 2, 3])
+def test_tiny_channels_every_F_and_Fk(fs, orc, n_ch):
+    cfg = syn.CONFIGS[0]
+    chans = _channels(orc, cfg, n_ch)
+    par = syn.draw_particles(cfg).copy()
+    par[5, 1] = -1.0                                       # one invalid particle flies
+    edges = chans[0][0].edges(4)
+    F, Fk = _gpu(fs, chans, edges, par)
+    _compare(orc, chans, edges, par, F, Fk)
+
+
+def test_fine_slice_three_channels_through_the_interpolating_kernel(fs, orc):
+    """A 2.5-yr slice (the interpolating kernel does all the work), X + Y + Z, every F and F_k."""
+    year = syn.YEAR_S
+    cfg = syn.Config(17, "ch_slice", 2.5 * year, 0.0200, 0.0202, (8,), (96,), 3.5 * year, "wide")
+    chans = _channels(orc, cfg, 3)
+    par = syn.draw_particles(cfg)
+    edges = chans[0][0].edges(8)
+    F, Fk = _gpu(fs, chans, edges, par)
+    _compare(orc, chans, edges, par, F, Fk)
+    F_d, Fk_d = _gpu(fs, chans, edges, par, force_level=-1)          # the direct kernel gives the same
+    assert np.max(np.abs(Fk - Fk_d) / np.abs(Fk_d)) <= 5e-6
+
+
+def test_first_stage_two_channels_sample(fs, orc):
+    """Config 1 at full size (N_p = 1024, P = 2048) with two channels; a sample of particles against the oracle."""
+    cfg = syn.CONFIGS[1]
+    chans = _channels(orc, cfg, 2)
+    par = syn.draw_particles(cfg)
+    edges = chans[0][0].edges(1024)
+    F, Fk = _gpu(fs, chans, edges, par)
+    sample = np.array([0, 167, 511, 1024, 1598, 2047])
+    _compare(orc, chans, edges, par[sample], F[sample], Fk[sample])
+
+
+def test_mismatching_plans_are_rejected(fs, orc):
+    import torch
+    cfg = syn.CONFIGS[0]
+    ds = syn.make_dataset(cfg, orc.template)
+    par = torch.as_tensor(syn.draw_particles(cfg), device="cuda")
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(4)) as a, \
+         fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(2)) as b:
+        with pytest.raises(fs.FstatError):
+            fs.fstat_eval_batch_channels([a, b], par)
+        with pytest.raises(fs.FstatError):
+            fs.fstat_eval_batch_channels([a, a], par)
+        F1, Fk1 = fs.fstat_eval_batch_channels([a], par)
+        F0, Fk0 = fs.fstat_eval_batch(a, par)
+        torch.cuda.synchronize()
+        assert torch.equal(F1, F0) and torch.equal(Fk1, Fk0)       # one channel: the same kernels, the same bits
