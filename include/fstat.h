@@ -150,6 +150,13 @@ FSTAT_API fstat_status fstat_eval_batch_bands(fstat_plan *plan, int64_t P, const
                                               int32_t edge_lattice, double *F, double *Fk, int64_t *band,
                                               void *cuda_stream);
 
+/* Rows f2 x f3: the extrinsic amplitudes a = M^-1 N (Eq. 10 :96) of every partition of every template's band, as
+ * fstat_eval_amplitudes gives them for the plan's partitions: amp [P][n_seg][4] DEVICE pointer, out (a_1..a_4; NaN
+ * for invalid particles, 0 for empty partitions).  n_seg = 1 is the coherent estimate over the template's band
+ * that App. B starts from.  EUNSUPPORTED with options.force_level == -1. */
+FSTAT_API fstat_status fstat_eval_amplitudes_bands(fstat_plan *plan, int64_t P, const double *params, int32_t n_seg,
+                                                   int32_t edge_lattice, double *amp, void *cuda_stream);
+
 /* fstat_eval_batch_bands with HOST buffers (params_host [P][6] in; F_host [P], Fk_host [P][n_seg] or NULL,
  * band_host [P][2] or NULL out): copies inside, returns after the results have landed.  Pinned buffers make the
  * copies asynchronous DMA. */

@@ -219,11 +219,12 @@ def band_edges(k_lo: int, k_hi: int, n_bins: int, n_seg: int, lattice: int = 1) 
 
 
 def fstat_bands(freq, dw, inv_sn, params, n_seg: int, lattice: int = 1, opt: Optional[Options] = None,
-                use_ld: bool = False):
+                use_ld: bool = False, want_amp: bool = False):
     """Row f2: the semi-coherent F-statistic with the paper's own segment limits: for every
     particle the template is windowed to its band [k_lo, k_hi) (t_f in [0, T_obs], T_obs = 1/df) and that
     band is cut into n_seg partitions (``band_edges``); F_k from the same inner products and 4x4 solve as
-    ``fstat_batch``; an empty partition contributes F_k = 0.  Returns F[P], Fk[P][n_seg], edges[P][n_seg+1]."""
+    ``fstat_batch``; an empty partition contributes F_k = 0.  Returns F[P], Fk[P][n_seg], edges[P][n_seg+1]
+    (and, with want_amp, the maximising amplitudes a[P][n_seg][4] of Eq. 10 :96; NaN for invalid particles)."""
     freq = np.ascontiguousarray(freq, dtype=np.float64)
     dw = np.ascontiguousarray(dw, dtype=np.complex128)
     inv_sn = np.ascontiguousarray(inv_sn, dtype=np.float64)
@@ -232,10 +233,11 @@ def fstat_bands(freq, dw, inv_sn, params, n_seg: int, lattice: int = 1, opt: Opt
     df = (freq[-1] - freq[0]) / (n - 1)
     P = params.shape[0]
     F, Fk = np.zeros(P), np.zeros((P, n_seg))
+    amp = np.zeros((P, n_seg, 4))
     edges = np.zeros((P, n_seg + 1), dtype=np.int64)
     for p in range(P):
         if not params_valid(params[p]):
-            F[p], Fk[p] = -np.inf, -np.inf
+            F[p], Fk[p], amp[p] = -np.inf, -np.inf, np.nan
             continue
         k_lo, k_hi = template_band(params[p], freq, 1.0 / df, opt)
         e = band_edges(k_lo, k_hi, n, n_seg, lattice)
@@ -249,8 +251,10 @@ def fstat_bands(freq, dw, inv_sn, params, n_seg: int, lattice: int = 1, opt: Opt
         for j in range(n_seg):
             if e[j + 1] > e[j]:
                 N, M = inner_products(dw, inv_sn, up, uc, df, int(e[j]), int(e[j + 1]), use_ld)
-                Fk[p, j] = fstat_from_NM(N, M)[0]
+                Fk[p, j], amp[p, j], _ = fstat_from_NM(N, M)
         F[p] = float(np.sum(Fk[p].astype(np.longdouble)))
+    if want_amp:
+        return F, Fk, edges, amp
     return F, Fk, edges
 
 

@@ -18,7 +18,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 # every symbol include/fstat.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
-    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_batch_channels", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
+    "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_amplitudes_bands", "fstat_eval_batch_channels", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error",
@@ -75,6 +75,8 @@ def load_library():
         L.fstat_eval_batch_bands.restype = C.c_int
         L.fstat_eval_batch_bands_host.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
         L.fstat_eval_batch_bands_host.restype = C.c_int
+        L.fstat_eval_amplitudes_bands.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp]
+        L.fstat_eval_amplitudes_bands.restype = C.c_int
         L.fstat_eval_batch_channels.argtypes = [C.POINTER(vp), C.c_int32, i64, vp, vp, vp, vp]
         L.fstat_eval_batch_channels.restype = C.c_int
         L.fstat_eval_batch_host.argtypes = [vp, i64, vp, vp, vp, vp]
@@ -288,6 +290,18 @@ def fstat_eval_batch_bands_host(plan: Plan, params, n_seg: int, edge_lattice: in
                                                       F.ctypes.data, Fk.ctypes.data, band.ctypes.data, _stream_ptr(stream)),
            "fstat_eval_batch_bands_host", plan)
     return F, Fk, band
+
+
+def fstat_eval_amplitudes_bands(plan: Plan, params, n_seg: int, edge_lattice: int = 1, stream=None):
+    """Rows f2 x f3: params [P][6] float64 CUDA tensor -> amp [P][n_seg][4] CUDA tensor, the amplitudes a = M^-1 N of
+    every partition of every template's own band."""
+    import torch
+    P = int(params.shape[0])
+    amp = torch.empty((P, int(n_seg), 4), dtype=torch.float64, device=params.device)
+    _check(load_library().fstat_eval_amplitudes_bands(plan.handle, P, _dev_ptr(params, "params", 6 * P), int(n_seg),
+                                                      int(edge_lattice), _dev_ptr(amp, "amp", 4 * P * int(n_seg)),
+                                                      _stream_ptr(stream)), "fstat_eval_amplitudes_bands", plan)
+    return amp
 
 
 def fstat_eval_batch_channels(plans, params, stream=None, want_Fk: bool = True):

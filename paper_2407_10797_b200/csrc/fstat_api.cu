@@ -618,6 +618,7 @@ struct BandReq {
     int32_t n_seg, lattice;   // partitions per template; lattice of the edge rule (reading A26)
     int32_t cell;             // width of the cells (= lattice, or kBandCell with edges that split the cells)
     int64_t *band_out;
+    double *amp;              // [P][n_seg][4] extrinsic amplitudes, or NULL
     fstat_plan *owner;        // the user's plan: timing ring and launch counter
 };
 
@@ -724,7 +725,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag, pl->d_part_seg, pl->d_valid,
                                               pl->d_perm, pl->d_band, pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins,
                                               pl->n_part, br->n_seg, br->lattice, br->cell, fa.part_sk, fa.part_sp, pl->orb,
-                                              F, Fk, st));
+                                              F, Fk, br->amp, st));
         tp->n_launches += rag ? 4 : 3;                 // band limits, [pieces], cells epilogue, F sums
         return FSTAT_OK;
     }
@@ -793,14 +794,20 @@ fstat_status fstat_eval_amplitudes(fstat_plan *pl, int64_t P, const double *para
     return eval_impl(pl, P, params, nullptr, nullptr, amp, stream);
 }
 
-fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *params, int32_t n_seg, int32_t edge_lattice,
-                                    double *F, double *Fk, int64_t *band, void *stream)
+static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, int32_t n_seg, int32_t edge_lattice,
+                               double *F, double *Fk, int64_t *band, double *amp, void *stream)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
     if (n_seg < 1 || edge_lattice < 1) return fail(pl, FSTAT_EINVAL, "n_seg < 1 or edge_lattice < 1");
     if (P == 0) return FSTAT_OK;
-    if (!params || !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    if (!params || (!F && !amp)) return fail(pl, FSTAT_EINVAL, "params or the output pointer is NULL");
+    if (!F) {                                          // amplitudes only: F goes to scratch
+        DeviceGuard g0(pl->device);
+        if (!g0.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+        CU_TRY(pl, grow(&pl->d_F, &pl->F_cap, (size_t)P));
+        F = pl->d_F;
+    }
     if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
     if (pl->n_bins >= ((int64_t)1 << 31) - edge_lattice) return fail(pl, FSTAT_EUNSUPPORTED, "grid too long for 32-bit bins");
     DeviceGuard g(pl->device);
@@ -827,15 +834,17 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
                                       (cell != edge_lattice ? (int64_t)(n_seg + 1) * kNAcc : 0)) * (int64_t)sizeof(double);
         int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
         if (batch < kThreads) batch = kThreads;
-        BandReq br{n_seg, edge_lattice, cell, nullptr, pl};
+        BandReq br{n_seg, edge_lattice, cell, nullptr, nullptr, pl};
         for (int64_t off = 0; off < P; off += batch) {
             const int64_t n = (P - off < batch) ? P - off : batch;
             br.band_out = band ? band + 2 * off : nullptr;
+            br.amp = amp ? amp + off * n_seg * 4 : nullptr;
             s = eval_impl(cp, n, params + 6 * off, F + off, Fk + off * n_seg, nullptr, stream, &br);
             if (s != FSTAT_OK) { pl->err = cp->err; return s; }
         }
         return FSTAT_OK;
     }
+    if (amp) return fail(pl, FSTAT_EUNSUPPORTED, "amplitudes need the interpolating path (force_level != -1, grid away from f = 0)");
     const int64_t n_groups = (P + kThreads - 1) / kThreads;
     const int64_t P_pad = n_groups * kThreads;
     // work segments: about 8 items per SM over the whole grid, whole tiles, 256 .. 8192 bins
@@ -889,6 +898,20 @@ fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *par
     CU_TRY(pl, launch_band_epilogue(pl->d_rec, pl->d_rec_idx, pl->d_valid, pl->d_perm, P_pad, (int32_t)n_wseg, n_seg, F, Fk, st));
     pl->n_launches += 5;                               // rank, prologue, band limits, band main, band epilogue
     return FSTAT_OK;
+}
+
+fstat_status fstat_eval_batch_bands(fstat_plan *pl, int64_t P, const double *params, int32_t n_seg, int32_t edge_lattice,
+                                    double *F, double *Fk, int64_t *band, void *stream)
+{
+    if (pl && P > 0 && !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    return bands_impl(pl, P, params, n_seg, edge_lattice, F, Fk, band, nullptr, stream);
+}
+
+fstat_status fstat_eval_amplitudes_bands(fstat_plan *pl, int64_t P, const double *params, int32_t n_seg,
+                                         int32_t edge_lattice, double *amp, void *stream)
+{
+    if (pl && P > 0 && !amp) return fail(pl, FSTAT_EINVAL, "params or amp is NULL");
+    return bands_impl(pl, P, params, n_seg, edge_lattice, nullptr, nullptr, nullptr, amp, stream);
 }
 
 fstat_status fstat_eval_batch_bands_host(fstat_plan *pl, int64_t P, const double *params_host, int32_t n_seg,

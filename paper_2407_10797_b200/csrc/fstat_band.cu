@@ -281,6 +281,23 @@ __global__ void __launch_bounds__(128) band_epilogue_kernel(const double *__rest
 //   LANES == 8: block = 32 slots (x) by 8 lanes (y), blockIdx.y walks the partitions and the lanes split the
 //               cells of one (slot, partition), combined through shared memory  (few, long partitions);
 //   LANES == 1: block = 32 slots by 8 partitions, one thread per (slot, partition)  (many short partitions).
+// F_k (and, rows f2 x f3, the extrinsic amplitudes a = M^-1 N of Eq. 10 :96) of one partition from its eight sums:
+// invalid particle: -inf / NaN; empty partition: 0 / 0.
+__device__ __forceinline__ void write_partition(const double (&v)[kNAcc], double cs_r, double cs_i, bool ok, bool live,
+                                                int64_t idx, double *__restrict__ Fk, double *__restrict__ amp)
+{
+    Fk[idx] = ok ? (live ? 0.5 * two_F(v) : 0.0) : -INFINITY;
+    if (amp != nullptr) {
+        double a1 = 0.0, a2 = 0.0, a3 = 0.0, a4 = 0.0;
+        if (ok && live) solve_amplitudes(v, cs_r, cs_i, a1, a2, a3, a4);
+        const double nan = __longlong_as_double(0x7ff8000000000000LL);
+        amp[4 * idx + 0] = ok ? a1 : nan;
+        amp[4 * idx + 1] = ok ? a2 : nan;
+        amp[4 * idx + 2] = ok ? a3 : nan;
+        amp[4 * idx + 3] = ok ? a4 : nan;
+    }
+}
+
 template <int LANES>
 __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *__restrict__ partial,
                                                                   const double *__restrict__ rag,
@@ -291,7 +308,7 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
                                                                   const int32_t *__restrict__ band_hi, int64_t P_pad,
                                                                   int32_t n_bins, int32_t n_cells, int32_t N, int32_t C,
                                                                   int32_t Cc, int64_t sk, int64_t sp,
-                                                                  double *__restrict__ Fk)
+                                                                  double *__restrict__ Fk, double *__restrict__ amp)
 {
     __shared__ double sV[LANES == 8 ? 8 : 1][kNAcc][32];
     const int tx = threadIdx.x, ty = threadIdx.y;
@@ -307,6 +324,7 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
 #pragma unroll
         for (int i = 0; i < kNAcc; ++i) v[i] = 0.0;
         bool live = false;                                   // a non-empty partition of a valid particle
+        double cs_r = 0.0, cs_i = 0.0;                       // the basis the sums are brought to
         if (ok) {
             const int32_t ea = band_edge(j, q_lo, D, N, C, n_bins), eb = band_edge(j + 1, q_lo, D, N, C, n_bins);
             if (eb > ea) {
@@ -322,7 +340,8 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
                 }
                 // common basis: the one of the cell that starts at or holds e_j (always evaluated for this group)
                 const double *first = partial + ((int64_t)part_seg[ea / Cc] * kNPartial) * P_pad + p * sp;
-                const double cs_r = first[8 * sk], cs_i = first[9 * sk];
+                cs_r = first[8 * sk];
+                cs_i = first[9 * sk];
                 // sgn x (left or right piece of the cell edge e splits), e = edge number je of this template
                 auto add_piece = [&](int32_t e, int je, bool want_left, double sgn) {
                     const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
@@ -370,11 +389,11 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
                     for (int y = 0; y < 8; ++y) acc += sV[y][i][tx];
                     v[i] = acc;
                 }
-                Fk[(int64_t)particle * N + j] = ok ? (live ? 0.5 * two_F(v) : 0.0) : -INFINITY;
+                write_partition(v, cs_r, cs_i, ok, live, (int64_t)particle * N + j, Fk, amp);
             }
             __syncthreads();
         } else if (particle >= 0) {
-            Fk[(int64_t)particle * N + j] = ok ? (live ? 0.5 * two_F(v) : 0.0) : -INFINITY;
+            write_partition(v, cs_r, cs_i, ok, live, (int64_t)particle * N + j, Fk, amp);
         }
     }
 }
@@ -471,7 +490,7 @@ cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, 
                                        const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
                                        int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
                                        int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
-                                       cudaStream_t st)
+                                       double *amp, cudaStream_t st)
 {
     cudaError_t e;
     if (rag != nullptr) {
@@ -486,12 +505,12 @@ cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, 
         if (gy > 4096) gy = 4096;
         band_cells_epilogue_kernel<1><<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
             partial, rag, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
-            part_sk, part_sp, Fk);
+            part_sk, part_sp, Fk, amp);
     } else {
         const int gy = n_seg_band < 4096 ? n_seg_band : 4096;
         band_cells_epilogue_kernel<8><<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
             partial, rag, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
-            part_sk, part_sp, Fk);
+            part_sk, part_sp, Fk, amp);
     }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     band_fsum_kernel<<<(unsigned)((P + 3) / 4), 128, 0, st>>>(Fk, P, n_seg_band, F);

@@ -81,4 +81,32 @@ __device__ __forceinline__ void add_segment(const double *__restrict__ partial, 
     add_record(t, cs_r, cs_i, v);
 }
 
+// Extrinsic amplitudes (Eq. 10): alpha = G^-1 z for the 2x2 Hermitian G of the eight sums v, which are
+// in the basis (u_+, u_x - c* u_+); returns a_1 = Re alpha_+, a_2 = Re alpha_x, a_3 = Im alpha_+, a_4 = Im alpha_x
+// of the plain basis.  Rank-deficient G: the degenerate component is set to 0 (reading A15).
+__device__ __forceinline__ void solve_amplitudes(const double (&v)[kNAcc], double cs_r, double cs_i, double &apr,
+                                                 double &acr, double &api, double &aci)
+{
+    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
+    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
+    apr = 0.0; api = 0.0; acr = 0.0; aci = 0.0;
+    if (mpp > 0.0) {
+        const double inv = 1.0 / mpp;
+        const double cr = mr * inv, ci = mi * inv;                          // m_pc / m_pp
+        const double schur = mcc - (mr * mr + mi * mi) * inv;
+        if (schur > 1e-13 * mcc) {
+            acr = (zcr - (cr * zpr - ci * zpi)) / schur;                    // alpha_x = (z_x - (m_pc/m_pp) z_+) / schur
+            aci = (zci - (cr * zpi + ci * zpr)) / schur;
+        }
+        apr = (zpr - (mr * acr + mi * aci)) * inv;                          // alpha_+ = (z_+ - conj(m_pc) alpha_x) / m_pp
+        api = (zpi - (mr * aci - mi * acr)) * inv;
+        // the sums are in the basis (u_+, u_x - c* u_+): h = alpha~_+ u_+ + alpha_x (u_x - c* u_+)
+        apr -= cs_r * acr - cs_i * aci;
+        api -= cs_r * aci + cs_i * acr;
+    } else if (mcc > 0.0) {
+        acr = zcr / mcc;
+        aci = zci / mcc;
+    }
+}
+
 }  // namespace fstat

@@ -174,7 +174,7 @@ cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, 
                                        const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
                                        int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
                                        int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
-                                       cudaStream_t st);
+                                       double *amp, cudaStream_t st);
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
                                double df, double arm_length_m, double *table, double *dwp,

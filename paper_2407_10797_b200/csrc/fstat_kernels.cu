@@ -492,26 +492,8 @@ __global__ void __launch_bounds__(128) amplitude_kernel(const double *__restrict
     const double cs_r = partial[((int64_t)s_first * kNPartial + 8) * P_pad + p];
     const double cs_i = partial[((int64_t)s_first * kNPartial + 9) * P_pad + p];
     for (int s = s_first; s < part_seg[k + 1]; ++s) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
-    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
-    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
-    double apr = 0.0, api = 0.0, acr = 0.0, aci = 0.0;
-    if (mpp > 0.0) {
-        const double inv = 1.0 / mpp;
-        const double cr = mr * inv, ci = mi * inv;                          // m_pc / m_pp
-        const double schur = mcc - (mr * mr + mi * mi) * inv;
-        if (schur > 1e-13 * mcc) {
-            acr = (zcr - (cr * zpr - ci * zpi)) / schur;                    // alpha_x = (z_x - (m_pc/m_pp) z_+) / schur
-            aci = (zci - (cr * zpi + ci * zpr)) / schur;
-        }
-        apr = (zpr - (mr * acr + mi * aci)) * inv;                          // alpha_+ = (z_+ - conj(m_pc) alpha_x) / m_pp
-        api = (zpi - (mr * aci - mi * acr)) * inv;
-        // the sums are in the basis (u_+, u_x - c* u_+): h = alpha~_+ u_+ + alpha_x (u_x - c* u_+)
-        apr -= cs_r * acr - cs_i * aci;
-        api -= cs_r * aci + cs_i * acr;
-    } else if (mcc > 0.0) {
-        acr = zcr / mcc;
-        aci = zci / mcc;
-    }
+    double apr, acr, api, aci;
+    solve_amplitudes(v, cs_r, cs_i, apr, acr, api, aci);
     const bool ok = valid[p] != 0;
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     double *out = amp + ((int64_t)perm[p] * n_part + k) * 4;
