@@ -104,6 +104,14 @@ def test_null_plan_calls_are_safe(fs):
     assert lib.fstat_plan_device(None) == -1
     assert lib.fstat_eval_batch(None, 1, None, None, None, None) == 1
     assert lib.fstat_plan_launch_count(None) == 0
+    # the rows built on top of the path (f2, f2 x f3, f4) answer FSTAT_EINVAL too
+    assert lib.fstat_eval_batch_bands(None, 1, None, 4, 1, None, None, None, None) == 1
+    assert lib.fstat_eval_batch_bands_host(None, 1, None, 4, 1, None, None, None, None) == 1
+    assert lib.fstat_eval_amplitudes_bands(None, 1, None, 4, 1, None, None) == 1
+    assert lib.fstat_eval_batch_channels(None, 2, 1, None, None, None, None) == 1
+    import ctypes
+    two_nulls = (ctypes.c_void_p * 2)(None, None)
+    assert lib.fstat_eval_batch_channels(two_nulls, 2, 1, None, None, None, None) == 1
 
 
 def test_no_cpu_fallback_without_a_device(fs):
