@@ -192,3 +192,19 @@ def test_bands_wide_band_in_particle_batches(fs, orc):
     assert np.max(np.abs(Fk[live] - Fk2[live]) / np.abs(Fk2[live])) <= 5e-6
     sample = np.array([0, 1500, 2047, 2048, 3000, 4095])      # both batches
     _check(orc, ds, par[sample], 16, 64, F[sample], Fk[sample], band[sample])
+
+
+@pytest.mark.parametrize("lattice", [1, 64])
+def test_bands_odd_sizes(fs, orc, lattice):
+    """A grid whose length is 3 modulo 64 (the last cell is shorter than the smallest node stride and goes to the
+    direct kernel), 37 particles (a partly filled group), 5 partitions."""
+    import dataclasses
+    T = syn.BANDS_SMALL.T
+    cfg = dataclasses.replace(syn.BANDS_SMALL, f_lo=0.020, f_hi=(380348 + 0.5) / T)
+    ds = syn.make_dataset(cfg, orc.template)
+    assert ds.n_bins % 64 == 3
+    par = syn.draw_particles(cfg, 37)
+    par[:, 0] = np.linspace(0.9, 2.2, 37) * syn.YEAR_S       # several bands reach the end of the grid
+    F, Fk, band = _gpu(fs, ds, par, 5, lattice)
+    n = _check(orc, ds, par, 5, lattice, F, Fk, band)
+    assert n >= 30 and (band[:, 1] == ds.n_bins).sum() >= 3
