@@ -118,18 +118,7 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
         const int n_bins = hi - lo;
         const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
         const double *src = a.table + (int64_t)lo * kTabW;
-        if (tid == 0) {
-#pragma unroll
-            for (int s = 0; s < kStages; ++s) {
-                if (s < n_tiles) {
-                    const int slot = (g0 + s) % kStages;
-                    const int nb = min(kTileBins, n_bins - s * kTileBins);
-                    const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
-                    mbar_expect_tx(&sm.full[slot], bytes);
-                    tma_load_1d(sm.tile[slot], src + (int64_t)s * kTileBins * kTabW, bytes, &sm.full[slot]);
-                }
-            }
-        }
+        if (tid == 0) ring_prologue(sm, src, n_bins, n_tiles, g0);
 
         double c[kNCoef];
 #pragma unroll
@@ -159,11 +148,8 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
         for (int i = 0; i < kNAcc; ++i) acc[i] = 0.0;
 
         for (int t = 0; t < n_tiles; ++t) {
-            const int g = g0 + t;
-            const int slot = g % kStages;
-            mbar_wait(&sm.full[slot], (uint32_t)((g / kStages) & 1));
+            const double *tile = ring_wait(sm, g0 + t);
             const int nb = min(kTileBins, n_bins - t * kTileBins);
-            const double *tile = sm.tile[slot];
             double in[kNAcc];
 #pragma unroll
             for (int i = 0; i < kNAcc; ++i) in[i] = 0.0;
@@ -211,13 +197,7 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
             for (int i = 0; i < kNAcc; ++i) acc[i] += in[i];
 
             __syncthreads();                             // every thread is done with this slot
-            if (tid == 0 && t + kStages < n_tiles) {
-                const int tn = t + kStages;
-                const int nbn = min(kTileBins, n_bins - tn * kTileBins);
-                const uint32_t bytes = (uint32_t)nbn * kTabW * sizeof(double);
-                mbar_expect_tx(&sm.full[slot], bytes);
-                tma_load_1d(sm.tile[slot], src + (int64_t)tn * kTileBins * kTabW, bytes, &sm.full[slot]);
-            }
+            if (tid == 0 && t + kStages < n_tiles) ring_issue(sm, src, n_bins, g0, t + kStages);
         }
         g0 += n_tiles;
 

@@ -13,6 +13,31 @@ struct __align__(16) MainSmem {
     uint64_t full[kStages];
 };
 
+// The ring of table-row tiles both full-model kernels stream their bins through (one elected thread issues the
+// TMA bulk copies; g0 = tiles this CTA has consumed so far = ring position of the work item's first tile).
+__device__ __forceinline__ void ring_issue(MainSmem &sm, const double *src, int n_bins, int g0, int t)
+{
+    const int slot = (g0 + t) % kStages;
+    const int nb = min(kTileBins, n_bins - t * kTileBins);
+    const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
+    mbar_expect_tx(&sm.full[slot], bytes);
+    tma_load_1d(sm.tile[slot], src + (int64_t)t * kTileBins * kTabW, bytes, &sm.full[slot]);
+}
+
+__device__ __forceinline__ void ring_prologue(MainSmem &sm, const double *src, int n_bins, int n_tiles, int g0)
+{
+#pragma unroll
+    for (int s = 0; s < kStages; ++s)
+        if (s < n_tiles) ring_issue(sm, src, n_bins, g0, s);
+}
+
+__device__ __forceinline__ const double *ring_wait(MainSmem &sm, int g)
+{
+    const int slot = g % kStages;
+    mbar_wait(&sm.full[slot], (uint32_t)((g / kStages) & 1));
+    return sm.tile[slot];
+}
+
 
 // One (particle, bin) of the direct kernel: model_eval() plus the linear phase term and the carrier.
 // Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1 included), its sine and
