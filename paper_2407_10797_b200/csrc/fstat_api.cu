@@ -719,10 +719,12 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     if (br) {
         double *rag = nullptr;
         if (br->cell != br->lattice) {                 // edges at any bin: the cells they fall into are split
-            CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(br->n_seg + 1) * kNAcc));
-            rag = pl->d_rag;
+            CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(2 * br->n_seg + 1) * kNAcc));
+            rag = pl->d_rag;                           // [P_pad][n_seg + 1] pieces, then [P_pad][n_seg] short partitions
         }
-        CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag, pl->d_part_seg, pl->d_valid,
+        CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag,
+                                              rag ? rag + (size_t)P_pad * (size_t)(br->n_seg + 1) * kNAcc : nullptr,
+                                              pl->d_part_seg, pl->d_valid,
                                               pl->d_perm, pl->d_band, pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins,
                                               pl->n_part, br->n_seg, br->lattice, br->cell, fa.part_sk, fa.part_sp, pl->orb,
                                               F, Fk, br->amp, st));
@@ -831,7 +833,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
         }
         // one record of 10 sums per (cell, particle): keep the workspace below ~24 GB by batching the particles
         const int64_t per_particle = ((int64_t)cp->n_part * kNPartial +
-                                      (cell != edge_lattice ? (int64_t)(n_seg + 1) * kNAcc : 0)) * (int64_t)sizeof(double);
+                                      (cell != edge_lattice ? (int64_t)(2 * n_seg + 1) * kNAcc : 0)) * (int64_t)sizeof(double);
         int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
         if (batch < kThreads) batch = kThreads;
         BandReq br{n_seg, edge_lattice, cell, nullptr, nullptr, pl};

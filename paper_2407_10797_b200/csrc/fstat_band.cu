@@ -256,8 +256,9 @@ __global__ void __launch_bounds__(128) band_epilogue_kernel(const double *__rest
 // cells; C = lattice of the edge rule.  rag == nullptr: C == Cc, every edge is a cell boundary.  Otherwise an
 // edge may split its cell and rag holds the two pieces (band_ragged_kernel): a partition is
 //   right piece of e_j  +  the whole cells between  +  left piece of e_{j+1},
-// or left(e_{j+1}) - left(e_j) when both edges fall into one cell.  Everything is brought to the basis of the
-// first whole cell (recentred basis, add_record) and summed in a fixed order.
+// except that a partition with no whole cell inside is evaluated in full, edge to edge (rag_short): short
+// partitions are the ill-conditioned ones.  Everything is brought to one basis (recentred basis, add_record) and
+// summed in a fixed order.
 //   LANES == 8: block = 32 slots (x) by 8 lanes (y), blockIdx.y walks the partitions and the lanes split the
 //               cells of one (slot, partition), combined through shared memory  (few, long partitions);
 //   LANES == 1: block = 32 slots by 8 partitions, one thread per (slot, partition)  (many short partitions).
@@ -281,6 +282,7 @@ __device__ __forceinline__ void write_partition(const double (&v)[kNAcc], double
 template <int LANES>
 __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *__restrict__ partial,
                                                                   const double *__restrict__ rag,
+                                                                  const double *__restrict__ rag_short,
                                                                   const int32_t *__restrict__ part_seg,
                                                                   const int32_t *__restrict__ valid,
                                                                   const int32_t *__restrict__ perm,
@@ -343,10 +345,13 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
                         }
                     }
                 };
-                if (ca > cb) {                               // both edges inside one cell: left(e_{j+1}) - left(e_j)
+                if (rag != nullptr && ca >= cb) {            // no whole cell inside: evaluated in full, edge to edge
+                    cs_r = 0.0;
+                    cs_i = 0.0;
                     if (lane == 0) {
-                        add_piece(eb, jb, true, 1.0);
-                        add_piece(ea, ja, true, -1.0);
+                        const double *r = rag_short + ((int64_t)p * N + j) * kNAcc;
+#pragma unroll
+                        for (int i = 0; i < kNAcc; ++i) v[i] = r[i];
                     }
                 } else {
                     if (!onA && lane == 0) add_piece(ea, ja, false, 1.0);
@@ -386,14 +391,15 @@ __global__ void __launch_bounds__(256) band_cells_epilogue_kernel(const double *
 // table: rag[(p (N + 1) + j) 8 + i], plain basis (c = 0); the other piece is the cell's record minus this one
 // (the cell's record carries the interpolation error of any other cell, the piece none).  A partition is then
 //   right piece of e_j  +  the whole cells between  +  left piece of e_{j+1}
-// (both edges in one cell: left(e_{j+1}) - left(e_j)), combined by band_cells_epilogue_kernel.
+// (a partition with no whole cell inside is evaluated edge to edge instead), combined by band_cells_epilogue_kernel.
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restrict__ table, const double *__restrict__ coef,
                                                           const int32_t *__restrict__ valid,
                                                           const int32_t *__restrict__ band_lo,
                                                           const int32_t *__restrict__ band_hi, int64_t P_pad,
                                                           int32_t n_bins, int32_t N, int32_t C, int32_t Cc,
-                                                          const __grid_constant__ OrbitCoef orb, double *__restrict__ rag)
+                                                          const __grid_constant__ OrbitCoef orb, double *__restrict__ rag,
+                                                          double *__restrict__ rag_short)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P_pad || valid[p] == 0) return;
@@ -402,19 +408,13 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
     double c[kNCoef];
 #pragma unroll
     for (int i = 0; i < kNCoef; ++i) c[i] = coef[(int64_t)i * P_pad + p];
-    for (int j = blockIdx.y; j <= N; j += gridDim.y) {
-        const int32_t e = band_edge(j, q_lo, D, N, C, n_bins);
-        if (e >= n_bins || e % Cc == 0) continue;                       // a cell boundary: nothing to split
-        if (j > 0 && band_edge(j - 1, q_lo, D, N, C, n_bins) == e) continue;   // same edge as the previous one
-        const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
-        const bool left = (e - c0) <= (c1 - e);                         // the shorter piece; the other one is cell - piece
-        const int32_t b0 = left ? c0 : e, b1 = left ? e : c1;
-        double *out = rag + ((int64_t)p * (N + 1) + j) * kNAcc;
+    // sums of the full model over the bins [b0, b1) into out[0..7] (plain basis).  The next bin's table row is
+    // fetched while this one is evaluated (every thread walks its own rows: nothing to share through shared
+    // memory, and the loads would otherwise sit in front of 263 dependent FP64 instructions).
+    auto eval_range = [&](int32_t b0, int32_t b1, double *__restrict__ out) {
         double acc[kNAcc];
 #pragma unroll
         for (int i = 0; i < kNAcc; ++i) acc[i] = 0.0;
-        // the next bin's table row is fetched while this one is evaluated (every thread walks its own rows:
-        // nothing to share through shared memory, and the loads would otherwise sit in front of 263 dependent FP64s)
         double2 cur[12], nxt[12];
         {
             const double2 *r0 = reinterpret_cast<const double2 *>(table + (int64_t)b0 * kTabW);
@@ -447,6 +447,22 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
         }
 #pragma unroll
         for (int i = 0; i < kNAcc; ++i) out[i] = acc[i];
+    };
+    for (int j = blockIdx.y; j <= N; j += gridDim.y) {
+        const int32_t e = band_edge(j, q_lo, D, N, C, n_bins);
+        // (1) a partition that holds no whole cell is evaluated in full, edge to edge: short partitions have a
+        // near-singular M_k (conditioning note) and must not see the interpolation error of a cell record
+        if (j < N) {
+            const int32_t eb = band_edge(j + 1, q_lo, D, N, C, n_bins);
+            const int32_t ca = (e + Cc - 1) / Cc, cb = eb >= n_bins ? (n_bins + Cc - 1) / Cc : eb / Cc;
+            if (eb > e && ca >= cb) eval_range(e, eb, rag_short + ((int64_t)p * N + j) * kNAcc);
+        }
+        // (2) the shorter piece of the cell this edge splits (the other piece is the cell's record minus it)
+        if (e >= n_bins || e % Cc == 0) continue;                       // a cell boundary: nothing to split
+        if (j > 0 && band_edge(j - 1, q_lo, D, N, C, n_bins) == e) continue;   // same edge as the previous one
+        const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
+        const bool left = (e - c0) <= (c1 - e);
+        eval_range(left ? c0 : e, left ? e : c1, rag + ((int64_t)p * (N + 1) + j) * kNAcc);
     }
 }
 
@@ -466,7 +482,7 @@ __global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict
 
 // rag == nullptr: every edge is a cell boundary (lattice == cell); else the pieces are computed first.
 cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, const double *partial, double *rag,
-                                       const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
+                                       double *rag_short, const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
                                        const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
                                        int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
                                        int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
@@ -477,19 +493,19 @@ cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, 
         int gy = n_seg_band + 1;
         if (gy > 2048) gy = 2048;
         band_ragged_kernel<<<dim3((unsigned)(P_pad / 128), (unsigned)gy), 128, 0, st>>>(
-            table, coef, valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, orb, rag);
+            table, coef, valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, orb, rag, rag_short);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     if ((int64_t)n_cells < (int64_t)32 * n_seg_band) {      // a few cells per partition: one thread per partition
         int gy = (n_seg_band + 7) / 8;
         if (gy > 4096) gy = 4096;
         band_cells_epilogue_kernel<1><<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
-            partial, rag, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
+            partial, rag, rag_short, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
             part_sk, part_sp, Fk, amp);
     } else {
         const int gy = n_seg_band < 4096 ? n_seg_band : 4096;
         band_cells_epilogue_kernel<8><<<dim3((unsigned)(P_pad / 32), (unsigned)gy), dim3(32, 8), 0, st>>>(
-            partial, rag, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
+            partial, rag, rag_short, part_seg, valid, perm, band_lo, band_hi, P_pad, n_bins, n_cells, n_seg_band, lattice, cell,
             part_sk, part_sp, Fk, amp);
     }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;

@@ -208,3 +208,38 @@ def test_bands_odd_sizes(fs, orc, lattice):
     F, Fk, band = _gpu(fs, ds, par, 5, lattice)
     n = _check(orc, ds, par, 5, lattice, F, Fk, band)
     assert n >= 30 and (band[:, 1] == ds.n_bins).sum() >= 3
+
+
+@pytest.mark.parametrize("n_seg", [256, 1024])
+def test_bands_narrow_bands_and_short_partitions_against_full_model(fs, n_seg):
+    """A harder population than BASELINE.json's (M_c 10-60, e_0 up to 0.3) on the 2.5-yr grid: slowly evolving
+    templates have bands of a few thousand bins, i.e. partitions far shorter than a cell.  A partition with no whole
+    cell inside is evaluated edge to edge with the full model (an earlier version built it from differences of cell
+    records and was off by up to 7e-4 there: short partitions have a near-singular M_k and amplify the interpolation
+    error of a record); every F_k of partitions of >= 16 bins against the full-model kernel.  (Shorter ones are
+    beyond FP64 for any evaluation order.)"""
+    import torch
+    from synthetic import lisa_data as L
+    cfg = syn.CONFIGS[1]
+    _, n, f = syn.frequency_grid(cfg.T, cfg.f_lo, cfg.f_hi)
+    sn = syn.psd_tdi_x(f)
+    d = syn.coloured_noise(sn, cfg.T, 7)
+    rng = np.random.default_rng(1003)
+    par = L._wide_particles(rng, 2048, cfg.T)
+    par[:, 5] = rng.uniform(0.0, 0.3, 2048)
+    par[:, 1] = rng.uniform(10.0, 60.0, 2048)
+    direct = fs.fstat_default_options()
+    direct.force_level = -1
+    out = []
+    for opts in (None, direct):
+        with fs.fstat_plan_create(f, d / sn, 1.0 / sn, syn.equal_bin_edges(n, 1), opts) as plan:
+            p = torch.as_tensor(par, device="cuda")
+            F, Fk, band = fs.fstat_eval_batch_bands(plan, p, n_seg, 1)
+            torch.cuda.synchronize()
+            out.append((Fk.cpu().numpy(), band.cpu().numpy()))
+    (Fk_a, b_a), (Fk_b, b_b) = out
+    assert np.array_equal(b_a, b_b) and np.array_equal(Fk_a == 0.0, Fk_b == 0.0)
+    width = b_a[:, 1] - b_a[:, 0]
+    assert ((width > 0) & (width < 64 * n_seg)).sum() >= 10          # templates whose partitions are shorter than a cell
+    long_enough = (width // n_seg >= 16)[:, None] & (Fk_b != 0.0)
+    assert np.max(np.abs(Fk_a[long_enough] - Fk_b[long_enough]) / np.abs(Fk_b[long_enough])) <= 5e-6
