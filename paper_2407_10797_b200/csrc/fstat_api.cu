@@ -668,6 +668,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         bs.n_seg_band = br->n_seg;
         bs.lattice = br->lattice;
         bs.n_bins = (int32_t)pl->n_bins;
+        bs.min_len = br->cell != br->lattice ? br->cell : 1;
     }
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
                                pl->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,

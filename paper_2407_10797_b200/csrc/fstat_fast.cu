@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
                 level[(int64_t)grp * n_seg + seg] = (int8_t)-2;
                 continue;
             }
-            q.kl = 0.05 * (double)g_len;
+            q.kl = 0.05 * (double)max(g_len, bands.min_len);
         }
         const double om = fma(c3, q.p1, c9 * q.p2);
         const double d3 = fma(c3, q.r1, fma(c9, q.r2, q.ad * (128.0 / 3.0) * om * om * om));   // |D3|, quarter turns

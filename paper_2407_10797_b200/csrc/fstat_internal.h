@@ -140,6 +140,7 @@ struct BandSched {
     int32_t n_seg_band;       // partitions per template
     int32_t lattice;
     int32_t n_bins;
+    int32_t min_len;          // shorter partitions do not use the cell records (they are evaluated edge to edge)
 };
 
 // row f2 (fstat_band.cu): per-particle bands and partition edges
