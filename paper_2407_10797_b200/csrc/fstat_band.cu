@@ -6,24 +6,31 @@
 //
 //   band_kernel          k_lo = #{bins with t_f < 0}, k_hi = #{bins with t_f <= T_obs} per particle, by
 //                        bisection over the per-bin table (t_f increases along the grid)
-//   fstat_band_kernel    the direct kernel (full model at every bin) with per-THREAD partition edges:
-//                        a partition that opens and closes inside one work segment is finished in the
-//                        thread (2 F_k written at once); the fragment before the first edge and the
-//                        one after the last edge of a work segment go to head / tail records
-//   band_epilogue_kernel stitches head / tail records of consecutive work segments into the partitions
-//                        that straddle them, writes their F_k, then F = sum_k F_k in a fixed order
 //
-// That path takes edges at ANY bin (edge_lattice < 32) and pays the full model at every in-band bin.  With
-// edges on a lattice of C >= 32 bins the interpolating kernel does the work instead: the lattice cells are
-// the (data-side) partitions of an internal plan, fstat_fast_kernel / fstat_main_kernel run unchanged and
-// leave one record of sums per (cell, particle), the stride selection skips the cells no template of a group
-// is in band for, and
+// The normal path is the interpolating kernel over CELLS of the grid: the cells are the (data-side) partitions of
+// an internal plan, fstat_fast_kernel / fstat_main_kernel run unchanged and leave one record of sums per (cell,
+// particle), the stride selection skips the cells no template of a group is in band for, and
 //
-//   band_cells_epilogue_kernel   adds, per particle and partition, the records of the cells between its
-//                                edges (recentred basis, add_segment) and writes F_k
+//   band_cells_epilogue_kernel   adds, per particle and partition, the records of the cells between its edges
+//                                (recentred basis, add_segment) and writes F_k [and the amplitudes a = M^-1 N]
 //   band_fsum_kernel             F = sum_k F_k in a fixed order
-// and below 32 bins (edges at any bin) the cells are 64 bins wide and
-//   band_ragged_kernel           evaluates, with the full model, the two pieces of every cell an edge splits
+//
+// With edges on a lattice of C >= 32 bins the cells are the lattice.  Below that (default: edges at ANY bin) the
+// cells are 64..512 bins wide and an edge may split a cell:
+//
+//   band_ragged_kernel           full model over the shorter piece of every cell an edge splits (the other piece
+//                                is the cell's record minus it), and over every partition that holds no whole
+//                                cell, edge to edge
+//
+// The first version of the row is kept as the full-size reference of the above (options.force_level == -1, or a
+// grid too close to f = 0 for the node table):
+//
+//   fstat_band_kernel    the direct kernel (full model at every in-band bin) with per-THREAD partition edges: a
+//                        partition that opens and closes inside one work segment is finished in the thread
+//                        (2 F_k written at once); the fragment before the first edge and the one after the last
+//                        edge of a work segment go to head / tail records
+//   band_epilogue_kernel stitches head / tail records of consecutive work segments into the partitions that
+//                        straddle them, writes their F_k, then F = sum_k F_k in a fixed order
 #include "fstat_device.cuh"
 #include "fstat_direct.cuh"
 #include "fstat_internal.h"
