@@ -62,6 +62,8 @@ struct fstat_plan {
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
     double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
     int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
+    int32_t *d_piece_scratch = nullptr; size_t piece_scratch_cap = 0;   // length-class counts and starts of the piece list
+    int2 *d_piece_list = nullptr; size_t piece_list_cap = 0;            // [P_pad (n_seg + 1)] (slot, edge) ordered by length
     double *d_rag = nullptr; size_t rag_cap = 0;          // [P_pad][n_seg + 1][kNAcc] the shorter piece of every cell an edge splits
     double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
     int64_t *d_band_out = nullptr; size_t band_out_cap = 0; // [P][2] (host-buffer call)
@@ -448,7 +450,7 @@ static void plan_free(fstat_plan *pl)
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
-    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out); cudaFree(pl->d_rag);
+    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out); cudaFree(pl->d_rag); cudaFree(pl->d_piece_scratch); cudaFree(pl->d_piece_list);
     cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
@@ -721,11 +723,13 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         double *rag = nullptr;
         if (br->cell != br->lattice) {                 // edges at any bin: the cells they fall into are split
             CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(2 * br->n_seg + 1) * kNAcc));
+            CU_TRY(pl, grow(&pl->d_piece_scratch, &pl->piece_scratch_cap, (size_t)256));
+            CU_TRY(pl, grow(&pl->d_piece_list, &pl->piece_list_cap, (size_t)P_pad * (size_t)(br->n_seg + 1)));
             rag = pl->d_rag;                           // [P_pad][n_seg + 1] pieces, then [P_pad][n_seg] short partitions
         }
         CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag,
                                               rag ? rag + (size_t)P_pad * (size_t)(br->n_seg + 1) * kNAcc : nullptr,
-                                              pl->d_part_seg, pl->d_valid,
+                                              rag ? pl->d_piece_scratch : nullptr, pl->d_piece_list, pl->d_part_seg, pl->d_valid,
                                               pl->d_perm, pl->d_band, pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins,
                                               pl->n_part, br->n_seg, br->lattice, br->cell, fa.part_sk, fa.part_sp, pl->orb,
                                               F, Fk, br->amp, st));
@@ -834,7 +838,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
         }
         // one record of 10 sums per (cell, particle): keep the workspace below ~24 GB by batching the particles
         const int64_t per_particle = ((int64_t)cp->n_part * kNPartial +
-                                      (cell != edge_lattice ? (int64_t)(2 * n_seg + 1) * kNAcc : 0)) * (int64_t)sizeof(double);
+                                      (cell != edge_lattice ? (int64_t)(2 * n_seg + 1) * kNAcc + (n_seg + 1) : 0)) * (int64_t)sizeof(double);
         int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
         if (batch < kThreads) batch = kThreads;
         BandReq br{n_seg, edge_lattice, cell, nullptr, nullptr, pl};

@@ -20,7 +20,8 @@
 //
 //   band_ragged_kernel           full model over the shorter piece of every cell an edge splits (the other piece
 //                                is the cell's record minus it), and over every partition that holds no whole
-//                                cell, edge to edge
+//                                cell, edge to edge (for N_seg >= 128 the pieces go through piece_list_kernel /
+//                                band_ragged_sorted_kernel: ordered by length, one list entry per thread)
 //
 // The first version of the row is kept as the full-size reference of the above (options.force_level == -1, or a
 // grid too close to f = 0 for the node table):
@@ -258,6 +259,124 @@ __global__ void __launch_bounds__(128) band_epilogue_kernel(const double *__rest
     F[particle] = f;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// The same pieces ordered by length, for many partitions (cells of at most 128 bins): the piece lengths are
+// uniform in 1 .. Cc/2, so a warp of band_ragged_kernel runs with half of its lanes masked.  piece_list_kernel
+// enumerates the pieces twice (count, then fill) into a list ordered by length -- per-block shared-memory
+// histograms, one global atomic per (block, length) -- and band_ragged_sorted_kernel evaluates one list entry
+// per thread: the lanes of a warp then run the same number of bins.  The order inside a length class depends
+// on atomics; the values do not.  (Partitions with no whole cell inside stay with band_ragged_kernel.)
+// ---------------------------------------------------------------------------------------------------
+constexpr int kMaxPieceLen = 64;                              // Cc / 2 for Cc <= 128
+
+template <bool FILL>
+__global__ void __launch_bounds__(128) piece_list_kernel(const int32_t *__restrict__ valid,
+                                                         const int32_t *__restrict__ band_lo,
+                                                         const int32_t *__restrict__ band_hi, int64_t P_pad,
+                                                         int32_t n_bins, int32_t N, int32_t C, int32_t Cc,
+                                                         int32_t *__restrict__ len_count,          // [kMaxPieceLen + 1]
+                                                         const int32_t *__restrict__ len_start,    // [kMaxPieceLen + 2]
+                                                         int2 *__restrict__ list)
+{
+    __shared__ int32_t hist[kMaxPieceLen + 1], base[kMaxPieceLen + 1];
+    const int tid = threadIdx.x;
+    for (int i = tid; i <= kMaxPieceLen; i += 128) hist[i] = 0;
+    __syncthreads();
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + tid;
+    const int j = blockIdx.y;                                 // one edge per block row: gridDim.y = N + 1
+    int32_t len = 0, rank = 0;
+    if (p < P_pad && valid[p] != 0) {
+        const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
+        if (D > 0) {
+            const int32_t e = band_edge(j, q_lo, D, N, C, n_bins);
+            if (e < n_bins && e % Cc != 0 && !(j > 0 && band_edge(j - 1, q_lo, D, N, C, n_bins) == e)) {
+                const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
+                len = min(e - c0, c1 - e);                    // >= 1
+                rank = atomicAdd(&hist[len], 1);
+            }
+        }
+    }
+    __syncthreads();
+    if (tid <= kMaxPieceLen && hist[tid] > 0) base[tid] = atomicAdd(&len_count[tid], hist[tid]);
+    if (tid + 128 <= kMaxPieceLen && hist[tid + 128] > 0) base[tid + 128] = atomicAdd(&len_count[tid + 128], hist[tid + 128]);
+    __syncthreads();
+    if (FILL && len > 0) list[len_start[len] + base[len] + rank] = make_int2((int)p, j);
+}
+
+// exclusive prefix of the length classes, longest first (long pieces start first: shorter tail); zeroes the counts
+__global__ void piece_scan_kernel(int32_t *__restrict__ len_count, int32_t *__restrict__ len_start)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int32_t run = 0;
+    for (int l = kMaxPieceLen; l >= 0; --l) {
+        len_start[l] = run;
+        run += len_count[l];
+        len_count[l] = 0;
+    }
+    len_start[kMaxPieceLen + 1] = run;                        // the number of pieces
+}
+
+__global__ void __launch_bounds__(128) band_ragged_sorted_kernel(const double *__restrict__ table,
+                                                                 const double *__restrict__ coef,
+                                                                 const int32_t *__restrict__ band_lo,
+                                                                 const int32_t *__restrict__ band_hi, int64_t P_pad,
+                                                                 int32_t n_bins, int32_t N, int32_t C, int32_t Cc,
+                                                                 const int32_t *__restrict__ len_start,
+                                                                 const int2 *__restrict__ list,
+                                                                 const __grid_constant__ OrbitCoef orb,
+                                                                 double *__restrict__ rag)
+{
+    const int32_t n_pieces = len_start[kMaxPieceLen + 1];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pieces; i += (int64_t)gridDim.x * blockDim.x) {
+        const int2 pj = list[i];
+        const int64_t p = pj.x;
+        const int32_t q_lo = (band_lo[p] + C / 2) / C, D = (band_hi[p] + C / 2) / C - q_lo;
+        const int32_t e = band_edge(pj.y, q_lo, D, N, C, n_bins);
+        const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
+        const bool left = (e - c0) <= (c1 - e);
+        const int32_t b0 = left ? c0 : e, b1 = left ? e : c1;
+        double c[kNCoef];
+#pragma unroll
+        for (int q = 0; q < kNCoef; ++q) c[q] = coef[(int64_t)q * P_pad + p];
+        double acc[kNAcc];
+#pragma unroll
+        for (int q = 0; q < kNAcc; ++q) acc[q] = 0.0;
+        double2 cur[12], nxt[12];
+        {
+            const double2 *r0 = reinterpret_cast<const double2 *>(table + (int64_t)b0 * kTabW);
+#pragma unroll
+            for (int q = 0; q < 12; ++q) cur[q] = r0[q];
+        }
+#pragma unroll 1
+        for (int k = b0; k < b1; ++k) {
+            {
+                const double2 *rn = reinterpret_cast<const double2 *>(table + (int64_t)min(k + 1, b1 - 1) * kTabW);
+#pragma unroll
+                for (int q = 0; q < 12; ++q) nxt[q] = rn[q];
+            }
+            const double2 dwv = cur[10];
+            double psi, sps, cps, tpr, tpi, tcr, tci;
+            bin_template(cur, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
+            const double qr = fma(dwv.x, cps, -dwv.y * sps);
+            const double qi = fma(dwv.x, sps, dwv.y * cps);
+            acc[0] = fma(qr, tpr, fma(qi, tpi, acc[0]));
+            acc[1] = fma(qi, tpr, fma(-qr, tpi, acc[1]));
+            acc[2] = fma(qr, tcr, fma(qi, tci, acc[2]));
+            acc[3] = fma(qi, tcr, fma(-qr, tci, acc[3]));
+            const double wgt = cur[11].x;
+            acc[4] = fma(wgt, fma(tpr, tpr, tpi * tpi), acc[4]);
+            acc[5] = fma(wgt, fma(tcr, tcr, tci * tci), acc[5]);
+            acc[6] = fma(wgt, fma(tpr, tcr, tpi * tci), acc[6]);
+            acc[7] = fma(wgt, fma(tpi, tcr, -tpr * tci), acc[7]);
+#pragma unroll
+            for (int q = 0; q < 12; ++q) cur[q] = nxt[q];
+        }
+        double *out = rag + ((int64_t)p * (N + 1) + pj.y) * kNAcc;
+#pragma unroll
+        for (int q = 0; q < kNAcc; ++q) out[q] = acc[q];
+    }
+}
+
 // The partitions of the templates from the cell records.  Cell c of the internal plan is its partition c: its
 // records are segments part_seg[c] .. part_seg[c + 1], slot-major or value-major (sk, sp).  Cc = width of the
 // cells; C = lattice of the edge rule.  rag == nullptr: C == Cc, every edge is a cell boundary.  Otherwise an
@@ -406,7 +525,7 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
                                                           const int32_t *__restrict__ band_hi, int64_t P_pad,
                                                           int32_t n_bins, int32_t N, int32_t C, int32_t Cc,
                                                           const __grid_constant__ OrbitCoef orb, double *__restrict__ rag,
-                                                          double *__restrict__ rag_short)
+                                                          double *__restrict__ rag_short, int32_t short_only)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P_pad || valid[p] == 0) return;
@@ -465,6 +584,7 @@ __global__ void __launch_bounds__(128) band_ragged_kernel(const double *__restri
             if (eb > e && ca >= cb) eval_range(e, eb, rag_short + ((int64_t)p * N + j) * kNAcc);
         }
         // (2) the shorter piece of the cell this edge splits (the other piece is the cell's record minus it)
+        if (short_only) continue;                                       // (done by band_ragged_sorted_kernel)
         if (e >= n_bins || e % Cc == 0) continue;                       // a cell boundary: nothing to split
         if (j > 0 && band_edge(j - 1, q_lo, D, N, C, n_bins) == e) continue;   // same edge as the previous one
         const int32_t c0 = (e / Cc) * Cc, c1 = min(c0 + Cc, n_bins);
@@ -489,7 +609,7 @@ __global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict
 
 // rag == nullptr: every edge is a cell boundary (lattice == cell); else the pieces are computed first.
 cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, const double *partial, double *rag,
-                                       double *rag_short, const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
+                                       double *rag_short, int32_t *piece_scratch, int2 *piece_list, const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
                                        const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
                                        int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
                                        int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
@@ -499,9 +619,25 @@ cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, 
     if (rag != nullptr) {
         int gy = n_seg_band + 1;
         if (gy > 2048) gy = 2048;
+        const bool sorted = piece_scratch != nullptr && cell <= 2 * kMaxPieceLen && n_seg_band >= 128 && n_seg_band < 65535;
         band_ragged_kernel<<<dim3((unsigned)(P_pad / 128), (unsigned)gy), 128, 0, st>>>(
-            table, coef, valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, orb, rag, rag_short);
+            table, coef, valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, orb, rag, rag_short, sorted ? 1 : 0);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        if (sorted) {                                         // many pieces: evaluate them in the order of their lengths
+            int32_t *count = piece_scratch, *start = piece_scratch + (kMaxPieceLen + 1);
+            const dim3 grd((unsigned)(P_pad / 128), (unsigned)(n_seg_band + 1));
+            if ((e = cudaMemsetAsync(count, 0, (kMaxPieceLen + 1) * sizeof(int32_t), st)) != cudaSuccess) return e;
+            piece_list_kernel<false><<<grd, 128, 0, st>>>(valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, count,
+                                                          nullptr, nullptr);
+            piece_scan_kernel<<<1, 32, 0, st>>>(count, start);
+            piece_list_kernel<true><<<grd, 128, 0, st>>>(valid, band_lo, band_hi, P_pad, n_bins, n_seg_band, lattice, cell, count,
+                                                         start, piece_list);
+            int64_t nb = (P_pad * (int64_t)(n_seg_band + 1) + 127) / 128;
+            if (nb > 148 * 48) nb = 148 * 48;
+            band_ragged_sorted_kernel<<<(unsigned)nb, 128, 0, st>>>(table, coef, band_lo, band_hi, P_pad, n_bins, n_seg_band,
+                                                                    lattice, cell, start, piece_list, orb, rag);
+            if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        }
     }
     if ((int64_t)n_cells < (int64_t)32 * n_seg_band) {      // a few cells per partition: one thread per partition
         int gy = (n_seg_band + 7) / 8;

@@ -171,7 +171,7 @@ cudaError_t launch_band_epilogue(const double *rec, const int32_t *rec_idx, cons
                                  int64_t P_pad, int32_t n_wseg, int32_t n_seg, double *F, double *Fk, cudaStream_t st);
 cudaError_t band_kernel_configure();
 cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, const double *partial, double *rag,
-                                       double *rag_short, const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
+                                       double *rag_short, int32_t *piece_scratch, int2 *piece_list, const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
                                        const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
                                        int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
                                        int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
