@@ -733,7 +733,8 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
                                               pl->d_perm, pl->d_band, pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins,
                                               pl->n_part, br->n_seg, br->lattice, br->cell, fa.part_sk, fa.part_sp, pl->orb,
                                               F, Fk, br->amp, st));
-        tp->n_launches += rag ? 4 : 3;                 // band limits, [pieces], cells epilogue, F sums
+        const bool sorted = rag && br->cell <= 128 && br->n_seg >= 128 && br->n_seg < 65535;    // as launch_band_cells_epilogue
+        tp->n_launches += (rag ? 4 : 3) + (sorted ? 4 : 0);   // band limits, [pieces [+ list x 2, scan, sorted pieces]], cells epilogue, F sums
         return FSTAT_OK;
     }
     if (F) {
