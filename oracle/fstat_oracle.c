@@ -32,9 +32,14 @@
  * Row f4 (Eq. 3 :62, the sum over TDI combinations with independent noise): fstat_batch_channels in oracle.py adds
  * the N and M of this file's oracle_fstat_batch over the channels; pins in tests/test_oracle_channels.py: P14 the
  * cyclic relabelling behind orbit_lambda + 2 pi/3, brute-force maximisation of Eq. 3, zero-noise network SNR.
- * PARITY UNPINNED (stated in DESIGN.md): the numerical values of alpha_k / phi_e against the
- * authors' code (textbook TaylorF2 values are used, A1/A3) and the paper's absolute SNR values
- * (their PSD file and orbit phase are not available, P10/T8).
+ * The coefficients the paper does not print (alpha_k, phi_e: "details in [85-88]") are pinned by
+ * tests/test_oracle_pn_pins.py against independent statements of that literature: P15 t_f = the 3PN TaylorT2
+ * t(v) of ref. [88]; P16 Psi_0 = 2 pi f t(v) - 2 phi_orb(v) - pi/4 with TaylorT2's two series; P17 the eccentric
+ * term = Peters' time to coalescence (157/43 e^2, e ~ f^(-19/18)); scratch copies of this file with any one of
+ * those constants corrupted fail them.
+ * PARITY UNPINNED (stated in DESIGN.md): only what needs the authors' own code and files -- whether THEIR
+ * alpha_k / phi_e are these textbook ones, and the paper's absolute SNR values (their PSD file and orbit phase
+ * are not available, P10/T8).
  */
 #include <math.h>
 #include <stdint.h>
