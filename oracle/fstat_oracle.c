@@ -404,6 +404,61 @@ int oracle_fstat_batch(int64_t n_bins, const double *freq, const double *dw, con
     return fail ? -1 : 0;
 }
 
+/* The same path for several partition sets over the same data (the hierarchy stages of PAPER.md:168-174 differ
+ * only in N_seg): the templates of a particle are written out ONCE (steps 1-4) and step 5 is repeated per set.
+ * Nothing else differs from oracle_fstat_batch -- same functions, same order of the sums -- so its results are
+ * bit-equal to one oracle_fstat_batch call per set (tests/test_oracle_pins.py checks that).
+ *   n_part[s], s < n_sets; edges = the sets' edge arrays one after the other (n_part[s] + 1 entries each);
+ *   F[s * P + p];  Fk = the sets' [P][n_part[s]] blocks one after the other. */
+int oracle_fstat_batch_multi(int64_t n_bins, const double *freq, const double *dw, const double *isn,
+                             int32_t n_sets, const int32_t *n_part, const int64_t *edges, int64_t P,
+                             const double *params, const oracle_options *opt, int use_ld, int n_threads,
+                             double *F, double *Fk)
+{
+    const double df = (n_bins > 1) ? (freq[n_bins - 1] - freq[0]) / (double)(n_bins - 1) : freq[0];
+    int fail = 0;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#else
+    (void)n_threads;
+#endif
+#pragma omp parallel
+    {
+        double *up = (double *)malloc(sizeof(double) * 2 * (size_t)(n_bins > 0 ? n_bins : 1));
+        double *uc = (double *)malloc(sizeof(double) * 2 * (size_t)(n_bins > 0 ? n_bins : 1));
+        if (!up || !uc) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t p = 0; p < P; ++p) {
+            if (!up || !uc) continue;
+            const double *par = params + 6 * p;
+            const int ok = oracle_params_valid(par);
+            if (ok) oracle_template(par, n_bins, freq, opt, up, uc);
+            const int64_t *e = edges;
+            double *fk = Fk;
+            for (int32_t s = 0; s < n_sets; ++s) {
+                long double tot = 0.0L;
+                for (int j = 0; j < n_part[s]; ++j) {
+                    double N[4], M[16], Fj = -INFINITY;
+                    if (ok) {
+                        oracle_inner_products(dw, isn, up, uc, df, e[j], e[j + 1], use_ld, N, M);
+                        oracle_fstat_from_NM(N, M, &Fj, NULL);
+                        tot += Fj;
+                    }
+                    fk[p * n_part[s] + j] = Fj;
+                }
+                F[(int64_t)s * P + p] = ok ? (double)tot : -INFINITY;
+                e += n_part[s] + 1;
+                fk += P * (int64_t)n_part[s];
+            }
+        }
+        free(up); free(uc);
+    }
+    return fail ? -1 : 0;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

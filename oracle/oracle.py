@@ -76,6 +76,12 @@ def lib():
                                          C.POINTER(C.c_int32)]
         L.oracle_fstat_batch.restype = C.c_int
         L.oracle_max_threads.restype = C.c_int
+        L.oracle_fstat_batch_multi.argtypes = [C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                               C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_int32),
+                                               C.POINTER(C.c_int64), C.c_int64, C.POINTER(C.c_double),
+                                               C.POINTER(Options), C.c_int, C.c_int, C.POINTER(C.c_double),
+                                               C.POINTER(C.c_double)]
+        L.oracle_fstat_batch_multi.restype = C.c_int
         L.oracle_template_band.argtypes = [C.POINTER(C.c_double), C.c_int64, C.POINTER(C.c_double), C.c_double,
                                            C.POINTER(Options), C.POINTER(C.c_int64), C.POINTER(C.c_int64),
                                            C.POINTER(C.c_int)]
@@ -194,6 +200,36 @@ def fstat_batch(freq, dw, inv_sn, edges, params, opt: Optional[Options] = None, 
     if want_NM:
         return F, Fk, NM, flags
     return F, Fk
+
+
+def fstat_batch_multi(freq, dw, inv_sn, edge_sets, params, opt: Optional[Options] = None, use_ld: bool = False,
+                      n_threads: int = 0):
+    """[(F[P], Fk[P][n_part_s]) for every edge set]: ``fstat_batch`` for several partition sets over the same data,
+    with each particle's templates written out once (bit-equal to one ``fstat_batch`` call per set)."""
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    dw = np.ascontiguousarray(dw, dtype=np.complex128)
+    inv_sn = np.ascontiguousarray(inv_sn, dtype=np.float64)
+    params = _par(params).reshape(-1, 6)
+    sets = [np.ascontiguousarray(e, dtype=np.int64) for e in edge_sets]
+    n = freq.shape[0]
+    for e in sets:
+        assert e[0] == 0 and e[-1] == n and np.all(np.diff(e) > 0)
+    P = params.shape[0]
+    n_part = np.array([e.shape[0] - 1 for e in sets], dtype=np.int32)
+    edges = np.concatenate(sets)
+    F = np.zeros((len(sets), P))
+    Fk = np.zeros(P * int(n_part.sum()))
+    rc = lib().oracle_fstat_batch_multi(n, _dp(freq), dw.ctypes.data_as(C.POINTER(C.c_double)), _dp(inv_sn),
+                                        len(sets), n_part.ctypes.data_as(C.POINTER(C.c_int32)),
+                                        edges.ctypes.data_as(C.POINTER(C.c_int64)), P, _dp(params),
+                                        C.byref(_opt(opt)), int(use_ld), int(n_threads), _dp(F), _dp(Fk))
+    if rc != 0:
+        raise MemoryError("oracle_fstat_batch_multi: allocation failed")
+    out, off = [], 0
+    for s, k in enumerate(n_part):
+        out.append((F[s].copy(), Fk[off:off + P * int(k)].reshape(P, int(k)).copy()))
+        off += P * int(k)
+    return out
 
 
 def template_band(par, freq, T_obs: float, opt: Optional[Options] = None) -> Tuple[int, int]:

@@ -143,6 +143,21 @@ def _wide_particles(rng, P: int, T: float) -> np.ndarray:
     return np.stack([tc, mc, eta, np.arccos(ct), phi, e0], axis=1)
 
 
+def paper_range_particles(P: int, seed: int = 105) -> np.ndarray:
+    """[P][6] particles uniform over the PAPER's own search ranges (PAPER.md:249-256 Table I, :313-325 Table III):
+    t_c 3.3-3.8 yr, M_c 20-80 Msun, delta_mu 0-0.9 (eta = (1 - delta_mu^2)/4, reading A18), theta 0-pi, phi 0-2pi,
+    e0 0-0.05.  BASELINE.json's configs use narrower masses and a wider t_c / e0 (reading A22); this population
+    checks the stride selection where the paper itself searches."""
+    rng = np.random.default_rng(seed)
+    tc = rng.uniform(3.3 * YEAR_S, 3.8 * YEAR_S, P)
+    mc = rng.uniform(20.0, 80.0, P)
+    dmu = rng.uniform(0.0, 0.9, P)
+    th = rng.uniform(0.0, np.pi, P)
+    phi = rng.uniform(0.0, 2.0 * np.pi, P)
+    e0 = rng.uniform(0.0, 0.05, P)
+    return np.stack([tc, mc, 0.25 * (1.0 - dmu * dmu), th, phi, e0], axis=1)
+
+
 def draw_particles(cfg: Config, P: Optional[int] = None) -> np.ndarray:
     """[P][6] float64 intrinsic parameters (tc, Mc, eta, theta, phi, e0) of config ``cfg``."""
     P = int(cfg.P[0] if P is None else P)

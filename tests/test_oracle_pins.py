@@ -152,6 +152,21 @@ def test_p4_np1_is_the_coherent_statistic_and_sums_add(orc, tiny):
     assert np.all(Fk7.sum(1) >= F1 - 1e-9)
 
 
+def test_p4b_several_partition_sets_in_one_pass_are_bit_equal(orc, tiny):
+    """`fstat_batch_multi` (templates written once, step 5 per partition set: what the full-size parity runs use)
+    returns exactly what one `fstat_batch` call per set returns, invalid particles included."""
+    ds = tiny
+    par = syn.draw_particles(ds.cfg)[:6].copy()
+    par[2, 2] = 0.3
+    sets = [ds.edges(1), ds.edges(4), ds.edges(16), np.array([0, 1, 3, 700, ds.n_bins])]
+    multi = orc.fstat_batch_multi(ds.freq, ds.dw, ds.inv_sn, sets, par)
+    for (F, Fk), e in zip(multi, sets):
+        F1, Fk1 = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, e, par)
+        np.testing.assert_array_equal(F, F1)
+        np.testing.assert_array_equal(Fk, Fk1)
+    assert np.isneginf(multi[1][0][2]) and np.all(np.isneginf(multi[1][1][2]))
+
+
 def test_p5_hermitian_closed_form_equals_4x4_solve(orc, tiny):
     """The 8-sum 2x2 Hermitian form the GPU epilogue uses equals the oracle's 4x4 Cholesky."""
     ds = tiny
