@@ -34,22 +34,66 @@ METRIC = "template_frequency_bins_per_s"
 UNIT = "template-bins/s"
 
 # FP64-pipe instructions (DFMA + DMUL + DADD + DSETP) of the two main kernels, per unit of work (DESIGN.md
-# "Roofline").  Per template-bin: SASS count of the per-bin loops, re-counted by tests/test_cabi.py.  Per node
-# interval and per work item: EXECUTED counts measured with ncu (sm__inst_executed_pipe_fp64.sum at forced
-# strides 8 / 512 and two segment lengths, profiles/r1_v6.md: 19 / 736 / 1105 (+ 17 per segment, neglected) reproduce all three totals exactly;
-# "work item" = one run of consecutive segments walked by one CTA).
-#   interpolating kernel: per template-bin (inner loop), per node interval of a particle (full-model node
-#   evaluation, interpolation coefficients, Gram products), per work item of a particle (three extra nodes);
-#   direct kernel: per template-bin.  2 flop each by the usual FMA convention.
+# "Roofline").  The numerator of the roofline is an EXECUTED-INSTRUCTION model, not a flop count:
+#   per template-bin of the interpolating kernel and of the direct kernel: counted in the SASS of the library that
+#       is loaded, at run time (sass_fp64_mix below; the constants here are only the fallback when cuobjdump is
+#       missing, and tests/test_cabi.py checks them against the SASS);
+#   per node interval and per work item of a particle: EXECUTED counts measured with ncu
+#       (sm__inst_executed_pipe_fp64.sum at forced strides 8 / 512 and two segment lengths; profiles/ names the build).
 FAST_FP64_PER_BIN = 19.0
 FAST_FP64_PER_INTERVAL = 736.0
 FAST_FP64_PER_ITEM = 1105.0
 DIRECT_FP64_PER_BIN = 263.0
-NOMINAL_FP64_TFLOPS = 148 * 64 * 1.965e9 * 2 / 1e12
+FP64_COUNTS_BUILD = "per node interval / per work item: ncu executed counts of round-1 build c21f730 (profiles/r1_v6.md)"
+NOMINAL_FP64_INST_PER_S = 148 * 64 * 1.965e9        # 148 SMs x 64 FP64 lanes x 1.965 GHz (B200_PROFILING.md)
 STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel
-# dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from
-# the ncu --set full capture summarised in profiles/ (None until that capture exists for the current kernel)
-NCU_DRAM_BYTES_PER_LAUNCH = 223.5e6     # profiles/r1_v6.md: 31.8 MB read + 191.7 MB written (config 1)
+# dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from the
+# ncu --set full capture named beside it (None when no capture of the current hot kernel exists)
+NCU_DRAM_BYTES_PER_LAUNCH = 223.5e6
+NCU_DRAM_CAPTURE = "profiles/r1_v6.md (31.8 MB read + 191.7 MB written), build c21f730"
+
+
+def sass_fp64_mix(lib_path):
+    """FP64-pipe instruction mix of the per-bin loop of fstat_fast_kernel, from `cuobjdump -sass` of the loaded
+    library: {"per_bin": FP64 instructions per bin, "dfma", "dadd", "dmul", "dsetp": each per bin, "all_per_bin":
+    instructions of every pipe per bin}.  None when cuobjdump is unavailable.  The per-bin loop is the innermost
+    loop that reads the folded data from shared memory (LDS) and holds >= 10 FP64 instructions."""
+    import re
+    try:
+        out = subprocess.run(["cuobjdump", "-sass", lib_path], capture_output=True, text=True, check=True).stdout
+    except (OSError, subprocess.CalledProcessError):
+        return None
+    m = re.search(r"Function : \S*fstat_fast_kernel", out)
+    if not m:
+        return None
+    j = out.find("Function :", m.end())
+    ins = []
+    for line in out[m.start():j if j > 0 else None].splitlines():
+        mm = re.search(r"/\*([0-9a-f]{4,5})\*/\s+(.*?);", line)
+        if mm:
+            w = mm.group(2).split()
+            op = w[1] if w[0].startswith("@") else w[0]
+            ins.append((int(mm.group(1), 16), op.split(".")[0], mm.group(2)))
+    loops = []
+    for a, op, text in ins:
+        if op == "BRA":
+            t = re.search(r"(0x[0-9a-f]+)\s*$", text)
+            if t and int(t.group(1), 16) < a:
+                loops.append((int(t.group(1), 16), a))
+    best = None
+    for lo, hi in loops:
+        if any(lo <= l2 and h2 <= hi and (l2, h2) != (lo, hi) for l2, h2 in loops):
+            continue
+        body = [op for a, op, _ in ins if lo <= a <= hi]
+        n_lds = body.count("LDS")
+        n64 = sum(body.count(o) for o in ("DFMA", "DADD", "DMUL", "DSETP"))
+        if n_lds >= 2 and n64 >= 10 * n_lds:                 # the unrolled 4-bin runs (one LDS.128 per bin)
+            cand = {"per_bin": n64 / n_lds, "dfma": body.count("DFMA") / n_lds, "dadd": body.count("DADD") / n_lds,
+                    "dmul": body.count("DMUL") / n_lds, "dsetp": body.count("DSETP") / n_lds,
+                    "all_per_bin": len(body) / n_lds}
+            if best is None or n_lds > best[0]:
+                best = (n_lds, cand)
+    return best[1] if best else None
 
 
 # ------------------------------------------------------------------------------------------ utilities
@@ -132,6 +176,7 @@ def parse_args():
     ap.add_argument("--channels", type=int, default=0, metavar="N",
                     help="also time fstat_eval_batch_channels (row f4: N TDI channels X, Y, Z with common amplitudes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the N_p sweep rows the default workload adds to the line")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
     return ap.parse_args()
 
@@ -216,6 +261,75 @@ def run_reference(args):
            "gpu_launches": 0}
     print(json.dumps(out))
     return 0
+
+
+def fp64_model(fs, plan, P, n_bins, mix):
+    """Executed FP64-pipe thread-instructions of the main kernels for the most recent evaluation on `plan` (P particles):
+    per-bin x bins at each stride + per-interval x node intervals + per-item x CTA runs + direct bins, summed over the
+    particle groups (fstat_plan_level_bins), x 128 particles per group."""
+    lvl_bins, lvl_sub = fs.fstat_plan_level_bins(plan)
+    n_items = fs.fstat_plan_n_ctas(plan, P)
+    per_bin = mix["per_bin"] if mix else FAST_FP64_PER_BIN
+    fast_share = float(lvl_bins[1:].sum()) / max(float(lvl_bins.sum()), 1.0)
+    inst = 128.0 * (per_bin * float(lvl_bins[1:].sum()) + FAST_FP64_PER_INTERVAL * float(lvl_sub.sum())
+                    + FAST_FP64_PER_ITEM * n_items * fast_share + DIRECT_FP64_PER_BIN * float(lvl_bins[0]))
+    # flops with DFMA = 2, DADD = DMUL = 1, DSETP = 0: the per-bin mix from the SASS for the per-bin part; the rest of
+    # the kernel (node evaluations, coefficients, Gram products) is FMA chains almost throughout: counted as the
+    # per-bin mix too (an under-estimate of its flops)
+    flop_per_inst = ((2.0 * mix["dfma"] + mix["dadd"] + mix["dmul"]) / mix["per_bin"]) if mix else 27.5 / 19.0
+    share = {str(S): float(b) / max(float(lvl_bins.sum()), 1.0) for S, b in zip(STRIDES, lvl_bins)}
+    return inst, inst * flop_per_inst, share, float(lvl_sub.sum()), n_items
+
+
+def timed_steps(fs, torch, plan, par, F, Fk, stream, scratch, steps, warmup):
+    """W warm-up evaluations, then `steps` evaluations each bracketed by its own CUDA event pair on the launch stream,
+    L2 flushed (256 MiB write, not timed) before each.  Returns (mean ms per step, mean ms of the main kernels)."""
+    for _ in range(warmup):
+        fs.fstat_eval_batch(plan, par, F, Fk, stream)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for e0, e1 in ev:
+        scratch.fill_(5)
+        e0.record(stream)
+        fs.fstat_eval_batch(plan, par, F, Fk, stream)
+        e1.record(stream)
+    torch.cuda.synchronize()
+    ms = float(np.mean([e0.elapsed_time(e1) for e0, e1 in ev]))
+    main_ms = fs.fstat_plan_main_kernel_ms(plan, min(steps, 128))
+    return ms, (float(np.mean(main_ms)) if len(main_ms) else float("nan"))
+
+
+def run_sweep(fs, torch, plan1, ds1, args, mix, fp64_rate, stream, scratch):
+    """north_star's "2.5-year N_p sweep" in the driver-run line: configs 2 (P = 8192; N_p = 256, 64, 16) and 3 (P = 4096,
+    N_p = 1) on config 1's data through fstat_plan_set_partitions, and one wide-band point (config 4, P = 4096,
+    N_p = 16).  Same timing rules as the headline step, fewer steps."""
+    rows = []
+    steps, warm = max(min(args.steps, 8), 3), 3
+
+    def point(cfg, ds, plan, n_part, P):
+        par = torch.as_tensor(np.ascontiguousarray(syn.draw_particles(cfg, P)), device="cuda")
+        F = torch.empty(P, dtype=torch.float64, device="cuda")
+        Fk = torch.empty((P, n_part), dtype=torch.float64, device="cuda")
+        ms, main_ms = timed_steps(fs, torch, plan, par, F, Fk, stream, scratch, steps, warm)
+        inst, _, share, _, _ = fp64_model(fs, plan, P, ds.n_bins, mix)
+        rows.append({"workload": cfg.name, "n_bins": ds.n_bins, "n_part": n_part, "particles": P, "steps": steps,
+                     "ms_per_step": ms, "value": float(P) * ds.n_bins / (ms * 1e-3), "unit": UNIT,
+                     "particles_per_s": float(P) / (ms * 1e-3), "main_kernel_ms": main_ms,
+                     "fp64_inst_per_template_bin": inst / (float(P) * ds.n_bins),
+                     "frac": inst / (main_ms * 1e-3) / fp64_rate if fp64_rate > 0 else None,
+                     "frac_of_nominal": inst / (main_ms * 1e-3) / NOMINAL_FP64_INST_PER_S,
+                     "direct_kernel_share_of_bins": share["0"]})
+
+    cfg2, cfg3, cfg4 = syn.CONFIGS[2], syn.CONFIGS[3], syn.CONFIGS[4]
+    for n_part in cfg2.n_part:
+        fs.fstat_plan_set_partitions(plan1, ds1.edges(n_part))
+        point(cfg2, ds1, plan1, n_part, cfg2.P[0])
+    fs.fstat_plan_set_partitions(plan1, ds1.edges(1))
+    point(cfg3, ds1, plan1, 1, cfg3.P[0])
+    ds4 = syn.make_dataset(cfg4, gpu_template_fn(fs, cfg4))
+    with fs.fstat_plan_create(ds4.freq, ds4.dw, ds4.inv_sn, ds4.edges(16)) as plan4:
+        point(cfg4, ds4, plan4, 16, 4096)
+    return rows
 
 
 def run_ours(args):
@@ -323,33 +437,41 @@ def run_ours(args):
 
     # ---- roofline of the dominant (main) kernels: FP64 pipe
     main_mean = float(np.mean(main_ms)) if len(main_ms) else float("nan")
-    lvl_bins, lvl_sub = fs.fstat_plan_level_bins(plan)           # per particle group: bins / node intervals per stride
-    n_items = fs.fstat_plan_n_ctas(plan, P)
-    fast_share = float(lvl_bins[1:].sum()) / max(float(lvl_bins.sum()), 1.0)
-    fp64_inst = 128.0 * (FAST_FP64_PER_BIN * float(lvl_bins[1:].sum()) + FAST_FP64_PER_INTERVAL * float(lvl_sub.sum())
-                         + FAST_FP64_PER_ITEM * n_items * fast_share + DIRECT_FP64_PER_BIN * float(lvl_bins[0]))
+    mix = sass_fp64_mix(fs.library_path())
+    fp64_inst, fp64_flop, stride_share, n_intervals, n_items = fp64_model(fs, plan, P, ds.n_bins, mix)
     fp64_rate, n_sm = fs.fstat_probe_pipe_peak(0, 60.0, local)
     fp32_rate, _ = fs.fstat_probe_pipe_peak(1, 30.0, local)
     mufu_rate, _ = fs.fstat_probe_pipe_peak(2, 30.0, local)
-    achieved = fp64_inst * 2.0 / (main_mean * 1e-3) / 1e12
-    peak = fp64_rate * 2.0 / 1e12
+    achieved = fp64_inst / (main_mean * 1e-3)                 # FP64-pipe thread-instructions per second
     hbm_peak, hbm_src = peaks()
     n_groups = (P + 127) // 128
     # algorithmic HBM bytes of one launch: every particle group streams the folded data (16 B/bin) once, reads
     # one 192-B node row and one 80-B Gram matrix per node interval, and writes one 80-B record of partial sums per
     # particle and segment (counted here per CTA run: a lower bound when a run holds several segments)
-    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * float(lvl_sub.sum()) + 80.0 * 128.0 * n_items
+    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * n_intervals + 80.0 * 128.0 * n_items
+    default_wl = cfg.name == "first_stage" and n_part == 1024 and P == 2048
     roofline = {"bound": "alu", "kernel": "fstat_fast_kernel (+ fstat_main_kernel for the work items it leaves)",
-                "pipe": "fp64", "achieved": achieved, "peak": peak,
-                "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (cfg.name == "first_stage" and n_part == 1024 and P == 2048) else None,
-                "peak_source": "dependent-free DFMA stream measured in this run (fstat_probe_pipe_peak), x2 flop",
-                "nominal_peak": NOMINAL_FP64_TFLOPS, "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                "pipe": "fp64",
+                "achieved": achieved / 1e12, "peak": fp64_rate / 1e12, "unit": "T FP64-pipe inst/s",
+                "frac": achieved / fp64_rate if fp64_rate > 0 else None,
+                "frac_is": "executed FP64-pipe instructions (DFMA, DADD, DMUL, DSETP: one issue slot each) per second / the "
+                           "builder-measured dependent-free DFMA stream of this run (fstat_probe_pipe_peak); a pipe-slot "
+                           "utilisation, not a flop rate",
+                "nominal_peak": NOMINAL_FP64_INST_PER_S / 1e12, "frac_of_nominal": achieved / NOMINAL_FP64_INST_PER_S,
+                "flop_tflops": fp64_flop / (main_mean * 1e-3) / 1e12,
+                "flop_frac": fp64_flop / (main_mean * 1e-3) / (2.0 * fp64_rate) if fp64_rate > 0 else None,
+                "flop_frac_is": "flops with DFMA = 2, DADD = DMUL = 1 (mix of the per-bin loop from the SASS) / (2 x the DFMA rate)",
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if default_wl else None,
+                "traffic_source": NCU_DRAM_CAPTURE if default_wl else None,
                 "fp64_inst_per_launch": fp64_inst, "fp64_inst_per_template_bin": fp64_inst / (float(P) * ds.n_bins),
-                "fp64_inst_model": {"fast_per_bin": FAST_FP64_PER_BIN, "fast_per_node_interval": FAST_FP64_PER_INTERVAL,
-                                    "fast_per_work_item": FAST_FP64_PER_ITEM, "direct_per_bin": DIRECT_FP64_PER_BIN},
-                "stride_share_of_bins": {str(S): float(b) / max(float(lvl_bins.sum()), 1.0)
-                                         for S, b in zip(STRIDES, lvl_bins)},
+                "fp64_inst_model": {"fast_per_bin": mix["per_bin"] if mix else FAST_FP64_PER_BIN,
+                                    "fast_per_bin_source": "SASS of the loaded library (cuobjdump) at run time" if mix
+                                                           else "constant in bench.py (cuobjdump unavailable)",
+                                    "fast_per_bin_mix": mix,
+                                    "fast_per_node_interval": FAST_FP64_PER_INTERVAL,
+                                    "fast_per_work_item": FAST_FP64_PER_ITEM, "direct_per_bin": DIRECT_FP64_PER_BIN,
+                                    "source": FP64_COUNTS_BUILD},
+                "stride_share_of_bins": stride_share,
                 "main_kernel_ms": main_mean, "main_kernel_share_of_step": main_mean / ms_step,
                 "measured_pipe_peaks_inst_per_s": {"fp64_fma": fp64_rate, "fp32_fma": fp32_rate, "mufu": mufu_rate},
                 "hbm": {"algorithmic_bytes_per_launch": hbm_bytes,
@@ -374,6 +496,9 @@ def run_ours(args):
                    "call": "fstat_eval_batch_host (pinned host params in; F and F_k out)"},
            "gpu_launches": int(launches_timed),
            "clocks": clk, "roofline": roofline}
+    if default_wl and world == 1 and not args.no_sweep:
+        out["sweep"] = run_sweep(fs, torch, plan, ds, args, mix, fp64_rate, stream, scratch)
+        fs.fstat_plan_set_partitions(plan, edges)
     if args.pso > 0:
         # row f1: ITERS iterations of the device PSO (update -> fstat_eval_batch -> personal bests) enqueued back to
         # back on the stream, no host synchronisation in between; box = the particle ranges of the workload

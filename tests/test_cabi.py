@@ -160,3 +160,8 @@ def test_bench_fp64_instruction_model_matches_the_sass(fs):
     assert direct["per_bin"] == bench.DIRECT_FP64_PER_BIN
     # the per-bin loop of the interpolating kernel is almost pure FP64: the pipe that bounds it
     assert bench.FAST_FP64_PER_BIN / fast["per_bin_all_pipes"] > 0.8
+    # what bench.py itself reads from the SASS at run time (its constants are only the fallback)
+    mix = bench.sass_fp64_mix(fs.library_path())
+    assert mix is not None and mix["per_bin"] == bench.FAST_FP64_PER_BIN
+    assert mix["dfma"] + mix["dadd"] + mix["dmul"] + mix["dsetp"] == pytest.approx(mix["per_bin"])
+    assert mix["dfma"] >= 8.0 and mix["all_per_bin"] < 23.0
