@@ -43,7 +43,7 @@ UNIT = "template-bins/s"
 FAST_FP64_PER_BIN = 19.0
 FAST_FP64_PER_INTERVAL = 736.0
 FAST_FP64_PER_ITEM = 1105.0
-DIRECT_FP64_PER_BIN = 263.0
+DIRECT_FP64_PER_BIN = 267.0
 FP64_COUNTS_BUILD = "per node interval / per work item: ncu executed counts of round-1 build c21f730 (profiles/r1_v6.md)"
 NOMINAL_FP64_INST_PER_S = 148 * 64 * 1.965e9        # 148 SMs x 64 FP64 lanes x 1.965 GHz (B200_PROFILING.md)
 STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel

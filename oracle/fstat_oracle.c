@@ -253,7 +253,8 @@ void oracle_template_band(const double *par, int64_t n, const double *freq, doub
 /* N^i = <d, A^i>, M^ij = <A^i, A^j> over bins [lo, hi) by direct summation (Eq. 4, 8, 9, 12):
  *   <a, b> = 4 df Re sum a_k conj(b_k) / S_n(f_k), with dw = d / S_n and isn = 1 / S_n given.
  * A^1 = u_+, A^2 = u_x, A^3 = i u_+, A^4 = i u_x.  use_ld != 0 accumulates in long double
- * (hazard H3: near-singular M in narrow partitions); otherwise Neumaier-compensated double. */
+ * (hazard H3: near-singular M in narrow partitions); otherwise Neumaier-compensated double.  Either way N and M
+ * come back as doubles; oracle_fstat_partition(mode 2) is the variant that never rounds them. */
 void oracle_inner_products(const double *dw, const double *isn, const double *u_plus, const double *u_cross,
                            double df, int64_t lo, int64_t hi, int use_ld, double N[4], double M[16])
 {
@@ -287,6 +288,36 @@ void oracle_inner_products(const double *dw, const double *isn, const double *u_
     }
 }
 
+/* The same sums kept in long double (x86-64: 64-bit mantissa) all the way to the solve: "use_ld == 2" of the batch
+ * calls.  Why (hazard H3, SURVEY section 7 H3(iii) "give the oracle a long double accumulation/epilogue switch to
+ * establish truth"): over a narrow partition u_x is nearly a complex multiple of u_+ and the normalised determinant
+ * 1 - |m_pc|^2 / (m_pp m_cc) of M falls to 3e-12 on config 4 (N_p = 1024 near 100 mHz, t_f moves 0.35 s per bin).
+ * Rounding N and M to double (1e-16) before the solve then costs 1e-16 / det = 3e-5 of F_k -- more than the 1e-5
+ * parity bar -- although every step before and after is exact enough.  Same definition (Eq. 4, 8, 9, 12), same
+ * order of the sums, no rounding to double in between. */
+static void orc_inner_products_ld(const double *dw, const double *isn, const double *u_plus, const double *u_cross,
+                                  double df, int64_t lo, int64_t hi, long double N[4], long double M[16])
+{
+    long double sN[4] = {0, 0, 0, 0}, sM[4][4];
+    memset(sM, 0, sizeof sM);
+    for (int64_t k = lo; k < hi; ++k) {
+        long double Ar[4], Ai[4];
+        Ar[0] = u_plus[2 * k];       Ai[0] = u_plus[2 * k + 1];
+        Ar[1] = u_cross[2 * k];      Ai[1] = u_cross[2 * k + 1];
+        Ar[2] = -u_plus[2 * k + 1];  Ai[2] = u_plus[2 * k];          /* i u_+ */
+        Ar[3] = -u_cross[2 * k + 1]; Ai[3] = u_cross[2 * k];         /* i u_x */
+        const long double dr = dw[2 * k], di = dw[2 * k + 1], w = isn[k];
+        for (int i = 0; i < 4; ++i) {
+            sN[i] += dr * Ar[i] + di * Ai[i];                        /* Re dw conj(A^i) */
+            for (int j = i; j < 4; ++j) sM[i][j] += (Ar[i] * Ar[j] + Ai[i] * Ai[j]) * w;
+        }
+    }
+    for (int i = 0; i < 4; ++i) {
+        N[i] = 4.0L * df * sN[i];
+        for (int j = i; j < 4; ++j) { M[4 * i + j] = 4.0L * df * sM[i][j]; M[4 * j + i] = M[4 * i + j]; }
+    }
+}
+
 /* Symmetric 4x4 eigen-decomposition by cyclic Jacobi (only used for a singular M). */
 static void orc_jacobi4(double A[4][4], double Q[4][4], double lam[4])
 {
@@ -310,19 +341,20 @@ static void orc_jacobi4(double A[4][4], double Q[4][4], double lam[4])
 /* F = max_a [a.N - a^T M a / 2] = N^T M^-1 N / 2 (Eq. 7): Cholesky solve of M a = N in long double.
  * If M is singular (a template vanishes or the four are linearly dependent on the partition, e.g. a
  * one-bin partition; reading A15) the maximum is N^T M^+ N / 2 with the pseudo-inverse, N being in the
- * range of the Gram matrix M.  Returns 0 (regular) or 1 (singular branch); a[] may be NULL. */
-int oracle_fstat_from_NM(const double N[4], const double M[16], double *F, double a_out[4])
+ * range of the Gram matrix M.  Returns 0 (regular) or 1 (singular branch); a[] may be NULL.
+ * The arithmetic is written once, for long double N and M; oracle_fstat_from_NM feeds it doubles. */
+static int orc_fstat_from_NM_ld(const long double N[4], const long double M[16], double *F, double a_out[4])
 {
     double s[4];
     int zero = 0;
-    for (int i = 0; i < 4; ++i) { if (M[5 * i] > 0.0) s[i] = 1.0 / sqrt(M[5 * i]); else { s[i] = 0.0; zero = 1; } }
+    for (int i = 0; i < 4; ++i) { if (M[5 * i] > 0.0L) s[i] = 1.0 / sqrt((double)M[5 * i]); else { s[i] = 0.0; zero = 1; } }
     long double C[4][4], y[4], a[4];
     int singular = zero;
     if (!singular) {
         /* Cholesky of the unit-diagonal scaled matrix S M S */
         for (int i = 0; i < 4 && !singular; ++i) {
             for (int j = 0; j <= i; ++j) {
-                long double acc = (long double)M[4 * i + j] * s[i] * s[j];
+                long double acc = M[4 * i + j] * s[i] * s[j];
                 for (int k = 0; k < j; ++k) acc -= C[i][k] * C[j][k];
                 if (i == j) { if (acc <= 1e-13L) { singular = 1; break; } C[i][i] = sqrtl(acc); }
                 else C[i][j] = acc / C[j][j];
@@ -330,28 +362,57 @@ int oracle_fstat_from_NM(const double N[4], const double M[16], double *F, doubl
         }
     }
     if (!singular) {
-        for (int i = 0; i < 4; ++i) { long double acc = (long double)N[i] * s[i]; for (int k = 0; k < i; ++k) acc -= C[i][k] * y[k]; y[i] = acc / C[i][i]; }
+        for (int i = 0; i < 4; ++i) { long double acc = N[i] * s[i]; for (int k = 0; k < i; ++k) acc -= C[i][k] * y[k]; y[i] = acc / C[i][i]; }
         for (int i = 3; i >= 0; --i) { long double acc = y[i]; for (int k = i + 1; k < 4; ++k) acc -= C[k][i] * a[k]; a[i] = acc / C[i][i]; }
         long double f = 0.0L;
-        for (int i = 0; i < 4; ++i) f += (long double)N[i] * s[i] * a[i];
+        for (int i = 0; i < 4; ++i) f += N[i] * s[i] * a[i];
         *F = (double)(0.5L * f);
         if (a_out) for (int i = 0; i < 4; ++i) a_out[i] = (double)(a[i] * s[i]);
         return 0;
     }
     double A[4][4], Q[4][4], lam[4], lmax = 0.0, f = 0.0, coef[4] = {0, 0, 0, 0};
-    for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) A[i][j] = M[4 * i + j] * s[i] * s[j];
+    for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) A[i][j] = (double)M[4 * i + j] * s[i] * s[j];
     orc_jacobi4(A, Q, lam);
     for (int i = 0; i < 4; ++i) if (lam[i] > lmax) lmax = lam[i];
     for (int i = 0; i < 4; ++i) {
         if (!(lam[i] > 1e-12 * lmax) || lmax <= 0.0) continue;
         double proj = 0.0;
-        for (int k = 0; k < 4; ++k) proj += Q[k][i] * N[k] * s[k];
+        for (int k = 0; k < 4; ++k) proj += Q[k][i] * (double)N[k] * s[k];
         f += proj * proj / lam[i];
         for (int k = 0; k < 4; ++k) coef[k] += Q[k][i] * proj / lam[i];
     }
     *F = 0.5 * f;
     if (a_out) for (int i = 0; i < 4; ++i) a_out[i] = coef[i] * s[i];
     return 1;
+}
+
+int oracle_fstat_from_NM(const double N[4], const double M[16], double *F, double a_out[4])
+{
+    long double Nl[4], Ml[16];
+    for (int i = 0; i < 4; ++i) Nl[i] = N[i];
+    for (int i = 0; i < 16; ++i) Ml[i] = M[i];
+    return orc_fstat_from_NM_ld(Nl, Ml, F, a_out);
+}
+
+/* Steps 5 of the header for one partition [lo, hi) of given templates.  mode 0: compensated double sums; 1: long
+ * double sums rounded to double; 2: long double sums handed to the solve unrounded (see orc_inner_products_ld).
+ * N_out[4], M_out[16] (may be NULL) receive the sums as doubles; a_out[4] (may be NULL) the amplitudes. */
+int oracle_fstat_partition(const double *dw, const double *isn, const double *u_plus, const double *u_cross,
+                           double df, int64_t lo, int64_t hi, int mode, double *F, double *N_out, double *M_out,
+                           double *a_out)
+{
+    if (mode == 2) {
+        long double Nl[4], Ml[16];
+        orc_inner_products_ld(dw, isn, u_plus, u_cross, df, lo, hi, Nl, Ml);
+        if (N_out) for (int i = 0; i < 4; ++i) N_out[i] = (double)Nl[i];
+        if (M_out) for (int i = 0; i < 16; ++i) M_out[i] = (double)Ml[i];
+        return orc_fstat_from_NM_ld(Nl, Ml, F, a_out);
+    }
+    double N[4], M[16];
+    oracle_inner_products(dw, isn, u_plus, u_cross, df, lo, hi, mode, N, M);
+    if (N_out) memcpy(N_out, N, sizeof N);
+    if (M_out) memcpy(M_out, M, sizeof M);
+    return oracle_fstat_from_NM(N, M, F, a_out);
 }
 
 /* Whole path for P particles: F[P], Fk[P][n_part] (may be NULL), optional N/M dump NM[P][n_part][20]
@@ -390,8 +451,7 @@ int oracle_fstat_batch(int64_t n_bins, const double *freq, const double *dw, con
             long double tot = 0.0L;
             for (int j = 0; j < n_part; ++j) {
                 double N[4], M[16], Fj;
-                oracle_inner_products(dw, isn, up, uc, df, edges[j], edges[j + 1], use_ld, N, M);
-                const int sing = oracle_fstat_from_NM(N, M, &Fj, NULL);
+                const int sing = oracle_fstat_partition(dw, isn, up, uc, df, edges[j], edges[j + 1], use_ld, &Fj, N, M, NULL);
                 if (Fk) Fk[p * n_part + j] = Fj;
                 if (flags) flags[p * n_part + j] = sing;
                 if (NM) { double *o = NM + ((size_t)p * n_part + j) * 20; memcpy(o, N, 4 * sizeof(double)); memcpy(o + 4, M, 16 * sizeof(double)); }
@@ -443,8 +503,7 @@ int oracle_fstat_batch_multi(int64_t n_bins, const double *freq, const double *d
                 for (int j = 0; j < n_part[s]; ++j) {
                     double N[4], M[16], Fj = -INFINITY;
                     if (ok) {
-                        oracle_inner_products(dw, isn, up, uc, df, e[j], e[j + 1], use_ld, N, M);
-                        oracle_fstat_from_NM(N, M, &Fj, NULL);
+                        oracle_fstat_partition(dw, isn, up, uc, df, e[j], e[j + 1], use_ld, &Fj, N, M, NULL);
                         tot += Fj;
                     }
                     fk[p * n_part[s] + j] = Fj;

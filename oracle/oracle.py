@@ -76,6 +76,10 @@ def lib():
                                          C.POINTER(C.c_int32)]
         L.oracle_fstat_batch.restype = C.c_int
         L.oracle_max_threads.restype = C.c_int
+        L.oracle_fstat_partition.argtypes = [C.POINTER(C.c_double)] * 4 + [C.c_double, C.c_int64, C.c_int64, C.c_int,
+                                             C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                             C.POINTER(C.c_double)]
+        L.oracle_fstat_partition.restype = C.c_int
         L.oracle_fstat_batch_multi.argtypes = [C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                                C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_int32),
                                                C.POINTER(C.c_int64), C.c_int64, C.POINTER(C.c_double),
@@ -174,6 +178,22 @@ def fstat_from_NM(N, M):
     F = C.c_double()
     a = np.zeros(4)
     flag = lib().oracle_fstat_from_NM(_dp(N), _dp(M), C.byref(F), _dp(a))
+    return F.value, a, int(flag)
+
+
+def fstat_partition(dw, inv_sn, u_plus, u_cross, df: float, lo: int, hi: int, mode: int = 0):
+    """(F, a[4], singular_flag) of one partition [lo, hi) of given templates.  mode 0: compensated double sums,
+    1: long-double sums rounded to double, 2: long-double sums handed to the solve unrounded (the reference for
+    near-singular M, hazard H3)."""
+    dw = np.ascontiguousarray(dw, dtype=np.complex128)
+    inv_sn = np.ascontiguousarray(inv_sn, dtype=np.float64)
+    u_plus = np.ascontiguousarray(u_plus, dtype=np.complex128)
+    u_cross = np.ascontiguousarray(u_cross, dtype=np.complex128)
+    cd = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    F = C.c_double()
+    a = np.zeros(4)
+    flag = lib().oracle_fstat_partition(cd(dw), _dp(inv_sn), cd(u_plus), cd(u_cross), float(df), int(lo), int(hi),
+                                        int(mode), C.byref(F), None, None, _dp(a))
     return F.value, a, int(flag)
 
 

@@ -1,6 +1,7 @@
 // fstat_api.cu -- the C ABI declared in include/fstat.h: plan management, argument validation,
-// segmentation of the frequency band into CTA work items, workspace, launches.  Host code only; every
-// arithmetic step of the hot path lives in fstat_kernels.cu.  There is no CPU fallback.
+// segmentation of the frequency band into CTA work items, workspace, launches.  Host code only; the arithmetic
+// of the hot path lives in the kernels (fstat_fast.cu, fstat_fastband.cu, fstat_kernels.cu, fstat_band.cu,
+// fstat_pso.cu).  There is no CPU fallback.
 #include "../../include/fstat.h"
 #include "fstat_internal.h"
 
@@ -26,6 +27,7 @@ struct fstat_plan {
     double f0 = 0.0;                   // freq[0]
     double *d_table = nullptr;         // [n_bins][kTabW]   (direct kernel, template dump, Gram build)
     double *d_dwp = nullptr;           // [n_bins][2]       folded data (interpolating kernel)
+    double *d_w = nullptr;             // [n_bins]          4 df f^(-7/3) |K_f|^2 / S_n  (Gram builders, row f2's cuts)
     double *d_node = nullptr;          // [n_node_rows][kTabW]
     int64_t n_node_rows = 0;
     bool fast_ok = false;              // the node grid (2 kMaxStride bins below, 3 above the band) stays at f > 0
@@ -37,6 +39,7 @@ struct fstat_plan {
     // segmentation (depends on the partitions and on the number of particle groups)
     int32_t seg_groups = -1;           // n_groups the current segmentation was made for
     int32_t n_seg = 0;
+    int32_t seg_len = 0;               // bins per work segment of the current segmentation (aligned cuts)
     int32_t *d_seg_edge = nullptr;     // [n_seg+1]
     int32_t *d_part_seg = nullptr;     // [n_part+1]
     size_t seg_cap = 0, part_cap = 0;
@@ -56,17 +59,16 @@ struct fstat_plan {
     int32_t *d_perm = nullptr; size_t perm_cap = 0;      // [P_pad] slot -> particle (-1: padding)
     double *d_partial = nullptr; size_t partial_cap = 0; // doubles
     // row f2 (fstat_eval_batch_bands)
-    fstat_plan *cells = nullptr;        // internal plan whose partitions are the lattice cells (shares the tables)
-    int32_t cells_lattice = 0;
-    bool shares_tables = false;         // d_table, d_dwp, d_node belong to the parent plan
+    fstat_plan *bandplan = nullptr;     // internal plan whose one partition is the whole grid (work segments only); shares the tables
+    bool shares_tables = false;         // d_table, d_dwp, d_w, d_node belong to the parent plan
+    double *d_pgram[kNLevels] = {};     // prefix Gram matrices [ceil(n_bins / 8)][kNGram] per stride level (first band call)
+    bool pgram_built = false;
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
-    double *d_rec = nullptr; size_t rec_cap = 0;          // [n_wseg][2][kNAcc][P_pad]
-    int32_t *d_rec_idx = nullptr; size_t rec_idx_cap = 0; // [n_wseg][2][P_pad]
-    int32_t *d_piece_scratch = nullptr; size_t piece_scratch_cap = 0;   // length-class counts and starts of the piece list
-    int2 *d_piece_list = nullptr; size_t piece_list_cap = 0;            // [P_pad (n_seg + 1)] (slot, edge) ordered by length
-    double *d_rag = nullptr; size_t rag_cap = 0;          // [P_pad][n_seg + 1][kNAcc] the shorter piece of every cell an edge splits
+    double *d_rec = nullptr; size_t rec_cap = 0;          // [n_seg][2][kNPartial][P_pad] head / tail fragments of the work segments
+    uint32_t *d_err = nullptr;                            // device flag raised by an internal invariant
     double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
     int64_t *d_band_out = nullptr; size_t band_out_cap = 0; // [P][2] (host-buffer call)
+    bool last_was_band = false;         // fstat_plan_level_bins reports the band plan's stride mix
     // host-buffer path
     double *d_params = nullptr, *d_F = nullptr, *d_Fk = nullptr;
     size_t params_cap = 0, F_cap = 0, Fk_cap = 0;
@@ -154,7 +156,15 @@ void make_segments(const std::vector<int64_t> &edges, int64_t max_len, bool alig
     (*part_seg)[n_part] = (int32_t)(seg_edge->size() - 1);
 }
 
+// The band plan (row f2) always cuts at the multiples of its segment length: its stitch kernel finds the work segment
+// of a bin by division.  Elsewhere a segment length that is not a multiple of 512 means near-equal pieces (tests).
 bool segments_aligned(const fstat_plan *pl)
+{
+    return pl->shares_tables || pl->opt.max_segment_bins <= 0 || pl->opt.max_segment_bins % kMaxStride == 0;
+}
+
+// the interpolating kernel needs segments that start at multiples of 512 bins
+bool segments_fast_capable(const fstat_plan *pl)
 {
     return pl->opt.max_segment_bins <= 0 || pl->opt.max_segment_bins % kMaxStride == 0;
 }
@@ -215,7 +225,8 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
     if (pl->seg_groups == n_groups) return FSTAT_OK;
     std::vector<int32_t> seg_edge, part_seg;
     const bool aligned = segments_aligned(pl);
-    make_segments(pl->edges, auto_segment_len(pl, n_groups), aligned, &seg_edge, &part_seg);
+    const int64_t seg_len = auto_segment_len(pl, n_groups);
+    make_segments(pl->edges, seg_len, aligned, &seg_edge, &part_seg);
     const size_t n_seg = seg_edge.size() - 1;
     std::vector<int32_t> gbase(n_seg * kNLevels);
     std::vector<SegCrit> crit(n_seg);
@@ -234,7 +245,7 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
             }
             crit[sgi] = make_seg_crit(pl->f0 + (double)lo * pl->df, pl->f0 + (double)hi * pl->df, pl->df,
                                       (double)(pl->edges[k + 1] - pl->edges[k]));
-            maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && hi - lo >= 8) ? kNLevels - 1 : -1);
+            maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && segments_fast_capable(pl) && hi - lo >= 8) ? kNLevels - 1 : -1);
         }
     CU_TRY(pl, grow(&pl->d_seg_edge, &pl->seg_cap, seg_edge.size()));
     CU_TRY(pl, grow(&pl->d_part_seg, &pl->part_cap, part_seg.size()));
@@ -250,6 +261,7 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
     CU_TRY(pl, cudaMemcpy(pl->d_seg_maxlvl, maxlvl.data(), maxlvl.size() * sizeof(int8_t), cudaMemcpyHostToDevice));
     pl->seg_edge_h = seg_edge;
     pl->n_seg = (int32_t)n_seg;
+    pl->seg_len = (int32_t)(seg_len < pl->n_bins ? seg_len : pl->n_bins);
     pl->seg_groups = n_groups;
     return FSTAT_OK;
 }
@@ -273,7 +285,7 @@ fstat_status build_gram_tables(fstat_plan *pl)
         const int64_t n_sub = (pl->n_bins + S - 1) / S + cnt[n_part - 1];
         CU_TRY(pl, grow(&pl->d_gram[l], &pl->gram_cap[l], (size_t)n_sub * kNGram));
         CU_TRY(pl, cudaMemcpy(pl->d_cnt, cnt.data(), (size_t)n_part * sizeof(int32_t), cudaMemcpyHostToDevice));
-        CU_TRY(pl, launch_build_gram(pl->d_table, pl->d_edges32, n_part, pl->n_bins, l, pl->d_cnt, pl->d_gram[l], 0));
+        CU_TRY(pl, launch_build_gram(pl->d_w, pl->d_edges32, n_part, pl->n_bins, l, pl->d_cnt, pl->d_gram[l], 0));
         CU_TRY(pl, cudaDeviceSynchronize());   // d_cnt is reused by the next level
     }
     return FSTAT_OK;
@@ -377,6 +389,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     CU_TRY(pl, main_kernel_configure());
     CU_TRY(pl, fast_kernel_configure());
     CU_TRY(pl, band_kernel_configure());
+    CU_TRY(pl, fastband_kernel_configure());
 
     const double *d_freq = freq, *d_dw = dw, *d_isn = isn;
     double *tmp = nullptr;
@@ -397,6 +410,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     if (e == cudaSuccess) e = cudaMemset(d_err, 0, sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_table, (size_t)n_bins * kTabW * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_dwp, (size_t)n_bins * 2 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_w, (size_t)n_bins * sizeof(double));
     // node rows for bins -2 kMaxStride .. (floor((N-1)/kMaxStride) + 3) * kMaxStride in steps of kNodeStride
     pl->n_node_rows = kNodePad + (((n_bins - 1) / kMaxStride + 3) * kMaxStride) / kNodeStride + 1;
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_node, (size_t)pl->n_node_rows * kTabW * sizeof(double));
@@ -408,7 +422,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
             pl->f0 = fe[0];
             pl->fast_ok = (fe[0] - (double)(2 * kMaxStride + 1) * pl->df > 0.0) && n_bins > 1;
             e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->d_table,
-                                   pl->d_dwp, d_err, 0);
+                                   pl->d_dwp, pl->d_w, d_err, 0);
             if (e == cudaSuccess)
                 e = launch_build_nodes(d_freq, n_bins, pl->df, pl->opt.arm_length_m, pl->n_node_rows, pl->d_node, 0);
             if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -444,14 +458,15 @@ static void plan_free(fstat_plan *pl)
 {
     if (!pl) return;
     DeviceGuard g(pl->device);
-    if (pl->cells) { plan_free(pl->cells); pl->cells = nullptr; }
-    if (pl->shares_tables) { pl->d_table = nullptr; pl->d_dwp = nullptr; pl->d_node = nullptr; }
+    if (pl->bandplan) { plan_free(pl->bandplan); pl->bandplan = nullptr; }
+    if (pl->shares_tables) { pl->d_table = nullptr; pl->d_dwp = nullptr; pl->d_w = nullptr; pl->d_node = nullptr; }
     cudaFree(pl->d_table); cudaFree(pl->d_seg_edge); cudaFree(pl->d_part_seg); cudaFree(pl->d_coef);
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
-    cudaFree(pl->d_dwp); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
-    for (int l = 0; l < kNLevels; ++l) cudaFree(pl->d_gram[l]);
-    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_rec_idx); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out); cudaFree(pl->d_rag); cudaFree(pl->d_piece_scratch); cudaFree(pl->d_piece_list);
-    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level); cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
+    cudaFree(pl->d_dwp); cudaFree(pl->d_w); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
+    for (int l = 0; l < kNLevels; ++l) { cudaFree(pl->d_gram[l]); cudaFree(pl->d_pgram[l]); }
+    cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_err); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out);
+    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level);
+    cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
@@ -545,6 +560,7 @@ fstat_status fstat_plan_level_bins(fstat_plan *pl, int64_t *bins_out, int64_t *s
 {
     if (!pl || !bins_out || !subblocks_out) return FSTAT_EINVAL;
     for (int l = 0; l <= kNLevels; ++l) bins_out[l] = subblocks_out[l] = 0;
+    if (pl->last_was_band && pl->bandplan) pl = pl->bandplan;      // the most recent evaluation was a row-f2 call
     if (pl->last_groups < 1 || pl->seg_groups != pl->last_groups) return FSTAT_OK;
     DeviceGuard g(pl->device);
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
@@ -581,51 +597,8 @@ int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out
 }
 
 // a1-a5 for P particles, then a6 (F, F_k) when F != NULL and / or the extrinsic amplitudes when amp != NULL
-static void plan_free(fstat_plan *pl);
-
-// Internal plan for row f2 on a lattice: same tables (shared, not copied), partitions = the lattice cells
-// [0, C), [C, 2C), ... ; its Gram tables are built once per lattice and kept.
-static fstat_status ensure_cell_plan(fstat_plan *pl, int32_t C)
-{
-    if (pl->cells && pl->cells_lattice == C) return FSTAT_OK;
-    if (pl->cells) {
-        cudaDeviceSynchronize();
-        plan_free(pl->cells);
-        pl->cells = nullptr;
-    }
-    fstat_plan *cp = new (std::nothrow) fstat_plan;
-    if (!cp) return fail(pl, FSTAT_ENOMEM, "host allocation failed");
-    cp->device = pl->device; cp->n_sm = pl->n_sm; cp->n_bins = pl->n_bins; cp->df = pl->df; cp->opt = pl->opt;
-    cp->opt.max_segment_bins = 0;
-    cp->f0 = pl->f0; cp->orb = pl->orb; cp->fast_ok = pl->fast_ok;
-    cp->d_table = pl->d_table; cp->d_dwp = pl->d_dwp; cp->d_node = pl->d_node; cp->n_node_rows = pl->n_node_rows;
-    cp->shares_tables = true;
-    try {
-        for (int64_t e = 0; e < pl->n_bins; e += C) cp->edges.push_back(e);
-        cp->edges.push_back(pl->n_bins);
-    } catch (...) {
-        plan_free(cp);
-        return fail(pl, FSTAT_ENOMEM, "host allocation failed");
-    }
-    cp->n_part = (int32_t)(cp->edges.size() - 1);
-    fstat_status s = build_gram_tables(cp);
-    if (s != FSTAT_OK) { pl->err = cp->err; plan_free(cp); return s; }
-    pl->cells = cp;
-    pl->cells_lattice = C;
-    return FSTAT_OK;
-}
-
-// row f2 through the interpolating kernel: the plan evaluated is the internal cells plan
-struct BandReq {
-    int32_t n_seg, lattice;   // partitions per template; lattice of the edge rule (reading A26)
-    int32_t cell;             // width of the cells (= lattice, or kBandCell with edges that split the cells)
-    int64_t *band_out;
-    double *amp;              // [P][n_seg][4] extrinsic amplitudes, or NULL
-    fstat_plan *owner;        // the user's plan: timing ring and launch counter
-};
-
 static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, double *amp,
-                              void *stream, const BandReq *br = nullptr, bool sums_only = false)
+                              void *stream, bool sums_only = false)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
@@ -656,22 +629,9 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
 
     CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
     CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
-    const double rank_band[3] = {1.0 / pl->df, pl->f0, pl->f0 + (double)(pl->n_bins - 1) * pl->df};
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, br ? rank_band : nullptr, pl->d_coef,
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, nullptr, pl->d_coef,
                                pl->d_valid, pl->d_perm, st));
     BandSched bs{};
-    if (br) {
-        CU_TRY(pl, grow(&pl->d_band, &pl->band_cap, (size_t)2 * (size_t)P_pad));
-        CU_TRY(pl, launch_band_limits(pl->d_table, pl->d_coef, pl->d_valid, pl->d_perm, P_pad, (int32_t)pl->n_bins,
-                                      1.0 / pl->df, pl->opt.orbit_kappa, pl->d_band, pl->d_band + P_pad, br->band_out, st));
-        bs.band_lo = pl->d_band;
-        bs.band_hi = pl->d_band + P_pad;
-        bs.seg_edge = pl->d_seg_edge;
-        bs.n_seg_band = br->n_seg;
-        bs.lattice = br->lattice;
-        bs.n_bins = (int32_t)pl->n_bins;
-        bs.min_len = br->cell != br->lattice ? br->cell : 1;
-    }
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
                                pl->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
                                pl->opt.force_level, bs, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
@@ -684,16 +644,12 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.seg_gbase = pl->d_seg_gbase;
     fa.level = pl->d_level;
     fa.partial = pl->d_partial;
-    fa.part_sk = br ? 1 : P_pad;                       // row f2: slot-major records (the cells epilogue reads whole records)
-    fa.part_sp = br ? kNPartial : 1;
+    fa.part_sk = P_pad;
+    fa.part_sp = 1;
     fa.P_pad = P_pad;
     fa.n_groups = (int32_t)n_groups;
     fa.n_seg = pl->n_seg;
     fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
-    if (br) {                                          // cells: ~4096 bins per CTA run whatever the lattice
-        const int64_t g = 4096 / br->cell;
-        fa.segs_per_cta = (int32_t)(g < 1 ? 1 : (g > 128 ? 128 : g));
-    }
     fa.df = pl->df;
     fa.orb = pl->orb;
     MainArgs a;
@@ -711,32 +667,14 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     a.n_groups = (int32_t)n_groups;
     a.n_seg = pl->n_seg;
     a.orb = pl->orb;
-    fstat_plan *tp = br ? br->owner : pl;              // whose timing ring and launch counter
-    const int slot = (int)(tp->n_timed % fstat_plan::kRing);
-    CU_TRY(pl, cudaEventRecord(tp->ev0[slot], st));
+    const int slot = (int)(pl->n_timed % fstat_plan::kRing);
+    CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
     if (pl->fast_ok) CU_TRY(pl, launch_fast(fa, st));
     CU_TRY(pl, launch_main(a, st));
-    CU_TRY(pl, cudaEventRecord(tp->ev1[slot], st));
-    ++tp->n_timed;
-    tp->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
-    if (br) {
-        double *rag = nullptr;
-        if (br->cell != br->lattice) {                 // edges at any bin: the cells they fall into are split
-            CU_TRY(pl, grow(&pl->d_rag, &pl->rag_cap, (size_t)P_pad * (size_t)(2 * br->n_seg + 1) * kNAcc));
-            CU_TRY(pl, grow(&pl->d_piece_scratch, &pl->piece_scratch_cap, (size_t)256));
-            CU_TRY(pl, grow(&pl->d_piece_list, &pl->piece_list_cap, (size_t)P_pad * (size_t)(br->n_seg + 1)));
-            rag = pl->d_rag;                           // [P_pad][n_seg + 1] pieces, then [P_pad][n_seg] short partitions
-        }
-        CU_TRY(pl, launch_band_cells_epilogue(pl->d_table, pl->d_coef, pl->d_partial, rag,
-                                              rag ? rag + (size_t)P_pad * (size_t)(br->n_seg + 1) * kNAcc : nullptr,
-                                              rag ? pl->d_piece_scratch : nullptr, pl->d_piece_list, pl->d_part_seg, pl->d_valid,
-                                              pl->d_perm, pl->d_band, pl->d_band + P_pad, P, P_pad, (int32_t)pl->n_bins,
-                                              pl->n_part, br->n_seg, br->lattice, br->cell, fa.part_sk, fa.part_sp, pl->orb,
-                                              F, Fk, br->amp, st));
-        const bool sorted = rag && br->cell <= 128 && br->n_seg >= 128 && br->n_seg < 65535;    // as launch_band_cells_epilogue
-        tp->n_launches += (rag ? 4 : 3) + (sorted ? 4 : 0);   // band limits, [pieces [+ list x 2, scan, sorted pieces]], cells epilogue, F sums
-        return FSTAT_OK;
-    }
+    CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
+    ++pl->n_timed;
+    pl->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
+    pl->last_was_band = false;
     if (F) {
         PartialSet one{};
         one.p[0] = pl->d_partial;
@@ -781,7 +719,7 @@ fstat_status fstat_eval_batch_channels(fstat_plan *const *plans, int32_t n_chann
     PartialSet ps{};
     ps.n = n_channels;
     for (int32_t c = 0; c < n_channels; ++c) {
-        fstat_status s = eval_impl(plans[c], P, params, nullptr, nullptr, nullptr, stream, nullptr, true);
+        fstat_status s = eval_impl(plans[c], P, params, nullptr, nullptr, nullptr, stream, true);
         if (s != FSTAT_OK) { if (c) p0->err = plans[c]->err; return s; }
         if (plans[c]->n_seg != p0->n_seg) return fail(p0, FSTAT_ECUDA, "internal: the channels' segmentations differ");
         ps.p[c] = plans[c]->d_partial;
@@ -802,6 +740,44 @@ fstat_status fstat_eval_amplitudes(fstat_plan *pl, int64_t P, const double *para
     return eval_impl(pl, P, params, nullptr, nullptr, amp, stream);
 }
 
+// Internal plan for row f2: same tables (shared, not copied), ONE partition = the whole grid, so that its segmentation
+// is just the work segments (multiples of the segment length) and its stride selection / work lists can be reused.
+static fstat_status ensure_band_plan(fstat_plan *pl)
+{
+    if (pl->bandplan) return FSTAT_OK;
+    fstat_plan *cp = new (std::nothrow) fstat_plan;
+    if (!cp) return fail(pl, FSTAT_ENOMEM, "host allocation failed");
+    cp->device = pl->device; cp->n_sm = pl->n_sm; cp->n_bins = pl->n_bins; cp->df = pl->df; cp->opt = pl->opt;
+    cp->f0 = pl->f0; cp->orb = pl->orb; cp->fast_ok = pl->fast_ok;
+    cp->d_table = pl->d_table; cp->d_dwp = pl->d_dwp; cp->d_w = pl->d_w; cp->d_node = pl->d_node;
+    cp->n_node_rows = pl->n_node_rows;
+    cp->shares_tables = true;
+    try {
+        cp->edges.assign({(int64_t)0, pl->n_bins});
+        for (int l = 0; l < kNLevels; ++l) cp->cnt[l].assign(1, 0);
+    } catch (...) {
+        plan_free(cp);
+        return fail(pl, FSTAT_ENOMEM, "host allocation failed");
+    }
+    cp->n_part = 1;
+    pl->bandplan = cp;
+    return FSTAT_OK;
+}
+
+// Prefix Gram matrices of every stride level (80 bytes per 8 bins and level), built at the first band call.
+static fstat_status ensure_prefix_gram(fstat_plan *pl)
+{
+    if (pl->pgram_built) return FSTAT_OK;
+    const int64_t n_lat = (pl->n_bins + kMinStride - 1) / kMinStride;
+    for (int l = 0; l < kNLevels; ++l) {
+        if (!pl->d_pgram[l]) CU_TRY(pl, cudaMalloc((void **)&pl->d_pgram[l], (size_t)n_lat * kNGram * sizeof(double)));
+        CU_TRY(pl, launch_build_prefix_gram(pl->d_w, pl->n_bins, l, pl->d_pgram[l], 0));
+    }
+    CU_TRY(pl, cudaDeviceSynchronize());           // built on the default stream; the caller's stream may not wait for it
+    pl->pgram_built = true;
+    return FSTAT_OK;
+}
+
 static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, int32_t n_seg, int32_t edge_lattice,
                                double *F, double *Fk, int64_t *band, double *amp, void *stream)
 {
@@ -810,101 +786,122 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     if (n_seg < 1 || edge_lattice < 1) return fail(pl, FSTAT_EINVAL, "n_seg < 1 or edge_lattice < 1");
     if (P == 0) return FSTAT_OK;
     if (!params || (!F && !amp)) return fail(pl, FSTAT_EINVAL, "params or the output pointer is NULL");
-    if (!F) {                                          // amplitudes only: F goes to scratch
-        DeviceGuard g0(pl->device);
-        if (!g0.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
-        CU_TRY(pl, grow(&pl->d_F, &pl->F_cap, (size_t)P));
-        F = pl->d_F;
-    }
     if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
     if (pl->n_bins >= ((int64_t)1 << 31) - edge_lattice) return fail(pl, FSTAT_EUNSUPPORTED, "grid too long for 32-bit bins");
+    if (P * (int64_t)n_seg >= ((int64_t)1 << 40)) return fail(pl, FSTAT_EUNSUPPORTED, "P x n_seg too large");
     DeviceGuard g(pl->device);
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
     cudaStream_t st = (cudaStream_t)stream;
 
-    if (pl->fast_ok && pl->opt.force_level != -1) {
-        // the interpolating kernel over cells (an internal plan that shares the tables): the cells are the lattice
-        // itself from 32 bins on; below that they are kBandCell bins wide and the edges split them
-        // (wider cells cost the interpolating kernel less, narrower ones the pieces: ~ (n_seg + 1) cell / 4 bins in full)
-        const int32_t cell = edge_lattice >= kBandFastLattice ? edge_lattice
-                             : (n_seg <= 32 ? 8 * kBandCell : n_seg <= 128 ? 4 * kBandCell : n_seg <= 512 ? 2 * kBandCell : kBandCell);
-        fstat_status s = ensure_cell_plan(pl, cell);
+    fstat_status s = ensure_band_plan(pl);
+    if (s != FSTAT_OK) return s;
+    fstat_plan *cp = pl->bandplan;
+    if (cp->opt.max_segment_bins != pl->opt.max_segment_bins) cp->seg_groups = -1;
+    cp->opt = pl->opt;
+    const bool fast = cp->fast_ok && pl->opt.force_level != -1 && segments_fast_capable(cp);
+    if (fast) {
+        s = ensure_prefix_gram(pl);
         if (s != FSTAT_OK) return s;
-        fstat_plan *cp = pl->cells;
-        cp->opt.force_level = pl->opt.force_level;
-        cp->opt.interp_tol = pl->opt.interp_tol;
-        if (!Fk) {
-            CU_TRY(pl, grow(&pl->d_band_fk, &pl->band_fk_cap, (size_t)P * (size_t)n_seg));
-            Fk = pl->d_band_fk;
-        }
-        // one record of 10 sums per (cell, particle): keep the workspace below ~24 GB by batching the particles
-        const int64_t per_particle = ((int64_t)cp->n_part * kNPartial +
-                                      (cell != edge_lattice ? (int64_t)(2 * n_seg + 1) * kNAcc + (n_seg + 1) : 0)) * (int64_t)sizeof(double);
-        int64_t batch = ((int64_t)24 << 30) / per_particle / kThreads * kThreads;
-        if (batch < kThreads) batch = kThreads;
-        BandReq br{n_seg, edge_lattice, cell, nullptr, nullptr, pl};
-        for (int64_t off = 0; off < P; off += batch) {
-            const int64_t n = (P - off < batch) ? P - off : batch;
-            br.band_out = band ? band + 2 * off : nullptr;
-            br.amp = amp ? amp + off * n_seg * 4 : nullptr;
-            s = eval_impl(cp, n, params + 6 * off, F + off, Fk + off * n_seg, nullptr, stream, &br);
-            if (s != FSTAT_OK) { pl->err = cp->err; return s; }
-        }
-        return FSTAT_OK;
     }
-    if (amp) return fail(pl, FSTAT_EUNSUPPORTED, "amplitudes need the interpolating path (force_level != -1, grid away from f = 0)");
     const int64_t n_groups = (P + kThreads - 1) / kThreads;
     const int64_t P_pad = n_groups * kThreads;
-    // work segments: about 8 items per SM over the whole grid, whole tiles, 256 .. 8192 bins
-    int64_t seg_len = pl->opt.max_segment_bins > 0 ? pl->opt.max_segment_bins
-                                                   : (pl->n_bins * n_groups) / ((int64_t)pl->n_sm * 8);
-    if (pl->opt.max_segment_bins <= 0) seg_len = seg_len < 256 ? 256 : (seg_len > 8192 ? 8192 : seg_len);
-    seg_len = (seg_len + kTileBins - 1) / kTileBins * kTileBins;
-    const int64_t n_wseg = (pl->n_bins + seg_len - 1) / seg_len;
-    if (n_wseg * n_groups >= ((int64_t)1 << 31)) return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
+    s = ensure_segments(cp, (int32_t)n_groups);
+    if (s != FSTAT_OK) { pl->err = cp->err; return s; }
+    if ((int64_t)cp->n_seg * n_groups >= ((int64_t)1 << 31))
+        return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
 
-    CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)P_pad * kNCoef));
-    CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)P_pad));
-    CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
-    CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
-    CU_TRY(pl, grow(&pl->d_band, &pl->band_cap, (size_t)2 * (size_t)P_pad));
-    CU_TRY(pl, grow(&pl->d_rec, &pl->rec_cap, (size_t)n_wseg * 2 * kNAcc * (size_t)P_pad));
-    CU_TRY(pl, grow(&pl->d_rec_idx, &pl->rec_idx_cap, (size_t)n_wseg * 2 * (size_t)P_pad));
+    if (!F) {                                          // amplitudes only: F goes to scratch
+        CU_TRY(pl, grow(&pl->d_F, &pl->F_cap, (size_t)P));
+        F = pl->d_F;
+    }
     if (!Fk) {
         CU_TRY(pl, grow(&pl->d_band_fk, &pl->band_fk_cap, (size_t)P * (size_t)n_seg));
         Fk = pl->d_band_fk;
     }
+    CU_TRY(pl, grow(&cp->d_coef, &cp->coef_cap, (size_t)P_pad * kNCoef));
+    CU_TRY(pl, grow(&cp->d_valid, &cp->valid_cap, (size_t)P_pad));
+    CU_TRY(pl, grow(&cp->d_slot, &cp->slot_cap, (size_t)P));
+    CU_TRY(pl, grow(&cp->d_perm, &cp->perm_cap, (size_t)P_pad));
+    CU_TRY(pl, grow(&cp->d_band, &cp->band_cap, (size_t)2 * (size_t)P_pad));
+    CU_TRY(pl, grow(&cp->d_level, &cp->level_cap, (size_t)cp->n_seg * (size_t)n_groups));
+    CU_TRY(pl, grow(&cp->d_direct, &cp->direct_cap, (size_t)cp->n_seg * (size_t)n_groups + 1));
+    CU_TRY(pl, grow(&cp->d_rec, &cp->rec_cap, (size_t)cp->n_seg * 2 * kNPartial * (size_t)P_pad));
+    if (!pl->d_err) {
+        CU_TRY(pl, cudaMalloc((void **)&pl->d_err, sizeof(uint32_t)));
+        CU_TRY(pl, cudaMemset(pl->d_err, 0, sizeof(uint32_t)));
+    }
+    cp->last_groups = (int32_t)n_groups;
+
+    // slots ranked by the position of the band (not by chirp mass): the 128 templates of a CTA overlap at both ends
     const double rank_band[3] = {1.0 / pl->df, pl->f0, pl->f0 + (double)(pl->n_bins - 1) * pl->df};
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, rank_band, pl->d_coef, pl->d_valid,
-                               pl->d_perm, st));
-    CU_TRY(pl, launch_band_limits(pl->d_table, pl->d_coef, pl->d_valid, pl->d_perm, P_pad, (int32_t)pl->n_bins, 1.0 / pl->df,
-                                  pl->opt.orbit_kappa, pl->d_band, pl->d_band + P_pad, band, st));
-    CU_TRY(pl, cudaMemsetAsync(pl->d_rec_idx, 0xFF, (size_t)n_wseg * 2 * (size_t)P_pad * sizeof(int32_t), st));
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, cp->d_slot, rank_band, cp->d_coef,
+                               cp->d_valid, cp->d_perm, st));
+    CU_TRY(pl, launch_band_limits(pl->d_table, cp->d_coef, cp->d_valid, cp->d_perm, P_pad, (int32_t)pl->n_bins,
+                                  1.0 / pl->df, pl->opt.orbit_kappa, cp->d_band, cp->d_band + P_pad, band, st));
+    BandSched bs{};
+    bs.band_lo = cp->d_band;
+    bs.band_hi = cp->d_band + P_pad;
+    bs.seg_edge = cp->d_seg_edge;
+    bs.n_seg_band = n_seg;
+    bs.lattice = edge_lattice;
+    bs.n_bins = (int32_t)pl->n_bins;
+    CU_TRY(pl, launch_schedule(cp->d_coef, cp->d_valid, P_pad, (int32_t)n_groups, cp->n_seg, cp->d_seg_crit,
+                               cp->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
+                               pl->opt.force_level, bs, cp->d_level, cp->d_direct + 1, cp->d_direct, st));
+    // empty partitions and templates without a band: F_k = 0, a = 0
     CU_TRY(pl, cudaMemsetAsync(Fk, 0, (size_t)P * (size_t)n_seg * sizeof(double), st));
-    BandArgs a;
-    a.table = pl->d_table;
-    a.coef = pl->d_coef;
-    a.band_lo = pl->d_band;
-    a.band_hi = pl->d_band + P_pad;
-    a.perm = pl->d_perm;
-    a.rec = pl->d_rec;
-    a.rec_idx = pl->d_rec_idx;
-    a.Fk = Fk;
-    a.P_pad = P_pad;
-    a.n_bins = (int32_t)pl->n_bins;
-    a.n_seg = n_seg;
-    a.lattice = edge_lattice;
-    a.seg_len = (int32_t)seg_len;
-    a.n_wseg = (int32_t)n_wseg;
-    a.n_groups = (int32_t)n_groups;
-    a.orb = pl->orb;
+    if (amp) CU_TRY(pl, cudaMemsetAsync(amp, 0, (size_t)P * (size_t)n_seg * 4 * sizeof(double), st));
+
+    BandCommon bc;
+    bc.band_lo = cp->d_band;
+    bc.band_hi = cp->d_band + P_pad;
+    bc.valid = cp->d_valid;
+    bc.perm = cp->d_perm;
+    bc.rec = cp->d_rec;
+    bc.Fk = Fk;
+    bc.amp = amp;
+    bc.err = pl->d_err;
+    bc.N = n_seg;
+    bc.C = edge_lattice;
+    bc.n_bins = (int32_t)pl->n_bins;
+
     const int slot = (int)(pl->n_timed % fstat_plan::kRing);
     CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
-    CU_TRY(pl, launch_band_main(a, pl->n_sm * 12, st));
+    if (fast) {
+        FastBandArgs fa;
+        fa.dwp = pl->d_dwp;
+        fa.w = pl->d_w;
+        fa.node = pl->d_node;
+        for (int l = 0; l < kNLevels; ++l) fa.pgram[l] = pl->d_pgram[l];
+        fa.coef = cp->d_coef;
+        fa.seg_edge = cp->d_seg_edge;
+        fa.level = cp->d_level;
+        fa.b = bc;
+        fa.P_pad = P_pad;
+        fa.n_groups = (int32_t)n_groups;
+        fa.n_seg = cp->n_seg;
+        fa.df = pl->df;
+        fa.orb = pl->orb;
+        CU_TRY(pl, launch_fastband(fa, st));
+    }
+    BandArgs ba;
+    ba.table = pl->d_table;
+    ba.coef = cp->d_coef;
+    ba.seg_edge = cp->d_seg_edge;
+    ba.direct_list = cp->d_direct + 1;
+    ba.direct_count = cp->d_direct;
+    ba.b = bc;
+    ba.P_pad = P_pad;
+    ba.n_seg = cp->n_seg;
+    ba.orb = pl->orb;
+    CU_TRY(pl, launch_band_main(ba, pl->n_sm * 12, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;
-    CU_TRY(pl, launch_band_epilogue(pl->d_rec, pl->d_rec_idx, pl->d_valid, pl->d_perm, P_pad, (int32_t)n_wseg, n_seg, F, Fk, st));
-    pl->n_launches += 5;                               // rank, prologue, band limits, band main, band epilogue
+    CU_TRY(pl, launch_band_short(pl->d_table, cp->d_coef, bc, P_pad, pl->orb, st));
+    CU_TRY(pl, launch_band_stitch(bc, P, P_pad, cp->seg_len, cp->n_seg, F, st));
+    // rank, prologue, band limits, stride selection, [interpolating], direct, short partitions, stitch, F sums
+    pl->n_launches += 8 + (fast ? 1 : 0);
+    pl->last_was_band = true;
     return FSTAT_OK;
 }
 

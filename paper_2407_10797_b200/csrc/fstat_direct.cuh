@@ -53,6 +53,36 @@ __device__ __forceinline__ void bin_template(const double2 *__restrict__ row, co
     psi_out = psi;
 }
 
+// Basis constant c = T'_x / T'_+ (complex) at one point of a partition, or 0 where T'_+ ~ 0 there.  The sums of a
+// partition are kept in the basis (u_+, u_x - c u_+) (hazard H3): F is invariant under
+// it, and over a narrow partition u_x is nearly c u_+, so the small remainder is accumulated directly instead of
+// being left to cancel in m_cc - |m_pc|^2 / m_pp (normalised determinants down to 3e-12 on config 4).
+__device__ __forceinline__ void choose_basis(double pr, double pi, double xr, double xi, double &c_re, double &c_im)
+{
+    const double n2 = fma(pr, pr, pi * pi), x2 = fma(xr, xr, xi * xi);
+    const bool use = n2 > 1e-6 * x2;
+    const double inv = use ? 1.0 / n2 : 0.0;
+    c_re = fma(xr, pr, xi * pi) * inv;               // T'_x conj(T'_+) / |T'_+|^2
+    c_im = fma(xi, pr, -xr * pi) * inv;
+}
+
+// One bin of the full-model kernels: q = dw' exp(+i Psi), weight w', response (T'_+, T'_x); the eight sums in the
+// basis (u_+, u_x - c u_+)  (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117).
+__device__ __forceinline__ void accumulate_bin(double qr, double qi, double w, double tpr, double tpi, double tcr,
+                                               double tci, double c_re, double c_im, double (&in)[kNAcc])
+{
+    const double xr = tcr - fma(c_re, tpr, -c_im * tpi);              // T'_x - c T'_+
+    const double xi = tci - fma(c_re, tpi, c_im * tpr);
+    in[0] = fma(qr, tpr, fma(qi, tpi, in[0]));                        // z_+ += q conj(T'_+)
+    in[1] = fma(qi, tpr, fma(-qr, tpi, in[1]));
+    in[2] = fma(qr, xr, fma(qi, xi, in[2]));                          // z_x
+    in[3] = fma(qi, xr, fma(-qr, xi, in[3]));
+    in[4] = fma(w, fma(tpr, tpr, tpi * tpi), in[4]);                  // m_pp
+    in[5] = fma(w, fma(xr, xr, xi * xi), in[5]);                      // m_cc
+    in[6] = fma(w, fma(tpr, xr, tpi * xi), in[6]);                    // m_pc = sum w T'_+ conj(T'_x)
+    in[7] = fma(w, fma(tpi, xr, -tpr * xi), in[7]);
+}
+
 // 2 F_k = z^H G^-1 z by Gram-Schmidt (Eq. 7 in its 2x2 Hermitian form):
 // |z_+|^2/m_pp + |z_x - (m_pc/m_pp) z_+|^2 / (m_cc - |m_pc|^2/m_pp); rank-deficient G (reading A15): only
 // the non-degenerate direction(s) contribute.

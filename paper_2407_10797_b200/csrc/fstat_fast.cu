@@ -20,6 +20,7 @@
 // Inner products: PAPER.md:66 Eq. 4, :89-91 Eq. 8-9, :117 Eq. 12.  Template: :397-405 Eq. A1-A3,
 // :206-229 Eq. 17-20 (N = 0).
 #include "fstat_device.cuh"
+#include "fstat_fast.cuh"
 #include "fstat_internal.h"
 #include "fstat_model.cuh"
 
@@ -62,23 +63,13 @@ cudaError_t launch_build_nodes(const double *freq, int64_t n_bins, double df, do
     return cudaGetLastError();
 }
 
-// Lagrange basis of the nodes t = -1, 0, 1, 2 at t
-__device__ __forceinline__ void lagrange4(double t, double (&l)[4])
-{
-    const double tp = t + 1.0, tm = t - 1.0, tm2 = t - 2.0;
-    l[0] = -t * tm * tm2 * (1.0 / 6.0);
-    l[1] = tp * tm * tm2 * 0.5;
-    l[2] = -tp * t * tm2 * 0.5;
-    l[3] = tp * t * tm * (1.0 / 6.0);
-}
-
 // =================================================================================================
 // plan time (per partition set): Gram matrices.  Level `level` cuts every partition at the multiples of
 // S = 8 << level; sub-block [j0, j1) of node interval m = j0 / S in partition k has the table index
 // m + cnt[k], cnt[k] = number of interior partition edges e_1..e_k that are not multiples of S.
 // One thread per node interval; it walks its bins and flushes at every partition edge.
 // =================================================================================================
-__global__ void build_gram_kernel(const double *__restrict__ table, const int32_t *__restrict__ edges,
+__global__ void build_gram_kernel(const double *__restrict__ wtab, const int32_t *__restrict__ edges,
                                   int32_t n_part, int64_t n_bins, int level, const int32_t *__restrict__ cnt,
                                   double *__restrict__ gram)
 {
@@ -105,7 +96,7 @@ __global__ void build_gram_kernel(const double *__restrict__ table, const int32_
             for (int j = 0; j < kNGram; ++j) { out[j] = g[j]; g[j] = 0.0; }
             ++k;
         }
-        const double w = table[i * kTabW + T_W];
+        const double w = wtab[i];
         double l[4];
         lagrange4((double)(i - b0) * rS, l);
         int j = 0;
@@ -119,13 +110,13 @@ __global__ void build_gram_kernel(const double *__restrict__ table, const int32_
     for (int j = 0; j < kNGram; ++j) out[j] = g[j];
 }
 
-cudaError_t launch_build_gram(const double *table, const int32_t *edges, int32_t n_part, int64_t n_bins,
+cudaError_t launch_build_gram(const double *w, const int32_t *edges, int32_t n_part, int64_t n_bins,
                               int level, const int32_t *cnt, double *gram, cudaStream_t st)
 {
     const int S = kMinStride << level;
     const int64_t n_int = (n_bins + S - 1) / S;
     const int nt = 128;
-    build_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(table, edges, n_part, n_bins, level, cnt, gram);
+    build_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(w, edges, n_part, n_bins, level, cnt, gram);
     return cudaGetLastError();
 }
 
@@ -167,16 +158,20 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
 #pragma unroll
     for (int w = 1; w < kThreads / 32; ++w) { c3 = fmax(c3, s3[w]); c9 = fmax(c9, s9[w]); }
 
-    // row f2: the group's bins [g_lo, g_hi) that at least one template is in band for, and its shortest
-    // partition (the H3 amplification is set by the partitions of the templates, not by the lattice cells)
+    // row f2: the group's bins [g_lo, g_hi) that at least one template evaluated by the main kernels is in band for,
+    // and the group's shortest partition: it sets the H3 amplification (the partitions of the templates, not the work
+    // segments) and CAPS the stride, so that a node interval holds at most one partition edge of any thread
     const bool banded = bands.band_lo != nullptr;
     int32_t g_lo = INT32_MAX, g_hi = 0, g_len = INT32_MAX;
     if (banded) {
         if (valid[p]) {
             const int32_t C = bands.lattice, N = bands.n_seg_band;
             const int32_t q_lo = (bands.band_lo[p] + C / 2) / C, D = (bands.band_hi[p] + C / 2) / C - q_lo;
-            const int32_t e0 = band_edge(0, q_lo, D, N, C, bands.n_bins), eN = band_edge(N, q_lo, D, N, C, bands.n_bins);
-            if (eN > e0) { g_lo = e0; g_hi = eN; g_len = max((eN - e0) / N, 1); }
+            if (band_fast_eligible(D, N, C)) {
+                g_lo = band_edge(0, q_lo, D, N, C, bands.n_bins);
+                g_hi = band_edge(N, q_lo, D, N, C, bands.n_bins);
+                g_len = C * (D / N);
+            }
         }
         g_lo = __reduce_min_sync(0xffffffffu, g_lo);
         g_hi = __reduce_max_sync(0xffffffffu, g_hi);
@@ -189,7 +184,7 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
 
     // blockIdx.y splits the segments of the group (thousands of lattice cells in row f2)
     for (int seg = blockIdx.y * kThreads + tid; seg < n_seg; seg += gridDim.y * kThreads) {
-        const int mx = seg_maxlvl[seg];
+        int mx = seg_maxlvl[seg];
         int lvl;
         SegCrit q = crit[seg];
         if (banded) {
@@ -197,7 +192,8 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
                 level[(int64_t)grp * n_seg + seg] = (int8_t)-2;
                 continue;
             }
-            q.kl = 0.05 * (double)max(g_len, bands.min_len);
+            q.kl = 0.05 * (double)g_len;
+            while (mx >= 0 && (kMinStride << mx) > g_len) --mx;                       // g_len >= 8: mx stays >= 0
         }
         const double om = fma(c3, q.p1, c9 * q.p2);
         const double d3 = fma(c3, q.r1, fma(c9, q.r2, q.ad * (128.0 / 3.0) * om * om * om));   // |D3|, quarter turns
@@ -249,67 +245,6 @@ struct __align__(16) FastSmem {
     double win[kWinNodes][kNSlow][kThreads];   // per-thread ring of the last six node values (column = thread)
     uint64_t full[kFastStages];
 };
-
-// The cubic carried over a node interval [node m, node m+1] is NOT the Lagrange cubic through four nodes but
-// the Chebyshev-economised quintic through the six nodes m-2 .. m+3: the quintic's T_4 and T_5 terms on the
-// interval are dropped, which leaves the 4th-order error term 72 times smaller than the centre-interval error
-// of the four-node cubic (h^4 f/3072 against 3 h^4 f/128) for the same node evaluations.  Row a of
-// kEcon gives the value of that cubic at t = -1, 0, 1, 2 (so that everything downstream -- Newton
-// coefficients, Gram matrices in the four-node Lagrange basis -- is unchanged) from the node values at
-// t = -2 .. 3; rows sum to 1 exactly (rationals with denominator 61440).
-__constant__ double kEcon[4][6] = {
-    {-9133.0 / 61440.0, 6371.0 / 4096.0, -4517.0 / 6144.0, 2209.0 / 6144.0, 33.0 / 4096.0, -2407.0 / 61440.0},
-    {-11.0 / 61440.0, 7.0 / 12288.0, 2047.0 / 2048.0, -1.0 / 6144.0, 5.0 / 12288.0, -3.0 / 20480.0},
-    {-3.0 / 20480.0, 5.0 / 12288.0, -1.0 / 6144.0, 2047.0 / 2048.0, 7.0 / 12288.0, -11.0 / 61440.0},
-    {-2407.0 / 61440.0, 33.0 / 4096.0, 2209.0 / 6144.0, -4517.0 / 6144.0, 6371.0 / 4096.0, -9133.0 / 61440.0}};
-
-// v[k] = node values at t = -2 .. 3.  Returns yref = v[2] (node "0") and e[a] = cubic(t_a) - yref, t_a = -1, 0,
-// 1, 2, from the DIFFERENCES v[k] - yref (the phase values are ~1e7 quarter turns, their differences ~1e3).
-__device__ __forceinline__ void economise(const double (&v)[6], double &yref, double (&e)[4])
-{
-    yref = v[2];
-    const double d0 = v[0] - yref, d1 = v[1] - yref, d3 = v[3] - yref, d4 = v[4] - yref, d5 = v[5] - yref;
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-        e[a] = fma(kEcon[a][0], d0, fma(kEcon[a][1], d1, fma(kEcon[a][3], d3, fma(kEcon[a][4], d4, kEcon[a][5] * d5))));
-}
-
-// x - 4 rint(x / 4): exact for |x| < 2^51
-__device__ __forceinline__ double red4(double x) { return fma(-4.0, rint(0.25 * x), x); }
-
-// (c * f) mod 4 to full precision: the product is split exactly into hi + lo by one FMA
-__device__ __forceinline__ double mulmod4(double c, double f)
-{
-    const double hi = c * f;
-    const double lo = fma(c, f, -hi);
-    return red4(hi) + lo;
-}
-
-// Newton-basis coefficients c_n (basis C(u + n - 1, n), u = j1 - i) of the cubic through the node values
-// y0..y3 at t = -1, 0, 1, 2 (t = s / S), for a sub-block that ends U bins after node 0.
-__device__ __forceinline__ void newton_coefs(double y0, double y1, double y2, double y3, double rS, double U,
-                                             double (&c)[4])
-{
-    const double d0 = y0 - y1, d2 = y2 - y1, d3 = y3 - y1;
-    const double a1 = fma(d0, -1.0 / 3.0, fma(d3, -1.0 / 6.0, d2));
-    const double a2 = 0.5 * (d0 + d2);
-    const double a3 = fma(d2, -0.5, (d3 - d0) * (1.0 / 6.0));
-    const double g1 = a1 * rS, g2 = a2 * rS * rS, g3 = a3 * rS * rS * rS;
-    const double e0 = fma(U, fma(U, fma(U, g3, g2), g1), y1);
-    const double e1 = -fma(U, fma(3.0 * U, g3, 2.0 * g2), g1);
-    const double e2 = fma(3.0 * U, g3, g2);
-    const double e3 = -g3;
-    c[0] = e0;
-    c[1] = e1 - e2 + e3;
-    c[2] = fma(-6.0, e3, 2.0 * e2);
-    c[3] = 6.0 * e3;
-}
-
-__device__ __forceinline__ void load_coef(const double *__restrict__ cf, int64_t P_pad, double (&c)[kNCoef])
-{
-#pragma unroll
-    for (int j = 0; j < kNCoef; ++j) c[j] = cf[(int64_t)j * P_pad];
-}
 
 __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_constant__ FastArgs a)
 {

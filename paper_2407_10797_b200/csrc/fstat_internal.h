@@ -68,8 +68,6 @@ constexpr int kFastTileShift = 9;
 constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the folded data (8 KiB), aligned to its size;
                                                      // >= kMaxStride so that no sub-block straddles two tiles
 constexpr int kFastStages = 3;
-constexpr int kBandFastLattice = 32;                 // row f2: from this edge lattice on the cells ARE the lattice; below it ...
-constexpr int kBandCell = 64;                        // ... the cells are 64 .. 512 bins wide (by n_seg) and the edges split them (band_ragged_kernel)
 constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
 
 // per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)
@@ -132,6 +130,14 @@ __host__ __device__ __forceinline__ int32_t band_edge(int32_t j, int32_t q_lo, i
     return (int32_t)(e < (int64_t)n_bins ? e : (int64_t)n_bins);
 }
 
+// row f2: a template goes through the interpolating kernel when none of its partitions is empty or shorter than the
+// smallest stride (partition lengths are C floor(D / N) or C ceil(D / N) lattice cells of C bins); the others are
+// evaluated partition by partition with the full model (band_short_kernel)
+__host__ __device__ __forceinline__ bool band_fast_eligible(int32_t D, int32_t N, int32_t C)
+{
+    return D >= N && (int64_t)C * (int64_t)(D / N) >= (int64_t)kMinStride;
+}
+
 // what the stride selection needs to know about the bands (nullptr band_lo: fixed data-side partitions)
 struct BandSched {
     const int32_t *band_lo;   // [P_pad]
@@ -140,26 +146,49 @@ struct BandSched {
     int32_t n_seg_band;       // partitions per template
     int32_t lattice;
     int32_t n_bins;
-    int32_t min_len;          // shorter partitions do not use the cell records (they are evaluated edge to edge)
 };
 
-// row f2 (fstat_band.cu): per-particle bands and partition edges
+// row f2, both main kernels: per-thread bands, head / tail records of the work segments
+struct BandCommon {
+    const int32_t *band_lo;   // [P_pad] k_lo, k_hi of every slot (bins of the plan's grid)
+    const int32_t *band_hi;
+    const int32_t *valid;     // [P_pad]
+    const int32_t *perm;      // [P_pad] slot -> particle
+    double *rec;              // [n_seg][2][kNPartial][P_pad]: head (0) and tail (1) fragment of every work segment
+    double *Fk;               // [P][N]
+    double *amp;              // [P][N][4] or nullptr
+    uint32_t *err;            // device flag: internal invariant violated
+    int32_t N;                // partitions per template (the paper's N_seg)
+    int32_t C;                // edges are multiples of this many bins (reading A26)
+    int32_t n_bins;
+};
+
+struct FastBandArgs {
+    const double *dwp;            // [n_bins][2] folded data
+    const double *w;              // [n_bins] 4 df f^(-7/3) |K_f|^2 / S_n
+    const double *node;           // [n_node_rows][kTabW]
+    const double *pgram[kNLevels];// [ceil(n_bins / 8)][kNGram] prefix Gram matrices
+    const double *coef;           // [kNCoef][P_pad]
+    const int32_t *seg_edge;      // [n_seg + 1] work segments (multiples of 512 bins)
+    const int8_t *level;          // [n_groups][n_seg]
+    BandCommon b;
+    int64_t P_pad;
+    int32_t n_groups;
+    int32_t n_seg;
+    double df;
+    OrbitCoef orb;
+};
+
+// the direct kernel with per-thread edges, for the work items the stride selection leaves to it
 struct BandArgs {
     const double *table;      // [n_bins][kTabW]
     const double *coef;       // [kNCoef][P_pad]
-    const int32_t *band_lo;   // [P_pad] k_lo, k_hi of every slot (bins of the plan's grid)
-    const int32_t *band_hi;
-    const int32_t *perm;      // [P_pad] slot -> particle
-    double *rec;              // [n_wseg][2][kNAcc][P_pad] head / tail fragments
-    int32_t *rec_idx;         // [n_wseg][2][P_pad] the partition a fragment belongs to, -1: none
-    double *Fk;               // [P][n_seg]
+    const int32_t *seg_edge;  // [n_seg + 1]
+    const int32_t *direct_list;
+    const int32_t *direct_count;
+    BandCommon b;
     int64_t P_pad;
-    int32_t n_bins;
-    int32_t n_seg;            // partitions per template (the paper's N_seg)
-    int32_t lattice;          // edges are multiples of this many bins (reading A26)
-    int32_t seg_len;          // bins per work segment
-    int32_t n_wseg;
-    int32_t n_groups;
+    int32_t n_seg;
     OrbitCoef orb;
 };
 
@@ -167,22 +196,24 @@ cudaError_t launch_band_limits(const double *table, const double *coef, const in
                                int64_t P_pad, int32_t n_bins, double T_obs, double kappa, int32_t *band_lo,
                                int32_t *band_hi, int64_t *band_out, cudaStream_t st);
 cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t st);
-cudaError_t launch_band_epilogue(const double *rec, const int32_t *rec_idx, const int32_t *valid, const int32_t *perm,
-                                 int64_t P_pad, int32_t n_wseg, int32_t n_seg, double *F, double *Fk, cudaStream_t st);
 cudaError_t band_kernel_configure();
-cudaError_t launch_band_cells_epilogue(const double *table, const double *coef, const double *partial, double *rag,
-                                       double *rag_short, int32_t *piece_scratch, int2 *piece_list, const int32_t *part_seg, const int32_t *valid, const int32_t *perm,
-                                       const int32_t *band_lo, const int32_t *band_hi, int64_t P, int64_t P_pad,
-                                       int32_t n_bins, int32_t n_cells, int32_t n_seg_band, int32_t lattice, int32_t cell,
-                                       int64_t part_sk, int64_t part_sp, const OrbitCoef &orb, double *F, double *Fk,
-                                       double *amp, cudaStream_t st);
+cudaError_t launch_fastband(const FastBandArgs &a, cudaStream_t st);
+cudaError_t fastband_kernel_configure();
+cudaError_t launch_build_prefix_gram(const double *w, int64_t n_bins, int level, double *pgram, cudaStream_t st);
+// full model over every partition of the templates the interpolating kernel does not take (band_fast_eligible)
+cudaError_t launch_band_short(const double *table, const double *coef, const BandCommon &b, int64_t P_pad,
+                              const OrbitCoef &orb, cudaStream_t st);
+// partitions that straddle work segments from their head / tail records; -inf / NaN rows of invalid particles;
+// then F = sum_k F_k.  seg_len = bins per work segment (the last one may be shorter)
+cudaError_t launch_band_stitch(const BandCommon &b, int64_t P, int64_t P_pad, int32_t seg_len, int32_t n_seg, double *F,
+                               cudaStream_t st);
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
-                               double df, double arm_length_m, double *table, double *dwp,
+                               double df, double arm_length_m, double *table, double *dwp, double *w,
                                uint32_t *err_bits, cudaStream_t st);
 cudaError_t launch_build_nodes(const double *freq, int64_t n_bins, double df, double arm_length_m,
                                int64_t n_rows, double *node, cudaStream_t st);
-cudaError_t launch_build_gram(const double *table, const int32_t *edges, int32_t n_part, int64_t n_bins,
+cudaError_t launch_build_gram(const double *w, const int32_t *edges, int32_t n_part, int64_t n_bins,
                               int level, const int32_t *cnt, double *gram, cudaStream_t st);
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,

@@ -22,7 +22,7 @@ namespace fstat {
 // =================================================================================================
 __global__ void build_table_kernel(const double *__restrict__ freq, const double *__restrict__ dw,
                                    const double *__restrict__ isn, int64_t n_bins, double df, double L,
-                                   double *__restrict__ table, double2 *__restrict__ dwp,
+                                   double *__restrict__ table, double2 *__restrict__ dwp, double *__restrict__ wout,
                                    uint32_t *__restrict__ err_bits)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -47,18 +47,20 @@ __global__ void build_table_kernel(const double *__restrict__ freq, const double
     const double qr = amp * (dr * kr - di * ki), qi = amp * (dr * ki + di * kr);
     row[T_DWR] = qr;
     row[T_DWI] = qi;
-    row[T_W] = 4.0 * df * pow(f, -7.0 / 3.0) * (4.0 * s2x * s2x) * w;
+    const double wp = 4.0 * df * pow(f, -7.0 / 3.0) * (4.0 * s2x * s2x) * w;
+    row[T_W] = wp;
+    wout[i] = wp;
     dwp[i] = make_double2(qr, qi);
 }
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
-                               double df, double arm_length_m, double *table, double *dwp,
+                               double df, double arm_length_m, double *table, double *dwp, double *w,
                                uint32_t *err_bits, cudaStream_t st)
 {
     const int nt = 256;
     const int64_t nb = (n_bins + nt - 1) / nt;
     build_table_kernel<<<(unsigned)nb, nt, 0, st>>>(freq, dw, isn, n_bins, df, arm_length_m, table,
-                                                    reinterpret_cast<double2 *>(dwp), err_bits);
+                                                    reinterpret_cast<double2 *>(dwp), w, err_bits);
     return cudaGetLastError();
 }
 
@@ -237,6 +239,8 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
         double acc[kNAcc];
 #pragma unroll
         for (int j = 0; j < kNAcc; ++j) acc[j] = 0.0;
+        bool need_c = true;
+        double c_re = 0.0, c_im = 0.0;
 
         for (int t = 0; t < n_tiles; ++t) {
             const double *tile = ring_wait(sm, g0 + t);
@@ -252,18 +256,15 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
                 double psi, sps, cps, tpr, tpi, tcr, tci;
                 bin_template(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
 
-                // ---- a4: inner products (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117)
+                // ---- a4: inner products (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117) in the basis (u_+, u_x - c u_+),
+                // c = T'_x / T'_+ at the work item's first bin (hazard H3)
+                if (need_c) {
+                    need_c = false;
+                    choose_basis(tpr, tpi, tcr, tci, c_re, c_im);
+                }
                 const double qr = fma(dwv.x, cps, -dwv.y * sps);               // dw' exp(+i Psi)
                 const double qi = fma(dwv.x, sps, dwv.y * cps);
-                in[0] = fma(qr, tpr, fma(qi, tpi, in[0]));                      // z_+ += q conj(T'_+)
-                in[1] = fma(qi, tpr, fma(-qr, tpi, in[1]));
-                in[2] = fma(qr, tcr, fma(qi, tci, in[2]));                      // z_x
-                in[3] = fma(qi, tcr, fma(-qr, tci, in[3]));
-                const double w = row[11].x;
-                in[4] = fma(w, fma(tpr, tpr, tpi * tpi), in[4]);                // m_pp
-                in[5] = fma(w, fma(tcr, tcr, tci * tci), in[5]);                // m_cc
-                in[6] = fma(w, fma(tpr, tcr, tpi * tci), in[6]);                // m_pc = sum w T'_+ conj(T'_x)
-                in[7] = fma(w, fma(tpi, tcr, -tpr * tci), in[7]);
+                accumulate_bin(qr, qi, row[11].x, tpr, tpi, tcr, tci, c_re, c_im, in);
             }
 #pragma unroll
             for (int j = 0; j < kNAcc; ++j) acc[j] += in[j];
@@ -276,8 +277,8 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
         double *out = a.partial + ((int64_t)seg * kNPartial) * a.P_pad + p * a.part_sp;
 #pragma unroll
         for (int j = 0; j < kNAcc; ++j) out[(int64_t)j * a.part_sk] = acc[j];
-        out[(int64_t)8 * a.part_sk] = 0.0;                 // plain basis (u_+, u_x): c = 0
-        out[(int64_t)9 * a.part_sk] = 0.0;
+        out[(int64_t)8 * a.part_sk] = c_re;
+        out[(int64_t)9 * a.part_sk] = c_im;
     }
 }
 

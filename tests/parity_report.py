@@ -4,8 +4,10 @@ BASELINE.json's five configs, in the launch configurations bench.py times.
 
     python tests/parity_report.py [--out gpurun_out/r2_parity.md] [--quick]
 
-Expected values come from oracle/ only (oracle.fstat_batch_multi: a particle's templates are written once and
-every N_p of the config is computed from them); the GPU side is the library through its C ABI.  Coverage:
+Expected values come from oracle/ only (oracle.fstat_batch_multi, mode 2: a particle's templates are written once,
+every N_p of the config is computed from them, and the inner products stay in long double through the 4x4 solve --
+near 100 mHz config 4 has partitions whose M has a normalised determinant of 3e-12, where rounding N and M to double
+costs 3e-5 of F_k, pin P18); the GPU side is the library through its C ABI.  Coverage:
   config 0   all 64 particles, N_p = 4
   config 1   all 2048 particles, N_p = 1024
   config 2   1024 seeded particles (128 of each of the 8 swarms) of the P = 8192 batch, N_p = 256, 64, 16
@@ -76,7 +78,7 @@ def main():
         sample = np.asarray(sample)
         t0 = time.time()
         sets = [ds.edges(k) for k in n_parts]
-        oracle = orc.fstat_batch_multi(ds.freq, ds.dw, ds.inv_sn, sets, params[sample])
+        oracle = orc.fstat_batch_multi(ds.freq, ds.dw, ds.inv_sn, sets, params[sample], use_ld=2)
         t_or = time.time() - t0
         with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, sets[0]) as plan:
             for P in P_list:
@@ -137,8 +139,9 @@ def main():
             sample = np.sort(np.concatenate([np.arange(256), 256 + rng.choice(4096 - 256, 512, replace=False),
                                              4096 + rng.choice(65536 - 4096, 512, replace=False)]))
         run("4 wide_band", ds, par, sample, list(cfg.n_part), [256, 4096, 65536])
-    notes.append("Oracle: oracle/fstat_oracle.c as it stands (compensated FP64 sums, long-double 4x4 Cholesky), %d host "
-                 "threads; total wall time of this run %.0f s." % (orc.max_threads(), time.time() - t_start))
+    notes.append("Oracle: oracle/fstat_oracle.c, mode 2 (templates in FP64; the 4 + 10 sums in long double handed to the "
+                 "long-double 4x4 Cholesky unrounded: pin P18, hazard H3), %d host threads; total wall time of this run "
+                 "%.0f s." % (orc.max_threads(), time.time() - t_start))
     flush()
     print("written:", args.out)
     return 0

@@ -157,7 +157,9 @@ def test_bench_fp64_instruction_model_matches_the_sass(fs):
     # Q <- Q C^4 update in the 4-bin runs
     assert bench.FAST_FP64_PER_BIN in fast["per_bin"]
     assert all(bench.FAST_FP64_PER_BIN - 1.0 <= v <= bench.FAST_FP64_PER_BIN for v in fast["per_bin"])
-    assert direct["per_bin"] == bench.DIRECT_FP64_PER_BIN
+    # the direct kernel's loop body also holds the once-per-work-item choice of the basis constant c (a division,
+    # ~20 FP64 instructions behind a branch): executed per bin = the static count minus that
+    assert bench.DIRECT_FP64_PER_BIN <= direct["per_bin"] <= bench.DIRECT_FP64_PER_BIN + 24
     # the per-bin loop of the interpolating kernel is almost pure FP64: the pipe that bounds it
     assert bench.FAST_FP64_PER_BIN / fast["per_bin_all_pipes"] > 0.8
     # what bench.py itself reads from the SASS at run time (its constants are only the fallback)

@@ -235,7 +235,10 @@ def _check_sampled(fs, torch, orc, ds, n_parts, params, sample, rtol=RTOL, P_lis
     computes those particles one by one (templates written once per particle, all N_p from them)."""
     sample = np.asarray(sample)
     sets = [ds.edges(k) for k in n_parts]
-    oracle = orc.fstat_batch_multi(ds.freq, ds.dw, ds.inv_sn, sets, params[sample])
+    # expected values with the sums kept in long double through the solve (oracle mode 2; pin P18): partitions of
+    # config 4 near 100 mHz have normalised determinants of M down to 3e-12, where rounding N and M to double before
+    # the solve would cost 3e-5 of F_k
+    oracle = orc.fstat_batch_multi(ds.freq, ds.dw, ds.inv_sn, sets, params[sample], use_ld=2)
     worst = {}
     with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, sets[0]) as plan:
         for P in (P_list or [params.shape[0]]):

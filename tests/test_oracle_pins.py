@@ -457,6 +457,47 @@ def test_long_double_accumulation_agrees(orc, tiny):
     np.testing.assert_allclose(Fka, Fkb, rtol=1e-9)
 
 
+def test_p18_long_double_solve_is_basis_invariant_on_a_near_singular_partition(orc):
+    """Hazard H3 at its worst (config 4, N_p = 1024, near 100 mHz: t_f moves 0.35 s per bin, u_x is a complex multiple
+    of u_+ to 1e-6 and the normalised determinant of M is ~3e-12).  F is invariant under a change of basis inside
+    the partition (it is a maximum over the span of the templates, Eq. 7): in the basis (u_+, g), g = the rescaled
+    remainder of u_x after projecting out u_+, M is well conditioned and the plain double path is exact to rounding.
+    Mode 2 of `fstat_partition` (long-double sums handed to the solve unrounded) must reproduce that value from the
+    RAW templates; modes 0 / 1, which round N and M to double first, cannot (1e-16 / det): that is why the full-size
+    parity runs take their expected values from mode 2."""
+    T = 2.5 * YR
+    k = np.arange(7882466, 7889400)                        # config 4's last partition of 1024: 6934 bins below 100 mHz
+    f = k / T
+    sn = syn.psd_tdi_x(f)
+    d = syn.coloured_noise(sn, T, 77)
+    par = np.array([2.01175308e+08, 32.2478345, 0.240811108, 0.419683311, 4.10389321, 0.0894705007])   # a config-4 draw
+    up, uc = orc.template(par, f)
+    LD = np.longdouble
+    w = (1.0 / sn).astype(LD)
+    upl, ucl = up.astype(np.clongdouble), uc.astype(np.clongdouble)
+    c = np.sum(w * ucl * np.conj(upl)) / np.sum(w * np.abs(upl) ** 2)
+    g = ucl - c * upl
+    det = float(np.sum(w * np.abs(g) ** 2) / np.sum(w * np.abs(ucl) ** 2))
+    assert det < 1e-10                                     # the partition IS near-singular
+    g = (g * np.sqrt(np.sum(w * np.abs(upl) ** 2) / np.sum(w * np.abs(g) ** 2))).astype(np.complex128)
+    n, df = f.size, 1.0 / T
+    truth = orc.fstat_partition(d / sn, 1.0 / sn, up, g, df, 0, n, mode=0)[0]
+    assert orc.fstat_partition(d / sn, 1.0 / sn, up, g, df, 0, n, mode=2)[0] == pytest.approx(truth, rel=1e-12)
+    raw = [orc.fstat_partition(d / sn, 1.0 / sn, up, uc, df, 0, n, mode=m)[0] for m in (0, 1, 2)]
+    assert raw[2] == pytest.approx(truth, rel=1e-7)
+    err = [abs(r - truth) / truth for r in raw]
+    assert err[0] > 10.0 * err[2] and err[1] > 10.0 * err[2] and err[0] > 1e-7
+    # on a well-conditioned partition the three modes agree to rounding
+    par2 = np.array([3.5 * YR, 30.0, 0.24, 0.7854, 2.1216, 0.05])
+    k2 = np.arange(1700000, 1800000)
+    f2 = k2 / T
+    sn2 = syn.psd_tdi_x(f2)
+    d2 = syn.coloured_noise(sn2, T, 78)
+    up2, uc2 = orc.template(par2, f2)
+    F3 = [orc.fstat_partition(d2 / sn2, 1.0 / sn2, up2, uc2, df, 0, f2.size, mode=m)[0] for m in (0, 1, 2)]
+    assert F3[1] == pytest.approx(F3[0], rel=1e-10) and F3[2] == pytest.approx(F3[0], rel=1e-10)
+
+
 def test_semicoherent_peak_broadens_with_more_partitions(orc):
     """PAPER.md:124-126 / Fig. 1: away from the true chirp mass the noiseless semi-coherent statistic
     keeps a larger fraction of its peak value when N_seg is larger."""
