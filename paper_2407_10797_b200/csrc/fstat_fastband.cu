@@ -168,7 +168,9 @@ __device__ __forceinline__ void finish_partition(const double (&v)[kNAcc], doubl
     }
 }
 
-__global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __grid_constant__ FastBandArgs a)
+// 168 registers, no spills in the per-bin loop, 3 CTAs per SM (at 128 registers / 4 CTAs the per-interval code spills
+// ~400 bytes and the call is 4 % slower)
+__global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __grid_constant__ FastBandArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     BandSmem &sm = *reinterpret_cast<BandSmem *>(smem_raw);
@@ -211,8 +213,11 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
     const int32_t q_lo = (a.b.band_lo[p] + C / 2) / C, D = (a.b.band_hi[p] + C / 2) / C - q_lo;
     int32_t j = N, cut = INT32_MAX;
     bool opened = false;                                     // partition j started inside this work segment (or exactly at lo)
+    int32_t my_lo = INT32_MAX, my_hi = 0;                    // this thread's band (empty: not evaluated by this kernel)
     if (a.b.valid[p] != 0 && band_fast_eligible(D, N, C)) {
         const int32_t e0 = band_edge(0, q_lo, D, N, C, a.b.n_bins), eN = band_edge(N, q_lo, D, N, C, a.b.n_bins);
+        my_lo = e0;
+        my_hi = eN;
         if (lo < eN && hi > e0) {
             if (lo < e0) { j = -1; cut = e0; }
             else {
@@ -227,6 +232,15 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
             }
         }
     }
+    // The node intervals of this work segment that hold an in-band bin of some lane of this WARP: [w_lo, w_hi).  The
+    // slots are ranked by the position of the band, so the bands of the 32 lanes of a warp nearly coincide while the
+    // four warps of a CTA are spread over the group's union: a warp skips the intervals outside its own range
+    // (nothing of what it would accumulate there is kept) and starts its node ring where it enters.
+    const int S = 1 << sh;
+    int w_lo = __reduce_min_sync(0xffffffffu, my_lo), w_hi = __reduce_max_sync(0xffffffffu, my_hi);
+    if (w_hi <= 0) w_hi = -1;                                // no lane of this warp is evaluated here
+    w_lo = max(lo, w_lo & ~(S - 1));
+    w_hi = min(hi, w_hi + 1);                                // + 1: an edge AT w_hi closes its partition in the interval that starts there
     const int32_t particle = a.b.perm[p];
     double *rec_head = a.b.rec + ((int64_t)(seg * 2 + 0) * kNPartial) * a.P_pad + p;
     double *rec_tail = a.b.rec + ((int64_t)(seg * 2 + 1) * kNPartial) * a.P_pad + p;
@@ -235,46 +249,40 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
     const double c0 = cf[0];
     const double slope = mulmod4(c0, a.df);
 
-    // node ring: (psi_nl, T'_+ re, im, T'_x re, im) at the last six nodes, slot = (node + 6) % 6
-    int m = lo >> sh;
-    {
-        double c[kNCoef];
-        load_coef(cf, a.P_pad, c);
-        for (int k = -2; k <= 2; ++k) {
-            const double2 *row = reinterpret_cast<const double2 *>(
-                a.node + ((int64_t)kNodePad + ((int64_t)(m + k) * (1 << lvl))) * kTabW);
-            double v0, v1, v2, v3, v4;
-            model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
-            const int slot = (m + k + kWinNodes) % kWinNodes;
-            sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
-            sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
-        }
-    }
-
     double acc[kNAcc];
 #pragma unroll
     for (int q = 0; q < kNAcc; ++q) acc[q] = 0.0;
     bool need_basis = true;
     double c_re = 0.0, c_im = 0.0;
-    int cur_tile = -1;
-    const int S = 1 << sh;
+    bool ring_ok = false;                                    // the node ring holds nodes m-2 .. m+2 of the next interval
 
-    for (int j0 = lo; j0 < hi; j0 += S, ++m) {
+  for (int tl = 0; tl < n_tiles; ++tl) {
+    const int tb0 = max(lo, (t_first + tl) << kFastTileShift), tb1 = min(hi, (t_first + tl + 1) << kFastTileShift);
+    // every warp waits for every tile, also those it skips: a slot is re-armed only after all phases of its barrier
+    // have been observed (a warp that skipped a phase would mistake the parity of a later one)
+    mbar_wait(&sm.full[tl % kBandStages], (uint32_t)((tl / kBandStages) & 1));
+    if (tb0 < w_hi && tb1 > w_lo) {                          // warp-uniform
+      for (int j0 = max(tb0, w_lo); j0 < min(tb1, w_hi); j0 += S) {
+        const int m = j0 >> sh;
         const int node0 = j0;                                // sub-blocks are whole node intervals (cut short only by the grid end)
         const int j1 = min(hi, node0 + S);
         const int s_base = (m - 2 + kWinNodes) % kWinNodes;  // ring slot of node m-2
-        // ---- new node m+3
+        // ---- node ring: (psi_nl, T'_+ re, im, T'_x re, im) at the last six nodes, slot = (node + 6) % 6: the new node
+        // m+3, and nodes m-2 .. m+2 where the warp enters its range
         const double fnode = a.node[((int64_t)kNodePad + ((int64_t)m << lvl)) * kTabW + T_F];
         {
             double c[kNCoef];
             load_coef(cf, a.P_pad, c);
-            const double2 *row = reinterpret_cast<const double2 *>(
-                a.node + ((int64_t)kNodePad + ((int64_t)(m + 3) * (1 << lvl))) * kTabW);
-            double v0, v1, v2, v3, v4;
-            model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
-            const int slot = (m + 3 + kWinNodes) % kWinNodes;
-            sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
-            sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
+            for (int k = ring_ok ? 3 : -2; k <= 3; ++k) {
+                const double2 *row = reinterpret_cast<const double2 *>(
+                    a.node + ((int64_t)kNodePad + ((int64_t)(m + k) * (1 << lvl))) * kTabW);
+                double v0, v1, v2, v3, v4;
+                model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
+                const int slot = (m + k + kWinNodes) % kWinNodes;
+                sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
+                sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
+            }
+            ring_ok = true;
         }
         // ---- carrier phase: economised cubic + exact linear term, as forward differences (s0 = 0: j0 is the node)
         double t, D1, D2, D3;
@@ -294,16 +302,6 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
             D1 = G3 + G2 + G1;
             D2 = fma(6.0, G3, 2.0 * G2);
             D3 = 6.0 * G3;
-        }
-        // ---- the tile that holds [j0, j1)
-        const int tl = (j0 >> kFastTileShift) - t_first;
-        if (tl != cur_tile) {
-            if (cur_tile >= 0) {
-                __syncthreads();                             // every thread is done with the previous tile
-                if (tid == 0 && cur_tile + kBandStages < n_tiles) issue_tile(cur_tile + kBandStages);
-            }
-            cur_tile = tl;
-            mbar_wait(&sm.full[tl % kBandStages], (uint32_t)((tl / kBandStages) & 1));
         }
         const double2 *tp = &sm.tile[tl % kBandStages][j0 & (kFastTile - 1)];
         const int nb = j1 - j0;
@@ -336,6 +334,7 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
             sm.snap[0][tid] = make_double2(A0r, A0i); sm.snap[1][tid] = make_double2(A1r, A1i);      \
             sm.snap[2][tid] = make_double2(A2r, A2i); sm.snap[3][tid] = make_double2(A3r, A3i);      \
         }
+        // which 4-bin runs hold a cut of some lane of this warp: one bit per 2^msh runs, warp-uniform
         int b = 0;
         for (; b + 4 <= nb; b += 4) {
             const double2 d0 = tp[b], d1 = tp[b + 1], d2 = tp[b + 2], d3 = tp[b + 3];
@@ -441,15 +440,19 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
                 newton_from_mono(mcr, U, cr);
                 newton_from_mono(mci, U, ci);
                 z_from_sums(cr, ci, Ar, Ai, pc[2], pc[3]);
+                // prefix Gram matrix up to the NEAREST point of the 8-bin lattice (or the interval's end), then the
+                // <= 4 bins between that point and the cut added or taken away directly from the cubic
                 double mm[4] = {0.0, 0.0, 0.0, 0.0};
-                const int u8 = (cut - node0) & ~(kMinStride - 1);
-                if (u8 > 0) {                                // prefix Gram matrix up to the 8-bin lattice
+                const int uc = cut - node0;
+                const int u8 = min((uc + kMinStride / 2) & ~(kMinStride - 1), j1 - node0);
+                if (u8 > 0) {
                     double g[kNGram];
-                    load_gram(a.pgram[lvl] + ((int64_t)((node0 + u8) >> kLevel0Shift) - 1) * kNGram, g);
+                    load_gram(a.pgram[lvl] + ((int64_t)((node0 + u8 - 1) >> kLevel0Shift)) * kNGram, g);
                     gram_quad(g, ypr, ypi, ycr, yci, mm);
                 }
-                for (int i = node0 + u8; i < cut; ++i) {     // <= 7 bins between the lattice and the cut, from the cubic
-                    const double s = (double)(i - node0), wi = a.w[i];
+                const double sgn = uc >= u8 ? 1.0 : -1.0;
+                for (int i = node0 + min(uc, u8); i < node0 + max(uc, u8); ++i) {
+                    const double s = (double)(i - node0), wi = sgn * a.w[i];
                     const double pr = horner3(mpr, s), pi = horner3(mpi, s), xr = horner3(mcr, s), xi = horner3(mci, s);
                     mm[0] = fma(wi, fma(pr, pr, pi * pi), mm[0]);
                     mm[1] = fma(wi, fma(xr, xr, xi * xi), mm[1]);
@@ -488,7 +491,11 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fastband_kernel(const __gri
             for (int q = 0; q < kNAcc; ++q) acc[q] = 0.0;
             add_record(t10, c_re, c_im, acc);
         }
+      }
     }
+    __syncthreads();                                         // every warp is done with this tile
+    if (tid == 0 && tl + kBandStages < n_tiles) issue_tile(tl + kBandStages);
+  }
     // ---- what is left after the last edge.  Partition j either goes on in the next work segment (tail fragment) or
     // closes exactly at the end of this one (cut == hi): finished here if it also began here, else its closing fragment
     if (j >= 0 && j < N) {
