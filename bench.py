@@ -174,7 +174,7 @@ def parse_args():
     ap.add_argument("--bands-lattice", type=int, default=1,
                     help="edge lattice of --bands in bins (1: edges at any bin; >= 32: the lattice cells are the work units)")
     ap.add_argument("--channels", type=int, default=0, metavar="N",
-                    help="also time fstat_eval_batch_channels (row f4: N TDI channels X, Y, Z with common amplitudes)")
+                    help="also time fstat_eval_batch_channels (row f4: the first N of the TDI channels A, E, T, common amplitudes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the N_p sweep rows the default workload adds to the line")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
@@ -563,15 +563,16 @@ def run_ours(args):
                                   else "fstat_fast_kernel over 64..512-bin cells + band_ragged_kernel (pieces of the "
                                        "cells the edges split, full model)"}
     if args.channels > 1:
-        # row f4: channel c = the same grid, partitions and particles, noise seed c, response with the spacecraft
-        # relabelled cyclically (orbit_lambda + 2 pi c / 3: X, Y, Z); a1-a5 once per channel, one joint epilogue
+        # row f4: the channel sum of Eq. 3 over A, E, T (the combinations with independent noise): the same
+        # grid, partitions and particles; channel data = seeded noise with that channel's PSD (timing does not depend on
+        # the data); a1-a5 once per channel with the A / E / T response at the nodes, one joint epilogue
         import dataclasses
-        plans = [plan]
-        for c in range(1, min(args.channels, 3)):
-            o = fs.fstat_default_options()
-            o.force_level, o.max_segment_bins, o.interp_tol = args.force_level, args.max_segment_bins, args.interp_tol
-            o.orbit_lambda = 2.0 * math.pi * c / 3.0
-            ds_c = syn.make_dataset(dataclasses.replace(cfg, noise_seed=cfg.noise_seed + c), None)
+        names = "AET"[:min(args.channels, 3)]
+        plans = []
+        for c, name in enumerate(names):
+            o = fs.fstat_default_options(force_level=args.force_level, max_segment_bins=args.max_segment_bins,
+                                         interp_tol=args.interp_tol, tdi_channel=fs.TDI_CHANNELS[name])
+            ds_c = syn.make_dataset(dataclasses.replace(cfg, noise_seed=cfg.noise_seed + 1 + c), None, channel=name)
             plans.append(fs.fstat_plan_create(ds_c.freq, ds_c.dw, ds_c.inv_sn, edges, o))
         for _ in range(2):
             fs.fstat_eval_batch_channels(plans, par, stream)
@@ -585,10 +586,10 @@ def run_ours(args):
             e1.record(stream)
         torch.cuda.synchronize()
         ms_c = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs]))
-        out["channels"] = {"n_channels": len(plans), "ms_per_step": ms_c, "ms_per_step_one_channel": ms_step,
+        out["channels"] = {"channels": list(names), "ms_per_step": ms_c, "ms_per_step_one_channel_X": ms_step,
                            "channel_template_bins_per_s": float(P) * ds.n_bins * len(plans) * world / (ms_c * 1e-3),
-                           "data": "noise only in channels 2.. (seeded); timing does not depend on the data"}
-        for pl in plans[1:]:
+                           "data": "seeded noise with each channel's own PSD; timing does not depend on the data"}
+        for pl in plans:
             fs.fstat_plan_destroy(pl)
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, ds, n_part, args.cpu_sample)

@@ -47,6 +47,13 @@ typedef enum {
     FSTAT_EUNSUPPORTED = 4   /* valid request outside this build's limits (e.g. n_bins >= 2^31)  */
 } fstat_status;
 
+/* TDI combinations the library can template: the first-generation Michelson combinations X, Y, Z
+ * (centred on spacecraft 1, 2, 3; reading A7) and A = (Z - X)/sqrt 2, E = (X - 2Y + Z)/sqrt 6,
+ * T = (X + Y + Z)/sqrt 3, "that have mutually independent noise of instrumental origin [64]" (reading A28). */
+typedef enum {
+    FSTAT_TDI_X = 0, FSTAT_TDI_Y = 1, FSTAT_TDI_Z = 2, FSTAT_TDI_A = 3, FSTAT_TDI_E = 4, FSTAT_TDI_T = 5
+} fstat_tdi_channel;
+
 /* Options of a plan.  Obtain defaults with fstat_default_options; opts == NULL means defaults. */
 typedef struct {
     double f_ref_e0;          /* frequency [Hz] at which e0 is defined; default 0.01      */
@@ -63,6 +70,8 @@ typedef struct {
                                * wherever the segment allows it, regardless of the bound (tests / tuning)          */
     double interp_tol;        /* scale of the interpolation error tolerances; 1.0 (default) = carrier phase        *
                                * 1.5e-7 rad and TDI response 2e-7 relative            */
+    int32_t tdi_channel;      /* fstat_tdi_channel: the TDI combination this plan's data and templates are in;     *
+                               * default FSTAT_TDI_X, the paper's                                     */
 } fstat_options;
 
 FSTAT_API void fstat_default_options(fstat_options *opts);

@@ -61,11 +61,12 @@ typedef struct {
     double arm_length_m;  /* 2.5e9 */
     double orbit_kappa;   /* initial orbital phase of the constellation centre */
     double orbit_lambda;  /* initial orientation of the constellation */
+    int32_t tdi_channel;  /* 0 X (the paper's), 1 Y, 2 Z, 3 A, 4 E, 5 T (reading A28) */
 } oracle_options;
 
 void oracle_default_options(oracle_options *o)
 {
-    o->f_ref_e0 = 0.01; o->arm_length_m = 2.5e9; o->orbit_kappa = 0.0; o->orbit_lambda = 0.0;
+    o->f_ref_e0 = 0.01; o->arm_length_m = 2.5e9; o->orbit_kappa = 0.0; o->orbit_lambda = 0.0; o->tdi_channel = 0;
 }
 
 /* params: tc [s], Mc [Msun], eta, theta [rad, ecliptic colatitude], phi [rad], e0 */
@@ -180,20 +181,19 @@ static void orc_link(const double ps[3], const double pr[3], double f, double L,
     Gc[0] = re * xi_c; Gc[1] = im * xi_c;
 }
 
-/* TDI-X transfer functions T_+(f), T_x(f) with the constellation at time t (reading A7):
- *   T_P = (1 - z^2) [ (G^{3->1} + z G^{1->3}) - (G^{2->1} + z G^{1->2}) ],  z = exp(-2 pi i f L/c). */
-void oracle_response(const double *par, double f, double t, const oracle_options *opt,
-                     double Tp[2], double Tc[2])
+/* First-generation Michelson combination centred on spacecraft v (v = 0, 1, 2 <-> X, Y, Z) with the constellation
+ * at positions p (reading A7; Y and Z are X with the spacecraft relabelled cyclically):
+ *   T_P = (1 - z^2) [ (G^{c->v} + z G^{v->c}) - (G^{b->v} + z G^{v->b}) ],  b = v + 1, c = v + 2 (mod 3),
+ *   z = exp(-2 pi i f L/c);   for X: (G^{3->1} + z G^{1->3}) - (G^{2->1} + z G^{1->2}). */
+static void orc_michelson(double p[3][3], int vtx, double f, double L, const double k[3], const double u[3],
+                          const double v[3], double Tp[2], double Tc[2])
 {
-    double p[3][3], k[3], u[3], v[3];
-    const double L = opt->arm_length_m;
-    oracle_orbit(t, opt, p);
-    oracle_sky_basis(par[3], par[4], k, u, v);
+    const double *pv = p[vtx], *pb = p[(vtx + 1) % 3], *pc = p[(vtx + 2) % 3];
     double g31p[2], g31c[2], g13p[2], g13c[2], g21p[2], g21c[2], g12p[2], g12c[2];
-    orc_link(p[2], p[0], f, L, k, u, v, g31p, g31c);
-    orc_link(p[0], p[2], f, L, k, u, v, g13p, g13c);
-    orc_link(p[1], p[0], f, L, k, u, v, g21p, g21c);
-    orc_link(p[0], p[1], f, L, k, u, v, g12p, g12c);
+    orc_link(pc, pv, f, L, k, u, v, g31p, g31c);
+    orc_link(pv, pc, f, L, k, u, v, g13p, g13c);
+    orc_link(pb, pv, f, L, k, u, v, g21p, g21c);
+    orc_link(pv, pb, f, L, k, u, v, g12p, g12c);
     const double w = 2.0 * ORC_PI * f * L / ORC_C_SI;
     const double zr = cos(w), zi = -sin(w);
     const double z2r = zr * zr - zi * zi, z2i = 2.0 * zr * zi;
@@ -205,6 +205,33 @@ void oracle_response(const double *par, double f, double t, const oracle_options
         const double si = (gA[P][1] + zr * gB[P][1] + zi * gB[P][0]) - (gC[P][1] + zr * gD[P][1] + zi * gD[P][0]);
         out[P][0] = fr * sr - fi * si;
         out[P][1] = fr * si + fi * sr;
+    }
+}
+
+/* Transfer functions T_+(f), T_x(f) of the TDI combination opt->tdi_channel with the constellation at time t.
+ * X, Y, Z: the Michelson combinations above.  A, E, T ("combinations called {A, E, T} that have
+ * mutually independent noise of instrumental origin [64]"; the paper prints no formula, reading A28 takes those of
+ * its ref. [64]):  A = (Z - X) / sqrt 2,  E = (X - 2 Y + Z) / sqrt 6,  T = (X + Y + Z) / sqrt 3. */
+void oracle_response(const double *par, double f, double t, const oracle_options *opt,
+                     double Tp[2], double Tc[2])
+{
+    double p[3][3], k[3], u[3], v[3];
+    const double L = opt->arm_length_m;
+    oracle_orbit(t, opt, p);
+    oracle_sky_basis(par[3], par[4], k, u, v);
+    const int ch = opt->tdi_channel;
+    if (ch >= 0 && ch <= 2) {
+        orc_michelson(p, ch, f, L, k, u, v, Tp, Tc);
+        return;
+    }
+    double Xp[2], Xc[2], Yp[2], Yc[2], Zp[2], Zc[2];
+    orc_michelson(p, 0, f, L, k, u, v, Xp, Xc);
+    orc_michelson(p, 1, f, L, k, u, v, Yp, Yc);
+    orc_michelson(p, 2, f, L, k, u, v, Zp, Zc);
+    for (int i = 0; i < 2; ++i) {
+        if (ch == 3)      { Tp[i] = (Zp[i] - Xp[i]) / sqrt(2.0);               Tc[i] = (Zc[i] - Xc[i]) / sqrt(2.0); }
+        else if (ch == 4) { Tp[i] = (Xp[i] - 2.0 * Yp[i] + Zp[i]) / sqrt(6.0); Tc[i] = (Xc[i] - 2.0 * Yc[i] + Zc[i]) / sqrt(6.0); }
+        else              { Tp[i] = (Xp[i] + Yp[i] + Zp[i]) / sqrt(3.0);       Tc[i] = (Xc[i] + Yc[i] + Zc[i]) / sqrt(3.0); }
     }
 }
 

@@ -27,7 +27,10 @@ _lib = None
 
 class Options(C.Structure):
     _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double),
-                ("orbit_kappa", C.c_double), ("orbit_lambda", C.c_double)]
+                ("orbit_kappa", C.c_double), ("orbit_lambda", C.c_double), ("tdi_channel", C.c_int32)]
+
+
+TDI_CHANNELS = {"X": 0, "Y": 1, "Z": 2, "A": 3, "E": 4, "T": 5}
 
 
 def build(force: bool = False) -> str:

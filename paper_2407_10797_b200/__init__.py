@@ -12,7 +12,7 @@ This package never imports ``oracle`` (the CPU oracle is test infrastructure) an
 from __future__ import annotations
 
 from .binding import (  # noqa: F401
-    FstatError, Options, Plan, STATUS,
+    FstatError, Options, Plan, STATUS, TDI_CHANNELS,
     fstat_default_options, fstat_plan_create, fstat_plan_set_partitions, fstat_eval_batch,
     fstat_eval_batch_host, fstat_eval_batch_bands, fstat_eval_batch_bands_host, fstat_eval_amplitudes_bands, fstat_eval_batch_channels, fstat_eval_amplitudes, fstat_eval_template, fstat_plan_destroy, fstat_plan_n_bins,
     fstat_plan_n_part, fstat_plan_device, fstat_plan_n_ctas, fstat_plan_launch_count,

@@ -37,7 +37,11 @@ class Options(C.Structure):
     """fstat_options of include/fstat.h."""
     _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double), ("orbit_kappa", C.c_double),
                 ("orbit_lambda", C.c_double), ("device", C.c_int32), ("inputs_on_device", C.c_int32),
-                ("max_segment_bins", C.c_int32), ("force_level", C.c_int32), ("interp_tol", C.c_double)]
+                ("max_segment_bins", C.c_int32), ("force_level", C.c_int32), ("interp_tol", C.c_double),
+                ("tdi_channel", C.c_int32)]
+
+
+TDI_CHANNELS = {"X": 0, "Y": 1, "Z": 2, "A": 3, "E": 4, "T": 5}      # fstat_tdi_channel
 
 
 class PsoOptions(C.Structure):

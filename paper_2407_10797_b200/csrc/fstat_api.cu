@@ -295,8 +295,10 @@ fstat_status build_gram_tables(fstat_plan *pl)
 
 // The orbit of PAPER.md:198 (analytic, second order in the eccentricity e = L / (2 sqrt(3) AU); formulas
 // of DESIGN.md reading A9) written as trigonometric polynomials in alpha = 2 pi t / yr + kappa.
-void fstat::make_orbit_coef(double L, double lambda, OrbitCoef *out)
+void fstat::make_orbit_coef(double L, double lambda_in, int32_t tdi_channel, OrbitCoef *out)
 {
+    // Y, Z: the Michelson combination centred on spacecraft 2, 3 = X of the constellation relabelled cyclically
+    const double lambda = lambda_in + ((tdi_channel == 1 || tdi_channel == 2) ? 2.0 * kPi * tdi_channel / 3.0 : 0.0);
     const long double R = kAU, pi = 3.14159265358979323846264338327950288L;
     const long double e = (long double)L / (2.0L * sqrtl(3.0L) * R);
     long double Pn[3][3][7];
@@ -335,6 +337,10 @@ void fstat::make_orbit_coef(double L, double lambda, OrbitCoef *out)
             out->c[1][i][j] = (double)((Pn[1][i][j] - Pn[0][i][j]) / (long double)L);
             out->c[2][i][j] = (double)((Pn[2][i][j] - Pn[0][i][j]) / (long double)L);
         }
+    // A = (Z - X)/sqrt 2, E = (X - 2Y + Z)/sqrt 6, T = (X + Y + Z)/sqrt 3   (reading A28)
+    const double r2 = sqrt(0.5), r6 = sqrt(1.0 / 6.0), r3 = sqrt(1.0 / 3.0);
+    const double W[3][3] = {{-r2, 0.0, r2}, {r6, -2.0 * r6, r6}, {r3, r3, r3}};
+    for (int i = 0; i < 3; ++i) out->wch[i] = (tdi_channel >= 3 && tdi_channel <= 5) ? W[tdi_channel - 3][i] : 0.0;
 }
 
 extern "C" {
@@ -352,6 +358,7 @@ void fstat_default_options(fstat_options *o)
     o->max_segment_bins = 0;
     o->force_level = -2;
     o->interp_tol = 1.0;
+    o->tdi_channel = FSTAT_TDI_X;
 }
 
 const char *fstat_status_str(fstat_status s)
@@ -442,7 +449,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
         if (bits & ERR_ISN_NONPOS) why += "inv_sn has an entry <= 0; ";
         return fail(pl, FSTAT_EINVAL, why);
     }
-    make_orbit_coef(pl->opt.arm_length_m, pl->opt.orbit_lambda, &pl->orb);
+    make_orbit_coef(pl->opt.arm_length_m, pl->opt.orbit_lambda, pl->opt.tdi_channel, &pl->orb);
     {
         fstat_status gs = build_gram_tables(pl);
         if (gs != FSTAT_OK) return gs;
@@ -490,7 +497,7 @@ fstat_status fstat_plan_create(fstat_plan **out, int64_t n_bins, const double *f
     if (opts) o = *opts;
     if (!(o.f_ref_e0 > 0.0) || !(o.arm_length_m > 0.0) || !isfinite(o.orbit_kappa) || !isfinite(o.orbit_lambda) ||
         o.max_segment_bins < 0 || o.force_level < -2 || o.force_level >= kNLevels || !(o.interp_tol > 0.0) ||
-        !isfinite(o.interp_tol))
+        !isfinite(o.interp_tol) || o.tdi_channel < FSTAT_TDI_X || o.tdi_channel > FSTAT_TDI_T)
         return fail(nullptr, FSTAT_EINVAL, "bad option value");
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
@@ -650,6 +657,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.n_groups = (int32_t)n_groups;
     fa.n_seg = pl->n_seg;
     fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
+    fa.aet = pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0;
     fa.df = pl->df;
     fa.orb = pl->orb;
     MainArgs a;
@@ -666,6 +674,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     a.P = (int32_t)P;
     a.n_groups = (int32_t)n_groups;
     a.n_seg = pl->n_seg;
+    a.aet = fa.aet;
     a.orb = pl->orb;
     const int slot = (int)(pl->n_timed % fstat_plan::kRing);
     CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
@@ -713,7 +722,8 @@ fstat_status fstat_eval_batch_channels(fstat_plan *const *plans, int32_t n_chann
             if (plans[b] == pc) return fail(p0, FSTAT_EINVAL, "the same plan given for two channels");
         if (pc->device != p0->device || pc->n_bins != p0->n_bins || pc->df != p0->df || pc->f0 != p0->f0 ||
             pc->edges != p0->edges || pc->opt.max_segment_bins != p0->opt.max_segment_bins ||
-            pc->opt.f_ref_e0 != p0->opt.f_ref_e0 || pc->opt.orbit_kappa != p0->opt.orbit_kappa)
+            pc->opt.f_ref_e0 != p0->opt.f_ref_e0 || pc->opt.orbit_kappa != p0->opt.orbit_kappa ||
+            pc->opt.arm_length_m != p0->opt.arm_length_m)
             return fail(p0, FSTAT_EINVAL, "the channels' plans differ in device, grid, partitions or options other than the response");
     }
     PartialSet ps{};
@@ -788,6 +798,8 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     if (!params || (!F && !amp)) return fail(pl, FSTAT_EINVAL, "params or the output pointer is NULL");
     if (P > ((int64_t)1 << 30)) return fail(pl, FSTAT_EUNSUPPORTED, "P > 2^30");
     if (pl->n_bins >= ((int64_t)1 << 31) - edge_lattice) return fail(pl, FSTAT_EUNSUPPORTED, "grid too long for 32-bit bins");
+    if (pl->opt.tdi_channel >= FSTAT_TDI_A)
+        return fail(pl, FSTAT_EUNSUPPORTED, "per-template bands are built for the Michelson responses X, Y, Z only");
     if (P * (int64_t)n_seg >= ((int64_t)1 << 40)) return fail(pl, FSTAT_EUNSUPPORTED, "P x n_seg too large");
     DeviceGuard g(pl->device);
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
@@ -991,7 +1003,8 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
     CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, nullptr, pl->d_coef,
                                pl->d_valid, nullptr, st));
-    CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, u_plus, u_cross, st));
+    CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0,
+                               u_plus, u_cross, st));
     CU_TRY(pl, cudaStreamSynchronize(st));
     return FSTAT_OK;
 }

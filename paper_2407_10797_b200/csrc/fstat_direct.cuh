@@ -42,12 +42,13 @@ __device__ __forceinline__ const double *ring_wait(MainSmem &sm, int g)
 // One (particle, bin) of the direct kernel: model_eval() plus the linear phase term and the carrier.
 // Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1 included), its sine and
 // cosine, and T'_+ , T'_x.
+template <bool AET = false>
 __device__ __forceinline__ void bin_template(const double2 *__restrict__ row, const double (&c)[kNCoef],
                                              const OrbitCoef &orb, double &psi_out, double &sps, double &cps,
                                              double &tpr, double &tpi, double &tcr, double &tci)
 {
     double psi_nl;
-    model_eval(row, c, orb, psi_nl, tpr, tpi, tcr, tci);
+    model_eval<AET>(row, c, orb, psi_nl, tpr, tpi, tcr, tci);
     const double psi = fma(c[0], row[0].x, psi_nl);                  // + 2 pi f t_c
     sincos_qt(psi, sps, cps);
     psi_out = psi;

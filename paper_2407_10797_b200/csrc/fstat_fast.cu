@@ -246,7 +246,8 @@ struct __align__(16) FastSmem {
     uint64_t full[kFastStages];
 };
 
-__global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_constant__ FastArgs a)
+template <bool AET>
+__device__ __forceinline__ void fast_kernel_body(const FastArgs &a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     FastSmem &sm = *reinterpret_cast<FastSmem *>(smem_raw);
@@ -308,7 +309,7 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             const double2 *row = reinterpret_cast<const double2 *>(
                 a.node + ((int64_t)kNodePad + ((int64_t)(m + k) * (1 << lvl))) * kTabW);
             double v0, v1, v2, v3, v4;
-            model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
+            model_eval<AET>(row, c, a.orb, v0, v1, v2, v3, v4);
             const int slot = (m + k + kWinNodes) % kWinNodes;
             sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
             sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
@@ -343,7 +344,7 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
             const double2 *row = reinterpret_cast<const double2 *>(
                 a.node + ((int64_t)kNodePad + ((int64_t)(m + 3) * (1 << lvl))) * kTabW);
             double v0, v1, v2, v3, v4;
-            model_eval(row, c, a.orb, v0, v1, v2, v3, v4);
+            model_eval<AET>(row, c, a.orb, v0, v1, v2, v3, v4);
             const int slot = (m + 3 + kWinNodes) % kWinNodes;
             sm.win[slot][0][tid] = v0; sm.win[slot][1][tid] = v1; sm.win[slot][2][tid] = v2;
             sm.win[slot][3][tid] = v3; sm.win[slot][4][tid] = v4;
@@ -523,9 +524,23 @@ __global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_co
   }
 }
 
+__global__ void __launch_bounds__(kThreads, 4) fstat_fast_kernel(const __grid_constant__ FastArgs a)
+{
+    fast_kernel_body<false>(a);
+}
+
+// the same with the A / E / T response at the nodes (row f4, reading A28)
+__global__ void __launch_bounds__(kThreads, 4) fstat_fast_aet_kernel(const __grid_constant__ FastArgs a)
+{
+    fast_kernel_body<true>(a);
+}
+
 cudaError_t fast_kernel_configure()
 {
-    return cudaFuncSetAttribute(fstat_fast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(fstat_fast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(FastSmem));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(fstat_fast_aet_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)sizeof(FastSmem));
 }
 
@@ -533,7 +548,8 @@ cudaError_t launch_fast(const FastArgs &a, cudaStream_t st)
 {
     const int64_t n_chunks = (a.n_seg + a.segs_per_cta - 1) / a.segs_per_cta;
     const int64_t n_cta = (int64_t)a.n_groups * n_chunks;
-    fstat_fast_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);
+    if (a.aet) fstat_fast_aet_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);
+    else fstat_fast_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);
     return cudaGetLastError();
 }
 

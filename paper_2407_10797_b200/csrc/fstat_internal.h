@@ -50,6 +50,7 @@ constexpr int kStages = 3;       // TMA ring depth
 // vec 0: 4 p_1 / c  [quarter turns per Hz];  vec 1: (p_2 - p_1)/L;  vec 2: (p_3 - p_1)/L.
 struct OrbitCoef {
     double c[3][3][7];
+    double wch[3];    // A, E, T (options.tdi_channel 3..5): weights of the Michelson X, Y, Z responses; else unused
 };
 
 // ---- interpolating ("fast") path: the slow factors of the template (carrier phase without its linear
@@ -95,6 +96,7 @@ struct MainArgs {
     int32_t P;
     int32_t n_groups;
     int32_t n_seg;
+    int32_t aet;                  // 1: the A / E / T response (model_eval<true>)
     OrbitCoef orb;
 };
 
@@ -118,6 +120,7 @@ struct FastArgs {
     int32_t n_groups;
     int32_t n_seg;
     int32_t segs_per_cta;         // consecutive segments one CTA walks (tiles, node ring carried across their edges)
+    int32_t aet;                  // 1: the A / E / T response (model_eval<true>)
     double df;
     OrbitCoef orb;
 };
@@ -240,11 +243,11 @@ cudaError_t launch_amplitudes(const double *partial, const int32_t *part_seg, co
                               const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, double *amp,
                               cudaStream_t st);
 cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
-                            const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st);
+                            const OrbitCoef &orb, int32_t aet, double *u_plus, double *u_cross, cudaStream_t st);
 cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaStream_t st);
 size_t main_kernel_smem_bytes();
 cudaError_t main_kernel_configure();
 
-void make_orbit_coef(double arm_length_m, double lambda, OrbitCoef *out);
+void make_orbit_coef(double arm_length_m, double lambda, int32_t tdi_channel, OrbitCoef *out);
 
 }  // namespace fstat

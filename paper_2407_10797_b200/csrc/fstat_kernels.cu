@@ -202,7 +202,8 @@ size_t main_kernel_smem_bytes() { return sizeof(MainSmem); }
 // The direct kernel: every bin of a work item evaluated in full.  Persistent CTAs walk the list of work
 // items the stride selection left to it (schedule_kernel: items for which no interpolation stride meets
 // the error bound -- all of config 0, partitions shorter than 8 bins); an empty list costs one read.
-__global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_constant__ MainArgs a)
+template <bool AET>
+__device__ __forceinline__ void main_kernel_body(const MainArgs &a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     MainSmem &sm = *reinterpret_cast<MainSmem *>(smem_raw);
@@ -254,7 +255,7 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
                 const double2 *row = reinterpret_cast<const double2 *>(tile + b * kTabW);
                 const double2 dwv = row[10];
                 double psi, sps, cps, tpr, tpi, tcr, tci;
-                bin_template(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
+                bin_template<AET>(row, c, a.orb, psi, sps, cps, tpr, tpi, tcr, tci);
 
                 // ---- a4: inner products (Eq. 4 :66, Eq. 8-9 :89-91, Eq. 12 :117) in the basis (u_+, u_x - c u_+),
                 // c = T'_x / T'_+ at the work item's first bin (hazard H3)
@@ -282,9 +283,22 @@ __global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_const
     }
 }
 
+__global__ void __launch_bounds__(kThreads) fstat_main_kernel(const __grid_constant__ MainArgs a)
+{
+    main_kernel_body<false>(a);
+}
+
+__global__ void __launch_bounds__(kThreads) fstat_main_aet_kernel(const __grid_constant__ MainArgs a)
+{
+    main_kernel_body<true>(a);
+}
+
 cudaError_t main_kernel_configure()
 {
-    return cudaFuncSetAttribute(fstat_main_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(fstat_main_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(MainSmem));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(fstat_main_aet_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)sizeof(MainSmem));
 }
 
@@ -292,7 +306,8 @@ cudaError_t launch_main(const MainArgs &a, cudaStream_t st)
 {
     int64_t n_cta = (int64_t)a.n_groups * a.n_seg;
     if (n_cta > a.max_ctas) n_cta = a.max_ctas;
-    fstat_main_kernel<<<(unsigned)n_cta, kThreads, sizeof(MainSmem), st>>>(a);
+    if (a.aet) fstat_main_aet_kernel<<<(unsigned)n_cta, kThreads, sizeof(MainSmem), st>>>(a);
+    else fstat_main_kernel<<<(unsigned)n_cta, kThreads, sizeof(MainSmem), st>>>(a);
     return cudaGetLastError();
 }
 
@@ -301,6 +316,7 @@ cudaError_t launch_main(const MainArgs &a, cudaStream_t st)
 // whole grid, one thread per bin, through the same bin_template() the main kernel uses.  Serves
 // fstat_eval_template (injection synthesis, element-wise parity tests of a2/a3).
 // =================================================================================================
+template <bool AET>
 __global__ void __launch_bounds__(128) template_kernel(const double *__restrict__ table,
                                                        const double *__restrict__ coef, int64_t P_pad,
                                                        int64_t n_bins, const __grid_constant__ OrbitCoef orb,
@@ -313,7 +329,7 @@ __global__ void __launch_bounds__(128) template_kernel(const double *__restrict_
     for (int j = 0; j < kNCoef; ++j) c[j] = coef[(int64_t)j * P_pad];
     const double2 *row = reinterpret_cast<const double2 *>(table + i * kTabW);
     double psi, sps, cps, tpr, tpi, tcr, tci;
-    bin_template(row, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
+    bin_template<AET>(row, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
     const double f = row[0].x;
     const double amp = pow(f, -7.0 / 6.0);
     const double c2x = row[9].x, s2x = row[9].y;
@@ -325,11 +341,16 @@ __global__ void __launch_bounds__(128) template_kernel(const double *__restrict_
 }
 
 cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
-                            const OrbitCoef &orb, double *u_plus, double *u_cross, cudaStream_t st)
+                            const OrbitCoef &orb, int32_t aet, double *u_plus, double *u_cross, cudaStream_t st)
 {
     const int nt = 128;
-    template_kernel<<<(unsigned)((n_bins + nt - 1) / nt), nt, 0, st>>>(
-        table, coef, P_pad, n_bins, orb, reinterpret_cast<double2 *>(u_plus), reinterpret_cast<double2 *>(u_cross));
+    const unsigned nb = (unsigned)((n_bins + nt - 1) / nt);
+    if (aet)
+        template_kernel<true><<<nb, nt, 0, st>>>(table, coef, P_pad, n_bins, orb, reinterpret_cast<double2 *>(u_plus),
+                                                 reinterpret_cast<double2 *>(u_cross));
+    else
+        template_kernel<false><<<nb, nt, 0, st>>>(table, coef, P_pad, n_bins, orb, reinterpret_cast<double2 *>(u_plus),
+                                                  reinterpret_cast<double2 *>(u_cross));
     return cudaGetLastError();
 }
 

@@ -55,10 +55,40 @@ __device__ __forceinline__ void arm_response(double xq, double c2x, double s2x, 
     gi = fma(ca, bi, -sa * br);
 }
 
+// The same arm seen from BOTH of its ends (rows f4: Y, Z, A, E, T need the Michelson combinations centred on all three
+// spacecraft): gf = g(mu) as above (vertex at the tail of n), gb = g(-mu) = exp(-i b) [ sinc(b) + z sinc(a) ] x (vertex
+// at the head), and dop = exp(-i (a - b)) = exp(-2 i x mu), the Doppler phase of the head relative to the tail.
+__device__ __forceinline__ void arm_response_both(double xq, double c2x, double s2x, double Pm, double Qm, double rho,
+                                                  double &gfr, double &gfi, double &gbr, double &gbi, double &dr,
+                                                  double &di)
+{
+    const bool a_direct = fabs(Pm) <= fabs(Qm);
+    double sd, cd;
+    sincos_qt(xq * (a_direct ? Pm : Qm), sd, cd);
+    const double so = fma(s2x, cd, -c2x * sd);           // sin(2x - d)
+    const double co = fma(c2x, cd, s2x * sd);            // cos(2x - d)
+    const double sa = a_direct ? sd : so, ca = a_direct ? cd : co, sb = a_direct ? so : sd, cb = a_direct ? co : cd;
+    const double sca = sa * Qm * rho;                    // x sinc(a) = sin(a) / (1 + mu)
+    const double scb = sb * Pm * rho;                    // x sinc(b) = sin(b) / (1 - mu)
+    const double br = fma(c2x, scb, sca), bi = -s2x * scb;
+    gfr = fma(ca, br, sa * bi);
+    gfi = fma(ca, bi, -sa * br);
+    const double cr = fma(c2x, sca, scb), ci = -s2x * sca;
+    gbr = fma(cb, cr, sb * ci);
+    gbi = fma(cb, ci, -sb * cr);
+    dr = fma(ca, cb, sa * sb);
+    di = fma(ca, sb, -sa * cb);
+}
+
 // a2 + a3 at one frequency.  `row` is a table row (layout TabCol), c[] the particle's coefficients.
 // Returns, in quarter turns, psi_nl = Psi_0 - 2 pi f t_c + Doppler phase of spacecraft 1 (reading A4)
 // -- the carrier phase without its linear term c[0] f -- and T'_+, T'_x with T_P = K_f T'_P,
 // K_f = -i (1 - z^2) folded into the data tables.
+// AET = false: first-generation Michelson X (Y, Z through the orbit coefficients of the relabelled constellation).
+// AET = true (reading A28): T' = w_X X' + w_Y Y' + w_Z Z' with the weights orb.wch of A = (Z - X)/sqrt 2,
+// E = (X - 2Y + Z)/sqrt 6 or T = (X + Y + Z)/sqrt 3; the three Michelson responses share the phase, t_f, the orbit and
+// the three arms (each arm evaluated once, seen from both ends), all relative to the Doppler phase of spacecraft 1.
+template <bool AET = false>
 __device__ __forceinline__ void model_eval(const double2 *__restrict__ row, const double (&c)[kNCoef],
                                            const OrbitCoef &orb, double &psi_nl, double &tpr, double &tpi,
                                            double &tcr, double &tci)
@@ -114,21 +144,52 @@ __device__ __forceinline__ void model_eval(const double2 *__restrict__ row, cons
 
     psi_nl = fma(f, kp, psi);                                       // + Doppler phase of spacecraft 1
 
-    // two arms
-    const double P2 = arm_nonzero(1.0 + mu2), Q2 = arm_nonzero(1.0 - mu2);
-    const double P3 = arm_nonzero(1.0 + mu3), Q3 = arm_nonzero(1.0 - mu3);
-    const double den2 = P2 * Q2, den3 = P3 * Q3;         // either sign (|mu| may exceed 1 by 0.0024), never 0
-    const double R = rcp_fast(den2 * den3);
-    double g2r, g2i, g3r, g3i;
-    arm_response(xq, zz.x, zz.y, P2, Q2, den3 * R, g2r, g2i);
-    arm_response(xq, zz.x, zz.y, P3, Q3, den2 * R, g3r, g3i);
-    const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;   // n.e_+.n, n.e_x.n
-    const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
-    // T'_P = xi_P3 g_3 - xi_P2 g_2   (TDI-X: arm 3 minus arm 2, reading A7)
-    tpr = fma(xp3, g3r, -xp2 * g2r);
-    tpi = fma(xp3, g3i, -xp2 * g2i);
-    tcr = fma(xc3, g3r, -xc2 * g2r);
-    tci = fma(xc3, g3i, -xc2 * g2i);
+    if (!AET) {
+        // two arms
+        const double P2 = arm_nonzero(1.0 + mu2), Q2 = arm_nonzero(1.0 - mu2);
+        const double P3 = arm_nonzero(1.0 + mu3), Q3 = arm_nonzero(1.0 - mu3);
+        const double den2 = P2 * Q2, den3 = P3 * Q3;         // either sign (|mu| may exceed 1 by 0.0024), never 0
+        const double R = rcp_fast(den2 * den3);
+        double g2r, g2i, g3r, g3i;
+        arm_response(xq, zz.x, zz.y, P2, Q2, den3 * R, g2r, g2i);
+        arm_response(xq, zz.x, zz.y, P3, Q3, den2 * R, g3r, g3i);
+        const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;   // n.e_+.n, n.e_x.n
+        const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
+        // T'_P = xi_P3 g_3 - xi_P2 g_2   (TDI-X: arm 3 minus arm 2, reading A7)
+        tpr = fma(xp3, g3r, -xp2 * g2r);
+        tpi = fma(xp3, g3i, -xp2 * g2i);
+        tcr = fma(xc3, g3r, -xc2 * g2r);
+        tci = fma(xc3, g3i, -xc2 * g2i);
+    } else {
+        // three arms 1->2, 1->3, 2->3 (n_23 = n_13 - n_12), each seen from both ends
+        const double mu23 = mu3 - mu2, un23 = un3 - un2, vn23 = vn3 - vn2;
+        const double P2 = arm_nonzero(1.0 + mu2), Q2 = arm_nonzero(1.0 - mu2);
+        const double P3 = arm_nonzero(1.0 + mu3), Q3 = arm_nonzero(1.0 - mu3);
+        const double P4 = arm_nonzero(1.0 + mu23), Q4 = arm_nonzero(1.0 - mu23);
+        const double den2 = P2 * Q2, den3 = P3 * Q3, den4 = P4 * Q4;
+        const double R = rcp_fast(den2 * den3 * den4);
+        double f2r, f2i, b2r, b2i, d2r, d2i, f3r, f3i, b3r, b3i, d3r, d3i, f4r, f4i, b4r, b4i, d4r, d4i;
+        arm_response_both(xq, zz.x, zz.y, P2, Q2, den3 * den4 * R, f2r, f2i, b2r, b2i, d2r, d2i);
+        arm_response_both(xq, zz.x, zz.y, P3, Q3, den2 * den4 * R, f3r, f3i, b3r, b3i, d3r, d3i);
+        arm_response_both(xq, zz.x, zz.y, P4, Q4, den2 * den3 * R, f4r, f4i, b4r, b4i, d4r, d4i);
+        const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;
+        const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
+        const double xp4 = fma(un23, un23, -vn23 * vn23), xc4 = 2.0 * un23 * vn23;
+        const double wx = orb.wch[0], wy = orb.wch[1], wz = orb.wch[2];
+        // X = xi_13 g(mu_13) - xi_12 g(mu_12);  Y = [xi_12 g(-mu_12) - xi_23 g(mu_23)] exp(-2 i x mu_12);
+        // Z = [xi_23 g(-mu_23) - xi_13 g(-mu_13)] exp(-2 i x mu_13)          (cyclic relabelling of reading A7)
+#pragma unroll
+        for (int pol = 0; pol < 2; ++pol) {
+            const double x2 = pol ? xc2 : xp2, x3 = pol ? xc3 : xp3, x4 = pol ? xc4 : xp4;
+            const double Xr = fma(x3, f3r, -x2 * f2r), Xi = fma(x3, f3i, -x2 * f2i);
+            const double yr = fma(x2, b2r, -x4 * f4r), yi = fma(x2, b2i, -x4 * f4i);
+            const double zr = fma(x4, b4r, -x3 * b3r), zi = fma(x4, b4i, -x3 * b3i);
+            const double Yr = fma(yr, d2r, -yi * d2i), Yi = fma(yr, d2i, yi * d2r);
+            const double Zr = fma(zr, d3r, -zi * d3i), Zi = fma(zr, d3i, zi * d3r);
+            const double tr = fma(wx, Xr, fma(wy, Yr, wz * Zr)), ti = fma(wx, Xi, fma(wy, Yi, wz * Zi));
+            if (pol == 0) { tpr = tr; tpi = ti; } else { tcr = tr; tci = ti; }
+        }
+    }
 }
 
 // The particle-independent columns of a table row at frequency f (phase basis B_j, derivative basis D_j,

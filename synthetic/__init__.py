@@ -9,6 +9,6 @@ callers use the oracle's template and the CUDA-side bench uses the library's own
 """
 from .lisa_data import (  # noqa: F401
     YEAR_S, C_SI, ARM_LENGTH_M, CONFIGS, BANDS_SMALL, Config, Dataset,
-    frequency_grid, psd_tdi_x, coloured_noise, equal_bin_edges, injection_params,
+    frequency_grid, psd_tdi_x, psd_tdi, coloured_noise, equal_bin_edges, injection_params,
     injection_amplitudes, draw_particles, paper_range_particles, make_dataset, config_by_name,
 )

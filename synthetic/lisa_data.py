@@ -101,6 +101,26 @@ def psd_tdi_x(f: np.ndarray, L: float = ARM_LENGTH_M) -> np.ndarray:
     return 16.0 * np.sin(x) ** 2 * (s_oms + (3.0 + np.cos(2.0 * x)) * s_acc)
 
 
+def psd_tdi(f: np.ndarray, channel: str = "X", L: float = ARM_LENGTH_M) -> np.ndarray:
+    """One-sided PSD of the first-generation TDI combination ``channel`` for equal arms and the noise levels of
+    reading A8.  X, Y, Z: ``psd_tdi_x``.  With the cross-spectrum S_XY = -8 sin^2 x cos x [S_oms + 4 S_acc] of two
+    Michelson combinations, A = (Z - X)/sqrt 2 and E = (X - 2Y + Z)/sqrt 6 have S_X - S_XY and T = (X + Y + Z)/sqrt 3
+    has S_X + 2 S_XY (the combinations with mutually independent noise of PAPER.md:48):
+        S_A = S_E = 8 sin^2 x [(2 + cos x) S_oms + 2 (3 + 2 cos x + cos 2x) S_acc],
+        S_T = 16 sin^2 x (1 - cos x) S_oms + 128 sin^2 x sin^4(x/2) S_acc,      x = 2 pi f L / c."""
+    if channel in ("X", "Y", "Z"):
+        return psd_tdi_x(f, L)
+    f = np.asarray(f, dtype=np.float64)
+    x = 2.0 * np.pi * f * L / C_SI
+    s_oms = (15e-12 * 2.0 * np.pi * f / C_SI) ** 2 * (1.0 + (2e-3 / f) ** 4)
+    s_acc = (3e-15 / (2.0 * np.pi * f * C_SI)) ** 2 * (1.0 + (0.4e-3 / f) ** 2) * (1.0 + (f / 8e-3) ** 4)
+    if channel in ("A", "E"):
+        return 8.0 * np.sin(x) ** 2 * ((2.0 + np.cos(x)) * s_oms + 2.0 * (3.0 + 2.0 * np.cos(x) + np.cos(2.0 * x)) * s_acc)
+    if channel == "T":
+        return 16.0 * np.sin(x) ** 2 * (1.0 - np.cos(x)) * s_oms + 128.0 * np.sin(x) ** 2 * np.sin(0.5 * x) ** 4 * s_acc
+    raise ValueError(channel)
+
+
 def coloured_noise(sn: np.ndarray, T: float, seed: int) -> np.ndarray:
     """n_k = sqrt(S_n T / 4) (x + i y), (x, y) standard normal (reading A17)."""
     xy = np.random.default_rng(seed).standard_normal((sn.shape[0], 2))
@@ -227,12 +247,12 @@ TemplateFn = Callable[[np.ndarray, np.ndarray], Tuple[np.ndarray, np.ndarray]]
 
 
 def make_dataset(cfg: Config, template_fn: Optional[TemplateFn] = None, noise: bool = True,
-                 snr: Optional[float] = None) -> Dataset:
+                 snr: Optional[float] = None, channel: str = "X") -> Dataset:
     """Noise (seeded) + injection.  ``template_fn(params6, freq) -> (u_plus, u_cross)`` supplies the
     two complex basis templates of the injection; ``None`` gives noise only.  The injection is
     h = (a1 + i a3) u_plus + (a2 + i a4) u_cross scaled so that 4 df sum |h|^2 / S_n = snr^2."""
     k_lo, n, f = frequency_grid(cfg.T, cfg.f_lo, cfg.f_hi)
-    sn = psd_tdi_x(f)
+    sn = psd_tdi(f, channel)                                # the TDI combination the data are in (default: the paper's X)
     d = coloured_noise(sn, cfg.T, cfg.noise_seed) if noise else np.zeros(n, dtype=np.complex128)
     inj = None
     pinj = injection_params(cfg)

@@ -60,8 +60,9 @@ class Chirp:
                 abs(c_cross) * a * np.cos(ph + np.angle(c_cross)))
 
 
-def tdi_x_time_domain(t, chirp, c_plus, c_cross, theta, phi, L):
-    """X(t) from the four one-way links with explicit delays."""
+def tdi_michelson_time_domain(t, chirp, c_plus, c_cross, theta, phi, L, vertex=0):
+    """First-generation Michelson combination centred on spacecraft `vertex` (0, 1, 2 <-> X, Y, Z) from its four
+    one-way links with explicit delays; Y and Z are X with the spacecraft relabelled cyclically."""
     st, ct, sp, cp = np.sin(theta), np.cos(theta), np.sin(phi), np.cos(phi)
     k = np.array([-st * cp, -st * sp, -ct])
     u = np.array([ct * cp, ct * sp, -st])
@@ -79,7 +80,13 @@ def tdi_x_time_domain(t, chirp, c_plus, c_cross, theta, phi, L):
         hp_r, hc_r = chirp.h(tt - (k @ pr) / C, c_plus, c_cross)
         return (xi_p * (hp_s - hp_r) + xi_c * (hc_s - hc_r)) / (2.0 * (1.0 - kn))
 
-    # spacecraft indices 0,1,2 <-> 1,2,3;  y_sr: photon leaves s, arrives at r
-    x = (link(2, 0, t) + link(0, 2, t - Lc) + link(1, 0, t - 2 * Lc) + link(0, 1, t - 3 * Lc)
-         - link(1, 0, t) - link(0, 1, t - Lc) - link(2, 0, t - 2 * Lc) - link(0, 2, t - 3 * Lc))
+    # spacecraft indices 0,1,2 <-> 1,2,3;  y_sr: photon leaves s, arrives at r.  For X: a = 0, b = 1, c = 2
+    a, b, c = vertex, (vertex + 1) % 3, (vertex + 2) % 3
+    x = (link(c, a, t) + link(a, c, t - Lc) + link(b, a, t - 2 * Lc) + link(a, b, t - 3 * Lc)
+         - link(b, a, t) - link(a, b, t - Lc) - link(c, a, t - 2 * Lc) - link(a, c, t - 3 * Lc))
     return x
+
+
+def tdi_x_time_domain(t, chirp, c_plus, c_cross, theta, phi, L):
+    """X(t) from the four one-way links with explicit delays."""
+    return tdi_michelson_time_domain(t, chirp, c_plus, c_cross, theta, phi, L, 0)

@@ -60,7 +60,7 @@ def test_default_options(fs):
     assert o.f_ref_e0 == 0.01 and o.arm_length_m == 2.5e9
     assert o.orbit_kappa == 0.0 and o.orbit_lambda == 0.0
     assert o.device == -1 and o.inputs_on_device == 0 and o.max_segment_bins == 0
-    assert o.force_level == -2 and o.interp_tol == 1.0
+    assert o.force_level == -2 and o.interp_tol == 1.0 and o.tdi_channel == fs.TDI_CHANNELS["X"]
 
 
 def test_status_strings(fs):

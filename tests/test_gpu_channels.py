@@ -102,6 +102,100 @@ def test_first_stage_two_channels_sample(fs, orc):
     _compare(orc, chans, edges, par[sample], F[sample], Fk[sample])
 
 
+# ------------------------------------------------------------------------------------------ A, E, T (reading A28)
+def _aet_channels(orc, cfg, names, snr=None):
+    """One data set per TDI combination: its own noise PSD (synthetic.psd_tdi), noise seed, and the injection seen
+    through its own response (the oracle's template with tdi_channel set)."""
+    out = []
+    for c, name in enumerate(names):
+        o = orc.default_options(tdi_channel=orc.TDI_CHANNELS[name])
+        ds = syn.make_dataset(dataclasses.replace(cfg, noise_seed=70 + c), lambda p, f, o=o: orc.template(p, f, o),
+                              channel=name, snr=snr)
+        out.append((ds, o, name))
+    return out
+
+
+def _gpu_named(fs, chans, edges, par, **opt_kw):
+    import torch
+    plans = []
+    try:
+        for ds, _, name in chans:
+            o = fs.fstat_default_options(tdi_channel=fs.TDI_CHANNELS[name], **opt_kw)
+            plans.append(fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, o))
+        p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+        F, Fk = fs.fstat_eval_batch_channels(plans, p)
+        torch.cuda.synchronize()
+        return F.cpu().numpy(), Fk.cpu().numpy()
+    finally:
+        for pl in plans:
+            fs.fstat_plan_destroy(pl)
+
+
+@pytest.mark.parametrize("names", ["Y", "Z", "A", "E", "T", "AET", "XYZ"])
+def test_tiny_every_channel_and_the_aet_sum_every_F_and_Fk(fs, orc, names):
+    """Every TDI combination the library templates, alone and (A, E, T: the set with independent noise)
+    summed as in Eq. 3, on config 0 through the direct kernel: every F and F_k against the oracle."""
+    cfg = syn.CONFIGS[0]
+    chans = _aet_channels(orc, cfg, names)
+    par = syn.draw_particles(cfg).copy()
+    par[9, 2] = 0.3                                        # one invalid particle flies
+    edges = chans[0][0].edges(4)
+    F, Fk = _gpu_named(fs, chans, edges, par)
+    _compare(orc, [(ds, o) for ds, o, _ in chans], edges, par, F, Fk)
+
+
+def test_aet_templates_match_the_oracle_bin_by_bin(fs, orc):
+    import torch
+    cfg = syn.CONFIGS[0]
+    ds = syn.make_dataset(cfg, None)
+    par = syn.draw_particles(cfg)
+    for name in "YZAET":
+        with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1),
+                                  fs.fstat_default_options(tdi_channel=fs.TDI_CHANNELS[name])) as plan:
+            for p in (3, 40):
+                up_o, uc_o = orc.template(par[p], ds.freq, orc.default_options(tdi_channel=orc.TDI_CHANNELS[name]))
+                up_g, uc_g = fs.fstat_eval_template(plan, par[p])
+                scale = max(np.abs(up_o).max(), np.abs(uc_o).max())
+                assert np.abs(up_g.cpu().numpy() - up_o).max() <= 1e-7 * scale, name
+                assert np.abs(uc_g.cpu().numpy() - uc_o).max() <= 1e-7 * scale, name
+
+
+def test_fine_slice_aet_through_the_interpolating_kernel(fs, orc):
+    """A 2.5-yr slice, A + E + T, every F and F_k: the interpolating kernel with the A / E / T response at its nodes
+    against the oracle, and against the direct kernel."""
+    year = syn.YEAR_S
+    cfg = syn.Config(18, "aet_slice", 2.5 * year, 0.0200, 0.0202, (8,), (96,), 3.5 * year, "wide")
+    chans = _aet_channels(orc, cfg, "AET")
+    par = syn.draw_particles(cfg)
+    edges = chans[0][0].edges(8)
+    F, Fk = _gpu_named(fs, chans, edges, par)
+    _compare(orc, [(ds, o) for ds, o, _ in chans], edges, par, F, Fk)
+    F_d, Fk_d = _gpu_named(fs, chans, edges, par, force_level=-1)
+    assert np.max(np.abs(Fk - Fk_d) / np.abs(Fk_d)) <= 5e-6
+
+
+def test_first_stage_aet_sample(fs, orc):
+    """Config 1 at full size (N_p = 1024, P = 2048) with A + E + T; a sample of particles against the oracle."""
+    cfg = syn.CONFIGS[1]
+    chans = _aet_channels(orc, cfg, "AET")
+    par = syn.draw_particles(cfg)
+    edges = chans[0][0].edges(1024)
+    F, Fk = _gpu_named(fs, chans, edges, par)
+    sample = np.array([0, 167, 511, 1024, 1598, 2047])
+    _compare(orc, [(ds, o) for ds, o, _ in chans], edges, par[sample], F[sample], Fk[sample])
+
+
+def test_bands_refuse_aet_plans(fs, orc):
+    import torch
+    cfg = syn.CONFIGS[0]
+    ds = syn.make_dataset(cfg, None)
+    par = torch.as_tensor(syn.draw_particles(cfg), device="cuda")
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1), fs.fstat_default_options(tdi_channel=3)) as plan:
+        with pytest.raises(fs.FstatError) as ei:
+            fs.fstat_eval_batch_bands(plan, par, 4, 1)
+        assert ei.value.status == 4
+
+
 def test_mismatching_plans_are_rejected(fs, orc):
     import torch
     cfg = syn.CONFIGS[0]

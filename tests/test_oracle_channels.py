@@ -107,3 +107,102 @@ def test_one_channel_is_the_single_channel_statistic_and_noise_stays_chi2(orc):
     _, Fk3 = orc.fstat_batch_channels(f, chans, edges, par)
     m = 2.0 * Fk3.mean()
     assert 4.0 - 0.9 < m < 4.0 + 0.9                       # 256 correlated-ish draws: loose, a factor-of-N_I slip fails
+
+
+# ----------------------------------------------------------------------------- P19: Y, Z, A, E, T responses
+def _resp(orc, par, f, t, ch, **kw):
+    return np.array(orc.response(par, f, t, orc.default_options(tdi_channel=orc.TDI_CHANNELS[ch], **kw)))
+
+
+def test_p19_y_and_z_are_x_of_the_relabelled_constellation(orc):
+    """Y and Z as the oracle builds them (Michelson centred on spacecraft 2, 3) equal the pinned X response of the
+    constellation with its spacecraft relabelled cyclically (orbit_lambda + 2 pi/3, + 4 pi/3: P14)."""
+    rng = np.random.default_rng(19)
+    for _ in range(20):
+        par = np.array([0.0, 30.0, 0.25, math.acos(rng.uniform(-1, 1)), rng.uniform(0, 2 * math.pi), 0.0])
+        f, t, lam = rng.uniform(1e-3, 0.1), rng.uniform(0, 3 * syn.YEAR_S), rng.uniform(-1, 1)
+        for ch, shift in (("Y", 2.0 * math.pi / 3.0), ("Z", 4.0 * math.pi / 3.0)):
+            a = _resp(orc, par, f, t, ch, orbit_lambda=lam)
+            b = _resp(orc, par, f, t, "X", orbit_lambda=lam + shift)
+            assert np.max(np.abs(a - b)) <= 1e-12 * np.max(np.abs(b))
+
+
+def test_p19_aet_are_the_combinations_of_ref_64(orc):
+    """A = (Z - X)/sqrt 2, E = (X - 2Y + Z)/sqrt 6, T = (X + Y + Z)/sqrt 3 (reading A28), and the long-wavelength
+    behaviour that makes T the 'null' channel: for f << c / (2 pi L) = 19 mHz the gravitational-wave response of
+    X + Y + Z cancels at leading order."""
+    par = np.array([0.0, 30.0, 0.25, 1.1, 2.3, 0.0])
+    t = 0.37 * syn.YEAR_S
+    ratio = {}
+    for f in (1e-4, 1e-3, 2e-2):
+        X, Y, Z = (_resp(orc, par, f, t, c) for c in "XYZ")
+        A, E, T = (_resp(orc, par, f, t, c) for c in "AET")
+        np.testing.assert_allclose(A, (Z - X) / math.sqrt(2.0), rtol=1e-13, atol=1e-16 * abs(X).max())
+        np.testing.assert_allclose(E, (X - 2.0 * Y + Z) / math.sqrt(6.0), rtol=1e-13, atol=1e-16 * abs(X).max())
+        np.testing.assert_allclose(T, (X + Y + Z) / math.sqrt(3.0), rtol=1e-13, atol=1e-14 * abs(X).max())
+        ratio[f] = np.abs(T).max() / np.abs(A).max()
+    # leading order cancels identically (xi is symmetric in the arm direction: sum_v [xi_(v,v+2) - xi_(v,v+1)] = 0),
+    # so T / A falls at least like (f / 19 mHz)^2 towards low frequencies
+    assert ratio[1e-4] < 1e-6 and ratio[1e-3] < 1e-3 and ratio[2e-2] > 1e-2
+    assert ratio[1e-3] / ratio[1e-4] > 90.0
+
+
+def test_p19_aet_frequency_domain_response_matches_time_domain_simulation(orc):
+    """The P9 check for the A and E templates: X(t), Y(t), Z(t) simulated in the time domain (explicit link delays,
+    Keplerian orbits, tests/td_sim.py), combined into A(t), E(t), T(t), Fourier transformed and compared as complex
+    overlaps with x~(f) = T_I(f) h~(f) of Eq. 17.  T carries little signal below 30 mHz: its amplitude is checked
+    instead of its phase-sensitive overlap to the same level."""
+    import td_sim
+    from scipy.signal.windows import tukey
+    L = 2.5e9
+    YR = syn.YEAR_S
+    par = np.array([1.6 * YR, 40.0, 0.24, 1.1, 2.3, 0.03])
+    dt, N = 16.0, 2 ** 20
+    T_obs = N * dt
+    fg = np.linspace(0.015, 0.03, 12001)
+    pt = np.array([orc.phase(par, f) for f in fg])
+    sel = (pt[:, 1] > -0.03 * YR) & (pt[:, 1] < T_obs + 0.03 * YR)
+    chirp = td_sim.Chirp(fg[sel], pt[sel, 0], pt[sel, 1])
+    cp, cc = 0.8 * np.exp(0.3j), 0.5 * np.exp(-1.1j)
+    t = np.arange(N) * dt
+    xyz = [td_sim.tdi_michelson_time_domain(t, chirp, cp, cc, par[3], par[4], L, v) for v in range(3)]
+    td = {"A": (xyz[2] - xyz[0]) / math.sqrt(2.0), "E": (xyz[0] - 2.0 * xyz[1] + xyz[2]) / math.sqrt(6.0),
+          "T": (xyz[0] + xyz[1] + xyz[2]) / math.sqrt(3.0)}
+    fk = np.arange(N // 2 + 1) / T_obs
+    tf_k = np.interp(fk, fg, pt[:, 1])
+    band = (tf_k > 0.25 * T_obs) & (tf_k < 0.75 * T_obs)
+    assert band.sum() > 20000
+    power = {}
+    for ch in "AET":
+        X = (np.fft.rfft(td[ch] * tukey(N, 0.2)) * dt)[band]
+        up, uc = orc.template(par, fk[band], orc.default_options(tdi_channel=orc.TDI_CHANNELS[ch]))
+        Xfd = cp * up + cc * uc
+        overlap = np.sum(X * np.conj(Xfd)) / math.sqrt(np.sum(abs(X) ** 2) * np.sum(abs(Xfd) ** 2))
+        power[ch] = (np.sum(abs(X) ** 2), np.sum(abs(Xfd) ** 2))
+        if ch in "AE":
+            assert overlap.real > 0.999 and abs(overlap.imag) < 0.03, (ch, overlap)
+        assert math.sqrt(power[ch][0] / power[ch][1]) == pytest.approx(1.0, abs=2e-2), ch
+    assert power["T"][1] < 0.2 * power["A"][1]
+
+
+def test_p19_aet_channel_sum_recovers_the_network_snr(orc):
+    """Zero noise, one signal seen in A, E and T with one amplitude vector: 2F over the three channels = the sum of
+    the three <h_I, h_I> (Eq. 3 :62); a single channel recovers only its share."""
+    cfg = syn.CONFIGS[0]
+    _, n, f = syn.frequency_grid(cfg.T, cfg.f_lo, cfg.f_hi)
+    par = syn.injection_params(cfg)
+    a = syn.injection_amplitudes()
+    edges = syn.equal_bin_edges(n, 4)
+    df = 1.0 / cfg.T
+    chans, snr2 = [], 0.0
+    sn = syn.psd_tdi_x(f)                                   # any positive weight will do for this identity
+    for ch in "AET":
+        o = orc.default_options(tdi_channel=orc.TDI_CHANNELS[ch])
+        up, uc = orc.template(par, f, o)
+        h = (a[0] + 1j * a[2]) * up + (a[1] + 1j * a[3]) * uc
+        snr2 += 4.0 * df * float(np.sum(np.abs(h) ** 2 / sn))
+        chans.append((h / sn, 1.0 / sn, o))
+    F, Fk = orc.fstat_batch_channels(f, chans, edges, par[None, :])
+    assert 2.0 * F[0] == pytest.approx(snr2, rel=1e-9)
+    F1, _ = orc.fstat_batch_channels(f, chans[:1], edges, par[None, :])
+    assert 0.0 < 2.0 * F1[0] < 0.9 * snr2

@@ -163,7 +163,7 @@ def test_taylor_t2_series_typed_here_are_mutually_consistent():
 # ------------------------------------------------------------------ the pins bite: corrupted scratch copies
 class _Opt(C.Structure):
     _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double), ("orbit_kappa", C.c_double),
-                ("orbit_lambda", C.c_double)]
+                ("orbit_lambda", C.c_double), ("tdi_channel", C.c_int32)]
 
 
 def _compile_phase(src_text, workdir, tag):
@@ -179,7 +179,7 @@ def _compile_phase(src_text, workdir, tag):
 
     def phase(par, f, f_ref=0.01):
         par = np.ascontiguousarray(par, dtype=np.float64)
-        o = _Opt(f_ref, 2.5e9, 0.0, 0.0)
+        o = _Opt(f_ref, 2.5e9, 0.0, 0.0, 0)
         psi, tf = C.c_double(), C.c_double()
         lib.oracle_phase(par.ctypes.data_as(C.POINTER(C.c_double)), float(f), C.byref(o), C.byref(psi), C.byref(tf))
         return psi.value, tf.value
