@@ -206,6 +206,29 @@ FSTAT_API fstat_status fstat_eval_amplitudes(fstat_plan *plan, int64_t P, const 
                                              void *cuda_stream);
 
 /*
+ * fstat_extrinsic_from_amplitudes -- App. B (Eq. B2-B3 :426-440): the maximum-likelihood extrinsic
+ * parameters from ONE amplitude vector a = M^-1 N (fstat_eval_amplitudes / _bands at the best intrinsic point, N_p = 1).
+ * Plain host arithmetic, no device, no plan.
+ *   a               HOST [4]: a_1..a_4.
+ *   chirp_mass_msun > 0: `a` are the library's amplitudes, whose templates drop the amplitude constant of Eq. A2 (:402,
+ *                   reading A21); it is restored and D_L comes out in metres.  <= 0: `a` are the paper's a_i and D_L
+ *                   comes out in their inverse units.
+ *   out             HOST [4]: D_L, iota, psi, phi_c.  iota in [0, pi]; psi in (-pi/4, pi/4] (the branch of the paper's
+ *                   arctan); phi_c in (-pi, pi]: the paper's arctan plus the half-plane that reproduces the sign of the
+ *                   amplitudes (reading A25).  All-zero amplitudes give D_L = +inf and zeros.
+ * D_L rests on the absolute normalisation of the library's response (link factor -i pi f L/c, TDI factor 1 - z^2, reading
+ * A7), which is pinned against a time-domain simulation of the links (amplitude ratio within 5e-3, pin P9), and on the
+ * amplitude / polarisation conventions behind Eq. B1, which the paper does not print (its ref. [89]): treat D_L as
+ * relative to this library's normalisation; iota is free of both.
+ * Errors: EINVAL (NULL pointer, non-finite input).
+ */
+FSTAT_API fstat_status fstat_extrinsic_from_amplitudes(const double *a, double chirp_mass_msun, double *out);
+
+/* Eq. B1 (:413-420), the forward map: a_out HOST [4] = a_1..a_4 of (D_L, psi, iota, phi_c), D_L > 0 in the inverse units of
+ * the amplitudes.  EINVAL for a NULL pointer, D_L <= 0 or non-finite input. */
+FSTAT_API fstat_status fstat_amplitudes_from_extrinsic(double d_l, double psi, double iota, double phi_c, double *a_out);
+
+/*
  * fstat_eval_batch_host -- the same evaluation with HOST buffers: copies params to the device,
  * evaluates, copies F (and Fk when non-NULL) back and waits for completion before returning.
  * Pinned host memory makes the copies asynchronous DMA; pageable memory works too.

@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = (
     "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_amplitudes_bands", "fstat_eval_batch_channels", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
-    "fstat_status_str", "fstat_last_error",
+    "fstat_status_str", "fstat_last_error", "fstat_extrinsic_from_amplitudes", "fstat_amplitudes_from_extrinsic",
     "fstat_pso_default_options", "fstat_pso_create", "fstat_pso_iterate", "fstat_pso_best", "fstat_pso_state",
     "fstat_pso_iterations_done", "fstat_pso_destroy",
 )
@@ -121,6 +121,10 @@ def load_library():
         L.fstat_pso_iterations_done.restype = i32
         L.fstat_pso_destroy.argtypes = [vp]
         L.fstat_pso_destroy.restype = None
+        L.fstat_extrinsic_from_amplitudes.argtypes = [dp, C.c_double, dp]
+        L.fstat_extrinsic_from_amplitudes.restype = C.c_int
+        L.fstat_amplitudes_from_extrinsic.argtypes = [C.c_double] * 4 + [dp]
+        L.fstat_amplitudes_from_extrinsic.restype = C.c_int
         L.fstat_status_str.argtypes = [C.c_int]
         L.fstat_status_str.restype = C.c_char_p
         L.fstat_last_error.argtypes = [vp]

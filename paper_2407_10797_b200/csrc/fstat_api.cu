@@ -16,6 +16,18 @@
 
 using namespace fstat;
 
+// Segment tables of one segment length (they depend on the partitions, the options and the segment length only):
+// kept per plan in a small cache, so that batches of different sizes -- a ragged last batch, swarms that shrink --
+// neither rebuild nor re-upload anything, and no evaluation has to wait for the device.
+struct SegTables {
+    int64_t seg_len = 0;
+    int32_t n_seg = 0;
+    int32_t *d_seg_edge = nullptr, *d_part_seg = nullptr, *d_seg_gbase = nullptr;
+    SegCrit *d_seg_crit = nullptr;
+    int8_t *d_seg_maxlvl = nullptr;
+    std::vector<int32_t> seg_edge_h;
+};
+
 struct fstat_plan {
     int device = 0;
     int n_sm = 0;
@@ -40,13 +52,14 @@ struct fstat_plan {
     int32_t seg_groups = -1;           // n_groups the current segmentation was made for
     int32_t n_seg = 0;
     int32_t seg_len = 0;               // bins per work segment of the current segmentation (aligned cuts)
+    std::vector<SegTables> seg_cache;  // one entry per segment length seen since the partitions were set (<= 8)
+    // the entry in use (aliases into seg_cache):
     int32_t *d_seg_edge = nullptr;     // [n_seg+1]
     int32_t *d_part_seg = nullptr;     // [n_part+1]
-    size_t seg_cap = 0, part_cap = 0;
     std::vector<int32_t> seg_edge_h;   // host copy of d_seg_edge
-    int32_t *d_seg_gbase = nullptr; size_t gbase_cap = 0;  // [n_seg][kNLevels]
-    SegCrit *d_seg_crit = nullptr; size_t crit_cap = 0;    // [n_seg]
-    int8_t *d_seg_maxlvl = nullptr; size_t maxlvl_cap = 0; // [n_seg]
+    int32_t *d_seg_gbase = nullptr;    // [n_seg][kNLevels]
+    SegCrit *d_seg_crit = nullptr;     // [n_seg]
+    int8_t *d_seg_maxlvl = nullptr;    // [n_seg]
     int8_t *d_level = nullptr; size_t level_cap = 0;       // [n_groups][n_seg] of the most recent evaluation
     int32_t *d_direct = nullptr; size_t direct_cap = 0;    // [1 + n_groups * n_seg]: count, then the work list
     int64_t n_launches = 0;                                 // kernels launched by evaluations so far
@@ -56,6 +69,7 @@ struct fstat_plan {
     double *d_coef = nullptr;  size_t coef_cap = 0;      // doubles
     int32_t *d_valid = nullptr; size_t valid_cap = 0;    // ints
     int32_t *d_slot = nullptr; size_t slot_cap = 0;      // [P] particle -> slot (sorted by chirp mass)
+    unsigned char *d_sort = nullptr; size_t sort_cap = 0; // scratch of the slot ranking (keys, radix sort buffers)
     int32_t *d_perm = nullptr; size_t perm_cap = 0;      // [P_pad] slot -> particle (-1: padding)
     double *d_partial = nullptr; size_t partial_cap = 0; // doubles
     // row f2 (fstat_eval_batch_bands)
@@ -220,12 +234,43 @@ SegCrit make_seg_crit(double f_lo, double f_hi, double df, double part_len)
     return q;
 }
 
+void free_seg_tables(SegTables &t)
+{
+    cudaFree(t.d_seg_edge); cudaFree(t.d_part_seg); cudaFree(t.d_seg_gbase); cudaFree(t.d_seg_crit); cudaFree(t.d_seg_maxlvl);
+    t = SegTables();
+}
+
+// Drop every cached segmentation (the partitions or the segment-length option changed).  Earlier evaluations may still
+// read the tables: wait for the device first.
+void invalidate_segments(fstat_plan *pl)
+{
+    if (!pl->seg_cache.empty()) cudaDeviceSynchronize();
+    for (SegTables &t : pl->seg_cache) free_seg_tables(t);
+    pl->seg_cache.clear();
+    pl->seg_groups = -1;
+    pl->d_seg_edge = pl->d_part_seg = pl->d_seg_gbase = nullptr;
+    pl->d_seg_crit = nullptr;
+    pl->d_seg_maxlvl = nullptr;
+}
+
+void use_seg_tables(fstat_plan *pl, const SegTables &t, int32_t n_groups)
+{
+    pl->d_seg_edge = t.d_seg_edge; pl->d_part_seg = t.d_part_seg; pl->d_seg_gbase = t.d_seg_gbase;
+    pl->d_seg_crit = t.d_seg_crit; pl->d_seg_maxlvl = t.d_seg_maxlvl;
+    pl->seg_edge_h = t.seg_edge_h;
+    pl->n_seg = t.n_seg;
+    pl->seg_len = (int32_t)(t.seg_len < pl->n_bins ? t.seg_len : pl->n_bins);
+    pl->seg_groups = n_groups;
+}
+
 fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
 {
     if (pl->seg_groups == n_groups) return FSTAT_OK;
+    const int64_t seg_len = auto_segment_len(pl, n_groups);
+    for (const SegTables &t : pl->seg_cache)
+        if (t.seg_len == seg_len) { use_seg_tables(pl, t, n_groups); return FSTAT_OK; }
     std::vector<int32_t> seg_edge, part_seg;
     const bool aligned = segments_aligned(pl);
-    const int64_t seg_len = auto_segment_len(pl, n_groups);
     make_segments(pl->edges, seg_len, aligned, &seg_edge, &part_seg);
     const size_t n_seg = seg_edge.size() - 1;
     std::vector<int32_t> gbase(n_seg * kNLevels);
@@ -247,22 +292,29 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
                                       (double)(pl->edges[k + 1] - pl->edges[k]));
             maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && segments_fast_capable(pl) && hi - lo >= 8) ? kNLevels - 1 : -1);
         }
-    CU_TRY(pl, grow(&pl->d_seg_edge, &pl->seg_cap, seg_edge.size()));
-    CU_TRY(pl, grow(&pl->d_part_seg, &pl->part_cap, part_seg.size()));
-    CU_TRY(pl, grow(&pl->d_seg_gbase, &pl->gbase_cap, gbase.size()));
-    CU_TRY(pl, grow(&pl->d_seg_crit, &pl->crit_cap, crit.size()));
-    CU_TRY(pl, grow(&pl->d_seg_maxlvl, &pl->maxlvl_cap, maxlvl.size()));
-    // synchronous copies: they order after any earlier evaluation that still reads the old arrays
-    CU_TRY(pl, cudaDeviceSynchronize());
-    CU_TRY(pl, cudaMemcpy(pl->d_seg_edge, seg_edge.data(), seg_edge.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-    CU_TRY(pl, cudaMemcpy(pl->d_part_seg, part_seg.data(), part_seg.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-    CU_TRY(pl, cudaMemcpy(pl->d_seg_gbase, gbase.data(), gbase.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-    CU_TRY(pl, cudaMemcpy(pl->d_seg_crit, crit.data(), crit.size() * sizeof(SegCrit), cudaMemcpyHostToDevice));
-    CU_TRY(pl, cudaMemcpy(pl->d_seg_maxlvl, maxlvl.data(), maxlvl.size() * sizeof(int8_t), cudaMemcpyHostToDevice));
-    pl->seg_edge_h = seg_edge;
-    pl->n_seg = (int32_t)n_seg;
-    pl->seg_len = (int32_t)(seg_len < pl->n_bins ? seg_len : pl->n_bins);
-    pl->seg_groups = n_groups;
+    if (pl->seg_cache.size() >= 8) {                       // (a ninth segment length: start over)
+        const int32_t keep = pl->seg_groups;
+        invalidate_segments(pl);
+        (void)keep;
+    }
+    // fresh arrays: no kernel in flight reads them, so the blocking copies below order nothing but themselves
+    SegTables t;
+    t.seg_len = seg_len;
+    t.n_seg = (int32_t)n_seg;
+    cudaError_t e = cudaMalloc((void **)&t.d_seg_edge, seg_edge.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&t.d_part_seg, part_seg.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&t.d_seg_gbase, gbase.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&t.d_seg_crit, crit.size() * sizeof(SegCrit));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&t.d_seg_maxlvl, maxlvl.size() * sizeof(int8_t));
+    if (e == cudaSuccess) e = cudaMemcpy(t.d_seg_edge, seg_edge.data(), seg_edge.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t.d_part_seg, part_seg.data(), part_seg.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t.d_seg_gbase, gbase.data(), gbase.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t.d_seg_crit, crit.data(), crit.size() * sizeof(SegCrit), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t.d_seg_maxlvl, maxlvl.data(), maxlvl.size() * sizeof(int8_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { free_seg_tables(t); CU_TRY(pl, e); }
+    t.seg_edge_h = seg_edge;
+    pl->seg_cache.push_back(t);
+    use_seg_tables(pl, pl->seg_cache.back(), n_groups);
     return FSTAT_OK;
 }
 
@@ -467,13 +519,14 @@ static void plan_free(fstat_plan *pl)
     DeviceGuard g(pl->device);
     if (pl->bandplan) { plan_free(pl->bandplan); pl->bandplan = nullptr; }
     if (pl->shares_tables) { pl->d_table = nullptr; pl->d_dwp = nullptr; pl->d_w = nullptr; pl->d_node = nullptr; }
-    cudaFree(pl->d_table); cudaFree(pl->d_seg_edge); cudaFree(pl->d_part_seg); cudaFree(pl->d_coef);
+    for (SegTables &t : pl->seg_cache) free_seg_tables(t);
+    cudaFree(pl->d_table); cudaFree(pl->d_coef);
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
     cudaFree(pl->d_dwp); cudaFree(pl->d_w); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) { cudaFree(pl->d_gram[l]); cudaFree(pl->d_pgram[l]); }
     cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_err); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out);
-    cudaFree(pl->d_seg_gbase); cudaFree(pl->d_seg_crit); cudaFree(pl->d_seg_maxlvl); cudaFree(pl->d_level);
-    cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm);
+    cudaFree(pl->d_level);
+    cudaFree(pl->d_fpart); cudaFree(pl->d_direct); cudaFree(pl->d_slot); cudaFree(pl->d_perm); cudaFree(pl->d_sort);
     for (int i = 0; i < fstat_plan::kRing; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
@@ -541,9 +594,9 @@ fstat_status fstat_plan_set_partitions(fstat_plan *pl, int32_t n_part, const int
         return fail(pl, FSTAT_ENOMEM, "host allocation failed");
     }
     pl->n_part = n_part;
-    pl->seg_groups = -1;    // re-segment on the next evaluation
     DeviceGuard g(pl->device);
     if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    invalidate_segments(pl);    // re-segment on the next evaluation
     return build_gram_tables(pl);
 }
 
@@ -636,8 +689,9 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
 
     CU_TRY(pl, grow(&pl->d_slot, &pl->slot_cap, (size_t)P));
     CU_TRY(pl, grow(&pl->d_perm, &pl->perm_cap, (size_t)P_pad));
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, nullptr, pl->d_coef,
-                               pl->d_valid, pl->d_perm, st));
+    CU_TRY(pl, grow(&pl->d_sort, &pl->sort_cap, prologue_scratch_bytes(P)));
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, pl->d_slot, nullptr, pl->d_sort,
+                               pl->d_coef, pl->d_valid, pl->d_perm, st));
     BandSched bs{};
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
                                pl->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
@@ -682,7 +736,8 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     CU_TRY(pl, launch_main(a, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;
-    pl->n_launches += 4 + (pl->fast_ok ? 1 : 0);     // rank, prologue, stride selection, [interpolating], direct
+    // keys, rank (or radix sort: counted as one), prologue, stride selection, [interpolating], direct
+    pl->n_launches += 5 + (pl->fast_ok ? 1 : 0);
     pl->last_was_band = false;
     if (F) {
         PartialSet one{};
@@ -808,7 +863,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     fstat_status s = ensure_band_plan(pl);
     if (s != FSTAT_OK) return s;
     fstat_plan *cp = pl->bandplan;
-    if (cp->opt.max_segment_bins != pl->opt.max_segment_bins) cp->seg_groups = -1;
+    if (cp->opt.max_segment_bins != pl->opt.max_segment_bins) invalidate_segments(cp);
     cp->opt = pl->opt;
     const bool fast = cp->fast_ok && pl->opt.force_level != -1 && segments_fast_capable(cp);
     if (fast) {
@@ -846,8 +901,9 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
 
     // slots ranked by the position of the band (not by chirp mass): the 128 templates of a CTA overlap at both ends
     const double rank_band[3] = {1.0 / pl->df, pl->f0, pl->f0 + (double)(pl->n_bins - 1) * pl->df};
-    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, cp->d_slot, rank_band, cp->d_coef,
-                               cp->d_valid, cp->d_perm, st));
+    CU_TRY(pl, grow(&cp->d_sort, &cp->sort_cap, prologue_scratch_bytes(P)));
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, cp->d_slot, rank_band, cp->d_sort,
+                               cp->d_coef, cp->d_valid, cp->d_perm, st));
     CU_TRY(pl, launch_band_limits(pl->d_table, cp->d_coef, cp->d_valid, cp->d_perm, P_pad, (int32_t)pl->n_bins,
                                   1.0 / pl->df, pl->opt.orbit_kappa, cp->d_band, cp->d_band + P_pad, band, st));
     BandSched bs{};
@@ -911,8 +967,8 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     ++pl->n_timed;
     CU_TRY(pl, launch_band_short(pl->d_table, cp->d_coef, bc, P_pad, pl->orb, st));
     CU_TRY(pl, launch_band_stitch(bc, P, P_pad, cp->seg_len, cp->n_seg, F, st));
-    // rank, prologue, band limits, stride selection, [interpolating], direct, short partitions, stitch, F sums
-    pl->n_launches += 8 + (fast ? 1 : 0);
+    // keys, rank, prologue, band limits, stride selection, [interpolating], direct, short partitions, stitch, F sums
+    pl->n_launches += 9 + (fast ? 1 : 0);
     pl->last_was_band = true;
     return FSTAT_OK;
 }
@@ -1001,8 +1057,8 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
     CU_TRY(pl, grow(&pl->d_coef, &pl->coef_cap, (size_t)kThreads * kNCoef));
     CU_TRY(pl, grow(&pl->d_valid, &pl->valid_cap, (size_t)kThreads));
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
-    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, nullptr, pl->d_coef,
-                               pl->d_valid, nullptr, st));
+    CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, nullptr, nullptr,
+                               pl->d_coef, pl->d_valid, nullptr, st));
     CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0,
                                u_plus, u_cross, st));
     CU_TRY(pl, cudaStreamSynchronize(st));
@@ -1051,6 +1107,65 @@ fstat_status fstat_probe_pipe_peak(int32_t device, int32_t which, double millis,
     cudaFree(sink);
     *inst_per_s = best;
     return rc;
+}
+
+
+/* ---- App. B: host arithmetic on one amplitude vector, no device involved ---- */
+
+// Eq. B1 (:413-420): the four amplitudes of (D_L, psi, iota, phi_c), D_L in the inverse units of the amplitudes
+static void b1_forward(double d_l, double psi, double iota, double phi_c, double a[4])
+{
+    const double ci = cos(iota), p = 0.5 * (1.0 + ci * ci);
+    const double c2 = cos(2.0 * psi), s2 = sin(2.0 * psi), cp = cos(phi_c), sp = sin(phi_c);
+    a[0] = (c2 * p * cp - s2 * ci * sp) / d_l;
+    a[1] = -(s2 * p * cp + c2 * ci * sp) / d_l;
+    a[2] = -(c2 * p * sp + s2 * ci * cp) / d_l;
+    a[3] = (s2 * p * sp - c2 * ci * cp) / d_l;
+}
+
+fstat_status fstat_amplitudes_from_extrinsic(double d_l, double psi, double iota, double phi_c, double *a_out)
+{
+    if (!a_out || !(d_l > 0.0) || !isfinite(d_l) || !isfinite(psi) || !isfinite(iota) || !isfinite(phi_c))
+        return FSTAT_EINVAL;
+    b1_forward(d_l, psi, iota, phi_c, a_out);
+    return FSTAT_OK;
+}
+
+fstat_status fstat_extrinsic_from_amplitudes(const double *a, double chirp_mass_msun, double *out)
+{
+    if (!a || !out) return FSTAT_EINVAL;
+    double a1 = a[0], a2 = a[1], a3 = a[2], a4 = a[3];
+    if (!isfinite(a1) || !isfinite(a2) || !isfinite(a3) || !isfinite(a4) || !isfinite(chirp_mass_msun)) return FSTAT_EINVAL;
+    if (chirp_mass_msun > 0.0) {
+        // the templates drop the amplitude constant of Eq. A2 (:402, reading A21): library amplitude = K_A x the
+        // paper's a_i with D_L in seconds, K_A = -sqrt(5/24) (G M_c / c^3)^(5/6) / pi^(2/3)
+        const double k = -sqrt(5.0 / 24.0) * pow(chirp_mass_msun * kGMsunC3, 5.0 / 6.0) / pow(kPi, 2.0 / 3.0);
+        a1 /= k; a2 /= k; a3 /= k; a4 /= k;
+    }
+    const double r_plus = hypot(a1 + a4, a2 - a3), r_minus = hypot(a1 - a4, a2 + a3);
+    const double A_plus = r_plus + r_minus, A_cross = r_plus - r_minus;        // Eq. B3
+    const double root = 2.0 * sqrt(r_plus * r_minus);                          // sqrt(A_+^2 - A_x^2), without the cancellation
+    const double A = A_plus + root;
+    if (!(A > 0.0)) { out[0] = INFINITY; out[1] = 0.0; out[2] = 0.0; out[3] = 0.0; return FSTAT_OK; }
+    double r = -A_cross / A;
+    r = r < -1.0 ? -1.0 : (r > 1.0 ? 1.0 : r);
+    const double iota = acos(r);                                               // Eq. B2
+    const double num = A_plus * a4 - A_cross * a1;
+    const double den_psi = -(A_cross * a2 + A_plus * a3);
+    const double psi = 0.5 * (den_psi != 0.0 ? atan(num / den_psi) : copysign(kPi / 2.0, num));
+    const double c = sin(2.0 * psi) >= 0.0 ? 1.0 : -1.0;
+    const double den = -c * (A_cross * a3 + A_plus * a2);
+    double phi_c = den != 0.0 ? atan(c * num / den) : copysign(kPi / 2.0, c * num);
+    // Eq. B2's arctan fixes phi_c only modulo pi, and phi_c -> phi_c + pi flips the sign of all four a_i in Eq. B1:
+    // the half-plane is the one that reproduces the sign of the amplitudes (reading A25)
+    double back[4];
+    b1_forward(2.0 / A, psi, iota, phi_c, back);
+    if (back[0] * a1 + back[1] * a2 + back[2] * a3 + back[3] * a4 < 0.0) phi_c = phi_c <= 0.0 ? phi_c + kPi : phi_c - kPi;
+    out[0] = (2.0 / A) * (chirp_mass_msun > 0.0 ? kC : 1.0);
+    out[1] = iota;
+    out[2] = psi;
+    out[3] = phi_c;
+    return FSTAT_OK;
 }
 
 }  // extern "C"

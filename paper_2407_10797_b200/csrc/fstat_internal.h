@@ -225,9 +225,11 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
 // rank_band: nullptr (slots ranked by chirp mass) or HOST {T_obs, f_first, f_last} (row f2: ranked by band)
+// scratch: prologue_scratch_bytes(P) bytes of device memory (keys and, for large batches, the radix sort's buffers)
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, const double *rank_band, double *coef, int32_t *valid, int32_t *perm,
-                            cudaStream_t st);
+                            int32_t *slot_of, const double *rank_band, void *scratch, double *coef, int32_t *valid,
+                            int32_t *perm, cudaStream_t st);
+size_t prologue_scratch_bytes(int64_t P);
 cudaError_t launch_main(const MainArgs &a, cudaStream_t st);
 // row f4 (Eq. 3 :62): the partial sums of up to kMaxChannels TDI channels, all with the same segment / slot layout
 constexpr int kMaxChannels = 4;

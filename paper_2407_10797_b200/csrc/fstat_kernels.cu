@@ -13,6 +13,7 @@
 #include "fstat_internal.h"
 #include "fstat_model.cuh"
 
+#include <cub/device/device_radix_sort.cuh>
 #include <math.h>
 
 namespace fstat {
@@ -133,9 +134,10 @@ __device__ __forceinline__ bool particle_ok(const double *__restrict__ q)
            (q[1] > 0.0) && (q[2] > 0.0) && (q[2] <= 0.25) && (q[5] >= 0.0);
 }
 
-// slot_of[i] = rank of particle i by (chirp mass rounded to float, index): a stable, deterministic sort by
-// brute force (P^2 integer comparisons through shared-memory tiles; ~1 ms at P = 65536, where one
-// evaluation takes ~200 ms).  Invalid particles sort last.
+// slot_of[i] = rank of particle i by (chirp mass rounded to float, index): a stable, deterministic order -- the keys
+// are computed once (rank_key_kernel), then ranked by brute force (P <= 16384: one launch of P^2 integer comparisons
+// through shared-memory tiles) or by a stable radix sort of (key, index) pairs (cub, larger batches: the same order).
+// Invalid particles sort last.
 // band_T > 0 (row f2; band_T = the observation time, [band_f0, band_f1] = the grid): the key is a weighted
 // mean of the Newtonian estimates of the template's frequencies at t = 0 and t = T, clipped to the grid,
 // f(t) = (1/pi) (5 / (256 (t_c - t)))^(3/8) (G M_c / c^3)^(-5/8), so that the bands of a group of 128 overlap
@@ -153,21 +155,28 @@ __device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, doubl
     return __float_as_uint((float)(0.4 * fa + 0.6 * fb));
 }
 
-__global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ params, int32_t P, double band_T, double band_f0,
-                                                   double band_f1,
+__global__ void __launch_bounds__(256) rank_key_kernel(const double *__restrict__ params, int32_t P, double band_T,
+                                                       double band_f0, double band_f1, uint32_t *__restrict__ keys,
+                                                       int32_t *__restrict__ index)
+{
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= P) return;
+    keys[i] = rank_key(params + 6 * (int64_t)i, band_T, band_f0, band_f1);
+    if (index != nullptr) index[i] = i;
+}
+
+// brute-force rank of the keys (P^2 integer comparisons through shared-memory tiles): one launch, for P <= kRankBrute
+__global__ void __launch_bounds__(256) rank_kernel(const uint32_t *__restrict__ keys, int32_t P,
                                                    int32_t *__restrict__ slot_of)
 {
     __shared__ uint32_t skey[256];
     const int i = blockIdx.x * 256 + threadIdx.x;
-    uint32_t my = 0xFFFFFFFFu;
-    if (i < P) my = rank_key(params + 6 * (int64_t)i, band_T, band_f0, band_f1);
+    const uint32_t my = i < P ? keys[i] : 0xFFFFFFFFu;
     int rank = 0;
     for (int j0 = 0; j0 < P; j0 += 256) {
         const int j = j0 + threadIdx.x;
-        uint32_t k = 0xFFFFFFFFu;
-        if (j < P) k = rank_key(params + 6 * (int64_t)j, band_T, band_f0, band_f1);
         __syncthreads();
-        skey[threadIdx.x] = k;
+        skey[threadIdx.x] = j < P ? keys[j] : 0xFFFFFFFFu;
         __syncthreads();
         const int n = min(256, P - j0);
         for (int t = 0; t < n; ++t) {
@@ -178,14 +187,58 @@ __global__ void __launch_bounds__(256) rank_kernel(const double *__restrict__ pa
     if (i < P) slot_of[i] = rank;
 }
 
+// slot_of[particle] = position of the particle in the list sorted by (key, index)
+__global__ void scatter_slots_kernel(const int32_t *__restrict__ sorted_index, int32_t P, int32_t *__restrict__ slot_of)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < P) slot_of[sorted_index[s]] = s;
+}
+
+constexpr int64_t kRankBrute = 16384;
+
+// bytes of scratch launch_prologue needs for P particles: keys [P] (+ for large batches: sorted keys, indices in and
+// out, and the radix sort's own temporary storage)
+size_t prologue_scratch_bytes(int64_t P)
+{
+    size_t n = ((size_t)P * sizeof(uint32_t) + 255) / 256 * 256;
+    if (P > kRankBrute) {
+        size_t tmp = 0;
+        cub::DeviceRadixSort::SortPairs(nullptr, tmp, (const uint32_t *)nullptr, (uint32_t *)nullptr, (const int32_t *)nullptr,
+                                        (int32_t *)nullptr, (int)P);
+        n += n + 2 * (((size_t)P * sizeof(int32_t) + 255) / 256 * 256) + tmp + 256;
+    }
+    return n;
+}
+
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,
-                            int32_t *slot_of, const double *rank_band, double *coef, int32_t *valid, int32_t *perm,
-                            cudaStream_t st)
+                            int32_t *slot_of, const double *rank_band, void *scratch, double *coef, int32_t *valid,
+                            int32_t *perm, cudaStream_t st)
 {
     if (slot_of != nullptr) {
-        rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_band ? rank_band[0] : 0.0,
-                                                                 rank_band ? rank_band[1] : 0.0, rank_band ? rank_band[2] : 0.0, slot_of);
+        const size_t kb = ((size_t)P * sizeof(uint32_t) + 255) / 256 * 256, ib = ((size_t)P * sizeof(int32_t) + 255) / 256 * 256;
+        unsigned char *base = static_cast<unsigned char *>(scratch);
+        uint32_t *keys = reinterpret_cast<uint32_t *>(base);
+        const bool big = P > kRankBrute;
+        int32_t *idx_in = big ? reinterpret_cast<int32_t *>(base + 2 * kb) : nullptr;
+        rank_key_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_band ? rank_band[0] : 0.0,
+                                                                     rank_band ? rank_band[1] : 0.0,
+                                                                     rank_band ? rank_band[2] : 0.0, keys, idx_in);
         cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        if (!big) {
+            rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(keys, (int32_t)P, slot_of);
+        } else {
+            // stable LSD radix sort of (key, index): the same order as the brute-force rank (ties by index)
+            uint32_t *keys_out = reinterpret_cast<uint32_t *>(base + kb);
+            int32_t *idx_out = reinterpret_cast<int32_t *>(base + 2 * kb + ib);
+            void *tmp = base + 2 * kb + 2 * ib;
+            size_t tmp_bytes = 0;
+            cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys_out, idx_in, idx_out, (int)P);
+            e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys_out, idx_in, idx_out, (int)P, 0, 32, st);
+            if (e != cudaSuccess) return e;
+            scatter_slots_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(idx_out, (int32_t)P, slot_of);
+        }
+        e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     const int nt = 128;
@@ -485,31 +538,32 @@ __global__ void __launch_bounds__(128) amplitude_kernel(const double *__restrict
                                                         int32_t n_part, double *__restrict__ amp)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int k = blockIdx.y;
     if (p >= P) return;
-    double v[kNAcc];
-#pragma unroll
-    for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
-    const int s_first = part_seg[k];
-    const double cs_r = partial[((int64_t)s_first * kNPartial + 8) * P_pad + p];
-    const double cs_i = partial[((int64_t)s_first * kNPartial + 9) * P_pad + p];
-    for (int s = s_first; s < part_seg[k + 1]; ++s) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
-    double apr, acr, api, aci;
-    solve_amplitudes(v, cs_r, cs_i, apr, acr, api, aci);
     const bool ok = valid[p] != 0;
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
-    double *out = amp + ((int64_t)perm[p] * n_part + k) * 4;
-    out[0] = ok ? apr : nan;     // a_1
-    out[1] = ok ? acr : nan;     // a_2
-    out[2] = ok ? api : nan;     // a_3
-    out[3] = ok ? aci : nan;     // a_4
+    for (int k = blockIdx.y; k < n_part; k += gridDim.y) {
+        double v[kNAcc];
+#pragma unroll
+        for (int j = 0; j < kNAcc; ++j) v[j] = 0.0;
+        const int s_first = part_seg[k];
+        const double cs_r = partial[((int64_t)s_first * kNPartial + 8) * P_pad + p];
+        const double cs_i = partial[((int64_t)s_first * kNPartial + 9) * P_pad + p];
+        for (int s = s_first; s < part_seg[k + 1]; ++s) add_segment(partial, s, P_pad, P_pad, 1, p, cs_r, cs_i, v);
+        double apr, acr, api, aci;
+        solve_amplitudes(v, cs_r, cs_i, apr, acr, api, aci);
+        double *out = amp + ((int64_t)perm[p] * n_part + k) * 4;
+        out[0] = ok ? apr : nan;     // a_1
+        out[1] = ok ? acr : nan;     // a_2
+        out[2] = ok ? api : nan;     // a_3
+        out[3] = ok ? aci : nan;     // a_4
+    }
 }
 
 cudaError_t launch_amplitudes(const double *partial, const int32_t *part_seg, const int32_t *valid,
                               const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, double *amp,
                               cudaStream_t st)
 {
-    const dim3 grd((unsigned)((P + 127) / 128), (unsigned)n_part);
+    const dim3 grd((unsigned)((P + 127) / 128), (unsigned)(n_part < 32768 ? n_part : 32768));
     amplitude_kernel<<<grd, 128, 0, st>>>(partial, part_seg, valid, perm, P, P_pad, n_part, amp);
     return cudaGetLastError();
 }

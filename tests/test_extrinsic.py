@@ -1,14 +1,18 @@
 """extrinsic amplitudes a = M^-1 N (Eq. 10) from the library against the oracle's
-4x4 solve, and the recovery of (D_L, iota, psi, phi_c) by Eq. B2-B3 (:426-440) pinned by the round trip through
-Eq. B1 (:413-420, retyped here)."""
+4x4 solve, and the recovery of (D_L, iota, psi, phi_c) by Eq. B2-B3 (:426-440): the library's host function
+fstat_extrinsic_from_amplitudes (through the C ABI) against the oracle's plain restatement of App. B
+(oracle/extrinsic_oracle.py), both pinned by the round trip through Eq. B1 (:413-420, retyped here)."""
 import math
 
 import numpy as np
 import pytest
 
 import synthetic as syn
-from paper_2407_10797_b200.extrinsic import (amplitude_constant, amplitudes_from_extrinsic,
-                                             extrinsic_from_amplitudes)
+from oracle import extrinsic_oracle as xo
+from paper_2407_10797_b200 import build as _cuda_build
+from paper_2407_10797_b200.extrinsic import amplitudes_from_extrinsic, extrinsic_from_amplitudes
+
+_cuda_build.build()                                       # host functions of the C-ABI library: no GPU needed
 
 
 def _b1(d_l, psi, iota, phi_c):
@@ -54,10 +58,33 @@ def test_outside_the_principal_branches_the_recovered_set_reproduces_the_amplitu
         assert r["D_L"] == pytest.approx(d_l, rel=1e-10) and r["iota"] == pytest.approx(iota, abs=2e-6 / max(math.sin(iota), 1e-3))
 
 
+def test_oracle_b2_b3_inverts_b1_and_the_library_agrees_with_it():
+    """The oracle's App. B (Eq. B2-B3 as printed + reading A25) is pinned by the round trip through Eq. B1 as printed;
+    the library's C function, called through the ABI, gives the oracle's four numbers on random amplitude vectors."""
+    rng = np.random.default_rng(9)
+    for _ in range(300):
+        d_l, psi = rng.uniform(0.3, 5.0), rng.uniform(-math.pi, math.pi)
+        iota, phi_c = rng.uniform(0.0, math.pi), rng.uniform(-math.pi, math.pi)
+        a = _b1(d_l, psi, iota, phi_c)
+        np.testing.assert_allclose(xo.b1(d_l, psi, iota, phi_c), a, rtol=0, atol=1e-15)
+        o = xo.b2_b3(a)
+        assert o[0] == pytest.approx(d_l, rel=1e-7) and o[1] == pytest.approx(iota, abs=2e-6 / max(math.sin(iota), 1e-3))
+        tol = 1e-8 / (d_l * max(1.0 - abs(math.cos(iota)), 1e-4))
+        np.testing.assert_allclose(_b1(*[o[0], o[2], o[1], o[3]]), a, rtol=0, atol=max(tol, 1e-7 / d_l))
+        r = extrinsic_from_amplitudes(a)
+        near_face_on = max(1.0 - abs(math.cos(iota)), 1e-4)
+        assert r["D_L"] == pytest.approx(o[0], rel=1e-6)      # the oracle keeps the printed sqrt(A_+^2 - A_x^2): cancellation
+        assert r["iota"] == pytest.approx(o[1], abs=1e-5 / max(math.sin(iota), 1e-3))
+        assert r["psi"] == pytest.approx(o[2], abs=1e-6 / near_face_on)
+        assert abs(math.remainder(r["phi_c"] - o[3], 2.0 * math.pi)) <= 1e-6 / near_face_on
+    with pytest.raises(Exception):
+        extrinsic_from_amplitudes([np.nan, 0.0, 0.0, 0.0])
+    assert extrinsic_from_amplitudes([0.0, 0.0, 0.0, 0.0])["D_L"] == math.inf
+
+
 def test_amplitude_constant_restores_metres():
     mc, d_l_m = 30.0, 3.0e24                                   # ~100 Mpc
-    k = amplitude_constant(mc)
-    assert k < 0.0 and k == pytest.approx(-math.sqrt(5 / 24) * (30 * 4.925490947641267e-6) ** (5 / 6) / math.pi ** (2 / 3))
+    k = -math.sqrt(5 / 24) * (30 * 4.925490947641267e-6) ** (5 / 6) / math.pi ** (2 / 3)      # Eq. A2 (:402) without 1/D_L
     a_lib = k * _b1(d_l_m / 299792458.0, 0.3, 1.0, -0.4)
     r = extrinsic_from_amplitudes(a_lib, chirp_mass_msun=mc)
     assert r["D_L"] == pytest.approx(d_l_m, rel=1e-10) and r["iota"] == pytest.approx(1.0, abs=1e-8)
