@@ -178,14 +178,23 @@ bool segments_aligned(const fstat_plan *pl)
 }
 
 // the interpolating kernel needs segments that start at multiples of 512 bins
-bool segments_fast_capable(const fstat_plan *pl)
+bool segments_fast_capable(int64_t seg_len)
 {
-    return pl->opt.max_segment_bins <= 0 || pl->opt.max_segment_bins % kMaxStride == 0;
+    return seg_len % kMaxStride == 0;
 }
 
 int64_t auto_segment_len(const fstat_plan *pl, int32_t n_groups)
 {
     if (pl->opt.max_segment_bins > 0) return pl->opt.max_segment_bins;
+    // Small problems (config 0: 2096 bins x one particle group): with segments of >= 2048 bins a handful of CTAs
+    // would walk the whole band one bin after the other.  Cut them into 64-bin tiles' worth of work for ~2 CTAs per
+    // SM instead; such segments are not multiples of 512 bins, so these items all go to the direct kernel.
+    const int64_t work = pl->n_bins * (int64_t)n_groups;
+    if (work < (int64_t)pl->n_sm * 2 * 4 * kMaxStride) {
+        int64_t len = work / ((int64_t)pl->n_sm * 2 * n_groups);
+        len = ((len + kTileBins - 1) / kTileBins) * kTileBins;
+        return len < kTileBins ? kTileBins : len;
+    }
     // aim at >= 48 work items per SM so that the tail wave is short; multiples of kMaxStride
     const int64_t target_ctas = (int64_t)pl->n_sm * 48;
     int64_t want_seg = (target_ctas + n_groups - 1) / n_groups;
@@ -290,7 +299,7 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
             }
             crit[sgi] = make_seg_crit(pl->f0 + (double)lo * pl->df, pl->f0 + (double)hi * pl->df, pl->df,
                                       (double)(pl->edges[k + 1] - pl->edges[k]));
-            maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && segments_fast_capable(pl) && hi - lo >= 8) ? kNLevels - 1 : -1);
+            maxlvl[sgi] = (int8_t)((pl->fast_ok && aligned && segments_fast_capable(seg_len) && hi - lo >= 8) ? kNLevels - 1 : -1);
         }
     if (pl->seg_cache.size() >= 8) {                       // (a ninth segment length: start over)
         const int32_t keep = pl->seg_groups;
@@ -865,15 +874,15 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     fstat_plan *cp = pl->bandplan;
     if (cp->opt.max_segment_bins != pl->opt.max_segment_bins) invalidate_segments(cp);
     cp->opt = pl->opt;
-    const bool fast = cp->fast_ok && pl->opt.force_level != -1 && segments_fast_capable(cp);
-    if (fast) {
-        s = ensure_prefix_gram(pl);
-        if (s != FSTAT_OK) return s;
-    }
     const int64_t n_groups = (P + kThreads - 1) / kThreads;
     const int64_t P_pad = n_groups * kThreads;
     s = ensure_segments(cp, (int32_t)n_groups);
     if (s != FSTAT_OK) { pl->err = cp->err; return s; }
+    const bool fast = cp->fast_ok && pl->opt.force_level != -1 && segments_fast_capable(auto_segment_len(cp, (int32_t)n_groups));
+    if (fast) {
+        s = ensure_prefix_gram(pl);
+        if (s != FSTAT_OK) return s;
+    }
     if ((int64_t)cp->n_seg * n_groups >= ((int64_t)1 << 31))
         return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
 
