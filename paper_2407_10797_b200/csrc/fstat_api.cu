@@ -913,7 +913,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     CU_TRY(pl, grow(&cp->d_sort, &cp->sort_cap, prologue_scratch_bytes(P)));
     CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, cp->d_slot, rank_band, cp->d_sort,
                                cp->d_coef, cp->d_valid, cp->d_perm, st));
-    CU_TRY(pl, launch_band_limits(pl->d_table, cp->d_coef, cp->d_valid, cp->d_perm, P_pad, (int32_t)pl->n_bins,
+    CU_TRY(pl, launch_band_limits(cp->d_coef, cp->d_valid, cp->d_perm, P_pad, (int32_t)pl->n_bins, pl->f0, pl->df,
                                   1.0 / pl->df, pl->opt.orbit_kappa, cp->d_band, cp->d_band + P_pad, band, st));
     BandSched bs{};
     bs.band_lo = cp->d_band;
@@ -976,8 +976,8 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     ++pl->n_timed;
     CU_TRY(pl, launch_band_short(pl->d_table, cp->d_coef, bc, P_pad, pl->orb, st));
     CU_TRY(pl, launch_band_stitch(bc, P, P_pad, cp->seg_len, cp->n_seg, F, st));
-    // keys, rank, prologue, band limits, stride selection, [interpolating], direct, short partitions, stitch, F sums
-    pl->n_launches += 9 + (fast ? 1 : 0);
+    // keys, rank, keys, rank, prologue, band limits, stride selection, [interpolating], direct, short partitions, stitch, F sums
+    pl->n_launches += 11 + (fast ? 1 : 0);
     pl->last_was_band = true;
     return FSTAT_OK;
 }

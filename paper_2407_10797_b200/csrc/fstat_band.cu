@@ -6,7 +6,7 @@
 // kernel with per-thread edges (fstat_fastband.cu):
 //
 //   band_kernel          k_lo = #{bins with t_f < 0}, k_hi = #{bins with t_f <= T_obs} per particle, by
-//                        bisection over the per-bin table (t_f increases along the grid)
+//                        bisection over the grid (t_f increases along it)
 //   fstat_band_kernel    the DIRECT kernel (full model at every in-band bin) with per-thread partition edges, for
 //                        the (particle group, work segment) items the stride selection leaves to it
 //                        (options.force_level == -1: all of them); same head / tail records and in-thread
@@ -27,21 +27,33 @@
 
 namespace fstat {
 
-// Orbital phase at t_f in quarter turns of a year, alpha_q = c10 + sum_j c_j D_j(f) (same FMA chain as
-// model_eval); t_f = (alpha_q - 2 kappa / pi) year / 4.
-__device__ __forceinline__ double tf_seconds(const double *__restrict__ row, const double (&c)[kNCoef], double kappa_qt)
+// t_f [s] (Eq. 20 :220, from Psi_0 only, reading A4) at frequency f: the orbital phase at t_f in quarter turns of a
+// year is alpha_q = c10 + sum_j c_j D_j(f), D_j = (dB_j/df) / year in the order of the phase basis (fill_basis_row),
+// and t_f = (alpha_q - 2 kappa / pi) year / 4.  Evaluated from f itself: the bisection below jumps across the whole
+// grid, and 42 dependent table reads would cost more than the arithmetic.
+__device__ __forceinline__ double tf_seconds(double f, const double (&c)[kNCoef], double kappa_qt)
 {
-    double alq = fma(c[2], row[T_D0 + 0], c[10]);
-#pragma unroll
-    for (int j = 1; j < 8; ++j) alq = fma(c[2 + j], row[T_D0 + j], alq);
-    return (alq - kappa_qt) * (0.25 * kYear);
+    const double lnf = log(f);
+    const double icb = 1.0 / cbrt(f);                  // f^(-1/3)
+    const double fm23 = icb * icb, fm1 = 1.0 / f, fm53 = fm1 * fm23;
+    const double fm349 = pow(f, -34.0 / 9.0);
+    double alq = c[10] * kYear;
+    alq = fma(c[2], fm1, alq);
+    alq = fma(c[3], (-5.0 / 3.0) * fm53 * fm1, alq);
+    alq = fma(c[4], -fm1 * fm1, alq);
+    alq = fma(c[5], (-2.0 / 3.0) * fm53, alq);
+    alq = fma(c[6], (-1.0 / 3.0) * icb * fm1, alq);
+    alq = fma(c[7], (1.0 / 3.0) * fm23, alq);
+    alq = fma(c[8], fm23 * (1.0 + lnf / 3.0), alq);
+    alq = fma(c[9], (-34.0 / 9.0) * fm349 * fm1, alq);
+    return (alq - kappa_qt * kYear) * 0.25;
 }
 
-__global__ void __launch_bounds__(128) band_kernel(const double *__restrict__ table, const double *__restrict__ coef,
-                                                   const int32_t *__restrict__ valid,
+__global__ void __launch_bounds__(128) band_kernel(const double *__restrict__ coef, const int32_t *__restrict__ valid,
                                                    const int32_t *__restrict__ perm, int64_t P_pad, int32_t n_bins,
-                                                   double T_obs, double kappa_qt, int32_t *__restrict__ band_lo,
-                                                   int32_t *__restrict__ band_hi, int64_t *__restrict__ band_out)
+                                                   double f0, double df, double T_obs, double kappa_qt,
+                                                   int32_t *__restrict__ band_lo, int32_t *__restrict__ band_hi,
+                                                   int64_t *__restrict__ band_out)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;       // slot
     if (p >= P_pad) return;
@@ -54,14 +66,14 @@ __global__ void __launch_bounds__(128) band_kernel(const double *__restrict__ ta
         int32_t a = 0, b = n_bins;
         while (a < b) {
             const int32_t m = a + ((b - a) >> 1);
-            if (tf_seconds(table + (int64_t)m * kTabW, c, kappa_qt) < 0.0) a = m + 1; else b = m;
+            if (tf_seconds(fma((double)m, df, f0), c, kappa_qt) < 0.0) a = m + 1; else b = m;
         }
         k_lo = a;
         // first bin with t_f > T_obs
         b = n_bins;
         while (a < b) {
             const int32_t m = a + ((b - a) >> 1);
-            if (tf_seconds(table + (int64_t)m * kTabW, c, kappa_qt) <= T_obs) a = m + 1; else b = m;
+            if (tf_seconds(fma((double)m, df, f0), c, kappa_qt) <= T_obs) a = m + 1; else b = m;
         }
         k_hi = a;
     }
@@ -369,7 +381,7 @@ __global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict
 cudaError_t launch_band_short(const double *table, const double *coef, const BandCommon &b, int64_t P_pad,
                               const OrbitCoef &orb, cudaStream_t st)
 {
-    int gy = b.N < 1024 ? b.N : 1024;
+    const int gy = b.N < 32 ? b.N : 32;                     // (usually no template takes this path: keep the grid small)
     band_short_kernel<<<dim3((unsigned)(P_pad / 128), (unsigned)gy), 128, 0, st>>>(table, coef, b, P_pad, orb);
     return cudaGetLastError();
 }
@@ -396,11 +408,11 @@ cudaError_t band_kernel_configure()
     return cudaFuncSetAttribute(fstat_band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MainSmem));
 }
 
-cudaError_t launch_band_limits(const double *table, const double *coef, const int32_t *valid, const int32_t *perm,
-                               int64_t P_pad, int32_t n_bins, double T_obs, double kappa, int32_t *band_lo,
+cudaError_t launch_band_limits(const double *coef, const int32_t *valid, const int32_t *perm, int64_t P_pad,
+                               int32_t n_bins, double f0, double df, double T_obs, double kappa, int32_t *band_lo,
                                int32_t *band_hi, int64_t *band_out, cudaStream_t st)
 {
-    band_kernel<<<(unsigned)((P_pad + 127) / 128), 128, 0, st>>>(table, coef, valid, perm, P_pad, n_bins, T_obs,
+    band_kernel<<<(unsigned)((P_pad + 127) / 128), 128, 0, st>>>(coef, valid, perm, P_pad, n_bins, f0, df, T_obs,
                                                                   2.0 * kappa / kPi, band_lo, band_hi, band_out);
     return cudaGetLastError();
 }

@@ -157,10 +157,33 @@ __device__ __forceinline__ void load_gram(const double *__restrict__ gp, double 
 }
 
 // F_k (and the amplitudes) of a finished partition, written through the slot -> particle map
+// 2 F_k as two_F (fstat_direct.cuh) with the two divisions replaced by rcp_fast (relative error ~1e-16: the hardware
+// seed and two Newton steps, no slow path): this runs inside the interpolating kernel, once per partition and thread
+__device__ __forceinline__ double two_F_inline(const double (&v)[kNAcc])
+{
+    const double zpr = v[0], zpi = v[1], zcr = v[2], zci = v[3];
+    const double mpp = v[4], mcc = v[5], mr = v[6], mi = v[7];
+    double twoF = 0.0;
+    if (mpp > 0.0) {
+        const double inv = rcp_fast(mpp);
+        twoF = (zpr * zpr + zpi * zpi) * inv;
+        const double cr = mr * inv, ci = mi * inv;                      // m_pc / m_pp
+        const double schur = mcc - (mr * mr + mi * mi) * inv;
+        if (schur > 1e-13 * mcc) {
+            const double yr = zcr - (cr * zpr - ci * zpi);
+            const double yi = zci - (cr * zpi + ci * zpr);
+            twoF += (yr * yr + yi * yi) * rcp_fast(schur);
+        }
+    } else if (mcc > 0.0) {
+        twoF = (zcr * zcr + zci * zci) * rcp_fast(mcc);
+    }
+    return twoF;
+}
+
 __device__ __forceinline__ void finish_partition(const double (&v)[kNAcc], double c_re, double c_im, int64_t idx,
                                                  double *__restrict__ Fk, double *__restrict__ amp)
 {
-    Fk[idx] = 0.5 * two_F(v);
+    Fk[idx] = 0.5 * two_F_inline(v);
     if (amp != nullptr) {
         double a1, a2, a3, a4;
         solve_amplitudes(v, c_re, c_im, a1, a2, a3, a4);
@@ -231,6 +254,15 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
                 opened = band_edge(j, q_lo, D, N, C, a.b.n_bins) == lo;
             }
         }
+    }
+    // the edges after `cut` follow by stepping floor(j D / N) incrementally: e_(j+1) from e_j costs two additions, not a
+    // 64-bit division (cut = min(C (q_lo + eq), n_bins), eq = floor((j + 1) D / N), er the remainder)
+    const int32_t dq = D > 0 ? D / N : 0, dr = D > 0 ? D % N : 0;
+    int32_t eq = 0, er = 0;
+    if (j < N) {
+        const int64_t jd = (int64_t)(j + 1) * D;
+        eq = (int32_t)(jd / N);
+        er = (int32_t)(jd - (int64_t)eq * N);
     }
     // The node intervals of this work segment that hold an in-band bin of some lane of this WARP: [w_lo, w_hi).  The
     // slots are ranked by the position of the band, so the bands of the 32 lanes of a warp nearly coincide while the
@@ -478,7 +510,13 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
             ++j;
             opened = true;
             if (j >= N) { j = N; cut = INT32_MAX; }
-            else cut = band_edge(j + 1, q_lo, D, N, C, a.b.n_bins);
+            else {
+                eq += dq;
+                er += dr;
+                if (er >= N) { er -= N; ++eq; }
+                const int64_t e = (int64_t)C * ((int64_t)q_lo + eq);
+                cut = (int32_t)(e < (int64_t)a.b.n_bins ? e : (int64_t)a.b.n_bins);
+            }
             if (cut < j1) atomicOr(a.b.err, 1u);               // (a second edge in one interval: excluded by the stride cap)
             double t10[kNPartial];
 #pragma unroll

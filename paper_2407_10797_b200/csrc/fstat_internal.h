@@ -195,8 +195,8 @@ struct BandArgs {
     OrbitCoef orb;
 };
 
-cudaError_t launch_band_limits(const double *table, const double *coef, const int32_t *valid, const int32_t *perm,
-                               int64_t P_pad, int32_t n_bins, double T_obs, double kappa, int32_t *band_lo,
+cudaError_t launch_band_limits(const double *coef, const int32_t *valid, const int32_t *perm, int64_t P_pad,
+                               int32_t n_bins, double f0, double df, double T_obs, double kappa, int32_t *band_lo,
                                int32_t *band_hi, int64_t *band_out, cudaStream_t st);
 cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t st);
 cudaError_t band_kernel_configure();

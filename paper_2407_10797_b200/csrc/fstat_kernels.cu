@@ -138,11 +138,10 @@ __device__ __forceinline__ bool particle_ok(const double *__restrict__ q)
 // are computed once (rank_key_kernel), then ranked by brute force (P <= 16384: one launch of P^2 integer comparisons
 // through shared-memory tiles) or by a stable radix sort of (key, index) pairs (cub, larger batches: the same order).
 // Invalid particles sort last.
-// band_T > 0 (row f2; band_T = the observation time, [band_f0, band_f1] = the grid): the key is a weighted
-// mean of the Newtonian estimates of the template's frequencies at t = 0 and t = T, clipped to the grid,
-// f(t) = (1/pi) (5 / (256 (t_c - t)))^(3/8) (G M_c / c^3)^(-5/8), so that the bands of a group of 128 overlap
-// at both ends (the upper end weighs more: it moves faster with t_c).  Only the ORDER matters: the bands
-// themselves come from band_kernel.
+// band_T > 0 (row f2; band_T = the observation time, [band_f0, band_f1] = the grid): the key is the Newtonian
+// estimate of the template's frequency at t = 0, clipped to the grid,
+// f(t) = (1/pi) (5 / (256 (t_c - t)))^(3/8) (G M_c / c^3)^(-5/8); a second pass (rank_key2) re-orders blocks of 256
+// slots by the frequency at t = T.  Only the ORDER matters: the bands themselves come from band_kernel.
 __device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, double band_T, double band_f0, double band_f1)
 {
     if (!particle_ok(q)) return 0xFFFFFFFFu;
@@ -150,22 +149,42 @@ __device__ __forceinline__ uint32_t rank_key(const double *__restrict__ q, doubl
     const double tc = q[0];
     if (!(tc > 0.0)) return 0u;
     const double m = pow(q[1] * kGMsunC3, -0.625) * (1.0 / kPi) * pow(5.0 / 256.0, 0.375);
-    const double fa = fmin(fmax(m * pow(tc, -0.375), band_f0), band_f1);
-    const double fb = (tc > band_T) ? fmin(fmax(m * pow(tc - band_T, -0.375), band_f0), band_f1) : band_f1;
-    return __float_as_uint((float)(0.4 * fa + 0.6 * fb));
+    return __float_as_uint((float)fmin(fmax(m * pow(tc, -0.375), band_f0), band_f1));      // f(t = 0), clipped to the grid
 }
 
+// Row f2, second key: blocks of `block` consecutive slots of the first order (by the lower end of the band) are
+// re-ordered by the UPPER end f(t = T), so that the 32 templates of a warp have bands that nearly coincide at both ends
+// (a warp walks the union of its lanes' bands).  key = block number x 2^20 + the upper end on a 2^20-step scale.
+__device__ __forceinline__ uint32_t rank_key2(const double *__restrict__ q, int32_t slot1, int32_t block, double band_T,
+                                              double band_f0, double band_f1)
+{
+    if (!particle_ok(q)) return 0xFFFFFFFFu;
+    const double tc = q[0];
+    double fb = band_f1;
+    if (tc > band_T) {
+        const double m = pow(q[1] * kGMsunC3, -0.625) * (1.0 / kPi) * pow(5.0 / 256.0, 0.375);
+        fb = fmin(fmax(m * pow(tc - band_T, -0.375), band_f0), band_f1);
+    } else if (!(tc > 0.0)) fb = band_f0;
+    const double u = band_f1 > band_f0 ? (fb - band_f0) / (band_f1 - band_f0) : 0.0;
+    return (uint32_t)(slot1 / block) * (1u << 20) + (uint32_t)(u * 1048575.0);
+}
+
+// slot1 == nullptr: first key; else the second key of row f2 (see rank_key2)
 __global__ void __launch_bounds__(256) rank_key_kernel(const double *__restrict__ params, int32_t P, double band_T,
-                                                       double band_f0, double band_f1, uint32_t *__restrict__ keys,
+                                                       double band_f0, double band_f1, const int32_t *__restrict__ slot1,
+                                                       int32_t block, uint32_t *__restrict__ keys,
                                                        int32_t *__restrict__ index)
 {
     const int i = blockIdx.x * 256 + threadIdx.x;
     if (i >= P) return;
-    keys[i] = rank_key(params + 6 * (int64_t)i, band_T, band_f0, band_f1);
+    keys[i] = slot1 == nullptr ? rank_key(params + 6 * (int64_t)i, band_T, band_f0, band_f1)
+                               : rank_key2(params + 6 * (int64_t)i, slot1[i], block, band_T, band_f0, band_f1);
     if (index != nullptr) index[i] = i;
 }
 
-// brute-force rank of the keys (P^2 integer comparisons through shared-memory tiles): one launch, for P <= kRankBrute
+// brute-force rank of the keys (P^2 integer comparisons through shared-memory tiles), for P <= kRankBrute: blockIdx.y
+// splits the keys a thread compares its own with; the partial counts are added with integer atomics (slot_of zeroed
+// by the caller), so the result does not depend on the order
 __global__ void __launch_bounds__(256) rank_kernel(const uint32_t *__restrict__ keys, int32_t P,
                                                    int32_t *__restrict__ slot_of)
 {
@@ -173,7 +192,7 @@ __global__ void __launch_bounds__(256) rank_kernel(const uint32_t *__restrict__ 
     const int i = blockIdx.x * 256 + threadIdx.x;
     const uint32_t my = i < P ? keys[i] : 0xFFFFFFFFu;
     int rank = 0;
-    for (int j0 = 0; j0 < P; j0 += 256) {
+    for (int j0 = blockIdx.y * 256; j0 < P; j0 += gridDim.y * 256) {
         const int j = j0 + threadIdx.x;
         __syncthreads();
         skey[threadIdx.x] = j < P ? keys[j] : 0xFFFFFFFFu;
@@ -184,7 +203,7 @@ __global__ void __launch_bounds__(256) rank_kernel(const uint32_t *__restrict__ 
             rank += (kt < my) || (kt == my && j0 + t < i);
         }
     }
-    if (i < P) slot_of[i] = rank;
+    if (i < P && rank != 0) atomicAdd(&slot_of[i], rank);
 }
 
 // slot_of[particle] = position of the particle in the list sorted by (key, index)
@@ -220,26 +239,32 @@ cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, doub
         uint32_t *keys = reinterpret_cast<uint32_t *>(base);
         const bool big = P > kRankBrute;
         int32_t *idx_in = big ? reinterpret_cast<int32_t *>(base + 2 * kb) : nullptr;
-        rank_key_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, rank_band ? rank_band[0] : 0.0,
-                                                                     rank_band ? rank_band[1] : 0.0,
-                                                                     rank_band ? rank_band[2] : 0.0, keys, idx_in);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        if (!big) {
-            rank_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(keys, (int32_t)P, slot_of);
-        } else {
-            // stable LSD radix sort of (key, index): the same order as the brute-force rank (ties by index)
-            uint32_t *keys_out = reinterpret_cast<uint32_t *>(base + kb);
-            int32_t *idx_out = reinterpret_cast<int32_t *>(base + 2 * kb + ib);
-            void *tmp = base + 2 * kb + 2 * ib;
-            size_t tmp_bytes = 0;
-            cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys_out, idx_in, idx_out, (int)P);
-            e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys_out, idx_in, idx_out, (int)P, 0, 32, st);
+        const double bT = rank_band ? rank_band[0] : 0.0, bf0 = rank_band ? rank_band[1] : 0.0, bf1 = rank_band ? rank_band[2] : 0.0;
+        int32_t block = 256;                                 // row f2: slots re-ordered by the upper band end inside blocks
+        while ((P + block - 1) / block > 4095) block *= 2;   // (the block number has 12 bits of the second key)
+        for (int pass = 0; pass < (rank_band ? 2 : 1); ++pass) {
+            rank_key_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(params, (int32_t)P, bT, bf0, bf1,
+                                                                         pass ? slot_of : nullptr, block, keys, idx_in);
+            cudaError_t e = cudaGetLastError();
             if (e != cudaSuccess) return e;
-            scatter_slots_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(idx_out, (int32_t)P, slot_of);
+            if (!big) {
+                const unsigned nb = (unsigned)((P + 255) / 256);
+                if ((e = cudaMemsetAsync(slot_of, 0, (size_t)P * sizeof(int32_t), st)) != cudaSuccess) return e;
+                rank_kernel<<<dim3(nb, nb < 16 ? nb : 16), 256, 0, st>>>(keys, (int32_t)P, slot_of);
+            } else {
+                // stable LSD radix sort of (key, index): the same order as the brute-force rank (ties by index)
+                uint32_t *keys_out = reinterpret_cast<uint32_t *>(base + kb);
+                int32_t *idx_out = reinterpret_cast<int32_t *>(base + 2 * kb + ib);
+                void *tmp = base + 2 * kb + 2 * ib;
+                size_t tmp_bytes = 0;
+                cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys_out, idx_in, idx_out, (int)P);
+                e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys_out, idx_in, idx_out, (int)P, 0, 32, st);
+                if (e != cudaSuccess) return e;
+                scatter_slots_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(idx_out, (int32_t)P, slot_of);
+            }
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
         }
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
     }
     const int nt = 128;
     prologue_kernel<<<(unsigned)((P_pad + nt - 1) / nt), nt, 0, st>>>(params, P, P_pad, f_ref_e0, kappa, slot_of, coef,
