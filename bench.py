@@ -318,7 +318,7 @@ def run_sweep(fs, torch, plan1, ds1, args, mix, fp64_rate, stream, scratch):
                      "fp64_inst_per_template_bin": inst / (float(P) * ds.n_bins),
                      "frac": inst / (main_ms * 1e-3) / fp64_rate if fp64_rate > 0 else None,
                      "frac_of_nominal": inst / (main_ms * 1e-3) / NOMINAL_FP64_INST_PER_S,
-                     "direct_kernel_share_of_bins": share["0"]})
+                     "direct_kernel_share_of_bins": share["0"], "plan_table_bytes": fs.fstat_plan_table_bytes(plan)})
 
     cfg2, cfg3, cfg4 = syn.CONFIGS[2], syn.CONFIGS[3], syn.CONFIGS[4]
     for n_part in cfg2.n_part:
@@ -488,7 +488,8 @@ def run_ours(args):
                       "n_ctas": fs.fstat_plan_n_ctas(plan, P), "n_sm": n_sm,
                       "plan_options": {"force_level": args.force_level, "max_segment_bins": args.max_segment_bins,
                                        "interp_tol": args.interp_tol},
-                      "plan_create_s": t_plan, "dataset_s": t_data},
+                      "plan_create_s": t_plan, "dataset_s": t_data,
+                      "plan_table_bytes": fs.fstat_plan_table_bytes(plan)},
            "particles_per_s": float(P) * world / (ms_step * 1e-3),
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(par_pin.numel() * 8),
                    "d2h_bytes_per_step": int(F_pin.numel() * 8 + Fk_pin.numel() * 8),

@@ -19,8 +19,13 @@
  * Conventions common to all calls
  *   - All floating-point data are IEEE double.  "host" / "device" is stated per pointer.
  *   - Every call returns an fstat_status and never throws or aborts.
- *   - A plan may be used by one host thread at a time and has one evaluation in flight at a time
- *     (its workspace lives inside the plan).  Distinct plans are independent.
+ *   - A plan may be used by one host thread at a time, from ONE stream at a time, and has one evaluation in flight
+ *     at a time: its workspace (coefficients, partial sums, work lists, the timing ring) lives inside the plan and is
+ *     not guarded, so two evaluations of one plan on different streams would race.  Distinct plans are independent.
+ *   - Evaluation calls only enqueue work on the caller's stream.  Host-side work happens when something changes: the
+ *     first evaluation with a new batch size builds (and caches, per work-segment length) the segment tables and may
+ *     grow the workspace (cudaMalloc / cudaFree, which can synchronise the device); the first
+ *     fstat_eval_batch_bands call builds its prefix tables.  Repeated calls with batch sizes seen before do neither.
  */
 #ifndef FSTAT_H_
 #define FSTAT_H_
@@ -149,11 +154,14 @@ FSTAT_API fstat_status fstat_eval_batch(fstat_plan *plan, int64_t P,
  *   F       [P] DEVICE pointer, out.   Fk  [P][n_seg] DEVICE pointer, out; may be NULL.
  *   band    [P][2] int64 DEVICE pointer, out: k_lo, k_hi of every particle; may be NULL.
  * Invalid particles get F = F_k = -inf and band (0, 0).  Asynchronous on cuda_stream.
- * Work: the interpolating kernel over cells of the grid (the lattice cells for edge_lattice >= 32, else cells of
- * 64..512 bins by n_seg) plus, for edges that split a cell, the full model over the shorter piece of that cell;
- * with options.force_level == -1 (or a grid that starts within 1025 bins of f = 0) the full model at every in-band
- * bin.  Workspace: 80 bytes per (cell, particle), evaluated in particle batches of at most 24 GB.
- * Errors: EINVAL (NULL plan/params/F, n_seg < 1, edge_lattice < 1), ENOMEM, ECUDA.
+ * Work: the interpolating kernel with per-THREAD partition edges: all templates of a CTA walk the
+ * same bins, each cuts its running sums at its own edges; a partition that lies inside one work segment is finished in
+ * the thread, the others are stitched from one head and one tail record per (work segment, template).  Templates with
+ * an empty partition or one shorter than 8 bins are evaluated partition by partition with the full model; with
+ * options.force_level == -1 (or a grid that starts within 1025 bins of f = 0) so is every in-band bin.
+ * Workspace: 160 bytes per (work segment, particle) -- 73 MB for 2048 particles on the 2.5-yr grid -- plus, once per
+ * plan, prefix tables of 70 bytes per bin.  X, Y, Z plans only (EUNSUPPORTED for tdi_channel A, E, T).
+ * Errors: EINVAL (NULL plan/params/F, n_seg < 1, edge_lattice < 1), ENOMEM, ECUDA, EUNSUPPORTED.
  */
 FSTAT_API fstat_status fstat_eval_batch_bands(fstat_plan *plan, int64_t P, const double *params, int32_t n_seg,
                                               int32_t edge_lattice, double *F, double *Fk, int64_t *band,
@@ -162,7 +170,7 @@ FSTAT_API fstat_status fstat_eval_batch_bands(fstat_plan *plan, int64_t P, const
 /* Rows f2 x f3: the extrinsic amplitudes a = M^-1 N (Eq. 10 :96) of every partition of every template's band, as
  * fstat_eval_amplitudes gives them for the plan's partitions: amp [P][n_seg][4] DEVICE pointer, out (a_1..a_4; NaN
  * for invalid particles, 0 for empty partitions).  n_seg = 1 is the coherent estimate over the template's band
- * that App. B starts from.  EUNSUPPORTED with options.force_level == -1. */
+ * that App. B starts from. */
 FSTAT_API fstat_status fstat_eval_amplitudes_bands(fstat_plan *plan, int64_t P, const double *params, int32_t n_seg,
                                                    int32_t edge_lattice, double *amp, void *cuda_stream);
 
@@ -177,10 +185,12 @@ FSTAT_API fstat_status fstat_eval_batch_bands_host(fstat_plan *plan, int64_t P, 
  * fstat_eval_batch_channels -- SURVEY row f4, the channel sum of PAPER.md:62 Eq. 3: with several TDI combinations I
  * of mutually independent noise, Lambda = sum_I [<s^I, h^I>_I - |h^I|_I^2 / 2] and the four amplitudes of Eq. 5 are
  * common to all of them, so N^i = sum_I <d_I, A^i_I>_I, M^ij = sum_I <A^i_I, A^j_I>_I and F_k = N.M^-1.N / 2.
- * One plan per channel: its own data and 1/S_n^I, and its own response through the options (this library's
- * response is first-generation Michelson X; Y and Z are X with the spacecraft relabelled cyclically, i.e. with
- * orbit_lambda + 2 pi/3 and + 4 pi/3).  All plans must share the device, the grid, the partition edges and the other
- * options.  The a1-a5 kernels run once per channel; one epilogue adds the channels' sums and solves.
+ * One plan per channel: its own data and 1/S_n^I, and its own response through options.tdi_channel.  Eq. 3 ASSUMES
+ * independent noise between the channels: that holds for {A, E, T} and NOT for {X, Y, Z}, whose noises
+ * are correlated -- the call adds whatever set it is given (the sum over X, Y, Z is then not a likelihood ratio; it
+ * is accepted because the paper leaves the choice of combinations open, and tests use it).  All plans must share the
+ * device, the grid, the partition edges and the other options.  The a1-a5 kernels run once per channel; one epilogue
+ * adds the channels' sums and solves.
  *
  *   plans   HOST array of n_channels (1..4) plan handles, all different.
  *   params, F, Fk, cuda_stream as in fstat_eval_batch (Fk is [P][N_p]).
@@ -263,9 +273,13 @@ FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
 /* Number of CTAs the interpolating main kernel launches for P particles: particle groups of 128 x chunks of
  * consecutive segments (a chunk is one segment unless the partitions are short). */
 FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
-/* Number of CUDA kernels the fstat_eval_batch / fstat_eval_batch_host calls on this plan have launched so
- * far (per call: particle ranking, prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and
- * the chunk sums of F when the partitions are split over several epilogue blocks). */
+/* Bytes of device memory held by the plan's persistent tables: the folded data and (f, w') (32 bytes per bin), the
+ * node rows (192 bytes per 8 bins), the Gram matrices of the current partitions and, after the first
+ * fstat_eval_batch_bands call, the prefix Gram tables (70 bytes per bin).  Workspace (grown per batch size) not included. */
+FSTAT_API int64_t fstat_plan_table_bytes(const fstat_plan *plan);
+/* Number of CUDA kernels the evaluation calls on this plan have launched so far (per fstat_eval_batch: slot keys,
+ * ranking, prologue, stride selection, interpolating main kernel, direct main kernel, epilogue, and the chunk sums of
+ * F when the partitions are split over several epilogue blocks; a radix sort above 16384 particles counts as one). */
 FSTAT_API int64_t fstat_plan_launch_count(const fstat_plan *plan);
 /* How the most recent fstat_eval_batch on this plan was split between the direct kernel and the seven
  * strides of the interpolating kernel: bins_out[0] / [1..7] = sum over the (particle group, segment) work

@@ -37,9 +37,8 @@ struct fstat_plan {
     int32_t n_part = 0;
     std::vector<int64_t> edges;        // host copy [n_part+1]
     double f0 = 0.0;                   // freq[0]
-    double *d_table = nullptr;         // [n_bins][kTabW]   (direct kernel, template dump, Gram build)
     double *d_dwp = nullptr;           // [n_bins][2]       folded data (interpolating kernel)
-    double *d_w = nullptr;             // [n_bins]          4 df f^(-7/3) |K_f|^2 / S_n  (Gram builders, row f2's cuts)
+    double *d_fw = nullptr;            // [n_bins][2]       (f, w' = 4 df f^(-7/3) |K_f|^2 / S_n): full-model kernels, Gram builders
     double *d_node = nullptr;          // [n_node_rows][kTabW]
     int64_t n_node_rows = 0;
     bool fast_ok = false;              // the node grid (2 kMaxStride bins below, 3 above the band) stays at f > 0
@@ -74,7 +73,7 @@ struct fstat_plan {
     double *d_partial = nullptr; size_t partial_cap = 0; // doubles
     // row f2 (fstat_eval_batch_bands)
     fstat_plan *bandplan = nullptr;     // internal plan whose one partition is the whole grid (work segments only); shares the tables
-    bool shares_tables = false;         // d_table, d_dwp, d_w, d_node belong to the parent plan
+    bool shares_tables = false;         // d_dwp, d_fw, d_node belong to the parent plan
     double *d_pgram[kNLevels] = {};     // prefix Gram matrices [ceil(n_bins / 8)][kNGram] per stride level (first band call)
     bool pgram_built = false;
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
@@ -186,15 +185,11 @@ bool segments_fast_capable(int64_t seg_len)
 int64_t auto_segment_len(const fstat_plan *pl, int32_t n_groups)
 {
     if (pl->opt.max_segment_bins > 0) return pl->opt.max_segment_bins;
-    // Small problems (config 0: 2096 bins x one particle group): with segments of >= 2048 bins a handful of CTAs
-    // would walk the whole band one bin after the other.  Cut them into 64-bin tiles' worth of work for ~2 CTAs per
-    // SM instead; such segments are not multiples of 512 bins, so these items all go to the direct kernel.
-    const int64_t work = pl->n_bins * (int64_t)n_groups;
-    if (work < (int64_t)pl->n_sm * 2 * 4 * kMaxStride) {
-        int64_t len = work / ((int64_t)pl->n_sm * 2 * n_groups);
-        len = ((len + kTileBins - 1) / kTileBins) * kTileBins;
-        return len < kTileBins ? kTileBins : len;
-    }
+    // Short grids (config 0: 2096 bins): with segments of >= 2048 bins a handful of CTAs would walk the whole band one bin
+    // after the other.  Below 4096 bins the work items are single 64-bin tiles instead; such segments are not multiples
+    // of 512 bins, so these items all go to the direct kernel (on so short a grid the interpolating kernel would pay its
+    // five start-up nodes per partition anyway).
+    if (pl->n_bins < 2 * 4 * kMaxStride) return kTileBins;
     // aim at >= 48 work items per SM so that the tail wave is short; multiples of kMaxStride
     const int64_t target_ctas = (int64_t)pl->n_sm * 48;
     int64_t want_seg = (target_ctas + n_groups - 1) / n_groups;
@@ -346,7 +341,7 @@ fstat_status build_gram_tables(fstat_plan *pl)
         const int64_t n_sub = (pl->n_bins + S - 1) / S + cnt[n_part - 1];
         CU_TRY(pl, grow(&pl->d_gram[l], &pl->gram_cap[l], (size_t)n_sub * kNGram));
         CU_TRY(pl, cudaMemcpy(pl->d_cnt, cnt.data(), (size_t)n_part * sizeof(int32_t), cudaMemcpyHostToDevice));
-        CU_TRY(pl, launch_build_gram(pl->d_w, pl->d_edges32, n_part, pl->n_bins, l, pl->d_cnt, pl->d_gram[l], 0));
+        CU_TRY(pl, launch_build_gram(pl->d_fw, pl->d_edges32, n_part, pl->n_bins, l, pl->d_cnt, pl->d_gram[l], 0));
         CU_TRY(pl, cudaDeviceSynchronize());   // d_cnt is reused by the next level
     }
     return FSTAT_OK;
@@ -476,9 +471,8 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
     uint32_t *d_err = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&d_err, sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMemset(d_err, 0, sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_table, (size_t)n_bins * kTabW * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_dwp, (size_t)n_bins * 2 * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_w, (size_t)n_bins * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_fw, (size_t)n_bins * 2 * sizeof(double));
     // node rows for bins -2 kMaxStride .. (floor((N-1)/kMaxStride) + 3) * kMaxStride in steps of kNodeStride
     pl->n_node_rows = kNodePad + (((n_bins - 1) / kMaxStride + 3) * kMaxStride) / kNodeStride + 1;
     if (e == cudaSuccess) e = cudaMalloc((void **)&pl->d_node, (size_t)pl->n_node_rows * kTabW * sizeof(double));
@@ -489,8 +483,8 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
         else {
             pl->f0 = fe[0];
             pl->fast_ok = (fe[0] - (double)(2 * kMaxStride + 1) * pl->df > 0.0) && n_bins > 1;
-            e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->d_table,
-                                   pl->d_dwp, pl->d_w, d_err, 0);
+            e = launch_build_table(d_freq, d_dw, d_isn, n_bins, pl->df, pl->opt.arm_length_m, pl->d_dwp, pl->d_fw,
+                                   d_err, 0);
             if (e == cudaSuccess)
                 e = launch_build_nodes(d_freq, n_bins, pl->df, pl->opt.arm_length_m, pl->n_node_rows, pl->d_node, 0);
             if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -527,11 +521,11 @@ static void plan_free(fstat_plan *pl)
     if (!pl) return;
     DeviceGuard g(pl->device);
     if (pl->bandplan) { plan_free(pl->bandplan); pl->bandplan = nullptr; }
-    if (pl->shares_tables) { pl->d_table = nullptr; pl->d_dwp = nullptr; pl->d_w = nullptr; pl->d_node = nullptr; }
+    if (pl->shares_tables) { pl->d_dwp = nullptr; pl->d_fw = nullptr; pl->d_node = nullptr; }
     for (SegTables &t : pl->seg_cache) free_seg_tables(t);
-    cudaFree(pl->d_table); cudaFree(pl->d_coef);
+    cudaFree(pl->d_coef);
     cudaFree(pl->d_valid); cudaFree(pl->d_partial); cudaFree(pl->d_params); cudaFree(pl->d_F); cudaFree(pl->d_Fk);
-    cudaFree(pl->d_dwp); cudaFree(pl->d_w); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
+    cudaFree(pl->d_dwp); cudaFree(pl->d_fw); cudaFree(pl->d_node); cudaFree(pl->d_edges32); cudaFree(pl->d_cnt);
     for (int l = 0; l < kNLevels; ++l) { cudaFree(pl->d_gram[l]); cudaFree(pl->d_pgram[l]); }
     cudaFree(pl->d_band); cudaFree(pl->d_rec); cudaFree(pl->d_err); cudaFree(pl->d_band_fk); cudaFree(pl->d_band_out);
     cudaFree(pl->d_level);
@@ -615,6 +609,18 @@ int64_t fstat_plan_n_bins(const fstat_plan *pl) { return pl ? pl->n_bins : 0; }
 int32_t fstat_plan_n_part(const fstat_plan *pl) { return pl ? pl->n_part : 0; }
 int32_t fstat_plan_device(const fstat_plan *pl) { return pl ? pl->device : -1; }
 int64_t fstat_plan_launch_count(const fstat_plan *pl) { return pl ? pl->n_launches : 0; }
+
+int64_t fstat_plan_table_bytes(const fstat_plan *pl)
+{
+    if (!pl) return 0;
+    int64_t b = (int64_t)pl->n_bins * 4 * (int64_t)sizeof(double)                 // folded data, (f, w')
+                + pl->n_node_rows * kTabW * (int64_t)sizeof(double);             // node rows
+    for (int l = 0; l < kNLevels; ++l) {
+        b += (int64_t)pl->gram_cap[l] * (int64_t)sizeof(double);                 // Gram matrices of the partitions
+        if (pl->d_pgram[l]) b += ((pl->n_bins + kMinStride - 1) / kMinStride) * kNGram * (int64_t)sizeof(double);
+    }
+    return b;
+}
 
 int64_t fstat_plan_n_ctas(const fstat_plan *pl, int64_t P)
 {
@@ -724,7 +730,9 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.df = pl->df;
     fa.orb = pl->orb;
     MainArgs a;
-    a.table = pl->d_table;
+    a.dwp = pl->d_dwp;
+    a.fw = pl->d_fw;
+    a.arm_length_m = pl->opt.arm_length_m;
     a.coef = pl->d_coef;
     a.seg_edge = pl->d_seg_edge;
     a.direct_list = pl->d_direct + 1;
@@ -823,7 +831,7 @@ static fstat_status ensure_band_plan(fstat_plan *pl)
     if (!cp) return fail(pl, FSTAT_ENOMEM, "host allocation failed");
     cp->device = pl->device; cp->n_sm = pl->n_sm; cp->n_bins = pl->n_bins; cp->df = pl->df; cp->opt = pl->opt;
     cp->f0 = pl->f0; cp->orb = pl->orb; cp->fast_ok = pl->fast_ok;
-    cp->d_table = pl->d_table; cp->d_dwp = pl->d_dwp; cp->d_w = pl->d_w; cp->d_node = pl->d_node;
+    cp->d_dwp = pl->d_dwp; cp->d_fw = pl->d_fw; cp->d_node = pl->d_node;
     cp->n_node_rows = pl->n_node_rows;
     cp->shares_tables = true;
     try {
@@ -845,7 +853,7 @@ static fstat_status ensure_prefix_gram(fstat_plan *pl)
     const int64_t n_lat = (pl->n_bins + kMinStride - 1) / kMinStride;
     for (int l = 0; l < kNLevels; ++l) {
         if (!pl->d_pgram[l]) CU_TRY(pl, cudaMalloc((void **)&pl->d_pgram[l], (size_t)n_lat * kNGram * sizeof(double)));
-        CU_TRY(pl, launch_build_prefix_gram(pl->d_w, pl->n_bins, l, pl->d_pgram[l], 0));
+        CU_TRY(pl, launch_build_prefix_gram(pl->d_fw, pl->n_bins, l, pl->d_pgram[l], 0));
     }
     CU_TRY(pl, cudaDeviceSynchronize());           // built on the default stream; the caller's stream may not wait for it
     pl->pgram_built = true;
@@ -947,7 +955,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     if (fast) {
         FastBandArgs fa;
         fa.dwp = pl->d_dwp;
-        fa.w = pl->d_w;
+        fa.fw = pl->d_fw;
         fa.node = pl->d_node;
         for (int l = 0; l < kNLevels; ++l) fa.pgram[l] = pl->d_pgram[l];
         fa.coef = cp->d_coef;
@@ -962,7 +970,9 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
         CU_TRY(pl, launch_fastband(fa, st));
     }
     BandArgs ba;
-    ba.table = pl->d_table;
+    ba.dwp = pl->d_dwp;
+    ba.fw = pl->d_fw;
+    ba.arm_length_m = pl->opt.arm_length_m;
     ba.coef = cp->d_coef;
     ba.seg_edge = cp->d_seg_edge;
     ba.direct_list = cp->d_direct + 1;
@@ -974,7 +984,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     CU_TRY(pl, launch_band_main(ba, pl->n_sm * 12, st));
     CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
     ++pl->n_timed;
-    CU_TRY(pl, launch_band_short(pl->d_table, cp->d_coef, bc, P_pad, pl->orb, st));
+    CU_TRY(pl, launch_band_short(pl->d_dwp, pl->d_fw, pl->opt.arm_length_m, cp->d_coef, bc, P_pad, pl->orb, st));
     CU_TRY(pl, launch_band_stitch(bc, P, P_pad, cp->seg_len, cp->n_seg, F, st));
     // keys, rank, keys, rank, prologue, band limits, stride selection, [interpolating], direct, short partitions, stitch, F sums
     pl->n_launches += 11 + (fast ? 1 : 0);
@@ -1068,7 +1078,7 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
     CU_TRY(pl, launch_prologue(pl->d_params, 1, kThreads, pl->opt.f_ref_e0, pl->opt.orbit_kappa, nullptr, nullptr, nullptr,
                                pl->d_coef, pl->d_valid, nullptr, st));
-    CU_TRY(pl, launch_template(pl->d_table, pl->d_coef, kThreads, pl->n_bins, pl->orb, pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0,
+    CU_TRY(pl, launch_template(pl->d_fw, pl->opt.arm_length_m, pl->d_coef, kThreads, pl->n_bins, pl->orb, pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0,
                                u_plus, u_cross, st));
     CU_TRY(pl, cudaStreamSynchronize(st));
     return FSTAT_OK;

@@ -152,8 +152,8 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
 
         const int n_bins = hi - lo;
         const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
-        const double *src = a.table + (int64_t)lo * kTabW;
-        if (tid == 0) ring_prologue(sm, src, n_bins, n_tiles, g0);
+        const BinSource src{reinterpret_cast<const double2 *>(a.dwp), reinterpret_cast<const double2 *>(a.fw)};
+        if (tid == 0) ring_prologue(sm, src, lo, n_bins, n_tiles, g0);
 
         double c[kNCoef];
 #pragma unroll
@@ -170,8 +170,9 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
         double c_re = 0.0, c_im = 0.0;
 
         for (int t = 0; t < n_tiles; ++t) {
-            const double *tile = ring_wait(sm, g0 + t);
             const int nb = min(kTileBins, n_bins - t * kTileBins);
+            const double *tile = ring_wait(sm, g0 + t, nb, a.arm_length_m);
+            if (tid == 0 && t + kStages < n_tiles) ring_issue(sm, src, lo, n_bins, g0, t + kStages);   // its slot is free: expanded
             double in[kNAcc];
 #pragma unroll
             for (int i = 0; i < kNAcc; ++i) in[i] = 0.0;
@@ -215,9 +216,6 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
             }
 #pragma unroll
             for (int i = 0; i < kNAcc; ++i) acc[i] += in[i];
-
-            __syncthreads();                             // every thread is done with this slot
-            if (tid == 0 && t + kStages < n_tiles) ring_issue(sm, src, n_bins, g0, t + kStages);
         }
         g0 += n_tiles;
 
@@ -236,13 +234,13 @@ __global__ void __launch_bounds__(kThreads) fstat_band_kernel(const __grid_const
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Templates the main kernels do not take: every partition edge to edge with the full model, straight from the
-// per-bin table (every thread walks its own rows; the next bin's row is fetched while this one is evaluated).
+// Templates the main kernels do not take: every partition edge to edge with the full model (every thread walks its
+// own bins and expands their rows itself).
 // Grid = slots (x) by partitions (y, strided).  Recentred basis (c at the partition's first bin).
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) band_short_kernel(const double *__restrict__ table, const double *__restrict__ coef,
-                                                         const BandCommon b, int64_t P_pad,
-                                                         const __grid_constant__ OrbitCoef orb)
+__global__ void __launch_bounds__(128) band_short_kernel(const double2 *__restrict__ dwp, const double2 *__restrict__ fw,
+                                                         double L, const double *__restrict__ coef, const BandCommon b,
+                                                         int64_t P_pad, const __grid_constant__ OrbitCoef orb)
 {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P_pad || b.valid[p] == 0) return;
@@ -260,28 +258,17 @@ __global__ void __launch_bounds__(128) band_short_kernel(const double *__restric
 #pragma unroll
         for (int i = 0; i < kNAcc; ++i) acc[i] = 0.0;
         double c_re = 0.0, c_im = 0.0;                       // recentred basis: c = T'_x / T'_+ at the partition's first bin
-        double2 cur[12], nxt[12];
-        {
-            const double2 *r0 = reinterpret_cast<const double2 *>(table + (int64_t)b0 * kTabW);
-#pragma unroll
-            for (int i = 0; i < 12; ++i) cur[i] = r0[i];
-        }
 #pragma unroll 1
         for (int k = b0; k < b1; ++k) {
-            {
-                const double2 *rn = reinterpret_cast<const double2 *>(table + (int64_t)min(k + 1, b1 - 1) * kTabW);
-#pragma unroll
-                for (int i = 0; i < 12; ++i) nxt[i] = rn[i];
-            }
-            const double2 dwv = cur[10];
+            const double2 dwv = dwp[k], fwv = fw[k];
+            __align__(16) double rowbuf[kTabW];
+            fill_basis_row(fwv.x, L, rowbuf);                // every thread walks its own bins: rows expanded in registers
             double psi, sps, cps, tpr, tpi, tcr, tci;
-            bin_template(cur, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
+            bin_template(reinterpret_cast<const double2 *>(rowbuf), c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
             if (k == b0) choose_basis(tpr, tpi, tcr, tci, c_re, c_im);
             const double qr = fma(dwv.x, cps, -dwv.y * sps);
             const double qi = fma(dwv.x, sps, dwv.y * cps);
-            accumulate_bin(qr, qi, cur[11].x, tpr, tpi, tcr, tci, c_re, c_im, acc);
-#pragma unroll
-            for (int i = 0; i < 12; ++i) cur[i] = nxt[i];
+            accumulate_bin(qr, qi, fwv.y, tpr, tpi, tcr, tci, c_re, c_im, acc);
         }
         write_partition(acc, c_re, c_im, (int64_t)particle * N + j, b.Fk, b.amp);
     }
@@ -378,11 +365,12 @@ __global__ void __launch_bounds__(128) band_fsum_kernel(const double *__restrict
     if (lane == 0) F[q] = f;
 }
 
-cudaError_t launch_band_short(const double *table, const double *coef, const BandCommon &b, int64_t P_pad,
-                              const OrbitCoef &orb, cudaStream_t st)
+cudaError_t launch_band_short(const double *dwp, const double *fw, double arm_length_m, const double *coef,
+                              const BandCommon &b, int64_t P_pad, const OrbitCoef &orb, cudaStream_t st)
 {
     const int gy = b.N < 32 ? b.N : 32;                     // (usually no template takes this path: keep the grid small)
-    band_short_kernel<<<dim3((unsigned)(P_pad / 128), (unsigned)gy), 128, 0, st>>>(table, coef, b, P_pad, orb);
+    band_short_kernel<<<dim3((unsigned)(P_pad / 128), (unsigned)gy), 128, 0, st>>>(
+        reinterpret_cast<const double2 *>(dwp), reinterpret_cast<const double2 *>(fw), arm_length_m, coef, b, P_pad, orb);
     return cudaGetLastError();
 }
 

@@ -1,6 +1,7 @@
 // fstat_direct.cuh -- device pieces shared by the two kernels that evaluate the model at every bin
 // (fstat_main_kernel in fstat_kernels.cu, fstat_band_kernel in fstat_band.cu) and by the epilogues:
-// the TMA ring of table rows, one (particle, bin) of the template, and 2 F_k from the eight sums.
+// the TMA ring of per-bin inputs and their expansion into rows, one (particle, bin) of the template, and 2 F_k from
+// the eight sums.
 #pragma once
 #include "fstat_device.cuh"
 #include "fstat_internal.h"
@@ -8,36 +9,61 @@
 
 namespace fstat {
 
+// The full-model kernels stream their bins through shared memory in tiles of kTileBins: the per-bin inputs -- the folded
+// data dw' (16 bytes per bin) and the pair (f, w') (16 bytes per bin) -- arrive by TMA bulk copies into a ring of
+// staging slots, and the CTA expands each tile into the 24-column rows model_eval reads (the particle-independent
+// basis of the phase, its derivative and the arm phases: fill_basis_row, one thread per bin), so that no 192-byte
+// per-bin table has to live in HBM.  The expansion costs ~1.5 % of a tile's evaluation (64 threads x ~500
+// instructions against 128 threads x 64 bins x ~530).
 struct __align__(16) MainSmem {
-    double tile[kStages][kTileBins * kTabW];
+    double tile[kTileBins * kTabW];            // the expanded rows of the tile being evaluated
+    double2 stage[kStages][2][kTileBins];      // [slot][0: dw', 1: (f, w')][bin]
     uint64_t full[kStages];
 };
 
-// The ring of table-row tiles both full-model kernels stream their bins through (one elected thread issues the
-// TMA bulk copies; g0 = tiles this CTA has consumed so far = ring position of the work item's first tile).
-__device__ __forceinline__ void ring_issue(MainSmem &sm, const double *src, int n_bins, int g0, int t)
+struct BinSource {
+    const double2 *dwp;    // [n_bins] folded data
+    const double2 *fw;     // [n_bins] (f, w')
+};
+
+// (one elected thread issues the TMA bulk copies; g0 = tiles this CTA has consumed so far = ring position of the work
+// item's first tile; lo = the work item's first bin)
+__device__ __forceinline__ void ring_issue(MainSmem &sm, const BinSource &src, int lo, int n_bins, int g0, int t)
 {
     const int slot = (g0 + t) % kStages;
     const int nb = min(kTileBins, n_bins - t * kTileBins);
-    const uint32_t bytes = (uint32_t)nb * kTabW * sizeof(double);
-    mbar_expect_tx(&sm.full[slot], bytes);
-    tma_load_1d(sm.tile[slot], src + (int64_t)t * kTileBins * kTabW, bytes, &sm.full[slot]);
+    const uint32_t bytes = (uint32_t)nb * (uint32_t)sizeof(double2);
+    mbar_expect_tx(&sm.full[slot], 2 * bytes);
+    tma_load_1d(sm.stage[slot][0], src.dwp + lo + t * kTileBins, bytes, &sm.full[slot]);
+    tma_load_1d(sm.stage[slot][1], src.fw + lo + t * kTileBins, bytes, &sm.full[slot]);
 }
 
-__device__ __forceinline__ void ring_prologue(MainSmem &sm, const double *src, int n_bins, int n_tiles, int g0)
+__device__ __forceinline__ void ring_prologue(MainSmem &sm, const BinSource &src, int lo, int n_bins, int n_tiles, int g0)
 {
 #pragma unroll
     for (int s = 0; s < kStages; ++s)
-        if (s < n_tiles) ring_issue(sm, src, n_bins, g0, s);
+        if (s < n_tiles) ring_issue(sm, src, lo, n_bins, g0, s);
 }
 
-__device__ __forceinline__ const double *ring_wait(MainSmem &sm, int g)
+// Wait for tile g of the ring and expand it into sm.tile (all threads of the CTA call this; two barriers: the previous
+// tile's rows are no longer read, the new rows are complete).  Returns the rows.
+__device__ __forceinline__ const double *ring_wait(MainSmem &sm, int g, int nb, double L)
 {
     const int slot = g % kStages;
     mbar_wait(&sm.full[slot], (uint32_t)((g / kStages) & 1));
-    return sm.tile[slot];
+    __syncthreads();
+    const int b = threadIdx.x;
+    if (b < nb) {
+        const double2 dw = sm.stage[slot][0][b], fw = sm.stage[slot][1][b];
+        double *row = sm.tile + b * kTabW;
+        fill_basis_row(fw.x, L, row);
+        row[T_DWR] = dw.x;
+        row[T_DWI] = dw.y;
+        row[T_W] = fw.y;
+    }
+    __syncthreads();
+    return sm.tile;
 }
-
 
 // One (particle, bin) of the direct kernel: model_eval() plus the linear phase term and the carrier.
 // Returns the carrier phase psi (quarter turns, Doppler phase of spacecraft 1 included), its sine and

@@ -69,7 +69,7 @@ cudaError_t launch_build_nodes(const double *freq, int64_t n_bins, double df, do
 // m + cnt[k], cnt[k] = number of interior partition edges e_1..e_k that are not multiples of S.
 // One thread per node interval; it walks its bins and flushes at every partition edge.
 // =================================================================================================
-__global__ void build_gram_kernel(const double *__restrict__ wtab, const int32_t *__restrict__ edges,
+__global__ void build_gram_kernel(const double2 *__restrict__ fw, const int32_t *__restrict__ edges,
                                   int32_t n_part, int64_t n_bins, int level, const int32_t *__restrict__ cnt,
                                   double *__restrict__ gram)
 {
@@ -96,7 +96,7 @@ __global__ void build_gram_kernel(const double *__restrict__ wtab, const int32_t
             for (int j = 0; j < kNGram; ++j) { out[j] = g[j]; g[j] = 0.0; }
             ++k;
         }
-        const double w = wtab[i];
+        const double w = fw[i].y;
         double l[4];
         lagrange4((double)(i - b0) * rS, l);
         int j = 0;
@@ -110,13 +110,13 @@ __global__ void build_gram_kernel(const double *__restrict__ wtab, const int32_t
     for (int j = 0; j < kNGram; ++j) out[j] = g[j];
 }
 
-cudaError_t launch_build_gram(const double *w, const int32_t *edges, int32_t n_part, int64_t n_bins,
+cudaError_t launch_build_gram(const double *fw, const int32_t *edges, int32_t n_part, int64_t n_bins,
                               int level, const int32_t *cnt, double *gram, cudaStream_t st)
 {
     const int S = kMinStride << level;
     const int64_t n_int = (n_bins + S - 1) / S;
     const int nt = 128;
-    build_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(w, edges, n_part, n_bins, level, cnt, gram);
+    build_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(reinterpret_cast<const double2 *>(fw), edges, n_part, n_bins, level, cnt, gram);
     return cudaGetLastError();
 }
 

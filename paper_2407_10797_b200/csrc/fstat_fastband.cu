@@ -36,7 +36,7 @@ namespace fstat {
 // four nodes): the Gram matrix of the interval's bins up to the END of 8-bin lattice cell k.  The entry of an
 // interval's last cell is the interval's total.  One thread per node interval.
 // =================================================================================================
-__global__ void build_prefix_gram_kernel(const double *__restrict__ w, int64_t n_bins, int level,
+__global__ void build_prefix_gram_kernel(const double2 *__restrict__ fw, int64_t n_bins, int level,
                                          double *__restrict__ pgram)
 {
     const int S = kMinStride << level;
@@ -49,7 +49,7 @@ __global__ void build_prefix_gram_kernel(const double *__restrict__ w, int64_t n
 #pragma unroll
     for (int j = 0; j < kNGram; ++j) g[j] = 0.0;
     for (int64_t i = b0; i < b1; ++i) {
-        const double wi = w[i];
+        const double wi = fw[i].y;
         double l[4];
         lagrange4((double)(i - b0) * rS, l);
         int j = 0;
@@ -65,12 +65,12 @@ __global__ void build_prefix_gram_kernel(const double *__restrict__ w, int64_t n
     }
 }
 
-cudaError_t launch_build_prefix_gram(const double *w, int64_t n_bins, int level, double *pgram, cudaStream_t st)
+cudaError_t launch_build_prefix_gram(const double *fw, int64_t n_bins, int level, double *pgram, cudaStream_t st)
 {
     const int S = kMinStride << level;
     const int64_t n_int = (n_bins + S - 1) / S;
     const int nt = 128;
-    build_prefix_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(w, n_bins, level, pgram);
+    build_prefix_gram_kernel<<<(unsigned)((n_int + nt - 1) / nt), nt, 0, st>>>(reinterpret_cast<const double2 *>(fw), n_bins, level, pgram);
     return cudaGetLastError();
 }
 
@@ -484,7 +484,7 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
                 }
                 const double sgn = uc >= u8 ? 1.0 : -1.0;
                 for (int i = node0 + min(uc, u8); i < node0 + max(uc, u8); ++i) {
-                    const double s = (double)(i - node0), wi = sgn * a.w[i];
+                    const double s = (double)(i - node0), wi = sgn * a.fw[2 * (int64_t)i + 1];
                     const double pr = horner3(mpr, s), pi = horner3(mpi, s), xr = horner3(mcr, s), xi = horner3(mci, s);
                     mm[0] = fma(wi, fma(pr, pr, pi * pi), mm[0]);
                     mm[1] = fma(wi, fma(xr, xr, xi * xi), mm[1]);

@@ -14,8 +14,8 @@ constexpr double kYear = 31557600.0;               // Julian year [s]
 constexpr double kEulerGamma = 0.5772156649015329;
 constexpr double kPi = 3.14159265358979323846;
 
-// ---- per-bin table ("a0", plan time): kTabW doubles per frequency bin, one contiguous row so that a
-// tile of bins is ONE TMA bulk copy.  Phase basis B_j and its derivative D_j = (dB_j/df)/year:
+// ---- row layout of the per-bin basis ("a0"): kTabW doubles per frequency.  Rows exist in HBM only for the nodes of the
+// interpolating kernel (one every 8 bins); the full-model kernels expand their tiles in shared memory (fstat_direct.cuh).  Phase basis B_j and its derivative D_j = (dB_j/df)/year:
 //   Psi [quarter turns] = c1 + c0 f + sum_{j=2..9} c_j B_j(f),   alpha [quarter turns] = a0 + sum c_j D_j(f)
 enum TabCol : int {
     T_F = 0,      // f
@@ -83,7 +83,9 @@ struct SegCrit {
 };
 
 struct MainArgs {
-    const double *table;      // [n_bins][kTabW]
+    const double *dwp;        // [n_bins][2] folded data
+    const double *fw;         // [n_bins][2] (f, w')
+    double arm_length_m;
     const double *coef;       // [kNCoef][P_pad]
     const int32_t *seg_edge;  // [n_seg + 1]
     const int32_t *direct_list;   // work items (group * n_seg + segment) left to the direct kernel ...
@@ -168,7 +170,7 @@ struct BandCommon {
 
 struct FastBandArgs {
     const double *dwp;            // [n_bins][2] folded data
-    const double *w;              // [n_bins] 4 df f^(-7/3) |K_f|^2 / S_n
+    const double *fw;             // [n_bins][2] (f, w' = 4 df f^(-7/3) |K_f|^2 / S_n)
     const double *node;           // [n_node_rows][kTabW]
     const double *pgram[kNLevels];// [ceil(n_bins / 8)][kNGram] prefix Gram matrices
     const double *coef;           // [kNCoef][P_pad]
@@ -184,7 +186,9 @@ struct FastBandArgs {
 
 // the direct kernel with per-thread edges, for the work items the stride selection leaves to it
 struct BandArgs {
-    const double *table;      // [n_bins][kTabW]
+    const double *dwp;        // [n_bins][2] folded data
+    const double *fw;         // [n_bins][2] (f, w')
+    double arm_length_m;
     const double *coef;       // [kNCoef][P_pad]
     const int32_t *seg_edge;  // [n_seg + 1]
     const int32_t *direct_list;
@@ -202,21 +206,21 @@ cudaError_t launch_band_main(const BandArgs &a, int32_t max_ctas, cudaStream_t s
 cudaError_t band_kernel_configure();
 cudaError_t launch_fastband(const FastBandArgs &a, cudaStream_t st);
 cudaError_t fastband_kernel_configure();
-cudaError_t launch_build_prefix_gram(const double *w, int64_t n_bins, int level, double *pgram, cudaStream_t st);
+cudaError_t launch_build_prefix_gram(const double *fw, int64_t n_bins, int level, double *pgram, cudaStream_t st);
 // full model over every partition of the templates the interpolating kernel does not take (band_fast_eligible)
-cudaError_t launch_band_short(const double *table, const double *coef, const BandCommon &b, int64_t P_pad,
-                              const OrbitCoef &orb, cudaStream_t st);
+cudaError_t launch_band_short(const double *dwp, const double *fw, double arm_length_m, const double *coef,
+                              const BandCommon &b, int64_t P_pad, const OrbitCoef &orb, cudaStream_t st);
 // partitions that straddle work segments from their head / tail records; -inf / NaN rows of invalid particles;
 // then F = sum_k F_k.  seg_len = bins per work segment (the last one may be shorter)
 cudaError_t launch_band_stitch(const BandCommon &b, int64_t P, int64_t P_pad, int32_t seg_len, int32_t n_seg, double *F,
                                cudaStream_t st);
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
-                               double df, double arm_length_m, double *table, double *dwp, double *w,
-                               uint32_t *err_bits, cudaStream_t st);
+                               double df, double arm_length_m, double *dwp, double *fw, uint32_t *err_bits,
+                               cudaStream_t st);
 cudaError_t launch_build_nodes(const double *freq, int64_t n_bins, double df, double arm_length_m,
                                int64_t n_rows, double *node, cudaStream_t st);
-cudaError_t launch_build_gram(const double *w, const int32_t *edges, int32_t n_part, int64_t n_bins,
+cudaError_t launch_build_gram(const double *fw, const int32_t *edges, int32_t n_part, int64_t n_bins,
                               int level, const int32_t *cnt, double *gram, cudaStream_t st);
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
@@ -244,7 +248,7 @@ int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out);
 cudaError_t launch_amplitudes(const double *partial, const int32_t *part_seg, const int32_t *valid,
                               const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, double *amp,
                               cudaStream_t st);
-cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
+cudaError_t launch_template(const double *fw, double arm_length_m, const double *coef, int64_t P_pad, int64_t n_bins,
                             const OrbitCoef &orb, int32_t aet, double *u_plus, double *u_cross, cudaStream_t st);
 cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaStream_t st);
 size_t main_kernel_smem_bytes();

@@ -1,6 +1,6 @@
 // fstat_kernels.cu -- sm_100a kernels of the batched semi-coherent F-statistic (arXiv 2407.10797).
 //
-//   build_table_kernel   (a0, plan time)  per-bin, particle-independent factors of Eq. A1/A3 and Eq. 4
+//   build_table_kernel   (a0, plan time)  per-bin, particle-independent factors of Eq. A1 and Eq. 4 folded into the data
 //   prologue_kernel      (a1)             per-particle PN / eccentric phase coefficients and sky vectors
 //   fstat_main_kernel    (a2-a5)          fused phase + t_f + orbit + TDI-X response + inner products;
 //                                         one thread = one particle, bins streamed through shared memory
@@ -23,8 +23,7 @@ namespace fstat {
 // =================================================================================================
 __global__ void build_table_kernel(const double *__restrict__ freq, const double *__restrict__ dw,
                                    const double *__restrict__ isn, int64_t n_bins, double df, double L,
-                                   double *__restrict__ table, double2 *__restrict__ dwp, double *__restrict__ wout,
-                                   uint32_t *__restrict__ err_bits)
+                                   double2 *__restrict__ dwp, double2 *__restrict__ fw, uint32_t *__restrict__ err_bits)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_bins) return;
@@ -39,29 +38,24 @@ __global__ void build_table_kernel(const double *__restrict__ freq, const double
     else if (!(w > 0.0)) err |= ERR_ISN_NONPOS;
     if (err) { atomicOr(err_bits, err); return; }
 
-    double *row = table + i * kTabW;
-    fill_basis_row(f, L, row);
-    const double s2x = row[T_S2X], c2x = row[T_C2X];
+    double s2x, c2x;
+    sincos(2.0 * (kPi * f * L / kC), &s2x, &c2x);          // the same expression as fill_basis_row's T_S2X, T_C2X
     // conj(K_f) = 2 sin 2x (cos 2x + i sin 2x), |K_f|^2 = 4 sin^2 2x   (K_f = -i (1 - z^2))
     const double amp = 4.0 * df * pow(f, -7.0 / 6.0);
     const double kr = 2.0 * s2x * c2x, ki = 2.0 * s2x * s2x;
-    const double qr = amp * (dr * kr - di * ki), qi = amp * (dr * ki + di * kr);
-    row[T_DWR] = qr;
-    row[T_DWI] = qi;
-    const double wp = 4.0 * df * pow(f, -7.0 / 3.0) * (4.0 * s2x * s2x) * w;
-    row[T_W] = wp;
-    wout[i] = wp;
-    dwp[i] = make_double2(qr, qi);
+    dwp[i] = make_double2(amp * (dr * kr - di * ki), amp * (dr * ki + di * kr));
+    fw[i] = make_double2(f, 4.0 * df * pow(f, -7.0 / 3.0) * (4.0 * s2x * s2x) * w);
 }
 
 cudaError_t launch_build_table(const double *freq, const double *dw, const double *isn, int64_t n_bins,
-                               double df, double arm_length_m, double *table, double *dwp, double *w,
-                               uint32_t *err_bits, cudaStream_t st)
+                               double df, double arm_length_m, double *dwp, double *fw, uint32_t *err_bits,
+                               cudaStream_t st)
 {
     const int nt = 256;
     const int64_t nb = (n_bins + nt - 1) / nt;
-    build_table_kernel<<<(unsigned)nb, nt, 0, st>>>(freq, dw, isn, n_bins, df, arm_length_m, table,
-                                                    reinterpret_cast<double2 *>(dwp), w, err_bits);
+    build_table_kernel<<<(unsigned)nb, nt, 0, st>>>(freq, dw, isn, n_bins, df, arm_length_m,
+                                                    reinterpret_cast<double2 *>(dwp), reinterpret_cast<double2 *>(fw),
+                                                    err_bits);
     return cudaGetLastError();
 }
 
@@ -306,9 +300,9 @@ __device__ __forceinline__ void main_kernel_body(const MainArgs &a)
         const int lo = a.seg_edge[seg], hi = a.seg_edge[seg + 1];
         const int n_bins = hi - lo;
         const int n_tiles = (n_bins + kTileBins - 1) / kTileBins;
-        const double *src = a.table + (int64_t)lo * kTabW;
+        const BinSource src{reinterpret_cast<const double2 *>(a.dwp), reinterpret_cast<const double2 *>(a.fw)};
 
-        if (tid == 0) ring_prologue(sm, src, n_bins, n_tiles, g0);
+        if (tid == 0) ring_prologue(sm, src, lo, n_bins, n_tiles, g0);
 
         // per-particle coefficients (a1), coalesced
         double c[kNCoef];
@@ -322,8 +316,9 @@ __device__ __forceinline__ void main_kernel_body(const MainArgs &a)
         double c_re = 0.0, c_im = 0.0;
 
         for (int t = 0; t < n_tiles; ++t) {
-            const double *tile = ring_wait(sm, g0 + t);
             const int nb = min(kTileBins, n_bins - t * kTileBins);
+            const double *tile = ring_wait(sm, g0 + t, nb, a.arm_length_m);
+            if (tid == 0 && t + kStages < n_tiles) ring_issue(sm, src, lo, n_bins, g0, t + kStages);   // its slot is free: expanded
             double in[kNAcc];
 #pragma unroll
             for (int j = 0; j < kNAcc; ++j) in[j] = 0.0;
@@ -347,9 +342,6 @@ __device__ __forceinline__ void main_kernel_body(const MainArgs &a)
             }
 #pragma unroll
             for (int j = 0; j < kNAcc; ++j) acc[j] += in[j];
-
-            __syncthreads();                             // every thread is done with this slot
-            if (tid == 0 && t + kStages < n_tiles) ring_issue(sm, src, n_bins, g0, t + kStages);
         }
         g0 += n_tiles;
 
@@ -391,11 +383,11 @@ cudaError_t launch_main(const MainArgs &a, cudaStream_t st)
 
 // =================================================================================================
 // Template dump (not on the hot path): u_P(f_k) = f^(-7/6) K_f T'_P exp(-i psi) for ONE particle over the
-// whole grid, one thread per bin, through the same bin_template() the main kernel uses.  Serves
+// whole grid, one thread per bin (its row expanded in registers), through the same bin_template() the main kernel uses.  Serves
 // fstat_eval_template (injection synthesis, element-wise parity tests of a2/a3).
 // =================================================================================================
 template <bool AET>
-__global__ void __launch_bounds__(128) template_kernel(const double *__restrict__ table,
+__global__ void __launch_bounds__(128) template_kernel(const double2 *__restrict__ fw, double L,
                                                        const double *__restrict__ coef, int64_t P_pad,
                                                        int64_t n_bins, const __grid_constant__ OrbitCoef orb,
                                                        double2 *__restrict__ u_plus, double2 *__restrict__ u_cross)
@@ -405,10 +397,12 @@ __global__ void __launch_bounds__(128) template_kernel(const double *__restrict_
     double c[kNCoef];
 #pragma unroll
     for (int j = 0; j < kNCoef; ++j) c[j] = coef[(int64_t)j * P_pad];
-    const double2 *row = reinterpret_cast<const double2 *>(table + i * kTabW);
+    __align__(16) double rowbuf[kTabW];
+    const double f = fw[i].x;
+    fill_basis_row(f, L, rowbuf);
+    const double2 *row = reinterpret_cast<const double2 *>(rowbuf);
     double psi, sps, cps, tpr, tpi, tcr, tci;
     bin_template<AET>(row, c, orb, psi, sps, cps, tpr, tpi, tcr, tci);
-    const double f = row[0].x;
     const double amp = pow(f, -7.0 / 6.0);
     const double c2x = row[9].x, s2x = row[9].y;
     // K_f = 2 sin(2x) exp(-2 i x);  carrier exp(-i psi) = cps - i sps
@@ -418,17 +412,18 @@ __global__ void __launch_bounds__(128) template_kernel(const double *__restrict_
     u_cross[i] = make_double2(er * tcr - ei * tci, er * tci + ei * tcr);
 }
 
-cudaError_t launch_template(const double *table, const double *coef, int64_t P_pad, int64_t n_bins,
+cudaError_t launch_template(const double *fw, double arm_length_m, const double *coef, int64_t P_pad, int64_t n_bins,
                             const OrbitCoef &orb, int32_t aet, double *u_plus, double *u_cross, cudaStream_t st)
 {
     const int nt = 128;
     const unsigned nb = (unsigned)((n_bins + nt - 1) / nt);
+    const double2 *fw2 = reinterpret_cast<const double2 *>(fw);
     if (aet)
-        template_kernel<true><<<nb, nt, 0, st>>>(table, coef, P_pad, n_bins, orb, reinterpret_cast<double2 *>(u_plus),
-                                                 reinterpret_cast<double2 *>(u_cross));
+        template_kernel<true><<<nb, nt, 0, st>>>(fw2, arm_length_m, coef, P_pad, n_bins, orb,
+                                                 reinterpret_cast<double2 *>(u_plus), reinterpret_cast<double2 *>(u_cross));
     else
-        template_kernel<false><<<nb, nt, 0, st>>>(table, coef, P_pad, n_bins, orb, reinterpret_cast<double2 *>(u_plus),
-                                                  reinterpret_cast<double2 *>(u_cross));
+        template_kernel<false><<<nb, nt, 0, st>>>(fw2, arm_length_m, coef, P_pad, n_bins, orb,
+                                                  reinterpret_cast<double2 *>(u_plus), reinterpret_cast<double2 *>(u_cross));
     return cudaGetLastError();
 }
 

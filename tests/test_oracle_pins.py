@@ -498,6 +498,24 @@ def test_p18_long_double_solve_is_basis_invariant_on_a_near_singular_partition(o
     assert F3[1] == pytest.approx(F3[0], rel=1e-10) and F3[2] == pytest.approx(F3[0], rel=1e-10)
 
 
+def test_eq18_first_order_term_is_far_below_what_any_pin_resolves(orc):
+    """Reading A29: of Eq. 18 (:211) beyond its zeroth term the paper prints only T_A1 = (7/6) / (2 pi f) (Eq. 19 :215);
+    the a^eps_(N,k) of the F_(T_f) filter are 'defined in Appendix 2 of [76]' and not in the paper.  The one term that
+    could be formed from the text, -i T_A1 dG/dt at t_f (k = 1, N = 0), is at most ~1.2e-4 of the zeroth term over the
+    band -- three orders below the 1e-3 mismatch the paper itself accepts (:229) and below the resolution of the
+    time-domain pin P9 (5e-3 in amplitude, 0.03 rad in phase) -- so neither its sign (garbled in the extraction) nor
+    its presence can be checked against anything: it is not built."""
+    rng = np.random.default_rng(18)
+    worst = 0.0
+    for _ in range(100):
+        par = np.array([0.0, 30.0, 0.25, math.acos(rng.uniform(-1, 1)), rng.uniform(0, 2 * math.pi), 0.0])
+        f, t, h = rng.uniform(0.01, 0.1), rng.uniform(0.0, 2.5 * YR), 50.0
+        g0 = np.array(orc.response(par, f, t))
+        dg = (np.array(orc.response(par, f, t + h)) - np.array(orc.response(par, f, t - h))) / (2.0 * h)
+        worst = max(worst, (7.0 / 6.0) / (2.0 * math.pi * f) * np.abs(dg).max() / np.abs(g0).max())
+    assert 1e-6 < worst < 3e-4
+
+
 def test_semicoherent_peak_broadens_with_more_partitions(orc):
     """PAPER.md:124-126 / Fig. 1: away from the true chirp mass the noiseless semi-coherent statistic
     keeps a larger fraction of its peak value when N_seg is larger."""
