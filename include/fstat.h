@@ -273,6 +273,11 @@ FSTAT_API int32_t fstat_plan_device(const fstat_plan *plan);
 /* Number of CTAs the interpolating main kernel launches for P particles: particle groups of 128 x chunks of
  * consecutive segments (a chunk is one segment unless the partitions are short). */
 FSTAT_API int64_t fstat_plan_n_ctas(const fstat_plan *plan, int64_t P);
+/* Work of the interpolating kernel in the most recent fstat_eval_batch_bands call on this plan, counted per WARP of 32
+ * templates (a warp walks the union of its lanes' bands): out HOST [5] = bins, node intervals, node intervals in which
+ * some lane had a partition edge, runs (work segments entered), and the internal-invariant flag (0 = fine).
+ * Synchronises the device.  For the roofline of the bench line. */
+FSTAT_API fstat_status fstat_plan_band_stats(fstat_plan *plan, int64_t *out);
 /* Bytes of device memory held by the plan's persistent tables: the folded data and (f, w') (32 bytes per bin), the
  * node rows (192 bytes per 8 bins), the Gram matrices of the current partitions and, after the first
  * fstat_eval_batch_bands call, the prefix Gram tables (70 bytes per bin).  Workspace (grown per batch size) not included. */

@@ -19,7 +19,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
     "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_amplitudes_bands", "fstat_eval_batch_channels", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
-    "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count", "fstat_plan_table_bytes",
+    "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count", "fstat_plan_table_bytes", "fstat_plan_band_stats",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error", "fstat_extrinsic_from_amplitudes", "fstat_amplitudes_from_extrinsic",
     "fstat_pso_default_options", "fstat_pso_create", "fstat_pso_iterate", "fstat_pso_best", "fstat_pso_state",
@@ -99,6 +99,8 @@ def load_library():
         L.fstat_plan_n_ctas.restype = i64
         L.fstat_plan_launch_count.argtypes = [vp]
         L.fstat_plan_launch_count.restype = i64
+        L.fstat_plan_band_stats.argtypes = [vp, C.POINTER(i64)]
+        L.fstat_plan_band_stats.restype = C.c_int
         L.fstat_plan_table_bytes.argtypes = [vp]
         L.fstat_plan_table_bytes.restype = i64
         L.fstat_plan_level_bins.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
@@ -405,6 +407,14 @@ def fstat_plan_n_ctas(plan: Plan, P: int) -> int:
 
 def fstat_plan_launch_count(plan: Plan) -> int:
     return int(load_library().fstat_plan_launch_count(plan.handle))
+
+
+def fstat_plan_band_stats(plan: Plan) -> np.ndarray:
+    """[5] int64: warp-level bins, node intervals, intervals with a cut, runs of the last band call; invariant flag."""
+    out = np.zeros(5, dtype=np.int64)
+    _check(load_library().fstat_plan_band_stats(plan.handle, out.ctypes.data_as(C.POINTER(C.c_int64))),
+           "fstat_plan_band_stats", plan)
+    return out
 
 
 def fstat_plan_table_bytes(plan: Plan) -> int:

@@ -78,7 +78,7 @@ struct fstat_plan {
     bool pgram_built = false;
     int32_t *d_band = nullptr; size_t band_cap = 0;       // [2][P_pad] k_lo, k_hi per slot
     double *d_rec = nullptr; size_t rec_cap = 0;          // [n_seg][2][kNPartial][P_pad] head / tail fragments of the work segments
-    uint32_t *d_err = nullptr;                            // device flag raised by an internal invariant
+    uint32_t *d_err = nullptr;                            // device flag raised by an internal invariant, then [4] 64-bit work counters
     double *d_band_fk = nullptr; size_t band_fk_cap = 0;  // [P][n_seg] when the caller passes Fk = NULL
     int64_t *d_band_out = nullptr; size_t band_out_cap = 0; // [P][2] (host-buffer call)
     bool last_was_band = false;         // fstat_plan_level_bins reports the band plan's stride mix
@@ -610,6 +610,21 @@ int32_t fstat_plan_n_part(const fstat_plan *pl) { return pl ? pl->n_part : 0; }
 int32_t fstat_plan_device(const fstat_plan *pl) { return pl ? pl->device : -1; }
 int64_t fstat_plan_launch_count(const fstat_plan *pl) { return pl ? pl->n_launches : 0; }
 
+fstat_status fstat_plan_band_stats(fstat_plan *pl, int64_t *out)
+{
+    if (!pl || !out) return FSTAT_EINVAL;
+    for (int i = 0; i < 5; ++i) out[i] = 0;
+    if (!pl->d_err) return FSTAT_OK;
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    unsigned long long h[5];
+    CU_TRY(pl, cudaDeviceSynchronize());
+    CU_TRY(pl, cudaMemcpy(h, pl->d_err, sizeof h, cudaMemcpyDeviceToHost));
+    for (int i = 0; i < 4; ++i) out[i] = (int64_t)h[i + 1];
+    out[4] = (int64_t)(h[0] & 0xffffffffull);
+    return FSTAT_OK;
+}
+
 int64_t fstat_plan_table_bytes(const fstat_plan *pl)
 {
     if (!pl) return 0;
@@ -910,10 +925,11 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     CU_TRY(pl, grow(&cp->d_level, &cp->level_cap, (size_t)cp->n_seg * (size_t)n_groups));
     CU_TRY(pl, grow(&cp->d_direct, &cp->direct_cap, (size_t)cp->n_seg * (size_t)n_groups + 1));
     CU_TRY(pl, grow(&cp->d_rec, &cp->rec_cap, (size_t)cp->n_seg * 2 * kNPartial * (size_t)P_pad));
-    if (!pl->d_err) {
-        CU_TRY(pl, cudaMalloc((void **)&pl->d_err, sizeof(uint32_t)));
-        CU_TRY(pl, cudaMemset(pl->d_err, 0, sizeof(uint32_t)));
+    if (!pl->d_err) {                                  // [0]: flag (2 words), then four 64-bit counters
+        CU_TRY(pl, cudaMalloc((void **)&pl->d_err, 5 * sizeof(unsigned long long)));
+        CU_TRY(pl, cudaMemset(pl->d_err, 0, 5 * sizeof(unsigned long long)));
     }
+    CU_TRY(pl, cudaMemsetAsync(reinterpret_cast<unsigned long long *>(pl->d_err) + 1, 0, 4 * sizeof(unsigned long long), st));
     cp->last_groups = (int32_t)n_groups;
 
     // slots ranked by the position of the band (not by chirp mass): the 128 templates of a CTA overlap at both ends
@@ -946,6 +962,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     bc.Fk = Fk;
     bc.amp = amp;
     bc.err = pl->d_err;
+    bc.stats = reinterpret_cast<unsigned long long *>(pl->d_err) + 1;
     bc.N = n_seg;
     bc.C = edge_lattice;
     bc.n_bins = (int32_t)pl->n_bins;

@@ -287,6 +287,7 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
     bool need_basis = true;
     double c_re = 0.0, c_im = 0.0;
     bool ring_ok = false;                                    // the node ring holds nodes m-2 .. m+2 of the next interval
+    uint32_t st_bins = 0, st_int = 0, st_cut = 0;            // this warp's work, for the roofline of the bench line
 
   for (int tl = 0; tl < n_tiles; ++tl) {
     const int tb0 = max(lo, (t_first + tl) << kFastTileShift), tb1 = min(hi, (t_first + tl + 1) << kFastTileShift);
@@ -338,6 +339,9 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
         const double2 *tp = &sm.tile[tl % kBandStages][j0 & (kFastTile - 1)];
         const int nb = j1 - j0;
         const uint32_t cut_rel = (uint32_t)(cut - j0);       // >= nb: no cut of this thread in this interval
+        st_bins += (uint32_t)nb;
+        st_int += 1u;
+        st_cut += __any_sync(0xffffffffu, cut_rel < (uint32_t)nb) ? 1u : 0u;
 
         // ---- per bin: the same recurrences as fstat_fast_kernel (19 FP64 instructions per bin); a thread whose cut
         // falls into a 4-bin run stores A_0..A_3 as they stand IN FRONT of its cut bin
@@ -534,6 +538,12 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
     __syncthreads();                                         // every warp is done with this tile
     if (tid == 0 && tl + kBandStages < n_tiles) issue_tile(tl + kBandStages);
   }
+    if ((tid & 31) == 0 && st_int > 0u && a.b.stats != nullptr) {
+        atomicAdd(&a.b.stats[0], (unsigned long long)st_bins);
+        atomicAdd(&a.b.stats[1], (unsigned long long)st_int);
+        atomicAdd(&a.b.stats[2], (unsigned long long)st_cut);
+        atomicAdd(&a.b.stats[3], 1ull);
+    }
     // ---- what is left after the last edge.  Partition j either goes on in the next work segment (tail fragment) or
     // closes exactly at the end of this one (cut == hi): finished here if it also began here, else its closing fragment
     if (j >= 0 && j < N) {

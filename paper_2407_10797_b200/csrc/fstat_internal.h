@@ -163,6 +163,7 @@ struct BandCommon {
     double *Fk;               // [P][N]
     double *amp;              // [P][N][4] or nullptr
     uint32_t *err;            // device flag: internal invariant violated
+    unsigned long long *stats;// [4] warp-level work of the interpolating kernel in this call: bins, node intervals, intervals with a cut, runs
     int32_t N;                // partitions per template (the paper's N_seg)
     int32_t C;                // edges are multiples of this many bins (reading A26)
     int32_t n_bins;
