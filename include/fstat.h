@@ -343,6 +343,13 @@ FSTAT_API void fstat_pso_default_options(fstat_pso_options *opts);
 FSTAT_API fstat_status fstat_pso_create(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
                                         int32_t n_iter_total, const double *lo, const double *hi, uint64_t seed,
                                         const fstat_pso_options *opts, void *cuda_stream);
+/* The same with one box PER SWARM: lo, hi HOST [n_swarms][6].  The hierarchy of PAPER.md:168-174 runs its PSO runs over
+ * different boxes (24 t_c intervals in stage 1, 24 candidate-centred boxes in stage 2): one object and one batched
+ * evaluation per iteration serve them all; fstat_pso_best returns the best of every swarm, the best-of-runs per box
+ * (:160) is a maximum over the swarms that share a box. */
+FSTAT_API fstat_status fstat_pso_create_boxes(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
+                                              int32_t n_iter_total, const double *lo, const double *hi, uint64_t seed,
+                                              const fstat_pso_options *opts, void *cuda_stream);
 /* Advance all swarms by n_iter iterations; only enqueues work. */
 FSTAT_API fstat_status fstat_pso_iterate(fstat_pso *pso, int32_t n_iter, void *cuda_stream);
 /* Best position (physical parameters) and fitness of every swarm so far: HOST [n_swarms][6], [n_swarms].

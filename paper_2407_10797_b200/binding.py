@@ -22,7 +22,7 @@ EXPORTED_SYMBOLS = (
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count", "fstat_plan_table_bytes", "fstat_plan_band_stats",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
     "fstat_status_str", "fstat_last_error", "fstat_extrinsic_from_amplitudes", "fstat_amplitudes_from_extrinsic",
-    "fstat_pso_default_options", "fstat_pso_create", "fstat_pso_iterate", "fstat_pso_best", "fstat_pso_state",
+    "fstat_pso_default_options", "fstat_pso_create", "fstat_pso_create_boxes", "fstat_pso_iterate", "fstat_pso_best", "fstat_pso_state",
     "fstat_pso_iterations_done", "fstat_pso_destroy",
 )
 
@@ -115,6 +115,8 @@ def load_library():
         L.fstat_pso_default_options.restype = None
         L.fstat_pso_create.argtypes = [C.POINTER(vp), vp, i32, i32, i32, dp, dp, C.c_uint64, C.POINTER(PsoOptions), vp]
         L.fstat_pso_create.restype = C.c_int
+        L.fstat_pso_create_boxes.argtypes = [C.POINTER(vp), vp, i32, i32, i32, dp, dp, C.c_uint64, C.POINTER(PsoOptions), vp]
+        L.fstat_pso_create_boxes.restype = C.c_int
         L.fstat_pso_iterate.argtypes = [vp, i32, vp]
         L.fstat_pso_iterate.restype = C.c_int
         L.fstat_pso_best.argtypes = [vp, dp, dp, vp]
@@ -490,13 +492,20 @@ def fstat_pso_default_options(**kw) -> PsoOptions:
 
 def fstat_pso_create(plan: Plan, n_swarms: int, n_particles: int, n_iter_total: int, lo, hi, seed: int = 0,
                      opts: Optional[PsoOptions] = None, stream=None) -> Pso:
-    lo = np.ascontiguousarray(lo, dtype=np.float64).reshape(6)
-    hi = np.ascontiguousarray(hi, dtype=np.float64).reshape(6)
+    """lo, hi: [6] (one box for every swarm -> fstat_pso_create) or [n_swarms][6] (one box per swarm ->
+    fstat_pso_create_boxes)."""
+    lo = np.ascontiguousarray(lo, dtype=np.float64)
+    hi = np.ascontiguousarray(hi, dtype=np.float64)
+    per_swarm = lo.ndim == 2
+    lo = lo.reshape(int(n_swarms), 6) if per_swarm else lo.reshape(6)
+    hi = hi.reshape(int(n_swarms), 6) if per_swarm else hi.reshape(6)
     out = C.c_void_p()
     dp = C.POINTER(C.c_double)
-    st = load_library().fstat_pso_create(C.byref(out), plan.handle, int(n_swarms), int(n_particles), int(n_iter_total),
-                                         lo.ctypes.data_as(dp), hi.ctypes.data_as(dp), C.c_uint64(int(seed)),
-                                         C.byref(opts) if opts is not None else None, _stream_ptr(stream))
+    L = load_library()
+    fn = L.fstat_pso_create_boxes if per_swarm else L.fstat_pso_create
+    st = fn(C.byref(out), plan.handle, int(n_swarms), int(n_particles), int(n_iter_total),
+            lo.ctypes.data_as(dp), hi.ctypes.data_as(dp), C.c_uint64(int(seed)),
+            C.byref(opts) if opts is not None else None, _stream_ptr(stream))
     if st != 0:
         raise FstatError(st, "fstat_pso_create", fstat_last_error(plan))
     return Pso(out.value, plan, n_swarms, n_particles)

@@ -17,6 +17,7 @@
 
 #include <new>
 #include <string>
+#include <vector>
 
 namespace {
 
@@ -60,9 +61,11 @@ __device__ inline void write_params(const double *x, const double *lo, const dou
         par[d] = inside ? __dadd_rn(lo[d], __dmul_rn(x[d], __dsub_rn(hi[d], lo[d]))) : nan;
 }
 
-struct Box { double lo[kDim], hi[kDim]; };
+// boxes: [n_swarms][2][kDim] (lo, then hi) on the device: every swarm searches its own box (the hierarchy's stages run
+// one swarm set per t_c interval / candidate)
 
-__global__ void pso_init_kernel(int32_t n, uint64_t seed, double vmax, Box box, double *__restrict__ x,
+__global__ void pso_init_kernel(int32_t n, int32_t n_particles, uint64_t seed, double vmax,
+                                const double *__restrict__ boxes, double *__restrict__ x,
                                 double *__restrict__ v, double *__restrict__ params)
 {
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -75,7 +78,8 @@ __global__ void pso_init_kernel(int32_t n, uint64_t seed, double vmax, Box box, 
         x[g * kDim + d] = xx[d];
         v[g * kDim + d] = clampv(__dsub_rn(u[6 + d], xx[d]), vmax);   // v ~ U[a - x, b - x]  (:158)
     }
-    write_params(xx, box.lo, box.hi, params + (int64_t)g * kDim);
+    const double *bx = boxes + (g / n_particles) * 2 * kDim;
+    write_params(xx, bx, bx + kDim, params + (int64_t)g * kDim);
 }
 
 // first evaluation: the personal best is the initial position
@@ -90,7 +94,8 @@ __global__ void pso_first_best_kernel(int32_t n, const double *__restrict__ x, c
 }
 
 __global__ void pso_step_kernel(int32_t n, int32_t n_particles, uint32_t it, uint64_t seed, double w, double c1,
-                                double c2, double vmax, Box box, double *__restrict__ x, double *__restrict__ v,
+                                double c2, double vmax, const double *__restrict__ boxes, double *__restrict__ x,
+                                double *__restrict__ v,
                                 const double *__restrict__ pbest, const double *__restrict__ pbest_f,
                                 double *__restrict__ params)
 {
@@ -120,7 +125,8 @@ __global__ void pso_step_kernel(int32_t n, int32_t n_particles, uint32_t it, uin
     // touched here) -- x itself is private to the thread
 #pragma unroll
     for (int d = 0; d < kDim; ++d) x[g * kDim + d] = xx[d];
-    write_params(xx, box.lo, box.hi, params + (int64_t)g * kDim);
+    const double *bx = boxes + sw * 2 * kDim;
+    write_params(xx, bx, bx + kDim, params + (int64_t)g * kDim);
 }
 
 __global__ void pso_update_best_kernel(int32_t n, const double *__restrict__ x, const double *__restrict__ F,
@@ -136,7 +142,7 @@ __global__ void pso_update_best_kernel(int32_t n, const double *__restrict__ x, 
 }
 
 // one block per swarm: arg max of pbest_f (lowest index on ties), mapped to physical parameters
-__global__ void __launch_bounds__(128) pso_swarm_best_kernel(int32_t n_particles, Box box,
+__global__ void __launch_bounds__(128) pso_swarm_best_kernel(int32_t n_particles, const double *__restrict__ boxes,
                                                              const double *__restrict__ pbest,
                                                              const double *__restrict__ pbest_f,
                                                              double *__restrict__ best_params,
@@ -165,8 +171,9 @@ __global__ void __launch_bounds__(128) pso_swarm_best_kernel(int32_t n_particles
         const int i = (si[0] == 0x7fffffff) ? 0 : si[0];
         const double *pb = pbest + ((int64_t)sw * n_particles + i) * kDim;
         best_f[sw] = sf[0];
+        const double *lo = boxes + (int64_t)sw * 2 * kDim, *hi = lo + kDim;
         for (int d = 0; d < kDim; ++d)
-            best_params[(int64_t)sw * kDim + d] = __dadd_rn(box.lo[d], __dmul_rn(pb[d], __dsub_rn(box.hi[d], box.lo[d])));
+            best_params[(int64_t)sw * kDim + d] = __dadd_rn(lo[d], __dmul_rn(pb[d], __dsub_rn(hi[d], lo[d])));
     }
 }
 
@@ -181,7 +188,7 @@ struct fstat_pso {
     uint32_t it_done = 0;
     uint64_t seed = 0;
     fstat_pso_options opt{};
-    Box box{};
+    double *d_boxes = nullptr;            // [n_swarms][2][kDim]
     double *d_x = nullptr, *d_v = nullptr, *d_pbest = nullptr, *d_pbest_f = nullptr, *d_params = nullptr, *d_F = nullptr;
     double *d_best_params = nullptr, *d_best_f = nullptr;
     std::string err;
@@ -222,7 +229,7 @@ void fstat_pso_destroy(fstat_pso *ps)
     cudaGetDevice(&prev);
     if (dev >= 0) cudaSetDevice(dev);
     cudaFree(ps->d_x); cudaFree(ps->d_v); cudaFree(ps->d_pbest); cudaFree(ps->d_pbest_f); cudaFree(ps->d_params);
-    cudaFree(ps->d_F); cudaFree(ps->d_best_params); cudaFree(ps->d_best_f);
+    cudaFree(ps->d_F); cudaFree(ps->d_best_params); cudaFree(ps->d_best_f); cudaFree(ps->d_boxes);
     if (prev >= 0) cudaSetDevice(prev);
     delete ps;
 }
@@ -239,7 +246,8 @@ static fstat_status pso_create_impl(fstat_pso *ps, cudaStream_t st)
     PSO_TRY(ps, cudaMalloc((void **)&ps->d_best_params, (size_t)ps->n_swarms * kDim * sizeof(double)));
     PSO_TRY(ps, cudaMalloc((void **)&ps->d_best_f, (size_t)ps->n_swarms * sizeof(double)));
     const int nt = 128, nb = (ps->n + nt - 1) / nt;
-    pso_init_kernel<<<nb, nt, 0, st>>>(ps->n, ps->seed, ps->opt.v_max, ps->box, ps->d_x, ps->d_v, ps->d_params);
+    pso_init_kernel<<<nb, nt, 0, st>>>(ps->n, ps->n_particles, ps->seed, ps->opt.v_max, ps->d_boxes, ps->d_x, ps->d_v,
+                                       ps->d_params);
     PSO_TRY(ps, cudaGetLastError());
     fstat_status s = pso_fitness(ps, st);
     if (s != FSTAT_OK) { ps->err = fstat_last_error(ps->plan); return s; }
@@ -248,9 +256,11 @@ static fstat_status pso_create_impl(fstat_pso *ps, cudaStream_t st)
     return FSTAT_OK;
 }
 
-fstat_status fstat_pso_create(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
-                              int32_t n_iter_total, const double *lo, const double *hi, uint64_t seed,
-                              const fstat_pso_options *opts, void *stream)
+// boxes_h: HOST [n_box][2][kDim]-like input given as lo [n_box][kDim], hi [n_box][kDim]; n_box = 1 (one box for every
+// swarm) or n_swarms
+static fstat_status pso_create_common(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
+                                      int32_t n_iter_total, const double *lo, const double *hi, int32_t n_box,
+                                      uint64_t seed, const fstat_pso_options *opts, void *stream)
 {
     if (!out) return FSTAT_EINVAL;
     *out = nullptr;
@@ -263,21 +273,48 @@ fstat_status fstat_pso_create(fstat_pso **out, fstat_plan *plan, int32_t n_swarm
     if (!(o.v_max > 0.0) || !isfinite(o.c1) || !isfinite(o.c2) || !isfinite(o.w_start) || !isfinite(o.w_end) ||
         o.band_n_seg < 0 || (o.band_n_seg >= 1 && o.band_lattice < 1))
         return FSTAT_EINVAL;
-    for (int d = 0; d < kDim; ++d)
+    for (int64_t d = 0; d < (int64_t)n_box * kDim; ++d)
         if (!isfinite(lo[d]) || !isfinite(hi[d]) || !(hi[d] >= lo[d])) return FSTAT_EINVAL;
     fstat_pso *ps = new (std::nothrow) fstat_pso;
     if (!ps) return FSTAT_ENOMEM;
     ps->plan = plan; ps->n_swarms = n_swarms; ps->n_particles = n_particles; ps->n_iter_total = n_iter_total;
     ps->n = n_swarms * n_particles; ps->seed = seed; ps->opt = o;
-    for (int d = 0; d < kDim; ++d) { ps->box.lo[d] = lo[d]; ps->box.hi[d] = hi[d]; }
+    std::vector<double> boxes((size_t)n_swarms * 2 * kDim);
+    for (int32_t sw = 0; sw < n_swarms; ++sw) {
+        const int64_t b = n_box == 1 ? 0 : sw;
+        for (int d = 0; d < kDim; ++d) {
+            boxes[((size_t)sw * 2 + 0) * kDim + d] = lo[b * kDim + d];
+            boxes[((size_t)sw * 2 + 1) * kDim + d] = hi[b * kDim + d];
+        }
+    }
     int prev = -1;
     cudaGetDevice(&prev);
     cudaSetDevice(fstat_plan_device(plan));
-    const fstat_status s = pso_create_impl(ps, (cudaStream_t)stream);
+    fstat_status s = FSTAT_OK;
+    if (cudaMalloc((void **)&ps->d_boxes, boxes.size() * sizeof(double)) != cudaSuccess ||
+        cudaMemcpy(ps->d_boxes, boxes.data(), boxes.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        s = FSTAT_ECUDA;
+    }
+    if (s == FSTAT_OK) s = pso_create_impl(ps, (cudaStream_t)stream);
     if (prev >= 0) cudaSetDevice(prev);
     if (s != FSTAT_OK) { fstat_pso_destroy(ps); return s; }
     *out = ps;
     return FSTAT_OK;
+}
+
+fstat_status fstat_pso_create(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
+                              int32_t n_iter_total, const double *lo, const double *hi, uint64_t seed,
+                              const fstat_pso_options *opts, void *stream)
+{
+    return pso_create_common(out, plan, n_swarms, n_particles, n_iter_total, lo, hi, 1, seed, opts, stream);
+}
+
+fstat_status fstat_pso_create_boxes(fstat_pso **out, fstat_plan *plan, int32_t n_swarms, int32_t n_particles,
+                                    int32_t n_iter_total, const double *lo, const double *hi, uint64_t seed,
+                                    const fstat_pso_options *opts, void *stream)
+{
+    return pso_create_common(out, plan, n_swarms, n_particles, n_iter_total, lo, hi, n_swarms, seed, opts, stream);
 }
 
 fstat_status fstat_pso_iterate(fstat_pso *ps, int32_t n_iter, void *stream)
@@ -295,7 +332,7 @@ fstat_status fstat_pso_iterate(fstat_pso *ps, int32_t n_iter, void *stream)
         const double frac = (double)(it - 1) / (double)den;
         const double w = ps->opt.w_start + (ps->opt.w_end - ps->opt.w_start) * (frac < 1.0 ? frac : 1.0);
         pso_step_kernel<<<nb, nt, 0, st>>>(ps->n, ps->n_particles, it, ps->seed, w, ps->opt.c1, ps->opt.c2,
-                                           ps->opt.v_max, ps->box, ps->d_x, ps->d_v, ps->d_pbest, ps->d_pbest_f,
+                                           ps->opt.v_max, ps->d_boxes, ps->d_x, ps->d_v, ps->d_pbest, ps->d_pbest_f,
                                            ps->d_params);
         if (cudaGetLastError() != cudaSuccess) { ps->err = "pso_step_kernel launch failed"; rc = FSTAT_ECUDA; break; }
         rc = pso_fitness(ps, st);
@@ -316,7 +353,7 @@ fstat_status fstat_pso_best(fstat_pso *ps, double *best_params_host, double *bes
     cudaSetDevice(fstat_plan_device(ps->plan));
     cudaStream_t st = (cudaStream_t)stream;
     fstat_status rc = FSTAT_OK;
-    pso_swarm_best_kernel<<<ps->n_swarms, 128, 0, st>>>(ps->n_particles, ps->box, ps->d_pbest, ps->d_pbest_f,
+    pso_swarm_best_kernel<<<ps->n_swarms, 128, 0, st>>>(ps->n_particles, ps->d_boxes, ps->d_pbest, ps->d_pbest_f,
                                                         ps->d_best_params, ps->d_best_f);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(best_params_host, ps->d_best_params, (size_t)ps->n_swarms * kDim * sizeof(double), cudaMemcpyDeviceToHost, st);

@@ -104,6 +104,10 @@ def test_null_plan_calls_are_safe(fs):
     assert lib.fstat_plan_device(None) == -1
     assert lib.fstat_eval_batch(None, 1, None, None, None, None) == 1
     assert lib.fstat_plan_launch_count(None) == 0
+    assert lib.fstat_plan_table_bytes(None) == 0
+    assert lib.fstat_plan_band_stats(None, None) == 1
+    assert lib.fstat_extrinsic_from_amplitudes(None, 0.0, None) == 1
+    assert lib.fstat_amplitudes_from_extrinsic(1.0, 0.0, 0.0, 0.0, None) == 1
     # the rows built on top of the path (f2, f2 x f3, f4) answer FSTAT_EINVAL too
     assert lib.fstat_eval_batch_bands(None, 1, None, 4, 1, None, None, None, None) == 1
     assert lib.fstat_eval_batch_bands_host(None, 1, None, 4, 1, None, None, None, None) == 1

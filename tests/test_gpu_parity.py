@@ -198,6 +198,29 @@ def test_host_buffer_call_and_device_resident_inputs_agree(fs, torch_, orc, tiny
         np.testing.assert_array_equal(Fk2.cpu().numpy(), Fk_d)
 
 
+def test_changing_batch_sizes_reuse_cached_segment_tables_bit_for_bit(fs, torch_):
+    """The segment tables are cached per work-segment length: evaluating batches of different sizes in turn on one plan
+    (a ragged last batch, shrinking swarms) gives the bits of a fresh plan every time, before and after
+    fstat_plan_set_partitions, and the plan's table footprint has no 192-byte-per-bin table in it."""
+    cfg = syn.Config(21, "cache_slice", 2.5 * syn.YEAR_S, 0.0200, 0.0206, (8,), (700,), 3.5 * syn.YEAR_S, "wide")
+    ds = syn.make_dataset(cfg, None)
+    par = syn.draw_particles(cfg)
+    sizes = [700, 128, 513, 700, 1, 128]
+    ref = {}
+    for P in set(sizes):
+        ref[P] = _gpu_eval(fs, torch_, ds, ds.edges(8), par[:P])
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(8)) as plan:
+        assert fs.fstat_plan_table_bytes(plan) < 100 * ds.n_bins          # 32 + 24 + ~20 bytes per bin, not 268
+        for rnd in range(2):
+            for P in sizes:
+                F, Fk = fs.fstat_eval_batch(plan, torch_.as_tensor(np.ascontiguousarray(par[:P]), device="cuda"))
+                torch_.cuda.synchronize()
+                assert np.array_equal(F.cpu().numpy(), ref[P][0]) and np.array_equal(Fk.cpu().numpy(), ref[P][1]), (rnd, P)
+            fs.fstat_plan_set_partitions(plan, ds.edges(3))
+            fs.fstat_eval_batch(plan, torch_.as_tensor(np.ascontiguousarray(par[:64]), device="cuda"))
+            fs.fstat_plan_set_partitions(plan, ds.edges(8))
+
+
 def test_plan_create_rejects_bad_data_on_the_device(fs, torch_, tiny):
     ds = tiny
     e = ds.edges(4)

@@ -115,6 +115,41 @@ def test_device_swarms_follow_the_oracle_step_by_step(gpu, orc):
 
 
 @pytest.mark.gpu
+def test_one_box_per_swarm(gpu, orc):
+    """fstat_pso_create_boxes: three swarms, three different boxes (the hierarchy's stages search one box per t_c
+    interval / candidate).  The unit-box state is the oracle's (which never sees the boxes), the
+    physical parameters follow each swarm's own box bit for bit, and every best lies inside its swarm's box."""
+    fs = gpu
+    cfg = syn.CONFIGS[0]
+    ds = syn.make_dataset(cfg, orc.template)
+    inj = ds.inj_params
+    n_swarms, n_part, n_iter, seed = 3, 16, 4, 99
+    lo = np.array([[inj[0] - 3000.0 * (s + 1), inj[1] * (0.998 - 0.001 * s), 0.2, inj[3] - 0.1, inj[4] - 0.1, 0.0] for s in range(3)])
+    hi = np.array([[inj[0] + 3000.0 * (s + 1), inj[1] * (1.002 + 0.001 * s), 0.25, inj[3] + 0.1, inj[4] + 0.1, 0.1] for s in range(3)])
+    edges = ds.edges(4)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges) as plan:
+        with fs.fstat_pso_create(plan, n_swarms, n_part, n_iter, lo, hi, seed) as pso:
+            x_o, v_o = po.init(n_swarms, n_part, seed)
+            par_o = np.concatenate([po.to_params(x_o[s * n_part:(s + 1) * n_part], lo[s], hi[s]) for s in range(3)])
+            F_o, _ = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par_o)
+            x, v, pb, pbf, fl = fs.fstat_pso_state(pso)
+            np.testing.assert_array_equal(x, x_o)
+            fin = np.isfinite(F_o)
+            np.testing.assert_allclose(fl[fin], F_o[fin], rtol=1e-5)
+            fs.fstat_pso_iterate(pso, n_iter)
+            bp, bf = fs.fstat_pso_best(pso)
+            x, v, pb, pbf, fl = fs.fstat_pso_state(pso)
+            for s in range(3):
+                assert np.all((bp[s] >= lo[s]) & (bp[s] <= hi[s]))
+                sl = slice(s * n_part, (s + 1) * n_part)
+                j = int(np.argmax(pbf[sl]))
+                np.testing.assert_array_equal(bp[s], lo[s] + pb[sl][j] * (hi[s] - lo[s]))
+                assert bf[s] == pbf[sl][j]
+        with pytest.raises(fs.FstatError):
+            fs.fstat_pso_create(plan, 3, 16, 4, hi, lo)
+
+
+@pytest.mark.gpu
 def test_many_iterations_without_host_sync_improve_every_swarm(gpu, orc):
     fs = gpu
     import torch
