@@ -595,20 +595,34 @@ def run_ours(args):
                                          interp_tol=args.interp_tol, tdi_channel=fs.TDI_CHANNELS[name])
             ds_c = syn.make_dataset(dataclasses.replace(cfg, noise_seed=cfg.noise_seed + 1 + c), None, channel=name)
             plans.append(fs.fstat_plan_create(ds_c.freq, ds_c.dw, ds_c.inv_sn, edges, o))
-        for _ in range(2):
-            fs.fstat_eval_batch_channels(plans, par, stream)
-        torch.cuda.synchronize()
+        # the same set once more with options.no_channel_fusion on plans[0]: one pass per channel instead of the fused pass
+        o = fs.fstat_default_options(force_level=args.force_level, max_segment_bins=args.max_segment_bins,
+                                     interp_tol=args.interp_tol, tdi_channel=fs.TDI_CHANNELS[names[0]], no_channel_fusion=1)
+        ds_c = syn.make_dataset(dataclasses.replace(cfg, noise_seed=cfg.noise_seed + 1), None, channel=names[0])
+        plans.append(fs.fstat_plan_create(ds_c.freq, ds_c.dw, ds_c.inv_sn, edges, o))
+        del ds_c
         n_c = max(min(args.steps, 10), 1)
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_c)]
-        for e0, e1 in evs:
-            scratch.fill_(4)
-            e0.record(stream)
-            fs.fstat_eval_batch_channels(plans, par, stream)
-            e1.record(stream)
-        torch.cuda.synchronize()
-        ms_c = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs]))
-        out["channels"] = {"channels": list(names), "ms_per_step": ms_c, "ms_per_step_one_channel_X": ms_step,
-                           "channel_template_bins_per_s": float(P) * ds.n_bins * len(plans) * world / (ms_c * 1e-3),
+
+        def time_set(pset):
+            for _ in range(2):
+                fs.fstat_eval_batch_channels(pset, par, stream)
+            torch.cuda.synchronize()
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_c)]
+            for e0, e1 in evs:
+                scratch.fill_(4)
+                e0.record(stream)
+                fs.fstat_eval_batch_channels(pset, par, stream)
+                e1.record(stream)
+            torch.cuda.synchronize()
+            return float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs]))
+
+        n_ch = len(names)
+        ms_c = time_set(plans[:n_ch])
+        ms_sep = time_set([plans[n_ch]] + plans[1:n_ch])
+        out["channels"] = {"channels": list(names), "ms_per_step": ms_c, "ms_per_step_one_pass_per_channel": ms_sep,
+                           "ms_per_step_one_channel_X": ms_step,
+                           "channel_template_bins_per_s": float(P) * ds.n_bins * n_ch * world / (ms_c * 1e-3),
+                           "kernel": "fstat_fastmulti_kernel (one pass: node model and carrier shared by the channels)",
                            "data": "seeded noise with each channel's own PSD; timing does not depend on the data"}
         for pl in plans:
             fs.fstat_plan_destroy(pl)

@@ -77,6 +77,9 @@ typedef struct {
                                * 1.5e-7 rad and TDI response 2e-7 relative            */
     int32_t tdi_channel;      /* fstat_tdi_channel: the TDI combination this plan's data and templates are in;     *
                                * default FSTAT_TDI_X, the paper's                                     */
+    int32_t no_channel_fusion;/* 0 (default): fstat_eval_batch_channels evaluates two or three plans of the A / E / T  *
+                               * family in ONE pass of the interpolating kernel (shared node model and carrier);   *
+                               * 1 (read from plans[0]): one pass per channel, as for any other set (tests / tuning)*/
 } fstat_options;
 
 FSTAT_API void fstat_default_options(fstat_options *opts);
@@ -189,8 +192,12 @@ FSTAT_API fstat_status fstat_eval_batch_bands_host(fstat_plan *plan, int64_t P, 
  * independent noise between the channels: that holds for {A, E, T} and NOT for {X, Y, Z}, whose noises
  * are correlated -- the call adds whatever set it is given (the sum over X, Y, Z is then not a likelihood ratio; it
  * is accepted because the paper leaves the choice of combinations open, and tests use it).  All plans must share the
- * device, the grid, the partition edges and the other options.  The a1-a5 kernels run once per channel; one epilogue
- * adds the channels' sums and solves.
+ * device, the grid, the partition edges and the other options.  Two or three plans of the A / E / T family (any
+ * order, same orbit and tolerances) go through ONE pass of a fused interpolating kernel: the node model (phase, t_f,
+ * orbit, the three arms, X', Y', Z') and the per-bin carrier are evaluated once per template and shared, each channel
+ * keeps its own data stream, Gram tables and eight sums (csrc/fstat_fastmulti.cu; 9 + 10 n FP64 instructions per bin
+ * against 19 n).  Any other set (X, Y, Z plans, four channels, options.no_channel_fusion) runs the a1-a5 kernels once
+ * per channel.  One epilogue adds the channels' sums and solves.
  *
  *   plans   HOST array of n_channels (1..4) plan handles, all different.
  *   params, F, Fk, cuda_stream as in fstat_eval_batch (Fk is [P][N_p]).

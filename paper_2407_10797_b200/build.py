@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libfstat_b200.so")
-SOURCES = ("fstat_api.cu", "fstat_kernels.cu", "fstat_fast.cu", "fstat_fastband.cu", "fstat_pso.cu", "fstat_band.cu")
+SOURCES = ("fstat_api.cu", "fstat_kernels.cu", "fstat_fast.cu", "fstat_fastmulti.cu", "fstat_fastband.cu", "fstat_pso.cu", "fstat_band.cu")
 HEADERS = ("fstat_internal.h", "fstat_device.cuh", "fstat_model.cuh", "fstat_direct.cuh", "fstat_fast.cuh")
 
 

@@ -451,6 +451,7 @@ static fstat_status plan_create_impl(fstat_plan *pl, int64_t n_bins, const doubl
         return fail(pl, FSTAT_ECUDA, "device is not sm_100-class (this library ships sm_100a code only)");
     CU_TRY(pl, main_kernel_configure());
     CU_TRY(pl, fast_kernel_configure());
+    CU_TRY(pl, fastmulti_kernel_configure());
     CU_TRY(pl, band_kernel_configure());
     CU_TRY(pl, fastband_kernel_configure());
 
@@ -687,8 +688,11 @@ int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out
 }
 
 // a1-a5 for P particles, then a6 (F, F_k) when F != NULL and / or the extrinsic amplitudes when amp != NULL
+// fused != NULL (row f4): pl = fused[0]; the n_fused plans (A / E / T family, same grid, partitions and schedule) are
+// evaluated by one pass of the multi-channel interpolating kernel, each into its own partial sums.
 static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, double *amp,
-                              void *stream, bool sums_only = false)
+                              void *stream, bool sums_only = false, fstat_plan *const *fused = nullptr,
+                              int32_t n_fused = 0)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
@@ -763,6 +767,57 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     a.aet = fa.aet;
     a.orb = pl->orb;
     const int slot = (int)(pl->n_timed % fstat_plan::kRing);
+    if (n_fused > 1) {
+        FastMultiArgs fm;
+        memset(&fm, 0, sizeof(fm));
+        for (int32_t c = 0; c < n_fused; ++c) {
+            fstat_plan *pc = fused[c];
+            if (c) {
+                fstat_status sc = ensure_segments(pc, (int32_t)n_groups);
+                if (sc != FSTAT_OK) { pl->err = pc->err; return sc; }
+                if (pc->n_seg != pl->n_seg || pc->seg_len != pl->seg_len)
+                    return fail(pl, FSTAT_ECUDA, "internal: the channels' segmentations differ");
+                CU_TRY(pl, grow(&pc->d_partial, &pc->partial_cap, (size_t)pl->n_seg * kNPartial * (size_t)P_pad));
+                pc->last_groups = (int32_t)n_groups;
+                pc->last_was_band = false;
+            }
+            fm.dwp[c] = pc->d_dwp;
+            for (int l = 0; l < kNLevels; ++l) fm.gram[c][l] = pc->d_gram[l];
+            fm.partial[c] = pc->d_partial;
+            for (int i = 0; i < 3; ++i) fm.wch[c][i] = pc->orb.wch[i];
+        }
+        fm.node = pl->d_node;
+        fm.coef = pl->d_coef;
+        fm.seg_edge = pl->d_seg_edge;
+        fm.seg_gbase = pl->d_seg_gbase;
+        fm.level = pl->d_level;
+        fm.part_sk = fa.part_sk;
+        fm.part_sp = fa.part_sp;
+        fm.P_pad = P_pad;
+        fm.n_groups = (int32_t)n_groups;
+        fm.n_seg = pl->n_seg;
+        fm.segs_per_cta = fa.segs_per_cta;
+        fm.n_ch = n_fused;
+        fm.df = pl->df;
+        fm.orb = pl->orb;
+        CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
+        CU_TRY(pl, launch_fastmulti(fm, st));
+        for (int32_t c = 0; c < n_fused; ++c) {          // work items left to the direct kernel: one pass per channel
+            fstat_plan *pc = fused[c];
+            MainArgs ac = a;
+            ac.dwp = pc->d_dwp;
+            ac.fw = pc->d_fw;
+            ac.partial = pc->d_partial;
+            ac.orb = pc->orb;
+            CU_TRY(pl, launch_main(ac, st));
+        }
+        CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
+        ++pl->n_timed;
+        // keys, rank, prologue, stride selection, fused interpolating kernel, direct kernel per channel
+        pl->n_launches += 5 + n_fused;
+        pl->last_was_band = false;
+        return FSTAT_OK;
+    }
     CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
     if (pl->fast_ok) CU_TRY(pl, launch_fast(fa, st));
     CU_TRY(pl, launch_main(a, st));
@@ -815,7 +870,20 @@ fstat_status fstat_eval_batch_channels(fstat_plan *const *plans, int32_t n_chann
     }
     PartialSet ps{};
     ps.n = n_channels;
-    for (int32_t c = 0; c < n_channels; ++c) {
+    // two or three channels of the A / E / T family with one orbit and one set of tolerances: one fused pass
+    bool fuse = (n_channels == 2 || n_channels == 3) && !p0->opt.no_channel_fusion;
+    for (int32_t c = 0; fuse && c < n_channels; ++c) {
+        const fstat_plan *pc = plans[c];
+        fuse = pc->fast_ok && pc->opt.tdi_channel >= FSTAT_TDI_A && pc->opt.tdi_channel <= FSTAT_TDI_T &&
+               memcmp(pc->orb.c, p0->orb.c, sizeof(p0->orb.c)) == 0 && pc->opt.interp_tol == p0->opt.interp_tol &&
+               pc->opt.force_level == p0->opt.force_level;
+    }
+    if (fuse) {
+        fstat_status s = eval_impl(p0, P, params, nullptr, nullptr, nullptr, stream, true, plans, n_channels);
+        if (s != FSTAT_OK) return s;
+        for (int32_t c = 0; c < n_channels; ++c) ps.p[c] = plans[c]->d_partial;
+    }
+    for (int32_t c = 0; !fuse && c < n_channels; ++c) {
         fstat_status s = eval_impl(plans[c], P, params, nullptr, nullptr, nullptr, stream, true);
         if (s != FSTAT_OK) { if (c) p0->err = plans[c]->err; return s; }
         if (plans[c]->n_seg != p0->n_seg) return fail(p0, FSTAT_ECUDA, "internal: the channels' segmentations differ");

@@ -127,6 +127,29 @@ struct FastArgs {
     OrbitCoef orb;
 };
 
+// row f4: the interpolating kernel for 2 or 3 channels of the A / E / T family in one pass (fstat_fastmulti.cu); the
+// channels' plans share grid, partitions, segment tables and schedule, each has its own data, Gram tables and sums
+constexpr int kMaxFused = 3;
+struct FastMultiArgs {
+    const double *dwp[kMaxFused];
+    const double *gram[kMaxFused][kNLevels];
+    double *partial[kMaxFused];
+    double wch[kMaxFused][3];     // weights of the Michelson X', Y', Z' responses
+    const double *node;
+    const double *coef;
+    const int32_t *seg_edge;
+    const int32_t *seg_gbase;
+    const int8_t *level;
+    int64_t part_sk, part_sp;
+    int64_t P_pad;
+    int32_t n_groups;
+    int32_t n_seg;
+    int32_t segs_per_cta;
+    int32_t n_ch;
+    double df;
+    OrbitCoef orb;                // of the unrelabelled constellation (wch unused)
+};
+
 // row f2: edge j of a template's band, e_j = min(C (q_lo + floor(j D / N)), n_bins)   (reading A26)
 __host__ __device__ __forceinline__ int32_t band_edge(int32_t j, int32_t q_lo, int32_t D, int32_t N, int32_t C,
                                                       int32_t n_bins)
@@ -229,6 +252,8 @@ cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_
                             int32_t *direct_list, int32_t *direct_count, cudaStream_t st);
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
+cudaError_t launch_fastmulti(const FastMultiArgs &a, cudaStream_t st);
+cudaError_t fastmulti_kernel_configure();
 // rank_band: nullptr (slots ranked by chirp mass) or HOST {T_obs, f_first, f_last} (row f2: ranked by band)
 // scratch: prologue_scratch_bytes(P) bytes of device memory (keys and, for large batches, the radix sort's buffers)
 cudaError_t launch_prologue(const double *params, int64_t P, int64_t P_pad, double f_ref_e0, double kappa,

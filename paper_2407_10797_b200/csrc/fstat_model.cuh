@@ -80,18 +80,15 @@ __device__ __forceinline__ void arm_response_both(double xq, double c2x, double 
     di = fma(ca, sb, -sa * cb);
 }
 
-// a2 + a3 at one frequency.  `row` is a table row (layout TabCol), c[] the particle's coefficients.
-// Returns, in quarter turns, psi_nl = Psi_0 - 2 pi f t_c + Doppler phase of spacecraft 1 (reading A4)
-// -- the carrier phase without its linear term c[0] f -- and T'_+, T'_x with T_P = K_f T'_P,
-// K_f = -i (1 - z^2) folded into the data tables.
-// AET = false: first-generation Michelson X (Y, Z through the orbit coefficients of the relabelled constellation).
-// AET = true (PAPER.md:48, reading A28): T' = w_X X' + w_Y Y' + w_Z Z' with the weights orb.wch of A = (Z - X)/sqrt 2,
-// E = (X - 2Y + Z)/sqrt 6 or T = (X + Y + Z)/sqrt 3; the three Michelson responses share the phase, t_f, the orbit and
-// the three arms (each arm evaluated once, seen from both ends), all relative to the Doppler phase of spacecraft 1.
-template <bool AET = false>
-__device__ __forceinline__ void model_eval(const double2 *__restrict__ row, const double (&c)[kNCoef],
-                                           const OrbitCoef &orb, double &psi_nl, double &tpr, double &tpi,
-                                           double &tcr, double &tci)
+// a2 and the geometry half of a3 at one frequency: SPA phase (quarter turns) without its linear term, plus the Doppler
+// phase of spacecraft 1 (reading A4); k.n, u.n, v.n of the arms 1->2 and 1->3 at t_f.  `row` is a table row (layout
+// TabCol), c[] the particle's coefficients.
+struct NodeGeom {
+    double psi_nl, xq, c2x, s2x;
+    double mu2, mu3, un2, un3, vn2, vn3;
+};
+__device__ __forceinline__ void node_geometry(const double2 *__restrict__ row, const double (&c)[kNCoef],
+                                              const OrbitCoef &orb, NodeGeom &g)
 {
     const double kx = c[11], ky = c[12], kz = c[13];
     const double ux = c[14], uy = c[15], uz = c[16];
@@ -110,7 +107,9 @@ __device__ __forceinline__ void model_eval(const double2 *__restrict__ row, cons
     psi = fma(c[7], r3.x, psi);
     psi = fma(c[8], r3.y, psi);
     psi = fma(c[9], r4.x, psi);
-    const double xq = r4.y;
+    g.xq = r4.y;
+    g.c2x = zz.x;
+    g.s2x = zz.y;
     double alq = fma(c[2], d0.x, c[10]);
     alq = fma(c[3], d0.y, alq);
     alq = fma(c[4], d1.x, alq);
@@ -135,60 +134,87 @@ __device__ __forceinline__ void model_eval(const double2 *__restrict__ row, cons
     const double n3y = orb7(orb.c[2][1], c1, s1, c2, s2, c3, s3);
     const double n3z = orb5(orb.c[2][2], c1, s1, c2, s2);
     const double kp = fma(kx, p1x, fma(ky, p1y, kz * p1z));        // 4 k.p_1/c
-    const double mu2 = fma(kx, n2x, fma(ky, n2y, kz * n2z));
-    const double mu3 = fma(kx, n3x, fma(ky, n3y, kz * n3z));
-    const double un2 = fma(ux, n2x, fma(uy, n2y, uz * n2z));
-    const double un3 = fma(ux, n3x, fma(uy, n3y, uz * n3z));
-    const double vn2 = fma(vx, n2x, fma(vy, n2y, vz * n2z));
-    const double vn3 = fma(vx, n3x, fma(vy, n3y, vz * n3z));
+    g.mu2 = fma(kx, n2x, fma(ky, n2y, kz * n2z));
+    g.mu3 = fma(kx, n3x, fma(ky, n3y, kz * n3z));
+    g.un2 = fma(ux, n2x, fma(uy, n2y, uz * n2z));
+    g.un3 = fma(ux, n3x, fma(uy, n3y, uz * n3z));
+    g.vn2 = fma(vx, n2x, fma(vy, n2y, vz * n2z));
+    g.vn3 = fma(vx, n3x, fma(vy, n3y, vz * n3z));
+    g.psi_nl = fma(f, kp, psi);                                     // + Doppler phase of spacecraft 1
+}
 
-    psi_nl = fma(f, kp, psi);                                       // + Doppler phase of spacecraft 1
+// The three first-generation Michelson responses X', Y', Z' of one node, both polarisations, all relative to the
+// Doppler phase of spacecraft 1: three arms 1->2, 1->3, 2->3 (n_23 = n_13 - n_12), each evaluated once and seen from
+// both ends.  xyz[pol][0..5] = (X re, X im, Y re, Y im, Z re, Z im), pol 0 = +, 1 = x.
+//   X = xi_13 g(mu_13) - xi_12 g(mu_12);  Y = [xi_12 g(-mu_12) - xi_23 g(mu_23)] exp(-2 i x mu_12);
+//   Z = [xi_23 g(-mu_23) - xi_13 g(-mu_13)] exp(-2 i x mu_13)          (cyclic relabelling of reading A7)
+__device__ __forceinline__ void michelson_xyz(const NodeGeom &g, double (&xyz)[2][6])
+{
+    const double mu23 = g.mu3 - g.mu2, un23 = g.un3 - g.un2, vn23 = g.vn3 - g.vn2;
+    const double P2 = arm_nonzero(1.0 + g.mu2), Q2 = arm_nonzero(1.0 - g.mu2);
+    const double P3 = arm_nonzero(1.0 + g.mu3), Q3 = arm_nonzero(1.0 - g.mu3);
+    const double P4 = arm_nonzero(1.0 + mu23), Q4 = arm_nonzero(1.0 - mu23);
+    const double den2 = P2 * Q2, den3 = P3 * Q3, den4 = P4 * Q4;
+    const double R = rcp_fast(den2 * den3 * den4);
+    double f2r, f2i, b2r, b2i, d2r, d2i, f3r, f3i, b3r, b3i, d3r, d3i, f4r, f4i, b4r, b4i, d4r, d4i;
+    arm_response_both(g.xq, g.c2x, g.s2x, P2, Q2, den3 * den4 * R, f2r, f2i, b2r, b2i, d2r, d2i);
+    arm_response_both(g.xq, g.c2x, g.s2x, P3, Q3, den2 * den4 * R, f3r, f3i, b3r, b3i, d3r, d3i);
+    arm_response_both(g.xq, g.c2x, g.s2x, P4, Q4, den2 * den3 * R, f4r, f4i, b4r, b4i, d4r, d4i);
+    const double xp2 = fma(g.un2, g.un2, -g.vn2 * g.vn2), xc2 = 2.0 * g.un2 * g.vn2;
+    const double xp3 = fma(g.un3, g.un3, -g.vn3 * g.vn3), xc3 = 2.0 * g.un3 * g.vn3;
+    const double xp4 = fma(un23, un23, -vn23 * vn23), xc4 = 2.0 * un23 * vn23;
+#pragma unroll
+    for (int pol = 0; pol < 2; ++pol) {
+        const double x2 = pol ? xc2 : xp2, x3 = pol ? xc3 : xp3, x4 = pol ? xc4 : xp4;
+        xyz[pol][0] = fma(x3, f3r, -x2 * f2r);
+        xyz[pol][1] = fma(x3, f3i, -x2 * f2i);
+        const double yr = fma(x2, b2r, -x4 * f4r), yi = fma(x2, b2i, -x4 * f4i);
+        const double zr = fma(x4, b4r, -x3 * b3r), zi = fma(x4, b4i, -x3 * b3i);
+        xyz[pol][2] = fma(yr, d2r, -yi * d2i);
+        xyz[pol][3] = fma(yr, d2i, yi * d2r);
+        xyz[pol][4] = fma(zr, d3r, -zi * d3i);
+        xyz[pol][5] = fma(zr, d3i, zi * d3r);
+    }
+}
 
+// a2 + a3 at one frequency.  Returns, in quarter turns, psi_nl (the carrier phase without its linear term c[0] f) and
+// T'_+, T'_x with T_P = K_f T'_P, K_f = -i (1 - z^2) folded into the data tables.
+// AET = false: first-generation Michelson X (Y, Z through the orbit coefficients of the relabelled constellation).
+// AET = true (PAPER.md:48, reading A28): T' = w_X X' + w_Y Y' + w_Z Z' with the weights orb.wch of A = (Z - X)/sqrt 2,
+// E = (X - 2Y + Z)/sqrt 6 or T = (X + Y + Z)/sqrt 3; the three Michelson responses share the phase, t_f, the orbit and
+// the three arms.
+template <bool AET = false>
+__device__ __forceinline__ void model_eval(const double2 *__restrict__ row, const double (&c)[kNCoef],
+                                           const OrbitCoef &orb, double &psi_nl, double &tpr, double &tpi,
+                                           double &tcr, double &tci)
+{
+    NodeGeom g;
+    node_geometry(row, c, orb, g);
+    psi_nl = g.psi_nl;
     if (!AET) {
         // two arms
-        const double P2 = arm_nonzero(1.0 + mu2), Q2 = arm_nonzero(1.0 - mu2);
-        const double P3 = arm_nonzero(1.0 + mu3), Q3 = arm_nonzero(1.0 - mu3);
+        const double P2 = arm_nonzero(1.0 + g.mu2), Q2 = arm_nonzero(1.0 - g.mu2);
+        const double P3 = arm_nonzero(1.0 + g.mu3), Q3 = arm_nonzero(1.0 - g.mu3);
         const double den2 = P2 * Q2, den3 = P3 * Q3;         // either sign (|mu| may exceed 1 by 0.0024), never 0
         const double R = rcp_fast(den2 * den3);
         double g2r, g2i, g3r, g3i;
-        arm_response(xq, zz.x, zz.y, P2, Q2, den3 * R, g2r, g2i);
-        arm_response(xq, zz.x, zz.y, P3, Q3, den2 * R, g3r, g3i);
-        const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;   // n.e_+.n, n.e_x.n
-        const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
+        arm_response(g.xq, g.c2x, g.s2x, P2, Q2, den3 * R, g2r, g2i);
+        arm_response(g.xq, g.c2x, g.s2x, P3, Q3, den2 * R, g3r, g3i);
+        const double xp2 = fma(g.un2, g.un2, -g.vn2 * g.vn2), xc2 = 2.0 * g.un2 * g.vn2;   // n.e_+.n, n.e_x.n
+        const double xp3 = fma(g.un3, g.un3, -g.vn3 * g.vn3), xc3 = 2.0 * g.un3 * g.vn3;
         // T'_P = xi_P3 g_3 - xi_P2 g_2   (TDI-X: arm 3 minus arm 2, reading A7)
         tpr = fma(xp3, g3r, -xp2 * g2r);
         tpi = fma(xp3, g3i, -xp2 * g2i);
         tcr = fma(xc3, g3r, -xc2 * g2r);
         tci = fma(xc3, g3i, -xc2 * g2i);
     } else {
-        // three arms 1->2, 1->3, 2->3 (n_23 = n_13 - n_12), each seen from both ends
-        const double mu23 = mu3 - mu2, un23 = un3 - un2, vn23 = vn3 - vn2;
-        const double P2 = arm_nonzero(1.0 + mu2), Q2 = arm_nonzero(1.0 - mu2);
-        const double P3 = arm_nonzero(1.0 + mu3), Q3 = arm_nonzero(1.0 - mu3);
-        const double P4 = arm_nonzero(1.0 + mu23), Q4 = arm_nonzero(1.0 - mu23);
-        const double den2 = P2 * Q2, den3 = P3 * Q3, den4 = P4 * Q4;
-        const double R = rcp_fast(den2 * den3 * den4);
-        double f2r, f2i, b2r, b2i, d2r, d2i, f3r, f3i, b3r, b3i, d3r, d3i, f4r, f4i, b4r, b4i, d4r, d4i;
-        arm_response_both(xq, zz.x, zz.y, P2, Q2, den3 * den4 * R, f2r, f2i, b2r, b2i, d2r, d2i);
-        arm_response_both(xq, zz.x, zz.y, P3, Q3, den2 * den4 * R, f3r, f3i, b3r, b3i, d3r, d3i);
-        arm_response_both(xq, zz.x, zz.y, P4, Q4, den2 * den3 * R, f4r, f4i, b4r, b4i, d4r, d4i);
-        const double xp2 = fma(un2, un2, -vn2 * vn2), xc2 = 2.0 * un2 * vn2;
-        const double xp3 = fma(un3, un3, -vn3 * vn3), xc3 = 2.0 * un3 * vn3;
-        const double xp4 = fma(un23, un23, -vn23 * vn23), xc4 = 2.0 * un23 * vn23;
+        double xyz[2][6];
+        michelson_xyz(g, xyz);
         const double wx = orb.wch[0], wy = orb.wch[1], wz = orb.wch[2];
-        // X = xi_13 g(mu_13) - xi_12 g(mu_12);  Y = [xi_12 g(-mu_12) - xi_23 g(mu_23)] exp(-2 i x mu_12);
-        // Z = [xi_23 g(-mu_23) - xi_13 g(-mu_13)] exp(-2 i x mu_13)          (cyclic relabelling of reading A7)
-#pragma unroll
-        for (int pol = 0; pol < 2; ++pol) {
-            const double x2 = pol ? xc2 : xp2, x3 = pol ? xc3 : xp3, x4 = pol ? xc4 : xp4;
-            const double Xr = fma(x3, f3r, -x2 * f2r), Xi = fma(x3, f3i, -x2 * f2i);
-            const double yr = fma(x2, b2r, -x4 * f4r), yi = fma(x2, b2i, -x4 * f4i);
-            const double zr = fma(x4, b4r, -x3 * b3r), zi = fma(x4, b4i, -x3 * b3i);
-            const double Yr = fma(yr, d2r, -yi * d2i), Yi = fma(yr, d2i, yi * d2r);
-            const double Zr = fma(zr, d3r, -zi * d3i), Zi = fma(zr, d3i, zi * d3r);
-            const double tr = fma(wx, Xr, fma(wy, Yr, wz * Zr)), ti = fma(wx, Xi, fma(wy, Yi, wz * Zi));
-            if (pol == 0) { tpr = tr; tpi = ti; } else { tcr = tr; tci = ti; }
-        }
+        tpr = fma(wx, xyz[0][0], fma(wy, xyz[0][2], wz * xyz[0][4]));
+        tpi = fma(wx, xyz[0][1], fma(wy, xyz[0][3], wz * xyz[0][5]));
+        tcr = fma(wx, xyz[1][0], fma(wy, xyz[1][2], wz * xyz[1][4]));
+        tci = fma(wx, xyz[1][1], fma(wy, xyz[1][3], wz * xyz[1][5]));
     }
 }
 

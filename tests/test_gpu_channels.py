@@ -174,6 +174,28 @@ def test_fine_slice_aet_through_the_interpolating_kernel(fs, orc):
     assert np.max(np.abs(Fk - Fk_d) / np.abs(Fk_d)) <= 5e-6
 
 
+@pytest.mark.parametrize("names", ["AET", "AE", "TA"])
+def test_fused_pass_equals_one_pass_per_channel(fs, orc, names):
+    """Two or three A / E / T plans go through one pass of the fused interpolating kernel (csrc/fstat_fastmulti.cu);
+    options.no_channel_fusion sends the same plans through one pass per channel.  The two share the node model, the
+    carrier recurrence and the order of every sum, so they agree to rounding; ragged partition edges cut node intervals
+    and the fused kernel's 256-bin tiles at arbitrary bins, and a wide-stride level is forced so that a 512-bin
+    interval spans two tiles."""
+    year = syn.YEAR_S
+    cfg = syn.Config(19, "aet_fused", 2.5 * year, 0.0200, 0.0203, (8,), (200,), 3.5 * year, "wide")
+    chans = _aet_channels(orc, cfg, names)
+    par = syn.draw_particles(cfg)
+    n = chans[0][0].freq.size
+    edges = np.array([0, 1001, 2750, 2763, 5000, 7777, 9013, n - 5, n], dtype=np.int64)
+    for kw in ({}, {"force_level": 6}, {"force_level": 0}):
+        F_f, Fk_f = _gpu_named(fs, chans, edges, par, **kw)
+        F_s, Fk_s = _gpu_named(fs, chans, edges, par, no_channel_fusion=1, **kw)
+        assert np.max(np.abs(Fk_f - Fk_s) / np.abs(Fk_s)) <= 1e-10, kw
+        assert np.max(np.abs(F_f - F_s) / np.abs(F_s)) <= 1e-10, kw
+    F, Fk = _gpu_named(fs, chans, edges, par)
+    _compare(orc, [(ds, o) for ds, o, _ in chans], edges, par, F, Fk)
+
+
 def test_first_stage_aet_sample(fs, orc):
     """Config 1 at full size (N_p = 1024, P = 2048) with A + E + T; a sample of particles against the oracle."""
     cfg = syn.CONFIGS[1]
