@@ -51,6 +51,8 @@ STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from the
 # ncu --set full capture named beside it (None when no capture of the current hot kernel exists)
 NCU_DRAM_BYTES_PER_LAUNCH = 224.5e6
+# the same capture: smsp__inst_executed.sum = 30.1 warp instructions per template-bin, 24.2 of them on the FP64 pipe
+NCU_OTHER_INST_PER_TEMPLATE_BIN = 30.1 - 24.2
 NCU_DRAM_CAPTURE = "profiles/r2.md (32.5 MB read + 191.9 MB written), ncu --set full of build 1ecb204 (hot kernel unchanged since)"
 # row f2 (fstat_fastband_kernel), per WARP-level unit of work counted by the kernel itself (fstat_plan_band_stats): the
 # per-bin and per-interval counts are those of fstat_fast_kernel; a node interval in which some lane has a partition edge
@@ -448,7 +450,13 @@ def run_ours(args):
     fp64_rate, n_sm = fs.fstat_probe_pipe_peak(0, 60.0, local)
     fp32_rate, _ = fs.fstat_probe_pipe_peak(1, 30.0, local)
     mufu_rate, _ = fs.fstat_probe_pipe_peak(2, 30.0, local)
+    mixed_rate, _ = fs.fstat_probe_pipe_peak(3, 30.0, local)
     achieved = fp64_inst / (main_mean * 1e-3)                 # FP64-pipe thread-instructions per second
+    # What the kernel's OTHER instructions cost it: an FP64 warp instruction occupies an SM sub-partition's FP64 pipe for
+    # two cycles, and the 4 : 1 probe shows how many more cycles an instruction of another pipe takes there (about 0.2 on
+    # B200: they issue in the gaps).  With n64 FP64 and n_other other instructions per template-bin the FP64 pipe can be
+    # busy at most 2 n64 / (2 n64 + cost n_other) of the time: the bound this instruction mix allows.
+    other_cost = 8.0 * (fp64_rate / mixed_rate - 1.0) if mixed_rate > 0 else None
     hbm_peak, hbm_src = peaks()
     n_groups = (P + 127) // 128
     # algorithmic HBM bytes of one launch: every particle group streams the folded data (16 B/bin) once, reads
@@ -479,11 +487,22 @@ def run_ours(args):
                                     "source": FP64_COUNTS_BUILD},
                 "stride_share_of_bins": stride_share,
                 "main_kernel_ms": main_mean, "main_kernel_share_of_step": main_mean / ms_step,
-                "measured_pipe_peaks_inst_per_s": {"fp64_fma": fp64_rate, "fp32_fma": fp32_rate, "mufu": mufu_rate},
+                "measured_pipe_peaks_inst_per_s": {"fp64_fma": fp64_rate, "fp32_fma": fp32_rate, "mufu": mufu_rate,
+                                                   "fp64_fma_with_one_fp32_per_four": mixed_rate},
                 "hbm": {"algorithmic_bytes_per_launch": hbm_bytes,
                         "achieved_gbs": hbm_bytes / (main_mean * 1e-3) / 1e9,
                         "peak_gbs": hbm_peak, "peak_source": hbm_src}}
 
+    if default_wl and other_cost is not None and roofline["frac"]:
+        n64 = roofline["fp64_inst_per_template_bin"]
+        bound = 2.0 * n64 / (2.0 * n64 + other_cost * NCU_OTHER_INST_PER_TEMPLATE_BIN)
+        roofline["dispatch"] = {"other_inst_cost_cycles": other_cost,
+                                "other_inst_per_template_bin": NCU_OTHER_INST_PER_TEMPLATE_BIN,
+                                "other_inst_source": NCU_DRAM_CAPTURE,
+                                "frac_bound_of_this_mix": bound, "frac_of_bound": roofline["frac"] / bound,
+                                "is": "an FP64 warp instruction occupies the pipe for 2 cycles, another instruction costs "
+                                      "other_inst_cost_cycles more (4 : 1 probe of this run): the share of time the FP64 pipe CAN be "
+                                      "busy with this kernel's instruction mix; the rest of the gap is dependency and barrier stalls"}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",

@@ -26,6 +26,7 @@ struct SegTables {
     SegCrit *d_seg_crit = nullptr;
     int8_t *d_seg_maxlvl = nullptr;
     std::vector<int32_t> seg_edge_h;
+    std::vector<int32_t> part_seg_h;
 };
 
 struct fstat_plan {
@@ -56,6 +57,7 @@ struct fstat_plan {
     int32_t *d_seg_edge = nullptr;     // [n_seg+1]
     int32_t *d_part_seg = nullptr;     // [n_part+1]
     std::vector<int32_t> seg_edge_h;   // host copy of d_seg_edge
+    std::vector<int32_t> part_seg_h;   // host copy of d_part_seg
     int32_t *d_seg_gbase = nullptr;    // [n_seg][kNLevels]
     SegCrit *d_seg_crit = nullptr;     // [n_seg]
     int8_t *d_seg_maxlvl = nullptr;    // [n_seg]
@@ -85,6 +87,12 @@ struct fstat_plan {
     // host-buffer path
     double *d_params = nullptr, *d_F = nullptr, *d_Fk = nullptr;
     size_t params_cap = 0, F_cap = 0, Fk_cap = 0;
+    // fstat_eval_batch_host: the interpolating kernel is launched as up to kPipe ranges of partitions on streams of
+    // its own, so that the epilogue and the device-to-host copy of one range's F_k run under the next ranges' kernels
+    static constexpr int kPipe = 8;
+    int32_t pipe_ranges = 1;
+    cudaStream_t pipe_main[kPipe] = {}, pipe_copy = nullptr;
+    cudaEvent_t pipe_fork = nullptr, pipe_main_done[kPipe] = {}, pipe_copy_done = nullptr;
     OrbitCoef orb{};
     // ring of event pairs around the main kernel of the most recent evaluations (bench roofline)
     static constexpr int kRing = 128;
@@ -262,6 +270,7 @@ void use_seg_tables(fstat_plan *pl, const SegTables &t, int32_t n_groups)
     pl->d_seg_edge = t.d_seg_edge; pl->d_part_seg = t.d_part_seg; pl->d_seg_gbase = t.d_seg_gbase;
     pl->d_seg_crit = t.d_seg_crit; pl->d_seg_maxlvl = t.d_seg_maxlvl;
     pl->seg_edge_h = t.seg_edge_h;
+    pl->part_seg_h = t.part_seg_h;
     pl->n_seg = t.n_seg;
     pl->seg_len = (int32_t)(t.seg_len < pl->n_bins ? t.seg_len : pl->n_bins);
     pl->seg_groups = n_groups;
@@ -317,6 +326,7 @@ fstat_status ensure_segments(fstat_plan *pl, int32_t n_groups)
     if (e == cudaSuccess) e = cudaMemcpy(t.d_seg_maxlvl, maxlvl.data(), maxlvl.size() * sizeof(int8_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { free_seg_tables(t); CU_TRY(pl, e); }
     t.seg_edge_h = seg_edge;
+    t.part_seg_h = part_seg;
     pl->seg_cache.push_back(t);
     use_seg_tables(pl, pl->seg_cache.back(), n_groups);
     return FSTAT_OK;
@@ -535,6 +545,13 @@ static void plan_free(fstat_plan *pl)
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
     }
+    for (int i = 0; i < fstat_plan::kPipe; ++i) {
+        if (pl->pipe_main[i]) cudaStreamDestroy(pl->pipe_main[i]);
+        if (pl->pipe_main_done[i]) cudaEventDestroy(pl->pipe_main_done[i]);
+    }
+    if (pl->pipe_copy) cudaStreamDestroy(pl->pipe_copy);
+    if (pl->pipe_fork) cudaEventDestroy(pl->pipe_fork);
+    if (pl->pipe_copy_done) cudaEventDestroy(pl->pipe_copy_done);
     delete pl;
 }
 
@@ -688,11 +705,40 @@ int32_t fstat_plan_main_kernel_ms(fstat_plan *pl, int32_t n_last, double *ms_out
 }
 
 // a1-a5 for P particles, then a6 (F, F_k) when F != NULL and / or the extrinsic amplitudes when amp != NULL
+// Host buffers of fstat_eval_batch_host handed down to eval_impl: when the F_k block is large the evaluation is cut into
+// ranges of partitions and fk_copied is set (the caller then copies F only).
+struct HostOut {
+    double *Fk_host = nullptr;
+    bool fk_copied = false;
+};
+
+static fstat_status ensure_pipe(fstat_plan *pl)
+{
+    if (pl->pipe_copy_done) return FSTAT_OK;
+    // Priorities (numerically lower = served first): the copy stream highest -- an epilogue becomes ready while later
+    // ranges still have CTAs waiting and must not queue behind them -- then the ranges in order, so that concurrent
+    // ranges do not share the SMs evenly and finish together.
+    int prio_lo = 0, prio_hi = 0;
+    CU_TRY(pl, cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    for (int i = 0; i < fstat_plan::kPipe; ++i) {
+        const int pr = prio_hi + 1 + i < prio_lo ? prio_hi + 1 + i : prio_lo;
+        if (!pl->pipe_main[i]) CU_TRY(pl, cudaStreamCreateWithPriority(&pl->pipe_main[i], cudaStreamNonBlocking, pr));
+        if (!pl->pipe_main_done[i]) CU_TRY(pl, cudaEventCreateWithFlags(&pl->pipe_main_done[i], cudaEventDisableTiming));
+    }
+    if (!pl->pipe_copy) CU_TRY(pl, cudaStreamCreateWithPriority(&pl->pipe_copy, cudaStreamNonBlocking, prio_hi));
+    pl->pipe_ranges = prio_lo - prio_hi;
+    if (pl->pipe_ranges < 1) pl->pipe_ranges = 1;
+    if (pl->pipe_ranges > fstat_plan::kPipe) pl->pipe_ranges = fstat_plan::kPipe;
+    if (!pl->pipe_fork) CU_TRY(pl, cudaEventCreateWithFlags(&pl->pipe_fork, cudaEventDisableTiming));
+    CU_TRY(pl, cudaEventCreateWithFlags(&pl->pipe_copy_done, cudaEventDisableTiming));
+    return FSTAT_OK;
+}
+
 // fused != NULL (row f4): pl = fused[0]; the n_fused plans (A / E / T family, same grid, partitions and schedule) are
 // evaluated by one pass of the multi-channel interpolating kernel, each into its own partial sums.
 static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, double *amp,
                               void *stream, bool sums_only = false, fstat_plan *const *fused = nullptr,
-                              int32_t n_fused = 0)
+                              int32_t n_fused = 0, HostOut *host = nullptr)
 {
     if (!pl) return FSTAT_EINVAL;
     if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
@@ -746,6 +792,8 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     fa.n_seg = pl->n_seg;
     fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
     fa.aet = pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0;
+    fa.chunk_begin = 0;
+    fa.chunk_count = 0;
     fa.df = pl->df;
     fa.orb = pl->orb;
     MainArgs a;
@@ -817,6 +865,66 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         pl->n_launches += 5 + n_fused;
         pl->last_was_band = false;
         return FSTAT_OK;
+    }
+    {
+        // Host-buffer call with a large F_k block (N_p = 1024, P = 2048: 16.8 MB, 0.3 ms over PCIe against a 5.2 ms step):
+        // the interpolating kernel goes out as up to kPipe launches, each a range of partitions, on streams of its own
+        // (concurrent: a later range fills the SMs the earlier one's last CTAs leave free); a copy stream follows them
+        // range by range with that range's epilogue and the device-to-host copy of its F_k columns.  Only the last
+        // range's epilogue and copy remain after the kernels.
+        int32_t echunk = 0;
+        const int32_t n_echunk = epilogue_chunks(P, pl->n_part, &echunk);
+        const bool pipe = host && host->Fk_host && F && Fk && !amp && pl->fast_ok && n_echunk >= 2 &&
+                          (size_t)P * (size_t)pl->n_part * sizeof(double) >= ((size_t)2 << 20);
+        if (pipe) {
+            fstat_status sp = ensure_pipe(pl);
+            if (sp != FSTAT_OK) return sp;
+            // one range per stream priority below the copy stream's (5 on B200: 5.31 ms end to end against 5.23 ms on the
+            // device for config 1; ranges that share a priority share the SMs and finish together: 8 ranges 5.33 ms)
+            const int32_t K = n_echunk < pl->pipe_ranges ? n_echunk : pl->pipe_ranges;
+            const int32_t n_cta_chunks = (pl->n_seg + fa.segs_per_cta - 1) / fa.segs_per_cta;
+            PartialSet one{};
+            one.p[0] = pl->d_partial;
+            one.n = 1;
+            CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
+            CU_TRY(pl, launch_main(a, st));              // work items of the direct kernel: any partition, so first
+            CU_TRY(pl, cudaEventRecord(pl->pipe_fork, st));
+            int32_t cta_begin = 0;
+            for (int32_t r = 0; r < K; ++r) {
+                const int32_t c_lo = (int32_t)((int64_t)r * n_echunk / K), c_hi = (int32_t)((int64_t)(r + 1) * n_echunk / K);
+                const int32_t k_lo = c_lo * echunk;
+                const int32_t k_end = (int64_t)c_hi * echunk < pl->n_part ? c_hi * echunk : pl->n_part;
+                const int32_t s_end = pl->part_seg_h[k_end];
+                const int32_t cta_end = (r == K - 1) ? n_cta_chunks : (s_end + fa.segs_per_cta - 1) / fa.segs_per_cta;
+                cudaStream_t sm = pl->pipe_main[r];
+                CU_TRY(pl, cudaStreamWaitEvent(sm, pl->pipe_fork, 0));
+                if (cta_end > cta_begin) {
+                    fa.chunk_begin = cta_begin;
+                    fa.chunk_count = cta_end - cta_begin;
+                    CU_TRY(pl, launch_fast(fa, sm));
+                    pl->n_launches += 1;
+                    cta_begin = cta_end;
+                }
+                CU_TRY(pl, cudaEventRecord(pl->pipe_main_done[r], sm));
+                // the copy stream has already waited for the ranges before this one
+                CU_TRY(pl, cudaStreamWaitEvent(pl->pipe_copy, pl->pipe_main_done[r], 0));
+                CU_TRY(pl, launch_epilogue_range(one, pl->d_part_seg, pl->d_valid, pl->d_perm, P, P_pad, pl->n_part, pl->n_seg,
+                                                 c_lo, c_hi, pl->d_fpart, F, Fk, pl->pipe_copy));
+                CU_TRY(pl, cudaMemcpy2DAsync(host->Fk_host + k_lo, (size_t)pl->n_part * sizeof(double), Fk + k_lo,
+                                             (size_t)pl->n_part * sizeof(double), (size_t)(k_end - k_lo) * sizeof(double),
+                                             (size_t)P, cudaMemcpyDeviceToHost, pl->pipe_copy));
+                pl->n_launches += 1;
+            }
+            CU_TRY(pl, cudaEventRecord(pl->pipe_copy_done, pl->pipe_copy));
+            CU_TRY(pl, cudaStreamWaitEvent(st, pl->pipe_copy_done, 0));
+            CU_TRY(pl, cudaEventRecord(pl->ev1[slot], st));
+            ++pl->n_timed;
+            CU_TRY(pl, launch_fsum(pl->d_fpart, pl->d_valid, pl->d_perm, P, P_pad, n_echunk, F, st));
+            pl->n_launches += 5 + 1;                      // keys, rank, prologue, stride selection, direct; chunk sums of F
+            pl->last_was_band = false;
+            host->fk_copied = true;
+            return FSTAT_OK;
+        }
     }
     CU_TRY(pl, cudaEventRecord(pl->ev0[slot], st));
     if (pl->fast_ok) CU_TRY(pl, launch_fast(fa, st));
@@ -1134,10 +1242,12 @@ fstat_status fstat_eval_batch_host(fstat_plan *pl, int64_t P, const double *para
     CU_TRY(pl, grow(&pl->d_F, &pl->F_cap, (size_t)P));
     if (Fk_host) CU_TRY(pl, grow(&pl->d_Fk, &pl->Fk_cap, (size_t)P * (size_t)pl->n_part));
     CU_TRY(pl, cudaMemcpyAsync(pl->d_params, params_host, (size_t)P * 6 * sizeof(double), cudaMemcpyHostToDevice, st));
-    fstat_status s = fstat_eval_batch(pl, P, pl->d_params, pl->d_F, Fk_host ? pl->d_Fk : nullptr, stream);
+    HostOut ho;
+    ho.Fk_host = Fk_host;
+    fstat_status s = eval_impl(pl, P, pl->d_params, pl->d_F, Fk_host ? pl->d_Fk : nullptr, nullptr, stream, false, nullptr, 0, &ho);
     if (s != FSTAT_OK) return s;
     CU_TRY(pl, cudaMemcpyAsync(F_host, pl->d_F, (size_t)P * sizeof(double), cudaMemcpyDeviceToHost, st));
-    if (Fk_host)
+    if (Fk_host && !ho.fk_copied)
         CU_TRY(pl, cudaMemcpyAsync(Fk_host, pl->d_Fk, (size_t)P * (size_t)pl->n_part * sizeof(double),
                                    cudaMemcpyDeviceToHost, st));
     CU_TRY(pl, cudaStreamSynchronize(st));
@@ -1171,7 +1281,7 @@ fstat_status fstat_eval_template(fstat_plan *pl, const double *params_host, doub
 
 fstat_status fstat_probe_pipe_peak(int32_t device, int32_t which, double millis, double *inst_per_s, int32_t *n_sm_out)
 {
-    if (!inst_per_s || which < 0 || which > 2) return FSTAT_EINVAL;
+    if (!inst_per_s || which < 0 || which > 3) return FSTAT_EINVAL;
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); return FSTAT_ECUDA; }
     int dev = device;

@@ -254,7 +254,7 @@ __device__ __forceinline__ void fast_kernel_body(const FastArgs &a)
 
     const int tid = threadIdx.x;
     const int grp = blockIdx.x % a.n_groups;
-    const int chunk = blockIdx.x / a.n_groups;
+    const int chunk = blockIdx.x / a.n_groups + a.chunk_begin;
     const int seg_begin = chunk * a.segs_per_cta, seg_end = min(a.n_seg, seg_begin + a.segs_per_cta);
     const int8_t *level = a.level + (int64_t)grp * a.n_seg;
     const int64_t p = (int64_t)grp * kThreads + tid;         // < P_pad by construction
@@ -546,7 +546,7 @@ cudaError_t fast_kernel_configure()
 
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st)
 {
-    const int64_t n_chunks = (a.n_seg + a.segs_per_cta - 1) / a.segs_per_cta;
+    const int64_t n_chunks = a.chunk_count > 0 ? a.chunk_count : (a.n_seg + a.segs_per_cta - 1) / a.segs_per_cta;
     const int64_t n_cta = (int64_t)a.n_groups * n_chunks;
     if (a.aet) fstat_fast_aet_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);
     else fstat_fast_kernel<<<(unsigned)n_cta, kThreads, sizeof(FastSmem), st>>>(a);

@@ -123,6 +123,8 @@ struct FastArgs {
     int32_t n_seg;
     int32_t segs_per_cta;         // consecutive segments one CTA walks (tiles, node ring carried across their edges)
     int32_t aet;                  // 1: the A / E / T response (model_eval<true>)
+    int32_t chunk_begin;          // this launch walks the CTA chunks [chunk_begin, chunk_begin + chunk_count) ...
+    int32_t chunk_count;          // ... of segs_per_cta segments each; chunk_count = 0: all of them
     double df;
     OrbitCoef orb;
 };
@@ -270,6 +272,11 @@ struct PartialSet {
 cudaError_t launch_epilogue(const PartialSet &partials, const int32_t *part_seg, const int32_t *valid,
                             const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
                             double *Fpart, double *F, double *Fk, cudaStream_t st);
+cudaError_t launch_epilogue_range(const PartialSet &partials, const int32_t *part_seg, const int32_t *valid,
+                                  const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
+                                  int32_t chunk_lo, int32_t chunk_hi, double *Fpart, double *F, double *Fk, cudaStream_t st);
+cudaError_t launch_fsum(const double *Fpart, const int32_t *valid, const int32_t *perm, int64_t P, int64_t P_pad,
+                        int32_t n_chunk, double *F, cudaStream_t st);
 int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out);
 cudaError_t launch_amplitudes(const double *partial, const int32_t *part_seg, const int32_t *valid,
                               const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, double *amp,

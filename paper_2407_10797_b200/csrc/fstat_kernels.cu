@@ -446,8 +446,9 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const PartialSet
                                                                const int32_t *__restrict__ part_seg,
                                                                const int32_t *__restrict__ valid, int64_t P,
                                                                const int32_t *__restrict__ perm, int64_t P_pad,
-                                                               int32_t n_part, int32_t chunk,
-                                                               double *__restrict__ Fout, double *__restrict__ Fk)
+                                                               int32_t n_part, int32_t chunk, int32_t chunk0,
+                                                               int32_t n_chunk_total, double *__restrict__ Fout,
+                                                               double *__restrict__ Fk)
 {
     __shared__ int32_t sPerm[kEpiX];
     __shared__ double sF[kEpiY][kEpiX];
@@ -461,7 +462,8 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const PartialSet
     if (threadIdx.y == 0) sPerm[tx] = live ? perm[p] : -1;
     __syncthreads();
     const double ninf = -INFINITY;
-    const int k_lo = blockIdx.y * chunk, k_hi = min(n_part, k_lo + chunk);
+    const int cy = (int)blockIdx.y + chunk0;              // chunk of partitions (a launch may cover a range of them)
+    const int k_lo = cy * chunk, k_hi = min(n_part, k_lo + chunk);
     double fsum = 0.0;
     for (int k0 = k_lo; k0 < k_hi; k0 += kEpiY) {
         double fk = 0.0;
@@ -528,8 +530,8 @@ __global__ void __launch_bounds__(kEpiX *kEpiY) epilogue_kernel(const PartialSet
         double s = 0.0;
 #pragma unroll
         for (int y = 0; y < kEpiY; ++y) s += sF[y][tx];
-        if (gridDim.y == 1) Fout[sPerm[tx]] = ok ? s : ninf;                // F itself
-        else Fout[(int64_t)blockIdx.y * P_pad + p] = s;                      // chunk sum, see fsum_kernel
+        if (n_chunk_total == 1) Fout[sPerm[tx]] = ok ? s : ninf;            // F itself
+        else Fout[(int64_t)cy * P_pad + p] = s;                              // chunk sum, see fsum_kernel
     }
 }
 
@@ -602,23 +604,41 @@ int32_t epilogue_chunks(int64_t P, int32_t n_part, int32_t *chunk_out)
     return (n_part + chunk - 1) / chunk;
 }
 
+// chunks [chunk_lo, chunk_hi) of the partitions only, without the final sum over chunks (the host-buffer call overlaps
+// the copy of one range of F_k with the main kernels of the next, fstat_eval_batch_host)
+cudaError_t launch_epilogue_range(const PartialSet &partials, const int32_t *part_seg, const int32_t *valid,
+                                  const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
+                                  int32_t chunk_lo, int32_t chunk_hi, double *Fpart, double *F, double *Fk, cudaStream_t st)
+{
+    int32_t chunk = 0;
+    const int32_t n_chunk = epilogue_chunks(P, n_part, &chunk);
+    if (chunk_lo < 0 || chunk_hi > n_chunk || chunk_lo >= chunk_hi) return cudaErrorInvalidValue;
+    const dim3 blk(kEpiX, kEpiY);
+    const dim3 grd((unsigned)((P + kEpiX - 1) / kEpiX), (unsigned)(chunk_hi - chunk_lo));
+    double *out = (n_chunk == 1) ? F : Fpart;
+    if (n_seg >= 4 * n_part)
+        epilogue_kernel<true><<<grd, blk, 0, st>>>(partials, part_seg, valid, P, perm, P_pad, n_part, chunk, chunk_lo, n_chunk, out, Fk);
+    else
+        epilogue_kernel<false><<<grd, blk, 0, st>>>(partials, part_seg, valid, P, perm, P_pad, n_part, chunk, chunk_lo, n_chunk, out, Fk);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fsum(const double *Fpart, const int32_t *valid, const int32_t *perm, int64_t P, int64_t P_pad,
+                        int32_t n_chunk, double *F, cudaStream_t st)
+{
+    fsum_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(Fpart, valid, perm, P, P_pad, n_chunk, F);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_epilogue(const PartialSet &partials, const int32_t *part_seg, const int32_t *valid,
                             const int32_t *perm, int64_t P, int64_t P_pad, int32_t n_part, int32_t n_seg,
                             double *Fpart, double *F, double *Fk, cudaStream_t st)
 {
     int32_t chunk = 0;
     const int32_t n_chunk = epilogue_chunks(P, n_part, &chunk);
-    const dim3 blk(kEpiX, kEpiY);
-    const dim3 grd((unsigned)((P + kEpiX - 1) / kEpiX), (unsigned)n_chunk);
-    double *out = (n_chunk == 1) ? F : Fpart;
-    if (n_seg >= 4 * n_part)
-        epilogue_kernel<true><<<grd, blk, 0, st>>>(partials, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
-    else
-        epilogue_kernel<false><<<grd, blk, 0, st>>>(partials, part_seg, valid, P, perm, P_pad, n_part, chunk, out, Fk);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = launch_epilogue_range(partials, part_seg, valid, perm, P, P_pad, n_part, n_seg, 0, n_chunk, Fpart, F, Fk, st);
     if (e != cudaSuccess || n_chunk == 1) return e;
-    fsum_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(Fpart, valid, perm, P, P_pad, n_chunk, F);
-    return cudaGetLastError();
+    return launch_fsum(Fpart, valid, perm, P, P_pad, n_chunk, F, st);
 }
 
 // =================================================================================================
@@ -658,6 +678,32 @@ __global__ void __launch_bounds__(256) probe_kernel(int iters, double *sink)
 #pragma unroll
         for (int j = 0; j < 8; ++j) s += x[j];
         if (s == 123.456f) sink[0] = s;
+    } else if (WHICH == 3) {
+        // 8 FP64 FMA : 2 FP32 FMA per round -- what a non-FP64 instruction costs a stream that is bound by the FP64
+        // pipe (an FP64 warp instruction occupies the pipe for 2 cycles per SM sub-partition; measured on B200, the
+        // other instructions issue in the gaps and cost ~0.2 cycles each at this ratio: profiles/r2.md).  Counted
+        // as 64 FP64 instructions per iteration, like WHICH == 0.
+        double x[8];
+        float y[2];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = 1.0 + 1e-9 * (threadIdx.x + j);
+        y[0] = 1.0f + 1e-6f * threadIdx.x;
+        y[1] = 1.5f + 1e-6f * threadIdx.x;
+        const double m = 0.999999999, b = 1e-12;
+        const float mf = 0.9999999f, bf = 1e-9f;
+        for (int i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = fma(x[j], m, b);
+                y[0] = fmaf(y[0], mf, bf);
+                y[1] = fmaf(y[1], mf, bf);
+            }
+        }
+        double s = (double)(y[0] + y[1]);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += x[j];
+        if (s == 123.456) sink[0] = s;
     } else {
         float x[8];
 #pragma unroll
@@ -679,6 +725,7 @@ cudaError_t launch_probe(int which, int n_blocks, int iters, double *sink, cudaS
 {
     if (which == 0) probe_kernel<0><<<n_blocks, 256, 0, st>>>(iters, sink);
     else if (which == 1) probe_kernel<1><<<n_blocks, 256, 0, st>>>(iters, sink);
+    else if (which == 3) probe_kernel<3><<<n_blocks, 256, 0, st>>>(iters, sink);
     else probe_kernel<2><<<n_blocks, 256, 0, st>>>(iters, sink);
     return cudaGetLastError();
 }

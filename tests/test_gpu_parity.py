@@ -160,6 +160,45 @@ def test_invalid_particles_get_minus_infinity(fs, torch_, orc, tiny):
     assert _rel(Fk_g[good], Fk_o[good]).max() <= RTOL and _rel(F_g[good], F_o[good]).max() <= RTOL
 
 
+def test_host_buffer_call_with_a_large_Fk_block_is_cut_into_partition_ranges_bit_for_bit(fs, torch_, orc):
+    """fstat_eval_batch_host with P N_p 8 B >= 2 MiB launches the interpolating kernel as ranges of partitions on streams
+    of its own and copies every range's F_k columns while the next ranges compute.  Same kernels, same sums: F and F_k
+    equal the device-resident call's bit for bit -- with pageable and with pinned buffers, with a partition count that
+    does not divide into the ranges evenly, with partitions too short for the interpolating kernel (direct work items,
+    launched before the ranges), and twice in a row on the same plan (the range streams are reused)."""
+    year = syn.YEAR_S
+    cfg = syn.Config(21, "host_pipe", 2.5 * year, 0.0100, 0.0108, (600,), (512,), 3.5 * year, "wide")
+    ds = syn.make_dataset(cfg, orc.template)
+    par = syn.draw_particles(cfg)
+    rng = np.random.default_rng(5)
+    n = ds.freq.size
+    cuts = np.sort(rng.choice(np.arange(8, n - 8), 598, replace=False))
+    cuts[100] = cuts[99] + 3                               # a 3-bin partition: direct kernel
+    edges = np.unique(np.concatenate([[0], cuts, [n]])).astype(np.int64)
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges) as plan:
+        assert par.shape[0] * plan.n_part * 8 >= 2 << 20
+        F_d, Fk_d = fs.fstat_eval_batch(plan, torch_.as_tensor(par, device="cuda"))
+        torch_.cuda.synchronize()
+        F_d, Fk_d = F_d.cpu().numpy(), Fk_d.cpu().numpy()
+        n0 = fs.fstat_plan_launch_count(plan)
+        F_h, Fk_h = fs.fstat_eval_batch_host(plan, par)
+        assert fs.fstat_plan_launch_count(plan) - n0 > 12       # the ranges: more launches than the device call's 8
+        pin = torch_.as_tensor(par).pin_memory()
+        F_p, Fk_p = fs.fstat_eval_batch_host(plan, pin)
+        F_q, Fk_q = fs.fstat_eval_batch_host(plan, pin)
+        F_e, Fk_e = fs.fstat_eval_batch(plan, torch_.as_tensor(par, device="cuda"))      # and the plain call still works
+        torch_.cuda.synchronize()
+    np.testing.assert_array_equal(F_h, F_d)
+    np.testing.assert_array_equal(Fk_h, Fk_d)
+    np.testing.assert_array_equal(F_p.numpy(), F_d)
+    np.testing.assert_array_equal(Fk_p.numpy(), Fk_d)
+    np.testing.assert_array_equal(Fk_q.numpy(), Fk_d)
+    np.testing.assert_array_equal(Fk_e.cpu().numpy(), Fk_d)
+    sample = np.array([0, 100, 511])
+    F_o, Fk_o = orc.fstat_batch(ds.freq, ds.dw, ds.inv_sn, edges, par[sample])
+    assert _rel(Fk_h[sample], Fk_o).max() <= RTOL and _rel(F_h[sample], F_o).max() <= RTOL
+
+
 def test_empty_batch_and_null_Fk(fs, torch_, orc, tiny):
     ds = tiny
     par = syn.draw_particles(ds.cfg, 9)
