@@ -177,16 +177,26 @@ def parse_args():
     ap.add_argument("--interp-tol", type=float, default=1.0, help="plan option interp_tol")
     ap.add_argument("--pso", type=int, default=0, metavar="ITERS",
                     help="also time ITERS iterations of the device PSO (row f1) on this plan: swarms of 128 particles")
-    ap.add_argument("--bands", type=int, default=0, metavar="N_SEG",
-                    help="also time fstat_eval_batch_bands (row f2: per-template bands, N_SEG partitions) on this plan")
+    ap.add_argument("--bands", type=int, default=None, metavar="N_SEG",
+                    help="also time fstat_eval_batch_bands (row f2: per-template bands, N_SEG partitions) on this plan; default: "
+                         "1024 on the default workload unless --no-sweep, else off")
     ap.add_argument("--bands-lattice", type=int, default=1,
                     help="edge lattice of --bands in bins (1: edges at any bin; >= 32: the lattice cells are the work units)")
-    ap.add_argument("--channels", type=int, default=0, metavar="N",
-                    help="also time fstat_eval_batch_channels (row f4: the first N of the TDI channels A, E, T, common amplitudes)")
+    ap.add_argument("--channels", type=int, default=None, metavar="N",
+                    help="also time fstat_eval_batch_channels (row f4: the first N of the TDI channels A, E, T, common amplitudes); "
+                         "default: 3 on the default workload unless --no-sweep, else off")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-sweep", action="store_true", help="skip the N_p sweep rows the default workload adds to the line")
+    ap.add_argument("--no-sweep", action="store_true",
+                    help="skip what the default workload adds to the line: the N_p sweep rows and the rows f2 / f4 legs (bands, channels)")
     ap.add_argument("--cpu-sample", type=int, default=None, help="particles in the cpu_baseline sample")
-    return ap.parse_args()
+    args = ap.parse_args()
+    default_wl = args.config == "first_stage" and args.n_part is None and args.particles is None and args.impl == "ours"
+    extras = default_wl and not args.no_sweep
+    if args.bands is None:
+        args.bands = 1024 if extras else 0
+    if args.channels is None:
+        args.channels = 3 if extras else 0
+    return args
 
 
 def dataset_for(cfg, template_fn):
