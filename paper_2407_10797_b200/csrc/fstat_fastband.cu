@@ -77,13 +77,14 @@ cudaError_t launch_build_prefix_gram(const double *fw, int64_t n_bins, int level
 // =================================================================================================
 // the kernel
 // =================================================================================================
-constexpr int kBandStages = 2;
+constexpr int kBandStages = 3;
 
 struct __align__(16) BandSmem {
     double2 tile[kBandStages][kFastTile];      // folded data, 512-bin tiles (TMA bulk copies)
     double win[kWinNodes][kNSlow][kThreads];   // per-thread ring of the last six node values
     double2 snap[4][kThreads];                 // A_0..A_3 of a thread at its cut
     uint64_t full[kBandStages];
+    uint32_t released[kBandStages];            // warps that have left the tile in this stage
 };
 
 // monomial coefficients in s = bin - node0 of the cubic through y0..y3 at t = -1, 0, 1, 2 (t = s / S)
@@ -209,7 +210,7 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kBandStages; ++s) mbar_init(&sm.full[s], 1);
+        for (int s = 0; s < kBandStages; ++s) { mbar_init(&sm.full[s], 1); sm.released[s] = 0u; }
         mbar_fence_init();
     }
     __syncthreads();
@@ -535,8 +536,22 @@ __global__ void __launch_bounds__(kThreads, 3) fstat_fastband_kernel(const __gri
         }
       }
     }
-    __syncthreads();                                         // every warp is done with this tile
-    if (tid == 0 && tl + kBandStages < n_tiles) issue_tile(tl + kBandStages);
+    // The warps are not held together tile by tile: a warp that has left this tile says so, and the LAST of the four to
+    // leave re-arms the stage with the tile kBandStages further on.  A warp runs ahead of the slowest one by up to
+    // kBandStages tiles; nobody waits for anything but the data.
+    __syncwarp();
+    if ((tid & 31) == 0) {
+        __threadfence_block();                               // this warp's reads of the tile come before its release
+        const uint32_t old = atomicAdd(&sm.released[tl % kBandStages], 1u);
+        if (old == (uint32_t)(kThreads / 32 - 1)) {
+            atomicExch(&sm.released[tl % kBandStages], 0u);
+            __threadfence_block();
+            if (tl + kBandStages < n_tiles) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                issue_tile(tl + kBandStages);
+            }
+        }
+    }
   }
     if ((tid & 31) == 0 && st_int > 0u && a.b.stats != nullptr) {
         atomicAdd(&a.b.stats[0], (unsigned long long)st_bins);
