@@ -349,7 +349,7 @@ fstat_status build_gram_tables(fstat_plan *pl)
         for (int32_t k = 1; k < n_part; ++k) cnt[k] = cnt[k - 1] + ((pl->edges[k] % S) != 0 ? 1 : 0);
         if (!pl->fast_ok) continue;
         const int64_t n_sub = (pl->n_bins + S - 1) / S + cnt[n_part - 1];
-        CU_TRY(pl, grow(&pl->d_gram[l], &pl->gram_cap[l], (size_t)n_sub * kNGram));
+        CU_TRY(pl, grow(&pl->d_gram[l], &pl->gram_cap[l], (size_t)n_sub * kNW));
         CU_TRY(pl, cudaMemcpy(pl->d_cnt, cnt.data(), (size_t)n_part * sizeof(int32_t), cudaMemcpyHostToDevice));
         CU_TRY(pl, launch_build_gram(pl->d_fw, pl->d_edges32, n_part, pl->n_bins, l, pl->d_cnt, pl->d_gram[l], 0));
         CU_TRY(pl, cudaDeviceSynchronize());   // d_cnt is reused by the next level

@@ -91,9 +91,13 @@ __global__ void build_gram_kernel(const double2 *__restrict__ fw, const int32_t 
     for (int j = 0; j < kNGram; ++j) g[j] = 0.0;
     for (int64_t i = b0; i < b1; ++i) {
         if (i == (int64_t)edges[k + 1]) {                  // partition edge inside the interval: flush
-            double *out = gram + (m + cnt[k]) * kNGram;
+            double W[kNW];
+            gram_to_w(g, W);
+            double *out = gram + (m + cnt[k]) * kNW;
 #pragma unroll
-            for (int j = 0; j < kNGram; ++j) { out[j] = g[j]; g[j] = 0.0; }
+            for (int j = 0; j < kNW; ++j) out[j] = W[j];
+#pragma unroll
+            for (int j = 0; j < kNGram; ++j) g[j] = 0.0;
             ++k;
         }
         const double w = fw[i].y;
@@ -105,9 +109,11 @@ __global__ void build_gram_kernel(const double2 *__restrict__ fw, const int32_t 
 #pragma unroll
             for (int b = a; b < 4; ++b) g[j++] += w * l[a] * l[b];
     }
-    double *out = gram + (m + cnt[k]) * kNGram;
+    double W[kNW];
+    gram_to_w(g, W);
+    double *out = gram + (m + cnt[k]) * kNW;
 #pragma unroll
-    for (int j = 0; j < kNGram; ++j) out[j] = g[j];
+    for (int j = 0; j < kNW; ++j) out[j] = W[j];
 }
 
 cudaError_t launch_build_gram(const double *fw, const int32_t *edges, int32_t n_part, int64_t n_bins,
@@ -321,7 +327,7 @@ __device__ __forceinline__ void fast_kernel_body(const FastArgs &a)
 #pragma unroll
     for (int j = 0; j < kNAcc; ++j) acc[j] = 0.0;
 
-    const double *gram = a.gram[lvl] + (int64_t)a.seg_gbase[seg * kNLevels + lvl] * kNGram;
+    const double *gram = a.gram[lvl] + (int64_t)a.seg_gbase[seg * kNLevels + lvl] * kNW;
     int cur_tile = -1;
     int cur_seg = seg;
     int seg_hi = a.seg_edge[cur_seg + 1];
@@ -428,83 +434,42 @@ __device__ __forceinline__ void fast_kernel_body(const FastArgs &a)
         }
 #undef FSTAT_BIN_STEP
 
-        // ---- the slow factors of this interval: economised cubic of T'_+, T'_x as values at t = -1, 0, 1, 2
-        double ypr[4], ypi[4], ycr[4], yci[4];
-        {
-            double v[6], yref;
+        // ---- the slow factors of this interval: node values of T'_+, T'_x at t = -2 .. 3 (the economised cubic through
+        // them is applied inside the sums, never formed)
+        double vpr[6], vpi[6], vcr[6], vci[6];
 #pragma unroll
-            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][1][tid];
-            economise(v, yref, ypr);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) ypr[q] += yref;
-#pragma unroll
-            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][2][tid];
-            economise(v, yref, ypi);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) ypi[q] += yref;
-#pragma unroll
-            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][3][tid];
-            economise(v, yref, ycr);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) ycr[q] += yref;
-#pragma unroll
-            for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][4][tid];
-            economise(v, yref, yci);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) yci[q] += yref;
+        for (int k = 0; k < 6; ++k) {
+            const int sl = (s_base + k) % kWinNodes;
+            vpr[k] = sm.win[sl][1][tid]; vpi[k] = sm.win[sl][2][tid];
+            vcr[k] = sm.win[sl][3][tid]; vci[k] = sm.win[sl][4][tid];
         }
         if (seg_start) {
             seg_start = false;
-            const double n2 = fma(ypr[1], ypr[1], ypi[1] * ypi[1]), x2 = fma(ycr[1], ycr[1], yci[1] * yci[1]);
+            const double n2 = fma(vpr[2], vpr[2], vpi[2] * vpi[2]), x2 = fma(vcr[2], vcr[2], vci[2] * vci[2]);
             const bool use = n2 > 1e-6 * x2;                                  // else T'_+ ~ 0 there: keep u_x
             const double inv = use ? 1.0 / n2 : 0.0;
-            c_re = fma(ycr[1], ypr[1], yci[1] * ypi[1]) * inv;               // T'_x conj(T'_+) / |T'_+|^2
-            c_im = fma(yci[1], ypr[1], -ycr[1] * ypi[1]) * inv;
+            c_re = fma(vcr[2], vpr[2], vci[2] * vpi[2]) * inv;               // T'_x conj(T'_+) / |T'_+|^2 at node "0"
+            c_im = fma(vci[2], vpr[2], -vcr[2] * vpi[2]) * inv;
         }
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {                                        // node values of T'_x - c T'_+
-            ycr[q] -= fma(c_re, ypr[q], -c_im * ypi[q]);
-            yci[q] -= fma(c_re, ypi[q], c_im * ypr[q]);
+        for (int k = 0; k < 6; ++k) {                                        // node values of T'_x - c T'_+
+            vcr[k] -= fma(c_re, vpr[k], -c_im * vpi[k]);
+            vci[k] -= fma(c_re, vpi[k], c_im * vpr[k]);
         }
-        // ---- z_P += sum_n conj(c^P_n) A_n
-        const double U = (double)(j1 - node0);
+        // ---- z_P += sum_i conj(T'_P(i)) q_i = sum_k conj(v^P_k) B_k
         {
-            double cr[4], ci[4];
-            newton_coefs(ypr[0], ypr[1], ypr[2], ypr[3], rS, U, cr);
-            newton_coefs(ypi[0], ypi[1], ypi[2], ypi[3], rS, U, ci);
-            acc[0] += fma(cr[0], A0r, fma(ci[0], A0i, fma(cr[1], A1r, fma(ci[1], A1i,
-                      fma(cr[2], A2r, fma(ci[2], A2i, fma(cr[3], A3r, ci[3] * A3i)))))));
-            acc[1] += fma(cr[0], A0i, fma(-ci[0], A0r, fma(cr[1], A1i, fma(-ci[1], A1r,
-                      fma(cr[2], A2i, fma(-ci[2], A2r, fma(cr[3], A3i, -ci[3] * A3r)))))));
-            newton_coefs(ycr[0], ycr[1], ycr[2], ycr[3], rS, U, cr);
-            newton_coefs(yci[0], yci[1], yci[2], yci[3], rS, U, ci);
-            acc[2] += fma(cr[0], A0r, fma(ci[0], A0i, fma(cr[1], A1r, fma(ci[1], A1i,
-                      fma(cr[2], A2r, fma(ci[2], A2i, fma(cr[3], A3r, ci[3] * A3i)))))));
-            acc[3] += fma(cr[0], A0i, fma(-ci[0], A0r, fma(cr[1], A1i, fma(-ci[1], A1r,
-                      fma(cr[2], A2i, fma(-ci[2], A2r, fma(cr[3], A3i, -ci[3] * A3r)))))));
+            const double A[8] = {A0r, A0i, A1r, A1i, A2r, A2i, A3r, A3i};
+            double Br[6], Bi[6];
+            subblock_weights(A, rS, (double)(j1 - node0), Br, Bi);
+            z_from_nodes(vpr, vpi, Br, Bi, acc[0], acc[1]);
+            z_from_nodes(vcr, vci, Br, Bi, acc[2], acc[3]);
         }
-        // ---- m_PQ += y^P G conj(y^Q)   (Gram matrix of the Lagrange basis over this sub-block)
+        // ---- m_PQ += (W v^P) . conj(W v^Q)   (W = L^T E of this sub-block: G = L L^T its Gram matrix)
         {
-            const double2 *gp = reinterpret_cast<const double2 *>(gram);
-            const double2 g01 = gp[0], g23 = gp[1], g45 = gp[2], g67 = gp[3], g89 = gp[4];
-            const double G[4][4] = {{g01.x, g01.y, g23.x, g23.y},
-                                    {g01.y, g45.x, g45.y, g67.x},
-                                    {g23.x, g45.y, g67.y, g89.x},
-                                    {g23.y, g67.x, g89.x, g89.y}};
-            double mpp = 0.0, mcc = 0.0, mre = 0.0, mim = 0.0;
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const double vpr = fma(G[r][0], ypr[0], fma(G[r][1], ypr[1], fma(G[r][2], ypr[2], G[r][3] * ypr[3])));
-                const double vpi = fma(G[r][0], ypi[0], fma(G[r][1], ypi[1], fma(G[r][2], ypi[2], G[r][3] * ypi[3])));
-                const double vcr = fma(G[r][0], ycr[0], fma(G[r][1], ycr[1], fma(G[r][2], ycr[2], G[r][3] * ycr[3])));
-                const double vci = fma(G[r][0], yci[0], fma(G[r][1], yci[1], fma(G[r][2], yci[2], G[r][3] * yci[3])));
-                mpp = fma(ypr[r], vpr, fma(ypi[r], vpi, mpp));
-                mcc = fma(ycr[r], vcr, fma(yci[r], vci, mcc));
-                mre = fma(ypr[r], vcr, fma(ypi[r], vci, mre));      // Re sum y^+ conj(v^x)
-                mim = fma(ypi[r], vcr, fma(-ypr[r], vci, mim));     // Im
-            }
+            double mpp, mcc, mre, mim;
+            gram_forms(gram, vpr, vpi, vcr, vci, mpp, mcc, mre, mim);
             acc[4] += mpp; acc[5] += mcc; acc[6] += mre; acc[7] += mim;
-            gram += kNGram;
+            gram += kNW;
         }
         if (j1 == seg_hi) {                                  // segment finished: flush its eight sums
             double *out = a.partial + ((int64_t)cur_seg * kNPartial) * a.P_pad + p * a.part_sp;

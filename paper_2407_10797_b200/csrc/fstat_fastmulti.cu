@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(kThreads, 2) fstat_fastmulti_kernel(const __gr
         c_re[ch] = c_im[ch] = 0.0;
     }
 
-    int64_t gidx = (int64_t)a.seg_gbase[seg * kNLevels + lvl] * kNGram;
+    int64_t gidx = (int64_t)a.seg_gbase[seg * kNLevels + lvl] * kNW;
     int cur_tile = -1;
     int cur_seg = seg;
     int seg_hi = a.seg_edge[cur_seg + 1];
@@ -233,86 +233,42 @@ __global__ void __launch_bounds__(kThreads, 2) fstat_fastmulti_kernel(const __gr
         const double U = (double)(j1 - node0);
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) {
-            // ---- the slow factors of this interval and channel: values of the economised cubic at t = -1, 0, 1, 2
-            double ypr[4], ypi[4], ycr[4], yci[4];
-            {
-                double v[6], yref;
+            // ---- the slow factors of this interval and channel: node values at t = -2 .. 3
+            double vpr[6], vpi[6], vcr[6], vci[6];
 #pragma unroll
-                for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][1 + 4 * ch][tid];
-                economise(v, yref, ypr);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) ypr[q] += yref;
-#pragma unroll
-                for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][2 + 4 * ch][tid];
-                economise(v, yref, ypi);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) ypi[q] += yref;
-#pragma unroll
-                for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][3 + 4 * ch][tid];
-                economise(v, yref, ycr);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) ycr[q] += yref;
-#pragma unroll
-                for (int k = 0; k < 6; ++k) v[k] = sm.win[(s_base + k) % kWinNodes][4 + 4 * ch][tid];
-                economise(v, yref, yci);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) yci[q] += yref;
+            for (int k = 0; k < 6; ++k) {
+                const int sl = (s_base + k) % kWinNodes;
+                vpr[k] = sm.win[sl][1 + 4 * ch][tid]; vpi[k] = sm.win[sl][2 + 4 * ch][tid];
+                vcr[k] = sm.win[sl][3 + 4 * ch][tid]; vci[k] = sm.win[sl][4 + 4 * ch][tid];
             }
             if (seg_start) {
-                const double n2 = fma(ypr[1], ypr[1], ypi[1] * ypi[1]), x2 = fma(ycr[1], ycr[1], yci[1] * yci[1]);
+                const double n2 = fma(vpr[2], vpr[2], vpi[2] * vpi[2]), x2 = fma(vcr[2], vcr[2], vci[2] * vci[2]);
                 const bool use = n2 > 1e-6 * x2;                              // else T'_+ ~ 0 there: keep u_x
                 const double inv = use ? 1.0 / n2 : 0.0;
-                c_re[ch] = fma(ycr[1], ypr[1], yci[1] * ypi[1]) * inv;       // T'_x conj(T'_+) / |T'_+|^2
-                c_im[ch] = fma(yci[1], ypr[1], -ycr[1] * ypi[1]) * inv;
+                c_re[ch] = fma(vcr[2], vpr[2], vci[2] * vpi[2]) * inv;       // T'_x conj(T'_+) / |T'_+|^2 at node "0"
+                c_im[ch] = fma(vci[2], vpr[2], -vcr[2] * vpi[2]) * inv;
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {                                    // node values of T'_x - c T'_+
-                ycr[q] -= fma(c_re[ch], ypr[q], -c_im[ch] * ypi[q]);
-                yci[q] -= fma(c_re[ch], ypi[q], c_im[ch] * ypr[q]);
+            for (int k = 0; k < 6; ++k) {                                    // node values of T'_x - c T'_+
+                vcr[k] -= fma(c_re[ch], vpr[k], -c_im[ch] * vpi[k]);
+                vci[k] -= fma(c_re[ch], vpi[k], c_im[ch] * vpr[k]);
             }
-            // ---- z_P += sum_n conj(c^P_n) A_n
+            // ---- z_P += sum_k conj(v^P_k) B_k
             {
-                const double A0r = A[ch][0], A0i = A[ch][1], A1r = A[ch][2], A1i = A[ch][3];
-                const double A2r = A[ch][4], A2i = A[ch][5], A3r = A[ch][6], A3i = A[ch][7];
-                double cr[4], ci[4];
-                newton_coefs(ypr[0], ypr[1], ypr[2], ypr[3], rS, U, cr);
-                newton_coefs(ypi[0], ypi[1], ypi[2], ypi[3], rS, U, ci);
-                acc[ch][0] += fma(cr[0], A0r, fma(ci[0], A0i, fma(cr[1], A1r, fma(ci[1], A1i,
-                              fma(cr[2], A2r, fma(ci[2], A2i, fma(cr[3], A3r, ci[3] * A3i)))))));
-                acc[ch][1] += fma(cr[0], A0i, fma(-ci[0], A0r, fma(cr[1], A1i, fma(-ci[1], A1r,
-                              fma(cr[2], A2i, fma(-ci[2], A2r, fma(cr[3], A3i, -ci[3] * A3r)))))));
-                newton_coefs(ycr[0], ycr[1], ycr[2], ycr[3], rS, U, cr);
-                newton_coefs(yci[0], yci[1], yci[2], yci[3], rS, U, ci);
-                acc[ch][2] += fma(cr[0], A0r, fma(ci[0], A0i, fma(cr[1], A1r, fma(ci[1], A1i,
-                              fma(cr[2], A2r, fma(ci[2], A2i, fma(cr[3], A3r, ci[3] * A3i)))))));
-                acc[ch][3] += fma(cr[0], A0i, fma(-ci[0], A0r, fma(cr[1], A1i, fma(-ci[1], A1r,
-                              fma(cr[2], A2i, fma(-ci[2], A2r, fma(cr[3], A3i, -ci[3] * A3r)))))));
+                double Br[6], Bi[6];
+                subblock_weights(A[ch], rS, U, Br, Bi);
+                z_from_nodes(vpr, vpi, Br, Bi, acc[ch][0], acc[ch][1]);
+                z_from_nodes(vcr, vci, Br, Bi, acc[ch][2], acc[ch][3]);
             }
-            // ---- m_PQ += y^P G conj(y^Q)   (Gram matrix of the Lagrange basis over this sub-block, this channel's weights)
+            // ---- m_PQ += (W v^P) . conj(W v^Q) with this channel's table (its own noise weights)
             {
-                const double2 *gp = reinterpret_cast<const double2 *>(a.gram[ch][lvl] + gidx);
-                const double2 g01 = gp[0], g23 = gp[1], g45 = gp[2], g67 = gp[3], g89 = gp[4];
-                const double G[4][4] = {{g01.x, g01.y, g23.x, g23.y},
-                                        {g01.y, g45.x, g45.y, g67.x},
-                                        {g23.x, g45.y, g67.y, g89.x},
-                                        {g23.y, g67.x, g89.x, g89.y}};
-                double mpp = 0.0, mcc = 0.0, mre = 0.0, mim = 0.0;
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const double vpr = fma(G[r][0], ypr[0], fma(G[r][1], ypr[1], fma(G[r][2], ypr[2], G[r][3] * ypr[3])));
-                    const double vpi = fma(G[r][0], ypi[0], fma(G[r][1], ypi[1], fma(G[r][2], ypi[2], G[r][3] * ypi[3])));
-                    const double vcr = fma(G[r][0], ycr[0], fma(G[r][1], ycr[1], fma(G[r][2], ycr[2], G[r][3] * ycr[3])));
-                    const double vci = fma(G[r][0], yci[0], fma(G[r][1], yci[1], fma(G[r][2], yci[2], G[r][3] * yci[3])));
-                    mpp = fma(ypr[r], vpr, fma(ypi[r], vpi, mpp));
-                    mcc = fma(ycr[r], vcr, fma(yci[r], vci, mcc));
-                    mre = fma(ypr[r], vcr, fma(ypi[r], vci, mre));      // Re sum y^+ conj(v^x)
-                    mim = fma(ypi[r], vcr, fma(-ypr[r], vci, mim));     // Im
-                }
+                double mpp, mcc, mre, mim;
+                gram_forms(a.gram[ch][lvl] + gidx, vpr, vpi, vcr, vci, mpp, mcc, mre, mim);
                 acc[ch][4] += mpp; acc[ch][5] += mcc; acc[ch][6] += mre; acc[ch][7] += mim;
             }
         }
         seg_start = false;
-        gidx += kNGram;
+        gidx += kNW;
         if (j1 == seg_hi) {                                  // segment finished: flush the eight sums of every channel
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {

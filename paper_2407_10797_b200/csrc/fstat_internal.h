@@ -69,7 +69,8 @@ constexpr int kFastTileShift = 9;
 constexpr int kFastTile = 1 << kFastTileShift;       // bins per TMA tile of the folded data (8 KiB), aligned to its size;
                                                      // >= kMaxStride so that no sub-block straddles two tiles
 constexpr int kFastStages = 3;
-constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block
+constexpr int kNGram = 10;                           // upper triangle of the 4x4 Gram matrix of a sub-block (prefix tables of row f2)
+constexpr int kNW = 24;                              // per sub-block table of the interpolating kernels: W = L^T E (4 x 6), G = L L^T (gram_to_w)
 
 // per-segment factors of the a-priori interpolation error bound (host-made, see make_seg_crit)
 struct SegCrit {
@@ -111,7 +112,7 @@ enum : uint32_t {
 struct FastArgs {
     const double *dwp;            // [n_bins][2] folded data 4 df f^(-7/6) conj(K_f) d/S_n
     const double *node;           // [n_node_rows][kTabW]; row r <-> bin (r - kNodePad) * kNodeStride
-    const double *gram[kNLevels]; // [n_sub(level)][kNGram]
+    const double *gram[kNLevels]; // [n_sub(level)][kNW]
     const double *coef;           // [kNCoef][P_pad]
     const int32_t *seg_edge;      // [n_seg + 1]
     const int32_t *seg_gbase;     // [n_seg][kNLevels] index of the segment's first sub-block in gram[level]

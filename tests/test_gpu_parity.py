@@ -249,7 +249,7 @@ def test_changing_batch_sizes_reuse_cached_segment_tables_bit_for_bit(fs, torch_
     for P in set(sizes):
         ref[P] = _gpu_eval(fs, torch_, ds, ds.edges(8), par[:P])
     with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(8)) as plan:
-        assert fs.fstat_plan_table_bytes(plan) < 100 * ds.n_bins          # 32 + 24 + ~20 bytes per bin, not 268
+        assert fs.fstat_plan_table_bytes(plan) < 140 * ds.n_bins          # 32 + 24 + ~48 bytes per bin, not 268 + 20
         for rnd in range(2):
             for P in sizes:
                 F, Fk = fs.fstat_eval_batch(plan, torch_.as_tensor(np.ascontiguousarray(par[:P]), device="cuda"))
