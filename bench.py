@@ -41,22 +41,25 @@ UNIT = "template-bins/s"
 #   per node interval and per work item of a particle: EXECUTED counts measured with ncu
 #       (sm__inst_executed_pipe_fp64.sum at forced strides 8 / 512 and two segment lengths; profiles/ names the build).
 FAST_FP64_PER_BIN = 19.0
-FAST_FP64_PER_INTERVAL = 736.0
-FAST_FP64_PER_ITEM = 1105.0
+FAST_FP64_PER_INTERVAL = 648.0
+FAST_FP64_PER_ITEM = 842.0
 DIRECT_FP64_PER_BIN = 267.0
-FP64_COUNTS_BUILD = ("per node interval / per work item: ncu executed counts of round-1 build c21f730 (profiles/r1_v6.md); the total "
-                     "they predict for the final build is within 0.6 % of its ncu capture (profiles/r2.md)")
+FP64_COUNTS_BUILD = ("per node interval / per work item: least-squares fit to ncu executed counts (smsp__inst_executed_pipe_fp64.sum) of "
+                     "build bd29abd at six settings (automatic strides, forced strides 8 / 64 / 512, another segment length, config 2 "
+                     "N_p = 16); the fit reproduces each of the six totals within 0.2 % (profiles/r2.md)")
 NOMINAL_FP64_INST_PER_S = 148 * 64 * 1.965e9        # 148 SMs x 64 FP64 lanes x 1.965 GHz (B200_PROFILING.md)
 STRIDES = (0, 8, 16, 32, 64, 128, 256, 512)          # index 0 = direct kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of one fstat_fast_kernel launch on the default workload, from the
 # ncu --set full capture named beside it (None when no capture of the current hot kernel exists)
-NCU_DRAM_BYTES_PER_LAUNCH = 224.5e6
-# the same capture: smsp__inst_executed.sum = 30.1 warp instructions per template-bin, 24.2 of them on the FP64 pipe
-NCU_OTHER_INST_PER_TEMPLATE_BIN = 30.1 - 24.2
-NCU_DRAM_CAPTURE = "profiles/r2.md (32.5 MB read + 191.9 MB written), ncu --set full of build 1ecb204 (hot kernel unchanged since)"
+NCU_DRAM_BYTES_PER_LAUNCH = 222.4e6
+# the same capture: smsp__inst_executed.sum = 29.72 warp instructions per template-bin, 23.51 of them on the FP64 pipe
+NCU_OTHER_INST_PER_TEMPLATE_BIN = 29.72 - 23.51
+NCU_DRAM_CAPTURE = "profiles/r2.md (34.3 MB read + 188.1 MB written), ncu capture of build bd29abd"
 # row f2 (fstat_fastband_kernel), per WARP-level unit of work counted by the kernel itself (fstat_plan_band_stats): the
 # per-bin and per-interval counts are those of fstat_fast_kernel; a node interval in which some lane has a partition edge
 # runs the cut path as well (calibrated on the ncu capture of profiles/r2_bands.md: 9.897e8 FP64 warp-instructions)
+BAND_FP64_PER_INTERVAL = 736.0      # fstat_fastband_kernel keeps the four-node sub-block code of round-2 build 1ecb204
+BAND_FP64_PER_RUN = 1105.0
 BAND_FP64_PER_CUT_INTERVAL = 350.0
 NCU_BAND_DRAM_BYTES = 106.6e6     # profiles/r2_bands.md: N_seg = 1024, edges at any bin, config 1 data, build 1ecb204
 
@@ -592,8 +595,8 @@ def run_ours(args):
         ms_b_e2e = (time.perf_counter() - t0) * 1e3 / n_b
         st = fs.fstat_plan_band_stats(plan)               # warp-level bins, intervals, intervals with a cut, runs
         per_bin = mix["per_bin"] if mix else FAST_FP64_PER_BIN
-        b_inst = 32.0 * (per_bin * st[0] + FAST_FP64_PER_INTERVAL * st[1] + BAND_FP64_PER_CUT_INTERVAL * st[2]
-                         + FAST_FP64_PER_ITEM * st[3])
+        b_inst = 32.0 * (per_bin * st[0] + BAND_FP64_PER_INTERVAL * st[1] + BAND_FP64_PER_CUT_INTERVAL * st[2]
+                         + BAND_FP64_PER_RUN * st[3])
         kms_mean = float(np.mean(kms)) if len(kms) else float("nan")
         band_roofline = {"bound": "alu", "pipe": "fp64", "kernel": "fstat_fastband_kernel",
                          "achieved": b_inst / (kms_mean * 1e-3) / 1e12, "peak": fp64_rate / 1e12, "unit": "T FP64-pipe inst/s",
@@ -602,9 +605,9 @@ def run_ours(args):
                          "fp64_inst_per_call": b_inst, "fp64_inst_per_in_band_template_bin": b_inst / max(in_band, 1.0),
                          "warp_bins": int(st[0]), "warp_node_intervals": int(st[1]), "warp_intervals_with_a_cut": int(st[2]),
                          "warp_runs": int(st[3]), "bins_walked_share_of_grid": 32.0 * st[0] / (float(P) * ds.n_bins),
-                         "fp64_inst_model": {"per_bin": per_bin, "per_node_interval": FAST_FP64_PER_INTERVAL,
+                         "fp64_inst_model": {"per_bin": per_bin, "per_node_interval": BAND_FP64_PER_INTERVAL,
                                              "per_interval_with_a_cut": BAND_FP64_PER_CUT_INTERVAL,
-                                             "per_run": FAST_FP64_PER_ITEM}}
+                                             "per_run": BAND_FP64_PER_RUN}}
         assert st[4] == 0, "fstat_fastband_kernel raised its internal-invariant flag"
         out["bands"] = {"n_seg": args.bands, "edge_lattice": args.bands_lattice, "ms_per_step": ms_b, "roofline": band_roofline,
                         "main_kernel_ms": float(np.mean(kms)) if len(kms) else None,
