@@ -141,6 +141,27 @@ FSTAT_API fstat_status fstat_eval_batch(fstat_plan *plan, int64_t P,
                                         void *cuda_stream);
 
 /*
+ * fstat_eval_batch_noalloc -- fstat_eval_batch for callers that cannot allocate device memory inside the call (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): same arguments, same kernels, same results
+ * bit for bit, but the workspace (coefficients, slot ranking, stride levels, work list, partial sums) is carved from ONE
+ * static device array of fstat_noalloc_scratch_bytes() = 32 MiB that every GPU which loads the library holds until the
+ * process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   Limit: the workspace of the batch must fit: about n_work_segments x 10 KiB + 24 KiB per 128 particles (one swarm of
+ *   128 particles on a 2.5-yr grid with N_p = 1024: 18 MB; 1024 particles with N_p = 64 on the same grid: 29 MB), and
+ *   P <= 16384.  Beyond that: EUNSUPPORTED, with the sizes in fstat_last_error.
+ *   Set-up: the plan's segment tables for this batch size are plan state (device memory the plan owns): they exist once
+ *   fstat_eval_batch has been called with a batch of this size (number of 128-particle groups) since the last
+ *   fstat_plan_create / fstat_plan_set_partitions; without them the call returns EUNSUPPORTED and says so.
+ *   Sharing: EVERY call, on any plan and any stream of the device, uses the same array, which keeps the last call's
+ *   contents (the call clears what it needs cleared).  Calls that overlap on the GPU -- two streams, two host threads --
+ *   RACE: keep them on one stream, or order them with events.  F and Fk are written only by this call's last kernels.
+ * Errors: as fstat_eval_batch, plus EUNSUPPORTED as above; never ENOMEM.
+ */
+FSTAT_API fstat_status fstat_eval_batch_noalloc(fstat_plan *plan, int64_t P, const double *params, double *F, double *Fk,
+                                                void *cuda_stream);
+FSTAT_API int64_t fstat_noalloc_scratch_bytes(void);
+
+/*
  * fstat_eval_batch_bands -- SURVEY row f2: the semi-coherent F-statistic with the paper's OWN segment
  * limits (the number of segments is the same for all templates; the lowest and highest
  * limits are "the lowest and highest instantaneous frequencies occurring during the observation period

@@ -14,6 +14,7 @@ from __future__ import annotations
 from .binding import (  # noqa: F401
     FstatError, Options, Plan, STATUS, TDI_CHANNELS,
     fstat_default_options, fstat_plan_create, fstat_plan_set_partitions, fstat_eval_batch,
+    fstat_eval_batch_noalloc, fstat_noalloc_scratch_bytes,
     fstat_eval_batch_host, fstat_eval_batch_bands, fstat_eval_batch_bands_host, fstat_eval_amplitudes_bands, fstat_eval_batch_channels, fstat_eval_amplitudes, fstat_eval_template, fstat_plan_destroy, fstat_plan_n_bins,
     fstat_plan_n_part, fstat_plan_device, fstat_plan_n_ctas, fstat_plan_launch_count, fstat_plan_table_bytes, fstat_plan_band_stats,
     fstat_plan_main_kernel_ms, fstat_plan_level_bins, fstat_edges_equal_bins, fstat_probe_pipe_peak,

@@ -18,6 +18,7 @@ STATUS = {0: "FSTAT_OK", 1: "FSTAT_EINVAL", 2: "FSTAT_ENOMEM", 3: "FSTAT_ECUDA",
 # every symbol include/fstat.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "fstat_default_options", "fstat_plan_create", "fstat_plan_set_partitions", "fstat_eval_batch",
+    "fstat_eval_batch_noalloc", "fstat_noalloc_scratch_bytes",
     "fstat_eval_batch_host", "fstat_eval_batch_bands", "fstat_eval_batch_bands_host", "fstat_eval_amplitudes_bands", "fstat_eval_batch_channels", "fstat_eval_amplitudes", "fstat_eval_template", "fstat_plan_destroy", "fstat_plan_n_bins",
     "fstat_plan_n_part", "fstat_plan_device", "fstat_plan_n_ctas", "fstat_plan_launch_count", "fstat_plan_table_bytes", "fstat_plan_band_stats",
     "fstat_plan_main_kernel_ms", "fstat_plan_level_bins", "fstat_edges_equal_bins", "fstat_probe_pipe_peak",
@@ -73,6 +74,10 @@ def load_library():
         L.fstat_plan_set_partitions.restype = C.c_int
         L.fstat_eval_batch.argtypes = [vp, i64, vp, vp, vp, vp]
         L.fstat_eval_batch.restype = C.c_int
+        L.fstat_eval_batch_noalloc.argtypes = [vp, i64, vp, vp, vp, vp]
+        L.fstat_eval_batch_noalloc.restype = C.c_int
+        L.fstat_noalloc_scratch_bytes.argtypes = []
+        L.fstat_noalloc_scratch_bytes.restype = i64
         L.fstat_eval_amplitudes.argtypes = [vp, i64, vp, vp, vp]
         L.fstat_eval_amplitudes.restype = C.c_int
         L.fstat_eval_batch_bands.argtypes = [vp, i64, vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
@@ -274,6 +279,23 @@ def fstat_eval_batch(plan: Plan, params, F=None, Fk=None, stream=None, want_Fk: 
     pFk = _dev_ptr(Fk, "Fk", P * plan.n_part) if Fk is not None else None
     _check(load_library().fstat_eval_batch(plan.handle, P, pp, pF, pFk, _stream_ptr(stream)), "fstat_eval_batch", plan)
     return F, Fk
+
+
+def fstat_eval_batch_noalloc(plan: Plan, params, F, Fk=None, stream=None):
+    """fstat_eval_batch with the workspace in the library's static 32 MiB device array: no device allocation inside the call
+    (the caller passes every buffer: params [P][6], F [P], Fk [P][N_p] or None, float64 CUDA tensors).  Calls that overlap
+    on the GPU race on that array; see include/fstat.h for the size limit and the set-up it needs."""
+    P = int(params.shape[0])
+    pp = _dev_ptr(params, "params", 6 * P)
+    pF = _dev_ptr(F, "F", P)
+    pFk = _dev_ptr(Fk, "Fk", P * plan.n_part) if Fk is not None else None
+    _check(load_library().fstat_eval_batch_noalloc(plan.handle, P, pp, pF, pFk, _stream_ptr(stream)),
+           "fstat_eval_batch_noalloc", plan)
+    return F, Fk
+
+
+def fstat_noalloc_scratch_bytes() -> int:
+    return int(load_library().fstat_noalloc_scratch_bytes())
 
 
 def fstat_eval_batch_bands(plan: Plan, params, n_seg: int, edge_lattice: int = 1, stream=None, want_Fk: bool = True,

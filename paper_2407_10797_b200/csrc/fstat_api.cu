@@ -1383,3 +1383,160 @@ fstat_status fstat_extrinsic_from_amplitudes(const double *a, double chirp_mass_
 }
 
 }  // extern "C"
+
+/* ---- fstat_eval_batch_noalloc: the evaluation of fstat_eval_batch with its workspace in a static device array ---- */
+
+// Every GPU that loads the library holds this array until the process exits.  In host code the NAME is only a stand-in
+// for the symbol, not a device address: the address comes from cudaGetSymbolAddress, once per device, with that device
+// current (noalloc_scratch_base below).
+constexpr size_t kNoAllocBytes = (size_t)32 << 20;
+constexpr int64_t kNoAllocMaxP = 16384;       // = kRankBrute of fstat_kernels.cu: above it launch_prologue calls the cub radix sort
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+unsigned char *g_noalloc_base[kNoAllocMaxDevices] = {};
+
+// device address of the scratch array on `device` (which must be current); nullptr + *err on failure
+unsigned char *noalloc_scratch_base(int device, cudaError_t *err)
+{
+    *err = cudaSuccess;
+    if (device < 0 || device >= kNoAllocMaxDevices) { *err = cudaErrorInvalidDevice; return nullptr; }
+    if (!g_noalloc_base[device]) {
+        void *ptr = nullptr;
+        *err = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (*err != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        g_noalloc_base[device] = static_cast<unsigned char *>(ptr);
+    }
+    return g_noalloc_base[device];
+}
+
+// bump allocator over the scratch array: 256-byte aligned pieces
+struct Carver {
+    unsigned char *base;
+    size_t used = 0;
+    template <class T> T *take(size_t n)
+    {
+        T *p = reinterpret_cast<T *>(base + used);
+        used += (n * sizeof(T) + 255) / 256 * 256;
+        return p;
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+int64_t fstat_noalloc_scratch_bytes(void) { return (int64_t)kNoAllocBytes; }
+
+fstat_status fstat_eval_batch_noalloc(fstat_plan *pl, int64_t P, const double *params, double *F, double *Fk, void *stream)
+{
+    if (!pl) return FSTAT_EINVAL;
+    if (P < 0) return fail(pl, FSTAT_EINVAL, "P < 0");
+    if (P == 0) return FSTAT_OK;
+    if (!params || !F) return fail(pl, FSTAT_EINVAL, "params or F is NULL");
+    if (P > kNoAllocMaxP)
+        return fail(pl, FSTAT_EUNSUPPORTED, "fstat_eval_batch_noalloc: P > 16384 (the slot ranking above that size uses a library sort)");
+    DeviceGuard g(pl->device);
+    if (!g.ok) return fail(pl, FSTAT_ECUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)stream;
+
+    const int64_t n_groups = (P + kThreads - 1) / kThreads;
+    const int64_t P_pad = n_groups * kThreads;
+    // The segment tables of this batch size belong to the plan and are built (cudaMalloc) the first time a batch of this
+    // many 128-particle groups is evaluated: this call only looks them up.
+    if (pl->seg_groups != (int32_t)n_groups) {
+        const int64_t seg_len = auto_segment_len(pl, (int32_t)n_groups);
+        const SegTables *hit = nullptr;
+        for (const SegTables &t : pl->seg_cache)
+            if (t.seg_len == seg_len) { hit = &t; break; }
+        if (!hit)
+            return fail(pl, FSTAT_EUNSUPPORTED,
+                        "fstat_eval_batch_noalloc: the plan has no segment tables for this batch size yet; they are part of "
+                        "plan set-up: call fstat_eval_batch once with a batch of this size after fstat_plan_create / "
+                        "fstat_plan_set_partitions");
+        use_seg_tables(pl, *hit, (int32_t)n_groups);
+    }
+    if ((int64_t)pl->n_seg * n_groups >= ((int64_t)1 << 31))
+        return fail(pl, FSTAT_EUNSUPPORTED, "too many work items for one launch");
+
+    cudaError_t ce = cudaSuccess;
+    Carver cv{noalloc_scratch_base(pl->device, &ce)};
+    if (!cv.base) return fail(pl, FSTAT_ECUDA, std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(ce));
+    int32_t chunk = 0;
+    const int32_t n_chunk = epilogue_chunks(P, pl->n_part, &chunk);
+    double *d_coef = cv.take<double>((size_t)P_pad * kNCoef);
+    int32_t *d_valid = cv.take<int32_t>((size_t)P_pad);
+    int32_t *d_slot = cv.take<int32_t>((size_t)P);
+    int32_t *d_perm = cv.take<int32_t>((size_t)P_pad);
+    unsigned char *d_sort = cv.take<unsigned char>(prologue_scratch_bytes(P));
+    int8_t *d_level = cv.take<int8_t>((size_t)pl->n_seg * (size_t)n_groups);
+    int32_t *d_direct = cv.take<int32_t>((size_t)pl->n_seg * (size_t)n_groups + 1);
+    double *d_fpart = cv.take<double>((size_t)n_chunk * (size_t)P_pad);
+    double *d_partial = cv.take<double>((size_t)pl->n_seg * kNPartial * (size_t)P_pad);
+    if (cv.used > kNoAllocBytes) {
+        char msg[256];
+        snprintf(msg, sizeof(msg), "fstat_eval_batch_noalloc: this batch needs %zu bytes of workspace (%d work segments x %lld "
+                 "slots), the static scratch array holds %zu", cv.used, (int)pl->n_seg, (long long)P_pad, kNoAllocBytes);
+        return fail(pl, FSTAT_EUNSUPPORTED, msg);
+    }
+
+    // the launch sequence of eval_impl; nothing in the scratch has to start at zero except the direct kernel's work
+    // counter, which launch_schedule clears (every partial sum that is read is written by one of the two main kernels)
+    CU_TRY(pl, launch_prologue(params, P, P_pad, pl->opt.f_ref_e0, pl->opt.orbit_kappa, d_slot, nullptr, d_sort, d_coef, d_valid,
+                               d_perm, st));
+    BandSched bs{};
+    CU_TRY(pl, launch_schedule(d_coef, d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit, pl->d_seg_maxlvl,
+                               pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7, pl->opt.force_level, bs,
+                               d_level, d_direct + 1, d_direct, st));
+    FastArgs fa;
+    fa.dwp = pl->d_dwp;
+    fa.node = pl->d_node;
+    for (int l = 0; l < kNLevels; ++l) fa.gram[l] = pl->d_gram[l];
+    fa.coef = d_coef;
+    fa.seg_edge = pl->d_seg_edge;
+    fa.seg_gbase = pl->d_seg_gbase;
+    fa.level = d_level;
+    fa.partial = d_partial;
+    fa.part_sk = P_pad;
+    fa.part_sp = 1;
+    fa.P_pad = P_pad;
+    fa.n_groups = (int32_t)n_groups;
+    fa.n_seg = pl->n_seg;
+    fa.segs_per_cta = segs_per_cta(pl->n_bins, pl->n_seg);
+    fa.aet = pl->opt.tdi_channel >= FSTAT_TDI_A ? 1 : 0;
+    fa.chunk_begin = 0;
+    fa.chunk_count = 0;
+    fa.df = pl->df;
+    fa.orb = pl->orb;
+    MainArgs a;
+    a.dwp = pl->d_dwp;
+    a.fw = pl->d_fw;
+    a.arm_length_m = pl->opt.arm_length_m;
+    a.coef = d_coef;
+    a.seg_edge = pl->d_seg_edge;
+    a.direct_list = d_direct + 1;
+    a.direct_count = d_direct;
+    a.max_ctas = pl->n_sm * 12;
+    a.partial = d_partial;
+    a.part_sk = fa.part_sk;
+    a.part_sp = fa.part_sp;
+    a.P_pad = P_pad;
+    a.P = (int32_t)P;
+    a.n_groups = (int32_t)n_groups;
+    a.n_seg = pl->n_seg;
+    a.aet = fa.aet;
+    a.orb = pl->orb;
+    if (pl->fast_ok) CU_TRY(pl, launch_fast(fa, st));
+    CU_TRY(pl, launch_main(a, st));
+    PartialSet one{};
+    one.p[0] = d_partial;
+    one.n = 1;
+    CU_TRY(pl, launch_epilogue(one, pl->d_part_seg, d_valid, d_perm, P, P_pad, pl->n_part, pl->n_seg, d_fpart, F, Fk, st));
+    // keys, rank, prologue, stride selection, [interpolating], direct, epilogue, [chunk sums of F]
+    pl->n_launches += 5 + (pl->fast_ok ? 1 : 0) + 1 + (n_chunk > 1 ? 1 : 0);
+    return FSTAT_OK;
+}
+
+}  // extern "C"
