@@ -254,10 +254,11 @@ FSTAT_API fstat_status fstat_eval_amplitudes(fstat_plan *plan, int64_t P, const 
  *   out             HOST [4]: D_L, iota, psi, phi_c.  iota in [0, pi]; psi in (-pi/4, pi/4] (the branch of the paper's
  *                   arctan); phi_c in (-pi, pi]: the paper's arctan plus the half-plane that reproduces the sign of the
  *                   amplitudes (reading A25).  All-zero amplitudes give D_L = +inf and zeros.
- * D_L rests on the absolute normalisation of the library's response (link factor -i pi f L/c, TDI factor 1 - z^2, reading
- * A7), which is pinned against a time-domain simulation of the links (amplitude ratio within 5e-3, pin P9), and on the
- * amplitude / polarisation conventions behind Eq. B1, which the paper does not print (its ref. [89]): treat D_L as
- * relative to this library's normalisation; iota is free of both.
+ * What the four numbers mean physically is fixed by a test, not by convention (pin P20, reading A31): amplitudes
+ * estimated from the time-domain TDI signal of a quadrupole-formula binary at a known distance and orientation give back
+ * D_L within 5 % (the residual of the paper's N = 0 response) and iota within 0.05 rad; iota is the angle between the
+ * orbital angular momentum and the propagation direction (source -> observer), psi = pi/2 - (angle of its sky
+ * projection from u towards v) modulo pi/2, and advancing the wave's phase lowers phi_c by as much.
  * Errors: EINVAL (NULL pointer, non-finite input).
  */
 FSTAT_API fstat_status fstat_extrinsic_from_amplitudes(const double *a, double chirp_mass_msun, double *out);

@@ -3,7 +3,9 @@
 shares nothing with paper_2407_10797_b200/ (whose C function fstat_extrinsic_from_amplitudes it checks).
 
 Pins (tests/test_extrinsic.py, CPU): B2-B3 invert B1 on random parameter sets inside the principal branches; outside
-them the recovered set reproduces the amplitudes through B1; D_L = 2 / A and iota are branch-free.
+them the recovered set reproduces the amplitudes through B1; D_L = 2 / A and iota are branch-free.  P20: amplitudes
+estimated from a quadrupole-formula binary's time-domain TDI signal (tests/td_sim.py PhysicalBinary) come back as its
+physical distance (5 %) and inclination (0.05 rad).
 
 Reading A25: Eq. B2's plain arctan fixes phi_c only modulo pi, while phi_c -> phi_c + pi flips the sign of
 all four a_i in Eq. B1.  `b2_b3` takes the paper's arctan values and adds pi to phi_c when that is what reproduces the

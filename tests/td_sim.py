@@ -90,3 +90,42 @@ def tdi_michelson_time_domain(t, chirp, c_plus, c_cross, theta, phi, L, vertex=0
 def tdi_x_time_domain(t, chirp, c_plus, c_cross, theta, phi, L):
     """X(t) from the four one-way links with explicit delays."""
     return tdi_michelson_time_domain(t, chirp, c_plus, c_cross, theta, phi, L, 0)
+
+
+class PhysicalBinary:
+    """Time-domain strain of a quasi-circular binary from the quadrupole formula, with NOTHING of App. A-B in it (pin P20):
+    two point masses on a circular orbit of phase Phi(t)/2 about the unit vector Lhat, seen at distance D,
+
+        h_ij(t) = -A(t) [ (e1 e1 - e2 e2)_ij cos Phi(t) + (e1 e2 + e2 e1)_ij sin Phi(t) ],
+        A(t) = 4 (G M_c / c^3)^(5/3) (pi f(t))^(2/3) / (D / c),
+
+    (x(t) = e1 cos(Phi/2) + e2 sin(Phi/2) the separation direction, e1, e2 orthonormal in the orbital plane, e1 x e2 = Lhat;
+    h_ij = (2 G / c^4 D) d^2 Q_ij / dt^2 at leading order, M_c^(5/3) = mu M^(2/3), omega = pi f), projected on the sky basis
+    of the propagation direction k: h_+ = (u.h.u - v.h.v)/2, h_x = u.h.v.  The orientation is given physically: iota = angle
+    between Lhat and k (k points from the source to the observer), pol = angle of Lhat's sky projection from u towards v.
+    Several (D, iota, pol, phi0) sets are carried at once: h() returns arrays [n_sets][len(t)], so that the links of
+    tdi_michelson_time_domain (whose cost is the Keplerian orbits) are evaluated once."""
+
+    def __init__(self, chirp, chirp_mass_s, k, u, v, sets):
+        self.chirp, self.tau = chirp, float(chirp_mass_s)
+        self.coef = []
+        for (dist_s, iota, pol, phi0) in sets:
+            lhat = np.cos(iota) * k + np.sin(iota) * (np.cos(pol) * u + np.sin(pol) * v)
+            e1 = np.cross(lhat, k)
+            e1 = e1 / np.linalg.norm(e1)
+            e2 = np.cross(lhat, e1)
+
+            def comp(a, b, e1=e1, e2=e2):               # (cos, sin) coefficients of a.h.b / (-A)
+                return ((a @ e1) * (b @ e1) - (a @ e2) * (b @ e2), (a @ e1) * (b @ e2) + (a @ e2) * (b @ e1))
+            uu, vv, uv = comp(u, u), comp(v, v), comp(u, v)
+            self.coef.append((dist_s, phi0, 0.5 * (uu[0] - vv[0]), 0.5 * (uu[1] - vv[1]), uv[0], uv[1]))
+
+    def h(self, t, c_plus=None, c_cross=None):
+        phi, f = self.chirp._phi(t), self.chirp._f(t)
+        amp = 4.0 * self.tau ** (5.0 / 3.0) * (np.pi * f) ** (2.0 / 3.0)
+        hp, hc = [], []
+        for (dist_s, phi0, pc, ps, cc, cs) in self.coef:
+            co, si = np.cos(phi + phi0), np.sin(phi + phi0)
+            hp.append(-(amp / dist_s) * (pc * co + ps * si))
+            hc.append(-(amp / dist_s) * (cc * co + cs * si))
+        return np.array(hp), np.array(hc)
