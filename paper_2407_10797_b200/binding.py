@@ -317,13 +317,25 @@ def fstat_eval_batch_bands(plan: Plan, params, n_seg: int, edge_lattice: int = 1
 
 
 def fstat_eval_batch_bands_host(plan: Plan, params, n_seg: int, edge_lattice: int = 1, stream=None):
-    """HOST buffers: params [P][6] float64 numpy array -> (F [P], Fk [P][n_seg], band [P][2] int64) numpy arrays,
-    filled when the call returns."""
-    par = np.ascontiguousarray(params, dtype=np.float64).reshape(-1, 6)
-    P = par.shape[0]
-    F, Fk, band = np.empty(P), np.empty((P, int(n_seg))), np.empty((P, 2), dtype=np.int64)
-    _check(load_library().fstat_eval_batch_bands_host(plan.handle, P, par.ctypes.data, int(n_seg), int(edge_lattice),
-                                                      F.ctypes.data, Fk.ctypes.data, band.ctypes.data, _stream_ptr(stream)),
+    """HOST buffers: params [P][6] float64 numpy array or CPU tensor (pinned for async DMA) -> (F [P], Fk [P][n_seg],
+    band [P][2] int64) of the same kind, filled when the call returns."""
+    if _is_tensor(params):
+        import torch
+        if params.is_cuda or params.dtype != torch.float64 or not params.is_contiguous():
+            raise TypeError("params must be a contiguous float64 CPU tensor or numpy array")
+        P = int(params.shape[0])
+        pin = params.is_pinned()
+        F = torch.empty(P, dtype=torch.float64, pin_memory=pin)
+        Fk = torch.empty((P, int(n_seg)), dtype=torch.float64, pin_memory=pin)
+        band = torch.empty((P, 2), dtype=torch.int64, pin_memory=pin)
+        ptrs = (params.data_ptr(), F.data_ptr(), Fk.data_ptr(), band.data_ptr())
+    else:
+        params = np.ascontiguousarray(params, dtype=np.float64).reshape(-1, 6)
+        P = params.shape[0]
+        F, Fk, band = np.empty(P), np.empty((P, int(n_seg))), np.empty((P, 2), dtype=np.int64)
+        ptrs = (params.ctypes.data, F.ctypes.data, Fk.ctypes.data, band.ctypes.data)
+    _check(load_library().fstat_eval_batch_bands_host(plan.handle, P, ptrs[0], int(n_seg), int(edge_lattice),
+                                                      ptrs[1], ptrs[2], ptrs[3], _stream_ptr(stream)),
            "fstat_eval_batch_bands_host", plan)
     return F, Fk, band
 

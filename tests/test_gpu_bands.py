@@ -118,7 +118,10 @@ def test_bands_host_buffers_give_the_same_bits(fs, bands, lattice):
     F, Fk, band = _gpu(fs, ds, par, 16, lattice)
     with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
         F_h, Fk_h, band_h = fs.fstat_eval_batch_bands_host(plan, par, 16, lattice)
+        import torch
+        F_p, Fk_p, band_p = fs.fstat_eval_batch_bands_host(plan, torch.as_tensor(par).pin_memory(), 16, lattice)    # pinned tensors
     assert np.array_equal(F, F_h) and np.array_equal(Fk, Fk_h) and np.array_equal(band, band_h)
+    assert F_p.is_pinned() and np.array_equal(F, F_p.numpy()) and np.array_equal(Fk, Fk_p.numpy()) and np.array_equal(band, band_p.numpy())
 
 
 @pytest.mark.parametrize("lattice", [1, 64])
