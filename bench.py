@@ -61,7 +61,7 @@ NCU_DRAM_CAPTURE = "profiles/r2.md (34.3 MB read + 188.1 MB written), ncu captur
 BAND_FP64_PER_INTERVAL = 736.0      # fstat_fastband_kernel keeps the four-node sub-block code of round-2 build 1ecb204
 BAND_FP64_PER_RUN = 1105.0
 BAND_FP64_PER_CUT_INTERVAL = 350.0
-NCU_BAND_DRAM_BYTES = 106.6e6     # profiles/r2_bands.md: N_seg = 1024, edges at any bin, config 1 data, build 1ecb204
+NCU_BAND_DRAM_BYTES = 120.6e6     # profiles/r2_bands.md: N_seg = 1024, edges at any bin, config 1 data, build 2d160f1 (84.5 MB read + 36.1 MB written)
 
 
 def sass_fp64_mix(lib_path):
