@@ -199,6 +199,30 @@ def test_host_buffer_call_with_a_large_Fk_block_is_cut_into_partition_ranges_bit
     assert _rel(Fk_h[sample], Fk_o).max() <= RTOL and _rel(F_h[sample], F_o).max() <= RTOL
 
 
+def test_random_grids_edges_and_batch_sizes_interpolating_against_direct_kernel(fs, torch_):
+    """Seeded fuzz over what the host logic branches on: band position (10-30 mHz), slice width, N_p from 1 to 600 with
+    partition edges at ARBITRARY bins (sub-blocks of one to three bins -- rank-deficient Gram matrices in the plan-time
+    W tables -- partitions shorter than the smallest stride, which go to the direct kernel), batch sizes around the
+    128-particle group size.  Every F_k of the interpolating path against the direct kernel (every bin in full) on
+    noise-only data, strict relative; 40 such cases gave a worst 5.4e-7 (profiles/r2.md)."""
+    rng = np.random.default_rng(1)
+    for trial in range(14):
+        f_lo = float(rng.choice([0.0100, 0.0150, 0.0200, 0.0300]))
+        width = float(rng.choice([0.0002, 0.0005, 0.001]))
+        cfg = syn.Config(30 + trial, "fuzz", 2.5 * syn.YEAR_S, f_lo, f_lo + width, (8,), (700,), 3.5 * syn.YEAR_S, "wide")
+        ds = syn.make_dataset(cfg, None)
+        n = ds.freq.size
+        n_part = int(rng.choice([1, 2, 7, 33, 150, 600]))
+        cuts = np.sort(rng.choice(np.arange(1, n), n_part - 1, replace=False)) if n_part > 1 else np.array([], dtype=np.int64)
+        edges = np.concatenate([[0], cuts, [n]]).astype(np.int64)
+        P = int(rng.choice([1, 33, 128, 129, 300, 700]))
+        par = syn.draw_particles(cfg)[:P]
+        F, Fk = _gpu_eval(fs, torch_, ds, edges, par)
+        F_d, Fk_d = _gpu_eval(fs, torch_, ds, edges, par, fs.fstat_default_options(force_level=-1))
+        assert np.max(np.abs(Fk - Fk_d) / np.abs(Fk_d)) <= 5e-6, (trial, f_lo, width, n_part, P)
+        assert np.max(np.abs(F - F_d) / np.abs(F_d)) <= 5e-6, (trial, f_lo, width, n_part, P)
+
+
 def test_empty_batch_and_null_Fk(fs, torch_, orc, tiny):
     ds = tiny
     par = syn.draw_particles(ds.cfg, 9)
