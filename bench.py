@@ -473,9 +473,9 @@ def run_ours(args):
     hbm_peak, hbm_src = peaks()
     n_groups = (P + 127) // 128
     # algorithmic HBM bytes of one launch: every particle group streams the folded data (16 B/bin) once, reads
-    # one 192-B node row and one 80-B Gram matrix per node interval, and writes one 80-B record of partial sums per
+    # one 192-B node row and one 192-B sub-block table per node interval, and writes one 80-B record of partial sums per
     # particle and segment (counted here per CTA run: a lower bound when a run holds several segments)
-    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 80.0) * n_intervals + 80.0 * 128.0 * n_items
+    hbm_bytes = 16.0 * ds.n_bins * n_groups + (192.0 + 192.0) * n_intervals + 80.0 * 128.0 * n_items
     default_wl = cfg.name == "first_stage" and n_part == 1024 and P == 2048
     roofline = {"bound": "alu", "kernel": "fstat_fast_kernel (+ fstat_main_kernel for the work items it leaves)",
                 "pipe": "fp64",

@@ -80,6 +80,11 @@ typedef struct {
     int32_t no_channel_fusion;/* 0 (default): fstat_eval_batch_channels evaluates two or three plans of the A / E / T  *
                                * family in ONE pass of the interpolating kernel (shared node model and carrier);   *
                                * 1 (read from plans[0]): one pass per channel, as for any other set (tests / tuning)*/
+    int32_t min_stride_level; /* smallest stride level 0..6 (stride 8 << level) the plan keeps tables for; -1 (set by      *
+                               * fstat_default_options) = automatic: 2 (stride 32), or force_level when that is 0 or 1.  *
+                               * Work items whose error bound asks for a smaller stride go to the direct kernel.  The    *
+                               * tables of levels 0 and 1 are 3/4 of the per-sub-block tables (36 of 48 bytes per bin);   *
+                               * no work item of the paper's band (>= 10 mHz, 2.5 yr) asks for them                       */
 } fstat_options;
 
 FSTAT_API void fstat_default_options(fstat_options *opts);

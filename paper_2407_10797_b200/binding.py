@@ -39,7 +39,7 @@ class Options(C.Structure):
     _fields_ = [("f_ref_e0", C.c_double), ("arm_length_m", C.c_double), ("orbit_kappa", C.c_double),
                 ("orbit_lambda", C.c_double), ("device", C.c_int32), ("inputs_on_device", C.c_int32),
                 ("max_segment_bins", C.c_int32), ("force_level", C.c_int32), ("interp_tol", C.c_double),
-                ("tdi_channel", C.c_int32), ("no_channel_fusion", C.c_int32)]
+                ("tdi_channel", C.c_int32), ("no_channel_fusion", C.c_int32), ("min_stride_level", C.c_int32)]
 
 
 TDI_CHANNELS = {"X": 0, "Y": 1, "Z": 2, "A": 3, "E": 4, "T": 5}      # fstat_tdi_channel

@@ -43,6 +43,7 @@ struct fstat_plan {
     double *d_node = nullptr;          // [n_node_rows][kTabW]
     int64_t n_node_rows = 0;
     bool fast_ok = false;              // the node grid (2 kMaxStride bins below, 3 above the band) stays at f > 0
+    int32_t min_level = 0;             // smallest stride level with per-sub-block tables (options.min_stride_level)
     // partition-dependent tables of the interpolating kernel
     int32_t *d_edges32 = nullptr; size_t edges32_cap = 0;
     int32_t *d_cnt = nullptr; size_t cnt_cap = 0;          // scratch [n_part]
@@ -347,7 +348,7 @@ fstat_status build_gram_tables(fstat_plan *pl)
         std::vector<int32_t> &cnt = pl->cnt[l];
         cnt.assign(n_part, 0);
         for (int32_t k = 1; k < n_part; ++k) cnt[k] = cnt[k - 1] + ((pl->edges[k] % S) != 0 ? 1 : 0);
-        if (!pl->fast_ok) continue;
+        if (!pl->fast_ok || l < pl->min_level) continue;   // (no work item is given a level below min_level)
         const int64_t n_sub = (pl->n_bins + S - 1) / S + cnt[n_part - 1];
         CU_TRY(pl, grow(&pl->d_gram[l], &pl->gram_cap[l], (size_t)n_sub * kNW));
         CU_TRY(pl, cudaMemcpy(pl->d_cnt, cnt.data(), (size_t)n_part * sizeof(int32_t), cudaMemcpyHostToDevice));
@@ -425,6 +426,7 @@ void fstat_default_options(fstat_options *o)
     o->force_level = -2;
     o->interp_tol = 1.0;
     o->tdi_channel = FSTAT_TDI_X;
+    o->min_stride_level = -1;
 }
 
 const char *fstat_status_str(fstat_status s)
@@ -571,7 +573,8 @@ fstat_status fstat_plan_create(fstat_plan **out, int64_t n_bins, const double *f
     if (opts) o = *opts;
     if (!(o.f_ref_e0 > 0.0) || !(o.arm_length_m > 0.0) || !isfinite(o.orbit_kappa) || !isfinite(o.orbit_lambda) ||
         o.max_segment_bins < 0 || o.force_level < -2 || o.force_level >= kNLevels || !(o.interp_tol > 0.0) ||
-        !isfinite(o.interp_tol) || o.tdi_channel < FSTAT_TDI_X || o.tdi_channel > FSTAT_TDI_T)
+        !isfinite(o.interp_tol) || o.tdi_channel < FSTAT_TDI_X || o.tdi_channel > FSTAT_TDI_T ||
+        o.min_stride_level < -1 || o.min_stride_level >= kNLevels)
         return fail(nullptr, FSTAT_EINVAL, "bad option value");
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
@@ -587,6 +590,9 @@ fstat_status fstat_plan_create(fstat_plan **out, int64_t n_bins, const double *f
     pl->device = dev;
     pl->n_bins = n_bins;
     pl->opt = o;
+    // automatic: stride 32 and up, unless a smaller stride is forced (tests, tuning); never above a forced level
+    pl->min_level = o.min_stride_level >= 0 ? o.min_stride_level : 2;
+    if (o.force_level >= 0 && o.force_level < pl->min_level) pl->min_level = o.force_level;
     pl->n_part = n_part;
     try {
         pl->edges.assign(part_edges, part_edges + n_part + 1);
@@ -775,7 +781,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
     BandSched bs{};
     CU_TRY(pl, launch_schedule(pl->d_coef, pl->d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit,
                                pl->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
-                               pl->opt.force_level, bs, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
+                               pl->opt.force_level, pl->min_level, bs, pl->d_level, pl->d_direct + 1, pl->d_direct, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;
     fa.node = pl->d_node;
@@ -984,7 +990,7 @@ fstat_status fstat_eval_batch_channels(fstat_plan *const *plans, int32_t n_chann
         const fstat_plan *pc = plans[c];
         fuse = pc->fast_ok && pc->opt.tdi_channel >= FSTAT_TDI_A && pc->opt.tdi_channel <= FSTAT_TDI_T &&
                memcmp(pc->orb.c, p0->orb.c, sizeof(p0->orb.c)) == 0 && pc->opt.interp_tol == p0->opt.interp_tol &&
-               pc->opt.force_level == p0->opt.force_level;
+               pc->opt.force_level == p0->opt.force_level && pc->min_level == p0->min_level;
     }
     if (fuse) {
         fstat_status s = eval_impl(p0, P, params, nullptr, nullptr, nullptr, stream, true, plans, n_channels);
@@ -1124,7 +1130,7 @@ static fstat_status bands_impl(fstat_plan *pl, int64_t P, const double *params, 
     bs.n_bins = (int32_t)pl->n_bins;
     CU_TRY(pl, launch_schedule(cp->d_coef, cp->d_valid, P_pad, (int32_t)n_groups, cp->n_seg, cp->d_seg_crit,
                                cp->d_seg_maxlvl, pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7,
-                               pl->opt.force_level, bs, cp->d_level, cp->d_direct + 1, cp->d_direct, st));
+                               pl->opt.force_level, 0, bs, cp->d_level, cp->d_direct + 1, cp->d_direct, st));
     // empty partitions and templates without a band: F_k = 0, a = 0
     CU_TRY(pl, cudaMemsetAsync(Fk, 0, (size_t)P * (size_t)n_seg * sizeof(double), st));
     if (amp) CU_TRY(pl, cudaMemsetAsync(amp, 0, (size_t)P * (size_t)n_seg * 4 * sizeof(double), st));
@@ -1488,8 +1494,8 @@ fstat_status fstat_eval_batch_noalloc(fstat_plan *pl, int64_t P, const double *p
                                d_perm, st));
     BandSched bs{};
     CU_TRY(pl, launch_schedule(d_coef, d_valid, P_pad, (int32_t)n_groups, pl->n_seg, pl->d_seg_crit, pl->d_seg_maxlvl,
-                               pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7, pl->opt.force_level, bs,
-                               d_level, d_direct + 1, d_direct, st));
+                               pl->opt.interp_tol * 1.5e-7 * (2.0 / kPi), pl->opt.interp_tol * 2e-7, pl->opt.force_level,
+                               pl->min_level, bs, d_level, d_direct + 1, d_direct, st));
     FastArgs fa;
     fa.dwp = pl->d_dwp;
     fa.node = pl->d_node;

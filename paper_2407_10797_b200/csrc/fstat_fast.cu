@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
                                                             const int32_t *__restrict__ valid, int64_t P_pad,
                                                             int32_t n_seg, const SegCrit *__restrict__ crit,
                                                             const int8_t *__restrict__ seg_maxlvl, double tol_phi_qt,
-                                                            double tol_resp, int32_t force_level,
+                                                            double tol_resp, int32_t force_level, int32_t min_level,
                                                             const BandSched bands, int8_t *__restrict__ level,
                                                             int32_t *__restrict__ direct_list,
                                                             int32_t *__restrict__ direct_count)
@@ -221,6 +221,7 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
                 if (ephi1 * S4 <= tol_phi_qt && eT1 * S4 <= tol_resp) lvl = l;
             }
         }
+        if (lvl < min_level) lvl = -1;                    // the plan keeps no tables for strides that small: direct kernel
         level[(int64_t)grp * n_seg + seg] = (int8_t)lvl;
         if (lvl < 0) direct_list[atomicAdd(direct_count, 1)] = grp * n_seg + seg;   // order is irrelevant
     }
@@ -228,14 +229,14 @@ __global__ void __launch_bounds__(kThreads) schedule_kernel(const double *__rest
 
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
-                            double tol_resp, int32_t force_level, const BandSched &bands, int8_t *level,
+                            double tol_resp, int32_t force_level, int32_t min_level, const BandSched &bands, int8_t *level,
                             int32_t *direct_list, int32_t *direct_count, cudaStream_t st)
 {
     cudaError_t e = cudaMemsetAsync(direct_count, 0, sizeof(int32_t), st);
     if (e != cudaSuccess) return e;
     const unsigned gy = (unsigned)((n_seg + 16 * kThreads - 1) / (16 * kThreads));       // <= 16 segments per thread
     schedule_kernel<<<dim3((unsigned)n_groups, gy < 1 ? 1 : (gy > 64 ? 64 : gy)), kThreads, 0, st>>>(coef, valid, P_pad, n_seg, crit, seg_maxlvl,
-                                                            tol_phi_qt, tol_resp, force_level, bands, level,
+                                                            tol_phi_qt, tol_resp, force_level, min_level, bands, level,
                                                             direct_list, direct_count);
     return cudaGetLastError();
 }

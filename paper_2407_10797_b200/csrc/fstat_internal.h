@@ -251,7 +251,7 @@ cudaError_t launch_build_gram(const double *fw, const int32_t *edges, int32_t n_
                               int level, const int32_t *cnt, double *gram, cudaStream_t st);
 cudaError_t launch_schedule(const double *coef, const int32_t *valid, int64_t P_pad, int32_t n_groups,
                             int32_t n_seg, const SegCrit *crit, const int8_t *seg_maxlvl, double tol_phi_qt,
-                            double tol_resp, int32_t force_level, const BandSched &bands, int8_t *level,
+                            double tol_resp, int32_t force_level, int32_t min_level, const BandSched &bands, int8_t *level,
                             int32_t *direct_list, int32_t *direct_count, cudaStream_t st);
 cudaError_t launch_fast(const FastArgs &a, cudaStream_t st);
 cudaError_t fast_kernel_configure();
