@@ -223,6 +223,33 @@ def test_random_grids_edges_and_batch_sizes_interpolating_against_direct_kernel(
         assert np.max(np.abs(F - F_d) / np.abs(F_d)) <= 5e-6, (trial, f_lo, width, n_part, P)
 
 
+def test_min_stride_level_sends_smaller_strides_to_the_direct_kernel(fs, torch_):
+    """options.min_stride_level: the plan keeps per-sub-block tables from that stride up; a work item whose error bound
+    asks for a smaller stride is evaluated by the direct kernel instead -- same F_k to the interpolation tolerance, no
+    bin at a stride below the minimum, and a smaller table footprint.  Default (-1): strides 32 and up."""
+    cfg = syn.Config(24, "minlvl_slice", 2.5 * syn.YEAR_S, 0.0100, 0.0104, (8,), (256,), 3.5 * syn.YEAR_S, "wide")
+    ds = syn.make_dataset(cfg, None)
+    par = syn.draw_particles(cfg)
+    edges = ds.edges(8)
+    p = torch_.as_tensor(par, device="cuda")
+    out = {}
+    for lvl in (-1, 0, 4):
+        with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, fs.fstat_default_options(min_stride_level=lvl)) as plan:
+            F, Fk = fs.fstat_eval_batch(plan, p)
+            torch_.cuda.synchronize()
+            bins, _ = fs.fstat_plan_level_bins(plan)
+            out[lvl] = (Fk.cpu().numpy(), bins.copy(), fs.fstat_plan_table_bytes(plan))
+    F_d, Fk_d = _gpu_eval(fs, torch_, ds, edges, par, fs.fstat_default_options(force_level=-1))
+    for lvl, (Fk, bins, nbytes) in out.items():
+        assert np.max(np.abs(Fk - Fk_d) / np.abs(Fk_d)) <= 5e-6, lvl
+        assert bins.sum() == out[0][1].sum()
+    assert out[-1][1][1:3].sum() == 0 and out[4][1][1:5].sum() == 0            # no bin below the minimum stride
+    assert out[4][1][0] > out[0][1][0] and out[0][1][1:5].sum() > 0             # ... they went to the direct kernel
+    assert out[0][2] > out[-1][2] > out[4][2]
+    with pytest.raises(fs.FstatError):
+        fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges, fs.fstat_default_options(min_stride_level=7))
+
+
 def test_empty_batch_and_null_Fk(fs, torch_, orc, tiny):
     ds = tiny
     par = syn.draw_particles(ds.cfg, 9)
