@@ -140,7 +140,7 @@ def test_bands_first_stage_sample(fs, orc, first_stage, lattice):
     width = band[:, 1] - band[:, 0]
     assert (width > 0).sum() > 1500
     order = np.argsort(width)
-    sample = np.concatenate([order[-2:], order[(width[order] > 0).argmax():][:2], np.arange(0, 2048, 341)])
+    sample = np.unique(np.concatenate([order[-2:], order[(width[order] > 0).argmax():][:2], np.arange(0, 2048, 66)]))   # 35 particles
     _check(orc, ds, par[sample], 1024, lattice, F[sample], Fk[sample], band[sample])
 
 

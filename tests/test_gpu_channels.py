@@ -197,13 +197,14 @@ def test_fused_pass_equals_one_pass_per_channel(fs, orc, names):
 
 
 def test_first_stage_aet_sample(fs, orc):
-    """Config 1 at full size (N_p = 1024, P = 2048) with A + E + T; a sample of particles against the oracle."""
+    """Config 1 at full size (N_p = 1024, P = 2048) with A + E + T; 64 particles against the oracle (through
+    the fused three-channel kernel)."""
     cfg = syn.CONFIGS[1]
     chans = _aet_channels(orc, cfg, "AET")
     par = syn.draw_particles(cfg)
     edges = chans[0][0].edges(1024)
     F, Fk = _gpu_named(fs, chans, edges, par)
-    sample = np.array([0, 167, 511, 1024, 1598, 2047])
+    sample = np.arange(5, 2048, 32)                        # 64 particles, every F_k of each
     _compare(orc, [(ds, o) for ds, o, _ in chans], edges, par[sample], F[sample], Fk[sample])
 
 
