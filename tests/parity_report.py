@@ -18,6 +18,13 @@ Metric per value: |x_gpu - x_oracle| / max(|x_oracle|, tau), tau = 0 (strict) an
 noise-only mean of F_k is 2).  Target: <= 1e-5 strict on every value; values that miss it are listed (hazard H9).
 The oracle costs ~1 core-second per 2.5-yr / 20 mHz template and ~5 for the wide band: about 1e4 core-seconds in
 all.  --quick cuts every sample to 16 particles (a smoke run of this script, not a report).
+
+--rows adds the rows built on top of the hot path, at full size, in the launch configurations bench.py times:
+  f2   per-template bands (fstat_eval_batch_bands, edges at any bin) on config 1's data and all 2048 particles,
+       N_seg = 1024 and 16: 256 seeded particles against oracle.fstat_bands (non-empty partitions; empty ones must be 0)
+  f4   A + E + T (fstat_eval_batch_channels, the fused three-channel kernel) on config 1, N_p = 1024, all 2048 particles:
+       256 seeded particles against oracle.fstat_batch_channels
+oracle.fstat_bands is a serial Python loop over particles: this script only spreads the particles over worker processes.
 """
 from __future__ import annotations
 
@@ -35,11 +42,20 @@ if ROOT not in sys.path:
 import synthetic as syn  # noqa: E402
 
 
+def _bands_worker(job):
+    """One worker process: oracle.fstat_bands on its share of the particles (edge lattice 1)."""
+    from oracle import oracle as orc
+    freq, dw, inv_sn, par, n_seg = job
+    F, Fk, _ = orc.fstat_bands(freq, dw, inv_sn, par, n_seg, 1)
+    return F, Fk
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "r2_parity.md"))
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--configs", default="0,1,2,3,4")
+    ap.add_argument("--rows", default="", help="comma list of f2, f4: also check these rows (see the docstring)")
     args = ap.parse_args()
 
     import torch
@@ -139,6 +155,70 @@ def main():
             sample = np.sort(np.concatenate([np.arange(256), 256 + rng.choice(4096 - 256, 512, replace=False),
                                              4096 + rng.choice(65536 - 4096, 512, replace=False)]))
         run("4 wide_band", ds, par, sample, list(cfg.n_part), [256, 4096, 65536])
+    extra = [r for r in args.rows.split(",") if r]
+    if extra:
+        import dataclasses
+        from concurrent.futures import ProcessPoolExecutor
+        cfg1 = syn.CONFIGS[1]
+        par = syn.draw_particles(cfg1)
+        sample = np.sort(np.random.default_rng(205).choice(par.shape[0], q or 256, replace=False))
+        workers = max(1, min(orc.max_threads(), len(sample)))
+        if "f2" in extra:
+            ds = syn.make_dataset(cfg1, orc.template)
+            with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, ds.edges(1)) as plan:
+                p = torch.as_tensor(np.ascontiguousarray(par), device="cuda")
+                for n_seg in (1024, 16):
+                    t0 = time.time()
+                    F_g, Fk_g, _ = fs.fstat_eval_batch_bands(plan, p, n_seg, 1)
+                    torch.cuda.synchronize()
+                    F_g, Fk_g = F_g.cpu().numpy()[sample], Fk_g.cpu().numpy()[sample]
+                    chunks = np.array_split(par[sample], workers)
+                    with ProcessPoolExecutor(workers) as ex:
+                        res = list(ex.map(_bands_worker, [(ds.freq, ds.dw, ds.inv_sn, c, n_seg) for c in chunks]))
+                    F_o = np.concatenate([r[0] for r in res])
+                    Fk_o = np.concatenate([r[1] for r in res])
+                    live = Fk_o != 0.0
+                    assert np.all(Fk_g[~live] == 0.0), "an empty partition is not exactly zero"
+                    x_g = np.concatenate([Fk_g[live], F_g[F_o != 0.0]])
+                    x_o = np.concatenate([Fk_o[live], F_o[F_o != 0.0]])
+                    strict = np.abs(x_g - x_o) / np.abs(x_o)
+                    loose = np.abs(x_g - x_o) / np.maximum(np.abs(x_o), 1.0)
+                    nbad = int((strict > 1e-5).sum())
+                    rows.append(("f2 bands (config 1 data)", par.shape[0], n_seg, int(sample.size), int(strict.size),
+                                 float(strict.max()), float(np.quantile(strict, 0.999)), nbad, float(loose.max())))
+                    print("f2 N_seg=%d: %d values, max strict %.3g, > 1e-5: %d  [%.0f s]" % (n_seg, strict.size, strict.max(), nbad, time.time() - t0), flush=True)
+                    flush()
+            del ds
+        if "f4" in extra:
+            t0 = time.time()
+            chans, plans = [], []
+            for c, name in enumerate("AET"):
+                o = orc.default_options(tdi_channel=orc.TDI_CHANNELS[name])
+                ds_c = syn.make_dataset(dataclasses.replace(cfg1, noise_seed=70 + c), lambda pp, f, o=o: orc.template(pp, f, o), channel=name)
+                chans.append((ds_c, o))
+            edges = chans[0][0].edges(1024)
+            try:
+                for (ds_c, _), name in zip(chans, "AET"):
+                    plans.append(fs.fstat_plan_create(ds_c.freq, ds_c.dw, ds_c.inv_sn, edges,
+                                                      fs.fstat_default_options(tdi_channel=fs.TDI_CHANNELS[name])))
+                F_g, Fk_g = fs.fstat_eval_batch_channels(plans, torch.as_tensor(np.ascontiguousarray(par), device="cuda"))
+                torch.cuda.synchronize()
+                F_g, Fk_g = F_g.cpu().numpy()[sample], Fk_g.cpu().numpy()[sample]
+            finally:
+                for pl in plans:
+                    fs.fstat_plan_destroy(pl)
+            F_o, Fk_o = orc.fstat_batch_channels(chans[0][0].freq, [(d.dw, d.inv_sn, o) for d, o in chans], edges, par[sample])
+            x_g = np.concatenate([Fk_g, F_g[:, None]], axis=1)
+            x_o = np.concatenate([Fk_o, F_o[:, None]], axis=1)
+            strict = np.abs(x_g - x_o) / np.abs(x_o)
+            loose = np.abs(x_g - x_o) / np.maximum(np.abs(x_o), 1.0)
+            nbad = int((strict > 1e-5).sum())
+            rows.append(("f4 A+E+T fused (config 1)", par.shape[0], 1024, int(sample.size), int(strict.size), float(strict.max()),
+                         float(np.quantile(strict, 0.999)), nbad, float(loose.max())))
+            print("f4 A+E+T: %d values, max strict %.3g, > 1e-5: %d  [%.0f s]" % (strict.size, strict.max(), nbad, time.time() - t0), flush=True)
+            flush()
+        notes.append("Rows f2 / f4: oracle.fstat_bands (edges at any bin; empty partitions checked to be exactly 0 on the GPU side) and "
+                     "oracle.fstat_batch_channels (A, E, T data sets with their own PSDs and noise seeds), double-mode sums.")
     notes.append("Oracle: oracle/fstat_oracle.c, mode 2 (templates in FP64; the 4 + 10 sums in long double handed to the "
                  "long-double 4x4 Cholesky unrounded: pin P18, hazard H3), %d host threads; total wall time of this run "
                  "%.0f s." % (orc.max_threads(), time.time() - t_start))
