@@ -188,6 +188,8 @@ def parse_args():
     ap.add_argument("--channels", type=int, default=None, metavar="N",
                     help="also time fstat_eval_batch_channels (row f4: the first N of the TDI channels A, E, T, common amplitudes); "
                          "default: 3 on the default workload unless --no-sweep, else off")
+    ap.add_argument("--graph", action="store_true",
+                    help="also time fstat_eval_batch_noalloc captured once in a CUDA graph and replayed (small problems are launch-bound)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip what the default workload adds to the line: the N_p sweep rows and the rows f2 / f4 legs (bands, channels)")
@@ -538,6 +540,35 @@ def run_ours(args):
     if default_wl and world == 1 and not args.no_sweep:
         out["sweep"] = run_sweep(fs, torch, plan, ds, args, mix, fp64_rate, stream, scratch)
         fs.fstat_plan_set_partitions(plan, edges)
+    if args.graph:
+        # the same step as `value`, through the no-allocation entry point captured once into a CUDA graph: a replay costs one
+        # launch on the host instead of seven.  Not timed with the L2 flush in between (a replay loop is the use case).
+        fs.fstat_eval_batch_noalloc(plan, par, F, Fk, stream)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            fs.fstat_eval_batch_noalloc(plan, par, F, Fk)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        n_g = max(args.steps, 1) * 10
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for _ in range(n_g):
+            g.replay()
+        g1.record()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n_g):
+            fs.fstat_eval_batch(plan, par, F, Fk, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        out["graph"] = {"call": "fstat_eval_batch_noalloc captured in a CUDA graph", "replays": n_g,
+                        "ms_per_replay": g0.elapsed_time(g1) / n_g,
+                        "ms_per_step_back_to_back_without_graph": e0.elapsed_time(e1) / n_g,
+                        "template_bins_per_s": float(P) * ds.n_bins / (g0.elapsed_time(g1) / n_g * 1e-3)}
+        del g
     if args.pso > 0:
         # row f1: ITERS iterations of the device PSO (update -> fstat_eval_batch -> personal bests) enqueued back to
         # back on the stream, no host synchronisation in between; box = the particle ranges of the workload

@@ -99,3 +99,33 @@ def test_noalloc_call_rejects_what_does_not_fit_or_is_not_set_up(fs):
             fs.fstat_eval_batch_noalloc(plan, bigger, Fb2, None)
         assert ei.value.status == 4
         torch.cuda.synchronize()
+
+
+def test_noalloc_call_can_be_captured_in_a_cuda_graph_and_replayed(fs):
+    """What the entry point is for: the whole evaluation (prologue, stride selection, main kernels, epilogue) captured once
+    into a CUDA graph and replayed on new parameters written into the same input buffer -- no allocation, no host work per
+    replay.  The replays equal fstat_eval_batch on the same parameters bit for bit."""
+    import torch
+    cfg = syn.Config(22, "noalloc_slice", 2.5 * syn.YEAR_S, 0.0200, 0.0203, (8,), (300,), 3.5 * syn.YEAR_S, "wide")
+    ds, edges, par = _case(cfg, 8, 256)
+    par2 = par[::-1].copy()
+    with fs.fstat_plan_create(ds.freq, ds.dw, ds.inv_sn, edges) as plan:
+        p = torch.as_tensor(par, device="cuda")
+        F_ref, Fk_ref = fs.fstat_eval_batch(plan, p)                       # set-up: segment tables of this batch size
+        F_ref2, Fk_ref2 = fs.fstat_eval_batch(plan, torch.as_tensor(par2, device="cuda"))
+        F = torch.empty(256, dtype=torch.float64, device="cuda")
+        Fk = torch.empty((256, plan.n_part), dtype=torch.float64, device="cuda")
+        fs.fstat_eval_batch_noalloc(plan, p, F, Fk)                        # resolves the scratch address before the capture
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            fs.fstat_eval_batch_noalloc(plan, p, F, Fk)                    # on torch's current (capturing) stream
+        F.zero_(); Fk.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(F, F_ref) and torch.equal(Fk, Fk_ref)
+        p.copy_(torch.as_tensor(par2))                                     # new particles, same buffers
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(F, F_ref2) and torch.equal(Fk, Fk_ref2)
+        del g
