@@ -44,6 +44,8 @@ import synthetic as syn  # noqa: E402
 
 def _bands_worker(job):
     """One worker process: oracle.fstat_bands on its share of the particles (edge lattice 1)."""
+    if ROOT not in sys.path:
+        sys.path.insert(0, ROOT)
     from oracle import oracle as orc
     freq, dw, inv_sn, par, n_seg = job
     F, Fk, _ = orc.fstat_bands(freq, dw, inv_sn, par, n_seg, 1)
@@ -158,6 +160,7 @@ def main():
     extra = [r for r in args.rows.split(",") if r]
     if extra:
         import dataclasses
+        import multiprocessing
         from concurrent.futures import ProcessPoolExecutor
         cfg1 = syn.CONFIGS[1]
         par = syn.draw_particles(cfg1)
@@ -173,7 +176,7 @@ def main():
                     torch.cuda.synchronize()
                     F_g, Fk_g = F_g.cpu().numpy()[sample], Fk_g.cpu().numpy()[sample]
                     chunks = np.array_split(par[sample], workers)
-                    with ProcessPoolExecutor(workers) as ex:
+                    with ProcessPoolExecutor(workers, mp_context=multiprocessing.get_context("spawn")) as ex:   # no fork of a CUDA process
                         res = list(ex.map(_bands_worker, [(ds.freq, ds.dw, ds.inv_sn, c, n_seg) for c in chunks]))
                     F_o = np.concatenate([r[0] for r in res])
                     Fk_o = np.concatenate([r[1] for r in res])
