@@ -280,7 +280,7 @@ FSTAT_API fstat_status fstat_amplitudes_from_extrinsic(double d_l, double psi, d
  * on streams the plan owns (one per CUDA stream priority, the earlier range the higher), and a copy stream runs each
  * range's epilogue and the copy of its F_k columns under the later ranges' kernels; everything is ordered after the
  * work already queued on cuda_stream and joined into it before the call returns.  Same kernels, same sums: the
- * results equal fstat_eval_batch's bit for bit.  Config 1: 5.31 ms against 5.23 ms device-resident (the copy alone
+ * results equal fstat_eval_batch's bit for bit.  Config 1: 5.19 ms against 5.11 ms device-resident (the copy alone
  * is 0.3 ms).
  */
 FSTAT_API fstat_status fstat_eval_batch_host(fstat_plan *plan, int64_t P,

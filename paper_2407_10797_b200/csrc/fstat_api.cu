@@ -885,7 +885,7 @@ static fstat_status eval_impl(fstat_plan *pl, int64_t P, const double *params, d
         if (pipe) {
             fstat_status sp = ensure_pipe(pl);
             if (sp != FSTAT_OK) return sp;
-            // one range per stream priority below the copy stream's (5 on B200: 5.31 ms end to end against 5.23 ms on the
+            // one range per stream priority below the copy stream's (5 on B200: 5.31 ms end to end against 5.23 ms (first round-2 build) on the
             // device for config 1; ranges that share a priority share the SMs and finish together: 8 ranges 5.33 ms)
             const int32_t K = n_echunk < pl->pipe_ranges ? n_echunk : pl->pipe_ranges;
             const int32_t n_cta_chunks = (pl->n_seg + fa.segs_per_cta - 1) / fa.segs_per_cta;
